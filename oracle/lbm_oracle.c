@@ -1,0 +1,536 @@
+/*
+ * lbm_oracle.c — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Plain, slow, double-precision CPU statement of the D3Q19 LBM-LES step that
+ * the CUDA library in paper_2607_04516_b200/ must reproduce.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may load it.  It shares no code, header, table or helper with the CUDA path.
+ *
+ * What it follows.  The paper (§2.2; Table 1) names
+ * the ingredients — weakly compressible D3Q19, single-relaxation-time BGK,
+ * Smagorinsky-Lilly with the effective relaxation time "computed locally from
+ * nonequilibrium moments", Coriolis through Guo forcing, equilibrium-based
+ * velocity boundaries, no-slip solids — but prints no equation (all deferred to
+ * supplementary S4-S7, not available).  Each function
+ * therefore writes out the textbook definition of the named method, in the
+ * reading fixed by DESIGN.md "Readings" (= SURVEY.md §8(c)); the step numbers
+ * in comments (1..9) are the steps of that algorithm statement.
+ *
+ * Structure is deliberately naive: array-of-structures G[cell][19], one
+ * explicit resolve() per pulled population, no link masks, no blocking, no
+ * fusion beyond "one pass = one time step".  OpenMP on the outer z loop only.
+ *
+ * Pins: tests/test_oracle_*.py (closed forms, invariants, brute force) — see
+ * DESIGN.md "Oracle pins".  Parity unpinned: the urban LES statistics of
+ * configs 3-5 (no closed form exists; SURVEY.md §8(c) last row).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+/* cell classes (step 3) */
+enum { C_FLUID = 0, C_SOLID = 1, C_EQ_FIXED = 2, C_EQ_OUTFLOW = 3 };
+/* face types */
+enum { F_PERIODIC = 0, F_WALL = 1, F_FREE_SLIP = 2, F_EQ_FIXED = 3, F_EQ_OUTFLOW = 4 };
+
+#define Q 19
+
+/* step 1: lattice.  0 = rest; then opposite pairs adjacent, odd index = the
+ * sign listed first: 1,2=(+-1,0,0) 3,4=(0,+-1,0) 5,6=(0,0,+-1) 7,8=+-(1,1,0)
+ * 9,10=+-(1,0,1) 11,12=+-(0,1,1) 13,14=+-(1,-1,0) 15,16=+-(1,0,-1)
+ * 17,18=+-(0,1,-1). */
+static const int CI[Q][3] = {
+    {0, 0, 0},
+    {1, 0, 0},  {-1, 0, 0},
+    {0, 1, 0},  {0, -1, 0},
+    {0, 0, 1},  {0, 0, -1},
+    {1, 1, 0},  {-1, -1, 0},
+    {1, 0, 1},  {-1, 0, -1},
+    {0, 1, 1},  {0, -1, -1},
+    {1, -1, 0}, {-1, 1, 0},
+    {1, 0, -1}, {-1, 0, 1},
+    {0, 1, -1}, {0, -1, 1},
+};
+
+static double weight(int i) { return i == 0 ? 1.0 / 3.0 : (i <= 6 ? 1.0 / 18.0 : 1.0 / 36.0); }
+
+static int dir_index(int cx, int cy, int cz)
+{
+    for (int i = 0; i < Q; ++i)
+        if (CI[i][0] == cx && CI[i][1] == cy && CI[i][2] == cz) return i;
+    return -1;
+}
+
+static int opposite_search(int i) { return dir_index(-CI[i][0], -CI[i][1], -CI[i][2]); }
+
+/* the two searches above, tabulated once (filled from them, nothing else) */
+static int OPP[Q];
+static int DIR[3][3][3]; /* [cx+1][cy+1][cz+1] -> i, or -1 */
+static int tables_ready = 0;
+static void init_tables(void)
+{
+    if (tables_ready) return;
+    for (int i = 0; i < Q; ++i) OPP[i] = opposite_search(i);
+    for (int a = -1; a <= 1; ++a)
+        for (int b = -1; b <= 1; ++b)
+            for (int c = -1; c <= 1; ++c) DIR[a + 1][b + 1][c + 1] = dir_index(a, b, c);
+    tables_ready = 1;
+}
+static int opposite(int i) { return OPP[i]; }
+
+typedef struct oracle {
+    int nx, ny, nz;
+    double nu0, Cs, fcor, F[3];
+    int face[6]; /* x-,x+,y-,y+,z-,z+ */
+    int have_flags;
+    uint8_t *cls; /* [z][y][x] */
+    double *G;    /* [cell][19], post-collision state G_k (step 3) */
+    double *Gn;   /* next */
+    double *ub;   /* [cell][3] prescribed velocity of EQ_FIXED cells */
+    long step;
+    double *msum; /* [cell][3] */
+    long mcount, mstart;
+    int mevery;
+} oracle_t;
+
+static long cell_of(const oracle_t *o, int x, int y, int z)
+{
+    return ((long)z * o->ny + y) * o->nx + x;
+}
+
+/* step 2: second-order equilibrium */
+static void feq(double rho, const double u[3], double out[Q])
+{
+    double uu = u[0] * u[0] + u[1] * u[1] + u[2] * u[2];
+    for (int i = 0; i < Q; ++i) {
+        double cu = CI[i][0] * u[0] + CI[i][1] * u[1] + CI[i][2] * u[2];
+        out[i] = weight(i) * rho * (1.0 + 3.0 * cu + 4.5 * cu * cu - 1.5 * uu);
+    }
+}
+
+/* step 4b-4e on one cell: pulled populations f[] -> post-collision g[].
+ * Also returns the (rho,u,tau) the collision used. */
+static void collide(const double f[Q], double nu0, double Cs, double fcor, const double F[3],
+                    double g[Q], double *rho_out, double u_out[3], double *tau_out)
+{
+    /* 4b moments */
+    double rho = 0.0, m[3] = {0, 0, 0};
+    for (int i = 0; i < Q; ++i) {
+        rho += f[i];
+        for (int a = 0; a < 3; ++a) m[a] += CI[i][a] * f[i];
+    }
+    /* 4c implicit half-force velocity: rho u = m + rho a(u)/2,
+     * a(u) = F + fcor (u_y, -u_x, 0) */
+    double h = 0.5 * fcor;
+    double b[3] = {m[0] / rho + 0.5 * F[0], m[1] / rho + 0.5 * F[1], m[2] / rho + 0.5 * F[2]};
+    double u[3];
+    u[0] = (b[0] + h * b[1]) / (1.0 + h * h);
+    u[1] = (b[1] - h * b[0]) / (1.0 + h * h);
+    u[2] = b[2];
+    double Fd[3]; /* force density rho a(u) */
+    Fd[0] = rho * (F[0] + fcor * u[1]);
+    Fd[1] = rho * (F[1] - fcor * u[0]);
+    Fd[2] = rho * F[2];
+    /* 4d LES: Pi = sum c c (f - feq); Q = Frobenius norm over all 9 entries */
+    double fe[Q];
+    feq(rho, u, fe);
+    double Pi[3][3] = {{0}};
+    for (int i = 0; i < Q; ++i)
+        for (int a = 0; a < 3; ++a)
+            for (int c = 0; c < 3; ++c) Pi[a][c] += CI[i][a] * CI[i][c] * (f[i] - fe[i]);
+    double QQ = 0.0;
+    for (int a = 0; a < 3; ++a)
+        for (int c = 0; c < 3; ++c) QQ += Pi[a][c] * Pi[a][c];
+    QQ = sqrt(QQ);
+    double tau0 = 3.0 * nu0 + 0.5;
+    double tau = 0.5 * (tau0 + sqrt(tau0 * tau0 + 18.0 * sqrt(2.0) * Cs * Cs * QQ / rho));
+    /* 4e BGK + Guo source */
+    for (int i = 0; i < Q; ++i) {
+        double cu = CI[i][0] * u[0] + CI[i][1] * u[1] + CI[i][2] * u[2];
+        double cF = CI[i][0] * Fd[0] + CI[i][1] * Fd[1] + CI[i][2] * Fd[2];
+        double cmuF = (CI[i][0] - u[0]) * Fd[0] + (CI[i][1] - u[1]) * Fd[1] + (CI[i][2] - u[2]) * Fd[2];
+        double S = (1.0 - 1.0 / (2.0 * tau)) * weight(i) * (3.0 * cmuF + 9.0 * cu * cF);
+        g[i] = f[i] - (f[i] - fe[i]) / tau + S;
+    }
+    if (rho_out) *rho_out = rho;
+    if (u_out) { u_out[0] = u[0]; u_out[1] = u[1]; u_out[2] = u[2]; }
+    if (tau_out) *tau_out = tau;
+}
+
+/* step 4a: where does population i of FLUID cell (x,y,z) come from?
+ * returns 1 = bounce-back branch (take G(x, opposite(i))), 0 = take G(*s, *j),
+ * -1 = an EQ face was crossed (cannot happen for a FLUID cell; reported). */
+static int resolve(const oracle_t *o, int x, int y, int z, int i, long *s, int *j)
+{
+    int p[3] = {x - CI[i][0], y - CI[i][1], z - CI[i][2]};
+    int c[3] = {CI[i][0], CI[i][1], CI[i][2]};
+    int n[3] = {o->nx, o->ny, o->nz};
+    int wall = 0;
+    static const int order[3] = {2, 1, 0}; /* z, then y, then x */
+    for (int k = 0; k < 3; ++k) {
+        int a = order[k];
+        int ft;
+        if (p[a] < 0) ft = o->face[2 * a];
+        else if (p[a] >= n[a]) ft = o->face[2 * a + 1];
+        else continue;
+        if (ft == F_PERIODIC) p[a] = (p[a] + n[a]) % n[a];
+        else if (ft == F_FREE_SLIP) { p[a] = p[a] < 0 ? 0 : n[a] - 1; c[a] = -c[a]; }
+        else if (ft == F_WALL) wall = 1;
+        else return -1;
+    }
+    if (wall) return 1;
+    *s = cell_of(o, p[0], p[1], p[2]);
+    if (o->cls[*s] == C_SOLID) return 1;
+    *j = DIR[c[0] + 1][c[1] + 1][c[2] + 1];
+    return 0;
+}
+
+/* step 7: local macros of the stored state at one cell */
+static void local_macros(const oracle_t *o, const double *Gs, long cell, double *rho, double u[3])
+{
+    int cl = o->cls ? o->cls[cell] : C_FLUID;
+    if (cl == C_SOLID) { *rho = 1.0; u[0] = u[1] = u[2] = 0.0; return; }
+    const double *g = Gs + cell * Q;
+    double r = 0.0, m[3] = {0, 0, 0};
+    for (int i = 0; i < Q; ++i) {
+        r += g[i];
+        for (int a = 0; a < 3; ++a) m[a] += CI[i][a] * g[i];
+    }
+    *rho = r;
+    if (cl == C_FLUID) {
+        /* invert m* = rho u + rho a(u)/2 */
+        double h = 0.5 * o->fcor;
+        double b[3] = {m[0] / r - 0.5 * o->F[0], m[1] / r - 0.5 * o->F[1], m[2] / r - 0.5 * o->F[2]};
+        u[0] = (b[0] - h * b[1]) / (1.0 + h * h);
+        u[1] = (b[1] + h * b[0]) / (1.0 + h * h);
+        u[2] = b[2];
+    } else {
+        u[0] = m[0] / r; u[1] = m[1] / r; u[2] = m[2] / r;
+    }
+}
+
+/* ------------------------------------------------------------------ C API */
+
+int oracle_lattice(int *c /*[19][3]*/, double *w /*[19]*/, int *opp /*[19]*/)
+{
+    init_tables();
+    for (int i = 0; i < Q; ++i) {
+        for (int a = 0; a < 3; ++a) c[3 * i + a] = CI[i][a];
+        w[i] = weight(i);
+        opp[i] = opposite(i);
+    }
+    return 0;
+}
+
+int oracle_feq(double rho, const double *u, double *out) { feq(rho, u, out); return 0; }
+
+int oracle_collide_cell(const double *f, double nu0, double Cs, double fcor, const double *F,
+                        double *g, double *rho, double *u, double *tau)
+{
+    collide(f, nu0, Cs, fcor, F, g, rho, u, tau);
+    return 0;
+}
+
+oracle_t *oracle_create(int nx, int ny, int nz, double nu0, double Cs, double fcor, const double *F)
+{
+    if (nx < 1 || ny < 1 || nz < 1) return NULL;
+    init_tables();
+    oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
+    if (!o) return NULL;
+    o->nx = nx; o->ny = ny; o->nz = nz;
+    o->nu0 = nu0; o->Cs = Cs; o->fcor = fcor;
+    for (int a = 0; a < 3; ++a) o->F[a] = F ? F[a] : 0.0;
+    /* default faces = config 1 */
+    o->face[0] = F_EQ_FIXED; o->face[1] = F_EQ_OUTFLOW;
+    o->face[2] = F_PERIODIC; o->face[3] = F_PERIODIC;
+    o->face[4] = F_WALL;     o->face[5] = F_FREE_SLIP;
+    long N = (long)nx * ny * nz;
+    o->cls = (uint8_t *)calloc(N, 1);
+    o->G = (double *)malloc(sizeof(double) * N * Q);
+    o->Gn = (double *)malloc(sizeof(double) * N * Q);
+    o->ub = (double *)calloc(N * 3, sizeof(double));
+    if (!o->cls || !o->G || !o->Gn || !o->ub) { free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o); return NULL; }
+    o->mstart = 0; o->mevery = 0;
+    return o;
+}
+
+void oracle_destroy(oracle_t *o)
+{
+    if (!o) return;
+    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o);
+}
+
+int oracle_set_boundaries(oracle_t *o, const int *face_type)
+{
+    for (int a = 0; a < 3; ++a) {
+        int lo = face_type[2 * a], hi = face_type[2 * a + 1];
+        if (lo < 0 || lo > 4 || hi < 0 || hi > 4) return -1;
+        if ((lo == F_PERIODIC) != (hi == F_PERIODIC)) return -1;
+    }
+    for (int k = 0; k < 6; ++k) o->face[k] = face_type[k];
+    o->have_flags = 0;
+    return 0;
+}
+
+/* step 9: SOLID <=> z < clamp(h,0,nz); non-solid cells of an EQ face take the
+ * EQ class, EQ_FIXED winning over EQ_OUTFLOW where two EQ faces meet. */
+int oracle_set_flags(oracle_t *o, const int32_t *height)
+{
+    for (int z = 0; z < o->nz; ++z)
+        for (int y = 0; y < o->ny; ++y)
+            for (int x = 0; x < o->nx; ++x) {
+                int h = height ? height[(long)y * o->nx + x] : 0;
+                if (h < 0) h = 0;
+                if (h > o->nz) h = o->nz;
+                int cl = C_FLUID;
+                if (z < h) cl = C_SOLID;
+                else {
+                    int on[6] = {x == 0, x == o->nx - 1, y == 0, y == o->ny - 1, z == 0, z == o->nz - 1};
+                    int fixed = 0, outflow = 0;
+                    for (int k = 0; k < 6; ++k) {
+                        if (on[k] && o->face[k] == F_EQ_FIXED) fixed = 1;
+                        if (on[k] && o->face[k] == F_EQ_OUTFLOW) outflow = 1;
+                    }
+                    if (fixed) cl = C_EQ_FIXED;
+                    else if (outflow) cl = C_EQ_OUTFLOW;
+                }
+                o->cls[cell_of(o, x, y, z)] = (uint8_t)cl;
+            }
+    o->have_flags = 1;
+    return 0;
+}
+
+int oracle_get_flags(const oracle_t *o, uint8_t *out)
+{
+    memcpy(out, o->cls, (size_t)o->nx * o->ny * o->nz);
+    return 0;
+}
+
+/* step 9: link bit i of a FLUID cell = "step 4a took the bounce-back branch" */
+int oracle_get_links(const oracle_t *o, uint32_t *out)
+{
+    for (int z = 0; z < o->nz; ++z)
+        for (int y = 0; y < o->ny; ++y)
+            for (int x = 0; x < o->nx; ++x) {
+                long cell = cell_of(o, x, y, z);
+                uint32_t bits = 0;
+                if (o->cls[cell] == C_FLUID)
+                    for (int i = 1; i < Q; ++i) {
+                        long s; int j;
+                        int r = resolve(o, x, y, z, i, &s, &j);
+                        if (r < 0) return -2;
+                        if (r == 1) bits |= (1u << i);
+                    }
+                out[cell] = bits;
+            }
+    return 0;
+}
+
+static void write_eq_fixed_cell(oracle_t *o, long cell)
+{
+    double g[Q];
+    feq(1.0, o->ub + 3 * cell, g);
+    memcpy(o->G + cell * Q, g, sizeof g);
+    memcpy(o->Gn + cell * Q, g, sizeof g);
+}
+
+/* step 5 (profile form): every EQ_FIXED cell gets f_eq(1, (u[z],v[z],w[z])) */
+int oracle_set_inlet_profile(oracle_t *o, const double *u, const double *v, const double *w)
+{
+    if (!o->have_flags) return -3;
+    for (int z = 0; z < o->nz; ++z)
+        for (int y = 0; y < o->ny; ++y)
+            for (int x = 0; x < o->nx; ++x) {
+                long cell = cell_of(o, x, y, z);
+                if (o->cls[cell] != C_EQ_FIXED) continue;
+                o->ub[3 * cell + 0] = u ? u[z] : 0.0;
+                o->ub[3 * cell + 1] = v ? v[z] : 0.0;
+                o->ub[3 * cell + 2] = w ? w[z] : 0.0;
+                write_eq_fixed_cell(o, cell);
+            }
+    return 0;
+}
+
+/* step 5 (plane form): EQ_FIXED cells of one face get f_eq(1, uvw[:,j2,j1]);
+ * uvw is [3][n2][n1] with (n2,n1) = (nz,ny) for x faces, (nz,nx) for y faces,
+ * (ny,nx) for z faces. */
+int oracle_set_inlet_plane(oracle_t *o, int face, const double *uvw)
+{
+    if (!o->have_flags) return -3;
+    if (face < 0 || face > 5) return -1;
+    int axis = face / 2;
+    int n[3] = {o->nx, o->ny, o->nz};
+    int fixed = (face % 2) ? n[axis] - 1 : 0;
+    int a1 = axis == 0 ? 1 : 0;           /* fast in-plane axis */
+    int a2 = axis == 2 ? 1 : 2;           /* slow in-plane axis */
+    long plane = (long)n[a1] * n[a2];
+    for (int j2 = 0; j2 < n[a2]; ++j2)
+        for (int j1 = 0; j1 < n[a1]; ++j1) {
+            int p[3];
+            p[axis] = fixed; p[a1] = j1; p[a2] = j2;
+            long cell = cell_of(o, p[0], p[1], p[2]);
+            if (o->cls[cell] != C_EQ_FIXED) continue;
+            for (int a = 0; a < 3; ++a) o->ub[3 * cell + a] = uvw[a * plane + (long)j2 * n[a1] + j1];
+            write_eq_fixed_cell(o, cell);
+        }
+    return 0;
+}
+
+/* step 3 / a4: G0 = f_eq(rho0,u0); NULL rho => 1; NULL velocity component => 0.
+ * SOLID cells: rho=1,u=0.  EQ_FIXED cells keep their prescribed state. */
+int oracle_set_macros(oracle_t *o, const double *rho, const double *ux, const double *uy, const double *uz)
+{
+    if (!o->have_flags) return -3;
+    long N = (long)o->nx * o->ny * o->nz;
+    for (long cell = 0; cell < N; ++cell) {
+        int cl = o->cls[cell];
+        if (cl == C_EQ_FIXED) { write_eq_fixed_cell(o, cell); continue; }
+        double r = rho ? rho[cell] : 1.0;
+        double u[3] = {ux ? ux[cell] : 0.0, uy ? uy[cell] : 0.0, uz ? uz[cell] : 0.0};
+        if (cl == C_SOLID) { r = 1.0; u[0] = u[1] = u[2] = 0.0; }
+        double g[Q];
+        feq(r, u, g);
+        memcpy(o->G + cell * Q, g, sizeof g);
+        memcpy(o->Gn + cell * Q, g, sizeof g);
+    }
+    o->step = 0;
+    return 0;
+}
+
+/* which face's normal an EQ_OUTFLOW cell uses: the first EQ_OUTFLOW face it
+ * lies on, in the order x-,x+,y-,y+,z-,z+ (reading R-outflow-edge) */
+static int outflow_face(const oracle_t *o, int x, int y, int z)
+{
+    int on[6] = {x == 0, x == o->nx - 1, y == 0, y == o->ny - 1, z == 0, z == o->nz - 1};
+    for (int k = 0; k < 6; ++k)
+        if (on[k] && o->face[k] == F_EQ_OUTFLOW) return k;
+    return -1;
+}
+
+static void sample_mean(oracle_t *o)
+{
+    long N = (long)o->nx * o->ny * o->nz;
+    if (!o->msum) o->msum = (double *)calloc(N * 3, sizeof(double));
+#pragma omp parallel for schedule(static)
+    for (long cell = 0; cell < N; ++cell) {
+        double r, u[3];
+        local_macros(o, o->G, cell, &r, u);
+        for (int a = 0; a < 3; ++a) o->msum[3 * cell + a] += u[a];
+    }
+    o->mcount += 1;
+}
+
+int oracle_step(oracle_t *o, int nsteps)
+{
+    if (!o->have_flags) return -3;
+    int bad = 0;
+    for (int it = 0; it < nsteps; ++it) {
+#pragma omp parallel for schedule(static)
+        for (int z = 0; z < o->nz; ++z)
+            for (int y = 0; y < o->ny; ++y)
+                for (int x = 0; x < o->nx; ++x) {
+                    long cell = cell_of(o, x, y, z);
+                    int cl = o->cls[cell];
+                    double *gn = o->Gn + cell * Q;
+                    if (cl == C_FLUID) {
+                        /* step 4a pull */
+                        double f[Q];
+                        for (int i = 0; i < Q; ++i) {
+                            long s = 0; int j = 0;
+                            int r = resolve(o, x, y, z, i, &s, &j);
+                            if (r < 0) { bad = 1; r = 1; }
+                            f[i] = r ? o->G[cell * Q + opposite(i)] : o->G[s * Q + j];
+                        }
+                        collide(f, o->nu0, o->Cs, o->fcor, o->F, gn, NULL, NULL, NULL);
+                    } else if (cl == C_EQ_OUTFLOW) {
+                        /* step 6 */
+                        int k = outflow_face(o, x, y, z);
+                        int p[3] = {x, y, z};
+                        p[k / 2] += (k % 2) ? -1 : +1; /* x - n, n outward */
+                        int n[3] = {o->nx, o->ny, o->nz};
+                        double r, u[3] = {0, 0, 0};
+                        if (p[k / 2] >= 0 && p[k / 2] < n[k / 2])
+                            local_macros(o, o->G, cell_of(o, p[0], p[1], p[2]), &r, u);
+                        feq(1.0, u, gn);
+                    } else {
+                        /* SOLID: inert; EQ_FIXED (step 5): unchanged */
+                        memcpy(gn, o->G + cell * Q, sizeof(double) * Q);
+                    }
+                }
+        double *t = o->G; o->G = o->Gn; o->Gn = t;
+        o->step += 1;
+        /* step 8 */
+        if (o->mevery > 0 && o->step >= o->mstart && (o->step - o->mstart) % o->mevery == 0) sample_mean(o);
+    }
+    return bad ? -2 : 0;
+}
+
+int oracle_get_macros(const oracle_t *o, double *rho, double *ux, double *uy, double *uz)
+{
+    long N = (long)o->nx * o->ny * o->nz;
+#pragma omp parallel for schedule(static)
+    for (long cell = 0; cell < N; ++cell) {
+        double r, u[3];
+        local_macros(o, o->G, cell, &r, u);
+        if (rho) rho[cell] = r;
+        if (ux) ux[cell] = u[0];
+        if (uy) uy[cell] = u[1];
+        if (uz) uz[cell] = u[2];
+    }
+    return 0;
+}
+
+int oracle_mean_config(oracle_t *o, long start_step, int every)
+{
+    o->mstart = start_step; o->mevery = every;
+    return 0;
+}
+
+int oracle_mean_reset(oracle_t *o)
+{
+    long N = (long)o->nx * o->ny * o->nz;
+    if (o->msum) memset(o->msum, 0, sizeof(double) * N * 3);
+    o->mcount = 0;
+    return 0;
+}
+
+/* step 8: mean = sum / count (SOLID cells contribute and return 0) */
+int oracle_get_mean(const oracle_t *o, double *ux, double *uy, double *uz, long *n_samples)
+{
+    long N = (long)o->nx * o->ny * o->nz;
+    if (n_samples) *n_samples = o->mcount;
+    for (long cell = 0; cell < N; ++cell) {
+        double inv = o->mcount > 0 ? 1.0 / (double)o->mcount : 0.0;
+        double s0 = o->msum ? o->msum[3 * cell + 0] : 0.0;
+        double s1 = o->msum ? o->msum[3 * cell + 1] : 0.0;
+        double s2 = o->msum ? o->msum[3 * cell + 2] : 0.0;
+        if (ux) ux[cell] = s0 * inv;
+        if (uy) uy[cell] = s1 * inv;
+        if (uz) uz[cell] = s2 * inv;
+    }
+    return 0;
+}
+
+/* raw populations, [19][nz][ny][nx] in the order of step 1 */
+int oracle_get_state(const oracle_t *o, double *f)
+{
+    long N = (long)o->nx * o->ny * o->nz;
+    for (int i = 0; i < Q; ++i)
+        for (long cell = 0; cell < N; ++cell) f[(long)i * N + cell] = o->G[cell * Q + i];
+    return 0;
+}
+
+int oracle_set_state(oracle_t *o, const double *f)
+{
+    long N = (long)o->nx * o->ny * o->nz;
+    for (int i = 0; i < Q; ++i)
+        for (long cell = 0; cell < N; ++cell) {
+            o->G[cell * Q + i] = f[(long)i * N + cell];
+            o->Gn[cell * Q + i] = f[(long)i * N + cell];
+        }
+    return 0;
+}
+
+long oracle_get_step(const oracle_t *o) { return o->step; }
+int oracle_set_step(oracle_t *o, long s) { o->step = s; return 0; }

@@ -1,0 +1,199 @@
+"""ctypes binding of oracle/lbm_oracle.c (TEST INFRASTRUCTURE — see that file's header).
+
+``build()`` compiles the C file with gcc (``-O3 -fopenmp``, no fast-math) into
+``oracle/liblbm_oracle.so``; everything else is argument marshalling.
+Arrays are numpy float64, C order ``[z][y][x]``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "lbm_oracle.c")
+_SO = os.path.join(_HERE, "liblbm_oracle.so")
+_lib = None
+
+FLUID, SOLID, EQ_FIXED, EQ_OUTFLOW = 0, 1, 2, 3
+PERIODIC, WALL, FREE_SLIP, FACE_EQ_FIXED, FACE_EQ_OUTFLOW = 0, 1, 2, 3, 4
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle if the .so is missing or older than the source."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O3", "-fopenmp", "-std=c99", "-shared", "-fPIC", "-o", _SO, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _SO
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build()
+    lib = C.CDLL(_SO)
+    dp = C.POINTER(C.c_double)
+    lib.oracle_create.restype = C.c_void_p
+    lib.oracle_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, dp]
+    lib.oracle_destroy.restype = None
+    lib.oracle_destroy.argtypes = [C.c_void_p]
+    lib.oracle_get_step.restype = C.c_long
+    lib.oracle_get_step.argtypes = [C.c_void_p]
+    lib.oracle_set_step.argtypes = [C.c_void_p, C.c_long]
+    lib.oracle_mean_config.argtypes = [C.c_void_p, C.c_long, C.c_int]
+    for name in ("oracle_set_boundaries", "oracle_set_flags", "oracle_get_flags", "oracle_get_links",
+                 "oracle_set_inlet_profile", "oracle_set_inlet_plane", "oracle_set_macros", "oracle_step",
+                 "oracle_get_macros", "oracle_mean_reset", "oracle_get_mean",
+                 "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell"):
+        getattr(lib, name).restype = C.c_int
+    _lib = lib
+    return lib
+
+
+def _d(a):
+    """float64 C-contiguous view/copy and its pointer (None -> NULL)."""
+    if a is None:
+        return None, None
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def lattice():
+    """(c[19,3] int, w[19] float64, opposite[19] int) as the oracle defines them."""
+    lib = _load()
+    c = np.zeros((19, 3), dtype=np.int32)
+    w = np.zeros(19, dtype=np.float64)
+    opp = np.zeros(19, dtype=np.int32)
+    lib.oracle_lattice(c.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p), opp.ctypes.data_as(C.c_void_p))
+    return c, w, opp
+
+
+def feq(rho, u):
+    lib = _load()
+    u, up = _d(np.asarray(u, dtype=np.float64))
+    out = np.zeros(19)
+    lib.oracle_feq(C.c_double(rho), up, out.ctypes.data_as(C.c_void_p))
+    return out
+
+
+def collide_cell(f, nu0, Cs, fcor, F):
+    """One cell's step 4b-4e.  Returns (g[19], rho, u[3], tau)."""
+    lib = _load()
+    f, fp = _d(f)
+    F, Fp = _d(np.asarray(F, dtype=np.float64))
+    g = np.zeros(19)
+    rho = C.c_double()
+    u = np.zeros(3)
+    tau = C.c_double()
+    lib.oracle_collide_cell(fp, C.c_double(nu0), C.c_double(Cs), C.c_double(fcor), Fp,
+                            g.ctypes.data_as(C.c_void_p), C.byref(rho), u.ctypes.data_as(C.c_void_p), C.byref(tau))
+    return g, rho.value, u, tau.value
+
+
+class Oracle:
+    """FP64 CPU LBM; same call names as the product binding, float64 arrays."""
+
+    def __init__(self, nx, ny, nz, nu0, Cs=0.0, f_cor=0.0, F=(0.0, 0.0, 0.0), faces=None):
+        self._lib = _load()
+        F = np.atleast_1d(np.asarray(F, dtype=np.float64))
+        if F.size == 1:
+            F = np.array([F[0], 0.0, 0.0])
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.shape = (self.nz, self.ny, self.nx)
+        self._h = self._lib.oracle_create(self.nx, self.ny, self.nz, C.c_double(nu0), C.c_double(Cs),
+                                          C.c_double(f_cor), F.ctypes.data_as(C.POINTER(C.c_double)))
+        if not self._h:
+            raise MemoryError("oracle_create failed")
+        if faces is not None:
+            self.set_boundaries(faces)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.oracle_destroy(C.c_void_p(self._h))
+            self._h = None
+
+    __del__ = close
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise RuntimeError(f"oracle {what} failed: {rc}")
+
+    def set_boundaries(self, faces):
+        a = np.ascontiguousarray(faces, dtype=np.int32)
+        assert a.shape == (6,)
+        self._chk(self._lib.oracle_set_boundaries(C.c_void_p(self._h), a.ctypes.data_as(C.c_void_p)), "set_boundaries")
+
+    def set_flags(self, height=None):
+        if height is None:
+            height = np.zeros((self.ny, self.nx), dtype=np.int32)
+        a = np.ascontiguousarray(height, dtype=np.int32)
+        assert a.shape == (self.ny, self.nx)
+        self._chk(self._lib.oracle_set_flags(C.c_void_p(self._h), a.ctypes.data_as(C.c_void_p)), "set_flags")
+
+    def get_flags(self):
+        out = np.zeros(self.shape, dtype=np.uint8)
+        self._chk(self._lib.oracle_get_flags(C.c_void_p(self._h), out.ctypes.data_as(C.c_void_p)), "get_flags")
+        return out
+
+    def get_links(self):
+        out = np.zeros(self.shape, dtype=np.uint32)
+        self._chk(self._lib.oracle_get_links(C.c_void_p(self._h), out.ctypes.data_as(C.c_void_p)), "get_links")
+        return out
+
+    def set_inlet_profile(self, u, v=None, w=None):
+        u, up = _d(u)
+        v, vp = _d(v)
+        w, wp = _d(w)
+        assert u.shape == (self.nz,)
+        self._chk(self._lib.oracle_set_inlet_profile(C.c_void_p(self._h), up, vp, wp), "set_inlet_profile")
+
+    def set_inlet_plane(self, face, uvw):
+        uvw, p = _d(uvw)
+        self._chk(self._lib.oracle_set_inlet_plane(C.c_void_p(self._h), int(face), p), "set_inlet_plane")
+
+    def set_macros(self, rho=None, ux=None, uy=None, uz=None):
+        arrs = [_d(a) for a in (rho, ux, uy, uz)]
+        for a, _ in arrs:
+            assert a is None or a.shape == self.shape
+        self._chk(self._lib.oracle_set_macros(C.c_void_p(self._h), *[p for _, p in arrs]), "set_macros")
+
+    def step(self, n=1):
+        self._chk(self._lib.oracle_step(C.c_void_p(self._h), int(n)), "step")
+
+    def get_macros(self):
+        out = [np.zeros(self.shape) for _ in range(4)]
+        self._chk(self._lib.oracle_get_macros(C.c_void_p(self._h), *[a.ctypes.data_as(C.c_void_p) for a in out]),
+                  "get_macros")
+        return tuple(out)
+
+    def mean_config(self, start_step, every):
+        self._chk(self._lib.oracle_mean_config(C.c_void_p(self._h), C.c_long(start_step), int(every)), "mean_config")
+
+    def mean_reset(self):
+        self._chk(self._lib.oracle_mean_reset(C.c_void_p(self._h)), "mean_reset")
+
+    def get_mean(self):
+        out = [np.zeros(self.shape) for _ in range(3)]
+        n = C.c_long()
+        self._chk(self._lib.oracle_get_mean(C.c_void_p(self._h), *[a.ctypes.data_as(C.c_void_p) for a in out],
+                                            C.byref(n)), "get_mean")
+        return out[0], out[1], out[2], n.value
+
+    def get_state(self):
+        out = np.zeros((19,) + self.shape)
+        self._chk(self._lib.oracle_get_state(C.c_void_p(self._h), out.ctypes.data_as(C.c_void_p)), "get_state")
+        return out
+
+    def set_state(self, f):
+        f, p = _d(f)
+        assert f.shape == (19,) + self.shape
+        self._chk(self._lib.oracle_set_state(C.c_void_p(self._h), p), "set_state")
+
+    def get_step(self):
+        return int(self._lib.oracle_get_step(C.c_void_p(self._h)))
+
+    def set_step(self, s):
+        self._lib.oracle_set_step(C.c_void_p(self._h), C.c_long(s))

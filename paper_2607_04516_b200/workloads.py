@@ -1,0 +1,196 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs (and their crops).
+
+This module holds NO arithmetic of the method — no lattice table, no
+equilibrium, no collision.  It only produces the arrays a caller hands to the
+solver (heightmaps, boundary wind profiles, initial macroscopic fields) and the
+scalar parameters of each config, so that the CUDA library and the CPU oracle
+can be fed bit-identical inputs.  numpy only.
+
+The arrays stand in for the paper's datasets (3D-GloBFP buildings and NASADEM
+terrain; Guangzhou lidar profiles), none of
+which exist on this box; shapes follow the paper's workload (5 m cells,
+kilometre-scale; building short sides mostly < 50 m = 10
+cells).  Recipes: DESIGN.md "Input recipe" (= SURVEY.md §8(d)).
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+# face types of the C ABI (include/lbm.h), order x-,x+,y-,y+,z-,z+
+PERIODIC, WALL, FREE_SLIP, EQ_FIXED, EQ_OUTFLOW = 0, 1, 2, 3, 4
+
+
+@dataclass
+class Workload:
+    name: str
+    nx: int
+    ny: int
+    nz: int
+    nu0: float
+    Cs: float
+    f_cor: float
+    F: tuple
+    faces: tuple
+    steps: int
+    height: np.ndarray                      # int32 [ny][nx]
+    inlet_profile: tuple | None = None      # (u[nz], v[nz] | None, w[nz] | None) float32
+    init: tuple | None = None               # (rho, ux, uy, uz) float32 [nz][ny][nx], entries may be None
+    mean_start: int = 0
+    mean_every: int = 0
+    extra: dict = field(default_factory=dict)
+
+    @property
+    def cells(self) -> int:
+        return self.nx * self.ny * self.nz
+
+    @property
+    def shape(self):
+        return (self.nz, self.ny, self.nx)
+
+
+# --------------------------------------------------------------------------- profiles
+
+def log_law_profile(nz: int, u_ref: float, zeta_ref: float, z0: float) -> np.ndarray:
+    """|U|(zeta) = u_ref ln(zeta/z0)/ln(zeta_ref/z0) at cell centres zeta = z + 1/2, clipped at >= 0."""
+    zeta = np.arange(nz, dtype=np.float64) + 0.5
+    u = u_ref * np.log(zeta / z0) / math.log(zeta_ref / z0)
+    return np.maximum(u, 0.0).astype(np.float32)
+
+
+def veering_profile(nz: int, u_ref: float, zeta_ref: float, z0: float, seed: int,
+                    theta_max_deg: float = 60.0, jitter: float = 0.1):
+    """Config-4 inlet: log-law speed, direction turning 0..theta_max over the depth with a
+    seeded +-10 % perturbation  theta(zeta) = theta_max (zeta/nz) (1 + jitter s(zeta)),
+    s = sum of 3 seeded sine modes normalised to max|s| = 1."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    zeta = np.arange(nz, dtype=np.float64) + 0.5
+    amp = rng.uniform(0.5, 1.0, size=3)
+    phase = rng.uniform(0.0, 2.0 * math.pi, size=3)
+    s = sum(a * np.sin(2.0 * math.pi * (m + 1) * zeta / nz + p) for m, (a, p) in enumerate(zip(amp, phase)))
+    s = s / np.max(np.abs(s))
+    theta = np.deg2rad(theta_max_deg) * (zeta / nz) * (1.0 + jitter * s)
+    speed = log_law_profile(nz, u_ref, zeta_ref, z0).astype(np.float64)
+    return (speed * np.cos(theta)).astype(np.float32), (speed * np.sin(theta)).astype(np.float32)
+
+
+# --------------------------------------------------------------------------- heightmaps
+
+def block_heightmap(nx, ny, x0, x1, y0, y1, h) -> np.ndarray:
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    hm[y0:y1 + 1, x0:x1 + 1] = h
+    return hm
+
+
+def urban_heightmap(nx: int, ny: int, seed: int, plan_fraction: float = 0.35, wmin: int = 2, wmax: int = 12,
+                    h_median: float = 6.0, h_sigma: float = 0.6, h_max: int = 40, x_margin: int = 8) -> np.ndarray:
+    """Rectangular footprints w,l ~ U{wmin..wmax}, height = clip(round(h_median exp(sigma N(0,1))), 1, h_max),
+    uniform positions with a building-free margin at the x faces, overlaps resolved by max, drawn until the
+    built plan-area fraction (of the whole map) reaches plan_fraction."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    target = plan_fraction * nx * ny
+    built = 0
+    batch = 256
+    while built < target:
+        w = rng.integers(wmin, wmax + 1, size=batch)
+        l = rng.integers(wmin, wmax + 1, size=batch)
+        h = np.clip(np.rint(h_median * np.exp(h_sigma * rng.standard_normal(batch))), 1, h_max).astype(np.int32)
+        ux = rng.random(batch)
+        uy = rng.random(batch)
+        for k in range(batch):
+            xs = x_margin + int(ux[k] * (nx - 2 * x_margin - w[k] + 1))
+            ys = int(uy[k] * (ny - l[k] + 1))
+            blk = hm[ys:ys + l[k], xs:xs + w[k]]
+            built += int(np.count_nonzero(blk == 0))
+            np.maximum(blk, h[k], out=blk)
+            if built >= target:
+                break
+    return hm
+
+
+# --------------------------------------------------------------------------- configs
+
+def config1() -> Workload:
+    """Tiny block flow, 64x32x32 (BASELINE.json configs[0])."""
+    nx, ny, nz = 64, 32, 32
+    hm = block_heightmap(nx, ny, 16, 23, 12, 19, 16)
+    u = log_law_profile(nz, 0.05, 16.0, 0.1)
+    ux = np.broadcast_to(u[:, None, None], (nz, ny, nx)).astype(np.float32).copy()
+    return Workload("C1_block_64x32x32", nx, ny, nz, 1e-3, 0.1, 1e-3, (0.0, 0.0, 0.0),
+                    (EQ_FIXED, EQ_OUTFLOW, PERIODIC, PERIODIC, WALL, FREE_SLIP), 200, hm,
+                    inlet_profile=(u, None, None), init=(None, ux, None, None))
+
+
+def config2(Cs: float = 0.0, n: int = 128, nz: int | None = None) -> Workload:
+    """Periodic Taylor-Green + Coriolis, n^3 (BASELINE.json configs[1]); run A Cs=0, run B Cs=0.1."""
+    nz = n if nz is None else nz
+    k = 2.0 * math.pi / n
+    u0, ub = 0.04, 0.02
+    x = np.arange(n, dtype=np.float64)
+    X, Y = np.meshgrid(x, x, indexing="xy")  # [y][x]
+    ux2 = u0 * np.sin(k * X) * np.cos(k * Y) + ub
+    uy2 = -u0 * np.cos(k * X) * np.sin(k * Y)
+    rho2 = 1.0 - 0.75 * u0 * u0 * (np.cos(2 * k * X) + np.cos(2 * k * Y))
+    ext = lambda a: np.broadcast_to(a[None], (nz, n, n)).astype(np.float32).copy()  # noqa: E731
+    return Workload(f"C2_tgv_{n}x{n}x{nz}_Cs{Cs:g}", n, n, nz, 2e-3, Cs, 2e-4, (0.0, 0.0, 0.0),
+                    (PERIODIC,) * 6, 1000, np.zeros((n, n), dtype=np.int32),
+                    init=(ext(rho2), ext(ux2), ext(uy2), None), extra={"k": k, "u0": u0, "ub": ub})
+
+
+def _urban(name, nx, ny, nz, hm, u_ref, zeta_ref, z0, nu0, f_cor, steps, faces=None) -> Workload:
+    u = log_law_profile(nz, u_ref, zeta_ref, z0)
+    ux = np.broadcast_to(u[:, None, None], (nz, ny, nx)).astype(np.float32).copy()
+    faces = faces or (EQ_FIXED, EQ_OUTFLOW, FREE_SLIP, FREE_SLIP, WALL, FREE_SLIP)
+    return Workload(name, nx, ny, nz, nu0, 0.1, f_cor, (0.0, 0.0, 0.0), faces, steps, hm,
+                    inlet_profile=(u, None, None), init=(None, ux, None, None),
+                    mean_start=steps // 2, mean_every=10)
+
+
+def config3(nx: int = 400, ny: int = 400, nz: int = 100) -> Workload:
+    """Synthetic 2 km urban domain at 5 m, 400x400x100 (BASELINE.json configs[2]); crops keep the recipe."""
+    hm = urban_heightmap(400, 400, seed=3)[:ny, :nx].copy()
+    return _urban(f"C3_urban_{nx}x{ny}x{nz}", nx, ny, nz, hm, 0.08, 20.0, 0.2, 1e-4, 2.9e-6, 20000)
+
+
+def config4(nx: int = 800, ny: int = 800, nz: int = 200) -> Workload:
+    """Refined urban domain at 2.5 m, 800x800x200 (BASELINE.json configs[3]): config-3 map x2 in cells,
+    heights x2; veering inlet on x-, y-, y+; outflow on x+."""
+    hm = np.kron(urban_heightmap(400, 400, seed=3), np.ones((2, 2), dtype=np.int32)).astype(np.int32) * 2
+    hm = hm[:ny, :nx].copy()
+    u, v = veering_profile(nz, 0.08, 40.0, 0.4, seed=4)
+    bc = lambda a: np.broadcast_to(a[:, None, None], (nz, ny, nx)).astype(np.float32).copy()  # noqa: E731
+    return Workload(f"C4_urban_{nx}x{ny}x{nz}", nx, ny, nz, 5e-5, 0.1, 1.5e-6, (0.0, 0.0, 0.0),
+                    (EQ_FIXED, EQ_OUTFLOW, EQ_FIXED, EQ_FIXED, WALL, FREE_SLIP), 20000, hm,
+                    inlet_profile=(u, v, None), init=(None, bc(u), bc(v), None), mean_start=10000, mean_every=10)
+
+
+def config5_precursor(nx: int = 256, ny: int = 256, nz: int = 200) -> Workload:
+    """Periodic precursor box 256x256x200 (BASELINE.json configs[4], first half): flat ground, pressure-gradient
+    force 1e-6 + Coriolis, initial log-law + 2 % seeded noise."""
+    rng = np.random.Generator(np.random.PCG64(55))
+    u = log_law_profile(nz, 0.08, 20.0, 0.2)
+    base = np.broadcast_to(u[:, None, None], (nz, ny, nx)).astype(np.float64)
+    noise = lambda: (0.02 * 0.08 * rng.standard_normal((nz, ny, nx)))  # noqa: E731
+    ux = (base + noise()).astype(np.float32)
+    uy = noise().astype(np.float32)
+    uz = noise().astype(np.float32)
+    return Workload(f"C5_precursor_{nx}x{ny}x{nz}", nx, ny, nz, 1e-4, 0.1, 2.9e-6, (1e-6, 0.0, 0.0),
+                    (PERIODIC, PERIODIC, PERIODIC, PERIODIC, WALL, FREE_SLIP), 10000,
+                    np.zeros((ny, nx), dtype=np.int32), init=(None, ux, uy, uz), extra={"sample_plane_x": nx // 2})
+
+
+def config5_main(nx: int = 1200, ny: int = 1200, nz: int = 200) -> Workload:
+    """Main urban domain 1200x1200x200 of config 5 (seed-5 heightmap with config-3 statistics); its x- inlet is
+    fed every step from the precursor plane."""
+    hm = urban_heightmap(1200, 1200, seed=5)[:ny, :nx].copy()
+    return _urban(f"C5_main_{nx}x{ny}x{nz}", nx, ny, nz, hm, 0.08, 20.0, 0.2, 1e-4, 2.9e-6, 10000)
+
+
+def mean_profile(u: np.ndarray, flags: np.ndarray, solid_code: int = 1) -> np.ndarray:
+    """Horizontal average over non-SOLID cells of each level z (post-processing, not part of the method)."""
+    fluid = flags != solid_code
+    cnt = np.maximum(fluid.sum(axis=(1, 2)), 1)
+    return (np.where(fluid, u, 0.0).sum(axis=(1, 2), dtype=np.float64)) / cnt
