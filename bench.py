@@ -1,0 +1,287 @@
+#!/usr/bin/env python
+"""bench.py — MLUPS of the fused D3Q19 stream-collide path on the 400x400x100 urban config (BASELINE.json).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-cpu-baseline]
+
+One bench "step" = one LBM time step of the whole lattice = one launch of the fused stream-collide kernel
+(pull + bounce-back/free-slip/periodic resolution + moments + Coriolis/F + Smagorinsky + BGK/Guo + store, outflow
+cells included).  `value` = cells x K / device time (CUDA events on the handle's stream, inputs resident in HBM).
+`e2e` = the same metric for the whole job through the C ABI with pinned HOST buffers: heightmap, inlet profile and
+initial field copied in, K steps, rho/u copied out — all inside the timed region.
+N > 1 (torchrun): the path does not shard (north_star: one GPU, no collectives) -> N independent replicas, weak scaling.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on the host cores on a bounded crop of the workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+BYTES_PER_CELL = 153  # 19x4 B loads + 19x4 B stores + 1 flag byte (BASELINE.json north_star)
+METRIC = "MLUPS (D3Q19 FP32), fused stream-collide, 400x400x100 urban config, 1 B200"
+
+
+def load_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_traffic():
+    """dram bytes per launch of the step kernel from the committed ncu summary, if any (profiles/roofline_traffic.json)."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["dram_bytes_per_launch"])
+        except Exception:
+            return None
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index = index
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(",") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, reasons, mx = [], set(), None
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+                for k, nme in enumerate(names):
+                    if r[3 + k].strip().lower().startswith("active"):
+                        reasons.add(nme)
+            except Exception:
+                continue
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=mx, reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def oracle_for(wl):
+    from oracle import Oracle
+    o = Oracle(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces)
+    o.set_flags(wl.height)
+    o.set_inlet_profile(*wl.inlet_profile)
+    o.set_macros(*wl.init)
+    return o
+
+
+def cpu_baseline(budget_s=15.0):
+    """The oracle as it stands, on this host's cores, on a bounded sample of the workload: the full 400x400 plan,
+    lowest 25 levels (where the buildings are), a few steps."""
+    from paper_2607_04516_b200 import workloads as W
+    cores = len(os.sched_getaffinity(0))
+    wl = W.config3(nz=25)
+    o = oracle_for(wl)
+    t0 = time.perf_counter(); o.step(1); t1 = time.perf_counter() - t0
+    n = max(2, min(50, int(budget_s / max(t1, 1e-3))))
+    t0 = time.perf_counter(); o.step(n); dt = time.perf_counter() - t0
+    return {"value": wl.cells * n / dt / 1e6, "unit": "MLUPS", "cores": cores, "kind": "oracle",
+            "sample": f"config-3 heightmap and inlet, 400x400x25 slab (4.0e6 cells), {n} steps, FP64, OpenMP {cores} threads"}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores; each step = one LBM step on a bounded crop of config 3."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2607_04516_b200 import workloads as W
+    cores = len(os.sched_getaffinity(0))
+    budget = 150.0
+    nz = 25
+    wl = W.config3(nz=nz)
+    o = oracle_for(wl)
+    t0 = time.perf_counter(); o.step(1); t1 = time.perf_counter() - t0
+    total = args.steps + args.warmup
+    if t1 * total > budget:  # shrink the crop in y so that the whole run fits the budget
+        ny = max(16, int(400 * budget / (t1 * total)) // 8 * 8)
+        wl = W.config3(ny=ny, nz=nz)
+        o = oracle_for(wl)
+    o.step(args.warmup)
+    t0 = time.perf_counter(); o.step(args.steps); dt = time.perf_counter() - t0
+    v = wl.cells * args.steps / dt / 1e6
+    sample = f"config-3 crop {wl.nx}x{wl.ny}x{wl.nz} ({wl.cells:.3g} cells), FP64 oracle, OpenMP {cores} threads"
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "MLUPS", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "C3 urban 400x400x100 (BASELINE.json configs[2]); reference arm runs a bounded crop", "sample": sample},
+            "cpu_baseline": {"value": v, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the LBM path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    from paper_2607_04516_b200 import binding, build, workloads as W
+    build.build()
+    wl = W.config3()
+    K, Wm = args.steps, max(args.warmup, 3)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------- device-resident timing: K launches of the fused kernel
+    sim = binding.from_workload(wl, want_mean=False, device=f"cuda:{local}")
+    if args.variant:
+        sim.set_variant(args.variant)
+    sim.step(Wm)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    l0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    reps = max(1, args.repeats)
+    best = None
+    for _ in range(reps):
+        barrier()
+        e0.record()
+        sim.step(K)
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    launches = (sim.launch_count() - l0) // reps
+    clocks = sampler.stop() if rank == 0 else None
+    rho, ux, uy, uz = sim.get_macros()
+    finite = bool(torch.isfinite(ux).all().item())
+    t = torch.tensor([best], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    mlups = wl.cells * K * world / (ms_total * 1e-3) / 1e6
+
+    # ---------------- end to end through the C ABI with pinned host buffers
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()  # noqa: E731
+    h_height, h_u, h_ux0 = pin(wl.height), pin(wl.inlet_profile[0]), pin(wl.init[1])
+    outs = [torch.empty(wl.shape, dtype=torch.float32).pin_memory() for _ in range(4)]
+    lib = binding.load_library()
+
+    def job(s):
+        s.set_flags(h_height)
+        s.set_inlet_profile(h_u)
+        s.set_macros(None, h_ux0, None, None)
+        s.step(K)
+        rc = lib.lbm_get_macros(s._h, *[o.data_ptr() for o in outs])
+        assert rc == 0
+    job(sim)  # warm-up of the copy paths
+    barrier()
+    t0 = time.perf_counter()
+    e0.record()
+    job(sim)
+    e1.record()
+    barrier()
+    wall = time.perf_counter() - t0
+    t = torch.tensor([max(e0.elapsed_time(e1) * 1e-3, wall)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_s = float(t.item())
+    h2d = h_height.nbytes + h_u.nbytes + h_ux0.nbytes
+    d2h = sum(o.numel() * 4 for o in outs)
+    e2e = {"value": wl.cells * K * world / e2e_s / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": h2d / K,
+           "d2h_bytes_per_step": d2h / K,
+           "what": f"one job = set_flags + set_inlet_profile + set_macros from pinned host buffers, lbm_step({K}), "
+                   "lbm_get_macros into pinned host buffers"}
+
+    if rank == 0:
+        peak, peak_src = load_peak()
+        per_launch_s = ms_total * 1e-3 / K
+        achieved = BYTES_PER_CELL * wl.cells / per_launch_s / 1e9
+        line = {
+            "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "C3 urban 400x400x100 (BASELINE.json configs[2]): seeded heightmap plan fraction 0.35, "
+                                   "log-law inlet, nu0 1e-4, Cs 0.1, f 2.9e-6",
+                       "cells": wl.cells, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "no flush needed: each step streams 2.4 GB (>> 126 MB L2)", "best_of": reps,
+                       "state_finite": finite},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": load_traffic(), "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": BYTES_PER_CELL * wl.cells,
+                         "frac_of_nominal_8000": achieved / 8000.0},
+            "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            line["cpu_baseline"] = cpu_baseline()
+        elif world > 1:
+            line["cpu_baseline"] = None
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--repeats", type=int, default=1, help="timed repetitions of the K-step region; best is reported")
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,153 @@
+/*
+ * lbm.h — C ABI of the B200-native D3Q19 LBM-LES stream-collide library
+ *         (paper_2607_04516_b200/liblbm_b200.so, built for sm_100a).
+ *
+ * What the calls are.  The paper's problem statement for the solver (§2, Table 1
+ * PAPER.md:77-89, boundary set-up PAPER.md:175-179): a voxelised solid mask on a uniform Cartesian
+ * lattice, boundary wind data on the outer faces, N explicit
+ * lattice-Boltzmann steps, then the macroscopic fields and their time averages
+ * ("per-step macroscopic reconstruction"; averaging window PAPER.md:388).  The arithmetic of
+ * every call is the algorithm statement in DESIGN.md §3 (steps 1-9), which restates the methods the paper
+ * names (D3Q19, BGK, Smagorinsky-Lilly from non-equilibrium moments, Guo-forced Coriolis, equilibrium
+ * velocity boundaries, no-slip solids: Table 1) — the paper prints no formula.
+ *
+ * Conventions (all calls)
+ *   - Every function returns LBM_OK (0) or a negative LBM_E* code; nothing throws or aborts.  After an
+ *     error lbm_last_error(h) describes it.  A NULL handle gives LBM_EINVAL.
+ *   - Arrays are C order [z][y][x] (x fastest); nx,ny,nz are cell counts.  "real" below is float for the
+ *     plain entry points and double for the *_f64 twins; both work on FP32 and FP64 handles.
+ *   - Input arrays are borrowed for the duration of the call and copied.  Output arrays are allocated by
+ *     the caller.  Array arguments may be HOST or DEVICE pointers unless stated; the library asks the
+ *     CUDA runtime which (cudaPointerGetAttributes).  Host arrays are copied on the handle's stream and
+ *     the call returns after the copy has completed.
+ *   - lbm_step is asynchronous on the handle's stream.  Getters that write to host memory synchronise;
+ *     getters that write to device memory are stream-ordered (call lbm_sync before reading elsewhere).
+ *   - The handle owns its device memory unless lbm_create_ex was given a caller-owned workspace, which the
+ *     caller must keep alive until lbm_destroy.
+ *   - There is no CPU fallback: without a CUDA device every call that needs one returns LBM_ECUDA.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbm lbm_t; /* opaque; owned by the library */
+
+enum { LBM_OK = 0, LBM_EINVAL = -1, LBM_ENOMEM = -2, LBM_ECUDA = -3, LBM_ESTATE = -4 };
+
+/* face types, used in face_type[6] = {x-, x+, y-, y+, z-, z+}  (DESIGN.md §3 step 4a, 5, 6) */
+enum {
+    LBM_PERIODIC   = 0, /* wrap; must be set on both faces of an axis                                  */
+    LBM_WALL       = 1, /* halfway bounce-back, wall half a cell outside the last node                 */
+    LBM_FREE_SLIP  = 2, /* halfway specular reflection                                                 */
+    LBM_EQ_FIXED   = 3, /* face cells hold f_eq(1, u_b): the "equilibrium-based velocity" face PAPER.md:175 */
+    LBM_EQ_OUTFLOW = 4  /* face cells hold f_eq(1, u of the inward neighbour at the previous step)     */
+};
+
+/* cell classes returned by lbm_get_flags (DESIGN.md §3 step 3, 9) */
+enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_CELL_EQ_FIXED = 2, LBM_CELL_EQ_OUTFLOW = 3 };
+
+/* Bytes of device workspace a handle of this size needs (two population buffers of 19 reals per cell,
+ * one flag byte per cell, optional 3 reals per cell of time-mean sums, small profile/plane scratch).
+ * fp64 != 0 sizes a double-precision handle. */
+int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int fp64, size_t *out);
+
+/* Create an FP32 handle that allocates its own workspace (cudaMalloc) and uses the default stream.
+ * nu0: molecular viscosity (tau0 = 3 nu0 + 1/2); Cs: Smagorinsky constant; f_cor: Coriolis parameter about z
+ * (acceleration f_cor (u_y, -u_x, 0)); F[3]: uniform acceleration (pressure-gradient drive), host pointer,
+ * NULL = 0.  All in lattice units.  Faces default to {EQ_FIXED, EQ_OUTFLOW, PERIODIC, PERIODIC, WALL,
+ * FREE_SLIP} (BASELINE.json configs[0]).  Mean sums are allocated (want_mean = 1). */
+int lbm_create(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3], lbm_t **out);
+
+/* Same, with a caller-owned DEVICE workspace of at least lbm_workspace_bytes() bytes (256-byte aligned;
+ * NULL = allocate), a cudaStream_t passed as void* (NULL = default stream), and the precision choice.
+ * want_mean = 0 omits the time-mean sums (lbm_mean_config then returns LBM_ESTATE). */
+int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3],
+                  void *dev_workspace, size_t workspace_bytes, void *cuda_stream, int fp64, int want_mean,
+                  lbm_t **out);
+
+int lbm_destroy(lbm_t *h);
+
+/* Face types, order x-,x+,y-,y+,z-,z+.  Invalidates the flags: call lbm_set_flags afterwards. */
+int lbm_set_boundaries(lbm_t *h, const int face_type[6]);
+
+/* Voxelise ("solid mask"; heightmap form per north_star): cell (x,y,z) is SOLID iff
+ * z < clamp(height[y][x], 0, nz); non-solid cells on an EQ face take the EQ class (EQ_FIXED wins);
+ * then classify the wall links of every FLUID cell.  Integer work, done on the device.
+ * height: int32 [ny][nx], host or device; NULL = flat ground (all 0).
+ * Resets the populations to the rest state (rho = 1, u = 0) and the step counter and mean sums to 0. */
+int lbm_set_flags(lbm_t *h, const int32_t *height);
+
+/* Boundary wind profile ("macroscopic boundary states"): every EQ_FIXED cell at level z is set
+ * to f_eq(1, (u[z], v[z], w[z])).  Each array [nz]; v, w may be NULL (= 0).  Needs flags. */
+int lbm_set_inlet_profile(lbm_t *h, const float *u, const float *v, const float *w);
+int lbm_set_inlet_profile_f64(lbm_t *h, const double *u, const double *v, const double *w);
+
+/* Per-cell boundary state of one face: uvw is [3][n2][n1] with (n2,n1) = (nz,ny) on x faces, (nz,nx) on
+ * y faces, (ny,nx) on z faces.  Only the EQ_FIXED cells of that face are written. */
+int lbm_set_inlet_plane(lbm_t *h, int face, const float *uvw);
+int lbm_set_inlet_plane_f64(lbm_t *h, int face, const double *uvw);
+
+/* Config-5 coupling, device to device, stream-ordered on dst's stream: local macros of src on the plane
+ * x = src_x_plane are written as f_eq(1, u) into the EQ_FIXED cells of dst's x- face, tiling y modulo
+ * src's ny; nz must match; SOLID src cells feed u = 0.  Both handles must share precision. */
+int lbm_feed_inlet(lbm_t *dst, const lbm_t *src, int src_x_plane);
+
+/* Initial state G0 = f_eq(rho, u) (DESIGN.md §3 step 3).  NULL rho = 1; NULL component = 0.  SOLID cells get
+ * rho = 1, u = 0; EQ_FIXED cells keep their boundary state.  Resets the step counter.  Needs flags. */
+int lbm_set_macros(lbm_t *h, const float *rho, const float *ux, const float *uy, const float *uz);
+int lbm_set_macros_f64(lbm_t *h, const double *rho, const double *ux, const double *uy, const double *uz);
+
+/* n fused stream-collide steps (DESIGN.md §3 steps 4 and 6): pull with bounce-back / specular / periodic
+ * resolution, moments, Coriolis + F with the implicit half-force velocity, Smagorinsky tau from the local
+ * non-equilibrium stress, BGK + Guo source, store; outflow cells refreshed; on sampling steps the time-mean
+ * sums are updated in the same kernel.  Asynchronous.  Needs flags (else LBM_ESTATE). */
+int lbm_step(lbm_t *h, int n);
+
+/* Time mean (DESIGN.md §3 step 8): after step k (k counted from the last set_macros/set_flags), if
+ * every > 0, k >= start_step and (k - start_step) % every == 0, u is added to the sums. */
+int lbm_mean_config(lbm_t *h, long start_step, int every);
+int lbm_mean_reset(lbm_t *h);
+
+/* Local macroscopic fields of the current state (DESIGN.md §3 step 7); any pointer may be NULL. */
+int lbm_get_macros(lbm_t *h, float *rho, float *ux, float *uy, float *uz);
+int lbm_get_macros_f64(lbm_t *h, double *rho, double *ux, double *uy, double *uz);
+
+/* mean = sum / n_samples (0 where n_samples == 0 and in SOLID cells); n_samples is a host pointer, may be NULL */
+int lbm_get_mean(lbm_t *h, float *ux, float *uy, float *uz, long *n_samples);
+int lbm_get_mean_f64(lbm_t *h, double *ux, double *uy, double *uz, long *n_samples);
+
+/* Parity exports.  flags: uint8 [nz][ny][nx] cell classes.  links: uint32 [nz][ny][nx], bit i (1..18) set
+ * iff pulling direction i into that FLUID cell takes the bounce-back branch; 0 for non-FLUID cells. */
+int lbm_get_flags(lbm_t *h, uint8_t *flags);
+int lbm_get_links(lbm_t *h, uint32_t *links);
+
+/* Checkpoint: populations f_i (NOT shifted), double, [19][nz][ny][nx], direction order of DESIGN.md §3
+ * step 1.  set_state leaves the step counter alone (use lbm_set_step). */
+int lbm_get_state(lbm_t *h, double *f);
+int lbm_set_state(lbm_t *h, const double *f);
+
+long lbm_get_step(const lbm_t *h);
+int lbm_set_step(lbm_t *h, long step);
+int lbm_sync(lbm_t *h);
+const char *lbm_last_error(const lbm_t *h);
+
+/* Kernel launches issued by this handle since creation (bench.py's gpu_launches). */
+long lbm_launch_count(const lbm_t *h);
+
+/* The lattice as the library defines it: c[19][3], opposite[19] (host arrays).  For tests. */
+int lbm_lattice(int *c, int *opposite);
+
+/* Tuning knob for experiments: selects the stream-collide kernel variant (0 = default).  Returns
+ * LBM_EINVAL for an unknown variant.  All variants compute the same arithmetic. */
+int lbm_set_variant(lbm_t *h, int variant);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */

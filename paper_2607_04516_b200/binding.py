@@ -1,0 +1,302 @@
+"""Thin Python binding of the C-ABI library (include/lbm.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of ``liblbm_b200.so``.  PyTorch is used for device memory (the
+workspace and output tensors) and for the stream; numpy arrays are passed as HOST pointers (the library copies
+them).  There is no CPU fallback: if the library has not been built, or no CUDA device exists, the binding raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "liblbm_b200.so")
+_lib = None
+
+PERIODIC, WALL, FREE_SLIP, EQ_FIXED, EQ_OUTFLOW = 0, 1, 2, 3, 4
+FLUID, SOLID, CELL_EQ_FIXED, CELL_EQ_OUTFLOW = 0, 1, 2, 3
+_ERR = {-1: "LBM_EINVAL", -2: "LBM_ENOMEM", -3: "LBM_ECUDA", -4: "LBM_ESTATE"}
+
+# every symbol include/lbm.h declares (tests check that the .so exports them all)
+SYMBOLS = [
+    "lbm_workspace_bytes", "lbm_create", "lbm_create_ex", "lbm_destroy", "lbm_set_boundaries", "lbm_set_flags",
+    "lbm_set_inlet_profile", "lbm_set_inlet_profile_f64", "lbm_set_inlet_plane", "lbm_set_inlet_plane_f64",
+    "lbm_feed_inlet", "lbm_set_macros", "lbm_set_macros_f64", "lbm_step", "lbm_mean_config", "lbm_mean_reset",
+    "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
+    "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
+    "lbm_launch_count", "lbm_lattice", "lbm_set_variant",
+]
+
+
+class LbmError(RuntimeError):
+    pass
+
+
+def library_path() -> str:
+    return _SO
+
+
+def load_library():
+    """dlopen the in-tree CUDA library.  Raises if it is missing — there is no fallback path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise LbmError(f"{_SO} not built: run `python -m paper_2607_04516_b200.build` (needs nvcc). "
+                       "There is no CPU fallback.")
+    lib = C.CDLL(_SO)
+    vp, i, d, l = C.c_void_p, C.c_int, C.c_double, C.c_long
+    lib.lbm_workspace_bytes.argtypes = [i, i, i, i, i, C.POINTER(C.c_size_t)]
+    lib.lbm_create.argtypes = [i, i, i, d, d, d, vp, C.POINTER(vp)]
+    lib.lbm_create_ex.argtypes = [i, i, i, d, d, d, vp, vp, C.c_size_t, vp, i, i, C.POINTER(vp)]
+    lib.lbm_destroy.argtypes = [vp]
+    lib.lbm_set_boundaries.argtypes = [vp, vp]
+    lib.lbm_set_flags.argtypes = [vp, vp]
+    for n in ("lbm_set_inlet_profile", "lbm_set_inlet_profile_f64"):
+        getattr(lib, n).argtypes = [vp, vp, vp, vp]
+    for n in ("lbm_set_inlet_plane", "lbm_set_inlet_plane_f64"):
+        getattr(lib, n).argtypes = [vp, i, vp]
+    lib.lbm_feed_inlet.argtypes = [vp, vp, i]
+    for n in ("lbm_set_macros", "lbm_set_macros_f64", "lbm_get_macros", "lbm_get_macros_f64"):
+        getattr(lib, n).argtypes = [vp, vp, vp, vp, vp]
+    lib.lbm_step.argtypes = [vp, i]
+    lib.lbm_mean_config.argtypes = [vp, l, i]
+    lib.lbm_mean_reset.argtypes = [vp]
+    for n in ("lbm_get_mean", "lbm_get_mean_f64"):
+        getattr(lib, n).argtypes = [vp, vp, vp, vp, C.POINTER(l)]
+    lib.lbm_get_flags.argtypes = [vp, vp]
+    lib.lbm_get_links.argtypes = [vp, vp]
+    lib.lbm_get_state.argtypes = [vp, vp]
+    lib.lbm_set_state.argtypes = [vp, vp]
+    lib.lbm_get_step.argtypes = [vp]
+    lib.lbm_get_step.restype = l
+    lib.lbm_set_step.argtypes = [vp, l]
+    lib.lbm_sync.argtypes = [vp]
+    lib.lbm_last_error.argtypes = [vp]
+    lib.lbm_last_error.restype = C.c_char_p
+    lib.lbm_launch_count.argtypes = [vp]
+    lib.lbm_launch_count.restype = l
+    lib.lbm_lattice.argtypes = [vp, vp]
+    lib.lbm_set_variant.argtypes = [vp, i]
+    _lib = lib
+    return lib
+
+
+def _ptr(a, dtype):
+    """Pointer of a numpy array (host) or torch tensor (host or device); None -> NULL.  Returns (keepalive, ptr)."""
+    if a is None:
+        return None, None
+    if isinstance(a, np.ndarray):
+        a = np.ascontiguousarray(a, dtype=dtype)
+        return a, a.ctypes.data
+    import torch
+    if isinstance(a, torch.Tensor):
+        want = {np.float32: torch.float32, np.float64: torch.float64, np.int32: torch.int32,
+                np.uint8: torch.uint8, np.uint32: torch.int32}[dtype]
+        if a.dtype != want or not a.is_contiguous():
+            a = a.to(want).contiguous()
+        return a, a.data_ptr()
+    a = np.ascontiguousarray(a, dtype=dtype)
+    return a, a.ctypes.data
+
+
+class Lbm:
+    """One lattice on one GPU.  Same call names as include/lbm.h without the ``lbm_`` prefix."""
+
+    def __init__(self, nx, ny, nz, nu0, Cs=0.0, f_cor=0.0, F=(0.0, 0.0, 0.0), faces=None, fp64=False,
+                 want_mean=True, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise LbmError("no CUDA device: the LBM path has no CPU fallback")
+        self._lib = load_library()
+        self._torch = torch
+        self.device = torch.device(device)
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.shape = (self.nz, self.ny, self.nx)
+        self.fp64 = bool(fp64)
+        F = np.atleast_1d(np.asarray(F, dtype=np.float64))
+        if F.size == 1:
+            F = np.array([F[0], 0.0, 0.0])
+        nbytes = C.c_size_t()
+        self._chk0(self._lib.lbm_workspace_bytes(self.nx, self.ny, self.nz, int(want_mean), int(fp64), C.byref(nbytes)),
+                   "workspace_bytes")
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
+            base = self._ws.data_ptr()
+            aligned = (base + 255) // 256 * 256
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+            h = C.c_void_p()
+            rc = self._lib.lbm_create_ex(self.nx, self.ny, self.nz, float(nu0), float(Cs), float(f_cor), F.ctypes.data,
+                                         aligned, nbytes.value, self._stream.cuda_stream, int(fp64), int(want_mean),
+                                         C.byref(h))
+        self._chk0(rc, "create_ex")
+        self._h = h
+        self.workspace_bytes = nbytes.value
+        if faces is not None:
+            self.set_boundaries(faces)
+
+    # -- plumbing
+    def _chk0(self, rc, what):
+        if rc != 0:
+            raise LbmError(f"lbm_{what} failed: {_ERR.get(rc, rc)}")
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            msg = self._lib.lbm_last_error(self._h)
+            raise LbmError(f"lbm_{what} failed: {_ERR.get(rc, rc)}: {msg.decode() if msg else ''}")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.lbm_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _new(self, dtype, shape=None):
+        t = self._torch
+        return t.empty(shape or self.shape, dtype=dtype, device=self.device)
+
+    # -- setup
+    def set_boundaries(self, faces):
+        a = np.ascontiguousarray(faces, dtype=np.int32)
+        if a.shape != (6,):
+            raise ValueError("faces must have 6 entries")
+        self._chk(self._lib.lbm_set_boundaries(self._h, a.ctypes.data), "set_boundaries")
+
+    def set_flags(self, height=None):
+        k, p = _ptr(height, np.int32)
+        if k is not None and tuple(k.shape) != (self.ny, self.nx):
+            raise ValueError("height must be [ny][nx]")
+        self._chk(self._lib.lbm_set_flags(self._h, p), "set_flags")
+
+    def set_inlet_profile(self, u, v=None, w=None, f64=False):
+        dt = np.float64 if f64 else np.float32
+        ks = [_ptr(a, dt) for a in (u, v, w)]
+        fn = self._lib.lbm_set_inlet_profile_f64 if f64 else self._lib.lbm_set_inlet_profile
+        self._chk(fn(self._h, *[p for _, p in ks]), "set_inlet_profile")
+
+    def set_inlet_plane(self, face, uvw, f64=False):
+        k, p = _ptr(uvw, np.float64 if f64 else np.float32)
+        fn = self._lib.lbm_set_inlet_plane_f64 if f64 else self._lib.lbm_set_inlet_plane
+        self._chk(fn(self._h, int(face), p), "set_inlet_plane")
+
+    def feed_inlet(self, src: "Lbm", src_x_plane: int):
+        self._chk(self._lib.lbm_feed_inlet(self._h, src._h, int(src_x_plane)), "feed_inlet")
+
+    def set_macros(self, rho=None, ux=None, uy=None, uz=None, f64=False):
+        dt = np.float64 if f64 else np.float32
+        ks = [_ptr(a, dt) for a in (rho, ux, uy, uz)]
+        for k, _ in ks:
+            if k is not None and tuple(k.shape) != self.shape:
+                raise ValueError("fields must be [nz][ny][nx]")
+        fn = self._lib.lbm_set_macros_f64 if f64 else self._lib.lbm_set_macros
+        self._chk(fn(self._h, *[p for _, p in ks]), "set_macros")
+
+    # -- the hot call
+    def step(self, n=1):
+        self._chk(self._lib.lbm_step(self._h, int(n)), "step")
+
+    def mean_config(self, start_step, every):
+        self._chk(self._lib.lbm_mean_config(self._h, int(start_step), int(every)), "mean_config")
+
+    def mean_reset(self):
+        self._chk(self._lib.lbm_mean_reset(self._h), "mean_reset")
+
+    # -- results.  out=None: fresh torch device tensors; out="host": numpy arrays filled through HOST pointers
+    def get_macros(self, out=None, f64=False):
+        t = self._torch
+        fn = self._lib.lbm_get_macros_f64 if f64 else self._lib.lbm_get_macros
+        if out == "host":
+            arrs = [np.empty(self.shape, dtype=np.float64 if f64 else np.float32) for _ in range(4)]
+            self._chk(fn(self._h, *[a.ctypes.data for a in arrs]), "get_macros")
+            return tuple(arrs)
+        arrs = out if out is not None else [self._new(t.float64 if f64 else t.float32) for _ in range(4)]
+        self._chk(fn(self._h, *[a.data_ptr() if a is not None else None for a in arrs]), "get_macros")
+        return tuple(arrs)
+
+    def get_mean(self, out=None, f64=False):
+        t = self._torch
+        fn = self._lib.lbm_get_mean_f64 if f64 else self._lib.lbm_get_mean
+        n = C.c_long()
+        if out == "host":
+            arrs = [np.empty(self.shape, dtype=np.float64 if f64 else np.float32) for _ in range(3)]
+            self._chk(fn(self._h, *[a.ctypes.data for a in arrs], C.byref(n)), "get_mean")
+            return arrs[0], arrs[1], arrs[2], n.value
+        arrs = out if out is not None else [self._new(t.float64 if f64 else t.float32) for _ in range(3)]
+        self._chk(fn(self._h, *[a.data_ptr() for a in arrs], C.byref(n)), "get_mean")
+        return arrs[0], arrs[1], arrs[2], n.value
+
+    def get_flags(self):
+        out = np.empty(self.shape, dtype=np.uint8)
+        self._chk(self._lib.lbm_get_flags(self._h, out.ctypes.data), "get_flags")
+        return out
+
+    def get_links(self):
+        out = np.empty(self.shape, dtype=np.uint32)
+        self._chk(self._lib.lbm_get_links(self._h, out.ctypes.data), "get_links")
+        return out
+
+    def get_state(self, out=None):
+        if out == "host":
+            a = np.empty((19,) + self.shape, dtype=np.float64)
+            self._chk(self._lib.lbm_get_state(self._h, a.ctypes.data), "get_state")
+            return a
+        a = self._new(self._torch.float64, (19,) + self.shape)
+        self._chk(self._lib.lbm_get_state(self._h, a.data_ptr()), "get_state")
+        return a
+
+    def set_state(self, f):
+        k, p = _ptr(f, np.float64)
+        if tuple(k.shape) != (19,) + self.shape:
+            raise ValueError("state must be [19][nz][ny][nx]")
+        self._chk(self._lib.lbm_set_state(self._h, p), "set_state")
+
+    def get_step(self):
+        return int(self._lib.lbm_get_step(self._h))
+
+    def set_step(self, s):
+        self._chk(self._lib.lbm_set_step(self._h, int(s)), "set_step")
+
+    def sync(self):
+        self._chk(self._lib.lbm_sync(self._h), "sync")
+
+    def launch_count(self):
+        return int(self._lib.lbm_launch_count(self._h))
+
+    def set_variant(self, v):
+        self._chk(self._lib.lbm_set_variant(self._h, int(v)), "set_variant")
+
+    @property
+    def cuda_stream(self):
+        return self._stream
+
+
+def lattice():
+    lib = load_library()
+    c = np.zeros((19, 3), dtype=np.int32)
+    opp = np.zeros(19, dtype=np.int32)
+    rc = lib.lbm_lattice(c.ctypes.data, opp.ctypes.data)
+    if rc != 0:
+        raise LbmError("lbm_lattice failed")
+    return c, opp
+
+
+def from_workload(wl, fp64=False, want_mean=True, device="cuda:0") -> Lbm:
+    """Create a handle for a workloads.Workload and load its flags, inlet profile and initial field."""
+    sim = Lbm(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces, fp64=fp64, want_mean=want_mean,
+              device=device)
+    sim.set_flags(wl.height)
+    if wl.inlet_profile is not None:
+        sim.set_inlet_profile(*wl.inlet_profile)
+    if wl.init is not None:
+        sim.set_macros(*wl.init)
+    else:
+        sim.set_macros()
+    return sim

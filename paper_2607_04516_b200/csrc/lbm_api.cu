@@ -1,0 +1,638 @@
+// lbm_api.cu — context, launch layer and C ABI (include/lbm.h) of the B200-native LBM-LES path.
+#include "../../include/lbm.h"
+#include "lbm_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+using namespace lbmk;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct Layout {
+    long long stride;
+    size_t off_A, off_B, off_flags, off_mean, off_scratch, total;
+    size_t scratch_bytes;
+};
+
+Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
+{
+    Layout L{};
+    const size_t N = (size_t)nx * ny * nz;
+    const size_t rs = fp64 ? 8 : 4;
+    L.stride = (long long)align_up(N, 64);
+    size_t o = 0;
+    L.off_A = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
+    L.off_B = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
+    L.off_flags = o; o += align_up(N, ALIGN);
+    L.off_mean = o; if (want_mean) o += align_up((size_t)3 * L.stride * rs, ALIGN);
+    // scratch: heightmap (nx*ny int32) or a profile (3 nz doubles) or one face plane (3 n1 n2 doubles)
+    const size_t plane = (size_t)std::max(std::max((size_t)nx * ny, (size_t)nx * nz), (size_t)ny * nz);
+    L.scratch_bytes = align_up(std::max(plane * 3 * sizeof(double), (size_t)nz * 3 * sizeof(double)), ALIGN);
+    L.off_scratch = o; o += L.scratch_bytes;
+    L.total = o;
+    return L;
+}
+
+} // namespace
+
+struct lbm {
+    int nx, ny, nz;
+    double nu0, Cs, fcor, F[3];
+    int face[6];
+    int fp64, want_mean;
+    Layout L;
+    char *ws;       // device workspace
+    bool own_ws;
+    cudaStream_t stream;
+    int cur;        // which buffer holds the current state (0 = A, 1 = B)
+    bool have_flags;
+    long step;
+    long mstart; int mevery; long mcount;
+    long launches;
+    int variant;
+    std::string err;
+
+    void *bufA() const { return ws + L.off_A; }
+    void *bufB() const { return ws + L.off_B; }
+    void *state() const { return cur ? bufB() : bufA(); }
+    void *other() const { return cur ? bufA() : bufB(); }
+    uint8_t *flags() const { return (uint8_t *)(ws + L.off_flags); }
+    void *mean() const { return want_mean ? ws + L.off_mean : nullptr; }
+    void *scratch() const { return ws + L.off_scratch; }
+    long long N() const { return (long long)nx * ny * nz; }
+};
+
+namespace {
+
+int fail(lbm_t *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg;
+    return code;
+}
+
+#define CUDA_TRY(h, expr)                                                                             \
+    do {                                                                                              \
+        cudaError_t e_ = (expr);                                                                      \
+        if (e_ != cudaSuccess)                                                                        \
+            return fail(h, LBM_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));            \
+    } while (0)
+
+template <typename real>
+Params<real> make_params(const lbm_t *h)
+{
+    Params<real> P{};
+    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.nxy = h->nx * h->ny;
+    P.N = (int)h->N();
+    P.stride = h->L.stride;
+    for (int k = 0; k < 6; ++k) P.face[k] = h->face[k];
+    P.tau0 = (real)(3.0 * h->nu0 + 0.5);
+    P.Kles = (real)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs);
+    P.fcor = (real)h->fcor;
+    P.h = (real)(0.5 * h->fcor);
+    P.inv1ph2 = (real)(1.0 / (1.0 + 0.25 * h->fcor * h->fcor));
+    P.Fx = (real)h->F[0]; P.Fy = (real)h->F[1]; P.Fz = (real)h->F[2];
+    return P;
+}
+
+inline unsigned blocks_for(long long n, int block) { return (unsigned)((n + block - 1) / block); }
+
+// is p a device-accessible pointer? (device or managed memory)
+bool is_device_ptr(const void *p)
+{
+    cudaPointerAttributes a{};
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { cudaGetLastError(); return false; }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+// Input staging.  Device sources are used in place; host sources are copied into the handle's scratch area when
+// they fit at the given offset, else into a temporary allocation.  release_in waits for the copies (so that the
+// caller's buffer is free on return) and frees temporaries.
+struct InBuf { const void *dev; void *tmp; bool host; };
+int stage_in(lbm_t *h, const void *src, size_t bytes, size_t scratch_off, InBuf *b)
+{
+    b->dev = nullptr; b->tmp = nullptr; b->host = false;
+    if (!src) return LBM_OK;
+    if (is_device_ptr(src)) { b->dev = src; return LBM_OK; }
+    void *d = nullptr;
+    if (scratch_off + bytes <= h->L.scratch_bytes) d = (char *)h->scratch() + scratch_off;
+    else {
+        cudaError_t e = cudaMalloc(&d, bytes);
+        if (e != cudaSuccess) { cudaGetLastError(); return fail(h, LBM_ENOMEM, std::string("cudaMalloc staging: ") + cudaGetErrorString(e)); }
+        b->tmp = d;
+    }
+    cudaError_t e = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, h->stream);
+    if (e != cudaSuccess) {
+        if (b->tmp) cudaFree(b->tmp);
+        b->tmp = nullptr;
+        return fail(h, LBM_ECUDA, std::string("H2D copy: ") + cudaGetErrorString(e));
+    }
+    b->dev = d; b->host = true;
+    return LBM_OK;
+}
+void release_in(lbm_t *h, InBuf *b, int n)
+{
+    bool any = false;
+    for (int k = 0; k < n; ++k) any |= b[k].host;
+    if (any) cudaStreamSynchronize(h->stream);
+    for (int k = 0; k < n; ++k)
+        if (b[k].tmp) { cudaFree(b[k].tmp); b[k].tmp = nullptr; }
+}
+
+// Output staging: if dst is a host pointer allocate a device buffer; finish_out copies back and frees.
+struct OutBuf { void *host; void *dev; size_t bytes; bool temp; };
+int stage_out(lbm_t *h, void *dst, size_t bytes, OutBuf *o)
+{
+    o->host = nullptr; o->dev = nullptr; o->bytes = bytes; o->temp = false;
+    if (!dst) return LBM_OK;
+    if (is_device_ptr(dst)) { o->dev = dst; return LBM_OK; }
+    cudaError_t e = cudaMalloc(&o->dev, bytes);
+    if (e != cudaSuccess) return fail(h, LBM_ENOMEM, std::string("cudaMalloc staging: ") + cudaGetErrorString(e));
+    o->host = dst; o->temp = true;
+    return LBM_OK;
+}
+int finish_out(lbm_t *h, OutBuf *outs, int n)
+{
+    int rc = LBM_OK;
+    bool any_host = false;
+    for (int k = 0; k < n; ++k)
+        if (outs[k].temp) {
+            any_host = true;
+            cudaError_t e = cudaMemcpyAsync(outs[k].host, outs[k].dev, outs[k].bytes, cudaMemcpyDeviceToHost, h->stream);
+            if (e != cudaSuccess) rc = fail(h, LBM_ECUDA, std::string("D2H copy: ") + cudaGetErrorString(e));
+        }
+    if (any_host) {
+        cudaError_t e = cudaStreamSynchronize(h->stream);
+        if (e != cudaSuccess) rc = fail(h, LBM_ECUDA, std::string("sync: ") + cudaGetErrorString(e));
+    }
+    for (int k = 0; k < n; ++k)
+        if (outs[k].temp) cudaFree(outs[k].dev);
+    return rc;
+}
+
+int check_launch(lbm_t *h, const char *what)
+{
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, LBM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    h->launches += 1;
+    return LBM_OK;
+}
+
+// ---- templated implementations -----------------------------------------------------------------------------------
+
+template <typename real>
+int do_set_flags(lbm_t *h, const int32_t *height)
+{
+    const Params<real> P = make_params<real>(h);
+    InBuf in;
+    int rc = stage_in(h, height, (size_t)h->nx * h->ny * sizeof(int32_t), 0, &in);
+    if (rc) return rc;
+    const int B = 256;
+    voxelise_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const int32_t *)in.dev, h->flags(), P);
+    rc = check_launch(h, "voxelise_kernel");
+    if (!rc) {
+        // in place: class bits are never changed by classify, only the SLOW bit is added
+        classify_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->flags(), h->flags(), nullptr, P);
+        rc = check_launch(h, "classify_kernel");
+    }
+    release_in(h, &in, 1);
+    if (rc) return rc;
+    const size_t rs = sizeof(real);
+    CUDA_TRY(h, cudaMemsetAsync(h->bufA(), 0, (size_t)Q * h->L.stride * rs, h->stream));
+    CUDA_TRY(h, cudaMemsetAsync(h->bufB(), 0, (size_t)Q * h->L.stride * rs, h->stream));
+    if (h->want_mean) CUDA_TRY(h, cudaMemsetAsync(h->mean(), 0, (size_t)3 * h->L.stride * rs, h->stream));
+    h->cur = 0; h->step = 0; h->mcount = 0; h->have_flags = true;
+    return LBM_OK;
+}
+
+template <typename real, typename in_t>
+int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, const in_t *w, size_t count)
+{
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inlet: flags not set");
+    if (!u) return fail(h, LBM_EINVAL, "set_inlet: u is NULL");
+    const Params<real> P = make_params<real>(h);
+    InBuf in[3];
+    const size_t bytes = count * sizeof(in_t);
+    int rc = stage_in(h, u, bytes, 0, &in[0]);
+    if (!rc) rc = stage_in(h, v, bytes, align_up(bytes, ALIGN), &in[1]); else in[1] = InBuf{nullptr, nullptr, false};
+    if (!rc) rc = stage_in(h, w, bytes, 2 * align_up(bytes, ALIGN), &in[2]); else in[2] = InBuf{nullptr, nullptr, false};
+    if (!rc) {
+        const int B = 256;
+        const long long threads = mode == 0 ? (long long)P.N : (long long)count;
+        inlet_kernel<real, in_t><<<blocks_for(threads, B), B, 0, h->stream>>>(
+            (real *)h->bufA(), (real *)h->bufB(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+            (const in_t *)in[2].dev, mode, face, P);
+        rc = check_launch(h, "inlet_kernel");
+    }
+    release_in(h, in, 3);
+    return rc;
+}
+
+template <typename in_t>
+int set_inlet_profile_any(lbm_t *h, const in_t *u, const in_t *v, const in_t *w)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_set_inlet<double, in_t>(h, 0, 0, u, v, w, (size_t)h->nz)
+                   : do_set_inlet<float, in_t>(h, 0, 0, u, v, w, (size_t)h->nz);
+}
+
+template <typename in_t>
+int set_inlet_plane_any(lbm_t *h, int face, const in_t *uvw)
+{
+    if (!h) return LBM_EINVAL;
+    if (face < 0 || face > 5) return fail(h, LBM_EINVAL, "set_inlet_plane: face out of range");
+    if (!uvw) return fail(h, LBM_EINVAL, "set_inlet_plane: uvw is NULL");
+    const int axis = face / 2;
+    const size_t n1 = axis == 0 ? h->ny : h->nx, n2 = axis == 2 ? h->ny : h->nz;
+    const size_t cnt = n1 * n2;
+    // stage the three planes as one array so that a host source is copied once (it fits the scratch area)
+    InBuf in;
+    int rc = stage_in(h, uvw, 3 * cnt * sizeof(in_t), 0, &in);
+    if (rc) return rc;
+    const in_t *p = (const in_t *)in.dev;
+    rc = h->fp64 ? do_set_inlet<double, in_t>(h, 1, face, p, p + cnt, p + 2 * cnt, cnt)
+                 : do_set_inlet<float, in_t>(h, 1, face, p, p + cnt, p + 2 * cnt, cnt);
+    release_in(h, &in, 1);
+    return rc;
+}
+
+template <typename real, typename in_t>
+int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, const in_t *uz)
+{
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_macros: flags not set");
+    const Params<real> P = make_params<real>(h);
+    const size_t bytes = (size_t)P.N * sizeof(in_t);
+    InBuf in[4] = {};
+    const in_t *src[4] = {rho, ux, uy, uz};
+    int rc = LBM_OK;
+    for (int k = 0; k < 4 && !rc; ++k) rc = stage_in(h, src[k], bytes, h->L.scratch_bytes, &in[k]); // never fits: temp
+    if (!rc) {
+        const int B = 256;
+        init_kernel<real, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            (real *)h->bufA(), (real *)h->bufB(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+            (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
+        rc = check_launch(h, "init_kernel");
+    }
+    release_in(h, in, 4);
+    if (!rc) { h->step = 0; h->cur = 0; }
+    return rc;
+}
+
+template <typename real>
+int launch_step(lbm_t *h, const Params<real> &P, bool sample)
+{
+    const real *A = (const real *)h->state();
+    real *B = (real *)h->other();
+    real *ms = (real *)h->mean();
+    const int BS = 256;
+    const unsigned grid = blocks_for(P.N, BS);
+    if (sample) step_kernel<real, true><<<grid, BS, 0, h->stream>>>(A, B, h->flags(), ms, P);
+    else step_kernel<real, false><<<grid, BS, 0, h->stream>>>(A, B, h->flags(), ms, P);
+    return check_launch(h, "step_kernel");
+}
+
+template <typename real>
+int do_step(lbm_t *h, int n)
+{
+    const Params<real> P = make_params<real>(h);
+    for (int it = 0; it < n; ++it) {
+        const long k = h->step + 1;
+        const bool sample = h->mevery > 0 && k >= h->mstart && (k - h->mstart) % h->mevery == 0;
+        int rc = launch_step<real>(h, P, sample);
+        if (rc) return rc;
+        h->cur ^= 1;
+        h->step = k;
+        if (sample) h->mcount += 1;
+    }
+    return LBM_OK;
+}
+
+template <typename real, typename out_t>
+int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
+{
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_macros: flags not set");
+    const Params<real> P = make_params<real>(h);
+    OutBuf o[4];
+    out_t *dst[4] = {rho, ux, uy, uz};
+    int rc = LBM_OK;
+    int staged = 0;
+    for (; staged < 4 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)P.N * sizeof(out_t), &o[staged]);
+    if (!rc) {
+        const int B = 256;
+        macros_kernel<real, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            (const real *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P);
+        rc = check_launch(h, "macros_kernel");
+    }
+    int rc2 = finish_out(h, o, staged);
+    return rc ? rc : rc2;
+}
+
+template <typename real, typename out_t>
+int do_get_mean(lbm_t *h, out_t *ux, out_t *uy, out_t *uz, long *n_samples)
+{
+    if (!h->want_mean) return fail(h, LBM_ESTATE, "get_mean: handle created without mean sums");
+    const Params<real> P = make_params<real>(h);
+    if (n_samples) *n_samples = h->mcount;
+    OutBuf o[3];
+    out_t *dst[3] = {ux, uy, uz};
+    int rc = LBM_OK;
+    int staged = 0;
+    for (; staged < 3 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)P.N * sizeof(out_t), &o[staged]);
+    if (!rc) {
+        const int B = 256;
+        const double inv = h->mcount > 0 ? 1.0 / (double)h->mcount : 0.0;
+        mean_out_kernel<real, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            (const real *)h->mean(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, inv, P);
+        rc = check_launch(h, "mean_out_kernel");
+    }
+    int rc2 = finish_out(h, o, staged);
+    return rc ? rc : rc2;
+}
+
+template <typename real>
+int do_get_links(lbm_t *h, uint32_t *links)
+{
+    const Params<real> P = make_params<real>(h);
+    OutBuf o;
+    int rc = stage_out(h, links, (size_t)P.N * sizeof(uint32_t), &o);
+    if (rc) return rc;
+    const int B = 256;
+    classify_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(nullptr, h->flags(), (uint32_t *)o.dev, P);
+    rc = check_launch(h, "classify_kernel");
+    int rc2 = finish_out(h, &o, 1);
+    return rc ? rc : rc2;
+}
+
+template <typename real>
+int do_get_state(lbm_t *h, double *f)
+{
+    const Params<real> P = make_params<real>(h);
+    OutBuf o;
+    int rc = stage_out(h, f, (size_t)Q * P.N * sizeof(double), &o);
+    if (rc) return rc;
+    const int B = 256;
+    state_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->state(), (double *)o.dev, P);
+    rc = check_launch(h, "state_out_kernel");
+    int rc2 = finish_out(h, &o, 1);
+    return rc ? rc : rc2;
+}
+
+template <typename real>
+int do_set_state(lbm_t *h, const double *f)
+{
+    const Params<real> P = make_params<real>(h);
+    InBuf in;
+    int rc = stage_in(h, f, (size_t)Q * P.N * sizeof(double), h->L.scratch_bytes, &in);
+    if (rc) return rc;
+    const int B = 256;
+    state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (const double *)in.dev, P);
+    rc = check_launch(h, "state_in_kernel");
+    release_in(h, &in, 1);
+    if (!rc) h->cur = 0;
+    return rc;
+}
+
+template <typename real>
+int do_feed(lbm_t *dst, const lbm_t *src, int sx)
+{
+    const Params<real> D = make_params<real>(dst), S = make_params<real>(src);
+    const int B = 128;
+    feed_kernel<real><<<blocks_for((long long)D.ny * D.nz, B), B, 0, dst->stream>>>(
+        (real *)dst->bufA(), (real *)dst->bufB(), dst->flags(), D, (const real *)src->state(), src->flags(), S, sx);
+    return check_launch(dst, "feed_kernel");
+}
+
+} // namespace
+
+// ---- C ABI -------------------------------------------------------------------------------------------------------------
+
+extern "C" {
+
+int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int fp64, size_t *out)
+{
+    if (!out || nx < 1 || ny < 1 || nz < 1) return LBM_EINVAL;
+    if ((long long)nx * ny * nz > 2000000000LL) return LBM_EINVAL;
+    *out = make_layout(nx, ny, nz, want_mean, fp64).total;
+    return LBM_OK;
+}
+
+int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3], void *dev_workspace,
+                  size_t workspace_bytes, void *cuda_stream, int fp64, int want_mean, lbm_t **out)
+{
+    if (!out) return LBM_EINVAL;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1 || (long long)nx * ny * nz > 2000000000LL) return LBM_EINVAL;
+    if (!(nu0 > 0.0) || Cs < 0.0 || !std::isfinite(nu0) || !std::isfinite(Cs) || !std::isfinite(f_cor)) return LBM_EINVAL;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return LBM_ECUDA; }
+    lbm_t *h = new (std::nothrow) lbm();
+    if (!h) return LBM_ENOMEM;
+    h->nx = nx; h->ny = ny; h->nz = nz;
+    h->nu0 = nu0; h->Cs = Cs; h->fcor = f_cor;
+    for (int a = 0; a < 3; ++a) h->F[a] = F ? F[a] : 0.0;
+    const int def[6] = {LBM_EQ_FIXED, LBM_EQ_OUTFLOW, LBM_PERIODIC, LBM_PERIODIC, LBM_WALL, LBM_FREE_SLIP};
+    for (int k = 0; k < 6; ++k) h->face[k] = def[k];
+    h->fp64 = fp64 ? 1 : 0; h->want_mean = want_mean ? 1 : 0;
+    h->L = make_layout(nx, ny, nz, h->want_mean, h->fp64);
+    h->stream = (cudaStream_t)cuda_stream;
+    h->cur = 0; h->have_flags = false; h->step = 0;
+    h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0;
+    if (dev_workspace) {
+        if (workspace_bytes < h->L.total || ((uintptr_t)dev_workspace % ALIGN) != 0 || !is_device_ptr(dev_workspace)) {
+            delete h;
+            return LBM_EINVAL;
+        }
+        h->ws = (char *)dev_workspace; h->own_ws = false;
+    } else {
+        void *p = nullptr;
+        cudaError_t e = cudaMalloc(&p, h->L.total);
+        if (e != cudaSuccess) { cudaGetLastError(); delete h; return e == cudaErrorMemoryAllocation ? LBM_ENOMEM : LBM_ECUDA; }
+        h->ws = (char *)p; h->own_ws = true;
+    }
+    *out = h;
+    return LBM_OK;
+}
+
+int lbm_create(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3], lbm_t **out)
+{
+    return lbm_create_ex(nx, ny, nz, nu0, Cs, f_cor, F, nullptr, 0, nullptr, 0, 1, out);
+}
+
+int lbm_destroy(lbm_t *h)
+{
+    if (!h) return LBM_EINVAL;
+    cudaStreamSynchronize(h->stream);
+    if (h->own_ws) cudaFree(h->ws);
+    delete h;
+    return LBM_OK;
+}
+
+int lbm_set_boundaries(lbm_t *h, const int face_type[6])
+{
+    if (!h) return LBM_EINVAL;
+    if (!face_type) return fail(h, LBM_EINVAL, "set_boundaries: NULL");
+    for (int a = 0; a < 3; ++a) {
+        const int lo = face_type[2 * a], hi = face_type[2 * a + 1];
+        if (lo < 0 || lo > 4 || hi < 0 || hi > 4) return fail(h, LBM_EINVAL, "set_boundaries: unknown face type");
+        if ((lo == LBM_PERIODIC) != (hi == LBM_PERIODIC)) return fail(h, LBM_EINVAL, "set_boundaries: PERIODIC must be set on both faces of an axis");
+    }
+    for (int k = 0; k < 6; ++k) h->face[k] = face_type[k];
+    h->have_flags = false;
+    return LBM_OK;
+}
+
+int lbm_set_flags(lbm_t *h, const int32_t *height)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_set_flags<double>(h, height) : do_set_flags<float>(h, height);
+}
+
+int lbm_set_inlet_profile(lbm_t *h, const float *u, const float *v, const float *w) { return set_inlet_profile_any<float>(h, u, v, w); }
+int lbm_set_inlet_profile_f64(lbm_t *h, const double *u, const double *v, const double *w) { return set_inlet_profile_any<double>(h, u, v, w); }
+int lbm_set_inlet_plane(lbm_t *h, int face, const float *uvw) { return set_inlet_plane_any<float>(h, face, uvw); }
+int lbm_set_inlet_plane_f64(lbm_t *h, int face, const double *uvw) { return set_inlet_plane_any<double>(h, face, uvw); }
+
+int lbm_feed_inlet(lbm_t *dst, const lbm_t *src, int src_x_plane)
+{
+    if (!dst || !src) return LBM_EINVAL;
+    if (!dst->have_flags || !src->have_flags) return fail(dst, LBM_ESTATE, "feed_inlet: flags not set");
+    if (dst->fp64 != src->fp64) return fail(dst, LBM_EINVAL, "feed_inlet: precision mismatch");
+    if (dst->nz != src->nz) return fail(dst, LBM_EINVAL, "feed_inlet: nz mismatch");
+    if (src_x_plane < 0 || src_x_plane >= src->nx) return fail(dst, LBM_EINVAL, "feed_inlet: plane out of range");
+    return dst->fp64 ? do_feed<double>(dst, src, src_x_plane) : do_feed<float>(dst, src, src_x_plane);
+}
+
+int lbm_set_macros(lbm_t *h, const float *rho, const float *ux, const float *uy, const float *uz)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_set_macros<double, float>(h, rho, ux, uy, uz) : do_set_macros<float, float>(h, rho, ux, uy, uz);
+}
+int lbm_set_macros_f64(lbm_t *h, const double *rho, const double *ux, const double *uy, const double *uz)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_set_macros<double, double>(h, rho, ux, uy, uz) : do_set_macros<float, double>(h, rho, ux, uy, uz);
+}
+
+int lbm_step(lbm_t *h, int n)
+{
+    if (!h) return LBM_EINVAL;
+    if (n < 0) return fail(h, LBM_EINVAL, "step: n < 0");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "step: flags not set");
+    return h->fp64 ? do_step<double>(h, n) : do_step<float>(h, n);
+}
+
+int lbm_mean_config(lbm_t *h, long start_step, int every)
+{
+    if (!h) return LBM_EINVAL;
+    if (!h->want_mean) return fail(h, LBM_ESTATE, "mean_config: handle created without mean sums");
+    if (every < 0 || start_step < 0) return fail(h, LBM_EINVAL, "mean_config: negative argument");
+    h->mstart = start_step; h->mevery = every;
+    return LBM_OK;
+}
+
+int lbm_mean_reset(lbm_t *h)
+{
+    if (!h) return LBM_EINVAL;
+    if (!h->want_mean) return fail(h, LBM_ESTATE, "mean_reset: handle created without mean sums");
+    CUDA_TRY(h, cudaMemsetAsync(h->mean(), 0, (size_t)3 * h->L.stride * (h->fp64 ? 8 : 4), h->stream));
+    h->mcount = 0;
+    return LBM_OK;
+}
+
+int lbm_get_macros(lbm_t *h, float *rho, float *ux, float *uy, float *uz)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_get_macros<double, float>(h, rho, ux, uy, uz) : do_get_macros<float, float>(h, rho, ux, uy, uz);
+}
+int lbm_get_macros_f64(lbm_t *h, double *rho, double *ux, double *uy, double *uz)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_get_macros<double, double>(h, rho, ux, uy, uz) : do_get_macros<float, double>(h, rho, ux, uy, uz);
+}
+
+int lbm_get_mean(lbm_t *h, float *ux, float *uy, float *uz, long *n_samples)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_get_mean<double, float>(h, ux, uy, uz, n_samples) : do_get_mean<float, float>(h, ux, uy, uz, n_samples);
+}
+int lbm_get_mean_f64(lbm_t *h, double *ux, double *uy, double *uz, long *n_samples)
+{
+    if (!h) return LBM_EINVAL;
+    return h->fp64 ? do_get_mean<double, double>(h, ux, uy, uz, n_samples) : do_get_mean<float, double>(h, ux, uy, uz, n_samples);
+}
+
+int lbm_get_flags(lbm_t *h, uint8_t *flags)
+{
+    if (!h) return LBM_EINVAL;
+    if (!flags) return fail(h, LBM_EINVAL, "get_flags: NULL");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_flags: flags not set");
+    OutBuf o;
+    int rc = stage_out(h, flags, (size_t)h->N(), &o);
+    if (rc) return rc;
+    const int B = 256;
+    flags_out_kernel<<<blocks_for(h->N(), B), B, 0, h->stream>>>(h->flags(), (uint8_t *)o.dev, (int)h->N());
+    rc = check_launch(h, "flags_out_kernel");
+    int rc2 = finish_out(h, &o, 1);
+    return rc ? rc : rc2;
+}
+
+int lbm_get_links(lbm_t *h, uint32_t *links)
+{
+    if (!h) return LBM_EINVAL;
+    if (!links) return fail(h, LBM_EINVAL, "get_links: NULL");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_links: flags not set");
+    return h->fp64 ? do_get_links<double>(h, links) : do_get_links<float>(h, links);
+}
+
+int lbm_get_state(lbm_t *h, double *f)
+{
+    if (!h) return LBM_EINVAL;
+    if (!f) return fail(h, LBM_EINVAL, "get_state: NULL");
+    return h->fp64 ? do_get_state<double>(h, f) : do_get_state<float>(h, f);
+}
+
+int lbm_set_state(lbm_t *h, const double *f)
+{
+    if (!h) return LBM_EINVAL;
+    if (!f) return fail(h, LBM_EINVAL, "set_state: NULL");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_state: flags not set");
+    return h->fp64 ? do_set_state<double>(h, f) : do_set_state<float>(h, f);
+}
+
+long lbm_get_step(const lbm_t *h) { return h ? h->step : -1; }
+int lbm_set_step(lbm_t *h, long step) { if (!h || step < 0) return LBM_EINVAL; h->step = step; return LBM_OK; }
+
+int lbm_sync(lbm_t *h)
+{
+    if (!h) return LBM_EINVAL;
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+
+const char *lbm_last_error(const lbm_t *h) { return h ? h->err.c_str() : "NULL handle"; }
+long lbm_launch_count(const lbm_t *h) { return h ? h->launches : -1; }
+
+int lbm_lattice(int *c, int *opposite)
+{
+    if (!c || !opposite) return LBM_EINVAL;
+    for (int i = 0; i < Q; ++i) {
+        c[3 * i + 0] = dir_cx(i); c[3 * i + 1] = dir_cy(i); c[3 * i + 2] = dir_cz(i);
+        opposite[i] = dir_opp(i);
+    }
+    return LBM_OK;
+}
+
+int lbm_set_variant(lbm_t *h, int variant)
+{
+    if (!h) return LBM_EINVAL;
+    if (variant != 0) return fail(h, LBM_EINVAL, "set_variant: unknown variant");
+    h->variant = variant;
+    return LBM_OK;
+}
+
+} // extern "C"

@@ -1,0 +1,353 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU FP64 oracle, on the same seeded inputs.
+
+Bars (BASELINE.json north_star): flags and link classes bit-exact; max-abs(rho, u) <= 1e-5 (lattice units) after
+100 steps for the FP32 path; the FP64 instantiation of the same kernels must agree to ~1e-12.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL32 = 1e-5    # north_star
+TOL64 = 2e-12   # rounding order only
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_04516_b200 import binding, build
+    build.build()
+    return binding
+
+
+def make_oracle(wl):
+    from oracle import Oracle
+    o = Oracle(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces)
+    o.set_flags(wl.height)
+    if wl.inlet_profile is not None:
+        o.set_inlet_profile(*wl.inlet_profile)
+    if wl.init is not None:
+        o.set_macros(*wl.init)
+    else:
+        o.set_macros()
+    return o
+
+
+def max_err(sim, o, f64=False):
+    g = [a.cpu().numpy() for a in sim.get_macros(f64=f64)]
+    r = o.get_macros()
+    assert all(np.isfinite(a).all() for a in g)
+    return max(float(np.abs(a.astype(np.float64) - b).max()) for a, b in zip(g, r))
+
+
+def check_flags_links(sim, o):
+    np.testing.assert_array_equal(sim.get_flags(), o.get_flags())
+    np.testing.assert_array_equal(sim.get_links(), o.get_links())
+
+
+# ---------------------------------------------------------------------------------------------- integer work
+
+FACE_SETS = [
+    (0, 0, 0, 0, 0, 0), (3, 4, 0, 0, 1, 2), (3, 4, 2, 2, 1, 2), (3, 4, 3, 3, 1, 2), (0, 0, 0, 0, 1, 2),
+    (1, 1, 1, 1, 1, 1), (2, 2, 2, 2, 2, 2), (2, 1, 0, 0, 2, 1), (4, 3, 1, 2, 0, 0),
+]
+
+
+@pytest.mark.parametrize("faces", FACE_SETS)
+def test_flags_and_links_bit_exact_small_ragged_boxes(B, faces):
+    from oracle import Oracle
+    rng = np.random.default_rng(abs(hash(faces)) % (2 ** 32))
+    for nx, ny, nz in [(6, 5, 4), (33, 7, 9), (70, 3, 5), (1, 1, 3), (5, 1, 1)]:
+        hm = rng.integers(-1, nz + 2, size=(ny, nx)).astype(np.int32)
+        hm[rng.random((ny, nx)) < 0.5] = 0
+        o = Oracle(nx, ny, nz, 1e-3, 0.1, 0.0, (0, 0, 0), faces)
+        o.set_flags(hm)
+        sim = B.Lbm(nx, ny, nz, 1e-3, 0.1, 0.0, (0, 0, 0), faces)
+        sim.set_flags(hm)
+        check_flags_links(sim, o)
+        sim.close()
+
+
+def test_flags_and_links_bit_exact_config3_full(B):
+    from paper_2607_04516_b200 import workloads as W
+    from oracle import Oracle
+    wl = W.config3()
+    o = Oracle(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces)
+    o.set_flags(wl.height)
+    sim = B.Lbm(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces, want_mean=False)
+    sim.set_flags(wl.height)
+    check_flags_links(sim, o)
+    assert int((sim.get_flags() == 1).sum()) == int(wl.height.sum())
+
+
+def test_null_heightmap_is_flat_ground_and_device_heightmap_works(B):
+    import torch
+    from oracle import Oracle
+    faces = (3, 4, 2, 2, 1, 2)
+    o = Oracle(20, 10, 6, 1e-3, 0.1, 0.0, (0, 0, 0), faces)
+    o.set_flags(None)
+    sim = B.Lbm(20, 10, 6, 1e-3, 0.1, 0.0, (0, 0, 0), faces)
+    sim.set_flags(None)
+    check_flags_links(sim, o)
+    hm = np.zeros((10, 20), dtype=np.int32)
+    hm[3:6, 5:9] = 4
+    o.set_flags(hm)
+    sim.set_flags(torch.from_numpy(hm).cuda())
+    check_flags_links(sim, o)
+
+
+# ---------------------------------------------------------------------------------------------- floating point
+
+def test_config1_100_and_200_steps(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config1()
+    o = make_oracle(wl)
+    sim = B.from_workload(wl)
+    check_flags_links(sim, o)
+    for upto in (100, 200):
+        o.step(upto - o.get_step())
+        sim.step(upto - sim.get_step())
+        e = max_err(sim, o)
+        print(f"C1 step {upto}: max|gpu32 - oracle| = {e:.3e}")
+        assert e <= TOL32
+    assert sim.get_step() == 200
+
+
+def test_config1_fp64_kernels_agree_to_rounding(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config1()
+    o = make_oracle(wl)
+    sim = B.from_workload(wl, fp64=True)
+    o.step(100)
+    sim.step(100)
+    e = max_err(sim, o, f64=True)
+    print(f"C1 step 100: max|gpu64 - oracle| = {e:.3e}")
+    assert e <= TOL64
+
+
+@pytest.mark.parametrize("Cs", [0.0, 0.1])
+def test_config2_taylor_green_100_steps(B, Cs):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config2(Cs=Cs)
+    o = make_oracle(wl)
+    sim = B.from_workload(wl)
+    o.step(100)
+    sim.step(100)
+    e = max_err(sim, o)
+    print(f"C2 Cs={Cs} step 100: max|gpu32 - oracle| = {e:.3e}")
+    assert e <= TOL32
+
+
+def test_config3_full_100_steps(B):
+    """The bench workload itself, in the launch configuration bench.py times, against the oracle on every cell."""
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config3()
+    o = make_oracle(wl)
+    sim = B.from_workload(wl, want_mean=False)
+    o.step(100)
+    sim.step(100)
+    e = max_err(sim, o)
+    print(f"C3 400x400x100 step 100: max|gpu32 - oracle| = {e:.3e}")
+    assert e <= TOL32
+
+
+def test_config3_crop_fp64_and_ragged_sizes(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config3(nx=150, ny=77, nz=50)   # 150 and 77 are not multiples of the warp or of 4
+    o = make_oracle(wl)
+    s32 = B.from_workload(wl)
+    s64 = B.from_workload(wl, fp64=True)
+    o.step(100)
+    s32.step(100)
+    s64.step(100)
+    e32, e64 = max_err(s32, o), max_err(s64, o, f64=True)
+    print(f"C3 crop step 100: fp32 {e32:.3e}  fp64 {e64:.3e}")
+    assert e32 <= TOL32 and e64 <= TOL64
+
+
+def test_config4_crop_veering_inlet_on_three_faces(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config4(nx=120, ny=90, nz=200)
+    o = make_oracle(wl)
+    sim = B.from_workload(wl)
+    check_flags_links(sim, o)
+    o.step(100)
+    sim.step(100)
+    e = max_err(sim, o)
+    print(f"C4 crop step 100: {e:.3e}")
+    assert e <= TOL32
+
+
+def test_config5_precursor_crop_with_pressure_gradient_force(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config5_precursor(nx=64, ny=48, nz=200)
+    o = make_oracle(wl)
+    sim = B.from_workload(wl)
+    o.step(100)
+    sim.step(100)
+    e = max_err(sim, o)
+    print(f"C5 precursor crop step 100: {e:.3e}")
+    assert e <= TOL32
+
+
+def test_config5_chain_precursor_plane_feeds_main_inlet_every_step(B):
+    """Coupled run (a8): each step the precursor plane x_s is written into the main x- inlet, then both advance.
+    The oracle side does the same through get_macros/set_inlet_plane."""
+    from paper_2607_04516_b200 import workloads as W
+    from oracle import Oracle
+    pre = W.config5_precursor(nx=32, ny=24, nz=40)
+    main = W.config5_main(nx=96, ny=60, nz=40)   # 60 is not a multiple of 24: the last tile is cut
+    xs = 16
+    op, om = make_oracle(pre), make_oracle(main)
+    gp, gm = B.from_workload(pre), B.from_workload(main)
+    reps = -(-main.ny // pre.ny)
+    for _ in range(30):
+        _, ux, uy, uz = op.get_macros()
+        plane = np.stack([np.tile(q[:, :, xs], (1, reps))[:, :main.ny] for q in (ux, uy, uz)])
+        om.set_inlet_plane(0, plane)
+        gm.feed_inlet(gp, xs)
+        op.step(1); om.step(1)
+        gp.step(1); gm.step(1)
+    e_pre, e_main = max_err(gp, op), max_err(gm, om)
+    print(f"C5 chain step 30: precursor {e_pre:.3e} main {e_main:.3e}")
+    assert e_pre <= TOL32 and e_main <= TOL32
+
+
+def test_inlet_plane_host_and_device_pointers(B):
+    import torch
+    from oracle import Oracle
+    rng = np.random.default_rng(12)
+    nx, ny, nz = 24, 10, 8
+    faces = (3, 4, 3, 3, 1, 2)
+    o = Oracle(nx, ny, nz, 2e-3, 0.1, 0.0, (0, 0, 0), faces)
+    o.set_flags()
+    sim = B.Lbm(nx, ny, nz, 2e-3, 0.1, 0.0, (0, 0, 0), faces)
+    sim.set_flags()
+    px = (0.03 + 0.01 * rng.random((3, nz, ny))).astype(np.float32)
+    py = (0.03 + 0.01 * rng.random((3, nz, nx))).astype(np.float32)
+    o.set_inlet_plane(0, px); o.set_inlet_plane(2, py); o.set_inlet_plane(3, py)
+    sim.set_inlet_plane(0, px)                             # host pointer
+    sim.set_inlet_plane(2, torch.from_numpy(py).cuda())    # device pointer
+    sim.set_inlet_plane(3, py.astype(np.float64), f64=True)
+    o.set_macros(None, np.full(o.shape, 0.03), np.full(o.shape, 0.03), None)
+    sim.set_macros(None, np.full(o.shape, 0.03, dtype=np.float32), np.full(o.shape, 0.03, dtype=np.float32), None)
+    o.step(40); sim.step(40)
+    assert max_err(sim, o) <= TOL32
+
+
+def test_time_mean_matches_oracle_and_fused_equals_standalone_definition(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config3(nx=96, ny=64, nz=40)
+    o = make_oracle(wl)
+    sim = B.from_workload(wl)
+    o.mean_config(20, 5); sim.mean_config(20, 5)
+    o.step(60); sim.step(60)
+    gm = sim.get_mean()
+    om = o.get_mean()
+    assert gm[3] == om[3] == 9
+    for a, b in zip(gm[:3], om[:3]):
+        assert float(np.abs(a.cpu().numpy() - b).max()) <= TOL32
+    flags = sim.get_flags()
+    assert np.all(gm[0].cpu().numpy()[flags == 1] == 0)
+    # horizontal mean profile within 1e-5 as well
+    pg = W.mean_profile(gm[0].cpu().numpy(), flags)
+    po = W.mean_profile(om[0], flags)
+    assert np.abs(pg - po).max() <= TOL32
+    sim.mean_reset()
+    assert sim.get_mean()[3] == 0
+
+
+def test_state_roundtrip_and_restart_from_a_developed_gpu_state(B):
+    """lbm_get_state at a developed step -> the oracle continues 100 steps from that state."""
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config1()
+    sim = B.from_workload(wl)
+    sim.step(700)
+    st = sim.get_state(out="host")
+    assert np.isfinite(st).all()
+    o = make_oracle(wl)
+    o.set_state(st)
+    o.set_step(700)
+    assert max_err(sim, o) <= 1e-7          # same state, FP32 vs FP64 evaluation of the macros
+    o.step(100); sim.step(100)
+    e = max_err(sim, o)
+    print(f"C1 restart 700 -> 800: {e:.3e}")
+    assert e <= TOL32
+    # round trip through set_state is the identity on the FP32 state
+    sim2 = B.from_workload(wl)
+    sim2.set_state(sim.get_state())
+    a, b = sim.get_state(out="host"), sim2.get_state(out="host")
+    assert np.array_equal(a, b)
+
+
+def test_rest_state_is_exactly_zero_in_shifted_storage(B):
+    hm = np.zeros((12, 16), dtype=np.int32)
+    hm[3:6, 4:8] = 5
+    _, w, _ = __import__("oracle").lattice()
+    for faces in [(3, 4, 0, 0, 1, 2), (2, 2, 1, 1, 0, 0), (0,) * 6]:
+        sim = B.Lbm(16, 12, 8, 1e-3, 0.1, 0.0, (0, 0, 0), faces)
+        sim.set_flags(hm)
+        sim.set_inlet_profile(np.zeros(8, dtype=np.float32))
+        sim.set_macros()
+        sim.step(50)
+        st = sim.get_state(out="host")
+        assert np.array_equal(st, np.broadcast_to(w[:, None, None, None], st.shape))
+        rho, ux, uy, uz = (a.cpu().numpy() for a in sim.get_macros())
+        assert np.all(rho == 1) and np.all(ux == 0) and np.all(uy == 0) and np.all(uz == 0)
+
+
+def test_mass_conservation_and_inertial_rotation_on_the_gpu(B):
+    """Properties that hold at any size, checked on the FP32 path itself: periodic-box mass is conserved to FP32
+    rounding and total momentum turns by -2 atan(f/2) per step."""
+    import math
+    import torch
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config2(Cs=0.1, n=64, nz=16)
+    wl.f_cor = 0.01
+    sim = B.from_workload(wl)
+    c, _ = B.lattice()
+    ct = torch.tensor(c, dtype=torch.float64, device="cuda")
+
+    def mom():
+        st = sim.get_state()
+        return torch.einsum("ia,izyx->a", ct, st).cpu().numpy(), float(st.sum())
+
+    P0, m0 = mom()
+    sim.step(200)
+    P1, m1 = mom()
+    assert abs(m1 / m0 - 1) < 1e-7
+    assert abs(np.hypot(*P1[:2]) / np.hypot(*P0[:2]) - 1) < 1e-4   # FP32 rounding over 200 steps (FP64 oracle: 1e-12)
+    dth = math.atan2(P1[1], P1[0]) - math.atan2(P0[1], P0[0])
+    assert dth == pytest.approx(-200 * 2 * math.atan(0.005), abs=1e-4)
+
+
+def test_zero_steps_and_call_order_errors(B):
+    sim = B.Lbm(8, 8, 8, 1e-3)
+    with pytest.raises(B.LbmError, match="LBM_ESTATE"):
+        sim.step(1)
+    with pytest.raises(B.LbmError, match="LBM_ESTATE"):
+        sim.set_macros()
+    with pytest.raises(B.LbmError, match="LBM_EINVAL"):
+        sim.set_boundaries((0, 1, 0, 0, 0, 0))
+    sim.set_flags()
+    sim.set_macros()
+    n0 = sim.launch_count()
+    sim.step(0)
+    assert sim.get_step() == 0 and sim.launch_count() == n0
+    with pytest.raises(B.LbmError, match="LBM_EINVAL"):
+        sim.step(-1)
+    nomean = B.Lbm(8, 8, 8, 1e-3, want_mean=False)
+    with pytest.raises(B.LbmError, match="LBM_ESTATE"):
+        nomean.mean_config(0, 1)
+
+
+def test_host_pointer_getters_equal_device_pointer_getters(B):
+    from paper_2607_04516_b200 import workloads as W
+    sim = B.from_workload(W.config1())
+    sim.step(10)
+    dev = [a.cpu().numpy() for a in sim.get_macros()]
+    host = sim.get_macros(out="host")
+    for a, b in zip(dev, host):
+        assert np.array_equal(a, b)
