@@ -283,17 +283,36 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     return rc;
 }
 
-template <typename real>
-int launch_step(lbm_t *h, const Params<real> &P, bool sample)
+template <typename real, int HINT, int BLOCK, int MINB>
+int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
     const real *A = (const real *)h->state();
     real *B = (real *)h->other();
     real *ms = (real *)h->mean();
-    const int BS = 256;
-    const unsigned grid = blocks_for(P.N, BS);
-    if (sample) step_kernel<real, true><<<grid, BS, 0, h->stream>>>(A, B, h->flags(), ms, P);
-    else step_kernel<real, false><<<grid, BS, 0, h->stream>>>(A, B, h->flags(), ms, P);
+    const unsigned grid = blocks_for(P.N, BLOCK);
+    if (sample) step_kernel<real, true, HINT, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), ms, P);
+    else step_kernel<real, false, HINT, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), ms, P);
     return check_launch(h, "step_kernel");
+}
+
+// kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes
+constexpr int N_VARIANTS = 8;
+template <typename real>
+int launch_step(lbm_t *h, const Params<real> &P, bool sample)
+{
+    if constexpr (std::is_same<real, float>::value) {
+        switch (h->variant) {
+        case 1: return launch_step_as<real, 1, 256, 4>(h, P, sample);
+        case 2: return launch_step_as<real, 2, 256, 4>(h, P, sample);
+        case 3: return launch_step_as<real, 3, 256, 4>(h, P, sample);
+        case 4: return launch_step_as<real, 0, 128, 8>(h, P, sample);
+        case 5: return launch_step_as<real, 0, 512, 2>(h, P, sample);
+        case 6: return launch_step_as<real, 0, 256, 5>(h, P, sample);
+        case 7: return launch_step_as<real, 0, 128, 12>(h, P, sample);
+        default: break;
+        }
+    }
+    return launch_step_as<real, 0, 256, 4>(h, P, sample);
 }
 
 template <typename real>
@@ -630,7 +649,7 @@ int lbm_lattice(int *c, int *opposite)
 int lbm_set_variant(lbm_t *h, int variant)
 {
     if (!h) return LBM_EINVAL;
-    if (variant != 0) return fail(h, LBM_EINVAL, "set_variant: unknown variant");
+    if (variant < 0 || variant >= N_VARIANTS) return fail(h, LBM_EINVAL, "set_variant: unknown variant");
     h->variant = variant;
     return LBM_OK;
 }

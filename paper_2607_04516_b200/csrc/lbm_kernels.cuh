@@ -15,7 +15,8 @@ constexpr int Q = 19;
 enum : int { FLUID = 0, SOLID = 1, EQ_FIXED = 2, EQ_OUTFLOW = 3 };
 enum : int { PERIODIC = 0, WALL = 1, FREE_SLIP = 2, FACE_EQ_FIXED = 3, FACE_EQ_OUTFLOW = 4 };
 constexpr uint8_t CLASS_MASK = 3;
-constexpr uint8_t SLOW_BIT = 0x80;
+constexpr uint8_t SLOW_BIT = 0x80; // FLUID cell with at least one wall link
+constexpr uint8_t EDGE_BIT = 0x40; // FLUID cell on a domain face (periodic / free-slip / wall resolution needed)
 
 // ---- lattice (DESIGN.md §3 step 1): pair k = 1..9 holds directions 2k-1 (+) and 2k (-) -------------------------
 // pair vectors: 1:(1,0,0) 2:(0,1,0) 3:(0,0,1) 4:(1,1,0) 5:(1,0,1) 6:(0,1,1) 7:(1,-1,0) 8:(1,0,-1) 9:(0,1,-1)
@@ -59,10 +60,19 @@ struct Macro { real rho, ux, uy, uz; };
 
 // ---- cache-hinted global access ----------------------------------------------------------------------------------
 // Every population is read exactly once and written exactly once per step: stream them.
-template <typename real>
-__device__ __forceinline__ real ld_stream(const real *p) { return __ldcs(p); }
-template <typename real>
-__device__ __forceinline__ void st_stream(real *p, real v) { __stcs(p, v); }
+// HINT: 0 = ld.cs / st.cs, 1 = default / default, 2 = default ld / st.cs, 3 = ld.cs / default st
+template <int HINT, typename real>
+__device__ __forceinline__ real ld_pop(const real *p)
+{
+    if constexpr (HINT == 0 || HINT == 3) return __ldcs(p);
+    else return *p;
+}
+template <int HINT, typename real>
+__device__ __forceinline__ void st_pop(real *p, real v)
+{
+    if constexpr (HINT == 0 || HINT == 2) __stcs(p, v);
+    else *p = v;
+}
 
 // ---- collision (DESIGN.md §3 steps 4b-4e) on shifted populations ---------------------------------------------------
 // In: pulled g[19].  Out: post-collision g[19]; returns the (rho,u) the collision used.
@@ -169,11 +179,10 @@ __device__ __forceinline__ void load_cell(real (&g)[Q], const real *__restrict__
 }
 
 // ---- pull resolution (DESIGN.md §3 step 4a) -------------------------------------------------------------------------
-// For FLUID cell (x,y,z) and direction I: returns true for the bounce-back branch, else the source cell and
-// source direction.  Axis order z, y, x; solidity of the resolved source tested last.
+// Geometry part, no memory access: for FLUID cell (x,y,z) and direction I, returns true if a WALL face is crossed;
+// else the source cell and source direction after periodic wrap / free-slip mirroring.  Axis order z, y, x.
 template <int I, typename real>
-__device__ __forceinline__ bool resolve(const Params<real> &P, const uint8_t *__restrict__ flags, int x, int y, int z,
-                                        int &src_cell, int &src_dir)
+__device__ __forceinline__ bool resolve_geom(const Params<real> &P, int x, int y, int z, int &src_cell, int &src_dir)
 {
     constexpr int cx = dir_cx(I), cy = dir_cy(I), cz = dir_cz(I);
     int sx = x - cx, sy = y - cy, sz = z - cz;
@@ -205,9 +214,6 @@ __device__ __forceinline__ bool resolve(const Params<real> &P, const uint8_t *__
             else wall = true;
         }
     }
-    if (wall) return true;
-    src_cell = (sz * P.ny + sy) * P.nx + sx;
-    if ((flags[src_cell] & CLASS_MASK) == SOLID) return true;
     // mirrored direction: a compile-time candidate per flip combination, selected by the three flip bits
     const int key = (fx ? 1 : 0) | (fy ? 2 : 0) | (fz ? 4 : 0);
     int j = I;
@@ -220,19 +226,41 @@ __device__ __forceinline__ bool resolve(const Params<real> &P, const uint8_t *__
         }
     });
     src_dir = j;
-    return false;
+    src_cell = wall ? (z * P.ny + y) * P.nx + x : (sz * P.ny + sy) * P.nx + sx;
+    return wall;
 }
 
+// Bit i set <=> pulling direction i takes the bounce-back branch.  All neighbour flag loads are independent of one
+// another (no branch between them), so they are issued as one batch.
 template <typename real>
-__device__ __forceinline__ uint32_t link_mask(const Params<real> &P, const uint8_t *__restrict__ flags, int x, int y, int z)
+__device__ __forceinline__ uint32_t link_mask_edge(const Params<real> &P, const uint8_t *__restrict__ flags, int x, int y, int z)
 {
     uint32_t bits = 0;
     static_for<1, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         int s, j;
-        if (resolve<i>(P, flags, x, y, z, s, j)) bits |= (1u << i);
+        const bool wall = resolve_geom<i>(P, x, y, z, s, j);
+        const uint8_t f = flags[s]; // own (FLUID) cell when a wall face was crossed
+        bits |= ((wall || (f & CLASS_MASK) == SOLID) ? 1u : 0u) << i;
     });
     return bits;
+}
+template <typename real>
+__device__ __forceinline__ uint32_t link_mask_interior(const Params<real> &P, const uint8_t *__restrict__ flags, int cell)
+{
+    uint32_t bits = 0;
+    static_for<1, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        const int off = dir_cx(i) + dir_cy(i) * P.nx + dir_cz(i) * P.nxy;
+        bits |= (((flags[cell - off] & CLASS_MASK) == SOLID) ? 1u : 0u) << i;
+    });
+    return bits;
+}
+
+template <typename real>
+__device__ __forceinline__ uint32_t link_mask(const Params<real> &P, const uint8_t *__restrict__ flags, int x, int y, int z)
+{
+    return link_mask_edge(P, flags, x, y, z);
 }
 
 // which face's normal an EQ_OUTFLOW cell uses: first EQ_OUTFLOW face it lies on, order x-,x+,y-,y+,z-,z+
@@ -286,7 +314,7 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags_out, const uint8_t *
     if (links) links[cell] = bits;
     if (flags_out) {
         const bool edge = x == 0 || x == P.nx - 1 || y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
-        flags_out[cell] = cls | ((cls == FLUID && (bits != 0 || edge)) ? SLOW_BIT : 0);
+        flags_out[cell] = cls | ((cls == FLUID && bits != 0) ? SLOW_BIT : 0) | ((cls == FLUID && edge) ? EDGE_BIT : 0);
     }
 }
 
@@ -375,8 +403,8 @@ __global__ void init_kernel(real *__restrict__ A, real *__restrict__ B, const ui
 }
 
 // ---- a5/a6: fused stream-collide, one cell per thread (variant 0) ----------------------------------------------------------
-template <typename real, bool MEAN>
-__global__ void __launch_bounds__(256)
+template <typename real, bool MEAN, int HINT, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
 step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, real *__restrict__ msum,
             Params<real> P)
 {
@@ -407,26 +435,40 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
         }
         equilibrium(g, real(0), m.ux, m.uy, m.uz);
     } else {
-        if (!(fl & SLOW_BIT)) {
+        if (!(fl & (SLOW_BIT | EDGE_BIT))) {
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 const int off = dir_cx(i) + dir_cy(i) * P.nx + dir_cz(i) * P.nxy;
-                g[i] = ld_stream(A + ((long long)i * P.stride + (cell - off)));
+                g[i] = ld_pop<HINT>(A + ((long long)i * P.stride + (cell - off)));
+            });
+        } else if (!(fl & EDGE_BIT)) {
+            // interior cell next to a solid: neighbours are plain offsets, some links bounce back
+            const uint32_t bb = link_mask_interior(P, flags, cell);
+            g[0] = ld_pop<HINT>(A + cell);
+            static_for<1, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                const int off = dir_cx(i) + dir_cy(i) * P.nx + dir_cz(i) * P.nxy;
+                const bool b = (bb >> i) & 1u;
+                const long long pop = b ? (long long)dir_opp(i) * P.stride : (long long)i * P.stride;
+                g[i] = ld_pop<HINT>(A + (pop + (b ? cell : cell - off)));
             });
         } else {
+            // cell on a domain face: periodic wrap / free-slip mirror / wall, then solidity of the resolved source
             const int x = cell % P.nx, y = (cell / P.nx) % P.ny, z = cell / P.nxy;
-            g[0] = ld_stream(A + cell);
+            const uint32_t bb = link_mask_edge(P, flags, x, y, z);
+            g[0] = ld_pop<HINT>(A + cell);
             static_for<1, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 int s, j;
-                if (resolve<i>(P, flags, x, y, z, s, j)) { s = cell; j = dir_opp(i); }
-                g[i] = ld_stream(A + ((long long)j * P.stride + s));
+                resolve_geom<i>(P, x, y, z, s, j);
+                const bool b = (bb >> i) & 1u;
+                g[i] = ld_pop<HINT>(A + ((long long)(b ? dir_opp(i) : j) * P.stride + (b ? cell : s)));
             });
         }
         m = collide(g, P);
     }
 #pragma unroll
-    for (int i = 0; i < Q; ++i) st_stream(B + ((long long)i * P.stride + cell), g[i]);
+    for (int i = 0; i < Q; ++i) st_pop<HINT>(B + ((long long)i * P.stride + cell), g[i]);
     if constexpr (MEAN) {
         msum[cell] += m.ux;
         msum[P.stride + cell] += m.uy;
