@@ -476,6 +476,239 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
     }
 }
 
+// ---- a5/a6: fused stream-collide, FOUR x-consecutive cells per thread, 128-bit loads and stores (default for FP32) --------
+// Thread t owns cells c = 4t .. 4t+3 of the linear [z][y][x] index (nx % 4 == 0, so c, nx and nx*ny are multiples of 4
+// and every population row is 16-byte aligned).  Pull of direction i for the four cells = elements (c - off_i .. c+3 - off_i):
+//   c_x = 0 : one aligned 128-bit load at c - off_yz;
+//   c_x = +1: the same aligned load, shifted right by one element: element -1 comes from the left lane (__shfl_up),
+//             lane 0 fetches it with one scalar load;  c_x = -1: mirror image with __shfl_down / lane 31.
+// This is the plain interior streaming.  Cells whose flag byte has SLOW_BIT / EDGE_BIT then overwrite the affected
+// directions (bounce-back from the stored link mask, periodic / free-slip / wall resolution on domain faces); static
+// cells (SOLID, EQ_FIXED, EQ_OUTFLOW) are not stored.  EQ face cells are served by the first `face_blocks` blocks of the
+// same launch (face_worker).  The arrays are padded by >= nx*ny + nx + 8 elements at both ends, so the unconditional
+// vector loads of cells next to the domain faces stay inside the allocation (their values are replaced above).
+template <typename real>
+struct alignas(4 * sizeof(real)) Vec4 { real x, y, z, w; };
+
+template <int J, typename real>
+__device__ __forceinline__ real &comp(Vec4<real> &v)
+{
+    if constexpr (J == 0) return v.x;
+    else if constexpr (J == 1) return v.y;
+    else if constexpr (J == 2) return v.z;
+    else return v.w;
+}
+template <typename real>
+__device__ __forceinline__ void set_comp(Vec4<real> &v, int j, real val)
+{
+    v.x = j == 0 ? val : v.x;
+    v.y = j == 1 ? val : v.y;
+    v.z = j == 2 ? val : v.z;
+    v.w = j == 3 ? val : v.w;
+}
+
+template <int HINT, typename real>
+__device__ __forceinline__ Vec4<real> ld_vec(const real *p)
+{
+    const Vec4<real> *q = reinterpret_cast<const Vec4<real> *>(p);
+    if constexpr (std::is_same<real, float>::value && (HINT == 0 || HINT == 3)) {
+        const float4 t = __ldcs(reinterpret_cast<const float4 *>(p));
+        return Vec4<real>{t.x, t.y, t.z, t.w};
+    } else return *q;
+}
+template <int HINT, typename real>
+__device__ __forceinline__ void st_vec(real *p, const Vec4<real> &v)
+{
+    if constexpr (std::is_same<real, float>::value && (HINT == 0 || HINT == 2)) __stcs(reinterpret_cast<float4 *>(p), make_float4(v.x, v.y, v.z, v.w));
+    else *reinterpret_cast<Vec4<real> *>(p) = v;
+}
+
+// EQ face cells (a6 and the EQ part of a7): worker thread w walks the planes of the faces that need per-step work.
+// A cell on several such faces is served from the first one in the order x-,x+,y-,y+,z-,z+ whose type matches its class.
+template <typename real, bool MEAN>
+__device__ __forceinline__ void face_worker(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+                                            real *__restrict__ msum, const Params<real> &P, long long w)
+{
+    int k = 0;
+    long long cnt = 0;
+    for (; k < 6; ++k) {
+        const int ft = P.face[k];
+        if (!(ft == FACE_EQ_OUTFLOW || (MEAN && ft == FACE_EQ_FIXED))) continue;
+        const int axis = k >> 1;
+        cnt = (long long)(axis == 0 ? P.ny : P.nx) * (axis == 2 ? P.ny : P.nz);
+        if (w < cnt) break;
+        w -= cnt;
+    }
+    if (k == 6) return;
+    const int axis = k >> 1;
+    const int n1 = axis == 0 ? P.ny : P.nx;
+    const int j1 = (int)(w % n1), j2 = (int)(w / n1);
+    const int nn[3] = {P.nx, P.ny, P.nz};
+    const int fixed = (k & 1) ? nn[axis] - 1 : 0;
+    int x, y, z;
+    if (axis == 0) { x = fixed; y = j1; z = j2; }
+    else if (axis == 1) { x = j1; y = fixed; z = j2; }
+    else { x = j1; y = j2; z = fixed; }
+    const int cell = (z * P.ny + y) * P.nx + x;
+    const int cls = flags[cell] & CLASS_MASK;
+    const int want = cls == EQ_OUTFLOW ? FACE_EQ_OUTFLOW : (cls == EQ_FIXED ? FACE_EQ_FIXED : -1);
+    if (want < 0 || P.face[k] != want) return;
+    const bool on[6] = {x == 0, x == P.nx - 1, y == 0, y == P.ny - 1, z == 0, z == P.nz - 1};
+    for (int q = 0; q < k; ++q)
+        if (on[q] && P.face[q] == want) return; // an earlier face owns this cell
+    real g[Q];
+    Macro<real> m{real(1), real(0), real(0), real(0)};
+    if (cls == EQ_OUTFLOW) {
+        const int nb = outflow_neighbour(P, x, y, z);
+        if (nb >= 0) {
+            load_cell(g, A, P.stride, nb);
+            m = local_macros(g, flags[nb] & CLASS_MASK, P);
+        }
+        equilibrium(g, real(0), m.ux, m.uy, m.uz);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) B[(long long)i * P.stride + cell] = g[i];
+    } else {
+        load_cell(g, A, P.stride, cell);
+        m = local_macros(g, EQ_FIXED, P);
+    }
+    if constexpr (MEAN) {
+        msum[cell] += m.ux;
+        msum[P.stride + cell] += m.uy;
+        msum[2 * P.stride + cell] += m.uz;
+    }
+}
+
+// number of worker threads face_worker needs
+template <typename real>
+inline long long face_work_items(const Params<real> &P, bool mean)
+{
+    long long n = 0;
+    for (int k = 0; k < 6; ++k) {
+        const int ft = P.face[k];
+        if (!(ft == FACE_EQ_OUTFLOW || (mean && ft == FACE_EQ_FIXED))) continue;
+        const int axis = k >> 1;
+        n += (long long)(axis == 0 ? P.ny : P.nx) * (axis == 2 ? P.ny : P.nz);
+    }
+    return n;
+}
+
+template <typename real, bool MEAN, int HINT, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+step4_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+             real *__restrict__ msum, Params<real> P, int face_blocks)
+{
+    using V = Vec4<real>;
+    if ((int)blockIdx.x < face_blocks) {
+        face_worker<real, MEAN>(A, B, flags, msum, P, (long long)blockIdx.x * BLOCK + threadIdx.x);
+        return;
+    }
+    const unsigned FULL = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const long long t = (long long)(blockIdx.x - face_blocks) * BLOCK + threadIdx.x;
+    const bool inside = 4 * t < P.N;
+    const int c = inside ? (int)(4 * t) : P.N - 4;
+    const uint32_t word = inside ? *reinterpret_cast<const uint32_t *>(flags + c) : 0x01010101u;
+    // byte j of nf: 1 = cell j is static (class != FLUID)
+    const uint32_t nf = (word | (word >> 1)) & 0x01010101u;
+    if (__all_sync(FULL, nf == 0x01010101u)) return;
+    // a lane's aligned vectors are needed by itself, by the right lane (its cell 0, c_x = +1) and the left lane (its cell 3)
+    const uint32_t nf_r = __shfl_down_sync(FULL, nf, 1), nf_l = __shfl_up_sync(FULL, nf, 1);
+    const bool need = nf != 0x01010101u || (lane < 31 && !(nf_r & 1u)) || (lane > 0 && !(nf_l >> 24));
+    const bool need_lo = lane == 0 && !(nf & 1u);         // element c-1 (c_x = +1 directions)
+    const bool need_hi = lane == 31 && !(nf >> 24);       // element c+4 (c_x = -1 directions)
+
+    V v[Q];
+    real e[Q];
+    const real *a = A + c;
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int cx = dir_cx(i), cy = dir_cy(i), cz = dir_cz(i);
+        const real *p = a + ((long long)i * P.stride - (cy * P.nx + cz * P.nxy));
+        v[i] = need ? ld_vec<HINT>(p) : V{real(0), real(0), real(0), real(0)};
+        if constexpr (cx == 1) e[i] = need_lo ? ld_pop<HINT>(p - 1) : real(0);
+        if constexpr (cx == -1) e[i] = need_hi ? ld_pop<HINT>(p + 4) : real(0);
+    });
+    static_for<1, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int cx = dir_cx(i);
+        if constexpr (cx == 1) {
+            real prev = __shfl_up_sync(FULL, v[i].w, 1);
+            if (lane == 0) prev = e[i];
+            v[i] = V{prev, v[i].x, v[i].y, v[i].z};
+        }
+        if constexpr (cx == -1) {
+            real next = __shfl_down_sync(FULL, v[i].x, 1);
+            if (lane == 31) next = e[i];
+            v[i] = V{v[i].y, v[i].z, v[i].w, next};
+        }
+    });
+
+    // cells with wall links or on a domain face: overwrite what plain streaming got wrong
+    if (word & 0xC0C0C0C0u) {
+#pragma unroll 1
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t fb = (word >> (8 * j)) & 0xFFu;
+            if (!(fb & (SLOW_BIT | EDGE_BIT))) continue;
+            const int cell = c + j;
+            const uint32_t bb = links[cell];
+            if (!(fb & EDGE_BIT)) {
+                static_for<1, Q>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    if ((bb >> i) & 1u) set_comp(v[i], j, A[(long long)dir_opp(i) * P.stride + cell]);
+                });
+            } else {
+                const int x = cell % P.nx, y = (cell / P.nx) % P.ny, z = cell / P.nxy;
+                static_for<1, Q>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    int s, jd;
+                    resolve_geom<i>(P, x, y, z, s, jd);
+                    const bool b = (bb >> i) & 1u;
+                    set_comp(v[i], j, A[(long long)(b ? dir_opp(i) : jd) * P.stride + (b ? cell : s)]);
+                });
+            }
+        }
+    }
+
+    V mu[3];
+    static_for<0, 4>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
+        real g[Q];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) g[i] = comp<j>(v[i]);
+        const Macro<real> m = collide(g, P);
+#pragma unroll
+        for (int i = 0; i < Q; ++i) comp<j>(v[i]) = g[i];
+        if constexpr (MEAN) { comp<j>(mu[0]) = m.ux; comp<j>(mu[1]) = m.uy; comp<j>(mu[2]) = m.uz; }
+    });
+
+    real *b = B + c;
+    if (nf == 0) {
+#pragma unroll
+        for (int i = 0; i < Q; ++i) st_vec<HINT>(b + (long long)i * P.stride, v[i]);
+        if constexpr (MEAN) {
+#pragma unroll
+            for (int k = 0; k < 3; ++k) {
+                V *mp = reinterpret_cast<V *>(msum + (long long)k * P.stride + c);
+                V s = *mp;
+                s.x += mu[k].x; s.y += mu[k].y; s.z += mu[k].z; s.w += mu[k].w;
+                *mp = s;
+            }
+        }
+    } else {
+        static_for<0, 4>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            if (!((nf >> (8 * j)) & 1u)) {
+#pragma unroll
+                for (int i = 0; i < Q; ++i) b[(long long)i * P.stride + j] = comp<j>(v[i]);
+                if constexpr (MEAN) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) msum[(long long)k * P.stride + c + j] += comp<j>(mu[k]);
+                }
+            }
+        });
+    }
+}
+
 // ---- a7: macros / mean / state ---------------------------------------------------------------------------------------------
 template <typename real, typename out_t>
 __global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
