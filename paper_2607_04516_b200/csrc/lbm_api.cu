@@ -1,6 +1,7 @@
 // lbm_api.cu — context, launch layer and C ABI (include/lbm.h) of the B200-native LBM-LES path.
 #include "../../include/lbm.h"
 #include "lbm_kernels.cuh"
+#include "lbm_step_tma.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -12,6 +13,7 @@ using namespace lbmk;
 namespace {
 
 constexpr size_t ALIGN = 256;
+constexpr size_t MAX_TILE = 1024; // largest tile (cells) of the bulk-copy step kernel
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 struct Layout {
@@ -26,10 +28,13 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
     const size_t N = (size_t)nx * ny * nz;
     const size_t rs = fp64 ? 8 : 4;
     L.stride = (long long)align_up(N, 64);
-    size_t o = 0;
-    L.off_A = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
-    L.off_B = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
-    L.off_flags = o; o += align_up(N, ALIGN);
+    // guard bands: the bulk-copy step kernel loads whole tiles "as if interior", so the first / last tiles of a
+    // population reach up to nx*ny + nx + 1 elements (+ one tile) outside it; those values are never used.
+    const size_t guard = align_up(((size_t)nx * ny + nx + 1 + MAX_TILE + 16) * rs, ALIGN);
+    size_t o = guard;
+    L.off_A = o; o += align_up((size_t)Q * L.stride * rs, ALIGN) + guard;
+    L.off_B = o; o += align_up((size_t)Q * L.stride * rs, ALIGN) + guard;
+    L.off_flags = o; o += align_up(N + MAX_TILE, ALIGN);
     L.off_mean = o; if (want_mean) o += align_up((size_t)3 * L.stride * rs, ALIGN);
     // scratch: heightmap (nx*ny int32) or a profile (3 nz doubles) or one face plane (3 n1 n2 doubles)
     const size_t plane = (size_t)std::max(std::max((size_t)nx * ny, (size_t)nx * nz), (size_t)ny * nz);
@@ -295,13 +300,52 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
     return check_launch(h, "step_kernel");
 }
 
-// kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes
-constexpr int N_VARIANTS = 8;
+// bulk-copy (TMA engine) persistent kernel: grid = CTAs that fit the device at once
+template <typename real, int T, int S, int MINB>
+int launch_tma_as(lbm_t *h, const Params<real> &P, bool sample)
+{
+    using C = TmaCfg<real, T>;
+    static_assert(T <= (int)MAX_TILE && T % 16 == 0, "tile size");
+    uint32_t tile_bytes = 0;
+    bool aligned = false;
+    const TmaTab tab = make_tma_tab<real>(P, T, &tile_bytes, &aligned);
+    const int ntiles = (int)((P.N + (long long)T - 1) / T);
+    const size_t smem = C::smem_bytes(S);
+    const real *A = (const real *)h->state();
+    real *B = (real *)h->other();
+    real *ms = (real *)h->mean();
+    // one-time set-up per kernel instantiation (the lambda's closure type, hence its statics, is unique per
+    // instantiation of launch_tma_as; `which` separates the four kernels launched from this one)
+    auto go = [&](auto kern, int which) -> int {
+        static int ctas_per_sm[4] = {0, 0, 0, 0}, sms = 0;
+        if (!ctas_per_sm[which]) {
+            CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            int dev = 0, n = 0;
+            CUDA_TRY(h, cudaGetDevice(&dev));
+            CUDA_TRY(h, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+            CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, T, smem));
+            if (n < 1) return fail(h, LBM_ECUDA, "step_tma_kernel does not fit an SM");
+            ctas_per_sm[which] = n;
+        }
+        const int grid = std::min(ntiles, ctas_per_sm[which] * sms);
+        kern<<<grid, T, smem, h->stream>>>(A, B, h->flags(), ms, P, tab, ntiles, tile_bytes);
+        return check_launch(h, "step_tma_kernel");
+    };
+    if (sample) return aligned ? go(step_tma_kernel<real, true, true, T, S, MINB>, 0) : go(step_tma_kernel<real, true, false, T, S, MINB>, 1);
+    return aligned ? go(step_tma_kernel<real, false, true, T, S, MINB>, 2) : go(step_tma_kernel<real, false, false, T, S, MINB>, 3);
+}
+
+// kernel variants (lbm_set_variant): same arithmetic, different kernels / cache hints / launch shapes.
+//   0      bulk-copy persistent kernel (FP32 default), T = 256, 4 stages, 2 CTAs per SM
+//   1..7   one-cell-per-thread LDG kernel (the FP64 path always uses it) with cache-hint / block-shape choices
+//   8..11  other tile / stage shapes of the bulk-copy kernel
+constexpr int N_VARIANTS = 12;
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
     if constexpr (std::is_same<real, float>::value) {
         switch (h->variant) {
+        case 0: return launch_tma_as<real, 256, 4, 2>(h, P, sample);
         case 1: return launch_step_as<real, 1, 256, 4>(h, P, sample);
         case 2: return launch_step_as<real, 2, 256, 4>(h, P, sample);
         case 3: return launch_step_as<real, 3, 256, 4>(h, P, sample);
@@ -309,10 +353,14 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         case 5: return launch_step_as<real, 0, 512, 2>(h, P, sample);
         case 6: return launch_step_as<real, 0, 256, 5>(h, P, sample);
         case 7: return launch_step_as<real, 0, 128, 12>(h, P, sample);
+        case 8: return launch_tma_as<real, 256, 3, 3>(h, P, sample);
+        case 9: return launch_tma_as<real, 128, 4, 5>(h, P, sample);
+        case 10: return launch_tma_as<real, 512, 4, 1>(h, P, sample);
+        case 11: return launch_tma_as<real, 256, 2, 4>(h, P, sample);
         default: break;
         }
     }
-    return launch_step_as<real, 0, 256, 4>(h, P, sample);
+    return launch_step_as<real, 1, 256, 4>(h, P, sample);
 }
 
 template <typename real>
