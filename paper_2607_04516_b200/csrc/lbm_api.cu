@@ -1,7 +1,9 @@
 // lbm_api.cu — context, launch layer and C ABI (include/lbm.h) of the B200-native LBM-LES path.
 #include "../../include/lbm.h"
-#include "lbm_kernels.cuh"
-#include "lbm_step_tma.cuh"
+#include "lbm_core.cuh"
+#include "lbm_setup.cuh"
+#include "lbm_step.cuh"
+#include "lbm_out.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -13,28 +15,29 @@ using namespace lbmk;
 namespace {
 
 constexpr size_t ALIGN = 256;
-constexpr size_t MAX_TILE = 1024; // largest tile (cells) of the bulk-copy step kernel
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Halo-padded box (lbm_core.cuh): x pitch = nx + 2 rounded up to 32, ny + 2 rows, nz + 2 planes.
 struct Layout {
-    long long stride;
-    size_t off_A, off_B, off_flags, off_mean, off_scratch, total;
+    int px, py;
+    long long Np, stride;
+    size_t off_A, off_B, off_flags, off_links, off_mean, off_scratch, total;
     size_t scratch_bytes;
 };
 
 Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
 {
     Layout L{};
-    const size_t N = (size_t)nx * ny * nz;
     const size_t rs = fp64 ? 8 : 4;
-    L.stride = (long long)align_up(N, 64);
-    // guard bands: the bulk-copy step kernel loads whole tiles "as if interior", so the first / last tiles of a
-    // population reach up to nx*ny + nx + 1 elements (+ one tile) outside it; those values are never used.
-    const size_t guard = align_up(((size_t)nx * ny + nx + 1 + MAX_TILE + 16) * rs, ALIGN);
-    size_t o = guard;
-    L.off_A = o; o += align_up((size_t)Q * L.stride * rs, ALIGN) + guard;
-    L.off_B = o; o += align_up((size_t)Q * L.stride * rs, ALIGN) + guard;
-    L.off_flags = o; o += align_up(N + MAX_TILE, ALIGN);
+    L.px = (nx + 2 + 31) / 32 * 32;
+    L.py = ny + 2;
+    L.Np = (long long)L.px * L.py * (nz + 2);
+    L.stride = (long long)align_up((size_t)L.Np, 64);
+    size_t o = 0;
+    L.off_A = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
+    L.off_B = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
+    L.off_flags = o; o += align_up((size_t)L.Np, ALIGN);
+    L.off_links = o; o += align_up((size_t)L.Np * sizeof(uint32_t), ALIGN);
     L.off_mean = o; if (want_mean) o += align_up((size_t)3 * L.stride * rs, ALIGN);
     // scratch: heightmap (nx*ny int32) or a profile (3 nz doubles) or one face plane (3 n1 n2 doubles)
     const size_t plane = (size_t)std::max(std::max((size_t)nx * ny, (size_t)nx * nz), (size_t)ny * nz);
@@ -42,6 +45,14 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
     L.off_scratch = o; o += L.scratch_bytes;
     L.total = o;
     return L;
+}
+
+// largest box: the padded cell count must fit a 32-bit int
+bool size_ok(int nx, int ny, int nz)
+{
+    if (nx < 1 || ny < 1 || nz < 1 || nz > 65535) return false;
+    const long long px = ((long long)nx + 2 + 31) / 32 * 32;
+    return px * ((long long)ny + 2) * ((long long)nz + 2) <= 2000000000LL;
 }
 
 } // namespace
@@ -68,6 +79,7 @@ struct lbm {
     void *state() const { return cur ? bufB() : bufA(); }
     void *other() const { return cur ? bufA() : bufB(); }
     uint8_t *flags() const { return (uint8_t *)(ws + L.off_flags); }
+    uint32_t *links() const { return (uint32_t *)(ws + L.off_links); }
     void *mean() const { return want_mean ? ws + L.off_mean : nullptr; }
     void *scratch() const { return ws + L.off_scratch; }
     long long N() const { return (long long)nx * ny * nz; }
@@ -92,8 +104,12 @@ template <typename real>
 Params<real> make_params(const lbm_t *h)
 {
     Params<real> P{};
-    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz; P.nxy = h->nx * h->ny;
+    P.nx = h->nx; P.ny = h->ny; P.nz = h->nz;
+    P.px = h->L.px; P.py = h->L.py; P.pxy = h->L.px * h->L.py;
+    P.Np = (int)h->L.Np;
     P.N = (int)h->N();
+    P.W = P.px / 32;
+    P.Wmagic = (unsigned)((0x100000000ULL + (unsigned)P.W - 1) / (unsigned)P.W);
     P.stride = h->L.stride;
     for (int k = 0; k < 6; ++k) P.face[k] = h->face[k];
     P.tau0 = (real)(3.0 * h->nu0 + 0.5);
@@ -198,11 +214,15 @@ int do_set_flags(lbm_t *h, const int32_t *height)
     int rc = stage_in(h, height, (size_t)h->nx * h->ny * sizeof(int32_t), 0, &in);
     if (rc) return rc;
     const int B = 256;
-    voxelise_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const int32_t *)in.dev, h->flags(), P);
+    voxelise_kernel<real><<<blocks_for(P.Np, B), B, 0, h->stream>>>((const int32_t *)in.dev, h->flags(), P);
     rc = check_launch(h, "voxelise_kernel");
     if (!rc) {
-        // in place: class bits are never changed by classify, only the SLOW bit is added
-        classify_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->flags(), h->flags(), nullptr, P);
+        rc = cudaMemsetAsync(h->links(), 0, (size_t)P.Np * sizeof(uint32_t), h->stream) == cudaSuccess ? LBM_OK
+             : fail(h, LBM_ECUDA, "memset links");
+    }
+    if (!rc) {
+        // in place: class bits are never changed by classify, only the SLOW / EDGE bits are added
+        classify_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->flags(), h->links(), P);
         rc = check_launch(h, "classify_kernel");
     }
     release_in(h, &in, 1);
@@ -279,7 +299,7 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     if (!rc) {
         const int B = 256;
         init_kernel<real, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (real *)h->bufA(), (real *)h->bufB(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+            (real *)h->bufA(), (real *)h->bufB(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
         rc = check_launch(h, "init_kernel");
     }
@@ -288,79 +308,41 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     return rc;
 }
 
-template <typename real, int HINT, int BLOCK, int MINB>
+template <typename real, int HINT, bool SPEC, int BLOCK, int MINB>
 int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
     const real *A = (const real *)h->state();
     real *B = (real *)h->other();
     real *ms = (real *)h->mean();
-    const unsigned grid = blocks_for(P.N, BLOCK);
-    if (sample) step_kernel<real, true, HINT, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), ms, P);
-    else step_kernel<real, false, HINT, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), ms, P);
+    constexpr int WPB = BLOCK / 32;
+    const dim3 grid(blocks_for((long long)P.W * P.ny, WPB), (unsigned)P.nz);
+    const StepPtrs<real> T = make_step_ptrs<real>(A, B, P);
+    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
+    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
     return check_launch(h, "step_kernel");
 }
 
-// bulk-copy (TMA engine) persistent kernel: grid = CTAs that fit the device at once
-template <typename real, int T, int S, int MINB>
-int launch_tma_as(lbm_t *h, const Params<real> &P, bool sample)
-{
-    using C = TmaCfg<real, T>;
-    static_assert(T <= (int)MAX_TILE && T % 16 == 0, "tile size");
-    uint32_t tile_bytes = 0;
-    bool aligned = false;
-    const TmaTab tab = make_tma_tab<real>(P, T, &tile_bytes, &aligned);
-    const int ntiles = (int)((P.N + (long long)T - 1) / T);
-    const size_t smem = C::smem_bytes(S);
-    const real *A = (const real *)h->state();
-    real *B = (real *)h->other();
-    real *ms = (real *)h->mean();
-    // one-time set-up per kernel instantiation (the lambda's closure type, hence its statics, is unique per
-    // instantiation of launch_tma_as; `which` separates the four kernels launched from this one)
-    auto go = [&](auto kern, int which) -> int {
-        static int ctas_per_sm[4] = {0, 0, 0, 0}, sms = 0;
-        if (!ctas_per_sm[which]) {
-            CUDA_TRY(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-            int dev = 0, n = 0;
-            CUDA_TRY(h, cudaGetDevice(&dev));
-            CUDA_TRY(h, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-            CUDA_TRY(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kern, T, smem));
-            if (n < 1) return fail(h, LBM_ECUDA, "step_tma_kernel does not fit an SM");
-            ctas_per_sm[which] = n;
-        }
-        const int grid = std::min(ntiles, ctas_per_sm[which] * sms);
-        kern<<<grid, T, smem, h->stream>>>(A, B, h->flags(), ms, P, tab, ntiles, tile_bytes);
-        return check_launch(h, "step_tma_kernel");
-    };
-    if (sample) return aligned ? go(step_tma_kernel<real, true, true, T, S, MINB>, 0) : go(step_tma_kernel<real, true, false, T, S, MINB>, 1);
-    return aligned ? go(step_tma_kernel<real, false, true, T, S, MINB>, 2) : go(step_tma_kernel<real, false, false, T, S, MINB>, 3);
-}
-
-// kernel variants (lbm_set_variant): same arithmetic, different kernels / cache hints / launch shapes.
-//   0      bulk-copy persistent kernel (FP32 default), T = 256, 4 stages, 2 CTAs per SM
-//   1..7   one-cell-per-thread LDG kernel (the FP64 path always uses it) with cache-hint / block-shape choices
-//   8..11  other tile / stage shapes of the bulk-copy kernel
-constexpr int N_VARIANTS = 12;
+// kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes / load issue order.
+constexpr int N_VARIANTS = 10;
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
     if constexpr (std::is_same<real, float>::value) {
         switch (h->variant) {
-        case 0: return launch_tma_as<real, 256, 4, 2>(h, P, sample);
-        case 1: return launch_step_as<real, 1, 256, 4>(h, P, sample);
-        case 2: return launch_step_as<real, 2, 256, 4>(h, P, sample);
-        case 3: return launch_step_as<real, 3, 256, 4>(h, P, sample);
-        case 4: return launch_step_as<real, 0, 128, 8>(h, P, sample);
-        case 5: return launch_step_as<real, 0, 512, 2>(h, P, sample);
-        case 6: return launch_step_as<real, 0, 256, 5>(h, P, sample);
-        case 7: return launch_step_as<real, 0, 128, 12>(h, P, sample);
-        case 8: return launch_tma_as<real, 256, 3, 3>(h, P, sample);
-        case 9: return launch_tma_as<real, 128, 4, 5>(h, P, sample);
-        case 10: return launch_tma_as<real, 512, 4, 1>(h, P, sample);
-        case 11: return launch_tma_as<real, 256, 2, 4>(h, P, sample);
+        case 0: return launch_step_as<real, 0, false, 256, 4>(h, P, sample);
+        case 1: return launch_step_as<real, 0, true, 256, 4>(h, P, sample);
+        case 2: return launch_step_as<real, 0, false, 128, 8>(h, P, sample);
+        case 3: return launch_step_as<real, 0, true, 128, 8>(h, P, sample);
+        case 4: return launch_step_as<real, 1, false, 256, 4>(h, P, sample);
+        case 5: return launch_step_as<real, 2, false, 256, 4>(h, P, sample);
+        case 6: return launch_step_as<real, 3, false, 256, 4>(h, P, sample);
+        case 7: return launch_step_as<real, 0, false, 512, 2>(h, P, sample);
+        case 8: return launch_step_as<real, 0, false, 64, 16>(h, P, sample);
+        case 9: return launch_step_as<real, 0, false, 256, 3>(h, P, sample);
         default: break;
         }
     }
-    return launch_step_as<real, 1, 256, 4>(h, P, sample);
+    return launch_step_as<real, 0, false, 256, 2>(h, P, sample);
 }
 
 template <typename real>
@@ -429,8 +411,8 @@ int do_get_links(lbm_t *h, uint32_t *links)
     int rc = stage_out(h, links, (size_t)P.N * sizeof(uint32_t), &o);
     if (rc) return rc;
     const int B = 256;
-    classify_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(nullptr, h->flags(), (uint32_t *)o.dev, P);
-    rc = check_launch(h, "classify_kernel");
+    links_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->links(), (uint32_t *)o.dev, P);
+    rc = check_launch(h, "links_out_kernel");
     int rc2 = finish_out(h, &o, 1);
     return rc ? rc : rc2;
 }
@@ -443,7 +425,7 @@ int do_get_state(lbm_t *h, double *f)
     int rc = stage_out(h, f, (size_t)Q * P.N * sizeof(double), &o);
     if (rc) return rc;
     const int B = 256;
-    state_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->state(), (double *)o.dev, P);
+    state_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->state(), h->flags(), (double *)o.dev, P);
     rc = check_launch(h, "state_out_kernel");
     int rc2 = finish_out(h, &o, 1);
     return rc ? rc : rc2;
@@ -457,7 +439,8 @@ int do_set_state(lbm_t *h, const double *f)
     int rc = stage_in(h, f, (size_t)Q * P.N * sizeof(double), h->L.scratch_bytes, &in);
     if (rc) return rc;
     const int B = 256;
-    state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (const double *)in.dev, P);
+    state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), h->flags(), h->links(),
+                                                                    (const double *)in.dev, P);
     rc = check_launch(h, "state_in_kernel");
     release_in(h, &in, 1);
     if (!rc) h->cur = 0;
@@ -482,8 +465,7 @@ extern "C" {
 
 int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int fp64, size_t *out)
 {
-    if (!out || nx < 1 || ny < 1 || nz < 1) return LBM_EINVAL;
-    if ((long long)nx * ny * nz > 2000000000LL) return LBM_EINVAL;
+    if (!out || !size_ok(nx, ny, nz)) return LBM_EINVAL;
     *out = make_layout(nx, ny, nz, want_mean, fp64).total;
     return LBM_OK;
 }
@@ -493,7 +475,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
 {
     if (!out) return LBM_EINVAL;
     *out = nullptr;
-    if (nx < 1 || ny < 1 || nz < 1 || (long long)nx * ny * nz > 2000000000LL) return LBM_EINVAL;
+    if (!size_ok(nx, ny, nz)) return LBM_EINVAL;
     if (!(nu0 > 0.0) || Cs < 0.0 || !std::isfinite(nu0) || !std::isfinite(Cs) || !std::isfinite(f_cor)) return LBM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return LBM_ECUDA; }
@@ -642,7 +624,8 @@ int lbm_get_flags(lbm_t *h, uint8_t *flags)
     int rc = stage_out(h, flags, (size_t)h->N(), &o);
     if (rc) return rc;
     const int B = 256;
-    flags_out_kernel<<<blocks_for(h->N(), B), B, 0, h->stream>>>(h->flags(), (uint8_t *)o.dev, (int)h->N());
+    const Params<float> P = make_params<float>(h);
+    flags_out_kernel<float><<<blocks_for(h->N(), B), B, 0, h->stream>>>(h->flags(), (uint8_t *)o.dev, P);
     rc = check_launch(h, "flags_out_kernel");
     int rc2 = finish_out(h, &o, 1);
     return rc ? rc : rc2;
@@ -660,6 +643,7 @@ int lbm_get_state(lbm_t *h, double *f)
 {
     if (!h) return LBM_EINVAL;
     if (!f) return fail(h, LBM_EINVAL, "get_state: NULL");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_state: flags not set");
     return h->fp64 ? do_get_state<double>(h, f) : do_get_state<float>(h, f);
 }
 

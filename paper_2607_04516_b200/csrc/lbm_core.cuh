@@ -1,0 +1,327 @@
+// lbm_core.cuh — lattice, layout, per-cell arithmetic and the write-side boundary rule of the D3Q19 LBM-LES path
+// (sm_100a).  Algorithm statement: DESIGN.md §3 (restating PAPER.md:61, Table 1).
+//
+// Storage.  Populations SoA g[i][Z][Y][X] on a HALO-PADDED box: one halo layer on every side, x pitch rounded up
+// to 32 cells (a warp never straddles a row; every row is 128-byte aligned).  g_i = f_i - w_i ("shifted": the rest
+// state is exactly 0, stored numbers are O(Ma), FP32 rounding stays two orders below the 1e-5 parity bar).
+// Two buffers A/B, pull scheme: every FLUID cell reads A[i][p - off_i] for ALL i with no case distinction.
+//
+// What makes that possible is a write-side boundary rule ("mailboxes").  A population j that leaves cell x
+// towards a cell that cannot be pulled from is stored, by x itself, where the pull of the next step will look:
+//   * target is SOLID (building, WALL face, or halo whose image is solid): slot (opp(j), x + c_j) <- g_j
+//     — halfway bounce-back: next step x pulls opp(j) from x - c_opp(j) = x + c_j  (DESIGN.md §3 step 4a);
+//   * target is a GHOST halo cell of a FREE_SLIP face: slot (flip(j), x with the out axes stepped into the halo)
+//     <- g_j — specular reflection; of a PERIODIC face: slot (j, x with the out axes moved to the far halo) <- g_j.
+// Every halo slot has exactly one writer, so there is no race; SOLID cells never run, so their slots are free.
+#pragma once
+#include <cstdint>
+#include <type_traits>
+#include <cuda_runtime.h>
+
+namespace lbmk {
+
+constexpr int Q = 19;
+// cell classes (3 bits).  GHOST exists only in the halo.
+enum : int { FLUID = 0, SOLID = 1, EQ_FIXED = 2, EQ_OUTFLOW = 3, GHOST = 4 };
+enum : int { PERIODIC = 0, WALL = 1, FREE_SLIP = 2, FACE_EQ_FIXED = 3, FACE_EQ_OUTFLOW = 4 };
+constexpr uint8_t CLASS_MASK = 7;
+constexpr uint8_t SLOW_BIT = 0x80; // FLUID cell with at least one wall link (mailbox stores needed)
+constexpr uint8_t EDGE_BIT = 0x40; // non-solid cell on a domain face (ghost stores may be needed)
+
+// ---- lattice (DESIGN.md §3 step 1): pair k = 1..9 holds directions 2k-1 (+) and 2k (-) -------------------------
+// pair vectors: 1:(1,0,0) 2:(0,1,0) 3:(0,0,1) 4:(1,1,0) 5:(1,0,1) 6:(0,1,1) 7:(1,-1,0) 8:(1,0,-1) 9:(0,1,-1)
+__host__ __device__ constexpr int pair_cx(int k) { return (k == 1 || k == 4 || k == 5 || k == 7 || k == 8) ? 1 : 0; }
+__host__ __device__ constexpr int pair_cy(int k) { return (k == 2 || k == 4 || k == 6 || k == 9) ? 1 : (k == 7 ? -1 : 0); }
+__host__ __device__ constexpr int pair_cz(int k) { return (k == 3 || k == 5 || k == 6) ? 1 : ((k == 8 || k == 9) ? -1 : 0); }
+__host__ __device__ constexpr int dir_cx(int i) { return i == 0 ? 0 : ((i & 1) ? pair_cx((i + 1) / 2) : -pair_cx(i / 2)); }
+__host__ __device__ constexpr int dir_cy(int i) { return i == 0 ? 0 : ((i & 1) ? pair_cy((i + 1) / 2) : -pair_cy(i / 2)); }
+__host__ __device__ constexpr int dir_cz(int i) { return i == 0 ? 0 : ((i & 1) ? pair_cz((i + 1) / 2) : -pair_cz(i / 2)); }
+__host__ __device__ constexpr int dir_opp(int i) { return i == 0 ? 0 : ((i & 1) ? i + 1 : i - 1); }
+__host__ __device__ constexpr int dir_find(int cx, int cy, int cz)
+{
+    for (int i = 0; i < Q; ++i)
+        if (dir_cx(i) == cx && dir_cy(i) == cy && dir_cz(i) == cz) return i;
+    return -1;
+}
+
+template <int B, int E, class F>
+__host__ __device__ __forceinline__ void static_for(F &&f)
+{
+    if constexpr (B < E) {
+        f(std::integral_constant<int, B>{});
+        static_for<B + 1, E>(f);
+    }
+}
+
+// ---- parameters and layout ---------------------------------------------------------------------------------------
+template <typename real>
+struct Params {
+    int nx, ny, nz;   // interior cells
+    int px, py, pxy;  // padded x pitch (multiple of 32, >= nx + 2), padded rows per plane (ny + 2), px * py
+    int Np;           // padded cells = pxy * (nz + 2)
+    int N;            // interior cells
+    int W;            // warps per padded row = px / 32
+    unsigned Wmagic;  // ceil(2^32 / W): q = umulhi(n, Wmagic) == n / W for n < 2^32 / W
+    long long stride; // elements between consecutive populations (>= Np, multiple of 64)
+    int face[6];
+    real tau0, Kles;       // Kles = 18 sqrt(2) Cs^2
+    real fcor, h, inv1ph2; // h = fcor/2, 1/(1+h^2)
+    real Fx, Fy, Fz;
+};
+
+// padded linear index of interior cell (x,y,z); also valid for halo coordinates -1 and n
+template <typename real>
+__host__ __device__ __forceinline__ int pidx(const Params<real> &P, int x, int y, int z)
+{
+    return ((z + 1) * P.py + (y + 1)) * P.px + (x + 1);
+}
+// offset (in cells) of the pull source of direction i relative to the cell: source = p - poff
+template <int I, typename real>
+__host__ __device__ __forceinline__ int poff(const Params<real> &P)
+{
+    return dir_cx(I) + dir_cy(I) * P.px + dir_cz(I) * P.pxy;
+}
+
+// c . a for a lattice vector known at compile time: only the non-zero components are touched (no 0 * x terms,
+// which IEEE arithmetic may not fold away)
+template <int CX, int CY, int CZ, typename real>
+__device__ __forceinline__ real cdot(real ax, real ay, real az)
+{
+    static_assert(CX != 0 || CY != 0 || CZ != 0, "zero vector");
+    if constexpr (CX != 0 && CY == 0 && CZ == 0) return CX > 0 ? ax : -ax;
+    else if constexpr (CX == 0 && CY != 0 && CZ == 0) return CY > 0 ? ay : -ay;
+    else if constexpr (CX == 0 && CY == 0 && CZ != 0) return CZ > 0 ? az : -az;
+    else if constexpr (CZ == 0) return (CX > 0) ? (CY > 0 ? ax + ay : ax - ay) : (CY > 0 ? ay - ax : -ax - ay);
+    else if constexpr (CY == 0) return (CX > 0) ? (CZ > 0 ? ax + az : ax - az) : (CZ > 0 ? az - ax : -ax - az);
+    else return (CY > 0) ? (CZ > 0 ? ay + az : ay - az) : (CZ > 0 ? az - ay : -ay - az);
+}
+
+template <typename real>
+struct Macro { real rho, ux, uy, uz; };
+
+// ---- collision (DESIGN.md §3 steps 4b-4e) on shifted populations ---------------------------------------------------
+// In: pulled g[19].  Out: post-collision g[19]; returns the (rho,u) the collision used.
+template <typename real>
+__device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> &P)
+{
+    real s[10], d[10];
+#pragma unroll
+    for (int k = 1; k <= 9; ++k) { s[k] = g[2 * k - 1] + g[2 * k]; d[k] = g[2 * k - 1] - g[2 * k]; }
+    // 4b: moments of the shifted populations (sum_i w_i = 1, sum_i w_i c_i = 0 drop out exactly)
+    const real drho = g[0] + (((s[1] + s[2]) + (s[3] + s[4])) + ((s[5] + s[6]) + (s[7] + s[8])) + s[9]);
+    const real mx = (d[1] + d[4]) + (d[5] + d[7]) + d[8];
+    const real my = (d[2] + d[4]) + (d[6] - d[7]) + d[9];
+    const real mz = (d[3] + d[5]) + (d[6] - d[8]) - d[9];
+    const real Mxx = (s[1] + s[4]) + (s[5] + s[7]) + s[8];
+    const real Myy = (s[2] + s[4]) + (s[6] + s[7]) + s[9];
+    const real Mzz = (s[3] + s[5]) + (s[6] + s[8]) + s[9];
+    const real Mxy = s[4] - s[7], Mxz = s[5] - s[8], Myz = s[6] - s[9];
+    const real rho = real(1) + drho;
+    const real inv = real(1) / rho;
+    // 4c: implicit half-force velocity
+    const real bx = mx * inv + real(0.5) * P.Fx, by = my * inv + real(0.5) * P.Fy, bz = mz * inv + real(0.5) * P.Fz;
+    const real ux = (bx + P.h * by) * P.inv1ph2;
+    const real uy = (by - P.h * bx) * P.inv1ph2;
+    const real uz = bz;
+    const real Fdx = rho * (P.Fx + P.fcor * uy), Fdy = rho * (P.Fy - P.fcor * ux), Fdz = rho * P.Fz;
+    // 4d: Pi = sum c c (f - feq) = M - (drho/3) I - rho u u   (second moment of the shifted equilibrium is exact)
+    const real third = real(1) / real(3);
+    const real Pxx = Mxx - third * drho - rho * ux * ux;
+    const real Pyy = Myy - third * drho - rho * uy * uy;
+    const real Pzz = Mzz - third * drho - rho * uz * uz;
+    const real Pxy = Mxy - rho * ux * uy, Pxz = Mxz - rho * ux * uz, Pyz = Myz - rho * uy * uz;
+    const real Qn = sqrt(Pxx * Pxx + Pyy * Pyy + Pzz * Pzz + real(2) * (Pxy * Pxy + Pxz * Pxz + Pyz * Pyz));
+    const real tau = real(0.5) * (P.tau0 + sqrt(P.tau0 * P.tau0 + P.Kles * Qn * inv));
+    const real omega = real(1) / tau;
+    const real phi = real(1) - real(0.5) * omega;
+    // 4e: BGK + Guo source.  With base = omega A0 - 3 phi uF, P1 = omega rho u, P2 = phi Fd and, per weight group,
+    //   E0 = w base,  v = w (4.5 P1 + 9 P2),  o = 3 w (P1 + P2):
+    //   even_k = E0 + (c_k.u)(c_k.v),  odd_k = c_k.o,  g'_{k+-} = (1 - omega) g_{k+-} + even_k +- odd_k
+    // which is the expansion of  g - omega (g - g_eq) + (1 - omega/2) w [3 (c - u).Fd + 9 (c.u)(c.Fd)]  pair by pair.
+    const real uF = ux * Fdx + uy * Fdy + uz * Fdz;
+    const real A0 = drho - real(1.5) * rho * (ux * ux + uy * uy + uz * uz);
+    const real keep = real(1) - omega;
+    const real base = omega * A0 - real(3) * phi * uF;
+    const real orho = omega * rho;
+    const real P1x = orho * ux, P1y = orho * uy, P1z = orho * uz;
+    const real P2x = phi * Fdx, P2y = phi * Fdy, P2z = phi * Fdz;
+    g[0] = keep * g[0] + third * base;
+    // group a: w = 1/18 (axis pairs 1..3); group b: w = 1/36 (diagonal pairs 4..9) = half of group a
+    const real E0a = base * (real(1) / real(18)), E0b = base * (real(1) / real(36));
+    const real vax = real(0.25) * P1x + real(0.5) * P2x, vay = real(0.25) * P1y + real(0.5) * P2y, vaz = real(0.25) * P1z + real(0.5) * P2z;
+    const real oax = (P1x + P2x) * (real(1) / real(6)), oay = (P1y + P2y) * (real(1) / real(6)), oaz = (P1z + P2z) * (real(1) / real(6));
+    const real vbx = real(0.5) * vax, vby = real(0.5) * vay, vbz = real(0.5) * vaz;
+    const real obx = real(0.5) * oax, oby = real(0.5) * oay, obz = real(0.5) * oaz;
+    static_for<1, 10>([&](auto kc) {
+        constexpr int k = decltype(kc)::value;
+        constexpr int cx = pair_cx(k), cy = pair_cy(k), cz = pair_cz(k);
+        const real E0 = (k <= 3) ? E0a : E0b;
+        const real vx = (k <= 3) ? vax : vbx, vy = (k <= 3) ? vay : vby, vz = (k <= 3) ? vaz : vbz;
+        const real ox = (k <= 3) ? oax : obx, oy = (k <= 3) ? oay : oby, oz = (k <= 3) ? oaz : obz;
+        const real cu = cdot<cx, cy, cz>(ux, uy, uz);
+        const real cv = cdot<cx, cy, cz>(vx, vy, vz);
+        const real co = cdot<cx, cy, cz>(ox, oy, oz);
+        const real even = E0 + cu * cv;
+        g[2 * k - 1] = keep * g[2 * k - 1] + (even + co);
+        g[2 * k] = keep * g[2 * k] + (even - co);
+    });
+    return Macro<real>{rho, ux, uy, uz};
+}
+
+// shifted equilibrium: g_eq,i = w_i (drho + rho (3 cu + 4.5 cu^2 - 1.5 u^2))
+template <typename real>
+__device__ __forceinline__ void equilibrium(real (&g)[Q], real drho, real ux, real uy, real uz)
+{
+    const real rho = real(1) + drho;
+    const real A0 = drho - real(1.5) * rho * (ux * ux + uy * uy + uz * uz);
+    g[0] = (real(1) / real(3)) * A0;
+    static_for<1, 10>([&](auto kc) {
+        constexpr int k = decltype(kc)::value;
+        constexpr int cx = pair_cx(k), cy = pair_cy(k), cz = pair_cz(k);
+        const real w = (k <= 3) ? real(1) / real(18) : real(1) / real(36);
+        const real cu = cdot<cx, cy, cz>(ux, uy, uz);
+        const real even = w * (A0 + real(4.5) * rho * cu * cu);
+        const real odd = w * real(3) * rho * cu;
+        g[2 * k - 1] = even + odd;
+        g[2 * k] = even - odd;
+    });
+}
+
+// local macros of a stored (post-collision) state (DESIGN.md §3 step 7)
+template <typename real>
+__device__ __forceinline__ Macro<real> local_macros(const real (&g)[Q], int cls, const Params<real> &P)
+{
+    if (cls == SOLID || cls == GHOST) return Macro<real>{real(1), real(0), real(0), real(0)};
+    real s[10], d[10];
+#pragma unroll
+    for (int k = 1; k <= 9; ++k) { s[k] = g[2 * k - 1] + g[2 * k]; d[k] = g[2 * k - 1] - g[2 * k]; }
+    const real drho = g[0] + (((s[1] + s[2]) + (s[3] + s[4])) + ((s[5] + s[6]) + (s[7] + s[8])) + s[9]);
+    const real mx = (d[1] + d[4]) + (d[5] + d[7]) + d[8];
+    const real my = (d[2] + d[4]) + (d[6] - d[7]) + d[9];
+    const real mz = (d[3] + d[5]) + (d[6] - d[8]) - d[9];
+    const real rho = real(1) + drho;
+    const real inv = real(1) / rho;
+    if (cls == FLUID) {
+        const real bx = mx * inv - real(0.5) * P.Fx, by = my * inv - real(0.5) * P.Fy, bz = mz * inv - real(0.5) * P.Fz;
+        return Macro<real>{rho, (bx - P.h * by) * P.inv1ph2, (by + P.h * bx) * P.inv1ph2, bz};
+    }
+    return Macro<real>{rho, mx * inv, my * inv, mz * inv};
+}
+
+template <typename real>
+__device__ __forceinline__ void load_cell(real (&g)[Q], const real *__restrict__ A, long long stride, int p)
+{
+#pragma unroll
+    for (int i = 0; i < Q; ++i) g[i] = A[(long long)i * stride + p];
+}
+
+// ---- the write-side boundary rule ------------------------------------------------------------------------------------
+// st(i, pt, jc): "slot (direction i, padded cell pt) <- g[jc]" with jc an integral_constant (register indexing).
+// Wall links: bit i of lk set <=> the pull source of direction i is SOLID <=> population opp(i) leaves towards it.
+template <typename real, class St>
+__device__ __forceinline__ void wall_stores(const Params<real> &P, int p, uint32_t lk, St &&st)
+{
+    static_for<1, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        if ((lk >> i) & 1u) st(i, p - poff<i>(P), std::integral_constant<int, dir_opp(i)>{});
+    });
+}
+
+// Ghost slots of a non-solid cell (x,y,z) on a domain face: for every direction j that leaves the box, unless it is
+// a wall link (then wall_stores owns it) or an out axis is a WALL / EQ face (nobody pulls from there).
+template <typename real, class St>
+__device__ __forceinline__ void ghost_stores(const Params<real> &P, int x, int y, int z, uint32_t lk, St &&st)
+{
+    static_for<1, Q>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
+        constexpr int cx = dir_cx(j), cy = dir_cy(j), cz = dir_cz(j);
+        bool out = false, ok = true, fx = false, fy = false, fz = false;
+        int hx = x, hy = y, hz = z;
+        if constexpr (cx != 0) {
+            const bool lo = x + cx < 0, hi = x + cx >= P.nx;
+            if (lo | hi) {
+                out = true;
+                const int ft = lo ? P.face[0] : P.face[1];
+                if (ft == PERIODIC) hx = x - cx * P.nx;
+                else if (ft == FREE_SLIP) { hx = x + cx; fx = true; }
+                else ok = false;
+            }
+        }
+        if constexpr (cy != 0) {
+            const bool lo = y + cy < 0, hi = y + cy >= P.ny;
+            if (lo | hi) {
+                out = true;
+                const int ft = lo ? P.face[2] : P.face[3];
+                if (ft == PERIODIC) hy = y - cy * P.ny;
+                else if (ft == FREE_SLIP) { hy = y + cy; fy = true; }
+                else ok = false;
+            }
+        }
+        if constexpr (cz != 0) {
+            const bool lo = z + cz < 0, hi = z + cz >= P.nz;
+            if (lo | hi) {
+                out = true;
+                const int ft = lo ? P.face[4] : P.face[5];
+                if (ft == PERIODIC) hz = z - cz * P.nz;
+                else if (ft == FREE_SLIP) { hz = z + cz; fz = true; }
+                else ok = false;
+            }
+        }
+        if (out && ok && !((lk >> dir_opp(j)) & 1u)) {
+            // reflected direction: a compile-time candidate per flip combination
+            const int key = (fx ? 1 : 0) | (fy ? 2 : 0) | (fz ? 4 : 0);
+            int i = j;
+            static_for<1, 8>([&](auto kc) {
+                constexpr int kk = decltype(kc)::value;
+                constexpr bool possible = !((kk & 1) && cx == 0) && !((kk & 2) && cy == 0) && !((kk & 4) && cz == 0);
+                if constexpr (possible) {
+                    constexpr int cand = dir_find((kk & 1) ? -cx : cx, (kk & 2) ? -cy : cy, (kk & 4) ? -cz : cz);
+                    if (key == kk) i = cand;
+                }
+            });
+            st(i, pidx(P, hx, hy, hz), jc);
+        }
+    });
+}
+
+// All stores of one cell's post-collision state into buffer B: own 19 slots, wall mailboxes, ghost slots.
+template <typename real>
+__device__ __forceinline__ void store_cell(real *__restrict__ B, const Params<real> &P, int p, int x, int y, int z, uint8_t fl,
+                                           uint32_t lk, const real (&g)[Q])
+{
+#pragma unroll
+    for (int i = 0; i < Q; ++i) B[(long long)i * P.stride + p] = g[i];
+    if (fl & (SLOW_BIT | EDGE_BIT)) {
+        auto st = [&](int i, int pt, auto jc) { B[(long long)i * P.stride + pt] = g[decltype(jc)::value]; };
+        if (fl & SLOW_BIT) wall_stores(P, p, lk, st);
+        if (fl & EDGE_BIT) ghost_stores(P, x, y, z, lk, st);
+    }
+}
+
+// which face's normal an EQ_OUTFLOW cell uses: first EQ_OUTFLOW face it lies on, order x-,x+,y-,y+,z-,z+.
+// Returns the padded index of the inward neighbour, -1 if the box is one cell thick on that axis.
+template <typename real>
+__device__ __forceinline__ int outflow_neighbour(const Params<real> &P, int x, int y, int z)
+{
+    if (x == 0 && P.face[0] == FACE_EQ_OUTFLOW) return (P.nx > 1) ? pidx(P, 1, y, z) : -1;
+    if (x == P.nx - 1 && P.face[1] == FACE_EQ_OUTFLOW) return (P.nx > 1) ? pidx(P, x - 1, y, z) : -1;
+    if (y == 0 && P.face[2] == FACE_EQ_OUTFLOW) return (P.ny > 1) ? pidx(P, x, 1, z) : -1;
+    if (y == P.ny - 1 && P.face[3] == FACE_EQ_OUTFLOW) return (P.ny > 1) ? pidx(P, x, y - 1, z) : -1;
+    if (z == 0 && P.face[4] == FACE_EQ_OUTFLOW) return (P.nz > 1) ? pidx(P, x, y, 1) : -1;
+    if (z == P.nz - 1 && P.face[5] == FACE_EQ_OUTFLOW) return (P.nz > 1) ? pidx(P, x, y, z - 1) : -1;
+    return -1;
+}
+
+// interior cell c = (z*ny + y)*nx + x  ->  coordinates (set-up and output kernels; not on the hot path)
+template <typename real>
+__device__ __forceinline__ void cell_xyz(const Params<real> &P, int c, int &x, int &y, int &z)
+{
+    x = c % P.nx;
+    const int r = c / P.nx;
+    y = r % P.ny;
+    z = r / P.ny;
+}
+
+__host__ __device__ inline double weight_f64(int i) { return i == 0 ? 1.0 / 3.0 : (i <= 6 ? 1.0 / 18.0 : 1.0 / 36.0); }
+
+} // namespace lbmk

@@ -1,0 +1,85 @@
+// lbm_out.cuh — a7: macroscopic fields and time means of the stored state, and the parity exports.
+// Outputs are un-padded C-order [nz][ny][nx] arrays; the internal state is halo-padded (lbm_core.cuh).
+#pragma once
+#include "lbm_core.cuh"
+
+namespace lbmk {
+
+// local macros of the stored state (DESIGN.md §3 step 7)
+template <typename real, typename out_t>
+__global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
+                              out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const int cls = flags[p] & CLASS_MASK;
+    real g[Q];
+    Macro<real> m{real(1), real(0), real(0), real(0)};
+    if (cls != SOLID) {
+        load_cell(g, A, P.stride, p);
+        m = local_macros(g, cls, P);
+    }
+    if (rho) rho[c] = out_t(m.rho);
+    if (ux) ux[c] = out_t(m.ux);
+    if (uy) uy[c] = out_t(m.uy);
+    if (uz) uz[c] = out_t(m.uz);
+}
+
+// standalone sample (a sample due at a step the fused kernel did not produce, e.g. step 0); DESIGN.md §3 step 8
+template <typename real>
+__global__ void mean_sample_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, real *__restrict__ msum, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const int cls = flags[p] & CLASS_MASK;
+    if (cls == SOLID) return;
+    real g[Q];
+    load_cell(g, A, P.stride, p);
+    const Macro<real> m = local_macros(g, cls, P);
+    msum[p] += m.ux;
+    msum[P.stride + p] += m.uy;
+    msum[2 * P.stride + p] += m.uz;
+}
+
+template <typename real, typename out_t>
+__global__ void mean_out_kernel(const real *__restrict__ msum, out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz,
+                                double inv_count, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    if (ux) ux[c] = out_t(double(msum[p]) * inv_count);
+    if (uy) uy[c] = out_t(double(msum[P.stride + p]) * inv_count);
+    if (uz) uz[c] = out_t(double(msum[2 * P.stride + p]) * inv_count);
+}
+
+// class bits only (SLOW / EDGE bits are internal)
+template <typename real>
+__global__ void flags_out_kernel(const uint8_t *__restrict__ flags, uint8_t *__restrict__ out, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    out[c] = flags[pidx(P, x, y, z)] & CLASS_MASK;
+}
+
+template <typename real>
+__global__ void links_out_kernel(const uint32_t *__restrict__ links, uint32_t *__restrict__ out, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    out[c] = links[pidx(P, x, y, z)];
+}
+
+} // namespace lbmk

@@ -1,0 +1,196 @@
+// lbm_setup.cuh — one-off kernels: voxelise (a1), link classification (a2), inlet write (a3), init (a4), precursor feed
+// (a8), checkpoint in/out.  Rows of SURVEY.md §8(a); arithmetic of DESIGN.md §3.  Layout: lbm_core.cuh.
+#pragma once
+#include "lbm_core.cuh"
+
+namespace lbmk {
+
+// ---- a1: voxelise the padded box ---------------------------------------------------------------------------------------
+// Interior: SOLID iff z < clamp(h[y][x], 0, nz); non-solid cells on an EQ face take the EQ class (EQ_FIXED wins).
+// Halo: SOLID behind a WALL or EQ face (never pulled from / bounce-back), else the class follows the in-box image
+// cell (PERIODIC: wrapped, FREE_SLIP: clamped): image solid -> SOLID (DESIGN.md §3 step 4a "mirrored source SOLID ->
+// bounce-back"), else GHOST.  x padding beyond the halo: SOLID.
+template <typename real>
+__global__ void voxelise_kernel(const int32_t *__restrict__ height, uint8_t *__restrict__ flags, Params<real> P)
+{
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= P.Np) return;
+    int x = p % P.px - 1, y = (p / P.px) % P.py - 1, z = p / P.pxy - 1;
+    if (x > P.nx) { flags[p] = SOLID; return; }
+    const int n[3] = {P.nx, P.ny, P.nz};
+    int c[3] = {x, y, z};
+    bool halo = false, dead = false;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const bool lo = c[a] < 0, hi = c[a] >= n[a];
+        if (lo | hi) {
+            halo = true;
+            const int ft = lo ? P.face[2 * a] : P.face[2 * a + 1];
+            if (ft == PERIODIC) c[a] = lo ? n[a] - 1 : 0;
+            else if (ft == FREE_SLIP) c[a] = lo ? 0 : n[a] - 1;
+            else dead = true;
+        }
+    }
+    if (dead) { flags[p] = SOLID; return; }
+    int h = height ? height[c[1] * P.nx + c[0]] : 0;
+    h = min(max(h, 0), P.nz);
+    int cls;
+    if (c[2] < h) cls = SOLID;
+    else if (halo) cls = GHOST;
+    else {
+        const bool on[6] = {x == 0, x == P.nx - 1, y == 0, y == P.ny - 1, z == 0, z == P.nz - 1};
+        bool fixed = false, outflow = false;
+#pragma unroll
+        for (int k = 0; k < 6; ++k) {
+            fixed |= on[k] && P.face[k] == FACE_EQ_FIXED;
+            outflow |= on[k] && P.face[k] == FACE_EQ_OUTFLOW;
+        }
+        cls = fixed ? EQ_FIXED : (outflow ? EQ_OUTFLOW : FLUID);
+    }
+    flags[p] = (uint8_t)cls;
+}
+
+// ---- a2: link classification ---------------------------------------------------------------------------------------------
+// Bit i (1..18) of links[p] <=> the pull source of direction i of FLUID cell p is SOLID in the padded box — exactly
+// "step 4a takes the bounce-back branch" (DESIGN.md §3 step 9).  Adds SLOW_BIT / EDGE_BIT to the flag byte in place
+// (class bits are never changed, and readers mask them, so in-place is race-free).
+template <typename real>
+__global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restrict__ links, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const int cls = flags[p] & CLASS_MASK;
+    uint32_t bits = 0;
+    if (cls == FLUID) {
+        static_for<1, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            bits |= (((flags[p - poff<i>(P)] & CLASS_MASK) == SOLID) ? 1u : 0u) << i;
+        });
+    }
+    links[p] = bits;
+    const bool edge = x == 0 || x == P.nx - 1 || y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
+    flags[p] = (uint8_t)(cls | (bits ? SLOW_BIT : 0) | ((cls != SOLID && edge) ? EDGE_BIT : 0));
+}
+
+// store one cell's state into BOTH buffers (set-up paths: the two buffers start identical)
+template <typename real>
+__device__ __forceinline__ void store_cell_both(real *__restrict__ A, real *__restrict__ B, const Params<real> &P, int p, int x, int y,
+                                                int z, uint8_t fl, uint32_t lk, const real (&g)[Q])
+{
+    store_cell(A, P, p, x, y, z, fl, lk, g);
+    store_cell(B, P, p, x, y, z, fl, lk, g);
+}
+
+// ---- a3: inlet write -------------------------------------------------------------------------------------------------
+// mode 0: profile prof[nz] per component by level; mode 1: plane uvw[3][n2][n1] of one face
+template <typename real, typename in_t>
+__global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+                             const in_t *__restrict__ pu, const in_t *__restrict__ pv, const in_t *__restrict__ pw,
+                             int mode, int face, Params<real> P)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    int x, y, z;
+    long long src;
+    if (mode == 0) {
+        if (t >= P.N) return;
+        cell_xyz(P, t, x, y, z);
+        src = z;
+    } else {
+        const int axis = face >> 1;
+        const int n1 = axis == 0 ? P.ny : P.nx;
+        const int n2 = axis == 2 ? P.ny : P.nz;
+        if (t >= n1 * n2) return;
+        const int j1 = t % n1, j2 = t / n1;
+        const int nn[3] = {P.nx, P.ny, P.nz};
+        const int fixed = (face & 1) ? nn[axis] - 1 : 0;
+        if (axis == 0) { x = fixed; y = j1; z = j2; }
+        else if (axis == 1) { x = j1; y = fixed; z = j2; }
+        else { x = j1; y = j2; z = fixed; }
+        src = t;
+    }
+    const int p = pidx(P, x, y, z);
+    const uint8_t fl = flags[p];
+    if ((fl & CLASS_MASK) != EQ_FIXED) return;
+    const real ux = real(pu[src]), uy = pv ? real(pv[src]) : real(0), uz = pw ? real(pw[src]) : real(0);
+    real g[Q];
+    equilibrium(g, real(0), ux, uy, uz);
+    store_cell_both(A, B, P, p, x, y, z, fl, 0u, g);
+}
+
+// ---- a8: precursor plane -> main inlet (config 5) -----------------------------------------------------------------------
+template <typename real>
+__global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, const uint8_t *__restrict__ dflags, Params<real> D,
+                            const real *__restrict__ sA, const uint8_t *__restrict__ sflags, Params<real> S, int sx)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= D.ny * D.nz) return;
+    const int y = t % D.ny, z = t / D.ny;
+    const int dp = pidx(D, 0, y, z);
+    const uint8_t fl = dflags[dp];
+    if ((fl & CLASS_MASK) != EQ_FIXED) return;
+    const int sp = pidx(S, sx, y % S.ny, z);
+    real g[Q];
+    load_cell(g, sA, S.stride, sp);
+    const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, S);
+    equilibrium(g, real(0), m.ux, m.uy, m.uz);
+    store_cell_both(dA, dB, D, dp, 0, y, z, fl, 0u, g);
+}
+
+// ---- a4: init ------------------------------------------------------------------------------------------------------------
+// G0 = f_eq(rho0, u0) in FLUID and EQ_OUTFLOW cells (EQ_FIXED keep their boundary state; SOLID cells hold mailboxes)
+template <typename real, typename in_t>
+__global__ void init_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+                            const uint32_t *__restrict__ links, const in_t *__restrict__ rho, const in_t *__restrict__ ux,
+                            const in_t *__restrict__ uy, const in_t *__restrict__ uz, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const uint8_t fl = flags[p];
+    const int cls = fl & CLASS_MASK;
+    if (cls == EQ_FIXED || cls == SOLID) return;
+    const real drho = rho ? real(rho[c] - in_t(1)) : real(0);
+    const real u = ux ? real(ux[c]) : real(0), v = uy ? real(uy[c]) : real(0), w = uz ? real(uz[c]) : real(0);
+    real g[Q];
+    equilibrium(g, drho, u, v, w);
+    store_cell_both(A, B, P, p, x, y, z, fl, links[p], g);
+}
+
+// ---- checkpoint ------------------------------------------------------------------------------------------------------------
+// f [19][nz][ny][nx] double, NOT shifted.  SOLID cells export the rest state w_i (their slots are mailboxes).
+template <typename real>
+__global__ void state_out_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, double *__restrict__ f, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const bool solid = (flags[p] & CLASS_MASK) == SOLID;
+#pragma unroll
+    for (int i = 0; i < Q; ++i) f[(long long)i * P.N + c] = (solid ? 0.0 : double(A[(long long)i * P.stride + p])) + weight_f64(i);
+}
+
+template <typename real>
+__global__ void state_in_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+                                const uint32_t *__restrict__ links, const double *__restrict__ f, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const uint8_t fl = flags[p];
+    if ((fl & CLASS_MASK) == SOLID) return;
+    real g[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) g[i] = real(f[(long long)i * P.N + c] - weight_f64(i));
+    store_cell_both(A, B, P, p, x, y, z, fl, links[p], g);
+}
+
+} // namespace lbmk

@@ -1,0 +1,124 @@
+// lbm_step.cuh — a5/a6 (+ the fused part of a7): the per-step fused stream-collide kernel for sm_100a.
+//
+// One cell per thread, one warp per 32 consecutive x cells of one padded row (128-byte aligned loads of the c_x = 0
+// populations, 128-byte aligned stores of all 19).  Every FLUID cell pulls A[i][p - off_i] for all 19 directions with
+// no case distinction: bounce-back, free-slip and periodic faces were resolved by the WRITER of the previous step
+// (lbm_core.cuh, "mailboxes"), so the read side is a pure 19-stream gather and the only divergent code is a few
+// extra predicated stores in cells that have a wall link or lie on a domain face.
+// Traffic per FLUID cell: 19 x 4 B read + 19 x 4 B write + 1 flag byte (+ 4 B link word only where SLOW_BIT is set).
+//
+// HINT: 0 = default loads / stores, 1 = ld.global.cs / st.global.cs (streaming), 2 = default ld / st.cs, 3 = ld.cs / default st.
+// SPEC: issue the 19 population loads before the flag byte has arrived (no dependent round trip; SOLID cells then
+//       cost their 76 B of reads).
+#pragma once
+#include "lbm_core.cuh"
+
+namespace lbmk {
+
+template <int HINT, typename real>
+__device__ __forceinline__ real ld_pop(const real *p)
+{
+    if constexpr (HINT == 1 || HINT == 3) return __ldcs(p);
+    else return *p;
+}
+template <int HINT, typename real>
+__device__ __forceinline__ void st_pop(real *p, real v)
+{
+    if constexpr (HINT == 1 || HINT == 2) __stcs(p, v);
+    else *p = v;
+}
+
+// Per-launch address table: src[i] = A + i stride - off_i (so the pull of direction i is src[i][p]), dst[i] = B + i stride.
+// One 64-bit multiply-add per access instead of rebuilding i * stride - off_i in every thread.
+template <typename real>
+struct StepPtrs {
+    const real *src[Q];
+    real *dst[Q];
+};
+template <typename real>
+inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> &P)
+{
+    StepPtrs<real> t;
+    for (int i = 0; i < Q; ++i) {
+        const long long off = dir_cx(i) + (long long)dir_cy(i) * P.px + (long long)dir_cz(i) * P.pxy;
+        t.src[i] = A + ((long long)i * P.stride - off);
+        t.dst[i] = B + (long long)i * P.stride;
+    }
+    return t;
+}
+
+template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB>
+__global__ void __launch_bounds__(BLOCK, MINB)
+step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+            real *__restrict__ msum, const Params<real> P, const StepPtrs<real> T)
+{
+    constexpr int WPB = BLOCK / 32;
+    const unsigned gw = blockIdx.x * WPB + (threadIdx.x >> 5);
+    const int y = P.W == 1 ? (int)gw : (int)__umulhi(gw, P.Wmagic); // gw / W
+    if (y >= P.ny) return;
+    const int xw = (int)gw - y * P.W;
+    const int z = blockIdx.y;
+    const int x = xw * 32 + (int)(threadIdx.x & 31) - 1;
+    const int p = ((z + 1) * P.py + (y + 1)) * P.px + (x + 1);
+
+    real g[Q];
+    uint8_t fl;
+    if constexpr (SPEC) {
+        fl = flags[p];
+        const bool in_row = x >= 0 && x < P.nx;
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            g[i] = in_row ? ld_pop<HINT>(T.src[i] + p) : real(0);
+        });
+    } else {
+        fl = flags[p];
+    }
+    const int cls = fl & CLASS_MASK;
+    if (cls == SOLID || cls == GHOST) return;
+    if (cls == EQ_FIXED) {
+        if constexpr (MEAN) {
+            load_cell(g, A, P.stride, p);
+            const Macro<real> m = local_macros(g, EQ_FIXED, P);
+            msum[p] += m.ux;
+            msum[P.stride + p] += m.uy;
+            msum[2 * P.stride + p] += m.uz;
+        }
+        return;
+    }
+    uint32_t lk = 0;
+    if (fl & SLOW_BIT) lk = links[p];
+    Macro<real> m;
+    if (cls == FLUID) {
+        if constexpr (!SPEC) {
+            static_for<0, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                g[i] = ld_pop<HINT>(T.src[i] + p);
+            });
+        }
+        m = collide(g, P);
+    } else { // EQ_OUTFLOW (a6): f_eq(1, u of the inward neighbour at the previous step)
+        const int nb = outflow_neighbour(P, x, y, z);
+        m = Macro<real>{real(1), real(0), real(0), real(0)};
+        if (nb >= 0) {
+            load_cell(g, A, P.stride, nb);
+            m = local_macros(g, flags[nb] & CLASS_MASK, P);
+        }
+        equilibrium(g, real(0), m.ux, m.uy, m.uz);
+    }
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        st_pop<HINT>(T.dst[i] + p, g[i]);
+    });
+    if (fl & (SLOW_BIT | EDGE_BIT)) {
+        auto st = [&](int i, int pt, auto jc) { B[(long long)i * P.stride + pt] = g[decltype(jc)::value]; };
+        if (fl & SLOW_BIT) wall_stores(P, p, lk, st);
+        if (fl & EDGE_BIT) ghost_stores(P, x, y, z, lk, st);
+    }
+    if constexpr (MEAN) {
+        msum[p] += m.ux;
+        msum[P.stride + p] += m.uy;
+        msum[2 * P.stride + p] += m.uz;
+    }
+}
+
+} // namespace lbmk

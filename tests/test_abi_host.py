@@ -35,9 +35,11 @@ def test_every_declared_symbol_is_exported(lib):
 def test_workspace_bytes_counts_two_buffers_flags_and_mean(lib):
     out = C.c_size_t()
     assert lib.lbm_workspace_bytes(400, 400, 100, 0, 0, C.byref(out)) == 0
-    n = 400 * 400 * 100
-    assert out.value >= 2 * 19 * 4 * n + n
-    assert out.value < 2 * 19 * 4 * n + n + 16 * 2 ** 20
+    # halo-padded box: x pitch = nx + 2 rounded up to 32, one halo layer in y and z
+    n = 416 * 402 * 102
+    per_cell = 2 * 19 * 4 + 1 + 4  # two population buffers, flag byte, link word
+    assert out.value >= per_cell * n
+    assert out.value < per_cell * n + 16 * 2 ** 20
     with_mean = C.c_size_t()
     assert lib.lbm_workspace_bytes(400, 400, 100, 1, 0, C.byref(with_mean)) == 0
     assert with_mean.value - out.value == pytest.approx(12 * n, rel=1e-3)

@@ -355,7 +355,7 @@ def test_host_pointer_getters_equal_device_pointer_getters(B):
 
 # ---------------------------------------------------------------------------------------------- kernel variants
 
-@pytest.mark.parametrize("variant", [0, 1, 8, 9, 10, 11])
+@pytest.mark.parametrize("variant", [0, 1, 3, 4, 7, 8])
 @pytest.mark.parametrize("shape", [(37, 11, 9), (64, 36, 20), (130, 50, 7)])
 def test_every_step_kernel_variant_matches_the_oracle(B, variant, shape):
     """The bulk-copy (TMA) kernels and the LDG kernel compute the same step: ragged and 16-byte-aligned boxes,
