@@ -29,7 +29,7 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
 {
     Layout L{};
     const size_t rs = fp64 ? 8 : 4;
-    L.px = (nx + 2 + 31) / 32 * 32;
+    L.px = (nx + XOFF + 1 + 31) / 32 * 32;
     L.py = ny + 2;
     L.Np = (long long)L.px * L.py * (nz + 2);
     L.stride = (long long)align_up((size_t)L.Np, 64);
@@ -51,7 +51,7 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
 bool size_ok(int nx, int ny, int nz)
 {
     if (nx < 1 || ny < 1 || nz < 1 || nz > 65535) return false;
-    const long long px = ((long long)nx + 2 + 31) / 32 * 32;
+    const long long px = ((long long)nx + XOFF + 1 + 31) / 32 * 32;
     return px * ((long long)ny + 2) * ((long long)nz + 2) <= 2000000000LL;
 }
 
@@ -108,8 +108,10 @@ Params<real> make_params(const lbm_t *h)
     P.px = h->L.px; P.py = h->L.py; P.pxy = h->L.px * h->L.py;
     P.Np = (int)h->L.Np;
     P.N = (int)h->N();
-    P.W = P.px / 32;
-    P.Wmagic = (unsigned)((0x100000000ULL + (unsigned)P.W - 1) / (unsigned)P.W);
+    P.nxy = h->nx * h->ny;
+    // exact for n < nxy + 1024 when (nxy + 1024) * nx < 2^32 (error term n * (magic * nx - 2^32) < 2^32)
+    P.nx_magic = (h->nx > 1 && ((unsigned long long)P.nxy + 1024ULL) * (unsigned long long)h->nx < 0x100000000ULL)
+                     ? (unsigned)((0x100000000ULL + (unsigned)h->nx - 1) / (unsigned)h->nx) : 0u;
     P.stride = h->L.stride;
     for (int k = 0; k < 6; ++k) P.face[k] = h->face[k];
     P.tau0 = (real)(3.0 * h->nu0 + 0.5);
@@ -308,22 +310,21 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     return rc;
 }
 
-template <typename real, int HINT, bool SPEC, int BLOCK, int MINB>
+template <typename real, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0>
 int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
     const real *A = (const real *)h->state();
     real *B = (real *)h->other();
     real *ms = (real *)h->mean();
-    constexpr int WPB = BLOCK / 32;
-    const dim3 grid(blocks_for((long long)P.W * P.ny, WPB), (unsigned)P.nz);
+    const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
     const StepPtrs<real> T = make_step_ptrs<real>(A, B, P);
-    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
-    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
+    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
+    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
     return check_launch(h, "step_kernel");
 }
 
 // kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes / load issue order.
-constexpr int N_VARIANTS = 10;
+constexpr int N_VARIANTS = 19;
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
@@ -339,6 +340,15 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         case 7: return launch_step_as<real, 0, false, 512, 2>(h, P, sample);
         case 8: return launch_step_as<real, 0, false, 64, 16>(h, P, sample);
         case 9: return launch_step_as<real, 0, false, 256, 3>(h, P, sample);
+        case 10: return launch_step_as<real, 0, true, 256, 4, 1>(h, P, sample);
+        case 11: return launch_step_as<real, 0, true, 128, 8, 1>(h, P, sample);
+        case 12: return launch_step_as<real, 0, true, 256, 4, 2>(h, P, sample);
+        case 13: return launch_step_as<real, 0, true, 128, 8, 2>(h, P, sample);
+        case 16: return launch_step_as<real, 0, true, 128, 8, 3>(h, P, sample);
+        case 17: return launch_step_as<real, 0, true, 128, 8, 4>(h, P, sample);
+        case 18: return launch_step_as<real, 0, true, 128, 8, 5>(h, P, sample);
+        case 14: return launch_step_as<real, 0, false, 256, 4, 1>(h, P, sample);
+        case 15: return launch_step_as<real, 0, false, 256, 4, 2>(h, P, sample);
         default: break;
         }
     }

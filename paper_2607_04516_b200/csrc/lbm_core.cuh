@@ -1,8 +1,8 @@
 // lbm_core.cuh — lattice, layout, per-cell arithmetic and the write-side boundary rule of the D3Q19 LBM-LES path
 // (sm_100a).  Algorithm statement: DESIGN.md §3 (restating PAPER.md:61, Table 1).
 //
-// Storage.  Populations SoA g[i][Z][Y][X] on a HALO-PADDED box: one halo layer on every side, x pitch rounded up
-// to 32 cells (a warp never straddles a row; every row is 128-byte aligned).  g_i = f_i - w_i ("shifted": the rest
+// Storage.  Populations SoA g[i][Z][Y][X] on a HALO-PADDED box: one halo layer on every side, interior rows starting
+// at padded x = 8, x pitch rounded up to 32 cells (every row is 128-byte aligned).  g_i = f_i - w_i ("shifted": the rest
 // state is exactly 0, stored numbers are O(Ma), FP32 rounding stays two orders below the 1e-5 parity bar).
 // Two buffers A/B, pull scheme: every FLUID cell reads A[i][p - off_i] for ALL i with no case distinction.
 //
@@ -57,11 +57,11 @@ __host__ __device__ __forceinline__ void static_for(F &&f)
 template <typename real>
 struct Params {
     int nx, ny, nz;   // interior cells
-    int px, py, pxy;  // padded x pitch (multiple of 32, >= nx + 2), padded rows per plane (ny + 2), px * py
+    int px, py, pxy;  // padded x pitch (multiple of 32, >= nx + XOFF + 1), padded rows per plane (ny + 2), px * py
     int Np;           // padded cells = pxy * (nz + 2)
     int N;            // interior cells
-    int W;            // warps per padded row = px / 32
-    unsigned Wmagic;  // ceil(2^32 / W): q = umulhi(n, Wmagic) == n / W for n < 2^32 / W
+    int nxy;          // nx * ny
+    unsigned nx_magic; // ceil(2^32 / nx) when umulhi(n, nx_magic) == n / nx for all n < nxy + 1024, else 0 (use a division)
     long long stride; // elements between consecutive populations (>= Np, multiple of 64)
     int face[6];
     real tau0, Kles;       // Kles = 18 sqrt(2) Cs^2
@@ -69,11 +69,14 @@ struct Params {
     real Fx, Fy, Fz;
 };
 
+// Interior x = 0 sits at padded x = XOFF = 8: every interior row starts on a 32-byte sector boundary (and ends on one
+// when nx % 8 == 0), so full-row stores never leave partially written sectors, which would cost a DRAM fill read each.
+constexpr int XOFF = 8;
 // padded linear index of interior cell (x,y,z); also valid for halo coordinates -1 and n
 template <typename real>
 __host__ __device__ __forceinline__ int pidx(const Params<real> &P, int x, int y, int z)
 {
-    return ((z + 1) * P.py + (y + 1)) * P.px + (x + 1);
+    return ((z + 1) * P.py + (y + 1)) * P.px + (x + XOFF);
 }
 // offset (in cells) of the pull source of direction i relative to the cell: source = p - poff
 template <int I, typename real>

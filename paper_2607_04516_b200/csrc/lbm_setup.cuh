@@ -15,8 +15,8 @@ __global__ void voxelise_kernel(const int32_t *__restrict__ height, uint8_t *__r
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P.Np) return;
-    int x = p % P.px - 1, y = (p / P.px) % P.py - 1, z = p / P.pxy - 1;
-    if (x > P.nx) { flags[p] = SOLID; return; }
+    int x = p % P.px - XOFF, y = (p / P.px) % P.py - 1, z = p / P.pxy - 1;
+    if (x < -1 || x > P.nx) { flags[p] = SOLID; return; }
     const int n[3] = {P.nx, P.ny, P.nz};
     int c[3] = {x, y, z};
     bool halo = false, dead = false;

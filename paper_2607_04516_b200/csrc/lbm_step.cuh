@@ -1,7 +1,7 @@
 // lbm_step.cuh — a5/a6 (+ the fused part of a7): the per-step fused stream-collide kernel for sm_100a.
 //
-// One cell per thread, one warp per 32 consecutive x cells of one padded row (128-byte aligned loads of the c_x = 0
-// populations, 128-byte aligned stores of all 19).  Every FLUID cell pulls A[i][p - off_i] for all 19 directions with
+// One cell per thread, threads linear over the interior cells of one z plane (a warp = 32 consecutive interior cells,
+// at most two contiguous row segments; no idle lanes).  Every FLUID cell pulls A[i][p - off_i] for all 19 directions with
 // no case distinction: bounce-back, free-slip and periodic faces were resolved by the WRITER of the previous step
 // (lbm_core.cuh, "mailboxes"), so the read side is a pure 19-stream gather and the only divergent code is a few
 // extra predicated stores in cells that have a wall link or lie on a domain face.
@@ -47,32 +47,33 @@ inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> 
     return t;
 }
 
-template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB>
+template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0>
 __global__ void __launch_bounds__(BLOCK, MINB)
 step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
             real *__restrict__ msum, const Params<real> P, const StepPtrs<real> T)
 {
-    constexpr int WPB = BLOCK / 32;
-    const unsigned gw = blockIdx.x * WPB + (threadIdx.x >> 5);
-    const int y = P.W == 1 ? (int)gw : (int)__umulhi(gw, P.Wmagic); // gw / W
-    if (y >= P.ny) return;
-    const int xw = (int)gw - y * P.W;
+    const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x; // cell of the z plane, linear over interior (y, x)
+    if (c2 >= (unsigned)P.nxy) return;
+    const int y = P.nx_magic ? (int)__umulhi(c2, P.nx_magic) : (int)(c2 / (unsigned)P.nx);
+    const int x = (int)c2 - y * P.nx;
     const int z = blockIdx.y;
-    const int x = xw * 32 + (int)(threadIdx.x & 31) - 1;
-    const int p = ((z + 1) * P.py + (y + 1)) * P.px + (x + 1);
+    const int p = pidx(P, x, y, z);
 
     real g[Q];
     uint8_t fl;
     if constexpr (SPEC) {
         fl = flags[p];
-        const bool in_row = x >= 0 && x < P.nx;
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            g[i] = in_row ? ld_pop<HINT>(T.src[i] + p) : real(0);
+            g[i] = ld_pop<HINT>(T.src[i] + p);
         });
     } else {
         fl = flags[p];
     }
+    if constexpr (EXP == 1) fl = 0; // timing experiment: every cell FLUID, no boundary stores
+    if constexpr (EXP >= 2) fl &= CLASS_MASK;                           // timing experiment: classes only, no boundary stores
+    if constexpr (EXP == 3 || EXP == 5) { if ((fl & CLASS_MASK) == EQ_OUTFLOW) return; }   // outflow cells static
+    if constexpr (EXP == 4 || EXP == 5) { if ((fl & CLASS_MASK) == SOLID) fl = 0; } // solids compute and store
     const int cls = fl & CLASS_MASK;
     if (cls == SOLID || cls == GHOST) return;
     if (cls == EQ_FIXED) {

@@ -36,7 +36,7 @@ def test_workspace_bytes_counts_two_buffers_flags_and_mean(lib):
     out = C.c_size_t()
     assert lib.lbm_workspace_bytes(400, 400, 100, 0, 0, C.byref(out)) == 0
     # halo-padded box: x pitch = nx + 2 rounded up to 32, one halo layer in y and z
-    n = 416 * 402 * 102
+    n = 416 * 402 * 102  # 400 + 8 (row offset) + 1 (halo) -> 416
     per_cell = 2 * 19 * 4 + 1 + 4  # two population buffers, flag byte, link word
     assert out.value >= per_cell * n
     assert out.value < per_cell * n + 16 * 2 ** 20
