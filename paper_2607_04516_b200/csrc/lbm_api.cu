@@ -21,7 +21,8 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 struct Layout {
     int px, py;
     long long Np, stride;
-    size_t off_A, off_B, off_flags, off_links, off_mean, off_scratch, total;
+    size_t off_A, off_B, off_flags, off_links, off_fu, off_mean, off_scratch, total;
+    size_t fu_bytes;
     size_t scratch_bytes;
 };
 
@@ -38,6 +39,9 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
     L.off_B = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
     L.off_flags = o; o += align_up((size_t)L.Np, ALIGN);
     L.off_links = o; o += align_up((size_t)L.Np * sizeof(uint32_t), ALIGN);
+    // outflow-velocity side buffer (a6): 2 halves x 3 components x one slot per face-plane cell of all six faces (upper bound)
+    L.fu_bytes = align_up((size_t)2 * 3 * 2 * ((size_t)ny * nz + (size_t)nx * nz + (size_t)nx * ny) * rs, ALIGN);
+    L.off_fu = o; o += L.fu_bytes;
     L.off_mean = o; if (want_mean) o += align_up((size_t)3 * L.stride * rs, ALIGN);
     // scratch: heightmap (nx*ny int32) or a profile (3 nz doubles) or one face plane (3 n1 n2 doubles)
     const size_t plane = (size_t)std::max(std::max((size_t)nx * ny, (size_t)nx * nz), (size_t)ny * nz);
@@ -80,6 +84,7 @@ struct lbm {
     void *other() const { return cur ? bufA() : bufB(); }
     uint8_t *flags() const { return (uint8_t *)(ws + L.off_flags); }
     uint32_t *links() const { return (uint32_t *)(ws + L.off_links); }
+    void *fu() const { return ws + L.off_fu; }
     void *mean() const { return want_mean ? ws + L.off_mean : nullptr; }
     void *scratch() const { return ws + L.off_scratch; }
     long long N() const { return (long long)nx * ny * nz; }
@@ -114,6 +119,12 @@ Params<real> make_params(const lbm_t *h)
                      ? (unsigned)((0x100000000ULL + (unsigned)h->nx - 1) / (unsigned)h->nx) : 0u;
     P.stride = h->L.stride;
     for (int k = 0; k < 6; ++k) P.face[k] = h->face[k];
+    P.F = 0;
+    for (int k = 0; k < 6; ++k) {
+        const int axis = k >> 1;
+        P.foff[k] = P.F;
+        if (h->face[k] == FACE_EQ_OUTFLOW) P.F += (axis == 0 ? h->ny : h->nx) * (axis == 2 ? h->ny : h->nz);
+    }
     P.tau0 = (real)(3.0 * h->nu0 + 0.5);
     P.Kles = (real)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs);
     P.fcor = (real)h->fcor;
@@ -233,6 +244,7 @@ int do_set_flags(lbm_t *h, const int32_t *height)
     CUDA_TRY(h, cudaMemsetAsync(h->bufA(), 0, (size_t)Q * h->L.stride * rs, h->stream));
     CUDA_TRY(h, cudaMemsetAsync(h->bufB(), 0, (size_t)Q * h->L.stride * rs, h->stream));
     if (h->want_mean) CUDA_TRY(h, cudaMemsetAsync(h->mean(), 0, (size_t)3 * h->L.stride * rs, h->stream));
+    CUDA_TRY(h, cudaMemsetAsync(h->fu(), 0, h->L.fu_bytes, h->stream));
     h->cur = 0; h->step = 0; h->mcount = 0; h->have_flags = true;
     return LBM_OK;
 }
@@ -252,7 +264,7 @@ int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, con
         const int B = 256;
         const long long threads = mode == 0 ? (long long)P.N : (long long)count;
         inlet_kernel<real, in_t><<<blocks_for(threads, B), B, 0, h->stream>>>(
-            (real *)h->bufA(), (real *)h->bufB(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+            (real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, mode, face, P);
         rc = check_launch(h, "inlet_kernel");
     }
@@ -301,7 +313,7 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     if (!rc) {
         const int B = 256;
         init_kernel<real, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (real *)h->bufA(), (real *)h->bufB(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+            (real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
         rc = check_launch(h, "init_kernel");
     }
@@ -318,8 +330,11 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
     real *ms = (real *)h->mean();
     const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
     const StepPtrs<real> T = make_step_ptrs<real>(A, B, P);
-    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
-    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, P, T);
+    // the side buffer's halves follow the population buffers: read the half written together with A, write B's
+    const real *fur = (const real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
+    real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
+    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
+    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
     return check_launch(h, "step_kernel");
 }
 
@@ -330,16 +345,16 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
     if constexpr (std::is_same<real, float>::value) {
         switch (h->variant) {
-        case 0: return launch_step_as<real, 0, false, 256, 4>(h, P, sample);
+        case 0: return launch_step_as<real, 0, true, 128, 10>(h, P, sample);
         case 1: return launch_step_as<real, 0, true, 256, 4>(h, P, sample);
         case 2: return launch_step_as<real, 0, false, 128, 8>(h, P, sample);
         case 3: return launch_step_as<real, 0, true, 128, 8>(h, P, sample);
-        case 4: return launch_step_as<real, 1, false, 256, 4>(h, P, sample);
-        case 5: return launch_step_as<real, 2, false, 256, 4>(h, P, sample);
-        case 6: return launch_step_as<real, 3, false, 256, 4>(h, P, sample);
-        case 7: return launch_step_as<real, 0, false, 512, 2>(h, P, sample);
-        case 8: return launch_step_as<real, 0, false, 64, 16>(h, P, sample);
-        case 9: return launch_step_as<real, 0, false, 256, 3>(h, P, sample);
+        case 4: return launch_step_as<real, 0, true, 128, 9>(h, P, sample);
+        case 5: return launch_step_as<real, 0, false, 256, 4>(h, P, sample);
+        case 6: return launch_step_as<real, 0, true, 128, 11>(h, P, sample);
+        case 7: return launch_step_as<real, 0, true, 128, 12>(h, P, sample);
+        case 8: return launch_step_as<real, 0, true, 128, 14>(h, P, sample);
+        case 9: return launch_step_as<real, 0, true, 64, 20>(h, P, sample);
         case 10: return launch_step_as<real, 0, true, 256, 4, 1>(h, P, sample);
         case 11: return launch_step_as<real, 0, true, 128, 8, 1>(h, P, sample);
         case 12: return launch_step_as<real, 0, true, 256, 4, 2>(h, P, sample);
@@ -421,7 +436,7 @@ int do_get_links(lbm_t *h, uint32_t *links)
     int rc = stage_out(h, links, (size_t)P.N * sizeof(uint32_t), &o);
     if (rc) return rc;
     const int B = 256;
-    links_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->links(), (uint32_t *)o.dev, P);
+    links_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->links(), h->flags(), (uint32_t *)o.dev, P);
     rc = check_launch(h, "links_out_kernel");
     int rc2 = finish_out(h, &o, 1);
     return rc ? rc : rc2;
@@ -449,7 +464,7 @@ int do_set_state(lbm_t *h, const double *f)
     int rc = stage_in(h, f, (size_t)Q * P.N * sizeof(double), h->L.scratch_bytes, &in);
     if (rc) return rc;
     const int B = 256;
-    state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), h->flags(), h->links(),
+    state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), h->links(),
                                                                     (const double *)in.dev, P);
     rc = check_launch(h, "state_in_kernel");
     release_in(h, &in, 1);
@@ -463,7 +478,7 @@ int do_feed(lbm_t *dst, const lbm_t *src, int sx)
     const Params<real> D = make_params<real>(dst), S = make_params<real>(src);
     const int B = 128;
     feed_kernel<real><<<blocks_for((long long)D.ny * D.nz, B), B, 0, dst->stream>>>(
-        (real *)dst->bufA(), (real *)dst->bufB(), dst->flags(), D, (const real *)src->state(), src->flags(), S, sx);
+        (real *)dst->bufA(), (real *)dst->bufB(), (real *)dst->fu(), dst->flags(), D, (const real *)src->state(), src->flags(), S, sx);
     return check_launch(dst, "feed_kernel");
 }
 

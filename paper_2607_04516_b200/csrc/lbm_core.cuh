@@ -27,6 +27,8 @@ enum : int { PERIODIC = 0, WALL = 1, FREE_SLIP = 2, FACE_EQ_FIXED = 3, FACE_EQ_O
 constexpr uint8_t CLASS_MASK = 7;
 constexpr uint8_t SLOW_BIT = 0x80; // FLUID cell with at least one wall link (mailbox stores needed)
 constexpr uint8_t EDGE_BIT = 0x40; // non-solid cell on a domain face (ghost stores may be needed)
+constexpr uint8_t FEED_BIT = 0x20; // non-solid cell one layer inside an EQ_OUTFLOW face: publishes its velocity (a6)
+constexpr uint8_t SURF_BIT = 0x10; // SOLID cell sharing a 32-byte sector with a cell that is rewritten every step
 
 // ---- lattice (DESIGN.md §3 step 1): pair k = 1..9 holds directions 2k-1 (+) and 2k (-) -------------------------
 // pair vectors: 1:(1,0,0) 2:(0,1,0) 3:(0,0,1) 4:(1,1,0) 5:(1,0,1) 6:(0,1,1) 7:(1,-1,0) 8:(1,0,-1) 9:(0,1,-1)
@@ -64,6 +66,8 @@ struct Params {
     unsigned nx_magic; // ceil(2^32 / nx) when umulhi(n, nx_magic) == n / nx for all n < nxy + 1024, else 0 (use a division)
     long long stride; // elements between consecutive populations (>= Np, multiple of 64)
     int face[6];
+    int foff[6];      // first slot of each EQ_OUTFLOW face in the outflow-velocity buffer (a6), slots = face-plane cells
+    int F;            // slots in total (0 if there is no outflow face)
     real tau0, Kles;       // Kles = 18 sqrt(2) Cs^2
     real fcor, h, inv1ph2; // h = fcor/2, 1/(1+h^2)
     real Fx, Fy, Fz;
@@ -301,18 +305,59 @@ __device__ __forceinline__ void store_cell(real *__restrict__ B, const Params<re
     }
 }
 
-// which face's normal an EQ_OUTFLOW cell uses: first EQ_OUTFLOW face it lies on, order x-,x+,y-,y+,z-,z+.
-// Returns the padded index of the inward neighbour, -1 if the box is one cell thick on that axis.
+// ---- a6: EQ_OUTFLOW cells ---------------------------------------------------------------------------------------------
+// G_{k+1}(c) = f_eq(1, u_loc(G_k, c - n)) (DESIGN.md §3 step 6), n = outward normal of c's owner face = the first
+// EQ_OUTFLOW face it lies on (order x-,x+,y-,y+,z-,z+).  u_loc(G_k, nb) is the velocity the cell nb itself holds while
+// it writes G_k (its collision velocity if FLUID), so nb publishes it into a small double-buffered side array
+// fu[3][F] ("feeds"), and the outflow cell reads 3 values next step instead of gathering nb's 19 populations:
+// no second dependent gather in the warps that contain a face cell.  Slots never fed (nb SOLID, box one cell
+// thick) stay 0 = the u = 0 the rule prescribes.
 template <typename real>
-__device__ __forceinline__ int outflow_neighbour(const Params<real> &P, int x, int y, int z)
+__device__ __forceinline__ int outflow_owner(const Params<real> &P, int x, int y, int z)
 {
-    if (x == 0 && P.face[0] == FACE_EQ_OUTFLOW) return (P.nx > 1) ? pidx(P, 1, y, z) : -1;
-    if (x == P.nx - 1 && P.face[1] == FACE_EQ_OUTFLOW) return (P.nx > 1) ? pidx(P, x - 1, y, z) : -1;
-    if (y == 0 && P.face[2] == FACE_EQ_OUTFLOW) return (P.ny > 1) ? pidx(P, x, 1, z) : -1;
-    if (y == P.ny - 1 && P.face[3] == FACE_EQ_OUTFLOW) return (P.ny > 1) ? pidx(P, x, y - 1, z) : -1;
-    if (z == 0 && P.face[4] == FACE_EQ_OUTFLOW) return (P.nz > 1) ? pidx(P, x, y, 1) : -1;
-    if (z == P.nz - 1 && P.face[5] == FACE_EQ_OUTFLOW) return (P.nz > 1) ? pidx(P, x, y, z - 1) : -1;
+    if (x == 0 && P.face[0] == FACE_EQ_OUTFLOW) return 0;
+    if (x == P.nx - 1 && P.face[1] == FACE_EQ_OUTFLOW) return 1;
+    if (y == 0 && P.face[2] == FACE_EQ_OUTFLOW) return 2;
+    if (y == P.ny - 1 && P.face[3] == FACE_EQ_OUTFLOW) return 3;
+    if (z == 0 && P.face[4] == FACE_EQ_OUTFLOW) return 4;
+    if (z == P.nz - 1 && P.face[5] == FACE_EQ_OUTFLOW) return 5;
     return -1;
+}
+template <typename real>
+__device__ __forceinline__ int outflow_slot(const Params<real> &P, int k, int x, int y, int z)
+{
+    const int axis = k >> 1;
+    const int j1 = axis == 0 ? y : x, j2 = axis == 2 ? y : z, n1 = axis == 0 ? P.ny : P.nx;
+    return P.foff[k] + j2 * n1 + j1;
+}
+// is (x,y,z) one layer inside some EQ_OUTFLOW face? (superset test used for FEED_BIT)
+template <typename real>
+__device__ __forceinline__ bool outflow_feeder(const Params<real> &P, int x, int y, int z)
+{
+    const int c[3] = {x, y, z}, n[3] = {P.nx, P.ny, P.nz};
+    bool f = false;
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const int a = k >> 1;
+        f |= P.face[k] == FACE_EQ_OUTFLOW && n[a] > 1 && c[a] == ((k & 1) ? n[a] - 2 : 1);
+    }
+    return f;
+}
+// publish velocity u of cell (x,y,z) to every outflow cell whose inward neighbour it is; w(slot, component, value)
+template <typename real, class W>
+__device__ __forceinline__ void outflow_feed(const Params<real> &P, int x, int y, int z, real ux, real uy, real uz, W &&w)
+{
+    const int n[3] = {P.nx, P.ny, P.nz};
+#pragma unroll
+    for (int k = 0; k < 6; ++k) {
+        const int a = k >> 1;
+        int c[3] = {x, y, z};
+        if (P.face[k] != FACE_EQ_OUTFLOW || n[a] < 2 || c[a] != ((k & 1) ? n[a] - 2 : 1)) continue;
+        c[a] = (k & 1) ? n[a] - 1 : 0;
+        if (outflow_owner(P, c[0], c[1], c[2]) != k) continue;
+        const int s = outflow_slot(P, k, c[0], c[1], c[2]);
+        w(s, 0, ux); w(s, 1, uy); w(s, 2, uz);
+    }
 }
 
 // interior cell c = (z*ny + y)*nx + x  ->  coordinates (set-up and output kernels; not on the hot path)

@@ -73,13 +73,15 @@ __global__ void flags_out_kernel(const uint8_t *__restrict__ flags, uint8_t *__r
 }
 
 template <typename real>
-__global__ void links_out_kernel(const uint32_t *__restrict__ links, uint32_t *__restrict__ out, Params<real> P)
+__global__ void links_out_kernel(const uint32_t *__restrict__ links, const uint8_t *__restrict__ flags, uint32_t *__restrict__ out,
+                                 Params<real> P)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
     int x, y, z;
     cell_xyz(P, c, x, y, z);
-    out[c] = links[pidx(P, x, y, z)];
+    const int p = pidx(P, x, y, z);
+    out[c] = (flags[p] & CLASS_MASK) == FLUID ? links[p] : 0u; // SOLID cells keep an internal mailbox mask there
 }
 
 } // namespace lbmk

@@ -51,9 +51,11 @@ __global__ void voxelise_kernel(const int32_t *__restrict__ height, uint8_t *__r
 }
 
 // ---- a2: link classification ---------------------------------------------------------------------------------------------
-// Bit i (1..18) of links[p] <=> the pull source of direction i of FLUID cell p is SOLID in the padded box — exactly
-// "step 4a takes the bounce-back branch" (DESIGN.md §3 step 9).  Adds SLOW_BIT / EDGE_BIT to the flag byte in place
-// (class bits are never changed, and readers mask them, so in-place is race-free).
+// FLUID cell: bit i (1..18) of links[p] <=> the pull source of direction i is SOLID in the padded box — exactly
+// "step 4a takes the bounce-back branch" (DESIGN.md §3 step 9).  SOLID cell: bit i <=> slot (i, p) is a mailbox, i.e.
+// the cell p + c_i is FLUID and stores its bounced population there (internal; lbm_get_links reports 0 for it).
+// Adds SLOW / EDGE / FEED / SURF bits to the flag byte in place (class bits are never changed, and readers mask them,
+// so in-place is race-free).
 template <typename real>
 __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restrict__ links, Params<real> P)
 {
@@ -64,30 +66,56 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restric
     const int p = pidx(P, x, y, z);
     const int cls = flags[p] & CLASS_MASK;
     uint32_t bits = 0;
+    uint8_t extra = 0;
     if (cls == FLUID) {
         static_for<1, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             bits |= (((flags[p - poff<i>(P)] & CLASS_MASK) == SOLID) ? 1u : 0u) << i;
         });
+        if (bits) extra |= SLOW_BIT;
+    } else if (cls == SOLID) {
+        static_for<1, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            bits |= (((flags[p + poff<i>(P)] & CLASS_MASK) == FLUID) ? 1u : 0u) << i;
+        });
+        const int s0 = p & ~7; // the 8 cells of this cell's 32-byte sector (FP32)
+        bool live = false;
+        for (int q = s0; q < s0 + 8; ++q) {
+            const int cq = flags[q] & CLASS_MASK;
+            live |= cq == FLUID || cq == EQ_OUTFLOW;
+        }
+        if (live) extra |= SURF_BIT;
     }
     links[p] = bits;
-    const bool edge = x == 0 || x == P.nx - 1 || y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
-    flags[p] = (uint8_t)(cls | (bits ? SLOW_BIT : 0) | ((cls != SOLID && edge) ? EDGE_BIT : 0));
+    if (cls != SOLID) {
+        const bool edge = x == 0 || x == P.nx - 1 || y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
+        if (edge) extra |= EDGE_BIT;
+        if (outflow_feeder(P, x, y, z)) extra |= FEED_BIT;
+    }
+    flags[p] = (uint8_t)(cls | extra);
 }
 
-// store one cell's state into BOTH buffers (set-up paths: the two buffers start identical)
+// store one cell's state into BOTH buffers (set-up paths: the two buffers start identical), and publish its velocity
+// to the outflow cells it feeds (both halves of the double-buffered side array)
 template <typename real>
-__device__ __forceinline__ void store_cell_both(real *__restrict__ A, real *__restrict__ B, const Params<real> &P, int p, int x, int y,
-                                                int z, uint8_t fl, uint32_t lk, const real (&g)[Q])
+__device__ __forceinline__ void store_cell_both(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const Params<real> &P,
+                                                int p, int x, int y, int z, uint8_t fl, uint32_t lk, const real (&g)[Q])
 {
     store_cell(A, P, p, x, y, z, fl, lk, g);
     store_cell(B, P, p, x, y, z, fl, lk, g);
+    if (fl & FEED_BIT) {
+        const Macro<real> m = local_macros(g, fl & CLASS_MASK, P);
+        outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int s, int comp, real v) {
+            fu[comp * P.F + s] = v;
+            fu[(3 + comp) * P.F + s] = v;
+        });
+    }
 }
 
 // ---- a3: inlet write -------------------------------------------------------------------------------------------------
 // mode 0: profile prof[nz] per component by level; mode 1: plane uvw[3][n2][n1] of one face
 template <typename real, typename in_t>
-__global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+__global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                              const in_t *__restrict__ pu, const in_t *__restrict__ pv, const in_t *__restrict__ pw,
                              int mode, int face, Params<real> P)
 {
@@ -117,12 +145,13 @@ __global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, const u
     const real ux = real(pu[src]), uy = pv ? real(pv[src]) : real(0), uz = pw ? real(pw[src]) : real(0);
     real g[Q];
     equilibrium(g, real(0), ux, uy, uz);
-    store_cell_both(A, B, P, p, x, y, z, fl, 0u, g);
+    store_cell_both(A, B, fu, P, p, x, y, z, fl, 0u, g);
 }
 
 // ---- a8: precursor plane -> main inlet (config 5) -----------------------------------------------------------------------
 template <typename real>
-__global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, const uint8_t *__restrict__ dflags, Params<real> D,
+__global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, real *__restrict__ dfu, const uint8_t *__restrict__ dflags,
+                            Params<real> D,
                             const real *__restrict__ sA, const uint8_t *__restrict__ sflags, Params<real> S, int sx)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -136,13 +165,13 @@ __global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, const 
     load_cell(g, sA, S.stride, sp);
     const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, S);
     equilibrium(g, real(0), m.ux, m.uy, m.uz);
-    store_cell_both(dA, dB, D, dp, 0, y, z, fl, 0u, g);
+    store_cell_both(dA, dB, dfu, D, dp, 0, y, z, fl, 0u, g);
 }
 
 // ---- a4: init ------------------------------------------------------------------------------------------------------------
 // G0 = f_eq(rho0, u0) in FLUID and EQ_OUTFLOW cells (EQ_FIXED keep their boundary state; SOLID cells hold mailboxes)
 template <typename real, typename in_t>
-__global__ void init_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+__global__ void init_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                             const uint32_t *__restrict__ links, const in_t *__restrict__ rho, const in_t *__restrict__ ux,
                             const in_t *__restrict__ uy, const in_t *__restrict__ uz, Params<real> P)
 {
@@ -158,7 +187,7 @@ __global__ void init_kernel(real *__restrict__ A, real *__restrict__ B, const ui
     const real u = ux ? real(ux[c]) : real(0), v = uy ? real(uy[c]) : real(0), w = uz ? real(uz[c]) : real(0);
     real g[Q];
     equilibrium(g, drho, u, v, w);
-    store_cell_both(A, B, P, p, x, y, z, fl, links[p], g);
+    store_cell_both(A, B, fu, P, p, x, y, z, fl, links[p], g);
 }
 
 // ---- checkpoint ------------------------------------------------------------------------------------------------------------
@@ -177,7 +206,7 @@ __global__ void state_out_kernel(const real *__restrict__ A, const uint8_t *__re
 }
 
 template <typename real>
-__global__ void state_in_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+__global__ void state_in_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                                 const uint32_t *__restrict__ links, const double *__restrict__ f, Params<real> P)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -190,7 +219,7 @@ __global__ void state_in_kernel(real *__restrict__ A, real *__restrict__ B, cons
     real g[Q];
 #pragma unroll
     for (int i = 0; i < Q; ++i) g[i] = real(f[(long long)i * P.N + c] - weight_f64(i));
-    store_cell_both(A, B, P, p, x, y, z, fl, links[p], g);
+    store_cell_both(A, B, fu, P, p, x, y, z, fl, links[p], g);
 }
 
 } // namespace lbmk

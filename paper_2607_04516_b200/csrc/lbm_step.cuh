@@ -21,6 +21,26 @@ __device__ __forceinline__ real ld_pop(const real *p)
     if constexpr (HINT == 1 || HINT == 3) return __ldcs(p);
     else return *p;
 }
+// A load the compiler may not sink below a later branch (volatile asm keeps its place): the 19 pulls of the
+// speculative kernels are issued before the flag byte is tested.
+__device__ __forceinline__ float ld_pinned(const float *p)
+{
+    float v;
+    asm volatile("ld.volatile.global.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double ld_pinned(const double *p)
+{
+    double v;
+    asm volatile("ld.volatile.global.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ uint8_t ld_pinned(const uint8_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(p));
+    return (uint8_t)v;
+}
 template <int HINT, typename real>
 __device__ __forceinline__ void st_pop(real *p, real v)
 {
@@ -50,7 +70,7 @@ inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> 
 template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0>
 __global__ void __launch_bounds__(BLOCK, MINB)
 step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-            real *__restrict__ msum, const Params<real> P, const StepPtrs<real> T)
+            real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T)
 {
     const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x; // cell of the z plane, linear over interior (y, x)
     if (c2 >= (unsigned)P.nxy) return;
@@ -62,11 +82,11 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
     real g[Q];
     uint8_t fl;
     if constexpr (SPEC) {
-        fl = flags[p];
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            g[i] = ld_pop<HINT>(T.src[i] + p);
+            g[i] = ld_pinned(T.src[i] + p);
         });
+        fl = ld_pinned(flags + p); // volatile asm statements keep their order: the flag test cannot move above the pulls
     } else {
         fl = flags[p];
     }
@@ -75,7 +95,18 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
     if constexpr (EXP == 3 || EXP == 5) { if ((fl & CLASS_MASK) == EQ_OUTFLOW) return; }   // outflow cells static
     if constexpr (EXP == 4 || EXP == 5) { if ((fl & CLASS_MASK) == SOLID) fl = 0; } // solids compute and store
     const int cls = fl & CLASS_MASK;
-    if (cls == SOLID || cls == GHOST) return;
+    if (cls == SOLID) {
+        // a solid cell that shares a 32-byte sector with live cells completes the sector with zeros in every slot that
+        // is not a neighbour's mailbox: the sector leaves L2 fully written, no DRAM fill read (same bytes written)
+        if (fl & SURF_BIT) {
+            const uint32_t mk = links[p];
+            static_for<0, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                if (!((mk >> i) & 1u)) st_pop<HINT>(T.dst[i] + p, real(0));
+            });
+        }
+        return;
+    }
     if (cls == EQ_FIXED) {
         if constexpr (MEAN) {
             load_cell(g, A, P.stride, p);
@@ -97,13 +128,10 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
             });
         }
         m = collide(g, P);
-    } else { // EQ_OUTFLOW (a6): f_eq(1, u of the inward neighbour at the previous step)
-        const int nb = outflow_neighbour(P, x, y, z);
-        m = Macro<real>{real(1), real(0), real(0), real(0)};
-        if (nb >= 0) {
-            load_cell(g, A, P.stride, nb);
-            m = local_macros(g, flags[nb] & CLASS_MASK, P);
-        }
+    } else { // EQ_OUTFLOW (a6): f_eq(1, u the inward neighbour published while it wrote the state being read)
+        const int k = outflow_owner(P, x, y, z);
+        const int sl = outflow_slot(P, k < 0 ? 0 : k, x, y, z);
+        m = Macro<real>{real(1), fur[sl], fur[P.F + sl], fur[2 * P.F + sl]};
         equilibrium(g, real(0), m.ux, m.uy, m.uz);
     }
     static_for<0, Q>([&](auto ic) {
@@ -115,6 +143,7 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
         if (fl & SLOW_BIT) wall_stores(P, p, lk, st);
         if (fl & EDGE_BIT) ghost_stores(P, x, y, z, lk, st);
     }
+    if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) { fuw[comp * P.F + sl] = v; });
     if constexpr (MEAN) {
         msum[p] += m.ux;
         msum[P.stride + p] += m.uy;
