@@ -123,7 +123,7 @@ Params<real> make_params(const lbm_t *h)
     for (int k = 0; k < 6; ++k) {
         const int axis = k >> 1;
         P.foff[k] = P.F;
-        if (h->face[k] == FACE_EQ_OUTFLOW) P.F += (axis == 0 ? h->ny : h->nx) * (axis == 2 ? h->ny : h->nz);
+        if (h->face[k] == FACE_EQ_OUTFLOW || h->face[k] == FACE_EQ_FIXED) P.F += (axis == 0 ? h->ny : h->nx) * (axis == 2 ? h->ny : h->nz);
     }
     P.tau0 = (real)(3.0 * h->nu0 + 0.5);
     P.Kles = (real)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs);
@@ -339,7 +339,7 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 }
 
 // kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes / load issue order.
-constexpr int N_VARIANTS = 19;
+constexpr int N_VARIANTS = 23;
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
@@ -362,6 +362,10 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         case 16: return launch_step_as<real, 0, true, 128, 8, 3>(h, P, sample);
         case 17: return launch_step_as<real, 0, true, 128, 8, 4>(h, P, sample);
         case 18: return launch_step_as<real, 0, true, 128, 8, 5>(h, P, sample);
+        case 19: return launch_step_as<real, 0, true, 128, 10, 1>(h, P, sample);
+        case 20: return launch_step_as<real, 0, true, 128, 10, 6>(h, P, sample);
+        case 21: return launch_step_as<real, 0, true, 128, 10, 7>(h, P, sample);
+        case 22: return launch_step_as<real, 0, true, 128, 10, 5>(h, P, sample);
         case 14: return launch_step_as<real, 0, false, 256, 4, 1>(h, P, sample);
         case 15: return launch_step_as<real, 0, false, 256, 4, 2>(h, P, sample);
         default: break;

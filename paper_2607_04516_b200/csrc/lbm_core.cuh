@@ -66,8 +66,8 @@ struct Params {
     unsigned nx_magic; // ceil(2^32 / nx) when umulhi(n, nx_magic) == n / nx for all n < nxy + 1024, else 0 (use a division)
     long long stride; // elements between consecutive populations (>= Np, multiple of 64)
     int face[6];
-    int foff[6];      // first slot of each EQ_OUTFLOW face in the outflow-velocity buffer (a6), slots = face-plane cells
-    int F;            // slots in total (0 if there is no outflow face)
+    int foff[6];      // first slot of each EQ face (FIXED or OUTFLOW) in the face-velocity side buffer, slots = face-plane cells
+    int F;            // slots in total (0 if there is no EQ face)
     real tau0, Kles;       // Kles = 18 sqrt(2) Cs^2
     real fcor, h, inv1ph2; // h = fcor/2, 1/(1+h^2)
     real Fx, Fy, Fz;
@@ -305,23 +305,34 @@ __device__ __forceinline__ void store_cell(real *__restrict__ B, const Params<re
     }
 }
 
-// ---- a6: EQ_OUTFLOW cells ---------------------------------------------------------------------------------------------
-// G_{k+1}(c) = f_eq(1, u_loc(G_k, c - n)) (DESIGN.md §3 step 6), n = outward normal of c's owner face = the first
-// EQ_OUTFLOW face it lies on (order x-,x+,y-,y+,z-,z+).  u_loc(G_k, nb) is the velocity the cell nb itself holds while
-// it writes G_k (its collision velocity if FLUID), so nb publishes it into a small double-buffered side array
-// fu[3][F] ("feeds"), and the outflow cell reads 3 values next step instead of gathering nb's 19 populations:
-// no second dependent gather in the warps that contain a face cell.  Slots never fed (nb SOLID, box one cell
-// thick) stay 0 = the u = 0 the rule prescribes.
+// ---- a3 / a6: EQ face cells -------------------------------------------------------------------------------------------
+// Both kinds of EQ cell hold f_eq(1, u) of a velocity that lives in a small side array fu[2 halves][3][F], one slot per
+// face-plane cell of every EQ face:
+//   EQ_FIXED   u = u_b, written (both halves) when the inlet profile / plane is set (DESIGN.md §3 step 5);
+//   EQ_OUTFLOW u = u_loc(G_k, c - n) (step 6), n = outward normal of the cell's owner face.  u_loc(G_k, nb) is the
+//              velocity the cell nb itself holds while it writes G_k (its collision velocity if FLUID), so nb
+//              publishes it ("feeds") into the half that belongs to the buffer it writes, and the outflow cell reads
+//              3 values next step instead of gathering nb's 19 populations.  Slots never fed (nb SOLID, box one
+//              cell thick) stay 0 = the u = 0 the rule prescribes.
+// Every EQ cell re-stores its 19 populations each step: a static cell inside a row would leave its 32-byte sector
+// partially written, and on this HBM a partially written sector costs far more than the bytes (measured: two static
+// cells per 400-cell row cost 10 % of the step).
+// Owner face of an EQ cell = the first face of the matching type it lies on (order x-,x+,y-,y+,z-,z+).
+template <typename real>
+__device__ __forceinline__ int eq_owner(const Params<real> &P, int ftype, int x, int y, int z)
+{
+    if (x == 0 && P.face[0] == ftype) return 0;
+    if (x == P.nx - 1 && P.face[1] == ftype) return 1;
+    if (y == 0 && P.face[2] == ftype) return 2;
+    if (y == P.ny - 1 && P.face[3] == ftype) return 3;
+    if (z == 0 && P.face[4] == ftype) return 4;
+    if (z == P.nz - 1 && P.face[5] == ftype) return 5;
+    return -1;
+}
 template <typename real>
 __device__ __forceinline__ int outflow_owner(const Params<real> &P, int x, int y, int z)
 {
-    if (x == 0 && P.face[0] == FACE_EQ_OUTFLOW) return 0;
-    if (x == P.nx - 1 && P.face[1] == FACE_EQ_OUTFLOW) return 1;
-    if (y == 0 && P.face[2] == FACE_EQ_OUTFLOW) return 2;
-    if (y == P.ny - 1 && P.face[3] == FACE_EQ_OUTFLOW) return 3;
-    if (z == 0 && P.face[4] == FACE_EQ_OUTFLOW) return 4;
-    if (z == P.nz - 1 && P.face[5] == FACE_EQ_OUTFLOW) return 5;
-    return -1;
+    return eq_owner(P, FACE_EQ_OUTFLOW, x, y, z);
 }
 template <typename real>
 __device__ __forceinline__ int outflow_slot(const Params<real> &P, int k, int x, int y, int z)
@@ -329,6 +340,13 @@ __device__ __forceinline__ int outflow_slot(const Params<real> &P, int k, int x,
     const int axis = k >> 1;
     const int j1 = axis == 0 ? y : x, j2 = axis == 2 ? y : z, n1 = axis == 0 ? P.ny : P.nx;
     return P.foff[k] + j2 * n1 + j1;
+}
+// slot of an EQ cell of class cls (EQ_FIXED / EQ_OUTFLOW); 0 if it has none (cannot happen for a voxelised EQ cell)
+template <typename real>
+__device__ __forceinline__ int eq_slot(const Params<real> &P, int cls, int x, int y, int z)
+{
+    const int k = eq_owner(P, cls == EQ_FIXED ? FACE_EQ_FIXED : FACE_EQ_OUTFLOW, x, y, z);
+    return k < 0 ? 0 : outflow_slot(P, k, x, y, z);
 }
 // is (x,y,z) one layer inside some EQ_OUTFLOW face? (superset test used for FEED_BIT)
 template <typename real>

@@ -52,8 +52,8 @@ __global__ void voxelise_kernel(const int32_t *__restrict__ height, uint8_t *__r
 
 // ---- a2: link classification ---------------------------------------------------------------------------------------------
 // FLUID cell: bit i (1..18) of links[p] <=> the pull source of direction i is SOLID in the padded box — exactly
-// "step 4a takes the bounce-back branch" (DESIGN.md §3 step 9).  SOLID cell: bit i <=> slot (i, p) is a mailbox, i.e.
-// the cell p + c_i is FLUID and stores its bounced population there (internal; lbm_get_links reports 0 for it).
+// "step 4a takes the bounce-back branch" (DESIGN.md §3 step 9).  SOLID cell: bit i <=> the cell stores 0 into its slot i
+// every step to complete a 32-byte sector that others write (internal; lbm_get_links reports 0 for it).
 // Adds SLOW / EDGE / FEED / SURF bits to the flag byte in place (class bits are never changed, and readers mask them,
 // so in-place is race-free).
 template <typename real>
@@ -74,17 +74,26 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restric
         });
         if (bits) extra |= SLOW_BIT;
     } else if (cls == SOLID) {
-        static_for<1, Q>([&](auto ic) {
-            constexpr int i = decltype(ic)::value;
-            bits |= (((flags[p + poff<i>(P)] & CLASS_MASK) == FLUID) ? 1u : 0u) << i;
-        });
-        const int s0 = p & ~7; // the 8 cells of this cell's 32-byte sector (FP32)
-        bool live = false;
+        // slot i of this cell must be zero-filled every step iff some cell of its 32-byte sector is written in
+        // population i (a live cell, or a solid cell whose slot i is a neighbour's mailbox) and this one is not
+        const int s0 = p & ~7; // the 8 cells of the sector (FP32; a superset of the FP64 sector)
+        uint32_t written = 0, own = 0;
         for (int q = s0; q < s0 + 8; ++q) {
             const int cq = flags[q] & CLASS_MASK;
-            live |= cq == FLUID || cq == EQ_OUTFLOW;
+            if (cq == FLUID || cq == EQ_OUTFLOW || cq == EQ_FIXED) written |= 0x7FFFFu;
+            else if (cq == SOLID) {
+                uint32_t mb = 0;
+                static_for<1, Q>([&](auto ic) {
+                    constexpr int i = decltype(ic)::value;
+                    const int t = q + poff<i>(P);
+                    if (t >= 0 && t < P.Np) mb |= (((flags[t] & CLASS_MASK) == FLUID) ? 1u : 0u) << i;
+                });
+                written |= mb;
+                if (q == p) own = mb;
+            }
         }
-        if (live) extra |= SURF_BIT;
+        bits = written & ~own;
+        if (bits) extra |= SURF_BIT;
     }
     links[p] = bits;
     if (cls != SOLID) {
@@ -103,12 +112,18 @@ __device__ __forceinline__ void store_cell_both(real *__restrict__ A, real *__re
 {
     store_cell(A, P, p, x, y, z, fl, lk, g);
     store_cell(B, P, p, x, y, z, fl, lk, g);
-    if (fl & FEED_BIT) {
-        const Macro<real> m = local_macros(g, fl & CLASS_MASK, P);
-        outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int s, int comp, real v) {
+    const int cls = fl & CLASS_MASK;
+    if ((fl & FEED_BIT) || cls == EQ_FIXED) {
+        const Macro<real> m = local_macros(g, cls, P);
+        auto w = [&](int s, int comp, real v) {
             fu[comp * P.F + s] = v;
             fu[(3 + comp) * P.F + s] = v;
-        });
+        };
+        if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, w);
+        if (cls == EQ_FIXED) { // the boundary velocity the step kernel re-expands every step
+            const int s = eq_slot(P, EQ_FIXED, x, y, z);
+            w(s, 0, m.ux); w(s, 1, m.uy); w(s, 2, m.uz);
+        }
     }
 }
 

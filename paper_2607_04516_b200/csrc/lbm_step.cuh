@@ -91,29 +91,21 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
         fl = flags[p];
     }
     if constexpr (EXP == 1) fl = 0; // timing experiment: every cell FLUID, no boundary stores
-    if constexpr (EXP >= 2) fl &= CLASS_MASK;                           // timing experiment: classes only, no boundary stores
+    if constexpr (EXP == 6) { if (fl == 0xFF) return; fl = 0; }             // EXP 1 + the flag load and a wait on it
+    if constexpr (EXP == 7) { fl = 0; if (x == 0 || x == P.nx - 1) return; } // EXP 1 + static cells at both row ends (partial sectors)
+    if constexpr (EXP >= 2 && EXP <= 5) fl &= CLASS_MASK;                           // timing experiment: classes only, no boundary stores
     if constexpr (EXP == 3 || EXP == 5) { if ((fl & CLASS_MASK) == EQ_OUTFLOW) return; }   // outflow cells static
     if constexpr (EXP == 4 || EXP == 5) { if ((fl & CLASS_MASK) == SOLID) fl = 0; } // solids compute and store
     const int cls = fl & CLASS_MASK;
     if (cls == SOLID) {
-        // a solid cell that shares a 32-byte sector with live cells completes the sector with zeros in every slot that
-        // is not a neighbour's mailbox: the sector leaves L2 fully written, no DRAM fill read (same bytes written)
+        // a solid cell whose 32-byte sector is written by others (live cells, neighbours' mailboxes) completes it with
+        // zeros: the sector leaves L2 fully written, no DRAM read-modify-write (same bytes written either way)
         if (fl & SURF_BIT) {
             const uint32_t mk = links[p];
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
-                if (!((mk >> i) & 1u)) st_pop<HINT>(T.dst[i] + p, real(0));
+                if ((mk >> i) & 1u) st_pop<HINT>(T.dst[i] + p, real(0));
             });
-        }
-        return;
-    }
-    if (cls == EQ_FIXED) {
-        if constexpr (MEAN) {
-            load_cell(g, A, P.stride, p);
-            const Macro<real> m = local_macros(g, EQ_FIXED, P);
-            msum[p] += m.ux;
-            msum[P.stride + p] += m.uy;
-            msum[2 * P.stride + p] += m.uz;
         }
         return;
     }
@@ -128,9 +120,8 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
             });
         }
         m = collide(g, P);
-    } else { // EQ_OUTFLOW (a6): f_eq(1, u the inward neighbour published while it wrote the state being read)
-        const int k = outflow_owner(P, x, y, z);
-        const int sl = outflow_slot(P, k < 0 ? 0 : k, x, y, z);
+    } else { // EQ_FIXED (a3) / EQ_OUTFLOW (a6): f_eq(1, u) of the cell's face velocity (lbm_core.cuh)
+        const int sl = eq_slot(P, cls, x, y, z);
         m = Macro<real>{real(1), fur[sl], fur[P.F + sl], fur[2 * P.F + sl]};
         equilibrium(g, real(0), m.ux, m.uy, m.uz);
     }
