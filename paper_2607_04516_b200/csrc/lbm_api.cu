@@ -339,7 +339,7 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 }
 
 // kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes / load issue order.
-constexpr int N_VARIANTS = 23;
+constexpr int N_VARIANTS = 11;
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
@@ -351,23 +351,11 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         case 3: return launch_step_as<real, 0, true, 128, 8>(h, P, sample);
         case 4: return launch_step_as<real, 0, true, 128, 9>(h, P, sample);
         case 5: return launch_step_as<real, 0, false, 256, 4>(h, P, sample);
-        case 6: return launch_step_as<real, 0, true, 128, 11>(h, P, sample);
-        case 7: return launch_step_as<real, 0, true, 128, 12>(h, P, sample);
-        case 8: return launch_step_as<real, 0, true, 128, 14>(h, P, sample);
+        case 6: return launch_step_as<real, 0, true, 256, 5>(h, P, sample);
+        case 7: return launch_step_as<real, 2, true, 128, 10>(h, P, sample);
+        case 8: return launch_step_as<real, 0, true, 96, 13>(h, P, sample);
         case 9: return launch_step_as<real, 0, true, 64, 20>(h, P, sample);
-        case 10: return launch_step_as<real, 0, true, 256, 4, 1>(h, P, sample);
-        case 11: return launch_step_as<real, 0, true, 128, 8, 1>(h, P, sample);
-        case 12: return launch_step_as<real, 0, true, 256, 4, 2>(h, P, sample);
-        case 13: return launch_step_as<real, 0, true, 128, 8, 2>(h, P, sample);
-        case 16: return launch_step_as<real, 0, true, 128, 8, 3>(h, P, sample);
-        case 17: return launch_step_as<real, 0, true, 128, 8, 4>(h, P, sample);
-        case 18: return launch_step_as<real, 0, true, 128, 8, 5>(h, P, sample);
-        case 19: return launch_step_as<real, 0, true, 128, 10, 1>(h, P, sample);
-        case 20: return launch_step_as<real, 0, true, 128, 10, 6>(h, P, sample);
-        case 21: return launch_step_as<real, 0, true, 128, 10, 7>(h, P, sample);
-        case 22: return launch_step_as<real, 0, true, 128, 10, 5>(h, P, sample);
-        case 14: return launch_step_as<real, 0, false, 256, 4, 1>(h, P, sample);
-        case 15: return launch_step_as<real, 0, false, 256, 4, 2>(h, P, sample);
+        case 10: return launch_step_as<real, 0, true, 128, 10, 1>(h, P, sample);
         default: break;
         }
     }

@@ -26,7 +26,7 @@ enum : int { FLUID = 0, SOLID = 1, EQ_FIXED = 2, EQ_OUTFLOW = 3, GHOST = 4 };
 enum : int { PERIODIC = 0, WALL = 1, FREE_SLIP = 2, FACE_EQ_FIXED = 3, FACE_EQ_OUTFLOW = 4 };
 constexpr uint8_t CLASS_MASK = 7;
 constexpr uint8_t SLOW_BIT = 0x80; // FLUID cell with at least one wall link (mailbox stores needed)
-constexpr uint8_t EDGE_BIT = 0x40; // non-solid cell on a domain face (ghost stores may be needed)
+constexpr uint8_t EDGE_BIT = 0x40; // non-solid cell on a domain face that has at least one ghost slot to store
 constexpr uint8_t FEED_BIT = 0x20; // non-solid cell one layer inside an EQ_OUTFLOW face: publishes its velocity (a6)
 constexpr uint8_t SURF_BIT = 0x10; // SOLID cell sharing a 32-byte sector with a cell that is rewritten every step
 

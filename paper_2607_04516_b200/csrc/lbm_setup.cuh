@@ -97,8 +97,11 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restric
     }
     links[p] = bits;
     if (cls != SOLID) {
+        // EDGE_BIT only where the ghost rule really stores something (not e.g. on the WALL ground or mid-face EQ cells)
         const bool edge = x == 0 || x == P.nx - 1 || y == 0 || y == P.ny - 1 || z == 0 || z == P.nz - 1;
-        if (edge) extra |= EDGE_BIT;
+        int nghost = 0;
+        if (edge) ghost_stores(P, x, y, z, bits, [&](int, int, auto) { ++nghost; });
+        if (nghost) extra |= EDGE_BIT;
         if (outflow_feeder(P, x, y, z)) extra |= FEED_BIT;
     }
     flags[p] = (uint8_t)(cls | extra);

@@ -81,37 +81,34 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
 
     real g[Q];
     uint8_t fl;
+    real fu0 = real(0), fu1 = real(0), fu2 = real(0); // face velocity of an EQ cell
     if constexpr (SPEC) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             g[i] = ld_pinned(T.src[i] + p);
         });
+        // a cell on an EQ face fetches its face velocity now, from geometry alone (EQ_FIXED wins, as in the voxeliser);
+        // if the flag then says SOLID the three values are simply not used
+        if (P.F > 0) {
+            int k = eq_owner(P, FACE_EQ_FIXED, x, y, z);
+            if (k < 0) k = eq_owner(P, FACE_EQ_OUTFLOW, x, y, z);
+            if (k >= 0) {
+                const int sl = outflow_slot(P, k, x, y, z);
+                fu0 = ld_pinned(fur + sl); fu1 = ld_pinned(fur + P.F + sl); fu2 = ld_pinned(fur + 2 * P.F + sl);
+            }
+        }
         fl = ld_pinned(flags + p); // volatile asm statements keep their order: the flag test cannot move above the pulls
     } else {
         fl = flags[p];
     }
     if constexpr (EXP == 1) fl = 0; // timing experiment: every cell FLUID, no boundary stores
-    if constexpr (EXP == 6) { if (fl == 0xFF) return; fl = 0; }             // EXP 1 + the flag load and a wait on it
-    if constexpr (EXP == 7) { fl = 0; if (x == 0 || x == P.nx - 1) return; } // EXP 1 + static cells at both row ends (partial sectors)
-    if constexpr (EXP >= 2 && EXP <= 5) fl &= CLASS_MASK;                           // timing experiment: classes only, no boundary stores
-    if constexpr (EXP == 3 || EXP == 5) { if ((fl & CLASS_MASK) == EQ_OUTFLOW) return; }   // outflow cells static
-    if constexpr (EXP == 4 || EXP == 5) { if ((fl & CLASS_MASK) == SOLID) fl = 0; } // solids compute and store
     const int cls = fl & CLASS_MASK;
-    if (cls == SOLID) {
-        // a solid cell whose 32-byte sector is written by others (live cells, neighbours' mailboxes) completes it with
-        // zeros: the sector leaves L2 fully written, no DRAM read-modify-write (same bytes written either way)
-        if (fl & SURF_BIT) {
-            const uint32_t mk = links[p];
-            static_for<0, Q>([&](auto ic) {
-                constexpr int i = decltype(ic)::value;
-                if ((mk >> i) & 1u) st_pop<HINT>(T.dst[i] + p, real(0));
-            });
-        }
-        return;
-    }
+    // link word: wall links of a FLUID cell / zero-fill mask of a surface SOLID cell; one predicated load for both,
+    // issued as soon as the flag is there and consumed only after the collision
     uint32_t lk = 0;
-    if (fl & SLOW_BIT) lk = links[p];
-    Macro<real> m;
+    if (fl & (SLOW_BIT | SURF_BIT)) lk = links[p];
+    if (cls == SOLID && !(fl & SURF_BIT)) return;
+    Macro<real> m{real(1), real(0), real(0), real(0)};
     if (cls == FLUID) {
         if constexpr (!SPEC) {
             static_for<0, Q>([&](auto ic) {
@@ -120,20 +117,36 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
             });
         }
         m = collide(g, P);
-    } else { // EQ_FIXED (a3) / EQ_OUTFLOW (a6): f_eq(1, u) of the cell's face velocity (lbm_core.cuh)
-        const int sl = eq_slot(P, cls, x, y, z);
-        m = Macro<real>{real(1), fur[sl], fur[P.F + sl], fur[2 * P.F + sl]};
+    } else if (cls != SOLID) { // EQ_FIXED (a3) / EQ_OUTFLOW (a6): f_eq(1, u) of the cell's face velocity (lbm_core.cuh)
+        if constexpr (!SPEC) {
+            const int sl = eq_slot(P, cls, x, y, z);
+            fu0 = fur[sl]; fu1 = fur[P.F + sl]; fu2 = fur[2 * P.F + sl];
+        }
+        m = Macro<real>{real(1), fu0, fu1, fu2};
         equilibrium(g, real(0), m.ux, m.uy, m.uz);
+    }
+    if (cls == SOLID) {
+        // a solid cell whose 32-byte sector is written by others (live cells, neighbours' mailboxes) completes it with
+        // zeros: the sector leaves L2 fully written, no DRAM read-modify-write (same bytes written either way)
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            if ((lk >> i) & 1u) st_pop<HINT>(T.dst[i] + p, real(0));
+        });
+        return;
     }
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         st_pop<HINT>(T.dst[i] + p, g[i]);
     });
-    if (fl & (SLOW_BIT | EDGE_BIT)) {
-        auto st = [&](int i, int pt, auto jc) { B[(long long)i * P.stride + pt] = g[decltype(jc)::value]; };
-        if (fl & SLOW_BIT) wall_stores(P, p, lk, st);
-        if (fl & EDGE_BIT) ghost_stores(P, x, y, z, lk, st);
+    if (fl & SLOW_BIT) {
+        // wall links (lbm_core.cuh wall_stores, with the launch's address table): slot (i, p - off_i) <- g[opp(i)]
+        static_for<1, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            if ((lk >> i) & 1u) T.dst[i][p - poff<i>(P)] = g[dir_opp(i)];
+        });
     }
+    if (fl & EDGE_BIT)
+        ghost_stores(P, x, y, z, lk, [&](int i, int pt, auto jc) { B[(long long)i * P.stride + pt] = g[decltype(jc)::value]; });
     if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) { fuw[comp * P.F + sl] = v; });
     if constexpr (MEAN) {
         msum[p] += m.ux;
