@@ -39,14 +39,18 @@ def load_peak():
 
 
 def load_traffic():
-    """dram bytes per launch of the step kernel from the committed ncu summary, if any (profiles/roofline_traffic.json)."""
-    p = os.path.join(ROOT, "profiles", "roofline_traffic.json")
-    if os.path.exists(p):
-        try:
-            return float(json.load(open(p))["dram_bytes_per_launch"])
-        except Exception:
-            return None
-    return None
+    """DRAM bytes per launch of the step kernel (dram__bytes_read.sum + dram__bytes_write.sum of the committed
+    `ncu --set full` capture): last data row of the newest profiles/r*_step_kernel_traffic.csv; None if absent."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_step_kernel_traffic.csv")))
+    if not files:
+        return None
+    try:
+        rows = list(csv.DictReader(open(files[-1])))
+        return float(rows[-1]["dram_bytes_total"])
+    except Exception:
+        return None
 
 
 class ClockSampler:
@@ -95,6 +99,22 @@ class ClockSampler:
         return out
 
 
+def max_over_ranks(value, world, device):
+    """Whole-job time = the slowest rank's device time (MAX all-reduce; identity for one rank)."""
+    if world <= 1:
+        return float(value)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_mlups(cells_per_rank, steps, world, seconds):
+    """Replicas only: every rank advances its own lattice; the job's units are the sum over ranks."""
+    return cells_per_rank * steps * world / seconds / 1e6
+
+
 def oracle_for(wl):
     from oracle import Oracle
     o = Oracle(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces)
@@ -125,7 +145,7 @@ def run_reference(args):
         return 0
     from paper_2607_04516_b200 import workloads as W
     cores = len(os.sched_getaffinity(0))
-    budget = 150.0
+    budget = float(args.reference_budget)
     nz = 25
     wl = W.config3(nz=nz)
     o = oracle_for(wl)
@@ -201,11 +221,8 @@ def run_ours(args):
     clocks = sampler.stop() if rank == 0 else None
     rho, ux, uy, uz = sim.get_macros()
     finite = bool(torch.isfinite(ux).all().item())
-    t = torch.tensor([best], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
-    mlups = wl.cells * K * world / (ms_total * 1e-3) / 1e6
+    ms_total = max_over_ranks(best, world, dev)
+    mlups = job_mlups(wl.cells, K, world, ms_total * 1e-3)
 
     # ---------------- end to end through the C ABI with pinned host buffers
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()  # noqa: E731
@@ -228,13 +245,10 @@ def run_ours(args):
     e1.record()
     barrier()
     wall = time.perf_counter() - t0
-    t = torch.tensor([max(e0.elapsed_time(e1) * 1e-3, wall)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_s = float(t.item())
+    e2e_s = max_over_ranks(max(e0.elapsed_time(e1) * 1e-3, wall), world, dev)
     h2d = h_height.nbytes + h_u.nbytes + h_ux0.nbytes
     d2h = sum(o.numel() * 4 for o in outs)
-    e2e = {"value": wl.cells * K * world / e2e_s / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": h2d / K,
+    e2e = {"value": job_mlups(wl.cells, K, world, e2e_s), "unit": "MLUPS", "h2d_bytes_per_step": h2d / K,
            "d2h_bytes_per_step": d2h / K,
            "what": f"one job = set_flags + set_inlet_profile + set_macros from pinned host buffers, lbm_step({K}), "
                    "lbm_get_macros into pinned host buffers"}
@@ -277,6 +291,7 @@ def main():
     ap.add_argument("--repeats", type=int, default=1, help="timed repetitions of the K-step region; best is reported")
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--reference-budget", type=float, default=150.0, help="seconds of CPU time the reference arm may use")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
