@@ -81,7 +81,7 @@ static int opposite(int i) { return OPP[i]; }
 
 typedef struct oracle {
     int nx, ny, nz;
-    double nu0, Cs, fcor, F[3];
+    double nu0, Cs, fv[3], F[3]; /* fv = Coriolis vector f = 2 Omega (lattice units); scalar f_cor = fv[2] */
     int face[6]; /* x-,x+,y-,y+,z-,z+ */
     int have_flags;
     uint8_t *cls; /* [z][y][x] */
@@ -111,7 +111,35 @@ static void feq(double rho, const double u[3], double out[Q])
 
 /* step 4b-4e on one cell: pulled populations f[] -> post-collision g[].
  * Also returns the (rho,u,tau) the collision used. */
-static void collide(const double f[Q], double nu0, double Cs, double fcor, const double F[3],
+/* Solve the 3x3 system M x = r by Cramer's rule (M is I +- C/2 with C skew: always regular). */
+static void solve3(const double M[3][3], const double r[3], double x[3])
+{
+    double det = M[0][0] * (M[1][1] * M[2][2] - M[1][2] * M[2][1])
+               - M[0][1] * (M[1][0] * M[2][2] - M[1][2] * M[2][0])
+               + M[0][2] * (M[1][0] * M[2][1] - M[1][1] * M[2][0]);
+    for (int k = 0; k < 3; ++k) {
+        double N[3][3];
+        for (int a = 0; a < 3; ++a)
+            for (int c = 0; c < 3; ++c) N[a][c] = (c == k) ? r[a] : M[a][c];
+        double dk = N[0][0] * (N[1][1] * N[2][2] - N[1][2] * N[2][1])
+                  - N[0][1] * (N[1][0] * N[2][2] - N[1][2] * N[2][0])
+                  + N[0][2] * (N[1][0] * N[2][1] - N[1][1] * N[2][0]);
+        x[k] = dk / det;
+    }
+}
+
+/* Coriolis acceleration of the full rotation vector (Table 1: "full rotation vector in the
+ * local ENU frame"): a_cor(u) = -2 Omega x u = -fv x u = C u with fv = 2 Omega and
+ *     C = [[0, fz, -fy], [-fz, 0, fx], [fy, -fx, 0]].
+ * fv = (0, 0, f) gives the scalar reading a_cor = f (u_y, -u_x, 0) of DESIGN.md §4 reading 5. */
+static void coriolis_matrix(const double fv[3], double Cm[3][3])
+{
+    Cm[0][0] = 0.0;    Cm[0][1] = fv[2];  Cm[0][2] = -fv[1];
+    Cm[1][0] = -fv[2]; Cm[1][1] = 0.0;    Cm[1][2] = fv[0];
+    Cm[2][0] = fv[1];  Cm[2][1] = -fv[0]; Cm[2][2] = 0.0;
+}
+
+static void collide(const double f[Q], double nu0, double Cs, const double fv[3], const double F[3],
                     double g[Q], double *rho_out, double u_out[3], double *tau_out)
 {
     /* 4b moments */
@@ -120,18 +148,17 @@ static void collide(const double f[Q], double nu0, double Cs, double fcor, const
         rho += f[i];
         for (int a = 0; a < 3; ++a) m[a] += CI[i][a] * f[i];
     }
-    /* 4c implicit half-force velocity: rho u = m + rho a(u)/2,
-     * a(u) = F + fcor (u_y, -u_x, 0) */
-    double h = 0.5 * fcor;
+    /* 4c implicit half-force velocity: rho u = m + rho a(u)/2, a(u) = F + C u
+     * => (I - C/2) u = m/rho + F/2 */
+    double Cm[3][3], M[3][3];
+    coriolis_matrix(fv, Cm);
+    for (int a = 0; a < 3; ++a)
+        for (int c = 0; c < 3; ++c) M[a][c] = (a == c ? 1.0 : 0.0) - 0.5 * Cm[a][c];
     double b[3] = {m[0] / rho + 0.5 * F[0], m[1] / rho + 0.5 * F[1], m[2] / rho + 0.5 * F[2]};
     double u[3];
-    u[0] = (b[0] + h * b[1]) / (1.0 + h * h);
-    u[1] = (b[1] - h * b[0]) / (1.0 + h * h);
-    u[2] = b[2];
+    solve3(M, b, u);
     double Fd[3]; /* force density rho a(u) */
-    Fd[0] = rho * (F[0] + fcor * u[1]);
-    Fd[1] = rho * (F[1] - fcor * u[0]);
-    Fd[2] = rho * F[2];
+    for (int a = 0; a < 3; ++a) Fd[a] = rho * (F[a] + Cm[a][0] * u[0] + Cm[a][1] * u[1] + Cm[a][2] * u[2]);
     /* 4d LES: Pi = sum c c (f - feq); Q = Frobenius norm over all 9 entries */
     double fe[Q];
     feq(rho, u, fe);
@@ -199,12 +226,13 @@ static void local_macros(const oracle_t *o, const double *Gs, long cell, double 
     }
     *rho = r;
     if (cl == C_FLUID) {
-        /* invert m* = rho u + rho a(u)/2 */
-        double h = 0.5 * o->fcor;
+        /* invert m* = rho u + rho a(u)/2, a(u) = F + C u  =>  (I + C/2) u = m* / rho - F/2 */
+        double Cm[3][3], M[3][3];
+        coriolis_matrix(o->fv, Cm);
+        for (int a = 0; a < 3; ++a)
+            for (int c = 0; c < 3; ++c) M[a][c] = (a == c ? 1.0 : 0.0) + 0.5 * Cm[a][c];
         double b[3] = {m[0] / r - 0.5 * o->F[0], m[1] / r - 0.5 * o->F[1], m[2] / r - 0.5 * o->F[2]};
-        u[0] = (b[0] - h * b[1]) / (1.0 + h * h);
-        u[1] = (b[1] + h * b[0]) / (1.0 + h * h);
-        u[2] = b[2];
+        solve3(M, b, u);
     } else {
         u[0] = m[0] / r; u[1] = m[1] / r; u[2] = m[2] / r;
     }
@@ -228,7 +256,16 @@ int oracle_feq(double rho, const double *u, double *out) { feq(rho, u, out); ret
 int oracle_collide_cell(const double *f, double nu0, double Cs, double fcor, const double *F,
                         double *g, double *rho, double *u, double *tau)
 {
-    collide(f, nu0, Cs, fcor, F, g, rho, u, tau);
+    const double fv[3] = {0.0, 0.0, fcor};
+    collide(f, nu0, Cs, fv, F, g, rho, u, tau);
+    return 0;
+}
+
+/* same with the full Coriolis vector fv = 2 Omega */
+int oracle_collide_cell_vec(const double *f, double nu0, double Cs, const double *fv, const double *F,
+                            double *g, double *rho, double *u, double *tau)
+{
+    collide(f, nu0, Cs, fv, F, g, rho, u, tau);
     return 0;
 }
 
@@ -239,7 +276,7 @@ oracle_t *oracle_create(int nx, int ny, int nz, double nu0, double Cs, double fc
     oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
     if (!o) return NULL;
     o->nx = nx; o->ny = ny; o->nz = nz;
-    o->nu0 = nu0; o->Cs = Cs; o->fcor = fcor;
+    o->nu0 = nu0; o->Cs = Cs; o->fv[0] = 0.0; o->fv[1] = 0.0; o->fv[2] = fcor;
     for (int a = 0; a < 3; ++a) o->F[a] = F ? F[a] : 0.0;
     /* default faces = config 1 */
     o->face[0] = F_EQ_FIXED; o->face[1] = F_EQ_OUTFLOW;
@@ -259,6 +296,14 @@ void oracle_destroy(oracle_t *o)
 {
     if (!o) return;
     free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o);
+}
+
+/* Coriolis vector f = 2 Omega in lattice units; replaces the scalar given at creation */
+int oracle_set_coriolis(oracle_t *o, const double *fv)
+{
+    if (!o || !fv) return -1;
+    for (int a = 0; a < 3; ++a) o->fv[a] = fv[a];
+    return 0;
 }
 
 int oracle_set_boundaries(oracle_t *o, const int *face_type)
@@ -442,7 +487,7 @@ int oracle_step(oracle_t *o, int nsteps)
                             if (r < 0) { bad = 1; r = 1; }
                             f[i] = r ? o->G[cell * Q + opposite(i)] : o->G[s * Q + j];
                         }
-                        collide(f, o->nu0, o->Cs, o->fcor, o->F, gn, NULL, NULL, NULL);
+                        collide(f, o->nu0, o->Cs, o->fv, o->F, gn, NULL, NULL, NULL);
                     } else if (cl == C_EQ_OUTFLOW) {
                         /* step 6 */
                         int k = outflow_face(o, x, y, z);

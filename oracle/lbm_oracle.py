@@ -47,7 +47,8 @@ def _load():
     for name in ("oracle_set_boundaries", "oracle_set_flags", "oracle_get_flags", "oracle_get_links",
                  "oracle_set_inlet_profile", "oracle_set_inlet_plane", "oracle_set_macros", "oracle_step",
                  "oracle_get_macros", "oracle_mean_reset", "oracle_get_mean",
-                 "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell"):
+                 "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell",
+                 "oracle_collide_cell_vec", "oracle_set_coriolis"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -93,6 +94,21 @@ def collide_cell(f, nu0, Cs, fcor, F):
     return g, rho.value, u, tau.value
 
 
+def collide_cell_vec(f, nu0, Cs, fvec, F):
+    """One cell's step 4b-4e with the full Coriolis vector f = 2 Omega.  Returns (g[19], rho, u[3], tau)."""
+    lib = _load()
+    f, fp = _d(f)
+    F, Fp = _d(np.asarray(F, dtype=np.float64))
+    fv, fvp = _d(np.asarray(fvec, dtype=np.float64))
+    g = np.zeros(19)
+    rho = C.c_double()
+    u = np.zeros(3)
+    tau = C.c_double()
+    lib.oracle_collide_cell_vec(fp, C.c_double(nu0), C.c_double(Cs), fvp, Fp,
+                                g.ctypes.data_as(C.c_void_p), C.byref(rho), u.ctypes.data_as(C.c_void_p), C.byref(tau))
+    return g, rho.value, u, tau.value
+
+
 class Oracle:
     """FP64 CPU LBM; same call names as the product binding, float64 arrays."""
 
@@ -120,6 +136,11 @@ class Oracle:
     def _chk(self, rc, what):
         if rc != 0:
             raise RuntimeError(f"oracle {what} failed: {rc}")
+
+    def set_coriolis(self, fvec):
+        """Full Coriolis vector f = 2 Omega (lattice units); (0, 0, f_cor) is the scalar form."""
+        a, ap = _d(np.asarray(fvec, dtype=np.float64).reshape(3))
+        self._chk(self._lib.oracle_set_coriolis(C.c_void_p(self._h), ap), "set_coriolis")
 
     def set_boundaries(self, faces):
         a = np.ascontiguousarray(faces, dtype=np.int32)
