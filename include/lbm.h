@@ -76,6 +76,12 @@ int lbm_destroy(lbm_t *h);
 /* Face types, order x-,x+,y-,y+,z-,z+.  Invalidates the flags: call lbm_set_flags afterwards. */
 int lbm_set_boundaries(lbm_t *h, const int face_type[6]);
 
+/* Full Coriolis rotation vector (Table 1: "full rotation vector in the local ENU frame ...
+ * evaluated directly within the GPU kernel"): f = 2 Omega in lattice units (rad per step), host pointer; the
+ * acceleration is -f x u, applied through Guo forcing with the implicit half-force velocity (DESIGN.md §3 step 4c).
+ * lbm_create's scalar f_cor is the vector (0, 0, f_cor).  Takes effect at the next lbm_step; may be called at any time. */
+int lbm_set_coriolis(lbm_t *h, const double f[3]);
+
 /* Voxelise ("solid mask"; heightmap form per north_star): cell (x,y,z) is SOLID iff
  * z < clamp(height[y][x], 0, nz); non-solid cells on an EQ face take the EQ class (EQ_FIXED wins);
  * then classify the wall links of every FLUID cell.  Integer work, done on the device.

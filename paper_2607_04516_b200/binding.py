@@ -26,7 +26,7 @@ SYMBOLS = [
     "lbm_feed_inlet", "lbm_set_macros", "lbm_set_macros_f64", "lbm_step", "lbm_mean_config", "lbm_mean_reset",
     "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
     "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
-    "lbm_launch_count", "lbm_lattice", "lbm_set_variant",
+    "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis",
 ]
 
 
@@ -53,6 +53,7 @@ def load_library():
     lib.lbm_create_ex.argtypes = [i, i, i, d, d, d, vp, vp, C.c_size_t, vp, i, i, C.POINTER(vp)]
     lib.lbm_destroy.argtypes = [vp]
     lib.lbm_set_boundaries.argtypes = [vp, vp]
+    lib.lbm_set_coriolis.argtypes = [vp, vp]
     lib.lbm_set_flags.argtypes = [vp, vp]
     for n in ("lbm_set_inlet_profile", "lbm_set_inlet_profile_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
@@ -169,6 +170,13 @@ class Lbm:
         if a.shape != (6,):
             raise ValueError("faces must have 6 entries")
         self._chk(self._lib.lbm_set_boundaries(self._h, a.ctypes.data), "set_boundaries")
+
+    def set_coriolis(self, f):
+        """Full Coriolis vector f = 2 Omega in lattice units; (0, 0, f_cor) is the scalar form of the constructor."""
+        a = np.ascontiguousarray(f, dtype=np.float64)
+        if a.shape != (3,):
+            raise ValueError("f must have 3 entries")
+        self._chk(self._lib.lbm_set_coriolis(self._h, a.ctypes.data), "set_coriolis")
 
     def set_flags(self, height=None):
         k, p = _ptr(height, np.int32)

@@ -63,7 +63,7 @@ bool size_ok(int nx, int ny, int nz)
 
 struct lbm {
     int nx, ny, nz;
-    double nu0, Cs, fcor, F[3];
+    double nu0, Cs, fv[3], F[3]; // fv = Coriolis vector f = 2 Omega; lbm_create's scalar f_cor is fv[2]
     int face[6];
     int fp64, want_mean;
     Layout L;
@@ -127,9 +127,9 @@ Params<real> make_params(const lbm_t *h)
     }
     P.tau0 = (real)(3.0 * h->nu0 + 0.5);
     P.Kles = (real)(18.0 * std::sqrt(2.0) * h->Cs * h->Cs);
-    P.fcor = (real)h->fcor;
-    P.h = (real)(0.5 * h->fcor);
-    P.inv1ph2 = (real)(1.0 / (1.0 + 0.25 * h->fcor * h->fcor));
+    P.fx = (real)h->fv[0]; P.fy = (real)h->fv[1]; P.fz = (real)h->fv[2];
+    P.hx = (real)(0.5 * h->fv[0]); P.hy = (real)(0.5 * h->fv[1]); P.hz = (real)(0.5 * h->fv[2]);
+    P.inv1ph2 = (real)(1.0 / (1.0 + 0.25 * (h->fv[0] * h->fv[0] + h->fv[1] * h->fv[1] + h->fv[2] * h->fv[2])));
     P.Fx = (real)h->F[0]; P.Fy = (real)h->F[1]; P.Fz = (real)h->F[2];
     return P;
 }
@@ -499,7 +499,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     lbm_t *h = new (std::nothrow) lbm();
     if (!h) return LBM_ENOMEM;
     h->nx = nx; h->ny = ny; h->nz = nz;
-    h->nu0 = nu0; h->Cs = Cs; h->fcor = f_cor;
+    h->nu0 = nu0; h->Cs = Cs; h->fv[0] = 0.0; h->fv[1] = 0.0; h->fv[2] = f_cor;
     for (int a = 0; a < 3; ++a) h->F[a] = F ? F[a] : 0.0;
     const int def[6] = {LBM_EQ_FIXED, LBM_EQ_OUTFLOW, LBM_PERIODIC, LBM_PERIODIC, LBM_WALL, LBM_FREE_SLIP};
     for (int k = 0; k < 6; ++k) h->face[k] = def[k];
@@ -549,6 +549,16 @@ int lbm_set_boundaries(lbm_t *h, const int face_type[6])
     }
     for (int k = 0; k < 6; ++k) h->face[k] = face_type[k];
     h->have_flags = false;
+    return LBM_OK;
+}
+
+int lbm_set_coriolis(lbm_t *h, const double f[3])
+{
+    if (!h) return LBM_EINVAL;
+    if (!f) return fail(h, LBM_EINVAL, "set_coriolis: NULL");
+    for (int a = 0; a < 3; ++a)
+        if (!std::isfinite(f[a])) return fail(h, LBM_EINVAL, "set_coriolis: not finite");
+    for (int a = 0; a < 3; ++a) h->fv[a] = f[a];
     return LBM_OK;
 }
 

@@ -69,7 +69,8 @@ struct Params {
     int foff[6];      // first slot of each EQ face (FIXED or OUTFLOW) in the face-velocity side buffer, slots = face-plane cells
     int F;            // slots in total (0 if there is no EQ face)
     real tau0, Kles;       // Kles = 18 sqrt(2) Cs^2
-    real fcor, h, inv1ph2; // h = fcor/2, 1/(1+h^2)
+    real fx, fy, fz;       // Coriolis vector f = 2 Omega; the scalar f_cor of lbm_create is fz
+    real hx, hy, hz, inv1ph2; // h = f/2, 1/(1+|h|^2)
     real Fx, Fy, Fz;
 };
 
@@ -125,12 +126,16 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
     const real Mxy = s[4] - s[7], Mxz = s[5] - s[8], Myz = s[6] - s[9];
     const real rho = real(1) + drho;
     const real inv = real(1) / rho;
-    // 4c: implicit half-force velocity
+    // 4c: implicit half-force velocity.  a(u) = F - f x u, so rho u = m + rho a(u)/2 reads u + h x u = b with h = f/2,
+    // b = m/rho + F/2, whose solution is u = (b - h x b + h (h.b)) / (1 + |h|^2)
     const real bx = mx * inv + real(0.5) * P.Fx, by = my * inv + real(0.5) * P.Fy, bz = mz * inv + real(0.5) * P.Fz;
-    const real ux = (bx + P.h * by) * P.inv1ph2;
-    const real uy = (by - P.h * bx) * P.inv1ph2;
-    const real uz = bz;
-    const real Fdx = rho * (P.Fx + P.fcor * uy), Fdy = rho * (P.Fy - P.fcor * ux), Fdz = rho * P.Fz;
+    const real hb = P.hx * bx + P.hy * by + P.hz * bz;
+    const real ux = (bx - (P.hy * bz - P.hz * by) + P.hx * hb) * P.inv1ph2;
+    const real uy = (by - (P.hz * bx - P.hx * bz) + P.hy * hb) * P.inv1ph2;
+    const real uz = (bz - (P.hx * by - P.hy * bx) + P.hz * hb) * P.inv1ph2;
+    const real Fdx = rho * (P.Fx - (P.fy * uz - P.fz * uy));
+    const real Fdy = rho * (P.Fy - (P.fz * ux - P.fx * uz));
+    const real Fdz = rho * (P.Fz - (P.fx * uy - P.fy * ux));
     // 4d: Pi = sum c c (f - feq) = M - (drho/3) I - rho u u   (second moment of the shifted equilibrium is exact)
     const real third = real(1) / real(3);
     const real Pxx = Mxx - third * drho - rho * ux * ux;
@@ -209,8 +214,12 @@ __device__ __forceinline__ Macro<real> local_macros(const real (&g)[Q], int cls,
     const real rho = real(1) + drho;
     const real inv = real(1) / rho;
     if (cls == FLUID) {
+        // m*/rho - F/2 = u - h x u  =>  u = (b + h x b + h (h.b)) / (1 + |h|^2)
         const real bx = mx * inv - real(0.5) * P.Fx, by = my * inv - real(0.5) * P.Fy, bz = mz * inv - real(0.5) * P.Fz;
-        return Macro<real>{rho, (bx - P.h * by) * P.inv1ph2, (by + P.h * bx) * P.inv1ph2, bz};
+        const real hb = P.hx * bx + P.hy * by + P.hz * bz;
+        return Macro<real>{rho, (bx + (P.hy * bz - P.hz * by) + P.hx * hb) * P.inv1ph2,
+                           (by + (P.hz * bx - P.hx * bz) + P.hy * hb) * P.inv1ph2,
+                           (bz + (P.hx * by - P.hy * bx) + P.hz * hb) * P.inv1ph2};
     }
     return Macro<real>{rho, mx * inv, my * inv, mz * inv};
 }

@@ -392,3 +392,65 @@ def test_every_step_kernel_variant_matches_the_oracle(B, variant, shape):
         em = max(float(np.abs(a.cpu().numpy().astype(np.float64) - b).max()) for a, b in zip(gm, om))
         assert em <= TOL32, (variant, shape, faces, em)
         sim.close()
+
+
+# ---------------------------------------------------------------------------------------------- full Coriolis vector
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_full_coriolis_vector_matches_the_oracle(B, fp64):
+    """PAPER.md:61 / Table 1: full rotation vector through Guo forcing.  Tilted axis, buildings, every face
+    rule, forcing, LES; 100 steps; FP32 within 1e-5, FP64 within rounding order."""
+    from oracle import Oracle
+    nx, ny, nz = 48, 40, 24
+    rng = np.random.default_rng(77)
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    for _ in range(5):
+        x0, y0 = int(rng.integers(4, nx - 10)), int(rng.integers(0, ny - 4))
+        hm[y0:y0 + 4, x0:x0 + 5] = int(rng.integers(1, nz - 4))
+    prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+    fv = (1.5e-3, -1.0e-3, 2.0e-3)
+    for faces in [(3, 4, 2, 2, 1, 2), (0, 0, 0, 0, 1, 2)]:
+        args = (nx, ny, nz, 2e-3, 0.1, 5e-4, (1e-6, -5e-7, 0.0), faces)
+        o = Oracle(*args)
+        o.set_coriolis(fv)
+        o.set_flags(hm)
+        o.set_inlet_profile(prof, 0.2 * prof, None)
+        ux0 = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+        o.set_macros(None, ux0, None, None)
+        sim = B.Lbm(*args, fp64=fp64)
+        sim.set_coriolis(fv)
+        sim.set_flags(hm)
+        sim.set_inlet_profile(prof, 0.2 * prof, None, f64=True)
+        sim.set_macros(None, ux0, None, None, f64=True)
+        o.step(100)
+        sim.step(100)
+        e = max_err(sim, o, f64=fp64)
+        assert e <= (TOL64 if fp64 else TOL32), (faces, fp64, e)
+        sim.close()
+
+
+def test_momentum_turns_about_a_tilted_axis_on_the_fp32_path(B):
+    """Closed form on the GPU path itself: periodic box, total momentum turns about f by 2 atan(|f|/2) per step."""
+    n = 32
+    fv = np.array([2e-3, -1e-3, 2.5e-3])
+    sim = B.Lbm(n, n, n, 5e-3, 0.1, 0.0, (0, 0, 0), (0, 0, 0, 0, 0, 0), fp64=True)
+    sim.set_coriolis(fv)
+    sim.set_flags(None)
+    x = np.arange(n) * 2 * np.pi / n
+    Z, Y, X = np.meshgrid(x, x, x, indexing="ij")
+    sim.set_macros(None, 0.03 + 0.01 * np.sin(Y), -0.02 + 0.01 * np.cos(Z), 0.015 + 0.01 * np.sin(X + Y), f64=True)
+    c, opp = B.lattice()
+
+    def P():
+        f = sim.get_state().cpu().numpy()
+        return np.array([(c[:, a][:, None, None, None] * f).sum() for a in range(3)])
+    P0 = P()
+    k = 40
+    sim.step(k)
+    Pk = P()
+    axis = fv / np.linalg.norm(fv)
+    th = -2.0 * np.arctan(0.5 * np.linalg.norm(fv)) * k
+    K = np.array([[0, -axis[2], axis[1]], [axis[2], 0, -axis[0]], [-axis[1], axis[0], 0]])
+    R = np.eye(3) + np.sin(th) * K + (1 - np.cos(th)) * (K @ K)
+    assert np.abs(Pk - R @ P0).max() < 1e-10 * n ** 3
+    sim.close()
