@@ -109,6 +109,11 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
     if (fl & (SLOW_BIT | SURF_BIT)) lk = links[p];
     if (cls == SOLID && !(fl & SURF_BIT)) return;
     Macro<real> m{real(1), real(0), real(0), real(0)};
+    const bool merged_solid = cls == SOLID; // a surface solid: it only completes sectors, with zeros
+    if (merged_solid) {
+#pragma unroll
+        for (int i = 0; i < Q; ++i) g[i] = real(0);
+    }
     if (cls == FLUID) {
         if constexpr (!SPEC) {
             static_for<0, Q>([&](auto ic) {
@@ -125,19 +130,24 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
         m = Macro<real>{real(1), fu0, fu1, fu2};
         equilibrium(g, real(0), m.ux, m.uy, m.uz);
     }
-    if (cls == SOLID) {
-        // a solid cell whose 32-byte sector is written by others (live cells, neighbours' mailboxes) completes it with
-        // zeros: the sector leaves L2 fully written, no DRAM read-modify-write (same bytes written either way)
+    // ONE store sequence for the whole warp.  A surface solid takes part in it with zeros, predicated by its completion
+    // mask: a solid cell whose 32-byte sector is written by others (live cells, neighbours' mailboxes) completes it, so
+    // that the sector leaves L2 fully written — no DRAM read-modify-write, same bytes written either way.  Warps without
+    // such a lane (the common case, a warp-uniform branch) store unpredicated.  A second, divergent store sequence for
+    // the solid lanes cost 2 % of the step.
+    const uint32_t wm = merged_solid ? lk : 0x7FFFFu;
+    if (__any_sync(__activemask(), merged_solid)) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            if ((lk >> i) & 1u) st_pop<HINT>(T.dst[i] + p, real(0));
+            if ((wm >> i) & 1u) st_pop<HINT>(T.dst[i] + p, g[i]);
         });
-        return;
+    } else {
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            st_pop<HINT>(T.dst[i] + p, g[i]);
+        });
     }
-    static_for<0, Q>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        st_pop<HINT>(T.dst[i] + p, g[i]);
-    });
+    if (merged_solid) return;
     if (fl & SLOW_BIT) {
         // wall links (lbm_core.cuh wall_stores, with the launch's address table): slot (i, p - off_i) <- g[opp(i)]
         static_for<1, Q>([&](auto ic) {
