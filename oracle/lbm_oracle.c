@@ -466,6 +466,57 @@ static void sample_mean(oracle_t *o)
     o->mcount += 1;
 }
 
+/* Global flux-balancing correction of the prescribed open-boundary velocities ("mass flux consistency
+ * correction ... the minimal normal velocity adjustment required to enforce near-zero net volume flow"
+ * "a global flux-balancing correction is applied over the full set of open boundaries"; sign convention PAPER.md:185
+ * "positive values indicate an outflow").  Open-boundary cells = the EQ_FIXED cells; each belongs to the first
+ * EQ_FIXED face it lies on (order x-,x+,y-,y+,z-,z+) and n is that face's outward normal.
+ *   Phi = sum over those cells of u_b . n        (unit cell faces, lattice units)
+ *   minimal (least-squares) adjustment with sum(delta u . n) = -Phi: the same shift on every cell,
+ *   u_b <- u_b - (Phi / N) n,   then G = f_eq(1, u_b) again.
+ * Returns the net flux before and after (after is recomputed from the corrected cells). */
+static int fixed_face(const oracle_t *o, int x, int y, int z)
+{
+    int on[6] = {x == 0, x == o->nx - 1, y == 0, y == o->ny - 1, z == 0, z == o->nz - 1};
+    for (int k = 0; k < 6; ++k)
+        if (on[k] && o->face[k] == F_EQ_FIXED) return k;
+    return -1;
+}
+
+int oracle_balance_flux(oracle_t *o, double *flux_before, double *flux_after)
+{
+    if (!o || !o->have_flags) return -3;
+    double phi = 0.0, phi2 = 0.0;
+    long n = 0;
+    for (int pass = 0; pass < 3; ++pass) {
+        for (int z = 0; z < o->nz; ++z)
+            for (int y = 0; y < o->ny; ++y)
+                for (int x = 0; x < o->nx; ++x) {
+                    long cell = cell_of(o, x, y, z);
+                    if (o->cls[cell] != C_EQ_FIXED) continue;
+                    int k = fixed_face(o, x, y, z);
+                    if (k < 0) continue;
+                    double nrm[3] = {0, 0, 0};
+                    nrm[k / 2] = (k & 1) ? 1.0 : -1.0;
+                    double rho, u[3];
+                    local_macros(o, o->G, cell, &rho, u);
+                    double un = u[0] * nrm[0] + u[1] * nrm[1] + u[2] * nrm[2];
+                    if (pass == 0) { phi += un; n += 1; }
+                    else if (pass == 1) {
+                        double shift = phi / (double)n;
+                        double ub[3] = {u[0] - shift * nrm[0], u[1] - shift * nrm[1], u[2] - shift * nrm[2]};
+                        feq(1.0, ub, o->G + cell * Q);
+                        feq(1.0, ub, o->Gn + cell * Q);
+                        for (int a = 0; a < 3; ++a) o->ub[3 * cell + a] = ub[a];
+                    } else phi2 += un;
+                }
+        if (pass == 0 && n == 0) break;
+    }
+    if (flux_before) *flux_before = phi;
+    if (flux_after) *flux_after = phi2;
+    return 0;
+}
+
 int oracle_step(oracle_t *o, int nsteps)
 {
     if (!o->have_flags) return -3;

@@ -48,7 +48,7 @@ def _load():
                  "oracle_set_inlet_profile", "oracle_set_inlet_plane", "oracle_set_macros", "oracle_step",
                  "oracle_get_macros", "oracle_mean_reset", "oracle_get_mean",
                  "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell",
-                 "oracle_collide_cell_vec", "oracle_set_coriolis"):
+                 "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -141,6 +141,12 @@ class Oracle:
         """Full Coriolis vector f = 2 Omega (lattice units); (0, 0, f_cor) is the scalar form."""
         a, ap = _d(np.asarray(fvec, dtype=np.float64).reshape(3))
         self._chk(self._lib.oracle_set_coriolis(C.c_void_p(self._h), ap), "set_coriolis")
+
+    def balance_flux(self):
+        """Global flux-balancing correction of the EQ_FIXED face velocities; returns (flux_before, flux_after)."""
+        a, b = C.c_double(), C.c_double()
+        self._chk(self._lib.oracle_balance_flux(C.c_void_p(self._h), C.byref(a), C.byref(b)), "balance_flux")
+        return a.value, b.value
 
     def set_boundaries(self, faces):
         a = np.ascontiguousarray(faces, dtype=np.int32)
