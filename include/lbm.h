@@ -99,6 +99,15 @@ int lbm_set_inlet_profile_f64(lbm_t *h, const double *u, const double *v, const 
 int lbm_set_inlet_plane(lbm_t *h, int face, const float *uvw);
 int lbm_set_inlet_plane_f64(lbm_t *h, int face, const double *uvw);
 
+/* Global flux-balancing correction of the prescribed open-boundary velocities ("the minimal normal velocity
+ * adjustment required to enforce near-zero net volume flow"; "applied over the full set of open boundaries").
+ * Open-boundary cells = the EQ_FIXED cells, each owned by the first EQ_FIXED face it lies on (order x-,x+,y-,y+,z-,z+),
+ * n = that face's outward normal.  Phi = sum u_b . n over them (positive = outflow); every such cell gets
+ * u_b <- u_b - (Phi / N) n and is rewritten to f_eq(1, u_b).  EQ_OUTFLOW faces take no part (their velocity is not
+ * prescribed).  flux_before / flux_after: host pointers, may be NULL; the call synchronises.  Call after the inlet
+ * profile / planes have been set; a later lbm_set_inlet_* or lbm_feed_inlet overwrites the corrected values. */
+int lbm_balance_flux(lbm_t *h, double *flux_before, double *flux_after);
+
 /* Config-5 coupling, device to device, stream-ordered on dst's stream: local macros of src on the plane
  * x = src_x_plane are written as f_eq(1, u) into the EQ_FIXED cells of dst's x- face, tiling y modulo
  * src's ny; nz must match; SOLID src cells feed u = 0.  Both handles must share precision. */

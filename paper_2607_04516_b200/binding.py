@@ -26,7 +26,7 @@ SYMBOLS = [
     "lbm_feed_inlet", "lbm_set_macros", "lbm_set_macros_f64", "lbm_step", "lbm_mean_config", "lbm_mean_reset",
     "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
     "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
-    "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis",
+    "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
 ]
 
 
@@ -54,6 +54,7 @@ def load_library():
     lib.lbm_destroy.argtypes = [vp]
     lib.lbm_set_boundaries.argtypes = [vp, vp]
     lib.lbm_set_coriolis.argtypes = [vp, vp]
+    lib.lbm_balance_flux.argtypes = [vp, vp, vp]
     lib.lbm_set_flags.argtypes = [vp, vp]
     for n in ("lbm_set_inlet_profile", "lbm_set_inlet_profile_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
@@ -177,6 +178,12 @@ class Lbm:
         if a.shape != (3,):
             raise ValueError("f must have 3 entries")
         self._chk(self._lib.lbm_set_coriolis(self._h, a.ctypes.data), "set_coriolis")
+
+    def balance_flux(self):
+        """Global flux-balancing correction of the EQ_FIXED face velocities; returns (flux_before, flux_after)."""
+        a, b = C.c_double(), C.c_double()
+        self._chk(self._lib.lbm_balance_flux(self._h, C.addressof(a), C.addressof(b)), "balance_flux")
+        return a.value, b.value
 
     def set_flags(self, height=None):
         k, p = _ptr(height, np.int32)

@@ -465,6 +465,33 @@ int do_set_state(lbm_t *h, const double *f)
 }
 
 template <typename real>
+int do_balance_flux(lbm_t *h, double *before, double *after)
+{
+    const Params<real> P = make_params<real>(h);
+    double *acc = (double *)h->scratch(); // acc[0..1] before, acc[2..3] after
+    double host[4] = {0, 0, 0, 0};
+    CUDA_TRY(h, cudaMemsetAsync(acc, 0, 4 * sizeof(double), h->stream));
+    if (P.F > 0) {
+        const int B = 128;
+        const unsigned grid = blocks_for(P.F, B);
+        flux_sum_kernel<real><<<grid, B, 0, h->stream>>>((const real *)h->fu(), h->flags(), acc, P);
+        int rc = check_launch(h, "flux_sum_kernel");
+        if (rc) return rc;
+        flux_apply_kernel<real><<<grid, B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), acc, P);
+        rc = check_launch(h, "flux_apply_kernel");
+        if (rc) return rc;
+        flux_sum_kernel<real><<<grid, B, 0, h->stream>>>((const real *)h->fu(), h->flags(), acc + 2, P);
+        rc = check_launch(h, "flux_sum_kernel");
+        if (rc) return rc;
+    }
+    CUDA_TRY(h, cudaMemcpyAsync(host, acc, sizeof host, cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (before) *before = host[0];
+    if (after) *after = host[2];
+    return LBM_OK;
+}
+
+template <typename real>
 int do_feed(lbm_t *dst, const lbm_t *src, int sx)
 {
     const Params<real> D = make_params<real>(dst), S = make_params<real>(src);
@@ -581,6 +608,13 @@ int lbm_feed_inlet(lbm_t *dst, const lbm_t *src, int src_x_plane)
     if (dst->nz != src->nz) return fail(dst, LBM_EINVAL, "feed_inlet: nz mismatch");
     if (src_x_plane < 0 || src_x_plane >= src->nx) return fail(dst, LBM_EINVAL, "feed_inlet: plane out of range");
     return dst->fp64 ? do_feed<double>(dst, src, src_x_plane) : do_feed<float>(dst, src, src_x_plane);
+}
+
+int lbm_balance_flux(lbm_t *h, double *flux_before, double *flux_after)
+{
+    if (!h) return LBM_EINVAL;
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "balance_flux: flags not set");
+    return h->fp64 ? do_balance_flux<double>(h, flux_before, flux_after) : do_balance_flux<float>(h, flux_before, flux_after);
 }
 
 int lbm_set_macros(lbm_t *h, const float *rho, const float *ux, const float *uy, const float *uz)

@@ -240,4 +240,68 @@ __global__ void state_in_kernel(real *__restrict__ A, real *__restrict__ B, real
     store_cell_both(A, B, fu, P, p, x, y, z, fl, links[p], g);
 }
 
+// ---- global flux-balancing correction of the open-boundary velocities -----------------------------------------------------
+// PAPER.md:55 ("the minimal normal velocity adjustment required to enforce near-zero net volume flow")
+// ("a global flux-balancing correction is applied over the full set of open boundaries"), sign PAPER.md:185 (positive =
+// outflow).  Open-boundary cells = EQ_FIXED cells, each owned by the first EQ_FIXED face it lies on; their velocities
+// live in the face-velocity buffer.  Phi = sum u_b . n; correction u_b <- u_b - (Phi / N) n, then f_eq(1, u_b) again.
+// One thread per face-velocity slot; (k, x, y, z) of slot sl, false if the slot is not an EQ_FIXED cell's own slot.
+template <typename real>
+__device__ __forceinline__ bool fixed_slot_cell(const Params<real> &P, const uint8_t *__restrict__ flags, int sl, int &k, int &x, int &y,
+                                                int &z)
+{
+    k = -1;
+    for (int q = 0; q < 6; ++q)
+        if ((P.face[q] == FACE_EQ_FIXED || P.face[q] == FACE_EQ_OUTFLOW) && sl >= P.foff[q]) k = q;
+    if (k < 0 || P.face[k] != FACE_EQ_FIXED) return false;
+    const int axis = k >> 1, idx = sl - P.foff[k];
+    const int n1 = axis == 0 ? P.ny : P.nx, n2 = axis == 2 ? P.ny : P.nz;
+    if (idx >= n1 * n2) return false;
+    const int j1 = idx % n1, j2 = idx / n1;
+    const int nn[3] = {P.nx, P.ny, P.nz};
+    const int fixed = (k & 1) ? nn[axis] - 1 : 0;
+    if (axis == 0) { x = fixed; y = j1; z = j2; }
+    else if (axis == 1) { x = j1; y = fixed; z = j2; }
+    else { x = j1; y = j2; z = fixed; }
+    if ((flags[pidx(P, x, y, z)] & CLASS_MASK) != EQ_FIXED) return false;
+    return eq_owner(P, FACE_EQ_FIXED, x, y, z) == k;
+}
+
+// acc[0] += sum of u_b . n, acc[1] += number of open-boundary cells
+template <typename real>
+__global__ void flux_sum_kernel(const real *__restrict__ fu, const uint8_t *__restrict__ flags, double *__restrict__ acc, Params<real> P)
+{
+    const int sl = blockIdx.x * blockDim.x + threadIdx.x;
+    double un = 0.0, cnt = 0.0;
+    int k, x, y, z;
+    if (sl < P.F && fixed_slot_cell(P, flags, sl, k, x, y, z)) {
+        un = (double)fu[(k >> 1) * P.F + sl] * ((k & 1) ? 1.0 : -1.0);
+        cnt = 1.0;
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        un += __shfl_down_sync(0xffffffffu, un, o);
+        cnt += __shfl_down_sync(0xffffffffu, cnt, o);
+    }
+    if ((threadIdx.x & 31) == 0 && cnt != 0.0) { atomicAdd(&acc[0], un); atomicAdd(&acc[1], cnt); }
+}
+
+template <typename real>
+__global__ void flux_apply_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+                                  const double *__restrict__ acc, Params<real> P)
+{
+    const int sl = blockIdx.x * blockDim.x + threadIdx.x;
+    int k, x, y, z;
+    if (sl >= P.F || !fixed_slot_cell(P, flags, sl, k, x, y, z)) return;
+    if (acc[1] == 0.0) return;
+    const double shift = acc[0] / acc[1];
+    real u[3] = {fu[sl], fu[P.F + sl], fu[2 * P.F + sl]};
+    u[k >> 1] = real((double)u[k >> 1] - shift * ((k & 1) ? 1.0 : -1.0));
+    real g[Q];
+    equilibrium(g, real(0), u[0], u[1], u[2]);
+    const int p = pidx(P, x, y, z);
+    store_cell_both(A, B, fu, P, p, x, y, z, flags[p], 0u, g);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) { fu[c * P.F + sl] = u[c]; fu[(3 + c) * P.F + sl] = u[c]; } // the exact corrected velocity
+}
+
 } // namespace lbmk

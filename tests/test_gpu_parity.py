@@ -454,3 +454,41 @@ def test_momentum_turns_about_a_tilted_axis_on_the_fp32_path(B):
     R = np.eye(3) + np.sin(th) * K + (1 - np.cos(th)) * (K @ K)
     assert np.abs(Pk - R @ P0).max() < 1e-10 * n ** 3
     sim.close()
+
+
+# ---------------------------------------------------------------------------------------------- flux balancing
+
+@pytest.mark.parametrize("fp64", [False, True])
+@pytest.mark.parametrize("faces", [(3, 3, 3, 3, 1, 3), (3, 4, 3, 3, 1, 2), (3, 3, 0, 0, 1, 2)])
+def test_flux_balancing_matches_the_oracle(B, faces, fp64):
+    """PAPER.md:55 / :175: global flux-balancing correction over the open (EQ_FIXED) faces, then 50 steps."""
+    from oracle import Oracle
+    nx, ny, nz = 37, 22, 14
+    rng = np.random.default_rng(11)
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    hm[3:6, 0:3] = 5           # a building standing in the x- face
+    hm[10:14, 15:20] = 9
+    args = (nx, ny, nz, 5e-3, 0.1, 1e-3, (0.0, 0.0, 0.0), faces)
+    o = Oracle(*args)
+    sim = B.Lbm(*args, fp64=fp64)
+    o.set_flags(hm)
+    sim.set_flags(hm)
+    for k in range(6):
+        if faces[k] == 3:
+            axis = k // 2
+            n1 = ny if axis == 0 else nx
+            n2 = ny if axis == 2 else nz
+            pl = (0.03 * rng.standard_normal((3, n2, n1))).astype(np.float32).astype(np.float64)
+            o.set_inlet_plane(k, pl)
+            sim.set_inlet_plane(k, pl, f64=True)
+    o.set_macros()
+    sim.set_macros()
+    ob, oa = o.balance_flux()
+    gb, ga = sim.balance_flux()
+    assert gb == pytest.approx(ob, rel=1e-6 if not fp64 else 1e-12, abs=1e-9)
+    assert abs(oa) < 1e-12 and abs(ga) < (1e-12 if fp64 else 2e-5)
+    assert max_err(sim, o, f64=fp64) <= (TOL64 if fp64 else 1e-7)
+    o.step(50)
+    sim.step(50)
+    assert max_err(sim, o, f64=fp64) <= (TOL64 if fp64 else TOL32)
+    sim.close()
