@@ -41,6 +41,7 @@ def make(O, faces, nx=10, ny=8, nz=6, seed=0):
             n1 = ny if axis == 0 else nx
             n2 = ny if axis == 2 else nz
             o.set_inlet_plane(k, 0.05 * rng.standard_normal((3, n2, n1)))
+    o.set_macros()            # interior at rest (rho = 1, u = 0): the state is defined everywhere before it is compared
     return o
 
 
