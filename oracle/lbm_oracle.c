@@ -88,6 +88,8 @@ typedef struct oracle {
     double *G;    /* [cell][19], post-collision state G_k (step 3) */
     double *Gn;   /* next */
     double *ub;   /* [cell][3] prescribed velocity of EQ_FIXED cells */
+    double *sig;  /* [cell] damping coefficient sigma(x) of the sponge / buffer zones (NULL = none) */
+    double *ut;   /* [3][nz] target state u_t(z) the damping relaxes towards */
     long step;
     double *msum; /* [cell][3] */
     long mcount, mstart;
@@ -139,7 +141,13 @@ static void coriolis_matrix(const double fv[3], double Cm[3][3])
     Cm[2][0] = fv[1];  Cm[2][1] = -fv[0]; Cm[2][2] = 0.0;
 }
 
+/* Damping zones ("relaxation-based damping regions adjacent to the upper and lateral boundaries,
+ * including a top sponge layer and boundary-adjacent buffer nudging toward the target boundary state"; Table 1
+ * PAPER.md:86 "sponge and buffer damping").  Reading (DESIGN.md §4 reading 20): a Rayleigh relaxation acceleration
+ * a_d(u) = sigma(x) (u_t - u) towards the target state u_t, added to the body force and integrated by the same
+ * implicit half-force rule as the Coriolis term.  sigma = 0 is the undamped step. */
 static void collide(const double f[Q], double nu0, double Cs, const double fv[3], const double F[3],
+                    double sigma, const double ut[3],
                     double g[Q], double *rho_out, double u_out[3], double *tau_out)
 {
     /* 4b moments */
@@ -148,17 +156,19 @@ static void collide(const double f[Q], double nu0, double Cs, const double fv[3]
         rho += f[i];
         for (int a = 0; a < 3; ++a) m[a] += CI[i][a] * f[i];
     }
-    /* 4c implicit half-force velocity: rho u = m + rho a(u)/2, a(u) = F + C u
-     * => (I - C/2) u = m/rho + F/2 */
+    /* 4c implicit half-force velocity: rho u = m + rho a(u)/2, a(u) = F + C u + sigma (u_t - u)
+     * => ((1 + sigma/2) I - C/2) u = m/rho + F/2 + (sigma/2) u_t */
     double Cm[3][3], M[3][3];
     coriolis_matrix(fv, Cm);
     for (int a = 0; a < 3; ++a)
-        for (int c = 0; c < 3; ++c) M[a][c] = (a == c ? 1.0 : 0.0) - 0.5 * Cm[a][c];
-    double b[3] = {m[0] / rho + 0.5 * F[0], m[1] / rho + 0.5 * F[1], m[2] / rho + 0.5 * F[2]};
+        for (int c = 0; c < 3; ++c) M[a][c] = (a == c ? 1.0 + 0.5 * sigma : 0.0) - 0.5 * Cm[a][c];
+    double b[3];
+    for (int a = 0; a < 3; ++a) b[a] = m[a] / rho + 0.5 * F[a] + 0.5 * sigma * (ut ? ut[a] : 0.0);
     double u[3];
     solve3(M, b, u);
     double Fd[3]; /* force density rho a(u) */
-    for (int a = 0; a < 3; ++a) Fd[a] = rho * (F[a] + Cm[a][0] * u[0] + Cm[a][1] * u[1] + Cm[a][2] * u[2]);
+    for (int a = 0; a < 3; ++a)
+        Fd[a] = rho * (F[a] + Cm[a][0] * u[0] + Cm[a][1] * u[1] + Cm[a][2] * u[2] + sigma * ((ut ? ut[a] : 0.0) - u[a]));
     /* 4d LES: Pi = sum c c (f - feq); Q = Frobenius norm over all 9 entries */
     double fe[Q];
     feq(rho, u, fe);
@@ -226,12 +236,16 @@ static void local_macros(const oracle_t *o, const double *Gs, long cell, double 
     }
     *rho = r;
     if (cl == C_FLUID) {
-        /* invert m* = rho u + rho a(u)/2, a(u) = F + C u  =>  (I + C/2) u = m* / rho - F/2 */
+        /* invert m* = rho u + rho a(u)/2, a(u) = F + C u + sigma (u_t - u)
+         * =>  ((1 - sigma/2) I + C/2) u = m* / rho - F/2 - (sigma/2) u_t   (regular for sigma < 2) */
         double Cm[3][3], M[3][3];
         coriolis_matrix(o->fv, Cm);
+        double sg = o->sig ? o->sig[cell] : 0.0;
+        long zc = cell / ((long)o->nx * o->ny);
         for (int a = 0; a < 3; ++a)
-            for (int c = 0; c < 3; ++c) M[a][c] = (a == c ? 1.0 : 0.0) + 0.5 * Cm[a][c];
-        double b[3] = {m[0] / r - 0.5 * o->F[0], m[1] / r - 0.5 * o->F[1], m[2] / r - 0.5 * o->F[2]};
+            for (int c = 0; c < 3; ++c) M[a][c] = (a == c ? 1.0 - 0.5 * sg : 0.0) + 0.5 * Cm[a][c];
+        double b[3];
+        for (int a = 0; a < 3; ++a) b[a] = m[a] / r - 0.5 * o->F[a] - 0.5 * sg * (o->ut ? o->ut[a * o->nz + zc] : 0.0);
         solve3(M, b, u);
     } else {
         u[0] = m[0] / r; u[1] = m[1] / r; u[2] = m[2] / r;
@@ -257,7 +271,7 @@ int oracle_collide_cell(const double *f, double nu0, double Cs, double fcor, con
                         double *g, double *rho, double *u, double *tau)
 {
     const double fv[3] = {0.0, 0.0, fcor};
-    collide(f, nu0, Cs, fv, F, g, rho, u, tau);
+    collide(f, nu0, Cs, fv, F, 0.0, NULL, g, rho, u, tau);
     return 0;
 }
 
@@ -265,7 +279,15 @@ int oracle_collide_cell(const double *f, double nu0, double Cs, double fcor, con
 int oracle_collide_cell_vec(const double *f, double nu0, double Cs, const double *fv, const double *F,
                             double *g, double *rho, double *u, double *tau)
 {
-    collide(f, nu0, Cs, fv, F, g, rho, u, tau);
+    collide(f, nu0, Cs, fv, F, 0.0, NULL, g, rho, u, tau);
+    return 0;
+}
+
+/* same inside a damping zone: coefficient sigma, target velocity ut[3] */
+int oracle_collide_cell_damped(const double *f, double nu0, double Cs, const double *fv, const double *F,
+                               double sigma, const double *ut, double *g, double *rho, double *u, double *tau)
+{
+    collide(f, nu0, Cs, fv, F, sigma, ut, g, rho, u, tau);
     return 0;
 }
 
@@ -295,7 +317,52 @@ oracle_t *oracle_create(int nx, int ny, int nz, double nu0, double Cs, double fc
 void oracle_destroy(oracle_t *o)
 {
     if (!o) return;
-    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o);
+    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o->sig); free(o->ut); free(o);
+}
+
+/* Damping zones (see collide()).  width[k] (cells) and peak[k] for the six faces x-,x+,y-,y+,z-,z+; a cell at
+ * distance d = 0, 1, ... (in cells) from the layer of cells adjacent to face k lies in that face's zone if d < width[k]
+ * and sees the ramp  peak[k] * sin^2( (pi/2) (1 - d / width[k]) )  (peak at the face layer, smoothly to 0 at d = width);
+ * sigma(x) = the LARGEST of the six (zones do not add up in edges and corners).  ut = [3][nz] target profile u_t(z).
+ * All widths 0 switch the damping off.  0 <= peak[k] <= 1 (sigma < 2 keeps the macro inversion regular). */
+int oracle_set_damping(oracle_t *o, const int *width, const double *peak, const double *ut)
+{
+    if (!o || !width || !peak) return -1;
+    int any = 0;
+    for (int k = 0; k < 6; ++k) {
+        if (width[k] < 0 || peak[k] < 0.0 || peak[k] > 1.0) return -1;
+        if (width[k] > 0 && peak[k] > 0.0) any = 1;
+    }
+    free(o->sig); free(o->ut); o->sig = NULL; o->ut = NULL;
+    if (!any) return 0;
+    if (!ut) return -1;
+    long N = (long)o->nx * o->ny * o->nz;
+    o->sig = (double *)calloc(N, sizeof(double));
+    o->ut = (double *)malloc(sizeof(double) * 3 * o->nz);
+    if (!o->sig || !o->ut) return -4;
+    memcpy(o->ut, ut, sizeof(double) * 3 * o->nz);
+    const double half_pi = 2.0 * atan(1.0);
+    for (int z = 0; z < o->nz; ++z)
+        for (int y = 0; y < o->ny; ++y)
+            for (int x = 0; x < o->nx; ++x) {
+                int d[6] = {x, o->nx - 1 - x, y, o->ny - 1 - y, z, o->nz - 1 - z};
+                double s = 0.0;
+                for (int k = 0; k < 6; ++k) {
+                    if (width[k] <= 0 || d[k] >= width[k]) continue;
+                    double r = sin(half_pi * (1.0 - (double)d[k] / (double)width[k]));
+                    double v = peak[k] * r * r;
+                    if (v > s) s = v;
+                }
+                o->sig[cell_of(o, x, y, z)] = s;
+            }
+    return 0;
+}
+
+int oracle_get_damping(const oracle_t *o, double *sigma)
+{
+    long N = (long)o->nx * o->ny * o->nz;
+    for (long c = 0; c < N; ++c) sigma[c] = o->sig ? o->sig[c] : 0.0;
+    return 0;
 }
 
 /* Coriolis vector f = 2 Omega in lattice units; replaces the scalar given at creation */
@@ -538,7 +605,9 @@ int oracle_step(oracle_t *o, int nsteps)
                             if (r < 0) { bad = 1; r = 1; }
                             f[i] = r ? o->G[cell * Q + opposite(i)] : o->G[s * Q + j];
                         }
-                        collide(f, o->nu0, o->Cs, o->fv, o->F, gn, NULL, NULL, NULL);
+                        double ut[3] = {0, 0, 0};
+                        if (o->ut) for (int a = 0; a < 3; ++a) ut[a] = o->ut[a * o->nz + z];
+                        collide(f, o->nu0, o->Cs, o->fv, o->F, o->sig ? o->sig[cell] : 0.0, ut, gn, NULL, NULL, NULL);
                     } else if (cl == C_EQ_OUTFLOW) {
                         /* step 6 */
                         int k = outflow_face(o, x, y, z);

@@ -48,7 +48,8 @@ def _load():
                  "oracle_set_inlet_profile", "oracle_set_inlet_plane", "oracle_set_macros", "oracle_step",
                  "oracle_get_macros", "oracle_mean_reset", "oracle_get_mean",
                  "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell",
-                 "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux"):
+                 "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux",
+                 "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -109,6 +110,22 @@ def collide_cell_vec(f, nu0, Cs, fvec, F):
     return g, rho.value, u, tau.value
 
 
+def collide_cell_damped(f, nu0, Cs, fvec, F, sigma, ut):
+    """One cell's step 4b-4e inside a damping zone (coefficient sigma, target velocity ut).  Returns (g, rho, u, tau)."""
+    lib = _load()
+    f, fp = _d(f)
+    F, Fp = _d(np.asarray(F, dtype=np.float64))
+    fv, fvp = _d(np.asarray(fvec, dtype=np.float64))
+    ut, utp = _d(np.asarray(ut, dtype=np.float64))
+    g = np.zeros(19)
+    rho = C.c_double()
+    u = np.zeros(3)
+    tau = C.c_double()
+    lib.oracle_collide_cell_damped(fp, C.c_double(nu0), C.c_double(Cs), fvp, Fp, C.c_double(sigma), utp,
+                                   g.ctypes.data_as(C.c_void_p), C.byref(rho), u.ctypes.data_as(C.c_void_p), C.byref(tau))
+    return g, rho.value, u, tau.value
+
+
 class Oracle:
     """FP64 CPU LBM; same call names as the product binding, float64 arrays."""
 
@@ -141,6 +158,18 @@ class Oracle:
         """Full Coriolis vector f = 2 Omega (lattice units); (0, 0, f_cor) is the scalar form."""
         a, ap = _d(np.asarray(fvec, dtype=np.float64).reshape(3))
         self._chk(self._lib.oracle_set_coriolis(C.c_void_p(self._h), ap), "set_coriolis")
+
+    def set_damping(self, width, peak, target=None):
+        """Sponge / buffer zones: per-face width (cells) and peak coefficient, target profile [3][nz]."""
+        w = np.ascontiguousarray(width, dtype=np.int32).reshape(6)
+        pk, pkp = _d(np.asarray(peak, dtype=np.float64).reshape(6))
+        t, tp = (None, None) if target is None else _d(np.asarray(target, dtype=np.float64).reshape(3, self.nz))
+        self._chk(self._lib.oracle_set_damping(C.c_void_p(self._h), w.ctypes.data_as(C.c_void_p), pkp, tp), "set_damping")
+
+    def get_damping(self):
+        s = np.zeros(self.shape)
+        self._chk(self._lib.oracle_get_damping(C.c_void_p(self._h), s.ctypes.data_as(C.c_void_p)), "get_damping")
+        return s
 
     def balance_flux(self):
         """Global flux-balancing correction of the EQ_FIXED face velocities; returns (flux_before, flux_after)."""
