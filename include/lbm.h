@@ -108,6 +108,20 @@ int lbm_set_inlet_plane_f64(lbm_t *h, int face, const double *uvw);
  * profile / planes have been set; a later lbm_set_inlet_* or lbm_feed_inlet overwrites the corrected values. */
 int lbm_balance_flux(lbm_t *h, double *flux_before, double *flux_after);
 
+/* Damping zones: top sponge layer and boundary-adjacent buffer nudging towards the target boundary state (PAPER.md:175
+ * "relaxation-based damping regions adjacent to the upper and lateral boundaries, including a top sponge layer and
+ * boundary-adjacent buffer nudging toward the target boundary state"; Table 1 PAPER.md:86 "sponge and buffer damping").
+ * The paper prints neither form nor coefficients (S7 missing); reading (DESIGN.md §4 reading 20): a Rayleigh relaxation
+ * acceleration a_d(u) = sigma(x) (u_t(z) - u) joins the body force of FLUID cells and is integrated by the same implicit
+ * half-force rule as the Coriolis term (unconditionally stable; per step a uniform defect shrinks by
+ * (1 - sigma/2) / (1 + sigma/2)).  width[k] (cells, >= 0) and peak[k] (0 <= peak <= 1) for the faces x-,x+,y-,y+,z-,z+:
+ * a cell d = 0, 1, ... cells away from the layer adjacent to face k sees  peak[k] sin^2((pi/2)(1 - d/width[k]))  while
+ * d < width[k];  sigma(x) = the largest of the six.  target: HOST array [3][nz] = u_t, v_t, w_t per level (e.g. the
+ * inlet profile), copied.  All width or peak zero: damping off (target may be NULL).  The zones cost no HBM traffic
+ * (coefficients come from three small per-axis tables); lbm_get_macros / lbm_get_mean stay exact inside them.
+ * Returns LBM_EINVAL for a negative width, a peak outside [0, 1] or a non-finite / device target.  Synchronises. */
+int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const double *target);
+
 /* Config-5 coupling, device to device, stream-ordered on dst's stream: local macros of src on the plane
  * x = src_x_plane are written as f_eq(1, u) into the EQ_FIXED cells of dst's x- face, tiling y modulo
  * src's ny; nz must match; SOLID src cells feed u = 0.  Both handles must share precision. */

@@ -27,6 +27,7 @@ SYMBOLS = [
     "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
     "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
+    "lbm_set_damping",
 ]
 
 
@@ -55,6 +56,7 @@ def load_library():
     lib.lbm_set_boundaries.argtypes = [vp, vp]
     lib.lbm_set_coriolis.argtypes = [vp, vp]
     lib.lbm_balance_flux.argtypes = [vp, vp, vp]
+    lib.lbm_set_damping.argtypes = [vp, vp, vp, vp]
     lib.lbm_set_flags.argtypes = [vp, vp]
     for n in ("lbm_set_inlet_profile", "lbm_set_inlet_profile_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
@@ -178,6 +180,20 @@ class Lbm:
         if a.shape != (3,):
             raise ValueError("f must have 3 entries")
         self._chk(self._lib.lbm_set_coriolis(self._h, a.ctypes.data), "set_coriolis")
+
+    def set_damping(self, width, peak, target=None):
+        """Sponge / buffer zones: per-face width (cells) and peak coefficient, host target profile [3][nz]."""
+        w = np.ascontiguousarray(width, dtype=np.int32)
+        pk = np.ascontiguousarray(peak, dtype=np.float64)
+        if w.shape != (6,) or pk.shape != (6,):
+            raise ValueError("width and peak must have 6 entries")
+        t = None
+        if target is not None:
+            t = np.ascontiguousarray(target, dtype=np.float64)
+            if t.shape != (3, self.nz):
+                raise ValueError("target must be [3][nz]")
+        self._chk(self._lib.lbm_set_damping(self._h, w.ctypes.data, pk.ctypes.data, t.ctypes.data if t is not None else None),
+                  "set_damping")
 
     def balance_flux(self):
         """Global flux-balancing correction of the EQ_FIXED face velocities; returns (flux_before, flux_after)."""

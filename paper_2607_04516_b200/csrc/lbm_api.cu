@@ -9,6 +9,8 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
+#include <algorithm>
 
 using namespace lbmk;
 
@@ -21,7 +23,7 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 struct Layout {
     int px, py;
     long long Np, stride;
-    size_t off_A, off_B, off_flags, off_links, off_fu, off_mean, off_scratch, total;
+    size_t off_A, off_B, off_flags, off_links, off_fu, off_mean, off_damp, off_scratch, total;
     size_t fu_bytes;
     size_t scratch_bytes;
 };
@@ -43,6 +45,8 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
     L.fu_bytes = align_up((size_t)2 * 3 * 2 * ((size_t)ny * nz + (size_t)nx * nz + (size_t)nx * ny) * rs, ALIGN);
     L.off_fu = o; o += L.fu_bytes;
     L.off_mean = o; if (want_mean) o += align_up((size_t)3 * L.stride * rs, ALIGN);
+    // damping tables (lbm_set_damping): sx[nx], sy[ny], sz[nz], ut[3][nz]
+    L.off_damp = o; o += align_up(((size_t)nx + ny + 4 * (size_t)nz) * rs, ALIGN);
     // scratch: heightmap (nx*ny int32) or a profile (3 nz doubles) or one face plane (3 n1 n2 doubles)
     const size_t plane = (size_t)std::max(std::max((size_t)nx * ny, (size_t)nx * nz), (size_t)ny * nz);
     L.scratch_bytes = align_up(std::max(plane * 3 * sizeof(double), (size_t)nz * 3 * sizeof(double)), ALIGN);
@@ -76,6 +80,7 @@ struct lbm {
     long mstart; int mevery; long mcount;
     long launches;
     int variant;
+    bool damp_on;   // damping zones configured (the DAMP instantiation of the step kernel runs)
     std::string err;
 
     void *bufA() const { return ws + L.off_A; }
@@ -86,6 +91,7 @@ struct lbm {
     uint32_t *links() const { return (uint32_t *)(ws + L.off_links); }
     void *fu() const { return ws + L.off_fu; }
     void *mean() const { return want_mean ? ws + L.off_mean : nullptr; }
+    void *damp() const { return ws + L.off_damp; }
     void *scratch() const { return ws + L.off_scratch; }
     long long N() const { return (long long)nx * ny * nz; }
 };
@@ -131,6 +137,7 @@ Params<real> make_params(const lbm_t *h)
     P.hx = (real)(0.5 * h->fv[0]); P.hy = (real)(0.5 * h->fv[1]); P.hz = (real)(0.5 * h->fv[2]);
     P.inv1ph2 = (real)(1.0 / (1.0 + 0.25 * (h->fv[0] * h->fv[0] + h->fv[1] * h->fv[1] + h->fv[2] * h->fv[2])));
     P.Fx = (real)h->F[0]; P.Fy = (real)h->F[1]; P.Fz = (real)h->F[2];
+    P.damp = h->damp_on ? (const real *)h->damp() : nullptr;
     return P;
 }
 
@@ -322,7 +329,7 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     return rc;
 }
 
-template <typename real, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0>
+template <typename real, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false>
 int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
     const real *A = (const real *)h->state();
@@ -333,16 +340,23 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
     // the side buffer's halves follow the population buffers: read the half written together with A, write B's
     const real *fur = (const real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
     real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
-    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
-    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
+    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB, EXP, DAMP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
+    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP, DAMP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
     return check_launch(h, "step_kernel");
 }
 
 // kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes / load issue order.
 constexpr int N_VARIANTS = 11;
+#ifndef DAMP_MINB
+#define DAMP_MINB 10
+#endif
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
+    if (h->damp_on) { // damping zones: the DAMP instantiation (same arithmetic outside the zones)
+        if constexpr (std::is_same<real, float>::value) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true>(h, P, sample);
+        else return launch_step_as<real, 0, false, 256, 2, 0, true>(h, P, sample);
+    }
     if constexpr (std::is_same<real, float>::value) {
         switch (h->variant) {
         case 0: return launch_step_as<real, 0, true, 128, 10>(h, P, sample);
@@ -492,6 +506,16 @@ int do_balance_flux(lbm_t *h, double *before, double *after)
 }
 
 template <typename real>
+int do_refeed(lbm_t *h)
+{
+    const Params<real> P = make_params<real>(h);
+    if (P.F == 0) return LBM_OK;
+    const int B = 256;
+    refeed_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->state(), (real *)h->fu(), h->flags(), P);
+    return check_launch(h, "refeed_kernel");
+}
+
+template <typename real>
 int do_feed(lbm_t *dst, const lbm_t *src, int sx)
 {
     const Params<real> D = make_params<real>(dst), S = make_params<real>(src);
@@ -534,7 +558,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     h->L = make_layout(nx, ny, nz, h->want_mean, h->fp64);
     h->stream = (cudaStream_t)cuda_stream;
     h->cur = 0; h->have_flags = false; h->step = 0;
-    h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0;
+    h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false;
     if (dev_workspace) {
         if (workspace_bytes < h->L.total || ((uintptr_t)dev_workspace % ALIGN) != 0 || !is_device_ptr(dev_workspace)) {
             delete h;
@@ -587,6 +611,60 @@ int lbm_set_coriolis(lbm_t *h, const double f[3])
         if (!std::isfinite(f[a])) return fail(h, LBM_EINVAL, "set_coriolis: not finite");
     for (int a = 0; a < 3; ++a) h->fv[a] = f[a];
     return LBM_OK;
+}
+
+int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const double *target)
+{
+    if (!h) return LBM_EINVAL;
+    if (!width || !peak) return fail(h, LBM_EINVAL, "set_damping: NULL");
+    bool any = false;
+    for (int k = 0; k < 6; ++k) {
+        if (width[k] < 0 || !(peak[k] >= 0.0) || peak[k] > 1.0) return fail(h, LBM_EINVAL, "set_damping: need width >= 0 and 0 <= peak <= 1");
+        any |= width[k] > 0 && peak[k] > 0.0;
+    }
+    // the outflow cells' next velocities are local macros of the current state: re-evaluate them under the new zones
+    auto refeed = [&]() { return !h->have_flags ? LBM_OK : (h->fp64 ? do_refeed<double>(h) : do_refeed<float>(h)); };
+    if (!any) {
+        const bool was = h->damp_on;
+        h->damp_on = false;
+        return was ? refeed() : LBM_OK;
+    }
+    if (!target) return fail(h, LBM_EINVAL, "set_damping: target is NULL");
+    if (is_device_ptr(target)) return fail(h, LBM_EINVAL, "set_damping: target must be a host array");
+    // per-axis tables in double, then cast to the handle's precision: ramp = peak sin^2((pi/2)(1 - d/width)), d = cells
+    // from the face layer; an axis table holds the larger of its two faces' ramps
+    const int n[3] = {h->nx, h->ny, h->nz};
+    const size_t cnt = (size_t)h->nx + h->ny + 4 * (size_t)h->nz;
+    std::vector<double> t(cnt, 0.0);
+    size_t base = 0;
+    for (int a = 0; a < 3; ++a) {
+        for (int c = 0; c < n[a]; ++c) {
+            double s = 0.0;
+            for (int side = 0; side < 2; ++side) {
+                const int k = 2 * a + side, d = side ? n[a] - 1 - c : c;
+                if (width[k] <= 0 || d >= width[k]) continue;
+                const double r = std::sin(1.5707963267948966 * (1.0 - (double)d / (double)width[k]));
+                s = std::max(s, peak[k] * r * r);
+            }
+            t[base + c] = s;
+        }
+        base += n[a];
+    }
+    for (size_t k = 0; k < 3 * (size_t)h->nz; ++k) {
+        if (!std::isfinite(target[k])) return fail(h, LBM_EINVAL, "set_damping: target not finite");
+        t[base + k] = target[k];
+    }
+    cudaError_t e;
+    if (h->fp64) e = cudaMemcpyAsync(h->damp(), t.data(), cnt * sizeof(double), cudaMemcpyHostToDevice, h->stream);
+    else {
+        std::vector<float> tf(t.begin(), t.end());
+        e = cudaMemcpyAsync(h->damp(), tf.data(), cnt * sizeof(float), cudaMemcpyHostToDevice, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream); // tf dies at the end of this block
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (e != cudaSuccess) return fail(h, LBM_ECUDA, std::string("set_damping: ") + cudaGetErrorString(e));
+    h->damp_on = true;
+    return refeed();
 }
 
 int lbm_set_flags(lbm_t *h, const int32_t *height)

@@ -72,6 +72,10 @@ struct Params {
     real fx, fy, fz;       // Coriolis vector f = 2 Omega; the scalar f_cor of lbm_create is fz
     real hx, hy, hz, inv1ph2; // h = f/2, 1/(1+|h|^2)
     real Fx, Fy, Fz;
+    // damping zones (lbm_set_damping; PAPER.md:175 top sponge + lateral buffer nudging): nullptr = none, else the per-axis
+    // coefficient tables sx[nx], sy[ny], sz[nz] (each the larger of the axis' two face ramps) followed by the target
+    // profile ut[3][nz];  sigma(x,y,z) = max(sx[x], sy[y], sz[z])
+    const real *damp;
 };
 
 // Interior x = 0 sits at padded x = XOFF = 8: every interior row starts on a 32-byte sector boundary (and ends on one
@@ -107,10 +111,23 @@ __device__ __forceinline__ real cdot(real ax, real ay, real az)
 template <typename real>
 struct Macro { real rho, ux, uy, uz; };
 
+// damping coefficient and target velocity of one cell (DESIGN.md §4 reading 20): a_d(u) = sg (ut - u)
+template <typename real>
+struct Damp { real sg, utx, uty, utz; };
+template <typename real>
+__device__ __forceinline__ Damp<real> damp_at(const Params<real> &P, int x, int y, int z)
+{
+    if (!P.damp) return Damp<real>{real(0), real(0), real(0), real(0)};
+    const real *d = P.damp;
+    const real sg = fmax(fmax(d[x], d[P.nx + y]), d[P.nx + P.ny + z]);
+    const real *t = d + (P.nx + P.ny + P.nz);
+    return Damp<real>{sg, t[z], t[P.nz + z], t[2 * P.nz + z]};
+}
+
 // ---- collision (DESIGN.md §3 steps 4b-4e) on shifted populations ---------------------------------------------------
 // In: pulled g[19].  Out: post-collision g[19]; returns the (rho,u) the collision used.
-template <typename real>
-__device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> &P)
+template <typename real, bool DAMP = false>
+__device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> &P, const Damp<real> dm = Damp<real>{})
 {
     real s[10], d[10];
 #pragma unroll
@@ -129,13 +146,32 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
     // 4c: implicit half-force velocity.  a(u) = F - f x u, so rho u = m + rho a(u)/2 reads u + h x u = b with h = f/2,
     // b = m/rho + F/2, whose solution is u = (b - h x b + h (h.b)) / (1 + |h|^2)
     const real bx = mx * inv + real(0.5) * P.Fx, by = my * inv + real(0.5) * P.Fy, bz = mz * inv + real(0.5) * P.Fz;
-    const real hb = P.hx * bx + P.hy * by + P.hz * bz;
-    const real ux = (bx - (P.hy * bz - P.hz * by) + P.hx * hb) * P.inv1ph2;
-    const real uy = (by - (P.hz * bx - P.hx * bz) + P.hy * hb) * P.inv1ph2;
-    const real uz = (bz - (P.hx * by - P.hy * bx) + P.hz * hb) * P.inv1ph2;
-    const real Fdx = rho * (P.Fx - (P.fy * uz - P.fz * uy));
-    const real Fdy = rho * (P.Fy - (P.fz * ux - P.fx * uz));
-    const real Fdz = rho * (P.Fz - (P.fx * uy - P.fy * ux));
+    real ux, uy, uz, Fdx, Fdy, Fdz;
+    bool damped = false;
+    if constexpr (DAMP) damped = dm.sg > real(0);
+    if (damped) {
+        // inside a damping zone a(u) gains sg (ut - u):  A u + h x u = b' with A = 1 + sg/2, b' = b + (sg/2) ut, whose
+        // solution is u = (A^2 b' - A h x b' + h (h.b')) / (A (A^2 + |h|^2))
+        const real hs = real(0.5) * dm.sg, A = real(1) + hs;
+        const real cx = bx + hs * dm.utx, cy = by + hs * dm.uty, cz = bz + hs * dm.utz;
+        const real hb = P.hx * cx + P.hy * cy + P.hz * cz;
+        const real den = real(1) / (A * (A * A + (P.hx * P.hx + P.hy * P.hy + P.hz * P.hz)));
+        const real A2 = A * A;
+        ux = (A2 * cx - A * (P.hy * cz - P.hz * cy) + P.hx * hb) * den;
+        uy = (A2 * cy - A * (P.hz * cx - P.hx * cz) + P.hy * hb) * den;
+        uz = (A2 * cz - A * (P.hx * cy - P.hy * cx) + P.hz * hb) * den;
+        Fdx = rho * (P.Fx - (P.fy * uz - P.fz * uy) + dm.sg * (dm.utx - ux));
+        Fdy = rho * (P.Fy - (P.fz * ux - P.fx * uz) + dm.sg * (dm.uty - uy));
+        Fdz = rho * (P.Fz - (P.fx * uy - P.fy * ux) + dm.sg * (dm.utz - uz));
+    } else {
+        const real hb = P.hx * bx + P.hy * by + P.hz * bz;
+        ux = (bx - (P.hy * bz - P.hz * by) + P.hx * hb) * P.inv1ph2;
+        uy = (by - (P.hz * bx - P.hx * bz) + P.hy * hb) * P.inv1ph2;
+        uz = (bz - (P.hx * by - P.hy * bx) + P.hz * hb) * P.inv1ph2;
+        Fdx = rho * (P.Fx - (P.fy * uz - P.fz * uy));
+        Fdy = rho * (P.Fy - (P.fz * ux - P.fx * uz));
+        Fdz = rho * (P.Fz - (P.fx * uy - P.fy * ux));
+    }
     // 4d: Pi = sum c c (f - feq) = M - (drho/3) I - rho u u   (second moment of the shifted equilibrium is exact)
     const real third = real(1) / real(3);
     const real Pxx = Mxx - third * drho - rho * ux * ux;
@@ -199,9 +235,9 @@ __device__ __forceinline__ void equilibrium(real (&g)[Q], real drho, real ux, re
     });
 }
 
-// local macros of a stored (post-collision) state (DESIGN.md §3 step 7)
+// local macros of a stored (post-collision) state (DESIGN.md §3 step 7); dm = the cell's damping (damp_at)
 template <typename real>
-__device__ __forceinline__ Macro<real> local_macros(const real (&g)[Q], int cls, const Params<real> &P)
+__device__ __forceinline__ Macro<real> local_macros(const real (&g)[Q], int cls, const Params<real> &P, const Damp<real> dm = Damp<real>{})
 {
     if (cls == SOLID || cls == GHOST) return Macro<real>{real(1), real(0), real(0), real(0)};
     real s[10], d[10];
@@ -213,6 +249,17 @@ __device__ __forceinline__ Macro<real> local_macros(const real (&g)[Q], int cls,
     const real mz = (d[3] + d[5]) + (d[6] - d[8]) - d[9];
     const real rho = real(1) + drho;
     const real inv = real(1) / rho;
+    if (cls == FLUID && dm.sg > real(0)) {
+        // m*/rho - F/2 - (sg/2) ut = A u - h x u with A = 1 - sg/2  =>  u = (A^2 b + A h x b + h (h.b)) / (A (A^2 + |h|^2))
+        const real hs = real(0.5) * dm.sg, A = real(1) - hs, A2 = A * A;
+        const real bx = mx * inv - real(0.5) * P.Fx - hs * dm.utx, by = my * inv - real(0.5) * P.Fy - hs * dm.uty,
+                   bz = mz * inv - real(0.5) * P.Fz - hs * dm.utz;
+        const real hb = P.hx * bx + P.hy * by + P.hz * bz;
+        const real den = real(1) / (A * (A2 + (P.hx * P.hx + P.hy * P.hy + P.hz * P.hz)));
+        return Macro<real>{rho, (A2 * bx + A * (P.hy * bz - P.hz * by) + P.hx * hb) * den,
+                           (A2 * by + A * (P.hz * bx - P.hx * bz) + P.hy * hb) * den,
+                           (A2 * bz + A * (P.hx * by - P.hy * bx) + P.hz * hb) * den};
+    }
     if (cls == FLUID) {
         // m*/rho - F/2 = u - h x u  =>  u = (b + h x b + h (h.b)) / (1 + |h|^2)
         const real bx = mx * inv - real(0.5) * P.Fx, by = my * inv - real(0.5) * P.Fy, bz = mz * inv - real(0.5) * P.Fz;

@@ -20,7 +20,7 @@ __global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restr
     Macro<real> m{real(1), real(0), real(0), real(0)};
     if (cls != SOLID) {
         load_cell(g, A, P.stride, p);
-        m = local_macros(g, cls, P);
+        m = local_macros(g, cls, P, damp_at(P, x, y, z));
     }
     if (rho) rho[c] = out_t(m.rho);
     if (ux) ux[c] = out_t(m.ux);
@@ -41,7 +41,7 @@ __global__ void mean_sample_kernel(const real *__restrict__ A, const uint8_t *__
     if (cls == SOLID) return;
     real g[Q];
     load_cell(g, A, P.stride, p);
-    const Macro<real> m = local_macros(g, cls, P);
+    const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
     msum[p] += m.ux;
     msum[P.stride + p] += m.uy;
     msum[2 * P.stride + p] += m.uz;

@@ -117,7 +117,7 @@ __device__ __forceinline__ void store_cell_both(real *__restrict__ A, real *__re
     store_cell(B, P, p, x, y, z, fl, lk, g);
     const int cls = fl & CLASS_MASK;
     if ((fl & FEED_BIT) || cls == EQ_FIXED) {
-        const Macro<real> m = local_macros(g, cls, P);
+        const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
         auto w = [&](int s, int comp, real v) {
             fu[comp * P.F + s] = v;
             fu[(3 + comp) * P.F + s] = v;
@@ -166,6 +166,28 @@ __global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, real *_
     store_cell_both(A, B, fu, P, p, x, y, z, fl, 0u, g);
 }
 
+// Re-publish the velocities the outflow cells will read next step from the CURRENT state (both halves of the side
+// array).  Needed when something that enters the local macro inversion changes between steps (lbm_set_damping): the
+// rule is u_loc(G_k, c - n) evaluated with the parameters in force when the step runs (DESIGN.md §3 step 6).
+template <typename real>
+__global__ void refeed_kernel(const real *__restrict__ A, real *__restrict__ fu, const uint8_t *__restrict__ flags, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const uint8_t fl = flags[p];
+    if (!(fl & FEED_BIT)) return;
+    real g[Q];
+    load_cell(g, A, P.stride, p);
+    const Macro<real> m = local_macros(g, fl & CLASS_MASK, P, damp_at(P, x, y, z));
+    outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int s, int comp, real v) {
+        fu[comp * P.F + s] = v;
+        fu[(3 + comp) * P.F + s] = v;
+    });
+}
+
 // ---- a8: precursor plane -> main inlet (config 5) -----------------------------------------------------------------------
 template <typename real>
 __global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, real *__restrict__ dfu, const uint8_t *__restrict__ dflags,
@@ -181,7 +203,7 @@ __global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, real *
     const int sp = pidx(S, sx, y % S.ny, z);
     real g[Q];
     load_cell(g, sA, S.stride, sp);
-    const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, S);
+    const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, S, damp_at(S, sx, y % S.ny, z));
     equilibrium(g, real(0), m.ux, m.uy, m.uz);
     store_cell_both(dA, dB, dfu, D, dp, 0, y, z, fl, 0u, g);
 }

@@ -10,6 +10,8 @@
 // HINT: 0 = default loads / stores, 1 = ld.global.cs / st.global.cs (streaming), 2 = default ld / st.cs, 3 = ld.cs / default st.
 // SPEC: issue the 19 population loads before the flag byte has arrived (no dependent round trip; SOLID cells then
 //       cost their 76 B of reads).
+// DAMP: the damping-zone instantiation (lbm_set_damping); launched only while zones are configured, so the plain
+//       kernel carries none of it.
 #pragma once
 #include "lbm_core.cuh"
 
@@ -67,7 +69,7 @@ inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> 
     return t;
 }
 
-template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0>
+template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
             real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T)
@@ -121,7 +123,8 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
                 g[i] = ld_pop<HINT>(T.src[i] + p);
             });
         }
-        m = collide(g, P);
+        if constexpr (DAMP) m = collide<real, true>(g, P, damp_at(P, x, y, z));
+        else m = collide(g, P);
     } else if (cls != SOLID) { // EQ_FIXED (a3) / EQ_OUTFLOW (a6): f_eq(1, u) of the cell's face velocity (lbm_core.cuh)
         if constexpr (!SPEC) {
             const int sl = eq_slot(P, cls, x, y, z);

@@ -492,3 +492,97 @@ def test_flux_balancing_matches_the_oracle(B, faces, fp64):
     sim.step(50)
     assert max_err(sim, o, f64=fp64) <= (TOL64 if fp64 else TOL32)
     sim.close()
+
+
+# ---------------------------------------------------------------------------------------------- damping zones
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_damping_zones_match_the_oracle(B, fp64):
+    """PAPER.md:175 / Table 1: top sponge + lateral buffer nudging towards the target boundary state.
+    Buildings, veering inlet on three faces + outflow (the paper's open-face set-up) and a periodic variant, Coriolis
+    vector, forcing, LES, zones on five faces with different widths / peaks; 100 steps; FP32 within 1e-5, FP64 within
+    rounding order; macros taken inside the zones (the inversion carries sigma) and the fused time mean."""
+    from oracle import Oracle
+    nx, ny, nz = 50, 42, 24
+    rng = np.random.default_rng(91)
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    for _ in range(5):
+        x0, y0 = int(rng.integers(10, nx - 14)), int(rng.integers(8, ny - 12))
+        hm[y0:y0 + 4, x0:x0 + 5] = int(rng.integers(1, nz - 8))
+    prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+    target = np.stack([prof, 0.2 * prof, np.zeros(nz)])
+    width, peak = (6, 9, 5, 5, 0, 7), (0.05, 0.2, 0.1, 0.1, 0.0, 0.3)
+    fv = (1.0e-3, -0.5e-3, 2.0e-3)
+    for faces in [(3, 4, 3, 3, 1, 2), (0, 0, 0, 0, 1, 2)]:
+        args = (nx, ny, nz, 2e-3, 0.1, 0.0, (1e-6, -5e-7, 0.0), faces)
+        o = Oracle(*args)
+        o.set_coriolis(fv)
+        o.set_flags(hm)
+        o.set_inlet_profile(prof, 0.2 * prof, None)
+        ux0 = np.broadcast_to((0.8 * prof)[:, None, None], (nz, ny, nx)).copy()   # off target: the zones act from step 1
+        o.set_macros(None, ux0, None, None)
+        o.set_damping(width, peak, target)
+        o.mean_config(50, 10)
+        sim = B.Lbm(*args, fp64=fp64)
+        sim.set_coriolis(fv)
+        sim.set_flags(hm)
+        sim.set_inlet_profile(prof, 0.2 * prof, None, f64=True)
+        sim.set_macros(None, ux0, None, None, f64=True)
+        sim.set_damping(width, peak, target)
+        sim.mean_config(50, 10)
+        # the zones must matter at the parity bar, or this test proves nothing
+        ref = Oracle(*args)
+        ref.set_coriolis(fv); ref.set_flags(hm); ref.set_inlet_profile(prof, 0.2 * prof, None); ref.set_macros(None, ux0, None, None)
+        o.step(100)
+        ref.step(100)
+        sim.step(100)
+        assert max(np.abs(a - b).max() for a, b in zip(o.get_macros(), ref.get_macros())) > 1e-3
+        e = max_err(sim, o, f64=fp64)
+        assert e <= (TOL64 if fp64 else TOL32), (faces, fp64, e)
+        gm = sim.get_mean(f64=fp64)
+        om = o.get_mean()
+        assert gm[3] == om[3] == 6
+        em = max(float(np.abs(a.cpu().numpy().astype(np.float64) - b).max()) for a, b in zip(gm[:3], om[:3]))
+        assert em <= (TOL64 if fp64 else TOL32), (faces, fp64, em)
+        # switching the zones off returns to the plain kernel: it follows the undamped oracle from the same state
+        sim.set_damping((0,) * 6, (0,) * 6, None)
+        o.set_damping((0,) * 6, (0,) * 6, None)
+        o.step(20)
+        sim.step(20)
+        e = max_err(sim, o, f64=fp64)
+        assert e <= (TOL64 if fp64 else TOL32), (faces, fp64, e)
+        sim.close()
+
+
+def test_uniform_zone_decays_by_the_trapezoidal_factor_on_the_fp32_path(B):
+    """The closed form that pins the oracle, checked on the GPU path itself: two-layer free-slip slab, width-1 zones on
+    z- and z+ (uniform sigma), uniform flow: u_k - u_t = (u_0 - u_t) q^(k-1) / (1 + sigma/2), q = (1 - s/2)/(1 + s/2)."""
+    nx, ny, nz, sigma = 40, 9, 2, 0.2
+    sim = B.Lbm(nx, ny, nz, 1e-2, 0.1, 0.0, (0, 0, 0), (0, 0, 0, 0, 2, 2))
+    sim.set_flags(None)
+    ut = np.zeros((3, nz)); ut[0] = 0.03; ut[1] = -0.01
+    sim.set_damping((0, 0, 0, 0, 1, 1), (0, 0, 0, 0, sigma, sigma), ut)
+    u0 = np.array([0.08, 0.02])
+    sim.set_macros(None, np.full((nz, ny, nx), u0[0]), np.full((nz, ny, nx), u0[1]), None, f64=True)
+    q = (1 - sigma / 2) / (1 + sigma / 2)
+    for k in (1, 2, 10, 30):
+        sim.step(k - sim.get_step())
+        r, ux, uy, uz = [a.cpu().numpy().astype(np.float64) for a in sim.get_macros()]
+        assert np.abs(ux - (ut[0, 0] + (u0[0] - ut[0, 0]) * q ** (k - 1) / (1 + sigma / 2))).max() < 2e-7
+        assert np.abs(uy - (ut[1, 0] + (u0[1] - ut[1, 0]) * q ** (k - 1) / (1 + sigma / 2))).max() < 2e-7
+        assert np.abs(r - 1).max() < 1e-6 and np.abs(uz).max() < 1e-7
+    sim.close()
+
+
+def test_set_damping_argument_errors(B):
+    sim = B.Lbm(8, 8, 8, 1e-2, 0.1, 0.0, (0, 0, 0), (0, 0, 0, 0, 1, 2))
+    sim.set_flags(None)
+    with pytest.raises(B.LbmError):
+        sim.set_damping((1,) * 6, (1.5,) * 6, np.zeros((3, 8)))
+    with pytest.raises(B.LbmError):
+        sim.set_damping((-1, 0, 0, 0, 0, 0), (0.1,) * 6, np.zeros((3, 8)))
+    with pytest.raises(B.LbmError):
+        sim.set_damping((2,) * 6, (0.1,) * 6, None)
+    sim.set_damping((0,) * 6, (0.5,) * 6, None)   # off: target not needed
+    sim.step(2)
+    sim.close()
