@@ -81,6 +81,7 @@ struct lbm {
     long launches;
     int variant;
     bool damp_on;   // damping zones configured (the DAMP instantiation of the step kernel runs)
+    int dlo[3], dhi[3]; // the zone-free inner box
     std::string err;
 
     void *bufA() const { return ws + L.off_A; }
@@ -138,6 +139,7 @@ Params<real> make_params(const lbm_t *h)
     P.inv1ph2 = (real)(1.0 / (1.0 + 0.25 * (h->fv[0] * h->fv[0] + h->fv[1] * h->fv[1] + h->fv[2] * h->fv[2])));
     P.Fx = (real)h->F[0]; P.Fy = (real)h->F[1]; P.Fz = (real)h->F[2];
     P.damp = h->damp_on ? (const real *)h->damp() : nullptr;
+    for (int a = 0; a < 3; ++a) { P.dlo[a] = h->dlo[a]; P.dhi[a] = h->dhi[a]; }
     return P;
 }
 
@@ -559,6 +561,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     h->stream = (cudaStream_t)cuda_stream;
     h->cur = 0; h->have_flags = false; h->step = 0;
     h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false;
+    for (int a = 0; a < 3; ++a) { h->dlo[a] = 0; h->dhi[a] = 0; }
     if (dev_workspace) {
         if (workspace_bytes < h->L.total || ((uintptr_t)dev_workspace % ALIGN) != 0 || !is_device_ptr(dev_workspace)) {
             delete h;
@@ -663,6 +666,11 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
     if (e != cudaSuccess) return fail(h, LBM_ECUDA, std::string("set_damping: ") + cudaGetErrorString(e));
+    for (int a = 0; a < 3; ++a) {
+        const bool lo_on = width[2 * a] > 0 && peak[2 * a] > 0.0, hi_on = width[2 * a + 1] > 0 && peak[2 * a + 1] > 0.0;
+        h->dlo[a] = lo_on ? std::min(width[2 * a], n[a]) : 0;
+        h->dhi[a] = hi_on ? std::max(n[a] - width[2 * a + 1], 0) : n[a];
+    }
     h->damp_on = true;
     return refeed();
 }

@@ -76,6 +76,7 @@ struct Params {
     // coefficient tables sx[nx], sy[ny], sz[nz] (each the larger of the axis' two face ramps) followed by the target
     // profile ut[3][nz];  sigma(x,y,z) = max(sx[x], sy[y], sz[z])
     const real *damp;
+    int dlo[3], dhi[3]; // cells with dlo <= (x,y,z) < dhi lie outside every zone: no table look-up there
 };
 
 // Interior x = 0 sits at padded x = XOFF = 8: every interior row starts on a 32-byte sector boundary (and ends on one
@@ -117,7 +118,8 @@ struct Damp { real sg, utx, uty, utz; };
 template <typename real>
 __device__ __forceinline__ Damp<real> damp_at(const Params<real> &P, int x, int y, int z)
 {
-    if (!P.damp) return Damp<real>{real(0), real(0), real(0), real(0)};
+    if (!P.damp || (x >= P.dlo[0] && x < P.dhi[0] && y >= P.dlo[1] && y < P.dhi[1] && z >= P.dlo[2] && z < P.dhi[2]))
+        return Damp<real>{real(0), real(0), real(0), real(0)};
     const real *d = P.damp;
     const real sg = fmax(fmax(d[x], d[P.nx + y]), d[P.nx + P.ny + z]);
     const real *t = d + (P.nx + P.ny + P.nz);
