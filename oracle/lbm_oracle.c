@@ -90,6 +90,9 @@ typedef struct oracle {
     double *ub;   /* [cell][3] prescribed velocity of EQ_FIXED cells */
     double *sig;  /* [cell] damping coefficient sigma(x) of the sponge / buffer zones (NULL = none) */
     double *ut;   /* [3][nz] target state u_t(z) the damping relaxes towards */
+    int nmodes;   /* synthetic inflow turbulence: number of Fourier modes (0 = off) */
+    double *modes; /* [nmodes][9] = kappa[3], sigma[3], psi, omega, dkappa */
+    double *uhat; /* [nmodes] mode amplitudes sqrt(E(|kappa|) dkappa) */
     long step;
     double *msum; /* [cell][3] */
     long mcount, mstart;
@@ -317,7 +320,7 @@ oracle_t *oracle_create(int nx, int ny, int nz, double nu0, double Cs, double fc
 void oracle_destroy(oracle_t *o)
 {
     if (!o) return;
-    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o->sig); free(o->ut); free(o);
+    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o->sig); free(o->ut); free(o->modes); free(o->uhat); free(o);
 }
 
 /* Damping zones (see collide()).  width[k] (cells) and peak[k] for the six faces x-,x+,y-,y+,z-,z+; a cell at
@@ -439,6 +442,101 @@ int oracle_get_links(const oracle_t *o, uint32_t *out)
     return 0;
 }
 
+/* ---- synthetic inflow turbulence ------------------------------------------------------------------------------
+ * PAPER.md:160 "On-the-fly synthetic turbulent fluctuations are superposed on this mean field" (which is "held fixed
+ * throughout the LBM-LES integration"); Table 1 PAPER.md:86 "synthetic von Karman fluctuations on active inflow
+ * cells".  The formulation is in Supplementary S7 (missing); reading (DESIGN.md §4 reading 21) = the textbook random
+ * Fourier mode synthesis (Kraichnan 1970; the form in Davidson's synthetic-inlet notes, the author PAPER.md:209 cites):
+ *     u'(x, t) = 2 sum_n uhat_n cos(kappa_n . x + psi_n - omega_n t) sigma_n,      sigma_n . kappa_n = 0,
+ *     uhat_n = sqrt(E(|kappa_n|) dkappa_n),
+ * with the von Karman-Pao energy spectrum
+ *     E(k) = alpha (u_rms^2 / k_e) (k/k_e)^4 / [1 + (k/k_e)^2]^(17/6) exp(-2 (k/k_eta)^2),   alpha = 1.453.
+ * x = cell indices (lattice units), t = step number.  The random draws (kappa_n, sigma_n, psi_n, omega_n, dkappa_n)
+ * are INPUTS.  An EQ_FIXED cell is an "active inflow cell" when its mean velocity points into the domain,
+ * ub . n < 0 with n the outward normal of its owner face; only those carry u'.  After k steps such a cell holds
+ * f_eq(1, ub + u'(x, k)). */
+static double vk_spectrum(double k, double u_rms, double k_e, double k_eta)
+{
+    const double alpha = 1.453;
+    double r = k / k_e;
+    double E = alpha * (u_rms * u_rms / k_e) * pow(r, 4.0) / pow(1.0 + r * r, 17.0 / 6.0);
+    if (k_eta > 0.0) E *= exp(-2.0 * (k / k_eta) * (k / k_eta));
+    return E;
+}
+int oracle_vk_spectrum(int n, const double *k, double u_rms, double k_e, double k_eta, double *E)
+{
+    for (int i = 0; i < n; ++i) E[i] = vk_spectrum(k[i], u_rms, k_e, k_eta);
+    return 0;
+}
+
+static int fixed_face(const oracle_t *o, int x, int y, int z);
+
+/* u'(x, t) of the stored modes */
+static void fluctuation(const oracle_t *o, int x, int y, int z, double t, double up[3])
+{
+    up[0] = up[1] = up[2] = 0.0;
+    for (int n = 0; n < o->nmodes; ++n) {
+        const double *m = o->modes + 9 * n;
+        double phase = m[0] * x + m[1] * y + m[2] * z + m[6] - m[7] * t;
+        double c = 2.0 * o->uhat[n] * cos(phase);
+        for (int a = 0; a < 3; ++a) up[a] += c * m[3 + a];
+    }
+}
+
+/* boundary velocity of EQ_FIXED cell (x,y,z) at time t: mean + fluctuation on active inflow cells */
+static void boundary_velocity(const oracle_t *o, int x, int y, int z, double t, double u[3])
+{
+    long cell = cell_of(o, x, y, z);
+    for (int a = 0; a < 3; ++a) u[a] = o->ub[3 * cell + a];
+    if (o->nmodes <= 0) return;
+    int k = fixed_face(o, x, y, z);
+    if (k < 0) return;
+    double un = (k % 2 ? 1.0 : -1.0) * u[k / 2]; /* ub . n, n outward */
+    if (!(un < 0.0)) return;
+    double up[3];
+    fluctuation(o, x, y, z, t, up);
+    for (int a = 0; a < 3; ++a) u[a] += up[a];
+}
+
+static void write_fixed_cells_at(oracle_t *o, double t)
+{
+    for (int z = 0; z < o->nz; ++z)
+        for (int y = 0; y < o->ny; ++y)
+            for (int x = 0; x < o->nx; ++x) {
+                long cell = cell_of(o, x, y, z);
+                if (o->cls[cell] != C_EQ_FIXED) continue;
+                double u[3], g[Q];
+                boundary_velocity(o, x, y, z, t, u);
+                feq(1.0, u, g);
+                memcpy(o->G + cell * Q, g, sizeof g);
+                memcpy(o->Gn + cell * Q, g, sizeof g);
+            }
+}
+
+/* modes = [n][9]: kappa[3], sigma[3], psi, omega, dkappa.  n = 0 switches the fluctuations off (cells return to the
+ * mean).  The EQ_FIXED cells are rewritten for the current step at once. */
+int oracle_set_inflow_turbulence(oracle_t *o, int n, const double *modes, double u_rms, double k_e, double k_eta)
+{
+    if (!o || n < 0 || (n > 0 && (!modes || !(k_e > 0.0) || u_rms < 0.0 || k_eta < 0.0))) return -1;
+    if (!o->have_flags) return -3;
+    free(o->modes); free(o->uhat); o->modes = NULL; o->uhat = NULL; o->nmodes = 0;
+    if (n > 0) {
+        o->modes = (double *)malloc(sizeof(double) * 9 * n);
+        o->uhat = (double *)malloc(sizeof(double) * n);
+        if (!o->modes || !o->uhat) return -4;
+        memcpy(o->modes, modes, sizeof(double) * 9 * n);
+        for (int i = 0; i < n; ++i) {
+            const double *m = modes + 9 * i;
+            double k = sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]);
+            if (!(m[8] >= 0.0)) return -1;
+            o->uhat[i] = sqrt(vk_spectrum(k, u_rms, k_e, k_eta) * m[8]);
+        }
+        o->nmodes = n;
+    }
+    write_fixed_cells_at(o, (double)o->step);
+    return 0;
+}
+
 static void write_eq_fixed_cell(oracle_t *o, long cell)
 {
     double g[Q];
@@ -450,7 +548,7 @@ static void write_eq_fixed_cell(oracle_t *o, long cell)
 /* step 5 (profile form): every EQ_FIXED cell gets f_eq(1, (u[z],v[z],w[z])) */
 int oracle_set_inlet_profile(oracle_t *o, const double *u, const double *v, const double *w)
 {
-    if (!o->have_flags) return -3;
+    if (!o->have_flags || o->nmodes > 0) return -3; /* the mean is fixed while fluctuations ride on it */
     for (int z = 0; z < o->nz; ++z)
         for (int y = 0; y < o->ny; ++y)
             for (int x = 0; x < o->nx; ++x) {
@@ -469,7 +567,7 @@ int oracle_set_inlet_profile(oracle_t *o, const double *u, const double *v, cons
  * (ny,nx) for z faces. */
 int oracle_set_inlet_plane(oracle_t *o, int face, const double *uvw)
 {
-    if (!o->have_flags) return -3;
+    if (!o->have_flags || o->nmodes > 0) return -3;
     if (face < 0 || face > 5) return -1;
     int axis = face / 2;
     int n[3] = {o->nx, o->ny, o->nz};
@@ -552,7 +650,7 @@ static int fixed_face(const oracle_t *o, int x, int y, int z)
 
 int oracle_balance_flux(oracle_t *o, double *flux_before, double *flux_after)
 {
-    if (!o || !o->have_flags) return -3;
+    if (!o || !o->have_flags || o->nmodes > 0) return -3;
     double phi = 0.0, phi2 = 0.0;
     long n = 0;
     for (int pass = 0; pass < 3; ++pass) {
@@ -617,6 +715,11 @@ int oracle_step(oracle_t *o, int nsteps)
                         double r, u[3] = {0, 0, 0};
                         if (p[k / 2] >= 0 && p[k / 2] < n[k / 2])
                             local_macros(o, o->G, cell_of(o, p[0], p[1], p[2]), &r, u);
+                        feq(1.0, u, gn);
+                    } else if (cl == C_EQ_FIXED && o->nmodes > 0) {
+                        /* step 5 with fluctuations: the state of step k+1 carries u'(x, k+1) */
+                        double u[3];
+                        boundary_velocity(o, x, y, z, (double)(o->step + 1), u);
                         feq(1.0, u, gn);
                     } else {
                         /* SOLID: inert; EQ_FIXED (step 5): unchanged */

@@ -49,7 +49,8 @@ def _load():
                  "oracle_get_macros", "oracle_mean_reset", "oracle_get_mean",
                  "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell",
                  "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux",
-                 "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping"):
+                 "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping",
+                 "oracle_vk_spectrum", "oracle_set_inflow_turbulence"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -126,6 +127,16 @@ def collide_cell_damped(f, nu0, Cs, fvec, F, sigma, ut):
     return g, rho.value, u, tau.value
 
 
+def vk_spectrum(k, u_rms, k_e, k_eta=0.0):
+    """von Karman-Pao energy spectrum E(k) (k_eta = 0: no Pao cut-off)."""
+    lib = _load()
+    k, kp = _d(np.atleast_1d(k))
+    E = np.zeros(k.size)
+    lib.oracle_vk_spectrum(C.c_int(k.size), kp, C.c_double(u_rms), C.c_double(k_e), C.c_double(k_eta),
+                           E.ctypes.data_as(C.c_void_p))
+    return E
+
+
 class Oracle:
     """FP64 CPU LBM; same call names as the product binding, float64 arrays."""
 
@@ -170,6 +181,17 @@ class Oracle:
         s = np.zeros(self.shape)
         self._chk(self._lib.oracle_get_damping(C.c_void_p(self._h), s.ctypes.data_as(C.c_void_p)), "get_damping")
         return s
+
+    def set_inflow_turbulence(self, modes, u_rms=0.0, k_e=1.0, k_eta=0.0):
+        """Synthetic von Karman fluctuations on active inflow cells; modes [n][9] = kappa, sigma, psi, omega, dkappa
+        (None / empty: off)."""
+        if modes is None or len(modes) == 0:
+            self._chk(self._lib.oracle_set_inflow_turbulence(C.c_void_p(self._h), 0, None, C.c_double(0), C.c_double(1),
+                                                             C.c_double(0)), "set_inflow_turbulence")
+            return
+        m, mp = _d(np.asarray(modes, dtype=np.float64).reshape(-1, 9))
+        self._chk(self._lib.oracle_set_inflow_turbulence(C.c_void_p(self._h), m.shape[0], mp, C.c_double(u_rms),
+                                                         C.c_double(k_e), C.c_double(k_eta)), "set_inflow_turbulence")
 
     def balance_flux(self):
         """Global flux-balancing correction of the EQ_FIXED face velocities; returns (flux_before, flux_after)."""

@@ -76,6 +76,30 @@ def veering_profile(nz: int, u_ref: float, zeta_ref: float, z0: float, seed: int
     return (speed * np.cos(theta)).astype(np.float32), (speed * np.sin(theta)).astype(np.float32)
 
 
+def inflow_modes(n: int, seed: int, k_min: float, k_max: float, convect=(0.0, 0.0, 0.0)) -> np.ndarray:
+    """The random draws of the synthetic inflow fluctuations (Table 1), as an input table
+    [n][9] = kappa[3], sigma[3], psi, omega, dkappa — no spectrum, no amplitudes: those are the method's arithmetic
+    and live in the library / the oracle.  Wavenumber magnitudes are n equal shells between k_min and k_max (shell
+    centres, dkappa = the shell width); directions are uniform on the sphere (phi ~ U(0, 2 pi), cos(theta) ~ U(-1, 1));
+    sigma is a unit vector in the plane normal to kappa at a uniform angle; psi ~ U(0, 2 pi); omega = kappa . convect
+    (frozen turbulence carried with the velocity `convect`, lattice units)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    dk = (k_max - k_min) / n
+    kmag = k_min + (np.arange(n) + 0.5) * dk
+    phi = rng.uniform(0.0, 2.0 * math.pi, n)
+    ct = rng.uniform(-1.0, 1.0, n)
+    st = np.sqrt(1.0 - ct * ct)
+    e = np.stack([st * np.cos(phi), st * np.sin(phi), ct], axis=1)                  # unit wave-vector directions
+    a = np.stack([-np.sin(phi), np.cos(phi), np.zeros(n)], axis=1)                  # two unit vectors spanning the normal plane
+    b = np.cross(e, a)
+    al = rng.uniform(0.0, 2.0 * math.pi, n)
+    sig = np.cos(al)[:, None] * a + np.sin(al)[:, None] * b
+    psi = rng.uniform(0.0, 2.0 * math.pi, n)
+    kap = kmag[:, None] * e
+    om = kap @ np.asarray(convect, dtype=np.float64)
+    return np.concatenate([kap, sig, psi[:, None], om[:, None], np.full((n, 1), dk)], axis=1)
+
+
 # --------------------------------------------------------------------------- heightmaps
 
 def block_heightmap(nx, ny, x0, x1, y0, y1, h) -> np.ndarray:
