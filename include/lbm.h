@@ -122,6 +122,25 @@ int lbm_balance_flux(lbm_t *h, double *flux_before, double *flux_after);
  * Returns LBM_EINVAL for a negative width, a peak outside [0, 1] or a non-finite / device target.  Synchronises. */
 int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const double *target);
 
+/* Synthetic inflow fluctuations ("On-the-fly synthetic turbulent fluctuations are superposed on this mean
+ * field", the mean being "held fixed throughout the LBM-LES integration"; Table 1 PAPER.md:86 "synthetic von Karman
+ * fluctuations on active inflow cells").  The formulation is in the paper's Supplementary S7 (missing); reading
+ * (DESIGN.md §4 reading 21) = random Fourier modes with the von Karman-Pao spectrum:
+ *     u'(x, t) = 2 sum_n uhat_n cos(kappa_n . x + psi_n - omega_n t) sigma_n,   uhat_n = sqrt(E(|kappa_n|) dkappa_n),
+ *     E(k) = 1.453 (u_rms^2 / k_e) (k/k_e)^4 / [1 + (k/k_e)^2]^(17/6) exp(-2 (k/k_eta)^2)      (k_eta = 0: no cut-off),
+ * x = cell indices, t = step number, all in lattice units.  The random draws are the caller's: modes = HOST array
+ * [n_modes][9] = kappa[3], sigma[3] (unit, normal to kappa), psi, omega, dkappa  (omega = kappa . U_c gives a frozen
+ * pattern carried with U_c).  Active inflow cells = EQ_FIXED cells whose mean velocity points into the domain
+ * (u_b . n < 0, n = outward normal of the owner face); after k steps such a cell holds f_eq(1, u_b + u'(x, k)); every
+ * other EQ_FIXED cell keeps the mean.  The mean is the boundary state in force when the call is made: while
+ * fluctuations are on, lbm_set_inlet_profile / _plane, lbm_feed_inlet and lbm_balance_flux return LBM_ESTATE.
+ * n_modes = 0 switches them off and restores the mean (modes may be NULL).  lbm_set_flags switches them off too.
+ * Cost per step: one extra small launch over the face slots (n_modes cosines per active cell), no lattice traffic.
+ * LBM_EINVAL: n_modes < 0 or > LBM_MAX_INFLOW_MODES, k_e <= 0, u_rms < 0, k_eta < 0, dkappa < 0, non-finite or device
+ * table.  Needs flags (else LBM_ESTATE).  Synchronises. */
+#define LBM_MAX_INFLOW_MODES 1024
+int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double u_rms, double k_e, double k_eta);
+
 /* Config-5 coupling, device to device, stream-ordered on dst's stream: local macros of src on the plane
  * x = src_x_plane are written as f_eq(1, u) into the EQ_FIXED cells of dst's x- face, tiling y modulo
  * src's ny; nz must match; SOLID src cells feed u = 0.  Both handles must share precision. */

@@ -605,6 +605,7 @@ int oracle_set_macros(oracle_t *o, const double *rho, const double *ux, const do
         memcpy(o->Gn + cell * Q, g, sizeof g);
     }
     o->step = 0;
+    if (o->nmodes > 0) write_fixed_cells_at(o, 0.0); /* the step counter restarts: inflow cells carry u'(x, 0) */
     return 0;
 }
 

@@ -27,7 +27,7 @@ SYMBOLS = [
     "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
     "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
-    "lbm_set_damping",
+    "lbm_set_damping", "lbm_set_inflow_turbulence",
 ]
 
 
@@ -57,6 +57,7 @@ def load_library():
     lib.lbm_set_coriolis.argtypes = [vp, vp]
     lib.lbm_balance_flux.argtypes = [vp, vp, vp]
     lib.lbm_set_damping.argtypes = [vp, vp, vp, vp]
+    lib.lbm_set_inflow_turbulence.argtypes = [vp, i, vp, C.c_double, C.c_double, C.c_double]
     lib.lbm_set_flags.argtypes = [vp, vp]
     for n in ("lbm_set_inlet_profile", "lbm_set_inlet_profile_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
@@ -194,6 +195,18 @@ class Lbm:
                 raise ValueError("target must be [3][nz]")
         self._chk(self._lib.lbm_set_damping(self._h, w.ctypes.data, pk.ctypes.data, t.ctypes.data if t is not None else None),
                   "set_damping")
+
+    def set_inflow_turbulence(self, modes, u_rms=0.0, k_e=1.0, k_eta=0.0):
+        """Synthetic von Karman fluctuations on active inflow cells; host table [n][9] = kappa, sigma, psi, omega,
+        dkappa (None / empty: off)."""
+        if modes is None or len(modes) == 0:
+            self._chk(self._lib.lbm_set_inflow_turbulence(self._h, 0, None, 0.0, 1.0, 0.0), "set_inflow_turbulence")
+            return
+        m = np.ascontiguousarray(modes, dtype=np.float64)
+        if m.ndim != 2 or m.shape[1] != 9:
+            raise ValueError("modes must be [n][9]")
+        self._chk(self._lib.lbm_set_inflow_turbulence(self._h, m.shape[0], m.ctypes.data, float(u_rms), float(k_e), float(k_eta)),
+                  "set_inflow_turbulence")
 
     def balance_flux(self):
         """Global flux-balancing correction of the EQ_FIXED face velocities; returns (flux_before, flux_after)."""

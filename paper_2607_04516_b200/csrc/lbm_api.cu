@@ -17,13 +17,14 @@ using namespace lbmk;
 namespace {
 
 constexpr size_t ALIGN = 256;
+constexpr int MAX_MODES = LBM_MAX_INFLOW_MODES;
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 // Halo-padded box (lbm_core.cuh): x pitch = nx + 2 rounded up to 32, ny + 2 rows, nz + 2 planes.
 struct Layout {
     int px, py;
     long long Np, stride;
-    size_t off_A, off_B, off_flags, off_links, off_fu, off_mean, off_damp, off_scratch, total;
+    size_t off_A, off_B, off_flags, off_links, off_fu, off_fum, off_modes, off_mean, off_damp, off_scratch, total;
     size_t fu_bytes;
     size_t scratch_bytes;
 };
@@ -44,6 +45,9 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
     // outflow-velocity side buffer (a6): 2 halves x 3 components x one slot per face-plane cell of all six faces (upper bound)
     L.fu_bytes = align_up((size_t)2 * 3 * 2 * ((size_t)ny * nz + (size_t)nx * nz + (size_t)nx * ny) * rs, ALIGN);
     L.off_fu = o; o += L.fu_bytes;
+    // mean boundary velocity of the EQ slots (3 components) and the mode table of the synthetic inflow fluctuations
+    L.off_fum = o; o += align_up(L.fu_bytes / 2, ALIGN);
+    L.off_modes = o; o += align_up((size_t)MAX_MODES * 8 * sizeof(double), ALIGN);
     L.off_mean = o; if (want_mean) o += align_up((size_t)3 * L.stride * rs, ALIGN);
     // damping tables (lbm_set_damping): sx[nx], sy[ny], sz[nz], ut[3][nz]
     L.off_damp = o; o += align_up(((size_t)nx + ny + 4 * (size_t)nz) * rs, ALIGN);
@@ -82,6 +86,7 @@ struct lbm {
     int variant;
     bool damp_on;   // damping zones configured (the DAMP instantiation of the step kernel runs)
     int dlo[3], dhi[3]; // the zone-free inner box
+    int nmodes;     // synthetic inflow fluctuations: modes in use (0 = off)
     std::string err;
 
     void *bufA() const { return ws + L.off_A; }
@@ -92,6 +97,8 @@ struct lbm {
     uint32_t *links() const { return (uint32_t *)(ws + L.off_links); }
     void *fu() const { return ws + L.off_fu; }
     void *mean() const { return want_mean ? ws + L.off_mean : nullptr; }
+    void *fum() const { return ws + L.off_fum; }
+    double *modes() const { return (double *)(ws + L.off_modes); }
     void *damp() const { return ws + L.off_damp; }
     void *scratch() const { return ws + L.off_scratch; }
     long long N() const { return (long long)nx * ny * nz; }
@@ -262,6 +269,7 @@ template <typename real, typename in_t>
 int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, const in_t *w, size_t count)
 {
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inlet: flags not set");
+    if (h->nmodes > 0) return fail(h, LBM_ESTATE, "set_inlet: the mean boundary state is fixed while inflow fluctuations are on");
     if (!u) return fail(h, LBM_EINVAL, "set_inlet: u is NULL");
     const Params<real> P = make_params<real>(h);
     InBuf in[3];
@@ -309,6 +317,9 @@ int set_inlet_plane_any(lbm_t *h, int face, const in_t *uvw)
     return rc;
 }
 
+template <typename real>
+int do_fluct(lbm_t *h, double t, bool cells);
+
 template <typename real, typename in_t>
 int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, const in_t *uz)
 {
@@ -328,6 +339,7 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     }
     release_in(h, in, 4);
     if (!rc) { h->step = 0; h->cur = 0; }
+    if (!rc && h->nmodes > 0) rc = do_fluct<real>(h, 0.0, true); // the step counter restarts: the inflow cells carry u'(x, 0)
     return rc;
 }
 
@@ -378,6 +390,19 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
     return launch_step_as<real, 0, false, 256, 2>(h, P, sample);
 }
 
+// boundary velocities of time t for the EQ_FIXED slots (mean + fluctuations on active inflow cells); cells = also rewrite
+// the cells' populations (set-up / switch-off / re-initialisation)
+template <typename real>
+int do_fluct(lbm_t *h, double t, bool cells)
+{
+    const Params<real> P = make_params<real>(h);
+    if (P.F == 0) return LBM_OK;
+    const int B = 128;
+    if (cells) fluct_kernel<real, true><<<blocks_for(P.F, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), (const real *)h->fum(), h->flags(), h->modes(), h->nmodes, t, P);
+    else fluct_kernel<real, false><<<blocks_for(P.F, B), B, 0, h->stream>>>(nullptr, nullptr, (real *)h->fu(), (const real *)h->fum(), h->flags(), h->modes(), h->nmodes, t, P);
+    return check_launch(h, "fluct_kernel");
+}
+
 template <typename real>
 int do_step(lbm_t *h, int n)
 {
@@ -385,7 +410,11 @@ int do_step(lbm_t *h, int n)
     for (int it = 0; it < n; ++it) {
         const long k = h->step + 1;
         const bool sample = h->mevery > 0 && k >= h->mstart && (k - h->mstart) % h->mevery == 0;
-        int rc = launch_step<real>(h, P, sample);
+        int rc = LBM_OK;
+        // the EQ_FIXED cells write G_{k+1} = f_eq(1, u_b(k+1)) in this launch: publish u_b(k+1) first
+        if (h->nmodes > 0) rc = do_fluct<real>(h, (double)k, false);
+        if (rc) return rc;
+        rc = launch_step<real>(h, P, sample);
         if (rc) return rc;
         h->cur ^= 1;
         h->step = k;
@@ -560,7 +589,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     h->L = make_layout(nx, ny, nz, h->want_mean, h->fp64);
     h->stream = (cudaStream_t)cuda_stream;
     h->cur = 0; h->have_flags = false; h->step = 0;
-    h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false;
+    h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false; h->nmodes = 0;
     for (int a = 0; a < 3; ++a) { h->dlo[a] = 0; h->dhi[a] = 0; }
     if (dev_workspace) {
         if (workspace_bytes < h->L.total || ((uintptr_t)dev_workspace % ALIGN) != 0 || !is_device_ptr(dev_workspace)) {
@@ -675,9 +704,52 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
     return refeed();
 }
 
+int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double u_rms, double k_e, double k_eta)
+{
+    if (!h) return LBM_EINVAL;
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inflow_turbulence: flags not set");
+    if (n_modes < 0 || n_modes > MAX_MODES) return fail(h, LBM_EINVAL, "set_inflow_turbulence: n_modes out of range");
+    auto rewrite = [&](double t) { return h->fp64 ? do_fluct<double>(h, t, true) : do_fluct<float>(h, t, true); };
+    if (n_modes == 0) {
+        if (h->nmodes == 0) return LBM_OK;
+        h->nmodes = 0;
+        int rc = rewrite((double)h->step); // no modes: the cells return to the mean
+        if (!rc) CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+        return rc;
+    }
+    if (!modes || is_device_ptr(modes)) return fail(h, LBM_EINVAL, "set_inflow_turbulence: modes must be a host array");
+    if (!(k_e > 0.0) || !(u_rms >= 0.0) || !(k_eta >= 0.0) || !std::isfinite(k_e) || !std::isfinite(u_rms) || !std::isfinite(k_eta))
+        return fail(h, LBM_EINVAL, "set_inflow_turbulence: need k_e > 0, u_rms >= 0, k_eta >= 0");
+    // device table [n][8]: kappa, a = 2 uhat sigma, psi, omega;  uhat = sqrt(E(|kappa|) dkappa), E = von Karman-Pao
+    std::vector<double> t((size_t)n_modes * 8);
+    for (int n = 0; n < n_modes; ++n) {
+        const double *m = modes + 9 * (size_t)n;
+        for (int c = 0; c < 9; ++c)
+            if (!std::isfinite(m[c])) return fail(h, LBM_EINVAL, "set_inflow_turbulence: table not finite");
+        if (m[8] < 0.0) return fail(h, LBM_EINVAL, "set_inflow_turbulence: dkappa < 0");
+        const double k = std::sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2]), r = k / k_e;
+        double E = 1.453 * (u_rms * u_rms / k_e) * (r * r) * (r * r) / std::pow(1.0 + r * r, 17.0 / 6.0);
+        if (k_eta > 0.0) E *= std::exp(-2.0 * (k / k_eta) * (k / k_eta));
+        const double amp = 2.0 * std::sqrt(E * m[8]);
+        double *d = t.data() + 8 * (size_t)n;
+        d[0] = m[0]; d[1] = m[1]; d[2] = m[2];
+        d[3] = amp * m[3]; d[4] = amp * m[4]; d[5] = amp * m[5];
+        d[6] = m[6]; d[7] = m[7];
+    }
+    const Layout &L = h->L;
+    if (h->nmodes == 0) // switching on: what the EQ slots hold now is the mean (both halves agree for EQ_FIXED slots)
+        CUDA_TRY(h, cudaMemcpyAsync(h->fum(), h->fu(), L.fu_bytes / 2, cudaMemcpyDeviceToDevice, h->stream));
+    CUDA_TRY(h, cudaMemcpyAsync(h->modes(), t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    h->nmodes = n_modes;
+    int rc = rewrite((double)h->step);
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream)); // t (host staging) must outlive the copy
+    return rc;
+}
+
 int lbm_set_flags(lbm_t *h, const int32_t *height)
 {
     if (!h) return LBM_EINVAL;
+    h->nmodes = 0; // a new voxelisation resets the state and the boundary velocities
     return h->fp64 ? do_set_flags<double>(h, height) : do_set_flags<float>(h, height);
 }
 
@@ -690,6 +762,7 @@ int lbm_feed_inlet(lbm_t *dst, const lbm_t *src, int src_x_plane)
 {
     if (!dst || !src) return LBM_EINVAL;
     if (!dst->have_flags || !src->have_flags) return fail(dst, LBM_ESTATE, "feed_inlet: flags not set");
+    if (dst->nmodes > 0) return fail(dst, LBM_ESTATE, "feed_inlet: the mean boundary state is fixed while inflow fluctuations are on");
     if (dst->fp64 != src->fp64) return fail(dst, LBM_EINVAL, "feed_inlet: precision mismatch");
     if (dst->nz != src->nz) return fail(dst, LBM_EINVAL, "feed_inlet: nz mismatch");
     if (src_x_plane < 0 || src_x_plane >= src->nx) return fail(dst, LBM_EINVAL, "feed_inlet: plane out of range");
@@ -700,6 +773,7 @@ int lbm_balance_flux(lbm_t *h, double *flux_before, double *flux_after)
 {
     if (!h) return LBM_EINVAL;
     if (!h->have_flags) return fail(h, LBM_ESTATE, "balance_flux: flags not set");
+    if (h->nmodes > 0) return fail(h, LBM_ESTATE, "balance_flux: the mean boundary state is fixed while inflow fluctuations are on");
     return h->fp64 ? do_balance_flux<double>(h, flux_before, flux_after) : do_balance_flux<float>(h, flux_before, flux_after);
 }
 

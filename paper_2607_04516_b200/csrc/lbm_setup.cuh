@@ -166,6 +166,64 @@ __global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, real *_
     store_cell_both(A, B, fu, P, p, x, y, z, fl, 0u, g);
 }
 
+// ---- synthetic inflow fluctuations (lbm_set_inflow_turbulence; Table 1) -------------------
+// One thread per face-velocity slot.  For an EQ_FIXED cell whose MEAN velocity (fum) points into the domain
+// (ub . n < 0, n = outward normal of the owner face) the boundary velocity of time t is
+//     u_b = ub + sum_n a_n cos(kappa_n . x + psi_n - omega_n t),     a_n = 2 sqrt(E(|kappa_n|) dkappa_n) sigma_n,
+// x = cell indices (DESIGN.md §4 reading 21); all other EQ_FIXED cells keep the mean.  modes = [n][8] doubles:
+// kappa[3], a[3], psi, omega (amplitudes folded on the host).  The phase is formed and reduced to [-pi, pi] in FP64 (t
+// reaches 1e4-1e5 steps, an FP32 phase would lose 1e-3 rad), the cosine is taken in the handle's precision.
+// The value goes to both halves of the side array: the step kernel re-expands f_eq(1, u_b) from it (a3).  CELLS = true
+// (set-up, switch-off, restart): the cell's populations are rewritten in both buffers as well.
+template <typename real, bool CELLS>
+__global__ void fluct_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const real *__restrict__ fum,
+                             const uint8_t *__restrict__ flags, const double *__restrict__ modes, int nmodes, double t, Params<real> P)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.F) return;
+    int k = 5;
+    while (k > 0 && s < P.foff[k]) --k; // the last face whose first slot is <= s (faces without slots share their successor's offset)
+    if (P.face[k] != FACE_EQ_FIXED) return;
+    const int axis = k >> 1;
+    const int n1 = axis == 0 ? P.ny : P.nx;
+    const int r = s - P.foff[k], j1 = r % n1, j2 = r / n1;
+    const int nn[3] = {P.nx, P.ny, P.nz};
+    const int fixed = (k & 1) ? nn[axis] - 1 : 0;
+    int x, y, z;
+    if (axis == 0) { x = fixed; y = j1; z = j2; }
+    else if (axis == 1) { x = j1; y = fixed; z = j2; }
+    else { x = j1; y = j2; z = fixed; }
+    if (eq_owner(P, FACE_EQ_FIXED, x, y, z) != k) return; // an edge cell belongs to the first EQ_FIXED face it lies on
+    const int p = pidx(P, x, y, z);
+    const uint8_t fl = flags[p];
+    if ((fl & CLASS_MASK) != EQ_FIXED) return;
+    const real mu[3] = {fum[s], fum[P.F + s], fum[2 * P.F + s]};
+    real u0 = mu[0], u1 = mu[1], u2 = mu[2];
+    const real un = (k & 1) ? mu[axis] : -mu[axis];
+    if (un < real(0)) {
+        real a0 = real(0), a1 = real(0), a2 = real(0);
+        for (int n = 0; n < nmodes; ++n) {
+            const double *m = modes + 8 * n;
+            double ph = fma(m[0], (double)x, fma(m[1], (double)y, fma(m[2], (double)z, fma(-m[7], t, m[6]))));
+            real c;
+            if constexpr (sizeof(real) == 8) c = cos(ph);
+            else {
+                ph = fma(-6.283185307179586, rint(ph * 0.15915494309189535), ph);
+                c = cosf((float)ph);
+            }
+            a0 = fma(c, real(m[3]), a0); a1 = fma(c, real(m[4]), a1); a2 = fma(c, real(m[5]), a2);
+        }
+        u0 += a0; u1 += a1; u2 += a2;
+    }
+    if constexpr (CELLS) {
+        real g[Q];
+        equilibrium(g, real(0), u0, u1, u2);
+        store_cell_both(A, B, fu, P, p, x, y, z, fl, 0u, g);
+    }
+    fu[s] = u0; fu[P.F + s] = u1; fu[2 * P.F + s] = u2;
+    fu[3 * P.F + s] = u0; fu[4 * P.F + s] = u1; fu[5 * P.F + s] = u2;
+}
+
 // Re-publish the velocities the outflow cells will read next step from the CURRENT state (both halves of the side
 // array).  Needed when something that enters the local macro inversion changes between steps (lbm_set_damping): the
 // rule is u_loc(G_k, c - n) evaluated with the parameters in force when the step runs (DESIGN.md §3 step 6).

@@ -586,3 +586,125 @@ def test_set_damping_argument_errors(B):
     sim.set_damping((0,) * 6, (0.5,) * 6, None)   # off: target not needed
     sim.step(2)
     sim.close()
+
+
+# ---------------------------------------------------------------------------------------------- synthetic inflow fluctuations
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_inflow_fluctuations_match_the_oracle(B, fp64):
+    """PAPER.md:160 / Table 1: synthetic von Karman fluctuations on active inflow cells.  The paper's open-face
+    set-up (veering mean on three EQ_FIXED faces + outflow: x- and y- see inflow, y+ outflow), buildings, LES, 64 modes
+    carried with the reference wind; switched on at step 0 and again from a developed state (t = 37), 100 steps;
+    FP32 within 1e-5, FP64 within rounding order; then switched off: the mean returns."""
+    from oracle import Oracle
+    from paper_2607_04516_b200 import workloads as W
+    nx, ny, nz = 50, 42, 24
+    rng = np.random.default_rng(17)
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    for _ in range(5):
+        x0, y0 = int(rng.integers(10, nx - 14)), int(rng.integers(8, ny - 12))
+        hm[y0:y0 + 4, x0:x0 + 5] = int(rng.integers(1, nz - 8))
+    prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+    modes = W.inflow_modes(64, 23, 2 * np.pi / 40, np.pi, convect=(0.05, 0.01, 0.0))
+    u_rms, k_e, k_eta = 0.004, 2 * np.pi / 15, 2.5
+    args = (nx, ny, nz, 2e-3, 0.1, 1e-4, (0.0, 0.0, 0.0), (3, 4, 3, 3, 1, 2))
+    ux0 = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+    uy0 = 0.2 * ux0
+
+    def setup(obj, f64kw):
+        obj.set_flags(hm)
+        obj.set_inlet_profile(prof, 0.2 * prof, None, **f64kw)
+        obj.set_macros(None, ux0, uy0, None, **f64kw)
+
+    o = Oracle(*args)
+    setup(o, {})
+    sim = B.Lbm(*args, fp64=fp64)
+    setup(sim, {"f64": True})
+    tol = TOL64 if fp64 else TOL32
+    o.set_inflow_turbulence(modes, u_rms, k_e, k_eta)
+    sim.set_inflow_turbulence(modes, u_rms, k_e, k_eta)
+    assert max_err(sim, o, f64=fp64) <= tol            # the inflow cells at t = 0
+    ref = Oracle(*args)
+    setup(ref, {})
+    for upto in (37, 100):
+        o.step(upto - o.get_step())
+        sim.step(upto - sim.get_step())
+        e = max_err(sim, o, f64=fp64)
+        assert e <= tol, (upto, fp64, e)
+    ref.step(100)
+    assert max(np.abs(a - b).max() for a, b in zip(o.get_macros(), ref.get_macros())) > 2e-3   # the fluctuations matter
+    # mean-changing calls are refused while the fluctuations ride on it
+    with pytest.raises(B.LbmError):
+        sim.set_inlet_profile(prof, None, None, f64=True)
+    with pytest.raises(B.LbmError):
+        sim.balance_flux()
+    # a different table from a developed state
+    modes2 = W.inflow_modes(17, 5, 0.2, 2.0, convect=(0.04, 0.0, 0.0))
+    o.set_inflow_turbulence(modes2, 0.002, 0.3)
+    sim.set_inflow_turbulence(modes2, 0.002, 0.3)
+    o.step(30)
+    sim.step(30)
+    assert max_err(sim, o, f64=fp64) <= tol
+    # off: the boundary returns to the mean, and the plain path continues
+    o.set_inflow_turbulence(None)
+    sim.set_inflow_turbulence(None)
+    fl = o.get_flags()
+    g = [a.cpu().numpy().astype(np.float64) for a in sim.get_macros(f64=fp64)]
+    assert np.abs(g[1][fl == 2] - ux0[fl == 2]).max() < 1e-7 and np.abs(g[2][fl == 2] - uy0[fl == 2]).max() < 1e-7
+    o.step(20)
+    sim.step(20)
+    assert max_err(sim, o, f64=fp64) <= tol
+    sim.set_inlet_profile(prof, 0.2 * prof, None, f64=True)    # allowed again
+    sim.close()
+
+
+def test_inflow_fluctuation_phase_stays_exact_at_large_step_numbers(B):
+    """t ~ 1e5 steps: the FP64 phase reduction keeps the FP32 path on the oracle (an FP32 phase would be off by ~1e-3 rad)."""
+    from oracle import Oracle
+    from paper_2607_04516_b200 import workloads as W
+    nx, ny, nz = 12, 40, 16
+    args = (nx, ny, nz, 1e-2, 0.0, 0.0, (0, 0, 0), (3, 4, 0, 0, 1, 2))
+    prof = np.full(nz, 0.05)
+    modes = W.inflow_modes(32, 2, 0.2, 3.0, convect=(0.05, 0.02, 0.0))
+    o = Oracle(*args)
+    sim = B.Lbm(*args)
+    for obj, kw in ((o, {}), (sim, {"f64": True})):
+        obj.set_flags(None)
+        obj.set_inlet_profile(prof, None, None, **kw)
+        obj.set_macros(None, np.full((nz, ny, nx), 0.05), None, None, **kw)
+    o.set_step(123456)
+    sim.set_step(123456)
+    o.set_inflow_turbulence(modes, 0.005, 0.5)
+    sim.set_inflow_turbulence(modes, 0.005, 0.5)
+    o.step(5)
+    sim.step(5)
+    g = [a.cpu().numpy().astype(np.float64) for a in sim.get_macros()]
+    r = o.get_macros()
+    for a, b in zip(g, r):
+        assert np.abs(a[:, :, 0] - b[:, :, 0]).max() < 2e-7      # the inflow cells themselves
+    assert max_err(sim, o) <= TOL32
+    sim.close()
+
+
+def test_set_inflow_turbulence_argument_errors(B):
+    sim = B.Lbm(8, 8, 8, 1e-2, 0.1, 0.0, (0, 0, 0), (3, 4, 0, 0, 1, 2))
+    m = np.zeros((2, 9)); m[:, 0] = 0.5; m[:, 4] = 1.0; m[:, 8] = 0.1
+    with pytest.raises(B.LbmError):
+        sim.set_inflow_turbulence(m, 0.01, 0.5)            # flags not set
+    sim.set_flags(None)
+    sim.set_inlet_profile(np.full(8, 0.05))
+    with pytest.raises(B.LbmError):
+        sim.set_inflow_turbulence(m, 0.01, 0.0)            # k_e must be > 0
+    with pytest.raises(B.LbmError):
+        sim.set_inflow_turbulence(m, -1.0, 0.5)
+    bad = m.copy(); bad[0, 8] = -0.1
+    with pytest.raises(B.LbmError):
+        sim.set_inflow_turbulence(bad, 0.01, 0.5)
+    with pytest.raises(B.LbmError):
+        sim.set_inflow_turbulence(np.zeros((2000, 9)), 0.01, 0.5)
+    sim.set_inflow_turbulence(None)                        # off while off: no-op
+    sim.set_inflow_turbulence(m, 0.01, 0.5)
+    sim.step(3)
+    sim.set_flags(None)                                    # re-voxelising switches the fluctuations off
+    sim.set_inlet_profile(np.full(8, 0.05))
+    sim.close()
