@@ -319,6 +319,8 @@ int set_inlet_plane_any(lbm_t *h, int face, const in_t *uvw)
 
 template <typename real>
 int do_fluct(lbm_t *h, double t, bool cells);
+template <typename real>
+int turb_publish(lbm_t *h, bool cells);
 
 template <typename real, typename in_t>
 int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, const in_t *uz)
@@ -339,23 +341,27 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     }
     release_in(h, in, 4);
     if (!rc) { h->step = 0; h->cur = 0; }
-    if (!rc && h->nmodes > 0) rc = do_fluct<real>(h, 0.0, true); // the step counter restarts: the inflow cells carry u'(x, 0)
+    if (!rc && h->nmodes > 0) rc = turb_publish<real>(h, true); // the step counter restarts: the inflow cells carry u'(x, 0)
     return rc;
 }
 
-template <typename real, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false>
+template <typename real, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false, bool TURB = false>
 int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
     const real *A = (const real *)h->state();
     real *B = (real *)h->other();
     real *ms = (real *)h->mean();
-    const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
+    dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
+    // TURB: leading block rows that carry the face slots; they publish the boundary velocity of step (this one) + 1
+    const int turb_planes = TURB ? (int)((blocks_for(P.F, BLOCK) + grid.x - 1) / grid.x) : 0;
+    grid.y += turb_planes;
+    const Turb<real> tb{(const real *)h->fum(), h->modes(), h->nmodes, (double)(h->step + 2)};
     const StepPtrs<real> T = make_step_ptrs<real>(A, B, P);
     // the side buffer's halves follow the population buffers: read the half written together with A, write B's
     const real *fur = (const real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
     real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
-    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB, EXP, DAMP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
-    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP, DAMP><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T);
+    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB, EXP, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
+    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
     return check_launch(h, "step_kernel");
 }
 
@@ -367,9 +373,17 @@ constexpr int N_VARIANTS = 11;
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
-    if (h->damp_on) { // damping zones: the DAMP instantiation (same arithmetic outside the zones)
-        if constexpr (std::is_same<real, float>::value) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true>(h, P, sample);
-        else return launch_step_as<real, 0, false, 256, 2, 0, true>(h, P, sample);
+    const bool turb = h->nmodes > 0 && P.F > 0;
+    if (h->damp_on || turb) { // damping zones / inflow fluctuations: their own instantiations (same arithmetic elsewhere)
+        if constexpr (std::is_same<real, float>::value) {
+            if (h->damp_on && turb) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true, true>(h, P, sample);
+            if (h->damp_on) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true, false>(h, P, sample);
+            return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, false, true>(h, P, sample);
+        } else {
+            if (h->damp_on && turb) return launch_step_as<real, 0, false, 256, 2, 0, true, true>(h, P, sample);
+            if (h->damp_on) return launch_step_as<real, 0, false, 256, 2, 0, true, false>(h, P, sample);
+            return launch_step_as<real, 0, false, 256, 2, 0, false, true>(h, P, sample);
+        }
     }
     if constexpr (std::is_same<real, float>::value) {
         switch (h->variant) {
@@ -398,9 +412,20 @@ int do_fluct(lbm_t *h, double t, bool cells)
     const Params<real> P = make_params<real>(h);
     if (P.F == 0) return LBM_OK;
     const int B = 128;
-    if (cells) fluct_kernel<real, true><<<blocks_for(P.F, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), (const real *)h->fum(), h->flags(), h->modes(), h->nmodes, t, P);
-    else fluct_kernel<real, false><<<blocks_for(P.F, B), B, 0, h->stream>>>(nullptr, nullptr, (real *)h->fu(), (const real *)h->fum(), h->flags(), h->modes(), h->nmodes, t, P);
+    const Turb<real> tb{(const real *)h->fum(), h->modes(), h->nmodes, t};
+    if (cells) fluct_kernel<real, true><<<blocks_for(P.F, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), tb, P);
+    else fluct_kernel<real, false><<<blocks_for(P.F, B), B, 0, h->stream>>>(nullptr, nullptr, (real *)h->fu(), h->flags(), tb, P);
     return check_launch(h, "fluct_kernel");
+}
+
+// Fluctuations on: the EQ_FIXED cells hold u_b(step) and both halves of the side array u_b(step + 1), which the next
+// launch re-expands; from then on every launch publishes the velocity of the step after its own (TURB blocks).
+template <typename real>
+int turb_publish(lbm_t *h, bool cells)
+{
+    int rc = cells ? do_fluct<real>(h, (double)h->step, true) : LBM_OK;
+    if (!rc) rc = do_fluct<real>(h, (double)(h->step + 1), false);
+    return rc;
 }
 
 template <typename real>
@@ -410,11 +435,7 @@ int do_step(lbm_t *h, int n)
     for (int it = 0; it < n; ++it) {
         const long k = h->step + 1;
         const bool sample = h->mevery > 0 && k >= h->mstart && (k - h->mstart) % h->mevery == 0;
-        int rc = LBM_OK;
-        // the EQ_FIXED cells write G_{k+1} = f_eq(1, u_b(k+1)) in this launch: publish u_b(k+1) first
-        if (h->nmodes > 0) rc = do_fluct<real>(h, (double)k, false);
-        if (rc) return rc;
-        rc = launch_step<real>(h, P, sample);
+        int rc = launch_step<real>(h, P, sample);
         if (rc) return rc;
         h->cur ^= 1;
         h->step = k;
@@ -709,11 +730,11 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
     if (!h) return LBM_EINVAL;
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inflow_turbulence: flags not set");
     if (n_modes < 0 || n_modes > MAX_MODES) return fail(h, LBM_EINVAL, "set_inflow_turbulence: n_modes out of range");
-    auto rewrite = [&](double t) { return h->fp64 ? do_fluct<double>(h, t, true) : do_fluct<float>(h, t, true); };
+    auto rewrite = [&]() { return h->fp64 ? turb_publish<double>(h, true) : turb_publish<float>(h, true); };
     if (n_modes == 0) {
         if (h->nmodes == 0) return LBM_OK;
         h->nmodes = 0;
-        int rc = rewrite((double)h->step); // no modes: the cells return to the mean
+        int rc = rewrite(); // no modes: the cells and the side array return to the mean
         if (!rc) CUDA_TRY(h, cudaStreamSynchronize(h->stream));
         return rc;
     }
@@ -741,7 +762,7 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
         CUDA_TRY(h, cudaMemcpyAsync(h->fum(), h->fu(), L.fu_bytes / 2, cudaMemcpyDeviceToDevice, h->stream));
     CUDA_TRY(h, cudaMemcpyAsync(h->modes(), t.data(), t.size() * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     h->nmodes = n_modes;
-    int rc = rewrite((double)h->step);
+    int rc = rewrite();
     CUDA_TRY(h, cudaStreamSynchronize(h->stream)); // t (host staging) must outlive the copy
     return rc;
 }
@@ -873,11 +894,20 @@ int lbm_set_state(lbm_t *h, const double *f)
     if (!h) return LBM_EINVAL;
     if (!f) return fail(h, LBM_EINVAL, "set_state: NULL");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_state: flags not set");
-    return h->fp64 ? do_set_state<double>(h, f) : do_set_state<float>(h, f);
+    int rc = h->fp64 ? do_set_state<double>(h, f) : do_set_state<float>(h, f);
+    // the state brought its own boundary cells; the next launch must still find u_b(step + 1) in the side array
+    if (!rc && h->nmodes > 0) rc = h->fp64 ? turb_publish<double>(h, false) : turb_publish<float>(h, false);
+    return rc;
 }
 
 long lbm_get_step(const lbm_t *h) { return h ? h->step : -1; }
-int lbm_set_step(lbm_t *h, long step) { if (!h || step < 0) return LBM_EINVAL; h->step = step; return LBM_OK; }
+int lbm_set_step(lbm_t *h, long step)
+{
+    if (!h || step < 0) return LBM_EINVAL;
+    h->step = step;
+    if (h->nmodes > 0 && h->have_flags) return h->fp64 ? turb_publish<double>(h, false) : turb_publish<float>(h, false);
+    return LBM_OK;
+}
 
 int lbm_sync(lbm_t *h)
 {

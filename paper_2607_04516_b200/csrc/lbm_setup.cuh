@@ -130,6 +130,16 @@ __device__ __forceinline__ void store_cell_both(real *__restrict__ A, real *__re
     }
 }
 
+// the boundary velocity of an EQ_FIXED cell exactly as prescribed (store_cell_both publishes the moments of the
+// equilibrium, which carry rounding noise: a prescribed 0 could become -1e-19 and flip the active-inflow test)
+template <typename real>
+__device__ __forceinline__ void publish_fixed(real *__restrict__ fu, const Params<real> &P, int x, int y, int z, real ux, real uy, real uz)
+{
+    const int s = eq_slot(P, EQ_FIXED, x, y, z);
+    fu[s] = ux; fu[P.F + s] = uy; fu[2 * P.F + s] = uz;
+    fu[3 * P.F + s] = ux; fu[4 * P.F + s] = uy; fu[5 * P.F + s] = uz;
+}
+
 // ---- a3: inlet write -------------------------------------------------------------------------------------------------
 // mode 0: profile prof[nz] per component by level; mode 1: plane uvw[3][n2][n1] of one face
 template <typename real, typename in_t>
@@ -164,6 +174,7 @@ __global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, real *_
     real g[Q];
     equilibrium(g, real(0), ux, uy, uz);
     store_cell_both(A, B, fu, P, p, x, y, z, fl, 0u, g);
+    publish_fixed(fu, P, x, y, z, ux, uy, uz);
 }
 
 // ---- synthetic inflow fluctuations (lbm_set_inflow_turbulence; Table 1) -------------------
@@ -173,22 +184,22 @@ __global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, real *_
 // x = cell indices (DESIGN.md §4 reading 21); all other EQ_FIXED cells keep the mean.  modes = [n][8] doubles:
 // kappa[3], a[3], psi, omega (amplitudes folded on the host).  The phase is formed and reduced to [-pi, pi] in FP64 (t
 // reaches 1e4-1e5 steps, an FP32 phase would lose 1e-3 rad), the cosine is taken in the handle's precision.
-// The value goes to both halves of the side array: the step kernel re-expands f_eq(1, u_b) from it (a3).  CELLS = true
-// (set-up, switch-off, restart): the cell's populations are rewritten in both buffers as well.
+// The value goes to the side array: the step kernel re-expands f_eq(1, u_b) from it (a3).
+template <typename real>
+struct Turb { const real *fum; const double *modes; int n; double t; };
+
+// one slot: boundary velocity of time t -> dst0 / dst1 (the halves to publish to; dst1 may be null)
 template <typename real, bool CELLS>
-__global__ void fluct_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const real *__restrict__ fum,
-                             const uint8_t *__restrict__ flags, const double *__restrict__ modes, int nmodes, double t, Params<real> P)
+__device__ __forceinline__ void fluct_slot(int s, real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, real *__restrict__ dst0,
+                                           real *__restrict__ dst1, const uint8_t *__restrict__ flags, const Turb<real> &tb, const Params<real> &P)
 {
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    if (s >= P.F) return;
     int k = 5;
     while (k > 0 && s < P.foff[k]) --k; // the last face whose first slot is <= s (faces without slots share their successor's offset)
     if (P.face[k] != FACE_EQ_FIXED) return;
     const int axis = k >> 1;
     const int n1 = axis == 0 ? P.ny : P.nx;
     const int r = s - P.foff[k], j1 = r % n1, j2 = r / n1;
-    const int nn[3] = {P.nx, P.ny, P.nz};
-    const int fixed = (k & 1) ? nn[axis] - 1 : 0;
+    const int fixed = (k & 1) ? (axis == 0 ? P.nx : (axis == 1 ? P.ny : P.nz)) - 1 : 0;
     int x, y, z;
     if (axis == 0) { x = fixed; y = j1; z = j2; }
     else if (axis == 1) { x = j1; y = fixed; z = j2; }
@@ -197,14 +208,15 @@ __global__ void fluct_kernel(real *__restrict__ A, real *__restrict__ B, real *_
     const int p = pidx(P, x, y, z);
     const uint8_t fl = flags[p];
     if ((fl & CLASS_MASK) != EQ_FIXED) return;
-    const real mu[3] = {fum[s], fum[P.F + s], fum[2 * P.F + s]};
-    real u0 = mu[0], u1 = mu[1], u2 = mu[2];
-    const real un = (k & 1) ? mu[axis] : -mu[axis];
+    real u0 = tb.fum[s], u1 = tb.fum[P.F + s], u2 = tb.fum[2 * P.F + s];
+    const real ua = axis == 0 ? u0 : (axis == 1 ? u1 : u2);
+    const real un = (k & 1) ? ua : -ua;
     if (un < real(0)) {
         real a0 = real(0), a1 = real(0), a2 = real(0);
-        for (int n = 0; n < nmodes; ++n) {
-            const double *m = modes + 8 * n;
-            double ph = fma(m[0], (double)x, fma(m[1], (double)y, fma(m[2], (double)z, fma(-m[7], t, m[6]))));
+        const double xd = (double)x, yd = (double)y, zd = (double)z;
+        for (int n = 0; n < tb.n; ++n) {
+            const double *m = tb.modes + 8 * n;
+            double ph = fma(m[0], xd, fma(m[1], yd, fma(m[2], zd, fma(-m[7], tb.t, m[6]))));
             real c;
             if constexpr (sizeof(real) == 8) c = cos(ph);
             else {
@@ -220,8 +232,19 @@ __global__ void fluct_kernel(real *__restrict__ A, real *__restrict__ B, real *_
         equilibrium(g, real(0), u0, u1, u2);
         store_cell_both(A, B, fu, P, p, x, y, z, fl, 0u, g);
     }
-    fu[s] = u0; fu[P.F + s] = u1; fu[2 * P.F + s] = u2;
-    fu[3 * P.F + s] = u0; fu[4 * P.F + s] = u1; fu[5 * P.F + s] = u2;
+    dst0[s] = u0; dst0[P.F + s] = u1; dst0[2 * P.F + s] = u2;
+    if (dst1) { dst1[s] = u0; dst1[P.F + s] = u1; dst1[2 * P.F + s] = u2; }
+}
+
+// stand-alone form (set-up, switch-off, re-initialisation): both halves; CELLS = also the cells' populations in both buffers.
+// During a run the step kernel itself carries the slots (lbm_step.cuh, TURB blocks): no extra launch.
+template <typename real, bool CELLS>
+__global__ void fluct_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+                             const Turb<real> tb, Params<real> P)
+{
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= P.F) return;
+    fluct_slot<real, CELLS>(s, A, B, fu, fu, fu + 3 * (size_t)P.F, flags, tb, P);
 }
 
 // Re-publish the velocities the outflow cells will read next step from the CURRENT state (both halves of the side
@@ -264,6 +287,7 @@ __global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, real *
     const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, S, damp_at(S, sx, y % S.ny, z));
     equilibrium(g, real(0), m.ux, m.uy, m.uz);
     store_cell_both(dA, dB, dfu, D, dp, 0, y, z, fl, 0u, g);
+    publish_fixed(dfu, D, 0, y, z, m.ux, m.uy, m.uz);
 }
 
 // ---- a4: init ------------------------------------------------------------------------------------------------------------

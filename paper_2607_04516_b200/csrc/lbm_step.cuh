@@ -10,10 +10,12 @@
 // HINT: 0 = default loads / stores, 1 = ld.global.cs / st.global.cs (streaming), 2 = default ld / st.cs, 3 = ld.cs / default st.
 // SPEC: issue the 19 population loads before the flag byte has arrived (no dependent round trip; SOLID cells then
 //       cost their 76 B of reads).
+// TURB: the launch carries the synthetic inflow fluctuations in extra leading block rows (lbm_set_inflow_turbulence).
 // DAMP: the damping-zone instantiation (lbm_set_damping); launched only while zones are configured, so the plain
 //       kernel carries none of it.
 #pragma once
 #include "lbm_core.cuh"
+#include "lbm_setup.cuh"
 
 namespace lbmk {
 
@@ -69,16 +71,29 @@ inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> 
     return t;
 }
 
-template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false>
+template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false, bool TURB = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-            real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T)
+            real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T,
+            const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
 {
+    int zb = blockIdx.y;
+    if constexpr (TURB) {
+        // the first turb_planes block rows carry the inflow fluctuations instead of lattice cells: one thread per face slot,
+        // boundary velocity of the step AFTER this one (tb.t) into the half this launch writes — the EQ_FIXED cells of the
+        // next launch read it from there.  They are dispatched first and run beside the memory-bound lattice blocks.
+        if (zb < turb_planes) {
+            const int s = (zb * (int)gridDim.x + (int)blockIdx.x) * BLOCK + (int)threadIdx.x;
+            if (s < P.F) fluct_slot<real, false>(s, nullptr, nullptr, nullptr, fuw, nullptr, flags, tb, P);
+            return;
+        }
+        zb -= turb_planes;
+    }
     const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x; // cell of the z plane, linear over interior (y, x)
     if (c2 >= (unsigned)P.nxy) return;
     const int y = P.nx_magic ? (int)__umulhi(c2, P.nx_magic) : (int)(c2 / (unsigned)P.nx);
     const int x = (int)c2 - y * P.nx;
-    const int z = blockIdx.y;
+    const int z = zb;
     const int p = pidx(P, x, y, z);
 
     real g[Q];

@@ -708,3 +708,42 @@ def test_set_inflow_turbulence_argument_errors(B):
     sim.set_flags(None)                                    # re-voxelising switches the fluctuations off
     sim.set_inlet_profile(np.full(8, 0.05))
     sim.close()
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_open_boundary_stack_together_matches_the_oracle(B, fp64):
+    """Everything PAPER.md:175 / Table 1 PAPER.md:86 lists for the open faces at once: equilibrium velocity faces, global
+    flux correction, sponge + buffer nudging, synthetic fluctuations on the active inflow cells (the DAMP + TURB
+    instantiation of the step kernel), with the time mean accumulating."""
+    from oracle import Oracle
+    from paper_2607_04516_b200 import workloads as W
+    nx, ny, nz = 44, 38, 20
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    hm[14:20, 16:22] = 9
+    hm[24:27, 28:33] = 5
+    prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+    args = (nx, ny, nz, 2e-3, 0.1, 2e-4, (0.0, 0.0, 0.0), (3, 3, 3, 3, 1, 3))   # four lateral faces + top: all open
+    target = np.stack([prof, 0.3 * prof, np.zeros(nz)])
+    modes = W.inflow_modes(48, 41, 2 * np.pi / 30, np.pi, convect=(0.05, 0.015, 0.0))
+    ux0 = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+    o = Oracle(*args)
+    sim = B.Lbm(*args, fp64=fp64)
+    for obj, kw in ((o, {}), (sim, {"f64": True})):
+        obj.set_flags(hm)
+        obj.set_inlet_profile(prof, 0.3 * prof, None, **kw)
+        obj.set_macros(None, ux0, 0.3 * ux0, None, **kw)
+        b, a = obj.balance_flux()
+        assert abs(a) < (1e-9 if (obj is o or fp64) else 2e-4)
+        obj.set_damping((5, 8, 5, 5, 0, 6), (0.05, 0.15, 0.05, 0.05, 0.0, 0.2), target)
+        obj.set_inflow_turbulence(modes, 0.003, 2 * np.pi / 12, 2.5)
+        obj.mean_config(20, 5)
+    o.step(100)
+    sim.step(100)
+    tol = TOL64 if fp64 else TOL32
+    e = max_err(sim, o, f64=fp64)
+    assert e <= tol, (fp64, e)
+    gm, om = sim.get_mean(f64=fp64), o.get_mean()
+    assert gm[3] == om[3] == 17
+    em = max(float(np.abs(a.cpu().numpy().astype(np.float64) - b).max()) for a, b in zip(gm[:3], om[:3]))
+    assert em <= tol, (fp64, em)
+    sim.close()
