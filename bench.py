@@ -1,7 +1,7 @@
 #!/usr/bin/env python
 """bench.py — MLUPS of the fused D3Q19 stream-collide path on the 400x400x100 urban config (BASELINE.json).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-cpu-baseline]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-cpu-baseline] [--workload c1..c5]
 
 One bench "step" = one LBM time step of the whole lattice = one launch of the fused stream-collide kernel
 (pull + bounce-back/free-slip/periodic resolution + moments + Coriolis/F + Smagorinsky + BGK/Guo + store, outflow
@@ -26,6 +26,66 @@ sys.path.insert(0, ROOT)
 
 BYTES_PER_CELL = 153  # 19x4 B loads + 19x4 B stores + 1 flag byte (BASELINE.json north_star)
 METRIC = "MLUPS (D3Q19 FP32), fused stream-collide, 400x400x100 urban config, 1 B200"
+
+# --workload: the headline is c3 (BASELINE.json: the config the metric is quoted on); the others are the parity configs,
+# timed here only for the per-config table of DESIGN.md §12 (SURVEY.md §8(d) "report per config")
+WORKLOADS = {
+    "c1": "C1 tiny block flow 64x32x32 (BASELINE.json configs[0])",
+    "c2": "C2 periodic Taylor-Green + Coriolis 128^3, Cs 0.1 (BASELINE.json configs[1])",
+    "c3": "C3 urban 400x400x100 (BASELINE.json configs[2]): seeded heightmap plan fraction 0.35, log-law inlet, nu0 1e-4, Cs 0.1, f 2.9e-6",
+    "c4": "C4 refined urban 800x800x200, veering inlet on three faces (BASELINE.json configs[3])",
+    "c5": "C5 chain: periodic precursor 256x256x200 feeding the x- inlet of the 1200x1200x200 urban domain every step (BASELINE.json configs[4])",
+}
+
+
+class Job:
+    """One workload resident on the device: a single lattice, or the config-5 chain (precursor -> feed -> main)."""
+
+    def __init__(self, name, binding, W, device):
+        self.name, self.binding, self.device = name, binding, device
+        if name == "c5":
+            self.wls = [W.config5_precursor(), W.config5_main()]
+        else:
+            self.wls = [{"c1": W.config1, "c2": lambda: W.config2(Cs=0.1), "c3": W.config3, "c4": W.config4}[name]()]
+        self.cells = sum(w.cells for w in self.wls)
+        self.sims = [binding.from_workload(w, want_mean=False, device=device) for w in self.wls]
+
+    def step(self, n):
+        if len(self.sims) == 1:
+            self.sims[0].step(n)
+            return
+        pre, main = self.sims
+        xs = self.wls[0].extra["sample_plane_x"]
+        for _ in range(n):
+            main.feed_inlet(pre, xs)
+            pre.step(1)
+            main.step(1)
+
+    def launch_count(self):
+        return sum(s.launch_count() for s in self.sims)
+
+    def host_inputs(self, pin):
+        """pinned host copies of everything the set-up of each lattice reads"""
+        out = []
+        for w in self.wls:
+            prof = None if w.inlet_profile is None else tuple(None if a is None else pin(a) for a in w.inlet_profile)
+            init = None if w.init is None else tuple(None if a is None else pin(a) for a in w.init)
+            out.append((pin(w.height), prof, init))
+        return out
+
+    @staticmethod
+    def nbytes(host):
+        n = 0
+        for h, prof, init in host:
+            n += h.nbytes + sum(a.nbytes for a in (prof or ()) if a is not None) + sum(a.nbytes for a in (init or ()) if a is not None)
+        return n
+
+    def setup_from_host(self, host):
+        for s, (h, prof, init) in zip(self.sims, host):
+            s.set_flags(h)
+            if prof is not None:
+                s.set_inlet_profile(*prof)
+            s.set_macros(*(init if init is not None else (None, None, None, None)))
 
 
 def load_peak():
@@ -188,7 +248,6 @@ def run_ours(args):
 
     from paper_2607_04516_b200 import binding, build, workloads as W
     build.build()
-    wl = W.config3()
     K, Wm = args.steps, max(args.warmup, 3)
 
     def barrier():
@@ -197,44 +256,45 @@ def run_ours(args):
         torch.cuda.synchronize()
 
     # ---------------- device-resident timing: K launches of the fused kernel
-    sim = binding.from_workload(wl, want_mean=False, device=f"cuda:{local}")
+    job_ = Job(args.workload, binding, W, f"cuda:{local}")
+    sim, wl = job_.sims[-1], job_.wls[-1]   # the (main) lattice whose macros are read back
+    cells = job_.cells
     if args.variant:
-        sim.set_variant(args.variant)
-    sim.step(Wm)
+        for s_ in job_.sims:
+            s_.set_variant(args.variant)
+    job_.step(Wm)
     barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
-    l0 = sim.launch_count()
+    l0 = job_.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     reps = max(1, args.repeats)
     best = None
     for _ in range(reps):
         barrier()
         e0.record()
-        sim.step(K)
+        job_.step(K)
         e1.record()
         barrier()
         ms = e0.elapsed_time(e1)
         best = ms if best is None else min(best, ms)
-    launches = (sim.launch_count() - l0) // reps
+    launches = (job_.launch_count() - l0) // reps
     clocks = sampler.stop() if rank == 0 else None
     rho, ux, uy, uz = sim.get_macros()
     finite = bool(torch.isfinite(ux).all().item())
     ms_total = max_over_ranks(best, world, dev)
-    mlups = job_mlups(wl.cells, K, world, ms_total * 1e-3)
+    mlups = job_mlups(cells, K, world, ms_total * 1e-3)
 
     # ---------------- end to end through the C ABI with pinned host buffers
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()  # noqa: E731
-    h_height, h_u, h_ux0 = pin(wl.height), pin(wl.inlet_profile[0]), pin(wl.init[1])
+    host = job_.host_inputs(pin)
     outs = [torch.empty(wl.shape, dtype=torch.float32).pin_memory() for _ in range(4)]
     lib = binding.load_library()
 
     def job(s):
-        s.set_flags(h_height)
-        s.set_inlet_profile(h_u)
-        s.set_macros(None, h_ux0, None, None)
-        s.step(K)
+        job_.setup_from_host(host)
+        job_.step(K)
         rc = lib.lbm_get_macros(s._h, *[o.data_ptr() for o in outs])
         assert rc == 0
     job(sim)  # warm-up of the copy paths
@@ -246,9 +306,9 @@ def run_ours(args):
     barrier()
     wall = time.perf_counter() - t0
     e2e_s = max_over_ranks(max(e0.elapsed_time(e1) * 1e-3, wall), world, dev)
-    h2d = h_height.nbytes + h_u.nbytes + h_ux0.nbytes
+    h2d = Job.nbytes(host)
     d2h = sum(o.numel() * 4 for o in outs)
-    e2e = {"value": job_mlups(wl.cells, K, world, e2e_s), "unit": "MLUPS", "h2d_bytes_per_step": h2d / K,
+    e2e = {"value": job_mlups(cells, K, world, e2e_s), "unit": "MLUPS", "h2d_bytes_per_step": h2d / K,
            "d2h_bytes_per_step": d2h / K,
            "what": f"one job = set_flags + set_inlet_profile + set_macros from pinned host buffers, lbm_step({K}), "
                    "lbm_get_macros into pinned host buffers"}
@@ -256,25 +316,27 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = load_peak()
         per_launch_s = ms_total * 1e-3 / K
-        achieved = BYTES_PER_CELL * wl.cells / per_launch_s / 1e9
+        achieved = BYTES_PER_CELL * cells / per_launch_s / 1e9
         line = {
             "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "C3 urban 400x400x100 (BASELINE.json configs[2]): seeded heightmap plan fraction 0.35, "
-                                   "log-law inlet, nu0 1e-4, Cs 0.1, f 2.9e-6",
-                       "cells": wl.cells, "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "l2": "no flush needed: each step streams 2.4 GB (>> 126 MB L2)", "best_of": reps,
+            "config": {"workload": WORKLOADS[args.workload],
+                       "cells": cells, "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": (f"no flush needed: each step streams {BYTES_PER_CELL * cells / 1e9:.1f} GB (>> 126 MB L2)"
+                              if BYTES_PER_CELL * cells > 4 * 126e6 else
+                              f"NOT flushed: the {2 * 76 * cells / 1e6:.0f} MB of this parity config stay L2-resident; not a bench line"),
+                       "best_of": reps,
                        "state_finite": finite},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": load_traffic(), "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": BYTES_PER_CELL * wl.cells,
+                         "traffic": load_traffic() if args.workload == "c3" else None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": BYTES_PER_CELL * cells,
                          "frac_of_nominal_8000": achieved / 8000.0},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
         }
-        if not args.no_cpu_baseline and world == 1:
+        if not args.no_cpu_baseline and world == 1 and args.workload == "c3":
             line["cpu_baseline"] = cpu_baseline()
-        elif world > 1:
+        else:
             line["cpu_baseline"] = None
         print(json.dumps(line))
     if world > 1:
@@ -290,6 +352,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--repeats", type=int, default=1, help="timed repetitions of the K-step region; best is reported")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--workload", default="c3", choices=sorted(WORKLOADS), help="c3 = the headline config; others: per-config table only")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--reference-budget", type=float, default=150.0, help="seconds of CPU time the reference arm may use")
     args = ap.parse_args()

@@ -390,7 +390,14 @@ int oracle_set_boundaries(oracle_t *o, const int *face_type)
 
 /* step 9: SOLID <=> z < clamp(h,0,nz); non-solid cells of an EQ face take the
  * EQ class, EQ_FIXED winning over EQ_OUTFLOW where two EQ faces meet. */
-int oracle_set_flags(oracle_t *o, const int32_t *height)
+static int set_flags_impl(oracle_t *o, const int32_t *height, const uint8_t *solid);
+int oracle_set_flags(oracle_t *o, const int32_t *height) { return set_flags_impl(o, height, NULL); }
+
+/* the same with a general solid mask merged in ("The final solid mask is assembled by the Boolean merging of
+ * a fixed-thickness base layer, the terrain layer, and the building layer"): SOLID <=> z < clamp(h) OR solid[z][y][x] != 0 */
+int oracle_set_flags_mask(oracle_t *o, const int32_t *height, const uint8_t *solid) { return set_flags_impl(o, height, solid); }
+
+static int set_flags_impl(oracle_t *o, const int32_t *height, const uint8_t *solid)
 {
     for (int z = 0; z < o->nz; ++z)
         for (int y = 0; y < o->ny; ++y)
@@ -398,6 +405,7 @@ int oracle_set_flags(oracle_t *o, const int32_t *height)
                 int h = height ? height[(long)y * o->nx + x] : 0;
                 if (h < 0) h = 0;
                 if (h > o->nz) h = o->nz;
+                if (solid && solid[cell_of(o, x, y, z)]) h = o->nz; /* merged in: this cell is solid whatever the column height */
                 int cl = C_FLUID;
                 if (z < h) cl = C_SOLID;
                 else {

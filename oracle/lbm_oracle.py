@@ -50,7 +50,7 @@ def _load():
                  "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell",
                  "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux",
                  "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping",
-                 "oracle_vk_spectrum", "oracle_set_inflow_turbulence"):
+                 "oracle_vk_spectrum", "oracle_set_inflow_turbulence", "oracle_set_flags_mask"):
         getattr(lib, name).restype = C.c_int
     _lib = lib
     return lib
@@ -210,6 +210,19 @@ class Oracle:
         a = np.ascontiguousarray(height, dtype=np.int32)
         assert a.shape == (self.ny, self.nx)
         self._chk(self._lib.oracle_set_flags(C.c_void_p(self._h), a.ctypes.data_as(C.c_void_p)), "set_flags")
+
+    def set_flags_mask(self, height=None, solid=None):
+        """Heightmap (or None) merged with a general solid mask uint8 [nz][ny][nx] (non-zero = SOLID)."""
+        if height is None:
+            height = np.zeros((self.ny, self.nx), dtype=np.int32)
+        a = np.ascontiguousarray(height, dtype=np.int32)
+        assert a.shape == (self.ny, self.nx)
+        m = None
+        if solid is not None:
+            m = np.ascontiguousarray(solid, dtype=np.uint8)
+            assert m.shape == self.shape
+        self._chk(self._lib.oracle_set_flags_mask(C.c_void_p(self._h), a.ctypes.data_as(C.c_void_p),
+                                                  m.ctypes.data_as(C.c_void_p) if m is not None else None), "set_flags_mask")
 
     def get_flags(self):
         out = np.zeros(self.shape, dtype=np.uint8)

@@ -218,3 +218,55 @@ def mean_profile(u: np.ndarray, flags: np.ndarray, solid_code: int = 1) -> np.nd
     fluid = flags != solid_code
     cnt = np.maximum(fluid.sum(axis=(1, 2)), 1)
     return (np.where(fluid, u, 0.0).sum(axis=(1, 2), dtype=np.float64)) / cnt
+
+
+# --------------------------------------------------------------------------- triangle meshes (inputs of the mesh voxeliser)
+
+def box_mesh(lo, hi) -> np.ndarray:
+    """12 outward-oriented triangles of the axis-aligned box [lo, hi]; float32 [12][3][3], lattice units."""
+    x0, y0, z0 = lo
+    x1, y1, z1 = hi
+    c = np.array([[x0, y0, z0], [x1, y0, z0], [x1, y1, z0], [x0, y1, z0],
+                  [x0, y0, z1], [x1, y0, z1], [x1, y1, z1], [x0, y1, z1]], dtype=np.float64)
+    quads = [(0, 3, 2, 1), (4, 5, 6, 7), (0, 1, 5, 4), (2, 3, 7, 6), (1, 2, 6, 5), (3, 0, 4, 7)]
+    tri = []
+    for a, b, d, e in quads:
+        tri.append([c[a], c[b], c[d]])
+        tri.append([c[a], c[d], c[e]])
+    return np.asarray(tri, dtype=np.float32)
+
+
+def icosphere_mesh(centre, radius: float, subdivisions: int = 2) -> np.ndarray:
+    """Closed triangle mesh inscribed in a sphere (icosahedron subdivided); float32 [20 * 4^s][3][3]."""
+    t = (1.0 + math.sqrt(5.0)) / 2.0
+    v = [(-1, t, 0), (1, t, 0), (-1, -t, 0), (1, -t, 0), (0, -1, t), (0, 1, t), (0, -1, -t), (0, 1, -t),
+         (t, 0, -1), (t, 0, 1), (-t, 0, -1), (-t, 0, 1)]
+    v = [np.asarray(p, dtype=np.float64) / math.sqrt(1 + t * t) for p in v]
+    f = [(0, 11, 5), (0, 5, 1), (0, 1, 7), (0, 7, 10), (0, 10, 11), (1, 5, 9), (5, 11, 4), (11, 10, 2), (10, 7, 6), (7, 1, 8),
+         (3, 9, 4), (3, 4, 2), (3, 2, 6), (3, 6, 8), (3, 8, 9), (4, 9, 5), (2, 4, 11), (6, 2, 10), (8, 6, 7), (9, 8, 1)]
+    tri = [[v[a], v[b], v[c]] for a, b, c in f]
+    for _ in range(subdivisions):
+        nxt = []
+        for a, b, c in tri:
+            ab, bc, ca = [(p + q) / np.linalg.norm(p + q) for p, q in ((a, b), (b, c), (c, a))]
+            nxt += [[a, ab, ca], [b, bc, ab], [c, ca, bc], [ab, bc, ca]]
+        tri = nxt
+    return (np.asarray(tri) * radius + np.asarray(centre, dtype=np.float64)).astype(np.float32)
+
+
+def urban_mesh(height: np.ndarray, z_shift: float = 0.0) -> np.ndarray:
+    """One closed box per maximal run of equal non-zero height along x in every row of a heightmap (buildings as
+    extruded footprints, the way a city model delivers them); float32 [n][3][3]."""
+    ny, nx = height.shape
+    out = []
+    for y in range(ny):
+        x = 0
+        while x < nx:
+            h = int(height[y, x])
+            x1 = x
+            while x1 < nx and int(height[y, x1]) == h:
+                x1 += 1
+            if h > 0:
+                out.append(box_mesh((x, y, -1.0 + z_shift), (x1, y + 1, h + z_shift)))
+            x = x1
+    return np.concatenate(out) if out else np.zeros((0, 3, 3), dtype=np.float32)
