@@ -89,6 +89,25 @@ int lbm_set_coriolis(lbm_t *h, const double f[3]);
  * Resets the populations to the rest state (rho = 1, u = 0) and the step counter and mean sums to 0. */
 int lbm_set_flags(lbm_t *h, const int32_t *height);
 
+/* a1 with a general solid mask merged in ("The final solid mask is assembled by the Boolean merging of a
+ * fixed-thickness base layer, the terrain layer, and the building layer"): SOLID <=> z < clamp(height[y][x], 0, nz) OR
+ * solid[z][y][x] != 0.  solid: uint8 [nz][ny][nx], host or device, borrowed for the call; NULL = lbm_set_flags.  Overhangs,
+ * bridges and hollow shapes are allowed: the link classification and the step kernel work from the flags alone. */
+int lbm_set_flags_mask(lbm_t *h, const int32_t *height, const uint8_t *solid);
+
+/* a1 in the paper's own form: voxelise a triangle mesh on the device ("casting axis-aligned rays through grid
+ * columns and computing ray-triangle intersections, using an odd-even parity rule along each column ... corroborate
+ * independent passes along different ray directions for solid labeling"), then merge it with the heightmap layer as above.
+ * tri: float [n_tri][3 vertices][x,y,z] in lattice units (cell (x,y,z) has its centre at (x+1/2, y+1/2, z+1/2); the ground
+ * face is z = 0), host or device, borrowed.  Reading (DESIGN.md §4 reading 22), exact integer arithmetic: vertices snapped
+ * to 1/256 cell (rint), must lie in [-1024, 2048) cells; pass d casts rays along axis d through the cell centres; a
+ * triangle is hit iff the ray's foot point lies inside its projection (taken counter-clockwise, top-left rule on edges,
+ * zero-area projections skipped); a crossing flips every cell whose centre is at or beyond it; SOLID iff at least
+ * min_votes (1..3; 2 = majority) of the three passes end odd.  Orientation of the triangles is irrelevant; the mesh
+ * should be closed (a hole corrupts only the rays through it, which the vote out-numbers).  n_tri = 0: heightmap only.
+ * LBM_EINVAL: min_votes out of range, NULL tri, a vertex not finite or out of range.  Synchronises. */
+int lbm_set_flags_mesh(lbm_t *h, const int32_t *height, int n_tri, const float *tri, int min_votes);
+
 /* Boundary wind profile ("macroscopic boundary states"): every EQ_FIXED cell at level z is set
  * to f_eq(1, (u[z], v[z], w[z])).  Each array [nz]; v, w may be NULL (= 0).  Needs flags. */
 int lbm_set_inlet_profile(lbm_t *h, const float *u, const float *v, const float *w);

@@ -27,7 +27,7 @@ SYMBOLS = [
     "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
     "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
-    "lbm_set_damping", "lbm_set_inflow_turbulence",
+    "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
 ]
 
 
@@ -59,6 +59,8 @@ def load_library():
     lib.lbm_set_damping.argtypes = [vp, vp, vp, vp]
     lib.lbm_set_inflow_turbulence.argtypes = [vp, i, vp, C.c_double, C.c_double, C.c_double]
     lib.lbm_set_flags.argtypes = [vp, vp]
+    lib.lbm_set_flags_mask.argtypes = [vp, vp, vp]
+    lib.lbm_set_flags_mesh.argtypes = [vp, vp, i, vp, i]
     for n in ("lbm_set_inlet_profile", "lbm_set_inlet_profile_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp]
     for n in ("lbm_set_inlet_plane", "lbm_set_inlet_plane_f64"):
@@ -219,6 +221,27 @@ class Lbm:
         if k is not None and tuple(k.shape) != (self.ny, self.nx):
             raise ValueError("height must be [ny][nx]")
         self._chk(self._lib.lbm_set_flags(self._h, p), "set_flags")
+
+    def set_flags_mask(self, height=None, solid=None):
+        """Heightmap (or None) merged with a general solid mask uint8 [nz][ny][nx] (host or device)."""
+        k, p = _ptr(height, np.int32)
+        if k is not None and tuple(k.shape) != (self.ny, self.nx):
+            raise ValueError("height must be [ny][nx]")
+        m, mp = _ptr(solid, np.uint8)
+        if m is not None and tuple(m.shape) != self.shape:
+            raise ValueError("solid must be [nz][ny][nx]")
+        self._chk(self._lib.lbm_set_flags_mask(self._h, p, mp), "set_flags_mask")
+
+    def set_flags_mesh(self, tri, height=None, min_votes=2):
+        """Voxelise a triangle mesh float32 [n][3][3] (lattice units, host or device) and merge it with the heightmap."""
+        k, p = _ptr(height, np.int32)
+        if k is not None and tuple(k.shape) != (self.ny, self.nx):
+            raise ValueError("height must be [ny][nx]")
+        t, tp = _ptr(tri, np.float32)
+        n = 0 if t is None else int(np.prod(tuple(t.shape))) // 9
+        if t is not None and int(np.prod(tuple(t.shape))) != 9 * n:
+            raise ValueError("tri must be [n][3][3]")
+        self._chk(self._lib.lbm_set_flags_mesh(self._h, p, n, tp, int(min_votes)), "set_flags_mesh")
 
     def set_inlet_profile(self, u, v=None, w=None, f64=False):
         dt = np.float64 if f64 else np.float32

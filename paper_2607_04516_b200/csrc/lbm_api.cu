@@ -4,6 +4,7 @@
 #include "lbm_setup.cuh"
 #include "lbm_step.cuh"
 #include "lbm_out.cuh"
+#include "lbm_mesh.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -236,14 +237,14 @@ int check_launch(lbm_t *h, const char *what)
 // ---- templated implementations -----------------------------------------------------------------------------------
 
 template <typename real>
-int do_set_flags(lbm_t *h, const int32_t *height)
+int do_set_flags(lbm_t *h, const int32_t *height, const uint8_t *dev_mask = nullptr, int thresh = 1)
 {
     const Params<real> P = make_params<real>(h);
     InBuf in;
     int rc = stage_in(h, height, (size_t)h->nx * h->ny * sizeof(int32_t), 0, &in);
     if (rc) return rc;
     const int B = 256;
-    voxelise_kernel<real><<<blocks_for(P.Np, B), B, 0, h->stream>>>((const int32_t *)in.dev, h->flags(), P);
+    voxelise_kernel<real><<<blocks_for(P.Np, B), B, 0, h->stream>>>((const int32_t *)in.dev, dev_mask, thresh, h->flags(), P);
     rc = check_launch(h, "voxelise_kernel");
     if (!rc) {
         rc = cudaMemsetAsync(h->links(), 0, (size_t)P.Np * sizeof(uint32_t), h->stream) == cudaSuccess ? LBM_OK
@@ -319,6 +320,48 @@ int set_inlet_plane_any(lbm_t *h, int face, const in_t *uvw)
 
 template <typename real>
 int do_fluct(lbm_t *h, double t, bool cells);
+
+// Mesh voxeliser (lbm_mesh.cuh): vote counts of the three ray passes, in the first N bytes of the link-word area (free
+// until classify_kernel rewrites it); the toggles of the running pass sit in the bytes behind them.
+int mesh_votes(lbm_t *h, int n_tri, const float *dev_tri, uint8_t **votes_out)
+{
+    const long long N = h->N();
+    uint8_t *votes = (uint8_t *)h->links();
+    const size_t tog_off = align_up((size_t)N, ALIGN), tog_bytes = align_up((size_t)N, 4) + 4;
+    uint8_t *toggles = votes + tog_off;
+    int *err = (int *)(toggles + align_up(tog_bytes, ALIGN));
+    // 4 Np bytes are there: N votes + N toggles + a flag word fit for every box (Np >= N + halo)
+    if (tog_off + align_up(tog_bytes, ALIGN) + sizeof(int) > (size_t)h->L.Np * sizeof(uint32_t))
+        return fail(h, LBM_ENOMEM, "set_flags_mesh: box too small for the scratch layout");
+    CUDA_TRY(h, cudaMemsetAsync(votes, 0, (size_t)N, h->stream));
+    CUDA_TRY(h, cudaMemsetAsync(err, 0, sizeof(int), h->stream));
+    const int B = 128;
+    const unsigned tg = blocks_for((long long)n_tri * 32, B);
+    const int n[3] = {h->nx, h->ny, h->nz};
+    for (int d = 0; d < 3 && n_tri > 0; ++d) {
+        CUDA_TRY(h, cudaMemsetAsync(toggles, 0, tog_bytes, h->stream));
+        const unsigned sg = blocks_for((long long)n[(d + 1) % 3] * n[(d + 2) % 3], B);
+        if (d == 0) {
+            mesh_toggle_kernel<0><<<tg, B, 0, h->stream>>>(dev_tri, n_tri, (uint32_t *)toggles, h->nx, h->ny, h->nz, err);
+            mesh_scan_kernel<0><<<sg, B, 0, h->stream>>>(toggles, votes, h->nx, h->ny, h->nz);
+        } else if (d == 1) {
+            mesh_toggle_kernel<1><<<tg, B, 0, h->stream>>>(dev_tri, n_tri, (uint32_t *)toggles, h->nx, h->ny, h->nz, err);
+            mesh_scan_kernel<1><<<sg, B, 0, h->stream>>>(toggles, votes, h->nx, h->ny, h->nz);
+        } else {
+            mesh_toggle_kernel<2><<<tg, B, 0, h->stream>>>(dev_tri, n_tri, (uint32_t *)toggles, h->nx, h->ny, h->nz, err);
+            mesh_scan_kernel<2><<<sg, B, 0, h->stream>>>(toggles, votes, h->nx, h->ny, h->nz);
+        }
+        int rc = check_launch(h, "mesh_toggle_kernel / mesh_scan_kernel");
+        if (rc) return rc;
+        h->launches += 1;
+    }
+    int bad = 0;
+    CUDA_TRY(h, cudaMemcpyAsync(&bad, err, sizeof(int), cudaMemcpyDeviceToHost, h->stream));
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    if (bad) return fail(h, LBM_EINVAL, "set_flags_mesh: a vertex is not finite or outside [-1024, 2048) cells");
+    *votes_out = votes;
+    return LBM_OK;
+}
 template <typename real>
 int turb_publish(lbm_t *h, bool cells);
 
@@ -765,6 +808,38 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
     int rc = rewrite();
     CUDA_TRY(h, cudaStreamSynchronize(h->stream)); // t (host staging) must outlive the copy
     return rc;
+}
+
+int lbm_set_flags_mask(lbm_t *h, const int32_t *height, const uint8_t *solid)
+{
+    if (!h) return LBM_EINVAL;
+    if (!solid) return lbm_set_flags(h, height);
+    h->nmodes = 0;
+    const uint8_t *dev = solid;
+    if (!is_device_ptr(solid)) { // a host mask is parked in the link-word area (4 Np bytes, rewritten by classify afterwards)
+        CUDA_TRY(h, cudaMemcpyAsync(h->links(), solid, (size_t)h->N(), cudaMemcpyHostToDevice, h->stream));
+        dev = (const uint8_t *)h->links();
+    }
+    int rc = h->fp64 ? do_set_flags<double>(h, height, dev, 1) : do_set_flags<float>(h, height, dev, 1);
+    if (!rc && dev != solid) CUDA_TRY(h, cudaStreamSynchronize(h->stream)); // the caller's buffer is free on return
+    return rc;
+}
+
+int lbm_set_flags_mesh(lbm_t *h, const int32_t *height, int n_tri, const float *tri, int min_votes)
+{
+    if (!h) return LBM_EINVAL;
+    if (n_tri < 0 || (n_tri > 0 && !tri)) return fail(h, LBM_EINVAL, "set_flags_mesh: bad triangle array");
+    if (min_votes < 1 || min_votes > 3) return fail(h, LBM_EINVAL, "set_flags_mesh: min_votes must be 1, 2 or 3");
+    h->nmodes = 0;
+    InBuf in;
+    int rc = stage_in(h, tri, (size_t)n_tri * 9 * sizeof(float), 0, &in);
+    if (rc) return rc;
+    uint8_t *votes = nullptr;
+    rc = mesh_votes(h, n_tri, (const float *)in.dev, &votes);
+    release_in(h, &in, 1);
+    if (rc) return rc;
+    // the heightmap staging of do_set_flags may reuse the scratch area now: the triangles are consumed
+    return h->fp64 ? do_set_flags<double>(h, height, votes, min_votes) : do_set_flags<float>(h, height, votes, min_votes);
 }
 
 int lbm_set_flags(lbm_t *h, const int32_t *height)

@@ -6,12 +6,15 @@
 namespace lbmk {
 
 // ---- a1: voxelise the padded box ---------------------------------------------------------------------------------------
-// Interior: SOLID iff z < clamp(h[y][x], 0, nz); non-solid cells on an EQ face take the EQ class (EQ_FIXED wins).
+// Interior: SOLID iff z < clamp(h[y][x], 0, nz), or mask[z][y][x] >= thresh when a solid mask is merged in (PAPER.md:51
+// Boolean merge of base / terrain / building layers; the mask is a user's or the vote count of the mesh voxeliser,
+// lbm_mesh.cuh); non-solid cells on an EQ face take the EQ class (EQ_FIXED wins).
 // Halo: SOLID behind a WALL or EQ face (never pulled from / bounce-back), else the class follows the in-box image
 // cell (PERIODIC: wrapped, FREE_SLIP: clamped): image solid -> SOLID (DESIGN.md §3 step 4a "mirrored source SOLID ->
 // bounce-back"), else GHOST.  x padding beyond the halo: SOLID.
 template <typename real>
-__global__ void voxelise_kernel(const int32_t *__restrict__ height, uint8_t *__restrict__ flags, Params<real> P)
+__global__ void voxelise_kernel(const int32_t *__restrict__ height, const uint8_t *__restrict__ mask, int thresh,
+                                uint8_t *__restrict__ flags, Params<real> P)
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P.Np) return;
@@ -34,6 +37,7 @@ __global__ void voxelise_kernel(const int32_t *__restrict__ height, uint8_t *__r
     if (dead) { flags[p] = SOLID; return; }
     int h = height ? height[c[1] * P.nx + c[0]] : 0;
     h = min(max(h, 0), P.nz);
+    if (mask && mask[((long long)c[2] * P.ny + c[1]) * P.nx + c[0]] >= thresh) h = P.nz;
     int cls;
     if (c[2] < h) cls = SOLID;
     else if (halo) cls = GHOST;
