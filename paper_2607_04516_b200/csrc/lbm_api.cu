@@ -88,6 +88,9 @@ struct lbm {
     bool damp_on;   // damping zones configured (the DAMP instantiation of the step kernel runs)
     int dlo[3], dhi[3]; // the zone-free inner box
     int nmodes;     // synthetic inflow fluctuations: modes in use (0 = off)
+    // staging buffers for HOST inputs / outputs that do not fit the scratch area (whole-lattice fields): kept between
+    // calls, grown on demand, freed by lbm_destroy — a cudaMalloc + cudaFree pair per field per call costs milliseconds
+    struct Slot { void *p; size_t cap; bool busy; } slots[4];
     std::string err;
 
     void *bufA() const { return ws + L.off_A; }
@@ -164,22 +167,57 @@ bool is_device_ptr(const void *p)
 // Input staging.  Device sources are used in place; host sources are copied into the handle's scratch area when
 // they fit at the given offset, else into a temporary allocation.  release_in waits for the copies (so that the
 // caller's buffer is free on return) and frees temporaries.
-struct InBuf { const void *dev; void *tmp; bool host; };
+constexpr size_t SLOT_MAX = (size_t)2 << 30; // larger requests are not cached
+// a cached staging buffer of at least `bytes`; *slot = its index, or -1 for a one-off allocation (caller frees)
+void *stage_alloc(lbm_t *h, size_t bytes, int *slot)
+{
+    *slot = -1;
+    if (bytes <= SLOT_MAX) {
+        int pick = -1;
+        for (int k = 0; k < 4; ++k)
+            if (!h->slots[k].busy && h->slots[k].cap >= bytes && (pick < 0 || h->slots[k].cap < h->slots[pick].cap)) pick = k;
+        if (pick < 0)
+            for (int k = 0; k < 4; ++k)
+                if (!h->slots[k].busy && (pick < 0 || h->slots[k].cap < h->slots[pick].cap)) pick = k;
+        if (pick >= 0) {
+            lbm::Slot &s = h->slots[pick];
+            if (s.cap < bytes) {
+                if (s.p) cudaFree(s.p);
+                s.p = nullptr; s.cap = 0;
+                if (cudaMalloc(&s.p, bytes) != cudaSuccess) { cudaGetLastError(); s.p = nullptr; return nullptr; }
+                s.cap = bytes;
+            }
+            s.busy = true;
+            *slot = pick;
+            return s.p;
+        }
+    }
+    void *d = nullptr;
+    if (cudaMalloc(&d, bytes) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+    return d;
+}
+void stage_free(lbm_t *h, void *p, int slot)
+{
+    if (slot >= 0) h->slots[slot].busy = false;
+    else if (p) cudaFree(p);
+}
+
+struct InBuf { const void *dev; void *tmp; bool host; int slot; };
 int stage_in(lbm_t *h, const void *src, size_t bytes, size_t scratch_off, InBuf *b)
 {
-    b->dev = nullptr; b->tmp = nullptr; b->host = false;
+    b->dev = nullptr; b->tmp = nullptr; b->host = false; b->slot = -1;
     if (!src) return LBM_OK;
     if (is_device_ptr(src)) { b->dev = src; return LBM_OK; }
     void *d = nullptr;
     if (scratch_off + bytes <= h->L.scratch_bytes) d = (char *)h->scratch() + scratch_off;
     else {
-        cudaError_t e = cudaMalloc(&d, bytes);
-        if (e != cudaSuccess) { cudaGetLastError(); return fail(h, LBM_ENOMEM, std::string("cudaMalloc staging: ") + cudaGetErrorString(e)); }
+        d = stage_alloc(h, bytes, &b->slot);
+        if (!d) return fail(h, LBM_ENOMEM, "cudaMalloc staging (input)");
         b->tmp = d;
     }
     cudaError_t e = cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, h->stream);
     if (e != cudaSuccess) {
-        if (b->tmp) cudaFree(b->tmp);
+        if (b->tmp) stage_free(h, b->tmp, b->slot);
         b->tmp = nullptr;
         return fail(h, LBM_ECUDA, std::string("H2D copy: ") + cudaGetErrorString(e));
     }
@@ -192,18 +230,18 @@ void release_in(lbm_t *h, InBuf *b, int n)
     for (int k = 0; k < n; ++k) any |= b[k].host;
     if (any) cudaStreamSynchronize(h->stream);
     for (int k = 0; k < n; ++k)
-        if (b[k].tmp) { cudaFree(b[k].tmp); b[k].tmp = nullptr; }
+        if (b[k].tmp) { stage_free(h, b[k].tmp, b[k].slot); b[k].tmp = nullptr; }
 }
 
 // Output staging: if dst is a host pointer allocate a device buffer; finish_out copies back and frees.
-struct OutBuf { void *host; void *dev; size_t bytes; bool temp; };
+struct OutBuf { void *host; void *dev; size_t bytes; bool temp; int slot; };
 int stage_out(lbm_t *h, void *dst, size_t bytes, OutBuf *o)
 {
-    o->host = nullptr; o->dev = nullptr; o->bytes = bytes; o->temp = false;
+    o->host = nullptr; o->dev = nullptr; o->bytes = bytes; o->temp = false; o->slot = -1;
     if (!dst) return LBM_OK;
     if (is_device_ptr(dst)) { o->dev = dst; return LBM_OK; }
-    cudaError_t e = cudaMalloc(&o->dev, bytes);
-    if (e != cudaSuccess) return fail(h, LBM_ENOMEM, std::string("cudaMalloc staging: ") + cudaGetErrorString(e));
+    o->dev = stage_alloc(h, bytes, &o->slot);
+    if (!o->dev) return fail(h, LBM_ENOMEM, "cudaMalloc staging (output)");
     o->host = dst; o->temp = true;
     return LBM_OK;
 }
@@ -222,7 +260,7 @@ int finish_out(lbm_t *h, OutBuf *outs, int n)
         if (e != cudaSuccess) rc = fail(h, LBM_ECUDA, std::string("sync: ") + cudaGetErrorString(e));
     }
     for (int k = 0; k < n; ++k)
-        if (outs[k].temp) cudaFree(outs[k].dev);
+        if (outs[k].temp) stage_free(h, outs[k].dev, outs[k].slot);
     return rc;
 }
 
@@ -276,8 +314,8 @@ int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, con
     InBuf in[3];
     const size_t bytes = count * sizeof(in_t);
     int rc = stage_in(h, u, bytes, 0, &in[0]);
-    if (!rc) rc = stage_in(h, v, bytes, align_up(bytes, ALIGN), &in[1]); else in[1] = InBuf{nullptr, nullptr, false};
-    if (!rc) rc = stage_in(h, w, bytes, 2 * align_up(bytes, ALIGN), &in[2]); else in[2] = InBuf{nullptr, nullptr, false};
+    if (!rc) rc = stage_in(h, v, bytes, align_up(bytes, ALIGN), &in[1]); else in[1] = InBuf{nullptr, nullptr, false, -1};
+    if (!rc) rc = stage_in(h, w, bytes, 2 * align_up(bytes, ALIGN), &in[2]); else in[2] = InBuf{nullptr, nullptr, false, -1};
     if (!rc) {
         const int B = 256;
         const long long threads = mode == 0 ? (long long)P.N : (long long)count;
@@ -655,6 +693,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     h->cur = 0; h->have_flags = false; h->step = 0;
     h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false; h->nmodes = 0;
     for (int a = 0; a < 3; ++a) { h->dlo[a] = 0; h->dhi[a] = 0; }
+    for (int k = 0; k < 4; ++k) h->slots[k] = lbm::Slot{nullptr, 0, false};
     if (dev_workspace) {
         if (workspace_bytes < h->L.total || ((uintptr_t)dev_workspace % ALIGN) != 0 || !is_device_ptr(dev_workspace)) {
             delete h;
@@ -681,6 +720,8 @@ int lbm_destroy(lbm_t *h)
     if (!h) return LBM_EINVAL;
     cudaStreamSynchronize(h->stream);
     if (h->own_ws) cudaFree(h->ws);
+    for (int k = 0; k < 4; ++k)
+        if (h->slots[k].p) cudaFree(h->slots[k].p);
     delete h;
     return LBM_OK;
 }
