@@ -106,7 +106,10 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
         });
         // a cell on an EQ face fetches its face velocity now, from geometry alone (EQ_FIXED wins, as in the voxeliser);
         // if the flag then says SOLID the three values are simply not used
-        if (P.F > 0) {
+        // (one unsigned compare per axis: c - 1 >= n - 2 <=> c == 0 or c == n - 1; interior warps skip the owner search)
+        const bool onface = ((unsigned)(x - 1) >= (unsigned)(P.nx - 2)) | ((unsigned)(y - 1) >= (unsigned)(P.ny - 2)) |
+                            ((unsigned)(z - 1) >= (unsigned)(P.nz - 2));
+        if (P.F > 0 && onface) {
             int k = eq_owner(P, FACE_EQ_FIXED, x, y, z);
             if (k < 0) k = eq_owner(P, FACE_EQ_OUTFLOW, x, y, z);
             if (k >= 0) {
@@ -119,6 +122,25 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
         fl = flags[p];
     }
     if constexpr (EXP == 1) fl = 0; // timing experiment: every cell FLUID, no boundary stores
+    if constexpr (SPEC) {
+        // Fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, no feed, nothing to complete)
+        // — the bulk of the lattice.  Straight-line collide + 19 stores, none of the per-feature tests below.
+        if (__all_sync(__activemask(), fl == 0)) {
+            Macro<real> m;
+            if constexpr (DAMP) m = collide<real, true>(g, P, damp_at(P, x, y, z));
+            else m = collide(g, P);
+            static_for<0, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                st_pop<HINT>(T.dst[i] + p, g[i]);
+            });
+            if constexpr (MEAN) {
+                msum[p] += m.ux;
+                msum[P.stride + p] += m.uy;
+                msum[2 * P.stride + p] += m.uz;
+            }
+            return;
+        }
+    }
     const int cls = fl & CLASS_MASK;
     // link word: wall links of a FLUID cell / zero-fill mask of a surface SOLID cell; one predicated load for both,
     // issued as soon as the flag is there and consumed only after the collision
