@@ -150,7 +150,7 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
  * x = cell indices, t = step number, all in lattice units.  The random draws are the caller's: modes = HOST array
  * [n_modes][9] = kappa[3], sigma[3] (unit, normal to kappa), psi, omega, dkappa  (omega = kappa . U_c gives a frozen
  * pattern carried with U_c).  Active inflow cells = EQ_FIXED cells whose mean velocity points into the domain
- * (u_b . n < 0, n = outward normal of the owner face); after k steps such a cell holds f_eq(1, u_b + u'(x, k)); every
+ * (u_b . n < -1e-7 lattice units — inward by more than rounding noise —, n = outward normal of the owner face); after k steps such a cell holds f_eq(1, u_b + u'(x, k)); every
  * other EQ_FIXED cell keeps the mean.  The mean is the boundary state in force when the call is made: while
  * fluctuations are on, lbm_set_inlet_profile / _plane, lbm_feed_inlet and lbm_balance_flux return LBM_ESTATE.
  * n_modes = 0 switches them off and restores the mean (modes may be NULL).  lbm_set_flags switches them off too.

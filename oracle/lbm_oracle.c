@@ -461,7 +461,9 @@ int oracle_get_links(const oracle_t *o, uint32_t *out)
  *     E(k) = alpha (u_rms^2 / k_e) (k/k_e)^4 / [1 + (k/k_e)^2]^(17/6) exp(-2 (k/k_eta)^2),   alpha = 1.453.
  * x = cell indices (lattice units), t = step number.  The random draws (kappa_n, sigma_n, psi_n, omega_n, dkappa_n)
  * are INPUTS.  An EQ_FIXED cell is an "active inflow cell" when its mean velocity points into the domain,
- * ub . n < 0 with n the outward normal of its owner face; only those carry u'.  After k steps such a cell holds
+ * ub . n < -1e-7 with n the outward normal of its owner face (the threshold, lattice units, keeps a normal component
+ * that is zero up to rounding — e.g. a top face with w = 0 after the flux correction of a balanced profile — from
+ * being "inflow" or not by the sign of its noise; DESIGN.md §4 reading 21); only those carry u'.  After k steps such a cell holds
  * f_eq(1, ub + u'(x, k)). */
 static double vk_spectrum(double k, double u_rms, double k_e, double k_eta)
 {
@@ -500,7 +502,7 @@ static void boundary_velocity(const oracle_t *o, int x, int y, int z, double t, 
     int k = fixed_face(o, x, y, z);
     if (k < 0) return;
     double un = (k % 2 ? 1.0 : -1.0) * u[k / 2]; /* ub . n, n outward */
-    if (!(un < 0.0)) return;
+    if (!(un < -1e-7)) return;
     double up[3];
     fluctuation(o, x, y, z, t, up);
     for (int a = 0; a < 3; ++a) u[a] += up[a];

@@ -183,7 +183,7 @@ __global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, real *_
 
 // ---- synthetic inflow fluctuations (lbm_set_inflow_turbulence; Table 1) -------------------
 // One thread per face-velocity slot.  For an EQ_FIXED cell whose MEAN velocity (fum) points into the domain
-// (ub . n < 0, n = outward normal of the owner face) the boundary velocity of time t is
+// (ub . n < -1e-7, n = outward normal of the owner face) the boundary velocity of time t is
 //     u_b = ub + sum_n a_n cos(kappa_n . x + psi_n - omega_n t),     a_n = 2 sqrt(E(|kappa_n|) dkappa_n) sigma_n,
 // x = cell indices (DESIGN.md §4 reading 21); all other EQ_FIXED cells keep the mean.  modes = [n][8] doubles:
 // kappa[3], a[3], psi, omega (amplitudes folded on the host).  The phase is formed and reduced to [-pi, pi] in FP64 (t
@@ -215,7 +215,7 @@ __device__ __forceinline__ void fluct_slot(int s, real *__restrict__ A, real *__
     real u0 = tb.fum[s], u1 = tb.fum[P.F + s], u2 = tb.fum[2 * P.F + s];
     const real ua = axis == 0 ? u0 : (axis == 1 ? u1 : u2);
     const real un = (k & 1) ? ua : -ua;
-    if (un < real(0)) {
+    if (un < real(-1e-7)) { // "active inflow": inward by more than rounding noise (DESIGN.md §4 reading 21)
         real a0 = real(0), a1 = real(0), a2 = real(0);
         const double xd = (double)x, yd = (double)y, zd = (double)z;
         for (int n = 0; n < tb.n; ++n) {
