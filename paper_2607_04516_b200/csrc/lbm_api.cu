@@ -88,6 +88,7 @@ struct lbm {
     bool damp_on;   // damping zones configured (the DAMP instantiation of the step kernel runs)
     int dlo[3], dhi[3]; // the zone-free inner box
     int nmodes;     // synthetic inflow fluctuations: modes in use (0 = off)
+    int loop_ok;    // multi-step cooperative launch: 0 = not probed yet, 1 = the whole grid is resident, -1 = no
     // staging buffers for HOST inputs / outputs that do not fit the scratch area (whole-lattice fields): kept between
     // calls, grown on demand, freed by lbm_destroy — a cudaMalloc + cudaFree pair per field per call costs milliseconds
     struct Slot { void *p; size_t cap; bool busy; } slots[4];
@@ -509,11 +510,58 @@ int turb_publish(lbm_t *h, bool cells)
     return rc;
 }
 
+// Small lattices (the whole grid resident at once): 2 * pairs steps in one cooperative launch (step_loop_kernel).
+// Returns the number of steps done (0 = not applicable here: use single launches), or a negative error code.
+template <typename real>
+int try_step_loop(lbm_t *h, const Params<real> &P, int want)
+{
+    if constexpr (!std::is_same<real, float>::value) return 0;
+    else {
+        if (h->variant != 0 || h->nmodes > 0 || want < 4 || h->loop_ok < 0) return 0;
+        constexpr int BLOCK = 128;
+        const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
+        const void *fn = h->damp_on ? (const void *)step_loop_kernel<float, BLOCK, 10, true> : (const void *)step_loop_kernel<float, BLOCK, 10, false>;
+        if (h->loop_ok == 0) { // once per handle: can the whole grid be resident?
+            int dev = 0, sms = 0, coop = 0, per_sm = 0;
+            cudaGetDevice(&dev);
+            cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+            cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, BLOCK, 0);
+            h->loop_ok = (coop && (long long)per_sm * sms >= (long long)grid.x * grid.y) ? 1 : -1;
+            cudaGetLastError();
+            if (h->loop_ok < 0) return 0;
+        }
+        int pairs = want / 2;
+        real *A = (real *)h->state(), *B = (real *)h->other();
+        real *fu0 = (real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F, *fu1 = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
+        StepPtrs<real> T0 = make_step_ptrs<real>(A, B, P), T1 = make_step_ptrs<real>(B, A, P);
+        const uint8_t *fl = h->flags();
+        const uint32_t *lk = h->links();
+        Params<real> Pc = P;
+        void *args[] = {&A, &B, &fl, &lk, &fu0, &fu1, &Pc, &T0, &T1, &pairs};
+        cudaError_t e = cudaLaunchCooperativeKernel(fn, grid, dim3(BLOCK), args, 0, h->stream);
+        if (e != cudaSuccess) { cudaGetLastError(); h->loop_ok = -1; return 0; } // e.g. too large after all: single launches
+        h->launches += 1;
+        return 2 * pairs;
+    }
+}
+
 template <typename real>
 int do_step(lbm_t *h, int n)
 {
     const Params<real> P = make_params<real>(h);
     for (int it = 0; it < n; ++it) {
+        {   // as many steps as possible before the next sampling step go into one cooperative launch (small lattices only)
+            long run = n - it;
+            if (h->mevery > 0) {
+                const long k0 = h->step + 1;
+                long ks = k0 <= h->mstart ? h->mstart : h->mstart + ((k0 - h->mstart + h->mevery - 1) / h->mevery) * h->mevery;
+                run = std::min(run, ks - k0); // steps k0 .. ks-1 do not sample
+            }
+            const int done = run >= 4 ? try_step_loop<real>(h, P, (int)std::min(run, 1000000L)) : 0;
+            if (done < 0) return done;
+            if (done > 0) { h->step += done; it += done - 1; continue; }
+        }
         const long k = h->step + 1;
         const bool sample = h->mevery > 0 && k >= h->mstart && (k - h->mstart) % h->mevery == 0;
         int rc = launch_step<real>(h, P, sample);
@@ -691,7 +739,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     h->L = make_layout(nx, ny, nz, h->want_mean, h->fp64);
     h->stream = (cudaStream_t)cuda_stream;
     h->cur = 0; h->have_flags = false; h->step = 0;
-    h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false; h->nmodes = 0;
+    h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false; h->nmodes = 0; h->loop_ok = 0;
     for (int a = 0; a < 3; ++a) { h->dlo[a] = 0; h->dhi[a] = 0; }
     for (int k = 0; k < 4; ++k) h->slots[k] = lbm::Slot{nullptr, 0, false};
     if (dev_workspace) {

@@ -16,6 +16,7 @@
 #pragma once
 #include "lbm_core.cuh"
 #include "lbm_setup.cuh"
+#include <cooperative_groups.h>
 
 namespace lbmk {
 
@@ -71,11 +72,13 @@ inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> 
     return t;
 }
 
-template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false, bool TURB = false>
-__global__ void __launch_bounds__(BLOCK, MINB)
-step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-            real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T,
-            const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
+// The step of one thread (one cell, or one face slot in a TURB block row).  A plain device function so that it can be
+// called once per launch (step_kernel) or in a loop with grid-wide barriers (step_loop_kernel, lattices that fit L2).
+template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int EXP, bool DAMP, bool TURB>
+__device__ __forceinline__ void step_body(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+                                          const uint32_t *__restrict__ links, real *__restrict__ msum, const real *__restrict__ fur,
+                                          real *__restrict__ fuw, const Params<real> &P, const StepPtrs<real> &T, const Turb<real> &tb,
+                                          const int turb_planes)
 {
     int zb = blockIdx.y;
     if constexpr (TURB) {
@@ -202,6 +205,37 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
         msum[p] += m.ux;
         msum[P.stride + p] += m.uy;
         msum[2 * P.stride + p] += m.uz;
+    }
+}
+
+template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false, bool TURB = false>
+__global__ void __launch_bounds__(BLOCK, MINB)
+step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+            real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T,
+            const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
+{
+    step_body<real, MEAN, HINT, SPEC, BLOCK, EXP, DAMP, TURB>(A, B, flags, links, msum, fur, fuw, P, T, tb, turb_planes);
+}
+
+// Several steps in ONE cooperative launch, a grid-wide barrier between them: for lattices whose whole grid is resident
+// at once (<= 10 CTAs x 148 SMs x 128 cells; config 1) a step is a few microseconds of work and one dependent launch per
+// step would dominate (8.2 us per step measured).  2 * pairs steps: A -> B with table T0, then B -> A with table T1.
+// Every pull, the flag byte and the face velocities are read with ld.volatile / from read-only data, the barrier orders
+// the stores of one step before the loads of the next.  No time mean, no inflow fluctuations on this path (the host
+// falls back to single launches for those steps).
+template <typename real, int BLOCK, int MINB, bool DAMP>
+__global__ void __launch_bounds__(BLOCK, MINB)
+step_loop_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+                 real *__restrict__ fu0, real *__restrict__ fu1, const Params<real> P, const StepPtrs<real> T0, const StepPtrs<real> T1,
+                 const int pairs)
+{
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();
+    const Turb<real> tb{};
+    for (int s = 0; s < pairs; ++s) {
+        step_body<real, false, 0, true, BLOCK, 0, DAMP, false>(A, B, flags, links, nullptr, fu0, fu1, P, T0, tb, 0);
+        grid.sync();
+        step_body<real, false, 0, true, BLOCK, 0, DAMP, false>(B, A, flags, links, nullptr, fu1, fu0, P, T1, tb, 0);
+        grid.sync();
     }
 }
 
