@@ -856,3 +856,30 @@ def test_flow_around_mesh_voxelised_overhangs_matches_the_oracle(B, fp64):
     e = max_err(sim, o, f64=fp64)
     assert e <= (TOL64 if fp64 else TOL32), (fp64, e)
     sim.close()
+
+
+def test_cooperative_multi_step_launch_equals_single_launches_bit_for_bit(B):
+    """lbm_step(n) on a lattice whose grid is resident runs in one cooperative launch (step_loop_kernel); stepping one at a
+    time uses one launch per step.  Same step body, same arithmetic: the states must be identical, with buildings,
+    every face rule, damping zones, and a time mean whose sampling steps cut the run into several loops."""
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config1()
+    prof = wl.inlet_profile[0].astype(np.float64)
+    target = np.stack([prof, np.zeros_like(prof), np.zeros_like(prof)])
+    sims = [B.from_workload(wl), B.from_workload(wl)]
+    for s in sims:
+        s.set_damping((0, 6, 0, 0, 0, 5), (0, 0.1, 0, 0, 0, 0.2), target)
+        s.mean_config(10, 7)
+    l0 = [s.launch_count() for s in sims]
+    sims[0].step(101)
+    for _ in range(101):
+        sims[1].step(1)
+    n_loop, n_single = sims[0].launch_count() - l0[0], sims[1].launch_count() - l0[1]
+    assert n_single == 101 and n_loop < 40, (n_loop, n_single)
+    assert np.array_equal(sims[0].get_state(out="host"), sims[1].get_state(out="host"))
+    m0, m1 = sims[0].get_mean(out="host"), sims[1].get_mean(out="host")
+    assert m0[3] == m1[3] == 14
+    for a, b in zip(m0[:3], m1[:3]):
+        assert np.array_equal(a, b)
+    for s in sims:
+        s.close()
