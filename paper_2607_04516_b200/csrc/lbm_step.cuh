@@ -102,6 +102,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     real g[Q];
     uint8_t fl;
     real fu0 = real(0), fu1 = real(0), fu2 = real(0); // face velocity of an EQ cell
+    real ms0 = real(0), ms1 = real(0), ms2 = real(0); // running mean sums (MEAN && SPEC: prefetched)
     if constexpr (SPEC) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
@@ -120,6 +121,9 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
                 fu0 = ld_pinned(fur + sl); fu1 = ld_pinned(fur + P.F + sl); fu2 = ld_pinned(fur + 2 * P.F + sl);
             }
         }
+        // sampling steps: the three running sums are fetched with the pulls (their latency hides behind the collision
+        // instead of a dependent read-modify-write at the end; SOLID cells simply do not use them)
+        if constexpr (MEAN) { ms0 = ld_pinned(msum + p); ms1 = ld_pinned(msum + P.stride + p); ms2 = ld_pinned(msum + 2 * P.stride + p); }
         fl = ld_pinned(flags + p); // volatile asm statements keep their order: the flag test cannot move above the pulls
     } else {
         fl = flags[p];
@@ -137,9 +141,9 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
                 st_pop<HINT>(T.dst[i] + p, g[i]);
             });
             if constexpr (MEAN) {
-                msum[p] += m.ux;
-                msum[P.stride + p] += m.uy;
-                msum[2 * P.stride + p] += m.uz;
+                msum[p] = ms0 + m.ux;
+                msum[P.stride + p] = ms1 + m.uy;
+                msum[2 * P.stride + p] = ms2 + m.uz;
             }
             return;
         }
@@ -202,9 +206,15 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
         ghost_stores(P, x, y, z, lk, [&](int i, int pt, auto jc) { B[(long long)i * P.stride + pt] = g[decltype(jc)::value]; });
     if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) { fuw[comp * P.F + sl] = v; });
     if constexpr (MEAN) {
-        msum[p] += m.ux;
-        msum[P.stride + p] += m.uy;
-        msum[2 * P.stride + p] += m.uz;
+        if constexpr (SPEC) {
+            msum[p] = ms0 + m.ux;
+            msum[P.stride + p] = ms1 + m.uy;
+            msum[2 * P.stride + p] = ms2 + m.uz;
+        } else {
+            msum[p] += m.ux;
+            msum[P.stride + p] += m.uy;
+            msum[2 * P.stride + p] += m.uz;
+        }
     }
 }
 
