@@ -452,7 +452,7 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 // kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes / load issue order.
 constexpr int N_VARIANTS = 11;
 #ifndef DAMP_MINB
-#define DAMP_MINB 10
+#define DAMP_MINB 9
 #endif
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
@@ -462,7 +462,7 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         if constexpr (std::is_same<real, float>::value) {
             if (h->damp_on && turb) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true, true>(h, P, sample);
             if (h->damp_on) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true, false>(h, P, sample);
-            return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, false, true>(h, P, sample);
+            return launch_step_as<real, 0, true, 128, 10, 0, false, true>(h, P, sample); // no prefetched table values: 48 registers do
         } else {
             if (h->damp_on && turb) return launch_step_as<real, 0, false, 256, 2, 0, true, true>(h, P, sample);
             if (h->damp_on) return launch_step_as<real, 0, false, 256, 2, 0, true, false>(h, P, sample);

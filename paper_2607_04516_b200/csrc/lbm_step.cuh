@@ -103,6 +103,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     uint8_t fl;
     real fu0 = real(0), fu1 = real(0), fu2 = real(0); // face velocity of an EQ cell
     real ms0 = real(0), ms1 = real(0), ms2 = real(0); // running mean sums (MEAN && SPEC: prefetched)
+    Damp<real> dmp{real(0), real(0), real(0), real(0)}; // damping coefficient / target of the cell (DAMP && SPEC: prefetched)
     if constexpr (SPEC) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
@@ -123,6 +124,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
         }
         // sampling steps: the three running sums are fetched with the pulls (their latency hides behind the collision
         // instead of a dependent read-modify-write at the end; SOLID cells simply do not use them)
+        if constexpr (DAMP) dmp = damp_at(P, x, y, z); // table look-ups in flight with the pulls
         if constexpr (MEAN) { ms0 = ld_pinned(msum + p); ms1 = ld_pinned(msum + P.stride + p); ms2 = ld_pinned(msum + 2 * P.stride + p); }
         fl = ld_pinned(flags + p); // volatile asm statements keep their order: the flag test cannot move above the pulls
     } else {
@@ -134,7 +136,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
         // — the bulk of the lattice.  Straight-line collide + 19 stores, none of the per-feature tests below.
         if (__all_sync(__activemask(), fl == 0)) {
             Macro<real> m;
-            if constexpr (DAMP) m = collide<real, true>(g, P, damp_at(P, x, y, z));
+            if constexpr (DAMP) m = collide<real, true>(g, P, dmp);
             else m = collide(g, P);
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
@@ -167,7 +169,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
                 g[i] = ld_pop<HINT>(T.src[i] + p);
             });
         }
-        if constexpr (DAMP) m = collide<real, true>(g, P, damp_at(P, x, y, z));
+        if constexpr (DAMP) m = collide<real, true>(g, P, SPEC ? dmp : damp_at(P, x, y, z));
         else m = collide(g, P);
     } else if (cls != SOLID) { // EQ_FIXED (a3) / EQ_OUTFLOW (a6): f_eq(1, u) of the cell's face velocity (lbm_core.cuh)
         if constexpr (!SPEC) {
