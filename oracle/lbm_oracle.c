@@ -55,6 +55,19 @@ static const int CI[Q][3] = {
 
 static double weight(int i) { return i == 0 ? 1.0 / 3.0 : (i <= 6 ? 1.0 / 18.0 : 1.0 / 36.0); }
 
+/* Thermal lattice D3Q7: the rest vector and the six axis vectors = directions 0..6 of CI;
+ * weights 1/4 and 1/8, lattice sound speed squared 1/4 (sum_i wT_i c_ia c_ib = delta_ab / 4). */
+#define QT 7
+static double weight_t(int i) { return i == 0 ? 0.25 : 0.125; }
+/* linear advection-diffusion equilibrium h_eq,i = wT_i theta (1 + c_i.u / c_sT^2) = wT_i theta (1 + 4 c_i.u) */
+static void heq(double theta, const double u[3], double out[QT])
+{
+    for (int i = 0; i < QT; ++i) {
+        double cu = CI[i][0] * u[0] + CI[i][1] * u[1] + CI[i][2] * u[2];
+        out[i] = weight_t(i) * theta * (1.0 + 4.0 * cu);
+    }
+}
+
 static int dir_index(int cx, int cy, int cz)
 {
     for (int i = 0; i < Q; ++i)
@@ -97,6 +110,11 @@ typedef struct oracle {
     double *msum; /* [cell][3] */
     long mcount, mstart;
     int mevery;
+    /* thermal lattice (Table 1 "Optional D3Q7 ... thermal lattice with Boussinesq coupling"; DESIGN.md §4
+     * reading 23): off unless oracle_set_thermal was called */
+    int thermal;
+    double alpha, gbeta, theta_ref; /* diffusivity, g*beta (buoyancy per unit theta, along +z), reference theta */
+    double *H, *Hn;                 /* [cell][7] post-collision thermal populations, directions 0..6 of CI */
 } oracle_t;
 
 static long cell_of(const oracle_t *o, int x, int y, int z)
@@ -247,8 +265,16 @@ static void local_macros(const oracle_t *o, const double *Gs, long cell, double 
         long zc = cell / ((long)o->nx * o->ny);
         for (int a = 0; a < 3; ++a)
             for (int c = 0; c < 3; ++c) M[a][c] = (a == c ? 1.0 - 0.5 * sg : 0.0) + 0.5 * Cm[a][c];
+        double Fl[3] = {o->F[0], o->F[1], o->F[2]};
+        if (o->thermal && Gs == o->G) {
+            /* Boussinesq: the buoyancy the cell's collision used is g beta (theta - theta_ref) with theta = sum_i h_i,
+             * which the thermal collision conserves: read it back from the stored thermal state */
+            double th = 0.0;
+            for (int i = 0; i < QT; ++i) th += o->H[cell * QT + i];
+            Fl[2] += o->gbeta * (th - o->theta_ref);
+        }
         double b[3];
-        for (int a = 0; a < 3; ++a) b[a] = m[a] / r - 0.5 * o->F[a] - 0.5 * sg * (o->ut ? o->ut[a * o->nz + zc] : 0.0);
+        for (int a = 0; a < 3; ++a) b[a] = m[a] / r - 0.5 * Fl[a] - 0.5 * sg * (o->ut ? o->ut[a * o->nz + zc] : 0.0);
         solve3(M, b, u);
     } else {
         u[0] = m[0] / r; u[1] = m[1] / r; u[2] = m[2] / r;
@@ -320,7 +346,7 @@ oracle_t *oracle_create(int nx, int ny, int nz, double nu0, double Cs, double fc
 void oracle_destroy(oracle_t *o)
 {
     if (!o) return;
-    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o->sig); free(o->ut); free(o->modes); free(o->uhat); free(o);
+    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o->sig); free(o->ut); free(o->modes); free(o->uhat); free(o->H); free(o->Hn); free(o);
 }
 
 /* Damping zones (see collide()).  width[k] (cells) and peak[k] for the six faces x-,x+,y-,y+,z-,z+; a cell at
@@ -716,7 +742,28 @@ int oracle_step(oracle_t *o, int nsteps)
                         }
                         double ut[3] = {0, 0, 0};
                         if (o->ut) for (int a = 0; a < 3; ++a) ut[a] = o->ut[a * o->nz + z];
-                        collide(f, o->nu0, o->Cs, o->fv, o->F, o->sig ? o->sig[cell] : 0.0, ut, gn, NULL, NULL, NULL);
+                        if (!o->thermal) {
+                            collide(f, o->nu0, o->Cs, o->fv, o->F, o->sig ? o->sig[cell] : 0.0, ut, gn, NULL, NULL, NULL);
+                        } else {
+                            /* thermal lattice (reading 23): pull the 7 thermal populations by the same rule 4a
+                             * (bounce-back on walls / solids and specular reflection on free-slip faces = no heat flux),
+                             * theta = sum_i h_i; the flow collision sees F + g beta (theta - theta_ref) e_z; the thermal
+                             * BGK relaxes towards h_eq(theta, u) with the velocity u of that flow collision */
+                            double h[QT], theta = 0.0;
+                            for (int i = 0; i < QT; ++i) {
+                                long s = 0; int j = 0;
+                                int r = resolve(o, x, y, z, i, &s, &j);
+                                if (r < 0) { bad = 1; r = 1; }
+                                h[i] = r ? o->H[cell * QT + opposite(i)] : o->H[s * QT + j];
+                                theta += h[i];
+                            }
+                            double Fb[3] = {o->F[0], o->F[1], o->F[2] + o->gbeta * (theta - o->theta_ref)};
+                            double u[3];
+                            collide(f, o->nu0, o->Cs, o->fv, Fb, o->sig ? o->sig[cell] : 0.0, ut, gn, NULL, u, NULL);
+                            double he[QT], tau_t = 4.0 * o->alpha + 0.5;
+                            heq(theta, u, he);
+                            for (int i = 0; i < QT; ++i) o->Hn[cell * QT + i] = h[i] - (h[i] - he[i]) / tau_t;
+                        }
                     } else if (cl == C_EQ_OUTFLOW) {
                         /* step 6 */
                         int k = outflow_face(o, x, y, z);
@@ -736,8 +783,10 @@ int oracle_step(oracle_t *o, int nsteps)
                         /* SOLID: inert; EQ_FIXED (step 5): unchanged */
                         memcpy(gn, o->G + cell * Q, sizeof(double) * Q);
                     }
+                    if (o->thermal && cl != C_FLUID) memcpy(o->Hn + cell * QT, o->H + cell * QT, sizeof(double) * QT);
                 }
         double *t = o->G; o->G = o->Gn; o->Gn = t;
+        if (o->thermal) { t = o->H; o->H = o->Hn; o->Hn = t; }
         o->step += 1;
         /* step 8 */
         if (o->mevery > 0 && o->step >= o->mstart && (o->step - o->mstart) % o->mevery == 0) sample_mean(o);
@@ -813,3 +862,57 @@ int oracle_set_state(oracle_t *o, const double *f)
 
 long oracle_get_step(const oracle_t *o) { return o->step; }
 int oracle_set_step(oracle_t *o, long s) { o->step = s; return 0; }
+
+/* ------------------------------------------------------------------ thermal lattice (reading 23) */
+
+/* Switch the D3Q7 thermal lattice on: diffusivity alpha (tau_theta = 4 alpha + 1/2), buoyancy coefficient gbeta
+ * (acceleration g beta (theta - theta_ref) along +z), reference theta.  The thermal state is set to theta_ref at rest.
+ * Faces must be PERIODIC / WALL / FREE_SLIP (the density-current set-up of PAPER.md:121 is a closed box); -1 otherwise. */
+int oracle_set_thermal(oracle_t *o, double alpha, double gbeta, double theta_ref)
+{
+    for (int k = 0; k < 6; ++k)
+        if (o->face[k] == F_EQ_FIXED || o->face[k] == F_EQ_OUTFLOW) return -1;
+    if (!(alpha > 0.0)) return -1;
+    long N = (long)o->nx * o->ny * o->nz;
+    if (!o->H) {
+        o->H = (double *)malloc(sizeof(double) * N * QT);
+        o->Hn = (double *)malloc(sizeof(double) * N * QT);
+        if (!o->H || !o->Hn) return -4;
+    }
+    o->alpha = alpha; o->gbeta = gbeta; o->theta_ref = theta_ref; o->thermal = 1;
+    for (long cell = 0; cell < N; ++cell)
+        for (int i = 0; i < QT; ++i) o->H[cell * QT + i] = o->Hn[cell * QT + i] = weight_t(i) * theta_ref;
+    return 0;
+}
+
+/* H0 = h_eq(theta0, u0); NULL velocity component => 0; SOLID cells: theta_ref at rest. */
+int oracle_set_theta(oracle_t *o, const double *theta, const double *ux, const double *uy, const double *uz)
+{
+    if (!o->thermal) return -3;
+    long N = (long)o->nx * o->ny * o->nz;
+    for (long cell = 0; cell < N; ++cell) {
+        double th = theta ? theta[cell] : o->theta_ref;
+        double u[3] = {ux ? ux[cell] : 0.0, uy ? uy[cell] : 0.0, uz ? uz[cell] : 0.0};
+        if (o->cls[cell] == C_SOLID) { th = o->theta_ref; u[0] = u[1] = u[2] = 0.0; }
+        double h[QT];
+        heq(th, u, h);
+        memcpy(o->H + cell * QT, h, sizeof h);
+        memcpy(o->Hn + cell * QT, h, sizeof h);
+    }
+    return 0;
+}
+
+/* theta = sum_i h_i of the stored state; SOLID cells report theta_ref */
+int oracle_get_theta(const oracle_t *o, double *theta)
+{
+    if (!o->thermal) return -3;
+    long N = (long)o->nx * o->ny * o->nz;
+    for (long cell = 0; cell < N; ++cell) {
+        double th = 0.0;
+        for (int i = 0; i < QT; ++i) th += o->H[cell * QT + i];
+        theta[cell] = o->cls[cell] == C_SOLID ? o->theta_ref : th;
+    }
+    return 0;
+}
+
+int oracle_heq(double theta, const double *u, double *out) { heq(theta, u, out); return 0; }

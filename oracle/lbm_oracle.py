@@ -50,8 +50,12 @@ def _load():
                  "oracle_get_state", "oracle_set_state", "oracle_lattice", "oracle_feq", "oracle_collide_cell",
                  "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux",
                  "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping",
-                 "oracle_vk_spectrum", "oracle_set_inflow_turbulence", "oracle_set_flags_mask"):
+                 "oracle_vk_spectrum", "oracle_set_inflow_turbulence", "oracle_set_flags_mask",
+                 "oracle_set_theta", "oracle_get_theta", "oracle_heq"):
         getattr(lib, name).restype = C.c_int
+    lib.oracle_set_thermal.restype = C.c_int
+    lib.oracle_set_thermal.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
+    lib.oracle_heq.argtypes = [C.c_double, dp, dp]
     _lib = lib
     return lib
 
@@ -125,6 +129,15 @@ def collide_cell_damped(f, nu0, Cs, fvec, F, sigma, ut):
     lib.oracle_collide_cell_damped(fp, C.c_double(nu0), C.c_double(Cs), fvp, Fp, C.c_double(sigma), utp,
                                    g.ctypes.data_as(C.c_void_p), C.byref(rho), u.ctypes.data_as(C.c_void_p), C.byref(tau))
     return g, rho.value, u, tau.value
+
+
+def heq(theta, u):
+    """D3Q7 thermal equilibrium h_eq[7] (directions 0..6 of the lattice)."""
+    lib = _load()
+    u, up = _d(np.asarray(u, dtype=np.float64))
+    out = np.zeros(7)
+    lib.oracle_heq(float(theta), up, out.ctypes.data_as(C.POINTER(C.c_double)))
+    return out
 
 
 def vk_spectrum(k, u_rms, k_e, k_eta=0.0):
@@ -250,6 +263,21 @@ class Oracle:
         for a, _ in arrs:
             assert a is None or a.shape == self.shape
         self._chk(self._lib.oracle_set_macros(C.c_void_p(self._h), *[p for _, p in arrs]), "set_macros")
+
+    def set_thermal(self, alpha, gbeta=0.0, theta_ref=0.0):
+        self._chk(self._lib.oracle_set_thermal(C.c_void_p(self._h), float(alpha), float(gbeta), float(theta_ref)),
+                  "set_thermal")
+
+    def set_theta(self, theta=None, ux=None, uy=None, uz=None):
+        arrs = [_d(a) for a in (theta, ux, uy, uz)]
+        for a, _ in arrs:
+            assert a is None or a.shape == self.shape
+        self._chk(self._lib.oracle_set_theta(C.c_void_p(self._h), *[p for _, p in arrs]), "set_theta")
+
+    def get_theta(self):
+        out = np.zeros(self.shape)
+        self._chk(self._lib.oracle_get_theta(C.c_void_p(self._h), out.ctypes.data_as(C.c_void_p)), "get_theta")
+        return out
 
     def step(self, n=1):
         self._chk(self._lib.oracle_step(C.c_void_p(self._h), int(n)), "step")

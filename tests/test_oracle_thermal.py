@@ -1,0 +1,155 @@
+"""Pins of the oracle's thermal lattice + Boussinesq coupling (Table 1 "Optional D3Q7 ... thermal lattice
+with Boussinesq coupling"; DESIGN.md §4 reading 23) against what the mathematics fixes: equilibrium moments, the
+constant-temperature fixed point, heat conservation in a closed box, the diffusion decay rate alpha k^2, the advection
+speed of a temperature wave, and the exact momentum input of a uniform buoyancy.  CPU only."""
+import numpy as np
+import pytest
+
+from oracle import lbm_oracle as O
+
+P, W, FS = O.PERIODIC, O.WALL, O.FREE_SLIP
+
+
+def test_heq_moments():
+    c, _, _ = O.lattice()
+    c7 = c[:7].astype(float)
+    rng = np.random.default_rng(1)
+    for _ in range(5):
+        th = rng.uniform(0.5, 2.0)
+        u = rng.uniform(-0.1, 0.1, 3)
+        h = O.heq(th, u)
+        assert abs(h.sum() - th) < 1e-15
+        assert np.abs(c7.T @ h - th * u).max() < 1e-16
+        # second moment of the linear equilibrium: theta c_sT^2 I with c_sT^2 = 1/4
+        M2 = np.einsum("i,ia,ib->ab", h, c7, c7)
+        assert np.abs(M2 - th / 4 * np.eye(3)).max() < 1e-15
+    # the seven directions are the rest vector and the six axis vectors
+    assert sorted(map(tuple, c[:7].tolist())) == sorted([(0, 0, 0), (1, 0, 0), (-1, 0, 0), (0, 1, 0), (0, -1, 0), (0, 0, 1), (0, 0, -1)])
+
+
+def _tgv(n):
+    k = 2 * np.pi / n
+    z, y, x = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    return 0.04 * np.sin(k * x) * np.cos(k * y), -0.04 * np.cos(k * x) * np.sin(k * y)
+
+
+def test_constant_theta_is_a_fixed_point_under_uniform_flow():
+    # (under a compressible flow theta obeys the conservative law d theta/dt = -div(theta u), so only a divergence-free
+    # flow keeps a constant temperature constant: a uniform one does so exactly)
+    n = 8
+    o = O.Oracle(n, n, n, 2e-3, 0.1, 0.0, faces=[P] * 6)
+    o.set_flags()
+    U = [np.full((n, n, n), v) for v in (0.03, -0.02, 0.01)]
+    o.set_macros(None, *U)
+    o.set_thermal(0.01, 0.0, 1.0)
+    o.set_theta(np.full((n, n, n), 1.5), *U)
+    o.step(20)
+    assert np.abs(o.get_theta() - 1.5).max() < 1e-14
+    o.close()
+
+
+def test_heat_conserved_in_closed_box_with_solids_and_buoyancy():
+    nx, ny, nz = 14, 10, 12
+    o = O.Oracle(nx, ny, nz, 5e-3, 0.1, 1e-3, faces=[W, FS, P, P, W, FS])
+    h = np.zeros((ny, nx), np.int32)
+    h[3:6, 4:8] = 5
+    o.set_flags(h)
+    o.set_macros()
+    o.set_thermal(0.02, 1e-3, 1.0)
+    rng = np.random.default_rng(2)
+    th = 1.0 + 0.2 * rng.standard_normal((nz, ny, nx))
+    o.set_theta(th)
+    fluid = o.get_flags() == O.FLUID
+    s0 = o.get_theta()[fluid].sum()
+    o.step(150)
+    s1 = o.get_theta()[fluid].sum()
+    assert abs(s1 - s0) < 1e-12 * abs(s0)
+    rho, ux, uy, uz = o.get_macros()
+    assert np.abs(uz[fluid]).max() > 1e-5  # buoyancy did set the fluid in motion
+    assert abs(rho[fluid].sum() - fluid.sum()) < 1e-10 * fluid.sum()
+    o.close()
+
+
+@pytest.mark.parametrize("alpha", [0.01, 0.05])
+def test_diffusion_decay_rate(alpha):
+    # u = 0, no buoyancy, periodic: theta = ref + A cos(kx) decays like exp(-alpha k^2 t) (c_sT^2 (tau - 1/2) = alpha)
+    n = 64
+    o = O.Oracle(n, 2, 2, 1e-2, 0.0, 0.0, faces=[P] * 6)
+    o.set_flags()
+    o.set_macros()
+    o.set_thermal(alpha, 0.0, 1.0)
+    k = 2 * np.pi / n
+    x = np.arange(n)
+    th = np.broadcast_to(1.0 + 0.1 * np.cos(k * x), (2, 2, n)).copy()
+    o.set_theta(th)
+    o.step(50)
+    a0 = 2 * np.abs(np.fft.fft(o.get_theta()[0, 0] - 1.0)[1]) / n
+    o.step(400)
+    a1 = 2 * np.abs(np.fft.fft(o.get_theta()[0, 0] - 1.0)[1]) / n
+    rate = np.log(a0 / a1) / 400
+    assert abs(rate / (alpha * k * k) - 1.0) < 5e-3
+    o.close()
+
+
+def test_advection_speed_of_a_temperature_wave():
+    # uniform flow U along y (periodic, no forces): the wave's phase moves at speed U
+    n, U = 64, 0.05
+    o = O.Oracle(2, n, 2, 1e-2, 0.0, 0.0, faces=[P] * 6)
+    o.set_flags()
+    o.set_macros(None, None, np.full((2, n, 2), U), None)
+    o.set_thermal(0.005, 0.0, 0.0)
+    k = 2 * np.pi / n
+    y = np.arange(n)
+    th = np.broadcast_to((0.3 * np.cos(k * y))[None, :, None], (2, n, 2)).copy()
+    o.set_theta(th, None, np.full((2, n, 2), U), None)
+    steps = 200
+    o.step(steps)
+    ph = -np.angle(np.fft.fft(o.get_theta()[0, :, 0])[1])  # cos(k (y - U t)) -> coefficient e^{-i k U t}
+    assert abs(ph / (k * U * steps) - 1.0) < 5e-3
+    o.close()
+
+
+def test_uniform_buoyancy_adds_momentum_exactly():
+    # uniform theta = ref + D in a periodic box at rest: every cell feels a = g beta D e_z, a uniform body force;
+    # Guo forcing adds exactly rho a per step to the post-collision momentum: P_z(k) = k N g beta D (warm air rises)
+    n, gb, D = 6, 2e-4, 0.5
+    o = O.Oracle(n, n, n, 1e-2, 0.1, 0.0, faces=[P] * 6)
+    o.set_flags()
+    o.set_macros()
+    o.set_thermal(0.02, gb, 2.0)
+    o.set_theta(np.full((n, n, n), 2.0 + D))
+    c, _, _ = O.lattice()
+    for k in (1, 7, 30):
+        o.step(k - o.get_step())
+        f = o.get_state()
+        Pm = np.einsum("iz...,ia->a", f.reshape(19, -1), c.astype(float))
+        assert np.abs(Pm - np.array([0, 0, k * n ** 3 * gb * D])).max() < 1e-13
+        # and the reported velocity is the half-force corrected one: u_z = (k - 1/2) a  (the collision velocity of step k)
+        _, _, _, uz = o.get_macros()
+        assert np.abs(uz - (k - 0.5) * gb * D).max() < 1e-15
+    # cold air sinks
+    o2 = O.Oracle(n, n, n, 1e-2, 0.0, 0.0, faces=[P] * 6)
+    o2.set_flags(); o2.set_macros(); o2.set_thermal(0.02, gb, 2.0); o2.set_theta(np.full((n, n, n), 1.0))
+    o2.step(3)
+    assert o2.get_macros()[3].max() < 0
+    o.close(); o2.close()
+
+
+def test_thermal_off_leaves_flow_untouched_and_eq_faces_refused():
+    n = 8
+    a = O.Oracle(n, n, n, 1e-2, 0.1, 1e-3, faces=[P] * 6)
+    b = O.Oracle(n, n, n, 1e-2, 0.1, 1e-3, faces=[P] * 6)
+    ux, uy = _tgv(n)
+    for o in (a, b):
+        o.set_flags(); o.set_macros(None, ux, uy, None)
+    b.set_thermal(0.01, 0.0, 1.0)  # gbeta = 0: the flow must not notice
+    rng = np.random.default_rng(3)
+    b.set_theta(1.0 + 0.1 * rng.standard_normal((n, n, n)))
+    a.step(10); b.step(10)
+    assert np.array_equal(a.get_state(), b.get_state())
+    c = O.Oracle(n, n, n, 1e-2)  # default faces have EQ_FIXED / EQ_OUTFLOW
+    c.set_flags()
+    with pytest.raises(Exception):
+        c.set_thermal(0.01, 0.0, 1.0)
+    for o in (a, b, c):
+        o.close()
