@@ -160,6 +160,28 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
 #define LBM_MAX_INFLOW_MODES 1024
 int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double u_rms, double k_e, double k_eta);
 
+/* Thermal lattice with Boussinesq coupling (Table 1 "Optional D3Q7 or D3Q19 thermal
+ * lattice with Boussinesq coupling", density-current workload PAPER.md:121; DESIGN.md §4 reading 23).  A D3Q7 BGK
+ * advection-diffusion lattice (rest vector + six axis vectors, weights 1/4 and 1/8, c_sT^2 = 1/4, linear equilibrium
+ * h_eq,i = wT_i theta (1 + 4 c_i.u), tau_theta = 4 alpha + 1/2) stepped in the same kernel as the flow: each FLUID
+ * cell pulls its 7 thermal populations by the rule of the flow pull (bounce-back on walls / solids and specular
+ * reflection on FREE_SLIP faces = zero heat flux; periodic wrap), theta = sum_i h_i, the flow collision sees the
+ * acceleration F + g_beta (theta - theta_ref) e_z (+z = up), and the thermal populations relax towards h_eq(theta, u)
+ * with the velocity of that collision.  lbm_get_macros then reports the velocity corrected by the same buoyancy.
+ * lbm_set_thermal switches it on with theta = theta_ref at rest; it allocates 2 x 7 population arrays of the handle's
+ * precision (library-owned, freed by lbm_destroy).  All six faces must be PERIODIC / WALL / FREE_SLIP, and damping zones
+ * and inflow fluctuations must be off (LBM_EINVAL otherwise, also from the calls that would switch those on later).
+ * alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
+int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref);
+/* Initial thermal state H0 = h_eq(theta, u): theta, ux, uy, uz each [nz][ny][nx], host or device; NULL theta =
+ * theta_ref, NULL component = 0; SOLID cells are skipped.  Needs lbm_set_thermal and flags (else LBM_ESTATE); a new
+ * lbm_set_flags* leaves the thermal state stale until this is called again. */
+int lbm_set_theta(lbm_t *h, const float *theta, const float *ux, const float *uy, const float *uz);
+int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const double *uy, const double *uz);
+/* theta = sum_i h_i of the current state, [nz][ny][nx], host or device; SOLID cells report theta_ref.  Synchronises. */
+int lbm_get_theta(lbm_t *h, float *theta);
+int lbm_get_theta_f64(lbm_t *h, double *theta);
+
 /* Config-5 coupling, device to device, stream-ordered on dst's stream: local macros of src on the plane
  * x = src_x_plane are written as f_eq(1, u) into the EQ_FIXED cells of dst's x- face, tiling y modulo
  * src's ny; nz must match; SOLID src cells feed u = 0.  Both handles must share precision. */

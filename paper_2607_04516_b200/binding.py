@@ -28,6 +28,7 @@ SYMBOLS = [
     "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
     "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
+    "lbm_set_thermal", "lbm_set_theta", "lbm_set_theta_f64", "lbm_get_theta", "lbm_get_theta_f64",
 ]
 
 
@@ -69,6 +70,11 @@ def load_library():
     for n in ("lbm_set_macros", "lbm_set_macros_f64", "lbm_get_macros", "lbm_get_macros_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp, vp]
     lib.lbm_step.argtypes = [vp, i]
+    lib.lbm_set_thermal.argtypes = [vp, C.c_double, C.c_double, C.c_double]
+    for n in ("lbm_set_theta", "lbm_set_theta_f64"):
+        getattr(lib, n).argtypes = [vp, vp, vp, vp, vp]
+    for n in ("lbm_get_theta", "lbm_get_theta_f64"):
+        getattr(lib, n).argtypes = [vp, vp]
     lib.lbm_mean_config.argtypes = [vp, l, i]
     lib.lbm_mean_reset.argtypes = [vp]
     for n in ("lbm_get_mean", "lbm_get_mean_f64"):
@@ -265,6 +271,30 @@ class Lbm:
                 raise ValueError("fields must be [nz][ny][nx]")
         fn = self._lib.lbm_set_macros_f64 if f64 else self._lib.lbm_set_macros
         self._chk(fn(self._h, *[p for _, p in ks]), "set_macros")
+
+    # -- thermal lattice + Boussinesq coupling
+    def set_thermal(self, alpha, g_beta=0.0, theta_ref=0.0):
+        self._chk(self._lib.lbm_set_thermal(self._h, float(alpha), float(g_beta), float(theta_ref)), "set_thermal")
+
+    def set_theta(self, theta=None, ux=None, uy=None, uz=None, f64=False):
+        dt = np.float64 if f64 else np.float32
+        ks = [_ptr(a, dt) for a in (theta, ux, uy, uz)]
+        for k, _ in ks:
+            if k is not None and tuple(k.shape) != self.shape:
+                raise ValueError("fields must be [nz][ny][nx]")
+        fn = self._lib.lbm_set_theta_f64 if f64 else self._lib.lbm_set_theta
+        self._chk(fn(self._h, *[p for _, p in ks]), "set_theta")
+
+    def get_theta(self, out=None, f64=False):
+        t = self._torch
+        fn = self._lib.lbm_get_theta_f64 if f64 else self._lib.lbm_get_theta
+        if out == "host":
+            a = np.empty(self.shape, dtype=np.float64 if f64 else np.float32)
+            self._chk(fn(self._h, a.ctypes.data), "get_theta")
+            return a
+        a = out if out is not None else self._new(t.float64 if f64 else t.float32)
+        self._chk(fn(self._h, a.data_ptr()), "get_theta")
+        return a
 
     # -- the hot call
     def step(self, n=1):

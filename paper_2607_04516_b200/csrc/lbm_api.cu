@@ -3,6 +3,7 @@
 #include "lbm_core.cuh"
 #include "lbm_setup.cuh"
 #include "lbm_step.cuh"
+#include "lbm_thermal.cuh"
 #include "lbm_out.cuh"
 #include "lbm_mesh.cuh"
 
@@ -88,6 +89,9 @@ struct lbm {
     bool damp_on;   // damping zones configured (the DAMP instantiation of the step kernel runs)
     int dlo[3], dhi[3]; // the zone-free inner box
     int nmodes;     // synthetic inflow fluctuations: modes in use (0 = off)
+    bool thermal;   // D3Q7 thermal lattice + Boussinesq coupling on (lbm_set_thermal); its two buffers are library-owned
+    double alpha, gbeta, theta_ref;
+    char *th_ws;    // [2][7][stride] reals, cudaMalloc'ed by lbm_set_thermal, freed by lbm_destroy
     int loop_ok;    // multi-step cooperative launch: 0 = not probed yet, 1 = the whole grid is resident, -1 = no
     // staging buffers for HOST inputs / outputs that do not fit the scratch area (whole-lattice fields): kept between
     // calls, grown on demand, freed by lbm_destroy — a cudaMalloc + cudaFree pair per field per call costs milliseconds
@@ -106,6 +110,9 @@ struct lbm {
     double *modes() const { return (double *)(ws + L.off_modes); }
     void *damp() const { return ws + L.off_damp; }
     void *scratch() const { return ws + L.off_scratch; }
+    size_t th_half() const { return (size_t)QT * (size_t)L.stride * (fp64 ? 8 : 4); }
+    void *th_state() const { return thermal ? th_ws + (cur ? th_half() : 0) : nullptr; }
+    void *th_other() const { return thermal ? th_ws + (cur ? 0 : th_half()) : nullptr; }
     long long N() const { return (long long)nx * ny * nz; }
 };
 
@@ -152,6 +159,10 @@ Params<real> make_params(const lbm_t *h)
     P.Fx = (real)h->F[0]; P.Fy = (real)h->F[1]; P.Fz = (real)h->F[2];
     P.damp = h->damp_on ? (const real *)h->damp() : nullptr;
     for (int a = 0; a < 3; ++a) { P.dlo[a] = h->dlo[a]; P.dhi[a] = h->dhi[a]; }
+    if (h->thermal) {
+        P.gbeta = (real)h->gbeta; P.theta_ref = (real)h->theta_ref;
+        P.omega_t = (real)(1.0 / (4.0 * h->alpha + 0.5));
+    }
     return P;
 }
 
@@ -457,6 +468,15 @@ constexpr int N_VARIANTS = 11;
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
+    if (h->thermal) { // fused flow + thermal step (lbm_thermal.cuh)
+        const real *A = (const real *)h->state();
+        real *B = (real *)h->other();
+        constexpr int BLOCK = 128, MINB = std::is_same<real, float>::value ? 6 : 2; // 80 registers: 19 + 7 populations without spills
+        dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
+        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
+        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
+        return check_launch(h, "thermal_step_kernel");
+    }
     const bool turb = h->nmodes > 0 && P.F > 0;
     if (h->damp_on || turb) { // damping zones / inflow fluctuations: their own instantiations (same arithmetic elsewhere)
         if constexpr (std::is_same<real, float>::value) {
@@ -519,7 +539,7 @@ int try_step_loop(lbm_t *h, const Params<real> &P, int want)
 {
     if constexpr (!std::is_same<real, float>::value) return 0;
     else {
-        if (h->variant != 0 || h->nmodes > 0 || want < 4 || h->loop_ok < 0) return 0;
+        if (h->variant != 0 || h->nmodes > 0 || h->thermal || want < 4 || h->loop_ok < 0) return 0;
         constexpr int BLOCK = 128;
         const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
         const void *fn = h->damp_on ? (const void *)step_loop_kernel<float, BLOCK, 10, true> : (const void *)step_loop_kernel<float, BLOCK, 10, false>;
@@ -588,7 +608,8 @@ int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
     if (!rc) {
         const int B = 256;
         macros_kernel<real, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (const real *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P);
+            (const real *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
+            (const real *)h->th_state());
         rc = check_launch(h, "macros_kernel");
     }
     int rc2 = finish_out(h, o, staged);
@@ -712,7 +733,86 @@ int do_feed(lbm_t *dst, const lbm_t *src, int sx)
 
 // ---- C ABI -------------------------------------------------------------------------------------------------------------
 
+template <typename real, typename in_t>
+int do_set_theta(lbm_t *h, const in_t *theta, const in_t *ux, const in_t *uy, const in_t *uz)
+{
+    const Params<real> P = make_params<real>(h);
+    const size_t bytes = (size_t)P.N * sizeof(in_t);
+    InBuf in[4] = {};
+    const in_t *src[4] = {theta, ux, uy, uz};
+    int rc = LBM_OK;
+    for (int k = 0; k < 4 && !rc; ++k) rc = stage_in(h, src[k], bytes, h->L.scratch_bytes, &in[k]);
+    if (!rc) {
+        const int B = 256;
+        real *H0 = (real *)h->th_ws, *H1 = (real *)(h->th_ws + h->th_half());
+        thermal_init_kernel<real, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            H0, H1, h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev, (const in_t *)in[2].dev,
+            (const in_t *)in[3].dev, P);
+        rc = check_launch(h, "thermal_init_kernel");
+    }
+    release_in(h, in, 4);
+    return rc;
+}
+
+template <typename in_t>
+int set_theta_any(lbm_t *h, const in_t *theta, const in_t *ux, const in_t *uy, const in_t *uz)
+{
+    if (!h) return LBM_EINVAL;
+    if (!h->thermal) return fail(h, LBM_ESTATE, "set_theta: thermal lattice is off (lbm_set_thermal)");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_theta: flags not set");
+    return h->fp64 ? do_set_theta<double, in_t>(h, theta, ux, uy, uz) : do_set_theta<float, in_t>(h, theta, ux, uy, uz);
+}
+
+template <typename real, typename out_t>
+int do_get_theta(lbm_t *h, out_t *theta)
+{
+    const Params<real> P = make_params<real>(h);
+    OutBuf o[1];
+    int rc = stage_out(h, theta, (size_t)P.N * sizeof(out_t), &o[0]);
+    if (!rc) {
+        const int B = 256;
+        theta_out_kernel<real, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->th_state(), h->flags(), (out_t *)o[0].dev, P);
+        rc = check_launch(h, "theta_out_kernel");
+    }
+    int rc2 = finish_out(h, o, 1);
+    return rc ? rc : rc2;
+}
+
+template <typename out_t>
+int get_theta_any(lbm_t *h, out_t *theta)
+{
+    if (!h || !theta) return LBM_EINVAL;
+    if (!h->thermal) return fail(h, LBM_ESTATE, "get_theta: thermal lattice is off (lbm_set_thermal)");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_theta: flags not set");
+    return h->fp64 ? do_get_theta<double, out_t>(h, theta) : do_get_theta<float, out_t>(h, theta);
+}
+
+bool has_eq_face(const int face[6])
+{
+    for (int k = 0; k < 6; ++k)
+        if (face[k] == FACE_EQ_FIXED || face[k] == FACE_EQ_OUTFLOW) return true;
+    return false;
+}
+
 extern "C" {
+
+int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
+{
+    if (!h) return LBM_EINVAL;
+    if (!(alpha > 0.0) || !std::isfinite(alpha) || !std::isfinite(g_beta) || !std::isfinite(theta_ref))
+        return fail(h, LBM_EINVAL, "set_thermal: alpha must be > 0 and all arguments finite");
+    if (has_eq_face(h->face)) return fail(h, LBM_EINVAL, "set_thermal: EQ_FIXED / EQ_OUTFLOW faces are not supported with the thermal lattice");
+    if (h->damp_on || h->nmodes > 0) return fail(h, LBM_EINVAL, "set_thermal: not combinable with damping zones / inflow fluctuations");
+    if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half()));
+    CUDA_TRY(h, cudaMemsetAsync(h->th_ws, 0, 2 * h->th_half(), h->stream)); // theta_ref at rest (shifted storage)
+    h->alpha = alpha; h->gbeta = g_beta; h->theta_ref = theta_ref; h->thermal = true;
+    CUDA_TRY(h, cudaStreamSynchronize(h->stream));
+    return LBM_OK;
+}
+int lbm_set_theta(lbm_t *h, const float *theta, const float *ux, const float *uy, const float *uz) { return set_theta_any<float>(h, theta, ux, uy, uz); }
+int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const double *uy, const double *uz) { return set_theta_any<double>(h, theta, ux, uy, uz); }
+int lbm_get_theta(lbm_t *h, float *theta) { return get_theta_any<float>(h, theta); }
+int lbm_get_theta_f64(lbm_t *h, double *theta) { return get_theta_any<double>(h, theta); }
 
 int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int fp64, size_t *out)
 {
@@ -742,6 +842,7 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     h->stream = (cudaStream_t)cuda_stream;
     h->cur = 0; h->have_flags = false; h->step = 0;
     h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false; h->nmodes = 0; h->loop_ok = 0;
+    h->thermal = false; h->alpha = 0; h->gbeta = 0; h->theta_ref = 0; h->th_ws = nullptr;
     for (int a = 0; a < 3; ++a) { h->dlo[a] = 0; h->dhi[a] = 0; }
     for (int k = 0; k < 4; ++k) h->slots[k] = lbm::Slot{nullptr, 0, false};
     if (dev_workspace) {
@@ -770,6 +871,7 @@ int lbm_destroy(lbm_t *h)
     if (!h) return LBM_EINVAL;
     cudaStreamSynchronize(h->stream);
     if (h->own_ws) cudaFree(h->ws);
+    if (h->th_ws) cudaFree(h->th_ws);
     for (int k = 0; k < 4; ++k)
         if (h->slots[k].p) cudaFree(h->slots[k].p);
     delete h;
@@ -785,6 +887,7 @@ int lbm_set_boundaries(lbm_t *h, const int face_type[6])
         if (lo < 0 || lo > 4 || hi < 0 || hi > 4) return fail(h, LBM_EINVAL, "set_boundaries: unknown face type");
         if ((lo == LBM_PERIODIC) != (hi == LBM_PERIODIC)) return fail(h, LBM_EINVAL, "set_boundaries: PERIODIC must be set on both faces of an axis");
     }
+    if (h->thermal && has_eq_face(face_type)) return fail(h, LBM_EINVAL, "set_boundaries: EQ faces are not supported while the thermal lattice is on");
     for (int k = 0; k < 6; ++k) h->face[k] = face_type[k];
     h->have_flags = false;
     return LBM_OK;
@@ -804,6 +907,7 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
 {
     if (!h) return LBM_EINVAL;
     if (!width || !peak) return fail(h, LBM_EINVAL, "set_damping: NULL");
+    if (h->thermal) return fail(h, LBM_EINVAL, "set_damping: not combinable with the thermal lattice");
     bool any = false;
     for (int k = 0; k < 6; ++k) {
         if (width[k] < 0 || !(peak[k] >= 0.0) || peak[k] > 1.0) return fail(h, LBM_EINVAL, "set_damping: need width >= 0 and 0 <= peak <= 1");

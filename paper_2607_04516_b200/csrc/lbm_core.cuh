@@ -77,6 +77,9 @@ struct Params {
     // profile ut[3][nz];  sigma(x,y,z) = max(sx[x], sy[y], sz[z])
     const real *damp;
     int dlo[3], dhi[3]; // cells with dlo <= (x,y,z) < dhi lie outside every zone: no table look-up there
+    // thermal lattice (lbm_set_thermal, lbm_thermal.cuh): buoyancy coefficient g beta, reference theta, 1 / tau_theta;
+    // all 0 while it is off
+    real gbeta, theta_ref, omega_t;
 };
 
 // Interior x = 0 sits at padded x = XOFF = 8: every interior row starts on a 32-byte sector boundary (and ends on one

@@ -5,10 +5,18 @@
 
 namespace lbmk {
 
+// theta - theta_ref of the stored thermal state of cell p (lbm_thermal.cuh: 7 shifted populations, directions 0..6)
+template <typename real>
+__device__ __forceinline__ real stored_theta_shift(const real *__restrict__ H, long long stride, int p)
+{
+    return H[p] + ((H[stride + p] + H[2 * stride + p]) + (H[3 * stride + p] + H[4 * stride + p]) + (H[5 * stride + p] + H[6 * stride + p]));
+}
+
 // local macros of the stored state (DESIGN.md §3 step 7)
 template <typename real, typename out_t>
 __global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
-                              out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz, Params<real> P)
+                              out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz, Params<real> P,
+                              const real *__restrict__ H = nullptr)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -20,6 +28,7 @@ __global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restr
     Macro<real> m{real(1), real(0), real(0), real(0)};
     if (cls != SOLID) {
         load_cell(g, A, P.stride, p);
+        if (H) P.Fz += P.gbeta * stored_theta_shift(H, P.stride, p); // Boussinesq: the buoyancy the cell's collision used
         m = local_macros(g, cls, P, damp_at(P, x, y, z));
     }
     if (rho) rho[c] = out_t(m.rho);
@@ -30,7 +39,8 @@ __global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restr
 
 // standalone sample (a sample due at a step the fused kernel did not produce, e.g. step 0); DESIGN.md §3 step 8
 template <typename real>
-__global__ void mean_sample_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, real *__restrict__ msum, Params<real> P)
+__global__ void mean_sample_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, real *__restrict__ msum, Params<real> P,
+                                   const real *__restrict__ H = nullptr)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -41,6 +51,7 @@ __global__ void mean_sample_kernel(const real *__restrict__ A, const uint8_t *__
     if (cls == SOLID) return;
     real g[Q];
     load_cell(g, A, P.stride, p);
+    if (H) P.Fz += P.gbeta * stored_theta_shift(H, P.stride, p);
     const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
     msum[p] += m.ux;
     msum[P.stride + p] += m.uy;

@@ -270,3 +270,20 @@ def urban_mesh(height: np.ndarray, z_shift: float = 0.0) -> np.ndarray:
                 out.append(box_mesh((x, y, -1.0 + z_shift), (x1, y + 1, h + z_shift)))
             x = x1
     return np.concatenate(out) if out else np.zeros((0, 3, 3), dtype=np.float32)
+
+
+def density_current(nx: int = 256, nz: int = 64, ny: int = 2, d_theta: float = -15.0, theta_ref: float = 300.0):
+    """Synthetic stand-in for the density-current workload ("initially quiescent, neutrally stratified
+    atmosphere with a cold elliptical potential-temperature perturbation in a 25.6 km by 6.4 km domain"): a 4:1 x-z box,
+    thin and periodic in y, at rest; theta = theta_ref + d_theta (cos(pi L) + 1) / 2 inside the ellipse L <= 1 centred on
+    the domain's vertical mid-plane at 3/6.4 of the height, radii 4/25.6 of the length and 2/6.4 of the height.
+    Returns (faces, theta[nz][ny][nx] float64).  Input generation only: no arithmetic of the method."""
+    x = (np.arange(nx) + 0.5) / nx          # fractions of the 25.6 km length
+    z = (np.arange(nz) + 0.5) / nz          # fractions of the 6.4 km height
+    Lx = (x - 0.5) / (4.0 / 25.6)
+    Lz = (z - 3.0 / 6.4) / (2.0 / 6.4)
+    L = np.sqrt(Lx[None, :] ** 2 + Lz[:, None] ** 2)
+    pert = np.where(L <= 1.0, 0.5 * d_theta * (np.cos(np.pi * L) + 1.0), 0.0)
+    theta = theta_ref + np.repeat(pert[:, None, :], ny, axis=1)
+    faces = (FREE_SLIP, FREE_SLIP, PERIODIC, PERIODIC, WALL, FREE_SLIP)
+    return faces, np.ascontiguousarray(theta, dtype=np.float64)

@@ -1,0 +1,150 @@
+"""Parity of the fused flow + thermal step (lbm_set_thermal / lbm_set_theta / lbm_get_theta; SURVEY.md §8(f) rank 3,
+PAPER.md:89, :121; DESIGN.md §4 reading 23) against the CPU FP64 oracle through the C ABI.
+Bars: max-abs(rho, u, theta - theta_ref) <= 1e-5 after 100 steps (FP32), <= 2e-12 (FP64 instantiation)."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL32 = 1e-5
+TOL64 = 2e-12
+P, W, FS = 0, 1, 2
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_04516_b200 import binding, build
+    build.build()
+    return binding
+
+
+def pair(B, nx, ny, nz, faces, hm, nu0, Cs, fcor, F, alpha, gb, tref, theta, u0=None, fp64=False, want_mean=False):
+    from oracle import Oracle
+    o = Oracle(nx, ny, nz, nu0, Cs, fcor, F, faces)
+    o.set_flags(hm)
+    sim = B.Lbm(nx, ny, nz, nu0, Cs, fcor, F, faces, fp64=fp64, want_mean=want_mean)
+    sim.set_flags(hm)
+    np.testing.assert_array_equal(sim.get_flags(), o.get_flags())
+    u0 = u0 or (None, None, None)
+    o.set_macros(None, *u0)
+    sim.set_macros(None, *u0, f64=True)
+    o.set_thermal(alpha, gb, tref)
+    sim.set_thermal(alpha, gb, tref)
+    o.set_theta(theta, *u0)
+    sim.set_theta(theta, *u0, f64=True)
+    return sim, o
+
+
+def errs(sim, o, tref):
+    g = [a.cpu().numpy().astype(np.float64) for a in sim.get_macros(f64=True)]
+    r = o.get_macros()
+    e_flow = max(float(np.abs(a - b).max()) for a, b in zip(g, r))
+    th = sim.get_theta(f64=True).cpu().numpy()
+    assert np.isfinite(th).all()
+    e_th = float(np.abs(th - o.get_theta()).max())
+    return e_flow, e_th
+
+
+FACES = [(P, P, P, P, P, P), (W, FS, P, P, W, FS), (FS, FS, FS, FS, FS, FS), (W, W, W, W, W, W), (FS, W, P, P, FS, W)]
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+@pytest.mark.parametrize("faces", FACES)
+def test_thermal_parity_ragged_boxes_with_solids(B, faces, fp64):
+    rng = np.random.default_rng(11 + FACES.index(faces))
+    for nx, ny, nz in [(33, 7, 9), (70, 5, 12)]:
+        hm = np.zeros((ny, nx), np.int32)
+        hm[1:4, 5:11] = 4
+        hm[ny - 2, nx - 9:nx - 3] = 2
+        theta = 1.0 + 0.3 * rng.standard_normal((nz, ny, nx))
+        u0 = tuple(0.02 * rng.standard_normal((nz, ny, nx)) for _ in range(3))
+        sim, o = pair(B, nx, ny, nz, faces, hm, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), 0.01, 2e-3, 1.0, theta, u0, fp64=fp64)
+        sim.step(100); o.step(100)
+        e_flow, e_th = errs(sim, o, 1.0)
+        tol = TOL64 if fp64 else TOL32
+        assert e_flow <= tol and e_th <= tol, (faces, (nx, ny, nz), e_flow, e_th)
+        sim.close(); o.close()
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_density_current_parity_and_time_mean(B, fp64):
+    from paper_2607_04516_b200 import workloads as Wl
+    nx, ny, nz = 128, 2, 32
+    faces, theta = Wl.density_current(nx, nz, ny, d_theta=-15.0, theta_ref=300.0)
+    hm = np.zeros((ny, nx), np.int32)
+    sim, o = pair(B, nx, ny, nz, faces, hm, 1e-3, 0.1, 0.0, (0, 0, 0), 1e-3, 2e-5, 300.0, theta, fp64=fp64, want_mean=True)
+    sim.mean_config(50, 10); o.mean_config(50, 10)
+    sim.step(200); o.step(200)
+    e_flow, e_th = errs(sim, o, 300.0)
+    tol = TOL64 if fp64 else TOL32
+    # theta' spans 15 K: the thermal bar is relative to that span (FP32 storage is shifted by theta_ref)
+    assert e_flow <= tol and e_th <= 15.0 * tol, (e_flow, e_th)
+    gm = sim.get_mean(f64=True); om = o.get_mean()
+    assert gm[3] == om[3] == 16
+    assert max(float(np.abs(a.cpu().numpy() - b).max()) for a, b in zip(gm[:3], om[:3])) <= tol
+    # the cold pool sinks: downward motion under the blob's centre
+    uz = o.get_macros()[3]
+    assert uz[nz // 2, 0, nx // 2] < -1e-4
+    sim.close(); o.close()
+
+
+def test_heat_and_mass_conserved_on_the_gpu_fp64(B):
+    nx, ny, nz = 40, 6, 20
+    rng = np.random.default_rng(5)
+    hm = np.zeros((ny, nx), np.int32); hm[2:4, 10:18] = 7
+    theta = 2.0 + 0.5 * rng.standard_normal((nz, ny, nx))
+    sim, o = pair(B, nx, ny, nz, (W, FS, P, P, W, FS), hm, 5e-3, 0.1, 1e-3, (0, 0, 0), 0.02, 1e-3, 2.0, theta, fp64=True)
+    fluid = sim.get_flags() == 0
+    s0 = sim.get_theta(f64=True).cpu().numpy()[fluid].sum()
+    sim.step(300)
+    s1 = sim.get_theta(f64=True).cpu().numpy()[fluid].sum()
+    assert abs(s1 - s0) <= 1e-12 * abs(s0)
+    rho = sim.get_macros(f64=True)[0].cpu().numpy()
+    assert abs(rho[fluid].sum() - fluid.sum()) <= 1e-11 * fluid.sum()
+    sim.close(); o.close()
+
+
+def test_zero_buoyancy_leaves_the_flow_unchanged(B):
+    # g_beta = 0: the fused kernel's flow half is the plain step's arithmetic; the two instantiations may contract
+    # multiply-adds differently around the (now per-cell) F_z, so equal up to FP32 rounding order, not bit for bit
+    nx, ny, nz = 48, 9, 10
+    rng = np.random.default_rng(6)
+    hm = np.zeros((ny, nx), np.int32); hm[3:6, 12:20] = 5
+    u0 = tuple(0.02 * rng.standard_normal((nz, ny, nx)) for _ in range(3))
+    faces = (P, P, FS, FS, W, FS)
+    a = B.Lbm(nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), faces, want_mean=False)
+    b = B.Lbm(nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), faces, want_mean=False)
+    for s in (a, b):
+        s.set_flags(hm); s.set_macros(None, *u0, f64=True)
+    b.set_thermal(0.01, 0.0, 1.0)
+    b.set_theta(1.0 + 0.1 * rng.standard_normal((nz, ny, nx)), f64=True)
+    a.step(37); b.step(37)
+    assert float(np.abs(a.get_state(out="host") - b.get_state(out="host")).max()) <= 1e-7
+    a.close(); b.close()
+
+
+def test_thermal_error_behaviour(B):
+    sim = B.Lbm(8, 8, 8, 1e-2)  # default faces carry EQ_FIXED / EQ_OUTFLOW
+    sim.set_flags(np.zeros((8, 8), np.int32))
+    with pytest.raises(B.LbmError):
+        sim.get_theta()
+    with pytest.raises(B.LbmError):
+        sim.set_thermal(0.01, 0.0, 1.0)
+    sim.set_boundaries([P] * 6)
+    with pytest.raises(B.LbmError):
+        sim.set_thermal(0.0, 0.0, 1.0)  # alpha must be > 0
+    sim.set_thermal(0.01, 1e-3, 1.0)
+    with pytest.raises(B.LbmError):
+        sim.set_theta()  # flags were invalidated by set_boundaries
+    with pytest.raises(B.LbmError):
+        sim.set_boundaries([3, 4, 0, 0, 1, 2])
+    with pytest.raises(B.LbmError):
+        sim.set_damping([0, 0, 0, 0, 0, 4], [0, 0, 0, 0, 0, 0.1])
+    sim.set_flags(np.zeros((8, 8), np.int32))
+    sim.set_macros(); sim.set_theta()
+    sim.step(3)
+    assert float(np.abs(sim.get_theta().cpu().numpy() - 1.0).max()) == 0.0  # isothermal rest state is exact
+    sim.close()
