@@ -13,6 +13,7 @@
 // Traffic per FLUID cell: (19 + 7) x 4 B read + (19 + 7) x 4 B write + 1 flag byte = 209 B.
 #pragma once
 #include "lbm_core.cuh"
+#include "lbm_step.cuh"
 
 namespace lbmk {
 
@@ -74,11 +75,51 @@ thermal_step_kernel(const real *__restrict__ A, real *__restrict__ B, const real
 {
     const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x;
     if (c2 >= (unsigned)P.nxy) return;
-    const int y = (int)(c2 / (unsigned)P.nx);
+    const int y = P.nx_magic ? (int)__umulhi(c2, P.nx_magic) : (int)(c2 / (unsigned)P.nx);
     const int x = (int)c2 - y * P.nx;
     const int z = blockIdx.y;
     const int p = pidx(P, x, y, z);
-    const uint8_t fl = flags[p];
+    // as in step_kernel's SPEC instantiations: all 26 pulls are issued before the flag byte has arrived (no dependent
+    // round trip; a SOLID cell then costs its reads), pinned by volatile asm so that the flag test cannot move above them
+    real g[Q], t[QT];
+    static_for<0, Q>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        g[i] = ld_pinned(A + ((long long)i * P.stride + (p - poff<i>(P))));
+    });
+    static_for<0, QT>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        t[i] = ld_pinned(HA + ((long long)i * P.stride + (p - poff<i>(P))));
+    });
+    const uint8_t fl = ld_pinned(flags + p);
+    // the collision pair of one FLUID cell: buoyancy from the pulled theta into the flow collision, thermal BGK towards
+    // h_eq(theta, u) of that collision's velocity
+    auto collide_both = [&]() {
+        const real dth = theta_shift(t);
+        const Macro<real> m = collide(g, with_buoyancy(P, dth));
+        real e[QT];
+        thermal_equilibrium(e, dth, P.theta_ref, m.ux, m.uy, m.uz);
+#pragma unroll
+        for (int i = 0; i < QT; ++i) t[i] = t[i] - P.omega_t * (t[i] - e[i]);
+        return m;
+    };
+    // fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, nothing to complete)
+    if (__all_sync(__activemask(), fl == 0)) {
+        const Macro<real> m = collide_both();
+        static_for<0, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            B[(long long)i * P.stride + p] = g[i];
+        });
+        static_for<0, QT>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            HB[(long long)i * P.stride + p] = t[i];
+        });
+        if constexpr (MEAN) {
+            msum[p] += m.ux;
+            msum[P.stride + p] += m.uy;
+            msum[2 * P.stride + p] += m.uz;
+        }
+        return;
+    }
     const int cls = fl & CLASS_MASK;
     uint32_t lk = 0;
     if (fl & (SLOW_BIT | SURF_BIT)) lk = links[p];
@@ -96,21 +137,7 @@ thermal_step_kernel(const real *__restrict__ A, real *__restrict__ B, const real
         return;
     }
     if (cls != FLUID) return; // no EQ cells while the thermal lattice is on (lbm_set_thermal refuses EQ faces)
-    real g[Q], t[QT];
-    static_for<0, Q>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        g[i] = A[(long long)i * P.stride + (p - poff<i>(P))];
-    });
-    static_for<0, QT>([&](auto ic) {
-        constexpr int i = decltype(ic)::value;
-        t[i] = HA[(long long)i * P.stride + (p - poff<i>(P))];
-    });
-    const real dth = theta_shift(t);
-    const Macro<real> m = collide(g, with_buoyancy(P, dth));
-    real e[QT];
-    thermal_equilibrium(e, dth, P.theta_ref, m.ux, m.uy, m.uz);
-#pragma unroll
-    for (int i = 0; i < QT; ++i) t[i] = t[i] - P.omega_t * (t[i] - e[i]);
+    const Macro<real> m = collide_both();
     store_cell(B, P, p, x, y, z, fl, lk, g);
     store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
     if constexpr (MEAN) {
