@@ -34,6 +34,7 @@ WORKLOADS = {
     "c2": "C2 periodic Taylor-Green + Coriolis 128^3, Cs 0.1 (BASELINE.json configs[1])",
     "c3": "C3 urban 400x400x100 (BASELINE.json configs[2]): seeded heightmap plan fraction 0.35, log-law inlet, nu0 1e-4, Cs 0.1, f 2.9e-6",
     "c4": "C4 refined urban 800x800x200, veering inlet on three faces (BASELINE.json configs[3])",
+    "thermal": "closed 400x400x100 city box with the D3Q7 thermal lattice + Boussinesq coupling on (DESIGN.md reading 23): 209 B/cell",
     "c5": "C5 chain: periodic precursor 256x256x200 feeding the x- inlet of the 1200x1200x200 urban domain every step (BASELINE.json configs[4])",
 }
 
@@ -46,7 +47,8 @@ class Job:
         if name == "c5":
             self.wls = [W.config5_precursor(), W.config5_main()]
         else:
-            self.wls = [{"c1": W.config1, "c2": lambda: W.config2(Cs=0.1), "c3": W.config3, "c4": W.config4}[name]()]
+            self.wls = [{"c1": W.config1, "c2": lambda: W.config2(Cs=0.1), "c3": W.config3, "c4": W.config4,
+                         "thermal": W.thermal_city}[name]()]
         self.cells = sum(w.cells for w in self.wls)
         self.sims = [binding.from_workload(w, want_mean=False, device=device) for w in self.wls]
 
@@ -71,6 +73,7 @@ class Job:
             prof = None if w.inlet_profile is None else tuple(None if a is None else pin(a) for a in w.inlet_profile)
             init = None if w.init is None else tuple(None if a is None else pin(a) for a in w.init)
             out.append((pin(w.height), prof, init))
+        self.theta_host = [None if w.extra.get("theta") is None else pin(w.extra["theta"]) for w in self.wls]
         return out
 
     @staticmethod
@@ -86,6 +89,9 @@ class Job:
             if prof is not None:
                 s.set_inlet_profile(*prof)
             s.set_macros(*(init if init is not None else (None, None, None, None)))
+        for s, th in zip(self.sims, getattr(self, "theta_host", [])):
+            if th is not None:
+                s.set_theta(th)  # thermal workload: the flags were re-set, so the thermal state is re-initialised too
 
 
 def load_peak():
@@ -319,6 +325,8 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = load_peak()
         per_launch_s = ms_total * 1e-3 / K
+        # thermal workload: (19 + 7) x 4 B loads + (19 + 7) x 4 B stores + 1 flag byte (lbm_thermal.cuh)
+        BYTES_PER_CELL = 209 if args.workload == "thermal" else globals()["BYTES_PER_CELL"]
         achieved = BYTES_PER_CELL * cells / per_launch_s / 1e9
         line = {
             "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": Wm,

@@ -396,4 +396,7 @@ def from_workload(wl, fp64=False, want_mean=True, device="cuda:0") -> Lbm:
         sim.set_macros(*wl.init)
     else:
         sim.set_macros()
+    if wl.extra.get("thermal") is not None:
+        sim.set_thermal(*wl.extra["thermal"])
+        sim.set_theta(wl.extra.get("theta"))
     return sim

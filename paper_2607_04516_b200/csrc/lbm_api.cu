@@ -471,10 +471,22 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
     if (h->thermal) { // fused flow + thermal step (lbm_thermal.cuh)
         const real *A = (const real *)h->state();
         real *B = (real *)h->other();
-        constexpr int BLOCK = 128, MINB = std::is_same<real, float>::value ? 6 : 2; // 80 registers: 19 + 7 populations without spills
-        dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
-        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
-        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
+        dim3 grid(blocks_for((long long)P.nxy, 128), (unsigned)P.nz);
+        auto go = [&](auto minb) {
+            constexpr int BLOCK = 128, MINB = decltype(minb)::value;
+            if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
+            else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
+        };
+        if constexpr (std::is_same<real, float>::value) {
+            // 19 + 7 populations: 72 registers hold them without spills = 7 CTAs per SM (measured 24 900 MLUPS; 6 CTAs / 80
+            // registers 24 000, 5 CTAs 22 600, 8 CTAs / 64 registers with 16 B of spills 24 900); lbm_set_variant 1..3 = 5 / 6 / 8
+            switch (h->variant) {
+            case 1: go(std::integral_constant<int, 5>{}); break;
+            case 2: go(std::integral_constant<int, 6>{}); break;
+            case 3: go(std::integral_constant<int, 8>{}); break;
+            default: go(std::integral_constant<int, 7>{}); break;
+            }
+        } else go(std::integral_constant<int, 2>{});
         return check_launch(h, "thermal_step_kernel");
     }
     const bool turb = h->nmodes > 0 && P.F > 0;

@@ -287,3 +287,15 @@ def density_current(nx: int = 256, nz: int = 64, ny: int = 2, d_theta: float = -
     theta = theta_ref + np.repeat(pert[:, None, :], ny, axis=1)
     faces = (FREE_SLIP, FREE_SLIP, PERIODIC, PERIODIC, WALL, FREE_SLIP)
     return faces, np.ascontiguousarray(theta, dtype=np.float64)
+
+
+def thermal_city(nx: int = 400, ny: int = 400, nz: int = 100, seed: int = 7) -> Workload:
+    """Timing / full-size parity workload of the thermal path: config 3's city in a CLOSED box (free-slip sides and top, WALL
+    ground — the thermal lattice takes no open faces), at rest, theta = 300 + seeded N(0, 1) K, buoyancy on.
+    extra["thermal"] = (alpha, g_beta, theta_ref); extra["theta"] = the initial field (float32)."""
+    c3 = config3(nx, ny, nz)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    theta = (300.0 + rng.standard_normal((nz, ny, nx))).astype(np.float32)
+    return Workload("thermal_city", nx, ny, nz, c3.nu0, c3.Cs, c3.f_cor, (1e-6, 0.0, 0.0),
+                    (FREE_SLIP, FREE_SLIP, FREE_SLIP, FREE_SLIP, WALL, FREE_SLIP), 1000, c3.height,
+                    extra={"thermal": (1e-3, 1e-5, 300.0), "theta": theta})

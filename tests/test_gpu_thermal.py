@@ -148,3 +148,29 @@ def test_thermal_error_behaviour(B):
     sim.step(3)
     assert float(np.abs(sim.get_theta().cpu().numpy() - 1.0).max()) == 0.0  # isothermal rest state is exact
     sim.close()
+
+
+def test_thermal_full_size_city_box_parity_and_conservation(B):
+    """The launch configuration `bench.py --workload thermal` times: closed 400x400x100 city box (config 3's heightmap),
+    theta = 300 + N(0,1) K, buoyancy on.  Whole-field parity against the oracle after 30 steps, and heat conservation."""
+    from paper_2607_04516_b200 import workloads as Wl
+    from oracle import Oracle
+    wl = Wl.thermal_city()
+    alpha, gb, tref = wl.extra["thermal"]
+    theta = wl.extra["theta"]
+    sim = B.from_workload(wl, want_mean=False)
+    o = Oracle(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces)
+    o.set_flags(wl.height)
+    o.set_macros()
+    o.set_thermal(alpha, gb, tref)
+    o.set_theta(theta.astype(np.float64))
+    fluid = sim.get_flags() == 0
+    np.testing.assert_array_equal(sim.get_flags(), o.get_flags())
+    s0 = float((sim.get_theta(f64=True).cpu().numpy() - tref)[fluid].sum())
+    sim.step(30); o.step(30)
+    e_flow, e_th = errs(sim, o, tref)
+    assert e_flow <= TOL32 and e_th <= TOL32, (e_flow, e_th)
+    th = sim.get_theta(f64=True).cpu().numpy() - tref
+    # sum of theta' over 1.56e7 fluid cells of O(1) K each: FP32 rounding of the stored populations only
+    assert abs(float(th[fluid].sum()) - s0) <= 1e-6 * float(np.abs(th[fluid]).sum())
+    sim.close(); o.close()
