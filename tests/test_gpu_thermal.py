@@ -174,3 +174,20 @@ def test_thermal_full_size_city_box_parity_and_conservation(B):
     # sum of theta' over 1.56e7 fluid cells of O(1) K each: FP32 rounding of the stored populations only
     assert abs(float(th[fluid].sum()) - s0) <= 1e-6 * float(np.abs(th[fluid]).sum())
     sim.close(); o.close()
+
+
+@pytest.mark.parametrize("faces", [(P, P, P, P, P, P), (W, FS, P, P, W, FS), (FS, FS, W, W, FS, FS)])
+def test_thermal_parity_degenerate_boxes(B, faces):
+    # boxes one cell thick along one or two axes (every pull wraps / reflects / bounces onto the cell itself)
+    rng = np.random.default_rng(21)
+    for nx, ny, nz in [(1, 1, 3), (5, 1, 1), (1, 4, 1), (6, 5, 4), (32, 1, 2)]:
+        hm = np.zeros((ny, nx), np.int32)
+        if nx >= 5 and nz >= 2:
+            hm[0, 2] = 1
+        theta = 1.0 + 0.3 * rng.standard_normal((nz, ny, nx))
+        u0 = tuple(0.02 * rng.standard_normal((nz, ny, nx)) for _ in range(3))
+        sim, o = pair(B, nx, ny, nz, faces, hm, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), 0.01, 2e-3, 1.0, theta, u0, fp64=True)
+        sim.step(40); o.step(40)
+        e_flow, e_th = errs(sim, o, 1.0)
+        assert e_flow <= TOL64 and e_th <= TOL64, (faces, (nx, ny, nz), e_flow, e_th)
+        sim.close(); o.close()
