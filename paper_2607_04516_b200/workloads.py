@@ -299,3 +299,39 @@ def thermal_city(nx: int = 400, ny: int = 400, nz: int = 100, seed: int = 7) -> 
     return Workload("thermal_city", nx, ny, nz, c3.nu0, c3.Cs, c3.f_cor, (1e-6, 0.0, 0.0),
                     (FREE_SLIP, FREE_SLIP, FREE_SLIP, FREE_SLIP, WALL, FREE_SLIP), 1000, c3.height,
                     extra={"thermal": (1e-3, 1e-5, 300.0), "theta": theta})
+
+
+def density_current_benchmark(dx_m: float = 100.0, u_lat: float = 0.1):
+    """The density-current benchmark of PAPER.md:121-125 in lattice units (input generation and unit conversion only).
+
+    Physical set-up as the paper describes it: quiescent neutral atmosphere, 25.6 km x 6.4 km (x >= 0 half of the symmetric
+    problem: the x- face is the symmetry plane), cold elliptical perturbation theta' = -15 (cos(pi L) + 1) / 2 K for L <= 1
+    centred at (0, 3 km) with radii (4 km, 2 km), constant kinematic viscosity and diffusivity 75 m^2/s (the "AV75"
+    configuration), g = 9.81 m/s^2, theta_0 = 300 K, free-slip box.  Lattice scaling: dx = dx_m, dt chosen so that 35 m/s
+    (the flow's peak speed) maps to u_lat.  The thermal lattice carries the PERTURBATION (theta_ref = 0): it transports theta
+    conservatively, so an absolute 300 K would turn the O(1e-3) density waves of the weakly compressible flow into O(1 K) noise.
+    Returns dict(nx, ny, nz, faces, nu, alpha, g_beta, theta_ref, theta[nz][1][nx] float64, dt, dx, x_m[nx])."""
+    nx, nz = int(round(25600.0 / dx_m)), int(round(6400.0 / dx_m))
+    dt = dx_m * u_lat / 35.0
+    nu = 75.0 * dt / dx_m ** 2
+    g_beta = 9.81 / 300.0 * dt * dt / dx_m
+    x = (np.arange(nx) + 0.5) * dx_m
+    z = (np.arange(nz) + 0.5) * dx_m
+    L = np.sqrt((x[None, :] / 4000.0) ** 2 + ((z[:, None] - 3000.0) / 2000.0) ** 2)
+    pert = np.where(L <= 1.0, -7.5 * (np.cos(np.pi * L) + 1.0), 0.0)
+    return dict(nx=nx, ny=1, nz=nz, faces=(FREE_SLIP, FREE_SLIP, PERIODIC, PERIODIC, FREE_SLIP, FREE_SLIP), nu=nu, alpha=nu,
+                g_beta=g_beta, theta_ref=0.0, theta=np.ascontiguousarray(pert[:, None, :]), dt=dt, dx=dx_m, x_m=x)
+
+
+def front_position_km(theta_pert: np.ndarray, x_m: np.ndarray, level: float = -1.0) -> float:
+    """Front of a cold pool: the largest x where min_z theta' crosses `level` (linear interpolation between columns).
+    theta_pert is [nz][nx].  A diagnostic on outputs (no arithmetic of the method)."""
+    prof = np.asarray(theta_pert, dtype=np.float64).min(axis=0)
+    cols = np.where(prof <= level)[0]
+    if cols.size == 0:
+        return float("nan")
+    i = int(cols.max())
+    xf = x_m[i]
+    if i + 1 < len(x_m) and prof[i + 1] > level:
+        xf = x_m[i] + (x_m[i + 1] - x_m[i]) * (prof[i] - level) / (prof[i] - prof[i + 1])
+    return float(xf) / 1000.0

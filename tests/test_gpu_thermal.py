@@ -191,3 +191,50 @@ def test_thermal_parity_degenerate_boxes(B, faces):
         e_flow, e_th = errs(sim, o, 1.0)
         assert e_flow <= TOL64 and e_th <= TOL64, (faces, (nx, ny, nz), e_flow, e_th)
         sim.close(); o.close()
+
+
+def _paper_fronts():
+    import os
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "density_current_fronts.txt"))
+            if l.strip() and not l.startswith("#")]
+    return [(int(r[0]), float(r[1]), float(r[2])) for r in rows]
+
+
+def _gpu_fronts(B, dx):
+    from paper_2607_04516_b200 import workloads as Wl
+    b = Wl.density_current_benchmark(dx, 0.1)
+    sim = B.Lbm(b["nx"], b["ny"], b["nz"], b["nu"], 0.0, 0.0, (0, 0, 0), b["faces"], want_mean=False)
+    sim.set_flags(np.zeros((b["ny"], b["nx"]), np.int32))
+    sim.set_macros()
+    sim.set_thermal(b["alpha"], b["g_beta"], b["theta_ref"])
+    sim.set_theta(b["theta"], f64=True)
+    got = {}
+    for T, _, _ in _paper_fronts():
+        sim.step(int(round(T / b["dt"])) - sim.get_step())
+        got[T] = Wl.front_position_km(sim.get_theta(f64=True).cpu().numpy()[:, 0, :], b["x_m"])
+    sim.close()
+    return b, got
+
+
+def test_density_current_fronts_gpu_vs_oracle_at_100m(B):
+    """The benchmark of PAPER.md:121-125 through the C ABI in FP32, 3150 steps: front positions equal the oracle's to 0.5 %
+    (a laminar AV75 run: no chaotic divergence) and the paper's printed ones within 8 %."""
+    from oracle import Oracle
+    from paper_2607_04516_b200 import workloads as Wl
+    b, got = _gpu_fronts(B, 100.0)
+    o = Oracle(b["nx"], b["ny"], b["nz"], b["nu"], 0.0, 0.0, (0, 0, 0), b["faces"])
+    o.set_flags(); o.set_macros(); o.set_thermal(b["alpha"], b["g_beta"], b["theta_ref"]); o.set_theta(b["theta"])
+    for T, ref, plat in _paper_fronts():
+        o.step(int(round(T / b["dt"])) - o.get_step())
+        xo = Wl.front_position_km(o.get_theta()[:, 0, :], b["x_m"])
+        assert abs(got[T] / xo - 1.0) < 5e-3, (T, got[T], xo)
+        assert abs(got[T] / ref - 1.0) < 0.08 and abs(got[T] / plat - 1.0) < 0.08, (T, got[T], ref, plat)
+    o.close()
+
+
+def test_density_current_fronts_gpu_at_25m_against_the_papers_printed_values(B):
+    """The paper's coarser comparison grid (25 m): 1024 x 256 cells, 12 600 steps on the GPU path."""
+    b, got = _gpu_fronts(B, 25.0)
+    for T, ref, plat in _paper_fronts():
+        assert abs(got[T] / ref - 1.0) < 0.08 and abs(got[T] / plat - 1.0) < 0.08, (T, got[T], ref, plat)
+    print("density current 25 m fronts (km):", got)
