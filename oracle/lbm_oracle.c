@@ -23,6 +23,11 @@
  * Pins: tests/test_oracle_*.py (closed forms, invariants, brute force) — see
  * DESIGN.md "Oracle pins".  Parity unpinned: the urban LES statistics of
  * configs 3-5 (no closed form exists; SURVEY.md §8(c) last row).
+ * The optional thermal lattice + Boussinesq coupling (heq(),
+ * oracle_set_thermal / _set_theta / _get_theta and the thermal branch of
+ * oracle_step; reading 23) is pinned by tests/test_oracle_thermal.py:
+ * closed forms and the density-current front positions the paper prints
+ * (tests/golden/density_current_fronts.txt).
  */
 #include <math.h>
 #include <stdint.h>
