@@ -315,11 +315,11 @@ def run_ours(args):
         wall = time.perf_counter() - t0
         t_job = max_over_ranks(max(e0.elapsed_time(e1) * 1e-3, wall), world, dev)
         e2e_s = t_job if e2e_s is None else min(e2e_s, t_job)
-    h2d = Job.nbytes(host)
+    h2d = Job.nbytes(host) + sum(t.nbytes for t in getattr(job_, "theta_host", []) if t is not None)  # + the thermal field
     d2h = sum(o.numel() * 4 for o in outs)
     e2e = {"value": job_mlups(cells, K, world, e2e_s), "unit": "MLUPS", "h2d_bytes_per_step": h2d / K,
            "d2h_bytes_per_step": d2h / K,
-           "what": f"one job = set_flags + set_inlet_profile + set_macros from pinned host buffers, lbm_step({K}), "
+           "what": f"one job = set_flags + set_inlet_profile + set_macros{' + set_theta' if args.workload == 'thermal' else ''} from pinned host buffers, lbm_step({K}), "
                    "lbm_get_macros into pinned host buffers; best of 2 jobs"}
 
     if rank == 0:
