@@ -104,12 +104,12 @@ def load_peak():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def load_traffic():
+def load_traffic(kernel="step"):
     """DRAM bytes per launch of the step kernel (dram__bytes_read.sum + dram__bytes_write.sum of the committed
-    `ncu --set full` capture): last data row of the newest profiles/r*_step_kernel_traffic.csv; None if absent."""
+    `ncu --set full` capture): last data row of the newest profiles/r*_<kernel>_kernel_traffic.csv; None if absent."""
     import csv
     import glob
-    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "r*_step_kernel_traffic.csv")))
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{kernel}_kernel_traffic.csv")))
     if not files:
         return None
     try:
@@ -340,7 +340,8 @@ def run_ours(args):
                        "best_of": reps,
                        "state_finite": finite},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": load_traffic() if args.workload == "c3" else None, "peak_source": peak_src,
+                         "traffic": (load_traffic("step") if args.workload == "c3" else
+                                     load_traffic("thermal") if args.workload == "thermal" else None), "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": BYTES_PER_CELL * cells,
                          "frac_of_nominal_8000": achieved / 8000.0},
             "e2e": e2e, "gpu_launches": int(launches), "clocks": clocks,
