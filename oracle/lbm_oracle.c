@@ -651,7 +651,7 @@ int oracle_set_macros(oracle_t *o, const double *rho, const double *ux, const do
 }
 
 /* which face's normal an EQ_OUTFLOW cell uses: the first EQ_OUTFLOW face it
- * lies on, in the order x-,x+,y-,y+,z-,z+ (reading R-outflow-edge) */
+ * lies on, in the order x-,x+,y-,y+,z-,z+ (DESIGN.md §4 reading 24) */
 static int outflow_face(const oracle_t *o, int x, int y, int z)
 {
     int on[6] = {x == 0, x == o->nx - 1, y == 0, y == o->ny - 1, z == 0, z == o->nz - 1};
@@ -742,7 +742,11 @@ int oracle_step(oracle_t *o, int nsteps)
                         for (int i = 0; i < Q; ++i) {
                             long s = 0; int j = 0;
                             int r = resolve(o, x, y, z, i, &s, &j);
-                            if (r < 0) { bad = 1; r = 1; }
+                            if (r < 0) {
+#pragma omp atomic write
+                                bad = 1;
+                                r = 1;
+                            }
                             f[i] = r ? o->G[cell * Q + opposite(i)] : o->G[s * Q + j];
                         }
                         double ut[3] = {0, 0, 0};
@@ -758,7 +762,11 @@ int oracle_step(oracle_t *o, int nsteps)
                             for (int i = 0; i < QT; ++i) {
                                 long s = 0; int j = 0;
                                 int r = resolve(o, x, y, z, i, &s, &j);
-                                if (r < 0) { bad = 1; r = 1; }
+                                if (r < 0) {
+#pragma omp atomic write
+                                    bad = 1;
+                                    r = 1;
+                                }
                                 h[i] = r ? o->H[cell * QT + opposite(i)] : o->H[s * QT + j];
                                 theta += h[i];
                             }

@@ -327,3 +327,43 @@ def test_time_mean_accumulates_the_local_macros():
     assert n == cnt == 4
     np.testing.assert_allclose(np.stack([mx, my, mz]), acc / cnt, atol=1e-16)
     assert np.all(mx[o.get_flags() == 1] == 0)
+
+
+def test_outflow_cell_on_two_outflow_faces_uses_the_first_face_in_order():
+    """DESIGN.md §4 reading 24 (outflow-edge owner): a cell on two EQ_OUTFLOW faces copies the velocity of its inward
+    neighbour across the FIRST such face in the order x-, x+, y-, y+, z-, z+.  Faces (EQ_FIXED, EQ_OUTFLOW, FREE_SLIP,
+    EQ_OUTFLOW, WALL, FREE_SLIP): the edge x = nx-1, y = ny-1 lies on x+ and y+; its neighbours across x+ and across y+
+    hold different velocities, so the neighbour used is identified by brute force over all six candidates."""
+    import oracle as O
+    nx, ny, nz = 7, 6, 5
+    faces = (3, 4, 2, 4, 1, 2)
+    o = O.Oracle(nx, ny, nz, 1e-2, 0.0, 0.0, (0, 0, 0), faces)
+    o.set_flags(None)
+    rng = np.random.default_rng(5)
+    o.set_inlet_profile(np.full(nz, 0.03))
+    u0 = [0.02 + 0.01 * rng.random((nz, ny, nx)) for _ in range(3)]
+    o.set_macros(None, *u0)
+    cls = o.get_flags()
+    assert cls[2, ny - 1, nx - 1] == 3 and cls[2, ny - 1, 3] == 3 and cls[2, 2, nx - 1] == 3
+    before = o.get_macros()
+    o.step(1)
+    r, ux, uy, uz = o.get_macros()
+    steps = {0: (1, 0, 0), 1: (-1, 0, 0), 2: (0, 1, 0), 3: (0, -1, 0), 4: (0, 0, 1), 5: (0, 0, -1)}  # x - n per face
+    used = {}
+    for z in range(nz):
+        for (y, x) in [(ny - 1, nx - 1), (ny - 1, 3), (2, nx - 1)]:
+            assert r[z, y, x] == pytest.approx(1.0, abs=1e-15)
+            got = np.array([ux[z, y, x], uy[z, y, x], uz[z, y, x]])
+            match = []
+            for k, (dx, dy, dz) in steps.items():
+                xs, ys, zs = x + dx, y + dy, z + dz
+                if 0 <= xs < nx and 0 <= ys < ny and 0 <= zs < nz:
+                    cand = np.array([before[1][zs, ys, xs], before[2][zs, ys, xs], before[3][zs, ys, xs]])
+                    if np.abs(cand - got).max() < 1e-15:
+                        match.append(k)
+            assert len(match) == 1, (z, y, x, match)
+            used[(y, x)] = match[0]
+    assert used[(ny - 1, nx - 1)] == 1      # edge cell: x+ comes before y+
+    assert used[(ny - 1, 3)] == 3           # y+ face proper
+    assert used[(2, nx - 1)] == 1           # x+ face proper
+    o.close()

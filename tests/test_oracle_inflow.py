@@ -158,3 +158,30 @@ def test_fluctuations_enter_the_flow_and_mass_flux_stays_bounded(O):
     assert np.isfinite(ux).all() and np.abs(r - 1).max() < 0.05
     assert np.abs(uz[:, :, 3]).max() > 1e-4 and np.abs(uy[:, :, 3]).max() > 1e-4
     o.close()
+
+
+def test_active_inflow_threshold_is_1e7_strict_and_in_lattice_units(O):
+    """DESIGN.md §4 reading 21: a cell is an 'active inflow cell' iff ub.n < -1e-7 (n outward, lattice units).  One x-
+    face whose cells carry different mean normal components straddling the constant: +5e-8 and +9.9e-8 (inward by less
+    than the threshold) and exactly 1e-7 (strict '<') keep the mean EXACTLY; 1.01e-7 and 2e-7 fluctuate.  The same
+    magnitudes with the opposite sign (outflow through x-) never fluctuate.  A typo in the constant (1e-6, 1e-8), a
+    '<=' or a dropped sign fails here."""
+    from paper_2607_04516_b200 import workloads as W
+    nx, ny, nz = 6, 10, 4
+    o = O.Oracle(nx, ny, nz, 1e-2, 0.0, 0.0, (0, 0, 0), (3, 4, 0, 0, 2, 2))
+    o.set_flags(None)
+    un = np.array([5e-8, 9.9e-8, 1e-7, 1.01e-7, 2e-7, -5e-8, -1e-7, -1.01e-7, -2e-7, 1e-6])   # u_x per y; x- face: ub.n = -u_x
+    plane = np.zeros((3, nz, ny))
+    plane[0] = un[None, :]
+    plane[1] = 0.01                                     # a tangential part: must not enter the test
+    o.set_inlet_plane(0, plane)
+    o.set_macros()
+    o.set_inflow_turbulence(W.inflow_modes(8, 21, 0.2, 2.0), 0.01, 0.5)
+    active = np.array([False, False, False, True, True, False, False, False, False, True])
+    for _ in range(3):
+        r, ux, uy, uz = o.get_macros()
+        dev = np.sqrt((ux[:, :, 0] - un[None, :]) ** 2 + (uy[:, :, 0] - 0.01) ** 2 + uz[:, :, 0] ** 2)
+        assert dev[:, ~active].max() < 1e-15, "a cell below the threshold must keep its mean (up to the rounding of the moment sums)"
+        assert dev[:, active].min() > 1e-4, "a cell above the threshold must fluctuate"
+        o.step(1)
+    o.close()

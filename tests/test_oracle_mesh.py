@@ -158,3 +158,70 @@ def test_extruded_footprints_equal_the_heightmap_voxeliser_and_merge_with_terrai
 def test_vertices_outside_the_allowed_range_are_refused(MV, W):
     with pytest.raises(ValueError):
         MV.voxelise(W.box_mesh((0, 0, 0), (3000, 2, 2)), 4, 4, 4)
+
+
+# ---- the plain definition, cell by cell (DESIGN.md §4 reading 22) -----------------------------------------
+# For every cell and every ray direction: count the triangles the ray through the cell centre crosses at or before the
+# centre, with exact rational arithmetic.  No toggle array, no prefix sum, no floor division — none of the decomposition
+# oracle/mesh_voxel.py (and the CUDA kernel) use — so a misconception shared by those two cannot pass here.
+
+def plain_parities(MV, tri, nx, ny, nz):
+    from fractions import Fraction as Fr
+    v = [[[Fr(int(c), 256) for c in p] for p in t] for t in MV.snap(tri)]      # the snapped vertices, exact
+    out = np.zeros((3, nz, ny, nx), dtype=np.uint8)
+    for d in range(3):
+        au, av, aw = (d + 1) % 3, (d + 2) % 3, d
+        for z in range(nz):
+            for y in range(ny):
+                for x in range(nx):
+                    ctr = (Fr(2 * x + 1, 2), Fr(2 * y + 1, 2), Fr(2 * z + 1, 2))
+                    pu, pv, pw = ctr[au], ctr[av], ctr[aw]
+                    crossings = 0
+                    for a, b, c in v:
+                        area = (b[au] - a[au]) * (c[av] - a[av]) - (b[av] - a[av]) * (c[au] - a[au])
+                        if area == 0:
+                            continue                                            # the ray lies in the triangle's plane
+                        if area < 0:
+                            b, c = c, b
+                            area = -area                                        # counter-clockwise projection
+                        lam = []
+                        inside = True
+                        for p, q in ((b, c), (c, a), (a, b)):                   # barycentric weight of a, b, c
+                            du, dv = q[au] - p[au], q[av] - p[av]
+                            e = du * (pv - p[av]) - dv * (pu - p[au])
+                            if e < 0 or (e == 0 and not (dv < 0 or (dv == 0 and du > 0))):   # top-left rule on an edge
+                                inside = False
+                            lam.append(e / area)
+                        if not inside:
+                            continue
+                        assert sum(lam) == 1
+                        w_star = lam[0] * a[aw] + lam[1] * b[aw] + lam[2] * c[aw]
+                        if w_star <= pw:                                        # crossing at or before the centre
+                            crossings += 1
+                    out[d, z, y, x] = crossings & 1
+    return out[0], out[1], out[2]
+
+
+def test_voxeliser_equals_the_plain_per_cell_definition_also_on_degenerate_meshes(MV, W):
+    nx, ny, nz = 9, 8, 7
+    rng = np.random.default_rng(12)
+    meshes = {
+        "corners on cell centres": W.box_mesh((1.5, 2.5, 1.5), (6.5, 5.5, 4.5)),
+        "faces on cell faces": W.box_mesh((1.0, 2.0, 1.0), (6.0, 5.0, 4.0)),
+        "two boxes sharing a face through centres": np.concatenate([W.box_mesh((1.25, 1.5, 0.75), (4.5, 6.25, 5.5)),
+                                                                    W.box_mesh((4.5, 1.5, 0.75), (8.75, 6.25, 5.5))]),
+        "clipped by the domain": W.box_mesh((-2.5, 3.5, -1.0), (4.5, 12.0, 3.5)),
+        "sphere with a vertex column through centres": W.icosphere_mesh((4.5, 3.5, 3.5), 2.5, 1),
+        "half a roof removed": np.delete(W.box_mesh((2.25, 2.25, 1.25), (7.75, 6.75, 5.75)), 10, axis=0),
+    }
+    # random triangles with vertices on the half-cell grid (every one of them degenerate for some ray), not closed
+    meshes["random soup on the half-cell grid"] = (rng.integers(0, 16, size=(14, 3, 3)) / 2.0).astype(np.float32)
+    meshes["random soup, generic"] = rng.uniform(-1, 9, size=(14, 3, 3)).astype(np.float32)
+    for name, tri in meshes.items():
+        want = plain_parities(MV, tri, nx, ny, nz)
+        got = MV.pass_parities(tri, nx, ny, nz)
+        for d in range(3):
+            np.testing.assert_array_equal(got[d], want[d], err_msg=f"{name}, pass {d}")
+        for votes in (1, 2, 3):
+            np.testing.assert_array_equal(MV.voxelise(tri, nx, ny, nz, votes),
+                                          ((want[0].astype(int) + want[1] + want[2]) >= votes).astype(np.uint8))
