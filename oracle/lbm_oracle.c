@@ -28,6 +28,9 @@
  * oracle_step; reading 23) is pinned by tests/test_oracle_thermal.py:
  * closed forms and the density-current front positions the paper prints
  * (tests/golden/density_current_fronts.txt).
+ * The optional 16-bit population storage (round_to_half, to_storage, oracle_set_storage16) is pinned by
+ * tests/test_oracle_storage16.py: numpy's float16 cast on a value sweep, the state lying on the half grid after every
+ * kind of write, and closed-form error budgets (Taylor-Green decay, Poiseuille, mass drift).
  */
 #include <math.h>
 #include <stdint.h>
@@ -120,11 +123,46 @@ typedef struct oracle {
     int thermal;
     double alpha, gbeta, theta_ref; /* diffusivity, g*beta (buoyancy per unit theta, along +z), reference theta */
     double *H, *Hn;                 /* [cell][7] post-collision thermal populations, directions 0..6 of CI */
+    /* 16-bit population storage: 0 = populations kept in FP64 (default),
+     * 1 = every population is rounded to IEEE binary16 at the moment it is written into the state */
+    int store16;
 } oracle_t;
 
 static long cell_of(const oracle_t *o, int x, int y, int z)
 {
     return ((long)z * o->ny + y) * o->nx + x;
+}
+
+/* ---- 16-bit population storage (SURVEY.md §8(f) row 5 "16-bit DDF storage") --------------------------
+ * The paper does not say how its populations are stored (PAPER.md:181-185 silent; SURVEY.md §6 infers from the printed
+ * wall-clock that they were not plain FP32).  Reading: arithmetic is unchanged; what is STORED for
+ * population i is the shifted value G_i - w_i rounded to IEEE 754 binary16 (1 sign, 5 exponent, 10 fraction bits;
+ * subnormals kept; round to nearest, ties to even), at the moment it is written.  The rest state is stored exactly (0).
+ * round_to_half writes the definition out: spacing 2^(E-10) for 2^E <= |x| < 2^(E+1), E clamped at -14 (below that the
+ * spacing stays 2^-24), overflow to infinity from 65520 on. */
+static double round_to_half(double x)
+{
+    if (x == 0.0 || x != x) return x;
+    double a = fabs(x);
+    if (a >= 65520.0) return x > 0 ? INFINITY : -INFINITY; /* halfway between the largest half (65504) and 2^16 */
+    int e;
+    frexp(a, &e);                 /* a = m 2^e with 1/2 <= m < 1: leading bit has exponent e - 1 */
+    int E = e - 1;
+    if (E < -14) E = -14;         /* subnormal range */
+    double ulp = ldexp(1.0, E - 10);
+    double q = nearbyint(a / ulp); /* a / ulp is exact (power of two); default rounding mode = ties to even */
+    return x > 0 ? q * ulp : -(q * ulp);
+}
+int oracle_round_half(int n, const double *in, double *out)
+{
+    for (int i = 0; i < n; ++i) out[i] = round_to_half(in[i]);
+    return 0;
+}
+/* what the state keeps of a freshly computed set of populations g[19] (in place) */
+static void to_storage(const oracle_t *o, double *g)
+{
+    if (!o->store16) return;
+    for (int i = 0; i < Q; ++i) g[i] = weight(i) + round_to_half(g[i] - weight(i));
 }
 
 /* step 2: second-order equilibrium */
@@ -549,6 +587,7 @@ static void write_fixed_cells_at(oracle_t *o, double t)
                 double u[3], g[Q];
                 boundary_velocity(o, x, y, z, t, u);
                 feq(1.0, u, g);
+                to_storage(o, g);
                 memcpy(o->G + cell * Q, g, sizeof g);
                 memcpy(o->Gn + cell * Q, g, sizeof g);
             }
@@ -582,6 +621,7 @@ static void write_eq_fixed_cell(oracle_t *o, long cell)
 {
     double g[Q];
     feq(1.0, o->ub + 3 * cell, g);
+    to_storage(o, g);
     memcpy(o->G + cell * Q, g, sizeof g);
     memcpy(o->Gn + cell * Q, g, sizeof g);
 }
@@ -642,6 +682,7 @@ int oracle_set_macros(oracle_t *o, const double *rho, const double *ux, const do
         if (cl == C_SOLID) { r = 1.0; u[0] = u[1] = u[2] = 0.0; }
         double g[Q];
         feq(r, u, g);
+        to_storage(o, g);
         memcpy(o->G + cell * Q, g, sizeof g);
         memcpy(o->Gn + cell * Q, g, sizeof g);
     }
@@ -713,7 +754,8 @@ int oracle_balance_flux(oracle_t *o, double *flux_before, double *flux_after)
                         double shift = phi / (double)n;
                         double ub[3] = {u[0] - shift * nrm[0], u[1] - shift * nrm[1], u[2] - shift * nrm[2]};
                         feq(1.0, ub, o->G + cell * Q);
-                        feq(1.0, ub, o->Gn + cell * Q);
+                        to_storage(o, o->G + cell * Q);
+                        memcpy(o->Gn + cell * Q, o->G + cell * Q, sizeof(double) * Q);
                         for (int a = 0; a < 3; ++a) o->ub[3 * cell + a] = ub[a];
                     } else phi2 += un;
                 }
@@ -753,6 +795,7 @@ int oracle_step(oracle_t *o, int nsteps)
                         if (o->ut) for (int a = 0; a < 3; ++a) ut[a] = o->ut[a * o->nz + z];
                         if (!o->thermal) {
                             collide(f, o->nu0, o->Cs, o->fv, o->F, o->sig ? o->sig[cell] : 0.0, ut, gn, NULL, NULL, NULL);
+                            to_storage(o, gn);
                         } else {
                             /* thermal lattice (reading 23): pull the 7 thermal populations by the same rule 4a
                              * (bounce-back on walls / solids and specular reflection on free-slip faces = no heat flux),
@@ -787,11 +830,13 @@ int oracle_step(oracle_t *o, int nsteps)
                         if (p[k / 2] >= 0 && p[k / 2] < n[k / 2])
                             local_macros(o, o->G, cell_of(o, p[0], p[1], p[2]), &r, u);
                         feq(1.0, u, gn);
+                        to_storage(o, gn);
                     } else if (cl == C_EQ_FIXED && o->nmodes > 0) {
                         /* step 5 with fluctuations: the state of step k+1 carries u'(x, k+1) */
                         double u[3];
                         boundary_velocity(o, x, y, z, (double)(o->step + 1), u);
                         feq(1.0, u, gn);
+                        to_storage(o, gn);
                     } else {
                         /* SOLID: inert; EQ_FIXED (step 5): unchanged */
                         memcpy(gn, o->G + cell * Q, sizeof(double) * Q);
@@ -865,11 +910,22 @@ int oracle_get_state(const oracle_t *o, double *f)
 int oracle_set_state(oracle_t *o, const double *f)
 {
     long N = (long)o->nx * o->ny * o->nz;
-    for (int i = 0; i < Q; ++i)
-        for (long cell = 0; cell < N; ++cell) {
-            o->G[cell * Q + i] = f[(long)i * N + cell];
-            o->Gn[cell * Q + i] = f[(long)i * N + cell];
-        }
+    for (long cell = 0; cell < N; ++cell) {
+        double g[Q];
+        for (int i = 0; i < Q; ++i) g[i] = f[(long)i * N + cell];
+        to_storage(o, g);
+        memcpy(o->G + cell * Q, g, sizeof g);
+        memcpy(o->Gn + cell * Q, g, sizeof g);
+    }
+    return 0;
+}
+
+/* 16-bit population storage on (1) / off (0); see round_to_half.  Takes effect for every population written from now
+ * on (set it before the state is initialised).  Not combinable with the thermal lattice (-1). */
+int oracle_set_storage16(oracle_t *o, int on)
+{
+    if (!o || (on && o->thermal)) return -1;
+    o->store16 = on ? 1 : 0;
     return 0;
 }
 
@@ -883,6 +939,7 @@ int oracle_set_step(oracle_t *o, long s) { o->step = s; return 0; }
  * Faces must be PERIODIC / WALL / FREE_SLIP (the density-current set-up of PAPER.md:121 is a closed box); -1 otherwise. */
 int oracle_set_thermal(oracle_t *o, double alpha, double gbeta, double theta_ref)
 {
+    if (o->store16) return -1;
     for (int k = 0; k < 6; ++k)
         if (o->face[k] == F_EQ_FIXED || o->face[k] == F_EQ_OUTFLOW) return -1;
     if (!(alpha > 0.0)) return -1;

@@ -51,7 +51,7 @@ def _load():
                  "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux",
                  "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping",
                  "oracle_vk_spectrum", "oracle_set_inflow_turbulence", "oracle_set_flags_mask",
-                 "oracle_set_theta", "oracle_get_theta", "oracle_heq"):
+                 "oracle_set_theta", "oracle_get_theta", "oracle_heq", "oracle_round_half", "oracle_set_storage16"):
         getattr(lib, name).restype = C.c_int
     lib.oracle_set_thermal.restype = C.c_int
     lib.oracle_set_thermal.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
@@ -140,6 +140,15 @@ def heq(theta, u):
     return out
 
 
+def round_half(x):
+    """The oracle's round-to-binary16 (ties to even, subnormals kept) of each element; float64 in and out."""
+    lib = _load()
+    x, xp = _d(np.atleast_1d(x))
+    out = np.zeros(x.size)
+    lib.oracle_round_half(C.c_int(x.size), xp, out.ctypes.data_as(C.c_void_p))
+    return out.reshape(x.shape)
+
+
 def vk_spectrum(k, u_rms, k_e, k_eta=0.0):
     """von Karman-Pao energy spectrum E(k) (k_eta = 0: no Pao cut-off)."""
     lib = _load()
@@ -177,6 +186,10 @@ class Oracle:
     def _chk(self, rc, what):
         if rc != 0:
             raise RuntimeError(f"oracle {what} failed: {rc}")
+
+    def set_storage16(self, on=True):
+        """Every population written from now on is kept as binary16 of its shifted value."""
+        self._chk(self._lib.oracle_set_storage16(C.c_void_p(self._h), int(bool(on))), "set_storage16")
 
     def set_coriolis(self, fvec):
         """Full Coriolis vector f = 2 Omega (lattice units); (0, 0, f_cor) is the scalar form."""
