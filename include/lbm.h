@@ -232,8 +232,15 @@ long lbm_launch_count(const lbm_t *h);
 /* The lattice as the library defines it: c[19][3], opposite[19] (host arrays).  For tests. */
 int lbm_lattice(int *c, int *opposite);
 
-/* Tuning knob for experiments: selects the stream-collide kernel variant (0 = default).  Returns
- * LBM_EINVAL for an unknown variant.  All variants compute the same arithmetic. */
+/* Launch shape of the FP32 stream-collide step, for A/B measurements.  Every variant computes the same arithmetic on
+ * the same stored state (tests/test_gpu_parity.py runs each against the oracle):
+ *   0  default: 4 x-cells per thread with 128-bit loads / stores where nx % 4 == 0, else one cell per thread; lattices
+ *      whose whole grid is resident at once run several steps per cooperative launch;
+ *   1  one cell per thread, 32-bit accesses, one launch per step;
+ *   2  2 x-cells per thread, 64-bit accesses (nx % 2 == 0, else as 1), one launch per step;
+ *   3  4 x-cells per thread, 128-bit accesses (nx % 4 == 0, else as 1), one launch per step.
+ * FP64 handles, damping zones, inflow fluctuations and the thermal lattice have one launch shape each and ignore it.
+ * Returns LBM_EINVAL for an unknown variant. */
 int lbm_set_variant(lbm_t *h, int variant);
 
 #ifdef __cplusplus

@@ -3,6 +3,7 @@
 #include "lbm_core.cuh"
 #include "lbm_setup.cuh"
 #include "lbm_step.cuh"
+#include "lbm_step_vec.cuh"
 #include "lbm_thermal.cuh"
 #include "lbm_out.cuh"
 #include "lbm_mesh.cuh"
@@ -438,7 +439,7 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     return rc;
 }
 
-template <typename real, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false, bool TURB = false>
+template <typename real, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
 int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
     const real *A = (const real *)h->state();
@@ -455,15 +456,54 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
     real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
     // sampling steps hold three more values per thread (the prefetched sums): one CTA per SM less, 56 registers, no spills
     constexpr int MINB_S = (SPEC && MINB == 10) ? 9 : MINB;
-    if (sample) step_kernel<real, true, HINT, SPEC, BLOCK, MINB_S, EXP, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
-    else step_kernel<real, false, HINT, SPEC, BLOCK, MINB, EXP, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
+    if (sample) step_kernel<real, true, SPEC, BLOCK, MINB_S, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
+    else step_kernel<real, false, SPEC, BLOCK, MINB, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
     return check_launch(h, "step_kernel");
 }
 
-// kernel variants (lbm_set_variant): same arithmetic, different cache hints / launch shapes / load issue order.
-constexpr int N_VARIANTS = 11;
+// V cells per thread, 64/128-bit accesses (lbm_step_vec.cuh); applicable when nx % V == 0 and the thread index divides exactly
+template <int V>
+bool vec_geom(const Params<float> &P, VecGeom *G)
+{
+    if (P.nx % V != 0) return false;
+    G->qpr = (unsigned)(P.nx / V);
+    G->nq = (unsigned)((long long)P.nxy / V);
+    G->qmagic = 0;
+    // exact for n < nq + 1024 when (nq + 1024) * qpr < 2^32 (error term n * (magic * qpr - 2^32) < 2^32)
+    if (G->qpr > 1 && ((unsigned long long)G->nq + 1024ULL) * G->qpr < 0x100000000ULL)
+        G->qmagic = (unsigned)((0x100000000ULL + G->qpr - 1) / G->qpr);
+    return true;
+}
+template <int V, int MINB, int MINB_S>
+int launch_step_vec(lbm_t *h, const Params<float> &P, const VecGeom &G, bool sample)
+{
+    constexpr int BLOCK = 128;
+    const float *A = (const float *)h->state();
+    float *B = (float *)h->other();
+    const dim3 grid(blocks_for((long long)G.nq, BLOCK), (unsigned)P.nz);
+    const VecPtrs<float> T = make_vec_ptrs<float>(A, B, P);
+    const float *fur = (const float *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
+    float *fuw = (float *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
+    if (sample) step_vec_kernel<float, V, true, BLOCK, MINB_S><<<grid, BLOCK, 0, h->stream>>>(h->flags(), h->links(), (float *)h->mean(), fur, fuw, P, T, G);
+    else step_vec_kernel<float, V, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(h->flags(), h->links(), nullptr, fur, fuw, P, T, G);
+    return check_launch(h, "step_vec_kernel");
+}
+
+// launch shapes of the FP32 step (lbm_set_variant): the same arithmetic and the same stored state in all of them
+//   0 = default: 4 cells per thread with 128-bit accesses where nx % 4 == 0, else one cell per thread; lattices whose whole
+//       grid is resident at once run several steps per cooperative launch (step_loop_kernel)
+//   1 = one cell per thread (32-bit accesses), one launch per step
+//   2 = 2 cells per thread with 64-bit accesses where nx % 2 == 0 (else as 1), one launch per step
+//   3 = 4 cells per thread with 128-bit accesses where nx % 4 == 0 (else as 1), one launch per step
+constexpr int N_VARIANTS = 4;
 #ifndef DAMP_MINB
 #define DAMP_MINB 9
+#endif
+#ifndef VEC4_MINB
+#define VEC4_MINB 4
+#endif
+#ifndef VEC2_MINB
+#define VEC2_MINB 6
 #endif
 template <typename real>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
@@ -472,52 +512,31 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         const real *A = (const real *)h->state();
         real *B = (real *)h->other();
         dim3 grid(blocks_for((long long)P.nxy, 128), (unsigned)P.nz);
-        auto go = [&](auto minb) {
-            constexpr int BLOCK = 128, MINB = decltype(minb)::value;
-            if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
-            else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
-        };
-        if constexpr (std::is_same<real, float>::value) {
-            // 19 + 7 populations: 72 registers hold them without spills = 7 CTAs per SM (measured 24 900 MLUPS; 6 CTAs / 80
-            // registers 24 000, 5 CTAs 22 600, 8 CTAs / 64 registers with 16 B of spills 24 900); lbm_set_variant 1..3 = 5 / 6 / 8
-            switch (h->variant) {
-            case 1: go(std::integral_constant<int, 5>{}); break;
-            case 2: go(std::integral_constant<int, 6>{}); break;
-            case 3: go(std::integral_constant<int, 8>{}); break;
-            default: go(std::integral_constant<int, 7>{}); break;
-            }
-        } else go(std::integral_constant<int, 2>{});
+        // 19 + 7 populations: 72 registers hold them without spills = 7 CTAs per SM (measured 24 900 MLUPS; 6 CTAs / 80
+        // registers 24 000, 5 CTAs 22 600, 8 CTAs / 64 registers with 16 B of spills 24 900)
+        constexpr int BLOCK = 128, MINB = std::is_same<real, float>::value ? 7 : 2;
+        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
+        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
         return check_launch(h, "thermal_step_kernel");
     }
     const bool turb = h->nmodes > 0 && P.F > 0;
     if (h->damp_on || turb) { // damping zones / inflow fluctuations: their own instantiations (same arithmetic elsewhere)
         if constexpr (std::is_same<real, float>::value) {
-            if (h->damp_on && turb) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true, true>(h, P, sample);
-            if (h->damp_on) return launch_step_as<real, 0, true, 128, DAMP_MINB, 0, true, false>(h, P, sample);
-            return launch_step_as<real, 0, true, 128, 10, 0, false, true>(h, P, sample); // no prefetched table values: 48 registers do
+            if (h->damp_on && turb) return launch_step_as<real, true, 128, DAMP_MINB, true, true>(h, P, sample);
+            if (h->damp_on) return launch_step_as<real, true, 128, DAMP_MINB, true, false>(h, P, sample);
+            return launch_step_as<real, true, 128, 10, false, true>(h, P, sample); // no prefetched table values: 48 registers do
         } else {
-            if (h->damp_on && turb) return launch_step_as<real, 0, false, 256, 2, 0, true, true>(h, P, sample);
-            if (h->damp_on) return launch_step_as<real, 0, false, 256, 2, 0, true, false>(h, P, sample);
-            return launch_step_as<real, 0, false, 256, 2, 0, false, true>(h, P, sample);
+            if (h->damp_on && turb) return launch_step_as<real, false, 256, 2, true, true>(h, P, sample);
+            if (h->damp_on) return launch_step_as<real, false, 256, 2, true, false>(h, P, sample);
+            return launch_step_as<real, false, 256, 2, false, true>(h, P, sample);
         }
     }
     if constexpr (std::is_same<real, float>::value) {
-        switch (h->variant) {
-        case 0: return launch_step_as<real, 0, true, 128, 10>(h, P, sample);
-        case 1: return launch_step_as<real, 0, true, 256, 4>(h, P, sample);
-        case 2: return launch_step_as<real, 0, false, 128, 8>(h, P, sample);
-        case 3: return launch_step_as<real, 0, true, 128, 8>(h, P, sample);
-        case 4: return launch_step_as<real, 0, true, 128, 9>(h, P, sample);
-        case 5: return launch_step_as<real, 0, false, 256, 4>(h, P, sample);
-        case 6: return launch_step_as<real, 0, true, 256, 5>(h, P, sample);
-        case 7: return launch_step_as<real, 2, true, 128, 10>(h, P, sample);
-        case 8: return launch_step_as<real, 0, true, 96, 13>(h, P, sample);
-        case 9: return launch_step_as<real, 0, true, 64, 20>(h, P, sample);
-        case 10: return launch_step_as<real, 0, true, 128, 10, 1>(h, P, sample);
-        default: break;
-        }
-    }
-    return launch_step_as<real, 0, false, 256, 2>(h, P, sample);
+        VecGeom G;
+        if ((h->variant == 0 || h->variant == 3) && vec_geom<4>(P, &G)) return launch_step_vec<4, VEC4_MINB, 3>(h, P, G, sample);
+        if (h->variant == 2 && vec_geom<2>(P, &G)) return launch_step_vec<2, VEC2_MINB, 5>(h, P, G, sample);
+        return launch_step_as<real, true, 128, 10>(h, P, sample);
+    } else return launch_step_as<real, false, 256, 2>(h, P, sample);
 }
 
 // boundary velocities of time t for the EQ_FIXED slots (mean + fluctuations on active inflow cells); cells = also rewrite

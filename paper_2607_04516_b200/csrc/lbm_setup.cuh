@@ -214,8 +214,8 @@ __device__ __forceinline__ void fluct_slot(int s, real *__restrict__ A, real *__
     if ((fl & CLASS_MASK) != EQ_FIXED) return;
     real u0 = tb.fum[s], u1 = tb.fum[P.F + s], u2 = tb.fum[2 * P.F + s];
     const real ua = axis == 0 ? u0 : (axis == 1 ? u1 : u2);
-    const real un = (k & 1) ? ua : -ua;
-    if (un < real(-1e-7)) { // "active inflow": inward by more than rounding noise (DESIGN.md §4 reading 21)
+    const double un = (k & 1) ? (double)ua : -(double)ua;
+    if (un < -1e-7) { // "active inflow": inward by more than rounding noise (DESIGN.md §4 reading 21); compared in FP64 like the oracle
         real a0 = real(0), a1 = real(0), a2 = real(0);
         const double xd = (double)x, yd = (double)y, zd = (double)z;
         for (int n = 0; n < tb.n; ++n) {

@@ -7,9 +7,8 @@
 // extra predicated stores in cells that have a wall link or lie on a domain face.
 // Traffic per FLUID cell: 19 x 4 B read + 19 x 4 B write + 1 flag byte (+ 4 B link word only where SLOW_BIT is set).
 //
-// HINT: 0 = default loads / stores, 1 = ld.global.cs / st.global.cs (streaming), 2 = default ld / st.cs, 3 = ld.cs / default st.
 // SPEC: issue the 19 population loads before the flag byte has arrived (no dependent round trip; SOLID cells then
-//       cost their 76 B of reads).
+//       cost their 76 B of reads).  The FP32 product kernels are SPEC; the FP64 reference twin is not.
 // TURB: the launch carries the synthetic inflow fluctuations in extra leading block rows (lbm_set_inflow_turbulence).
 // DAMP: the damping-zone instantiation (lbm_set_damping); launched only while zones are configured, so the plain
 //       kernel carries none of it.
@@ -20,12 +19,6 @@
 
 namespace lbmk {
 
-template <int HINT, typename real>
-__device__ __forceinline__ real ld_pop(const real *p)
-{
-    if constexpr (HINT == 1 || HINT == 3) return __ldcs(p);
-    else return *p;
-}
 // A load the compiler may not sink below a later branch (volatile asm keeps its place): the 19 pulls of the
 // speculative kernels are issued before the flag byte is tested.
 __device__ __forceinline__ float ld_pinned(const float *p)
@@ -45,12 +38,6 @@ __device__ __forceinline__ uint8_t ld_pinned(const uint8_t *p)
     uint32_t v;
     asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(p));
     return (uint8_t)v;
-}
-template <int HINT, typename real>
-__device__ __forceinline__ void st_pop(real *p, real v)
-{
-    if constexpr (HINT == 1 || HINT == 2) __stcs(p, v);
-    else *p = v;
 }
 
 // Per-launch address table: src[i] = A + i stride - off_i (so the pull of direction i is src[i][p]), dst[i] = B + i stride.
@@ -74,7 +61,7 @@ inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> 
 
 // The step of one thread (one cell, or one face slot in a TURB block row).  A plain device function so that it can be
 // called once per launch (step_kernel) or in a loop with grid-wide barriers (step_loop_kernel, lattices that fit L2).
-template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int EXP, bool DAMP, bool TURB>
+template <typename real, bool MEAN, bool SPEC, int BLOCK, bool DAMP, bool TURB>
 __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
                                           const uint32_t *__restrict__ links, real *__restrict__ msum, const real *__restrict__ fur,
                                           real *__restrict__ fuw, const Params<real> &P, const StepPtrs<real> &T, const Turb<real> &tb,
@@ -130,7 +117,6 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     } else {
         fl = flags[p];
     }
-    if constexpr (EXP == 1) fl = 0; // timing experiment: every cell FLUID, no boundary stores
     if constexpr (SPEC) {
         // Fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, no feed, nothing to complete)
         // — the bulk of the lattice.  Straight-line collide + 19 stores, none of the per-feature tests below.
@@ -140,7 +126,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
             else m = collide(g, P);
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
-                st_pop<HINT>(T.dst[i] + p, g[i]);
+                T.dst[i][p] = g[i];
             });
             if constexpr (MEAN) {
                 msum[p] = ms0 + m.ux;
@@ -166,7 +152,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
         if constexpr (!SPEC) {
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
-                g[i] = ld_pop<HINT>(T.src[i] + p);
+                g[i] = T.src[i][p];
             });
         }
         if constexpr (DAMP) m = collide<real, true>(g, P, SPEC ? dmp : damp_at(P, x, y, z));
@@ -188,12 +174,12 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     if (__any_sync(__activemask(), merged_solid)) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            if ((wm >> i) & 1u) st_pop<HINT>(T.dst[i] + p, g[i]);
+            if ((wm >> i) & 1u) T.dst[i][p] = g[i];
         });
     } else {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            st_pop<HINT>(T.dst[i] + p, g[i]);
+            T.dst[i][p] = g[i];
         });
     }
     if (merged_solid) return;
@@ -220,13 +206,13 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     }
 }
 
-template <typename real, bool MEAN, int HINT, bool SPEC, int BLOCK, int MINB, int EXP = 0, bool DAMP = false, bool TURB = false>
+template <typename real, bool MEAN, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
             real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T,
             const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
 {
-    step_body<real, MEAN, HINT, SPEC, BLOCK, EXP, DAMP, TURB>(A, B, flags, links, msum, fur, fuw, P, T, tb, turb_planes);
+    step_body<real, MEAN, SPEC, BLOCK, DAMP, TURB>(A, B, flags, links, msum, fur, fuw, P, T, tb, turb_planes);
 }
 
 // Several steps in ONE cooperative launch, a grid-wide barrier between them: for lattices whose whole grid is resident
@@ -244,9 +230,9 @@ step_loop_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__re
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const Turb<real> tb{};
     for (int s = 0; s < pairs; ++s) {
-        step_body<real, false, 0, true, BLOCK, 0, DAMP, false>(A, B, flags, links, nullptr, fu0, fu1, P, T0, tb, 0);
+        step_body<real, false, true, BLOCK, DAMP, false>(A, B, flags, links, nullptr, fu0, fu1, P, T0, tb, 0);
         grid.sync();
-        step_body<real, false, 0, true, BLOCK, 0, DAMP, false>(B, A, flags, links, nullptr, fu1, fu0, P, T1, tb, 0);
+        step_body<real, false, true, BLOCK, DAMP, false>(B, A, flags, links, nullptr, fu1, fu0, P, T1, tb, 0);
         grid.sync();
     }
 }

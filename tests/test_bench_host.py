@@ -77,7 +77,8 @@ def test_reference_arm_prints_one_line_from_rank_0_only():
 def test_traffic_figure_comes_from_the_committed_profile():
     sys.path.insert(0, ROOT)
     import bench
-    t = bench.load_traffic()
+    t, src = bench.load_traffic()
     assert t is None or 0.9 * 153 * 16e6 < t < 1.3 * 153 * 16e6
-    th = bench.load_traffic("thermal")  # fused flow + thermal kernel: (19 + 7) x 4 B x 2 + 1 flag byte = 209 B/cell
+    assert (t is None) == (src is None) and (src is None or os.path.exists(os.path.join(ROOT, src)))
+    th, _ = bench.load_traffic("thermal")  # fused flow + thermal kernel: (19 + 7) x 4 B x 2 + 1 flag byte = 209 B/cell
     assert th is None or 0.9 * 209 * 16e6 < th < 1.3 * 209 * 16e6

@@ -52,6 +52,7 @@ def check_flags_links(sim, o):
 FACE_SETS = [
     (0, 0, 0, 0, 0, 0), (3, 4, 0, 0, 1, 2), (3, 4, 2, 2, 1, 2), (3, 4, 3, 3, 1, 2), (0, 0, 0, 0, 1, 2),
     (1, 1, 1, 1, 1, 1), (2, 2, 2, 2, 2, 2), (2, 1, 0, 0, 2, 1), (4, 3, 1, 2, 0, 0),
+    (3, 4, 2, 4, 1, 2),     # two EQ_OUTFLOW faces meet (DESIGN.md §4 reading 24)
 ]
 
 
@@ -355,20 +356,22 @@ def test_host_pointer_getters_equal_device_pointer_getters(B):
 
 # ---------------------------------------------------------------------------------------------- kernel variants
 
-@pytest.mark.parametrize("variant", [0, 1, 3, 4, 7, 8])
-@pytest.mark.parametrize("shape", [(37, 11, 9), (64, 36, 20), (130, 50, 7)])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3])     # every launch shape lbm_set_variant offers (include/lbm.h)
+@pytest.mark.parametrize("shape", [(37, 11, 9), (64, 36, 20), (130, 50, 7), (132, 9, 6), (4, 5, 6), (8, 3, 3)])
 def test_every_step_kernel_variant_matches_the_oracle(B, variant, shape):
-    """The bulk-copy (TMA) kernels and the LDG kernel compute the same step: ragged and 16-byte-aligned boxes,
-    several tiles per CTA, partial last tile, buildings, every face rule, forcing, mean sampling."""
+    """One cell per thread, 2 and 4 x-cells per thread with 64 / 128-bit accesses, and the cooperative multi-step launch
+    compute the same step: ragged boxes (fall back to one cell per thread), nx % 4 == 0 and nx % 2 == 0 boxes, rows
+    shorter than a warp (several rows per warp, shuffles across row ends), a last warp that is partly beyond the plane,
+    buildings, every face rule, forcing, mean sampling."""
     from oracle import Oracle
     nx, ny, nz = shape
     rng = np.random.default_rng(nx * 1000 + ny)
     hm = np.zeros((ny, nx), dtype=np.int32)
     for _ in range(6):
-        x0, y0 = int(rng.integers(2, nx - 6)), int(rng.integers(0, ny - 3))
+        x0, y0 = int(rng.integers(0, max(nx - 6, 1))), int(rng.integers(0, max(ny - 3, 1)))
         hm[y0:y0 + 3, x0:x0 + 4] = int(rng.integers(1, nz))
     prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0).astype(np.float32)
-    for faces in [(3, 4, 0, 0, 1, 2), (3, 4, 2, 2, 1, 2), (0, 0, 0, 0, 1, 2), (3, 4, 3, 3, 1, 2)]:
+    for faces in [(3, 4, 0, 0, 1, 2), (3, 4, 2, 2, 1, 2), (0, 0, 0, 0, 1, 2), (3, 4, 3, 3, 1, 2), (3, 4, 2, 4, 1, 2)]:
         args = (nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), faces)
         o = Oracle(*args)
         o.set_flags(hm)
@@ -655,6 +658,39 @@ def test_inflow_fluctuations_match_the_oracle(B, fp64):
     sim.step(20)
     assert max_err(sim, o, f64=fp64) <= tol
     sim.set_inlet_profile(prof, 0.2 * prof, None, f64=True)    # allowed again
+    sim.close()
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_active_inflow_threshold_is_decided_like_the_oracle(B, fp64):
+    """DESIGN.md §4 reading 21: active inflow <=> ub.n < -1e-7, compared in FP64 on both sides.  One x- face whose mean
+    normal components straddle the constant — 5e-8 and the float32 just below 1e-7 keep the mean, the float32 just above
+    1e-7 (= float32(1e-7)) and 2e-7 fluctuate; the inputs are float32-representable, so the FP32 handle stores exactly
+    what the oracle gets.  Mirror of tests/test_oracle_inflow.py::test_active_inflow_threshold_..."""
+    from oracle import Oracle
+    from paper_2607_04516_b200 import workloads as W
+    nx, ny, nz = 8, 8, 4
+    above = np.float32(1e-7)
+    assert float(above) > 1e-7
+    below = np.nextafter(above, np.float32(0))
+    assert float(below) < 1e-7
+    un = np.array([5e-8, float(below), float(above), 2e-7, -2e-7, 1e-6, 0.0, -5e-8], dtype=np.float32).astype(np.float64)
+    active = np.array([False, False, True, True, False, True, False, False])
+    plane = np.zeros((3, nz, ny))
+    plane[0] = un[None, :]
+    plane[1] = 0.0078125
+    args = (nx, ny, nz, 1e-2, 0.0, 0.0, (0, 0, 0), (3, 4, 0, 0, 2, 2))
+    o = Oracle(*args); o.set_flags(None); o.set_inlet_plane(0, plane); o.set_macros()
+    sim = B.Lbm(*args, fp64=fp64); sim.set_flags(None); sim.set_inlet_plane(0, plane, f64=True); sim.set_macros()
+    modes = W.inflow_modes(8, 21, 0.2, 2.0)
+    o.set_inflow_turbulence(modes, 0.01, 0.5)
+    sim.set_inflow_turbulence(modes, 0.01, 0.5)
+    for _ in range(3):
+        g = [a.cpu().numpy().astype(np.float64) for a in sim.get_macros(f64=fp64)]
+        dev = np.sqrt((g[1][:, :, 0] - un[None, :]) ** 2 + (g[2][:, :, 0] - 0.0078125) ** 2 + g[3][:, :, 0] ** 2)
+        assert dev[:, ~active].max() < 1e-9 and dev[:, active].min() > 1e-4
+        assert max_err(sim, o, f64=fp64) <= (TOL64 if fp64 else TOL32)
+        o.step(1); sim.step(1)
     sim.close()
 
 
