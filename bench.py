@@ -33,6 +33,8 @@ def metric_for(workload):
     """The headline metric string names config 3; the other workloads are per-config table lines and say what they ran."""
     if workload == "c3":
         return METRIC
+    if workload == "c3-fp16":
+        return "MLUPS (D3Q19, FP32 arithmetic, 16-bit population storage), fused stream-collide, 400x400x100 urban config, 1 B200"
     return f"MLUPS (D3Q19 FP32), fused stream-collide, workload {workload} (per-config table line, not the headline), 1 B200"
 
 # --workload: the headline is c3 (BASELINE.json: the config the metric is quoted on); the others are the parity configs,
@@ -43,6 +45,8 @@ WORKLOADS = {
     "c3": "C3 urban 400x400x100 (BASELINE.json configs[2]): seeded heightmap plan fraction 0.35, log-law inlet, nu0 1e-4, Cs 0.1, f 2.9e-6",
     "c4": "C4 refined urban 800x800x200, veering inlet on three faces (BASELINE.json configs[3])",
     "thermal": "closed 400x400x100 city box with the D3Q7 thermal lattice + Boussinesq coupling on (DESIGN.md reading 23): 209 B/cell",
+    "c3-fp16": "C3 urban 400x400x100 with 16-bit population storage (LBM_PREC_F32_S16, DESIGN.md §13): FP32 arithmetic, binary16 "
+               "storage of the shifted populations, 77 B/cell — a separate line, NOT the FP32 headline",
     "c5": "C5 chain: periodic precursor 256x256x200 feeding the x- inlet of the 1200x1200x200 urban domain every step (BASELINE.json configs[4])",
 }
 
@@ -56,9 +60,9 @@ class Job:
             self.wls = [W.config5_precursor(), W.config5_main()]
         else:
             self.wls = [{"c1": W.config1, "c2": lambda: W.config2(Cs=0.1), "c3": W.config3, "c4": W.config4,
-                         "thermal": W.thermal_city}[name]()]
+                         "thermal": W.thermal_city, "c3-fp16": W.config3}[name]()]
         self.cells = sum(w.cells for w in self.wls)
-        self.sims = [binding.from_workload(w, want_mean=False, device=device) for w in self.wls]
+        self.sims = [binding.from_workload(w, want_mean=False, device=device, storage16=(name == "c3-fp16")) for w in self.wls]
 
     def step(self, n):
         if len(self.sims) == 1:
@@ -358,7 +362,8 @@ def run_ours(args):
         peak, peak_src = load_peak()
         per_launch_s = ms_total * 1e-3 / K
         # thermal workload: (19 + 7) x 4 B loads + (19 + 7) x 4 B stores + 1 flag byte (lbm_thermal.cuh)
-        BYTES_PER_CELL = 209 if args.workload == "thermal" else globals()["BYTES_PER_CELL"]
+        # 16-bit storage: 19 x 2 B loads + 19 x 2 B stores + 1 flag byte
+        BYTES_PER_CELL = {"thermal": 209, "c3-fp16": 77}.get(args.workload, globals()["BYTES_PER_CELL"])
         achieved = BYTES_PER_CELL * cells / per_launch_s / 1e9
         traffic, traffic_src = (load_traffic("step") if args.workload == "c3" else
                                 load_traffic("thermal") if args.workload == "thermal" else (None, None))
@@ -370,7 +375,7 @@ def run_ours(args):
         line = {
             "metric": metric_for(args.workload), "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic",
+            "dtype": "f32 arithmetic, f16 storage" if args.workload == "c3-fp16" else "f32", "data": "synthetic",
             "config": {"workload": WORKLOADS[args.workload],
                        "cells": cells, "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": (f"no flush needed: each step streams {BYTES_PER_CELL * cells / 1e9:.1f} GB (>> 126 MB L2)"

@@ -52,10 +52,20 @@ enum {
 /* cell classes returned by lbm_get_flags (DESIGN.md §3 step 3, 9) */
 enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_CELL_EQ_FIXED = 2, LBM_CELL_EQ_OUTFLOW = 3 };
 
-/* Bytes of device workspace a handle of this size needs (two population buffers of 19 reals per cell,
- * one flag byte per cell, optional 3 reals per cell of time-mean sums, small profile/plane scratch).
- * fp64 != 0 sizes a double-precision handle. */
-int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int fp64, size_t *out);
+/* Precision of a handle: what the arithmetic runs in and how the 19 populations per cell are stored.
+ *   LBM_PREC_F32      FP32 arithmetic, FP32 storage: 153 B per cell and step (BASELINE.json north_star; the headline path)
+ *   LBM_PREC_F64      FP64 arithmetic and storage: the reference twin of the same kernels (1 = the old `fp64 != 0`)
+ *   LBM_PREC_F32_S16  FP32 arithmetic, 16-bit population storage: what is stored
+ *                     of population i is the shifted value f_i - w_i rounded to IEEE binary16 (round to nearest even)
+ *                     every time it is written — 77 B per cell and step, half the memory.  Every call works the same;
+ *                     lbm_get_state returns the stored (rounded) values, lbm_set_state rounds its input.  Not combinable
+ *                     with the thermal lattice (lbm_set_thermal returns LBM_EINVAL). */
+enum { LBM_PREC_F32 = 0, LBM_PREC_F64 = 1, LBM_PREC_F32_S16 = 2 };
+
+/* Bytes of device workspace a handle of this size needs (two population buffers of 19 stored values per cell,
+ * one flag byte and one link word per cell, optional 3 reals per cell of time-mean sums, small profile/plane scratch).
+ * precision: LBM_PREC_*; anything else returns LBM_EINVAL. */
+int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int precision, size_t *out);
 
 /* Create an FP32 handle that allocates its own workspace (cudaMalloc) and uses the default stream.
  * nu0: molecular viscosity (tau0 = 3 nu0 + 1/2); Cs: Smagorinsky constant; f_cor: Coriolis parameter about z
@@ -65,10 +75,10 @@ int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int fp64, size_t 
 int lbm_create(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3], lbm_t **out);
 
 /* Same, with a caller-owned DEVICE workspace of at least lbm_workspace_bytes() bytes (256-byte aligned;
- * NULL = allocate), a cudaStream_t passed as void* (NULL = default stream), and the precision choice.
+ * NULL = allocate), a cudaStream_t passed as void* (NULL = default stream), and the precision (LBM_PREC_*).
  * want_mean = 0 omits the time-mean sums (lbm_mean_config then returns LBM_ESTATE). */
 int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3],
-                  void *dev_workspace, size_t workspace_bytes, void *cuda_stream, int fp64, int want_mean,
+                  void *dev_workspace, size_t workspace_bytes, void *cuda_stream, int precision, int want_mean,
                   lbm_t **out);
 
 int lbm_destroy(lbm_t *h);
@@ -181,6 +191,12 @@ int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const dou
 /* theta = sum_i h_i of the current state, [nz][ny][nx], host or device; SOLID cells report theta_ref.  Synchronises. */
 int lbm_get_theta(lbm_t *h, float *theta);
 int lbm_get_theta_f64(lbm_t *h, double *theta);
+/* Checkpoint of the thermal lattice: the 7 thermal populations h_i (NOT shifted), double, [7][nz][ny][nx], directions
+ * 0..6 of the flow lattice; host or device.  Together with lbm_get_state / lbm_set_state and lbm_set_step a thermal run
+ * restarts exactly.  Non-FLUID cells export the rest state wT_i theta_ref and ignore their input.  Needs
+ * lbm_set_thermal and flags (else LBM_ESTATE). */
+int lbm_get_thermal_state(lbm_t *h, double *hpop);
+int lbm_set_thermal_state(lbm_t *h, const double *hpop);
 
 /* Config-5 coupling, device to device, stream-ordered on dst's stream: local macros of src on the plane
  * x = src_x_plane are written as f_eq(1, u) into the EQ_FIXED cells of dst's x- face, tiling y modulo
@@ -217,7 +233,10 @@ int lbm_get_flags(lbm_t *h, uint8_t *flags);
 int lbm_get_links(lbm_t *h, uint32_t *links);
 
 /* Checkpoint: populations f_i (NOT shifted), double, [19][nz][ny][nx], direction order of DESIGN.md §3
- * step 1.  set_state leaves the step counter alone (use lbm_set_step). */
+ * step 1.  set_state leaves the step counter, the mean sums and the thermal state alone (lbm_set_step, lbm_mean_reset,
+ * lbm_set_thermal_state).  The boundary velocity of an EQ_FIXED cell becomes the velocity moment of the populations
+ * given for it (the cell is re-expanded from that velocity every step); prescribe the profile / plane again afterwards
+ * to impose an exact u_b.  SOLID cells export the rest state and ignore their input. */
 int lbm_get_state(lbm_t *h, double *f);
 int lbm_set_state(lbm_t *h, const double *f);
 

@@ -29,6 +29,7 @@ SYMBOLS = [
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
     "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
     "lbm_set_thermal", "lbm_set_theta", "lbm_set_theta_f64", "lbm_get_theta", "lbm_get_theta_f64",
+    "lbm_get_thermal_state", "lbm_set_thermal_state",
 ]
 
 
@@ -73,7 +74,7 @@ def load_library():
     lib.lbm_set_thermal.argtypes = [vp, C.c_double, C.c_double, C.c_double]
     for n in ("lbm_set_theta", "lbm_set_theta_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp, vp]
-    for n in ("lbm_get_theta", "lbm_get_theta_f64"):
+    for n in ("lbm_get_theta", "lbm_get_theta_f64", "lbm_get_thermal_state", "lbm_set_thermal_state"):
         getattr(lib, n).argtypes = [vp, vp]
     lib.lbm_mean_config.argtypes = [vp, l, i]
     lib.lbm_mean_reset.argtypes = [vp]
@@ -115,11 +116,14 @@ def _ptr(a, dtype):
     return a, a.ctypes.data
 
 
+PREC_F32, PREC_F64, PREC_F32_S16 = 0, 1, 2   # include/lbm.h LBM_PREC_*
+
+
 class Lbm:
     """One lattice on one GPU.  Same call names as include/lbm.h without the ``lbm_`` prefix."""
 
     def __init__(self, nx, ny, nz, nu0, Cs=0.0, f_cor=0.0, F=(0.0, 0.0, 0.0), faces=None, fp64=False,
-                 want_mean=True, device="cuda:0", stream=None):
+                 want_mean=True, device="cuda:0", stream=None, storage16=False):
         import torch
         if not torch.cuda.is_available():
             raise LbmError("no CUDA device: the LBM path has no CPU fallback")
@@ -129,11 +133,15 @@ class Lbm:
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.shape = (self.nz, self.ny, self.nx)
         self.fp64 = bool(fp64)
+        self.storage16 = bool(storage16)
+        if fp64 and storage16:
+            raise ValueError("fp64 and storage16 exclude each other")
+        precision = PREC_F64 if fp64 else (PREC_F32_S16 if storage16 else PREC_F32)     # include/lbm.h LBM_PREC_*
         F = np.atleast_1d(np.asarray(F, dtype=np.float64))
         if F.size == 1:
             F = np.array([F[0], 0.0, 0.0])
         nbytes = C.c_size_t()
-        self._chk0(self._lib.lbm_workspace_bytes(self.nx, self.ny, self.nz, int(want_mean), int(fp64), C.byref(nbytes)),
+        self._chk0(self._lib.lbm_workspace_bytes(self.nx, self.ny, self.nz, int(want_mean), precision, C.byref(nbytes)),
                    "workspace_bytes")
         with torch.cuda.device(self.device):
             self._ws = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
@@ -142,7 +150,7 @@ class Lbm:
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
             rc = self._lib.lbm_create_ex(self.nx, self.ny, self.nz, float(nu0), float(Cs), float(f_cor), F.ctypes.data,
-                                         aligned, nbytes.value, self._stream.cuda_stream, int(fp64), int(want_mean),
+                                         aligned, nbytes.value, self._stream.cuda_stream, precision, int(want_mean),
                                          C.byref(h))
         self._chk0(rc, "create_ex")
         self._h = h
@@ -296,6 +304,18 @@ class Lbm:
         self._chk(fn(self._h, a.data_ptr()), "get_theta")
         return a
 
+    def get_thermal_state(self):
+        """The 7 thermal populations [7][nz][ny][nx] float64 (host): the thermal half of a checkpoint."""
+        a = np.empty((7,) + self.shape, dtype=np.float64)
+        self._chk(self._lib.lbm_get_thermal_state(self._h, a.ctypes.data), "get_thermal_state")
+        return a
+
+    def set_thermal_state(self, hpop):
+        k, p = _ptr(hpop, np.float64)
+        if tuple(k.shape) != (7,) + self.shape:
+            raise ValueError("thermal state must be [7][nz][ny][nx]")
+        self._chk(self._lib.lbm_set_thermal_state(self._h, p), "set_thermal_state")
+
     # -- the hot call
     def step(self, n=1):
         self._chk(self._lib.lbm_step(self._h, int(n)), "step")
@@ -385,10 +405,10 @@ def lattice():
     return c, opp
 
 
-def from_workload(wl, fp64=False, want_mean=True, device="cuda:0") -> Lbm:
+def from_workload(wl, fp64=False, want_mean=True, device="cuda:0", storage16=False) -> Lbm:
     """Create a handle for a workloads.Workload and load its flags, inlet profile and initial field."""
     sim = Lbm(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces, fp64=fp64, want_mean=want_mean,
-              device=device)
+              device=device, storage16=storage16)
     sim.set_flags(wl.height)
     if wl.inlet_profile is not None:
         sim.set_inlet_profile(*wl.inlet_profile)

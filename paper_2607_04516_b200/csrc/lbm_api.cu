@@ -32,17 +32,23 @@ struct Layout {
     size_t scratch_bytes;
 };
 
-Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
+// precision: LBM_PREC_F32 / LBM_PREC_F64 / LBM_PREC_F32_S16 (include/lbm.h).  rs = bytes of the arithmetic type (side buffers,
+// mean sums, tables), ss = bytes of a stored population, xoff = padded x of interior x = 0 (one 32-byte sector)
+inline size_t real_bytes(int precision) { return precision == LBM_PREC_F64 ? 8 : 4; }
+inline size_t store_bytes(int precision) { return precision == LBM_PREC_F64 ? 8 : (precision == LBM_PREC_F32_S16 ? 2 : 4); }
+inline int xoff_of(int precision) { return precision == LBM_PREC_F32_S16 ? 16 : 8; }
+
+Layout make_layout(int nx, int ny, int nz, int want_mean, int precision)
 {
     Layout L{};
-    const size_t rs = fp64 ? 8 : 4;
-    L.px = (nx + XOFF + 1 + 31) / 32 * 32;
+    const size_t rs = real_bytes(precision), ss = store_bytes(precision);
+    L.px = (nx + xoff_of(precision) + 1 + 31) / 32 * 32;
     L.py = ny + 2;
     L.Np = (long long)L.px * L.py * (nz + 2);
     L.stride = (long long)align_up((size_t)L.Np, 64);
     size_t o = 0;
-    L.off_A = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
-    L.off_B = o; o += align_up((size_t)Q * L.stride * rs, ALIGN);
+    L.off_A = o; o += align_up((size_t)Q * L.stride * ss, ALIGN);
+    L.off_B = o; o += align_up((size_t)Q * L.stride * ss, ALIGN);
     L.off_flags = o; o += align_up((size_t)L.Np, ALIGN);
     L.off_links = o; o += align_up((size_t)L.Np * sizeof(uint32_t), ALIGN);
     // outflow-velocity side buffer (a6): 2 halves x 3 components x one slot per face-plane cell of all six faces (upper bound)
@@ -66,7 +72,7 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int fp64)
 bool size_ok(int nx, int ny, int nz)
 {
     if (nx < 1 || ny < 1 || nz < 1 || nz > 65535) return false;
-    const long long px = ((long long)nx + XOFF + 1 + 31) / 32 * 32;
+    const long long px = ((long long)nx + 16 + 1 + 31) / 32 * 32; // the widest row offset (16-bit storage)
     return px * ((long long)ny + 2) * ((long long)nz + 2) <= 2000000000LL;
 }
 
@@ -76,7 +82,9 @@ struct lbm {
     int nx, ny, nz;
     double nu0, Cs, fv[3], F[3]; // fv = Coriolis vector f = 2 Omega; lbm_create's scalar f_cor is fv[2]
     int face[6];
-    int fp64, want_mean;
+    int fp64, s16, want_mean; // fp64: FP64 arithmetic and storage; s16: FP32 arithmetic, binary16 population storage
+    int precision;            // LBM_PREC_*
+    int device;               // the CUDA device the handle was created on; every ABI call runs there (DevGuard)
     Layout L;
     char *ws;       // device workspace
     bool own_ws;
@@ -111,6 +119,7 @@ struct lbm {
     double *modes() const { return (double *)(ws + L.off_modes); }
     void *damp() const { return ws + L.off_damp; }
     void *scratch() const { return ws + L.off_scratch; }
+    size_t pop_bytes() const { return (size_t)Q * (size_t)L.stride * (fp64 ? 8 : (s16 ? 2 : 4)); } // one population buffer
     size_t th_half() const { return (size_t)QT * (size_t)L.stride * (fp64 ? 8 : 4); }
     void *th_state() const { return thermal ? th_ws + (cur ? th_half() : 0) : nullptr; }
     void *th_other() const { return thermal ? th_ws + (cur ? 0 : th_half()) : nullptr; }
@@ -118,6 +127,22 @@ struct lbm {
 };
 
 namespace {
+
+// Every ABI call runs on the handle's device whatever the caller's current device is, and restores the latter.
+struct DevGuard {
+    int prev = 0;
+    bool sw = false;
+    explicit DevGuard(const lbm_t *h)
+    {
+        if (!h) return;
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return; }
+        sw = prev != h->device;
+        if (sw) cudaSetDevice(h->device);
+    }
+    ~DevGuard() { if (sw) cudaSetDevice(prev); }
+    DevGuard(const DevGuard &) = delete;
+    DevGuard &operator=(const DevGuard &) = delete;
+};
 
 int fail(lbm_t *h, int code, const std::string &msg)
 {
@@ -132,12 +157,20 @@ int fail(lbm_t *h, int code, const std::string &msg)
             return fail(h, LBM_ECUDA, std::string(#expr) + ": " + cudaGetErrorString(e_));            \
     } while (0)
 
+// arithmetic type / storage type of a handle: <double, double>, <float, float> or <float, __half>
+#define DISPATCH(h, fn, ...)                                                                            \
+    ((h)->fp64 ? fn<double, double>(__VA_ARGS__) : ((h)->s16 ? fn<float, __half>(__VA_ARGS__) : fn<float, float>(__VA_ARGS__)))
+#define DISPATCH_T(h, fn, T, ...)                                                                       \
+    ((h)->fp64 ? fn<double, double, T>(__VA_ARGS__)                                                     \
+               : ((h)->s16 ? fn<float, __half, T>(__VA_ARGS__) : fn<float, float, T>(__VA_ARGS__)))
+
 template <typename real>
 Params<real> make_params(const lbm_t *h)
 {
     Params<real> P{};
     P.nx = h->nx; P.ny = h->ny; P.nz = h->nz;
     P.px = h->L.px; P.py = h->L.py; P.pxy = h->L.px * h->L.py;
+    P.xoff = h->s16 ? 16 : 8; P.sec = h->s16 ? 16 : 8;
     P.Np = (int)h->L.Np;
     P.N = (int)h->N();
     P.nxy = h->nx * h->ny;
@@ -287,7 +320,7 @@ int check_launch(lbm_t *h, const char *what)
 
 // ---- templated implementations -----------------------------------------------------------------------------------
 
-template <typename real>
+template <typename real, typename S>
 int do_set_flags(lbm_t *h, const int32_t *height, const uint8_t *dev_mask = nullptr, int thresh = 1)
 {
     const Params<real> P = make_params<real>(h);
@@ -309,15 +342,15 @@ int do_set_flags(lbm_t *h, const int32_t *height, const uint8_t *dev_mask = null
     release_in(h, &in, 1);
     if (rc) return rc;
     const size_t rs = sizeof(real);
-    CUDA_TRY(h, cudaMemsetAsync(h->bufA(), 0, (size_t)Q * h->L.stride * rs, h->stream));
-    CUDA_TRY(h, cudaMemsetAsync(h->bufB(), 0, (size_t)Q * h->L.stride * rs, h->stream));
+    CUDA_TRY(h, cudaMemsetAsync(h->bufA(), 0, h->pop_bytes(), h->stream));
+    CUDA_TRY(h, cudaMemsetAsync(h->bufB(), 0, h->pop_bytes(), h->stream));
     if (h->want_mean) CUDA_TRY(h, cudaMemsetAsync(h->mean(), 0, (size_t)3 * h->L.stride * rs, h->stream));
     CUDA_TRY(h, cudaMemsetAsync(h->fu(), 0, h->L.fu_bytes, h->stream));
     h->cur = 0; h->step = 0; h->mcount = 0; h->have_flags = true;
     return LBM_OK;
 }
 
-template <typename real, typename in_t>
+template <typename real, typename S, typename in_t>
 int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, const in_t *w, size_t count)
 {
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inlet: flags not set");
@@ -332,8 +365,8 @@ int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, con
     if (!rc) {
         const int B = 256;
         const long long threads = mode == 0 ? (long long)P.N : (long long)count;
-        inlet_kernel<real, in_t><<<blocks_for(threads, B), B, 0, h->stream>>>(
-            (real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+        inlet_kernel<real, S, in_t><<<blocks_for(threads, B), B, 0, h->stream>>>(
+            (S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, mode, face, P);
         rc = check_launch(h, "inlet_kernel");
     }
@@ -345,14 +378,15 @@ template <typename in_t>
 int set_inlet_profile_any(lbm_t *h, const in_t *u, const in_t *v, const in_t *w)
 {
     if (!h) return LBM_EINVAL;
-    return h->fp64 ? do_set_inlet<double, in_t>(h, 0, 0, u, v, w, (size_t)h->nz)
-                   : do_set_inlet<float, in_t>(h, 0, 0, u, v, w, (size_t)h->nz);
+    DevGuard dg_(h);
+    return DISPATCH_T(h, do_set_inlet, in_t, h, 0, 0, u, v, w, (size_t)h->nz);
 }
 
 template <typename in_t>
 int set_inlet_plane_any(lbm_t *h, int face, const in_t *uvw)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (face < 0 || face > 5) return fail(h, LBM_EINVAL, "set_inlet_plane: face out of range");
     if (!uvw) return fail(h, LBM_EINVAL, "set_inlet_plane: uvw is NULL");
     const int axis = face / 2;
@@ -363,13 +397,12 @@ int set_inlet_plane_any(lbm_t *h, int face, const in_t *uvw)
     int rc = stage_in(h, uvw, 3 * cnt * sizeof(in_t), 0, &in);
     if (rc) return rc;
     const in_t *p = (const in_t *)in.dev;
-    rc = h->fp64 ? do_set_inlet<double, in_t>(h, 1, face, p, p + cnt, p + 2 * cnt, cnt)
-                 : do_set_inlet<float, in_t>(h, 1, face, p, p + cnt, p + 2 * cnt, cnt);
+    rc = DISPATCH_T(h, do_set_inlet, in_t, h, 1, face, p, p + cnt, p + 2 * cnt, cnt);
     release_in(h, &in, 1);
     return rc;
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_fluct(lbm_t *h, double t, bool cells);
 
 // Mesh voxeliser (lbm_mesh.cuh): vote counts of the three ray passes, in the first N bytes of the link-word area (free
@@ -413,10 +446,10 @@ int mesh_votes(lbm_t *h, int n_tri, const float *dev_tri, uint8_t **votes_out)
     *votes_out = votes;
     return LBM_OK;
 }
-template <typename real>
+template <typename real, typename S>
 int turb_publish(lbm_t *h, bool cells);
 
-template <typename real, typename in_t>
+template <typename real, typename S, typename in_t>
 int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, const in_t *uz)
 {
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_macros: flags not set");
@@ -428,36 +461,36 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     for (int k = 0; k < 4 && !rc; ++k) rc = stage_in(h, src[k], bytes, h->L.scratch_bytes, &in[k]); // never fits: temp
     if (!rc) {
         const int B = 256;
-        init_kernel<real, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+        init_kernel<real, S, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            (S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
         rc = check_launch(h, "init_kernel");
     }
     release_in(h, in, 4);
     if (!rc) { h->step = 0; h->cur = 0; }
-    if (!rc && h->nmodes > 0) rc = turb_publish<real>(h, true); // the step counter restarts: the inflow cells carry u'(x, 0)
+    if (!rc && h->nmodes > 0) rc = turb_publish<real, S>(h, true); // the step counter restarts: the inflow cells carry u'(x, 0)
     return rc;
 }
 
-template <typename real, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
+template <typename real, typename S, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
 int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
-    const real *A = (const real *)h->state();
-    real *B = (real *)h->other();
+    const S *A = (const S *)h->state();
+    S *B = (S *)h->other();
     real *ms = (real *)h->mean();
     dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
     // TURB: leading block rows that carry the face slots; they publish the boundary velocity of step (this one) + 1
     const int turb_planes = TURB ? (int)((blocks_for(P.F, BLOCK) + grid.x - 1) / grid.x) : 0;
     grid.y += turb_planes;
     const Turb<real> tb{(const real *)h->fum(), h->modes(), h->nmodes, (double)(h->step + 2)};
-    const StepPtrs<real> T = make_step_ptrs<real>(A, B, P);
+    const StepPtrs<S> T = make_step_ptrs<S>(A, B, P);
     // the side buffer's halves follow the population buffers: read the half written together with A, write B's
     const real *fur = (const real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
     real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
     // sampling steps hold three more values per thread (the prefetched sums): one CTA per SM less, 56 registers, no spills
     constexpr int MINB_S = (SPEC && MINB == 10) ? 9 : MINB;
-    if (sample) step_kernel<real, true, SPEC, BLOCK, MINB_S, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
-    else step_kernel<real, false, SPEC, BLOCK, MINB, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
+    if (sample) step_kernel<real, S, true, SPEC, BLOCK, MINB_S, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
+    else step_kernel<real, S, false, SPEC, BLOCK, MINB, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
     return check_launch(h, "step_kernel");
 }
 
@@ -474,27 +507,27 @@ bool vec_geom(const Params<float> &P, VecGeom *G)
         G->qmagic = (unsigned)((0x100000000ULL + G->qpr - 1) / G->qpr);
     return true;
 }
-template <int V, int MINB, int MINB_S>
+template <typename S, int V, int MINB, int MINB_S>
 int launch_step_vec(lbm_t *h, const Params<float> &P, const VecGeom &G, bool sample)
 {
     constexpr int BLOCK = 128;
-    const float *A = (const float *)h->state();
-    float *B = (float *)h->other();
+    const S *A = (const S *)h->state();
+    S *B = (S *)h->other();
     const dim3 grid(blocks_for((long long)G.nq, BLOCK), (unsigned)P.nz);
-    const VecPtrs<float> T = make_vec_ptrs<float>(A, B, P);
+    const VecPtrs<S> T = make_vec_ptrs<S>(A, B, P);
     const float *fur = (const float *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
     float *fuw = (float *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
-    if (sample) step_vec_kernel<float, V, true, BLOCK, MINB_S><<<grid, BLOCK, 0, h->stream>>>(h->flags(), h->links(), (float *)h->mean(), fur, fuw, P, T, G);
-    else step_vec_kernel<float, V, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(h->flags(), h->links(), nullptr, fur, fuw, P, T, G);
+    if (sample) step_vec_kernel<S, V, true, BLOCK, MINB_S><<<grid, BLOCK, 0, h->stream>>>(h->flags(), h->links(), (float *)h->mean(), fur, fuw, P, T, G);
+    else step_vec_kernel<S, V, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(h->flags(), h->links(), nullptr, fur, fuw, P, T, G);
     return check_launch(h, "step_vec_kernel");
 }
 
 // launch shapes of the FP32 step (lbm_set_variant): the same arithmetic and the same stored state in all of them
-//   0 = default: 4 cells per thread with 128-bit accesses where nx % 4 == 0, else one cell per thread; lattices whose whole
-//       grid is resident at once run several steps per cooperative launch (step_loop_kernel)
-//   1 = one cell per thread (32-bit accesses), one launch per step
-//   2 = 2 cells per thread with 64-bit accesses where nx % 2 == 0 (else as 1), one launch per step
-//   3 = 4 cells per thread with 128-bit accesses where nx % 4 == 0 (else as 1), one launch per step
+//   0 = default: one cell per thread; lattices whose whole grid is resident at once run several steps per cooperative
+//       launch (step_loop_kernel)
+//   1 = one cell per thread, one launch per step
+//   2 = 2 cells per thread with 64-bit accesses where nx % 2 == 0 (16-bit storage: 8 cells, 128-bit, nx % 8 == 0), else as 1
+//   3 = 4 cells per thread with 128-bit accesses (16-bit storage: 64-bit) where nx % 4 == 0, else as 1
 constexpr int N_VARIANTS = 4;
 #ifndef DAMP_MINB
 #define DAMP_MINB 9
@@ -505,10 +538,10 @@ constexpr int N_VARIANTS = 4;
 #ifndef VEC2_MINB
 #define VEC2_MINB 6
 #endif
-template <typename real>
+template <typename real, typename S>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
-    if (h->thermal) { // fused flow + thermal step (lbm_thermal.cuh)
+    if (h->thermal) { // fused flow + thermal step (lbm_thermal.cuh); S = real there (lbm_set_thermal refuses 16-bit storage)
         const real *A = (const real *)h->state();
         real *B = (real *)h->other();
         dim3 grid(blocks_for((long long)P.nxy, 128), (unsigned)P.nz);
@@ -522,50 +555,54 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
     const bool turb = h->nmodes > 0 && P.F > 0;
     if (h->damp_on || turb) { // damping zones / inflow fluctuations: their own instantiations (same arithmetic elsewhere)
         if constexpr (std::is_same<real, float>::value) {
-            if (h->damp_on && turb) return launch_step_as<real, true, 128, DAMP_MINB, true, true>(h, P, sample);
-            if (h->damp_on) return launch_step_as<real, true, 128, DAMP_MINB, true, false>(h, P, sample);
-            return launch_step_as<real, true, 128, 10, false, true>(h, P, sample); // no prefetched table values: 48 registers do
+            if (h->damp_on && turb) return launch_step_as<real, S, true, 128, DAMP_MINB, true, true>(h, P, sample);
+            if (h->damp_on) return launch_step_as<real, S, true, 128, DAMP_MINB, true, false>(h, P, sample);
+            return launch_step_as<real, S, true, 128, 10, false, true>(h, P, sample); // no prefetched table values: 48 registers do
         } else {
-            if (h->damp_on && turb) return launch_step_as<real, false, 256, 2, true, true>(h, P, sample);
-            if (h->damp_on) return launch_step_as<real, false, 256, 2, true, false>(h, P, sample);
-            return launch_step_as<real, false, 256, 2, false, true>(h, P, sample);
+            if (h->damp_on && turb) return launch_step_as<real, S, false, 256, 2, true, true>(h, P, sample);
+            if (h->damp_on) return launch_step_as<real, S, false, 256, 2, true, false>(h, P, sample);
+            return launch_step_as<real, S, false, 256, 2, false, true>(h, P, sample);
         }
     }
     if constexpr (std::is_same<real, float>::value) {
         VecGeom G;
-        if ((h->variant == 0 || h->variant == 3) && vec_geom<4>(P, &G)) return launch_step_vec<4, VEC4_MINB, 3>(h, P, G, sample);
-        if (h->variant == 2 && vec_geom<2>(P, &G)) return launch_step_vec<2, VEC2_MINB, 5>(h, P, G, sample);
-        return launch_step_as<real, true, 128, 10>(h, P, sample);
-    } else return launch_step_as<real, false, 256, 2>(h, P, sample);
+        if (h->variant == 3 && vec_geom<4>(P, &G)) return launch_step_vec<S, 4, VEC4_MINB, 3>(h, P, G, sample);
+        if constexpr (std::is_same<S, float>::value) {
+            if (h->variant == 2 && vec_geom<2>(P, &G)) return launch_step_vec<S, 2, VEC2_MINB, 5>(h, P, G, sample);
+        } else {
+            if (h->variant == 2 && vec_geom<8>(P, &G)) return launch_step_vec<S, 8, 2, 2>(h, P, G, sample);
+        }
+        return launch_step_as<real, S, true, 128, 10>(h, P, sample);
+    } else return launch_step_as<real, S, false, 256, 2>(h, P, sample);
 }
 
 // boundary velocities of time t for the EQ_FIXED slots (mean + fluctuations on active inflow cells); cells = also rewrite
 // the cells' populations (set-up / switch-off / re-initialisation)
-template <typename real>
+template <typename real, typename S>
 int do_fluct(lbm_t *h, double t, bool cells)
 {
     const Params<real> P = make_params<real>(h);
     if (P.F == 0) return LBM_OK;
     const int B = 128;
     const Turb<real> tb{(const real *)h->fum(), h->modes(), h->nmodes, t};
-    if (cells) fluct_kernel<real, true><<<blocks_for(P.F, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), tb, P);
-    else fluct_kernel<real, false><<<blocks_for(P.F, B), B, 0, h->stream>>>(nullptr, nullptr, (real *)h->fu(), h->flags(), tb, P);
+    if (cells) fluct_kernel<real, S, true><<<blocks_for(P.F, B), B, 0, h->stream>>>((S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), tb, P);
+    else fluct_kernel<real, S, false><<<blocks_for(P.F, B), B, 0, h->stream>>>((S *)nullptr, (S *)nullptr, (real *)h->fu(), h->flags(), tb, P);
     return check_launch(h, "fluct_kernel");
 }
 
 // Fluctuations on: the EQ_FIXED cells hold u_b(step) and both halves of the side array u_b(step + 1), which the next
 // launch re-expands; from then on every launch publishes the velocity of the step after its own (TURB blocks).
-template <typename real>
+template <typename real, typename S>
 int turb_publish(lbm_t *h, bool cells)
 {
-    int rc = cells ? do_fluct<real>(h, (double)h->step, true) : LBM_OK;
-    if (!rc) rc = do_fluct<real>(h, (double)(h->step + 1), false);
+    int rc = cells ? do_fluct<real, S>(h, (double)h->step, true) : LBM_OK;
+    if (!rc) rc = do_fluct<real, S>(h, (double)(h->step + 1), false);
     return rc;
 }
 
 // Small lattices (the whole grid resident at once): 2 * pairs steps in one cooperative launch (step_loop_kernel).
 // Returns the number of steps done (0 = not applicable here: use single launches), or a negative error code.
-template <typename real>
+template <typename real, typename S>
 int try_step_loop(lbm_t *h, const Params<real> &P, int want)
 {
     if constexpr (!std::is_same<real, float>::value) return 0;
@@ -573,7 +610,7 @@ int try_step_loop(lbm_t *h, const Params<real> &P, int want)
         if (h->variant != 0 || h->nmodes > 0 || h->thermal || want < 4 || h->loop_ok < 0) return 0;
         constexpr int BLOCK = 128;
         const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
-        const void *fn = h->damp_on ? (const void *)step_loop_kernel<float, BLOCK, 10, true> : (const void *)step_loop_kernel<float, BLOCK, 10, false>;
+        const void *fn = h->damp_on ? (const void *)step_loop_kernel<float, S, BLOCK, 10, true> : (const void *)step_loop_kernel<float, S, BLOCK, 10, false>;
         if (h->loop_ok == 0) { // once per handle: can the whole grid be resident?
             int dev = 0, sms = 0, coop = 0, per_sm = 0;
             cudaGetDevice(&dev);
@@ -585,9 +622,9 @@ int try_step_loop(lbm_t *h, const Params<real> &P, int want)
             if (h->loop_ok < 0) return 0;
         }
         int pairs = want / 2;
-        real *A = (real *)h->state(), *B = (real *)h->other();
+        S *A = (S *)h->state(), *B = (S *)h->other();
         real *fu0 = (real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F, *fu1 = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
-        StepPtrs<real> T0 = make_step_ptrs<real>(A, B, P), T1 = make_step_ptrs<real>(B, A, P);
+        StepPtrs<S> T0 = make_step_ptrs<S>(A, B, P), T1 = make_step_ptrs<S>(B, A, P);
         const uint8_t *fl = h->flags();
         const uint32_t *lk = h->links();
         Params<real> Pc = P;
@@ -599,7 +636,7 @@ int try_step_loop(lbm_t *h, const Params<real> &P, int want)
     }
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_step(lbm_t *h, int n)
 {
     const Params<real> P = make_params<real>(h);
@@ -611,13 +648,13 @@ int do_step(lbm_t *h, int n)
                 long ks = k0 <= h->mstart ? h->mstart : h->mstart + ((k0 - h->mstart + h->mevery - 1) / h->mevery) * h->mevery;
                 run = std::min(run, ks - k0); // steps k0 .. ks-1 do not sample
             }
-            const int done = run >= 4 ? try_step_loop<real>(h, P, (int)std::min(run, 1000000L)) : 0;
+            const int done = run >= 4 ? try_step_loop<real, S>(h, P, (int)std::min(run, 1000000L)) : 0;
             if (done < 0) return done;
             if (done > 0) { h->step += done; it += done - 1; continue; }
         }
         const long k = h->step + 1;
         const bool sample = h->mevery > 0 && k >= h->mstart && (k - h->mstart) % h->mevery == 0;
-        int rc = launch_step<real>(h, P, sample);
+        int rc = launch_step<real, S>(h, P, sample);
         if (rc) return rc;
         h->cur ^= 1;
         h->step = k;
@@ -626,7 +663,7 @@ int do_step(lbm_t *h, int n)
     return LBM_OK;
 }
 
-template <typename real, typename out_t>
+template <typename real, typename S, typename out_t>
 int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
 {
     if (!h->have_flags) return fail(h, LBM_ESTATE, "get_macros: flags not set");
@@ -638,8 +675,8 @@ int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
     for (; staged < 4 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)P.N * sizeof(out_t), &o[staged]);
     if (!rc) {
         const int B = 256;
-        macros_kernel<real, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (const real *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
+        macros_kernel<real, S, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            (const S *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
             (const real *)h->th_state());
         rc = check_launch(h, "macros_kernel");
     }
@@ -647,7 +684,7 @@ int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
     return rc ? rc : rc2;
 }
 
-template <typename real, typename out_t>
+template <typename real, typename S, typename out_t>
 int do_get_mean(lbm_t *h, out_t *ux, out_t *uy, out_t *uz, long *n_samples)
 {
     if (!h->want_mean) return fail(h, LBM_ESTATE, "get_mean: handle created without mean sums");
@@ -669,7 +706,7 @@ int do_get_mean(lbm_t *h, out_t *ux, out_t *uy, out_t *uz, long *n_samples)
     return rc ? rc : rc2;
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_get_links(lbm_t *h, uint32_t *links)
 {
     const Params<real> P = make_params<real>(h);
@@ -683,7 +720,7 @@ int do_get_links(lbm_t *h, uint32_t *links)
     return rc ? rc : rc2;
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_get_state(lbm_t *h, double *f)
 {
     const Params<real> P = make_params<real>(h);
@@ -691,13 +728,13 @@ int do_get_state(lbm_t *h, double *f)
     int rc = stage_out(h, f, (size_t)Q * P.N * sizeof(double), &o);
     if (rc) return rc;
     const int B = 256;
-    state_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->state(), h->flags(), (double *)o.dev, P);
+    state_out_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), h->flags(), (double *)o.dev, P);
     rc = check_launch(h, "state_out_kernel");
     int rc2 = finish_out(h, &o, 1);
     return rc ? rc : rc2;
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_set_state(lbm_t *h, const double *f)
 {
     const Params<real> P = make_params<real>(h);
@@ -705,7 +742,7 @@ int do_set_state(lbm_t *h, const double *f)
     int rc = stage_in(h, f, (size_t)Q * P.N * sizeof(double), h->L.scratch_bytes, &in);
     if (rc) return rc;
     const int B = 256;
-    state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), h->links(),
+    state_in_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), h->links(),
                                                                     (const double *)in.dev, P);
     rc = check_launch(h, "state_in_kernel");
     release_in(h, &in, 1);
@@ -713,7 +750,7 @@ int do_set_state(lbm_t *h, const double *f)
     return rc;
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_balance_flux(lbm_t *h, double *before, double *after)
 {
     const Params<real> P = make_params<real>(h);
@@ -726,7 +763,7 @@ int do_balance_flux(lbm_t *h, double *before, double *after)
         flux_sum_kernel<real><<<grid, B, 0, h->stream>>>((const real *)h->fu(), h->flags(), acc, P);
         int rc = check_launch(h, "flux_sum_kernel");
         if (rc) return rc;
-        flux_apply_kernel<real><<<grid, B, 0, h->stream>>>((real *)h->bufA(), (real *)h->bufB(), (real *)h->fu(), h->flags(), acc, P);
+        flux_apply_kernel<real, S><<<grid, B, 0, h->stream>>>((S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), acc, P);
         rc = check_launch(h, "flux_apply_kernel");
         if (rc) return rc;
         flux_sum_kernel<real><<<grid, B, 0, h->stream>>>((const real *)h->fu(), h->flags(), acc + 2, P);
@@ -740,23 +777,32 @@ int do_balance_flux(lbm_t *h, double *before, double *after)
     return LBM_OK;
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_refeed(lbm_t *h)
 {
     const Params<real> P = make_params<real>(h);
     if (P.F == 0) return LBM_OK;
     const int B = 256;
-    refeed_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->state(), (real *)h->fu(), h->flags(), P);
+    refeed_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), (real *)h->fu(), h->flags(), P);
     return check_launch(h, "refeed_kernel");
 }
 
-template <typename real>
+template <typename real, typename S>
 int do_feed(lbm_t *dst, const lbm_t *src, int sx)
 {
-    const Params<real> D = make_params<real>(dst), S = make_params<real>(src);
+    const Params<real> D = make_params<real>(dst), Ps = make_params<real>(src);
     const int B = 128;
-    feed_kernel<real><<<blocks_for((long long)D.ny * D.nz, B), B, 0, dst->stream>>>(
-        (real *)dst->bufA(), (real *)dst->bufB(), (real *)dst->fu(), dst->flags(), D, (const real *)src->state(), src->flags(), S, sx);
+    if (src->stream != dst->stream) {
+        // the plane is read on dst's stream: order it after everything queued on src's stream (the precursor's last step)
+        cudaEvent_t ev;
+        CUDA_TRY(dst, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
+        cudaError_t e = cudaEventRecord(ev, src->stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(dst->stream, ev, 0);
+        cudaEventDestroy(ev); // released once the recorded work has completed
+        if (e != cudaSuccess) return fail(dst, LBM_ECUDA, std::string("feed_inlet: ") + cudaGetErrorString(e));
+    }
+    feed_kernel<real, S><<<blocks_for((long long)D.ny * D.nz, B), B, 0, dst->stream>>>(
+        (S *)dst->bufA(), (S *)dst->bufB(), (real *)dst->fu(), dst->flags(), D, (const S *)src->state(), src->flags(), Ps, sx);
     return check_launch(dst, "feed_kernel");
 }
 
@@ -764,7 +810,7 @@ int do_feed(lbm_t *dst, const lbm_t *src, int sx)
 
 // ---- C ABI -------------------------------------------------------------------------------------------------------------
 
-template <typename real, typename in_t>
+template <typename real, typename S, typename in_t>
 int do_set_theta(lbm_t *h, const in_t *theta, const in_t *ux, const in_t *uy, const in_t *uz)
 {
     const Params<real> P = make_params<real>(h);
@@ -789,12 +835,13 @@ template <typename in_t>
 int set_theta_any(lbm_t *h, const in_t *theta, const in_t *ux, const in_t *uy, const in_t *uz)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!h->thermal) return fail(h, LBM_ESTATE, "set_theta: thermal lattice is off (lbm_set_thermal)");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_theta: flags not set");
-    return h->fp64 ? do_set_theta<double, in_t>(h, theta, ux, uy, uz) : do_set_theta<float, in_t>(h, theta, ux, uy, uz);
+    return DISPATCH_T(h, do_set_theta, in_t, h, theta, ux, uy, uz);
 }
 
-template <typename real, typename out_t>
+template <typename real, typename S, typename out_t>
 int do_get_theta(lbm_t *h, out_t *theta)
 {
     const Params<real> P = make_params<real>(h);
@@ -813,9 +860,35 @@ template <typename out_t>
 int get_theta_any(lbm_t *h, out_t *theta)
 {
     if (!h || !theta) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!h->thermal) return fail(h, LBM_ESTATE, "get_theta: thermal lattice is off (lbm_set_thermal)");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "get_theta: flags not set");
-    return h->fp64 ? do_get_theta<double, out_t>(h, theta) : do_get_theta<float, out_t>(h, theta);
+    return DISPATCH_T(h, do_get_theta, out_t, h, theta);
+}
+
+template <typename real>
+int do_thermal_state(lbm_t *h, double *out, const double *in)
+{
+    const Params<real> P = make_params<real>(h);
+    const size_t bytes = (size_t)QT * P.N * sizeof(double);
+    const int B = 256;
+    if (out) {
+        OutBuf o;
+        int rc = stage_out(h, out, bytes, &o);
+        if (rc) return rc;
+        thermal_state_out_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>((const real *)h->th_state(), h->flags(), (double *)o.dev, P);
+        rc = check_launch(h, "thermal_state_out_kernel");
+        int rc2 = finish_out(h, &o, 1);
+        return rc ? rc : rc2;
+    }
+    InBuf ib;
+    int rc = stage_in(h, in, bytes, h->L.scratch_bytes, &ib);
+    if (rc) return rc;
+    real *H0 = (real *)h->th_ws, *H1 = (real *)(h->th_ws + h->th_half());
+    thermal_state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(H0, H1, h->flags(), h->links(), (const double *)ib.dev, P);
+    rc = check_launch(h, "thermal_state_in_kernel");
+    release_in(h, &ib, 1);
+    return rc;
 }
 
 bool has_eq_face(const int face[6])
@@ -830,8 +903,10 @@ extern "C" {
 int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!(alpha > 0.0) || !std::isfinite(alpha) || !std::isfinite(g_beta) || !std::isfinite(theta_ref))
         return fail(h, LBM_EINVAL, "set_thermal: alpha must be > 0 and all arguments finite");
+    if (h->s16) return fail(h, LBM_EINVAL, "set_thermal: not combinable with 16-bit population storage");
     if (has_eq_face(h->face)) return fail(h, LBM_EINVAL, "set_thermal: EQ_FIXED / EQ_OUTFLOW faces are not supported with the thermal lattice");
     if (h->damp_on || h->nmodes > 0) return fail(h, LBM_EINVAL, "set_thermal: not combinable with damping zones / inflow fluctuations");
     if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half()));
@@ -842,22 +917,40 @@ int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
 }
 int lbm_set_theta(lbm_t *h, const float *theta, const float *ux, const float *uy, const float *uz) { return set_theta_any<float>(h, theta, ux, uy, uz); }
 int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const double *uy, const double *uz) { return set_theta_any<double>(h, theta, ux, uy, uz); }
+int lbm_get_thermal_state(lbm_t *h, double *hpop)
+{
+    if (!h || !hpop) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!h->thermal) return fail(h, LBM_ESTATE, "get_thermal_state: thermal lattice is off (lbm_set_thermal)");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_thermal_state: flags not set");
+    return h->fp64 ? do_thermal_state<double>(h, hpop, nullptr) : do_thermal_state<float>(h, hpop, nullptr);
+}
+int lbm_set_thermal_state(lbm_t *h, const double *hpop)
+{
+    if (!h || !hpop) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!h->thermal) return fail(h, LBM_ESTATE, "set_thermal_state: thermal lattice is off (lbm_set_thermal)");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_thermal_state: flags not set");
+    return h->fp64 ? do_thermal_state<double>(h, nullptr, hpop) : do_thermal_state<float>(h, nullptr, hpop);
+}
 int lbm_get_theta(lbm_t *h, float *theta) { return get_theta_any<float>(h, theta); }
 int lbm_get_theta_f64(lbm_t *h, double *theta) { return get_theta_any<double>(h, theta); }
 
-int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int fp64, size_t *out)
+int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int precision, size_t *out)
 {
     if (!out || !size_ok(nx, ny, nz)) return LBM_EINVAL;
-    *out = make_layout(nx, ny, nz, want_mean, fp64).total;
+    if (precision != LBM_PREC_F32 && precision != LBM_PREC_F64 && precision != LBM_PREC_F32_S16) return LBM_EINVAL;
+    *out = make_layout(nx, ny, nz, want_mean, precision).total;
     return LBM_OK;
 }
 
 int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3], void *dev_workspace,
-                  size_t workspace_bytes, void *cuda_stream, int fp64, int want_mean, lbm_t **out)
+                  size_t workspace_bytes, void *cuda_stream, int precision, int want_mean, lbm_t **out)
 {
     if (!out) return LBM_EINVAL;
     *out = nullptr;
     if (!size_ok(nx, ny, nz)) return LBM_EINVAL;
+    if (precision != LBM_PREC_F32 && precision != LBM_PREC_F64 && precision != LBM_PREC_F32_S16) return LBM_EINVAL;
     if (!(nu0 > 0.0) || Cs < 0.0 || !std::isfinite(nu0) || !std::isfinite(Cs) || !std::isfinite(f_cor)) return LBM_EINVAL;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); return LBM_ECUDA; }
@@ -868,9 +961,11 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     for (int a = 0; a < 3; ++a) h->F[a] = F ? F[a] : 0.0;
     const int def[6] = {LBM_EQ_FIXED, LBM_EQ_OUTFLOW, LBM_PERIODIC, LBM_PERIODIC, LBM_WALL, LBM_FREE_SLIP};
     for (int k = 0; k < 6; ++k) h->face[k] = def[k];
-    h->fp64 = fp64 ? 1 : 0; h->want_mean = want_mean ? 1 : 0;
-    h->L = make_layout(nx, ny, nz, h->want_mean, h->fp64);
+    h->precision = precision; h->fp64 = precision == LBM_PREC_F64; h->s16 = precision == LBM_PREC_F32_S16;
+    h->want_mean = want_mean ? 1 : 0;
+    h->L = make_layout(nx, ny, nz, h->want_mean, precision);
     h->stream = (cudaStream_t)cuda_stream;
+    if (cudaGetDevice(&h->device) != cudaSuccess) { cudaGetLastError(); delete h; return LBM_ECUDA; }
     h->cur = 0; h->have_flags = false; h->step = 0;
     h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false; h->nmodes = 0; h->loop_ok = 0;
     h->thermal = false; h->alpha = 0; h->gbeta = 0; h->theta_ref = 0; h->th_ws = nullptr;
@@ -900,6 +995,7 @@ int lbm_create(int nx, int ny, int nz, double nu0, double Cs, double f_cor, cons
 int lbm_destroy(lbm_t *h)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     cudaStreamSynchronize(h->stream);
     if (h->own_ws) cudaFree(h->ws);
     if (h->th_ws) cudaFree(h->th_ws);
@@ -912,6 +1008,7 @@ int lbm_destroy(lbm_t *h)
 int lbm_set_boundaries(lbm_t *h, const int face_type[6])
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!face_type) return fail(h, LBM_EINVAL, "set_boundaries: NULL");
     for (int a = 0; a < 3; ++a) {
         const int lo = face_type[2 * a], hi = face_type[2 * a + 1];
@@ -927,6 +1024,7 @@ int lbm_set_boundaries(lbm_t *h, const int face_type[6])
 int lbm_set_coriolis(lbm_t *h, const double f[3])
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!f) return fail(h, LBM_EINVAL, "set_coriolis: NULL");
     for (int a = 0; a < 3; ++a)
         if (!std::isfinite(f[a])) return fail(h, LBM_EINVAL, "set_coriolis: not finite");
@@ -937,6 +1035,7 @@ int lbm_set_coriolis(lbm_t *h, const double f[3])
 int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const double *target)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!width || !peak) return fail(h, LBM_EINVAL, "set_damping: NULL");
     if (h->thermal) return fail(h, LBM_EINVAL, "set_damping: not combinable with the thermal lattice");
     bool any = false;
@@ -945,7 +1044,7 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
         any |= width[k] > 0 && peak[k] > 0.0;
     }
     // the outflow cells' next velocities are local macros of the current state: re-evaluate them under the new zones
-    auto refeed = [&]() { return !h->have_flags ? LBM_OK : (h->fp64 ? do_refeed<double>(h) : do_refeed<float>(h)); };
+    auto refeed = [&]() { return !h->have_flags ? LBM_OK : (DISPATCH(h, do_refeed, h)); };
     if (!any) {
         const bool was = h->damp_on;
         h->damp_on = false;
@@ -997,9 +1096,10 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
 int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double u_rms, double k_e, double k_eta)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inflow_turbulence: flags not set");
     if (n_modes < 0 || n_modes > MAX_MODES) return fail(h, LBM_EINVAL, "set_inflow_turbulence: n_modes out of range");
-    auto rewrite = [&]() { return h->fp64 ? turb_publish<double>(h, true) : turb_publish<float>(h, true); };
+    auto rewrite = [&]() { return DISPATCH(h, turb_publish, h, true); };
     if (n_modes == 0) {
         if (h->nmodes == 0) return LBM_OK;
         h->nmodes = 0;
@@ -1039,6 +1139,7 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
 int lbm_set_flags_mask(lbm_t *h, const int32_t *height, const uint8_t *solid)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!solid) return lbm_set_flags(h, height);
     h->nmodes = 0;
     const uint8_t *dev = solid;
@@ -1046,7 +1147,7 @@ int lbm_set_flags_mask(lbm_t *h, const int32_t *height, const uint8_t *solid)
         CUDA_TRY(h, cudaMemcpyAsync(h->links(), solid, (size_t)h->N(), cudaMemcpyHostToDevice, h->stream));
         dev = (const uint8_t *)h->links();
     }
-    int rc = h->fp64 ? do_set_flags<double>(h, height, dev, 1) : do_set_flags<float>(h, height, dev, 1);
+    int rc = DISPATCH(h, do_set_flags, h, height, dev, 1);
     if (!rc && dev != solid) CUDA_TRY(h, cudaStreamSynchronize(h->stream)); // the caller's buffer is free on return
     return rc;
 }
@@ -1054,6 +1155,7 @@ int lbm_set_flags_mask(lbm_t *h, const int32_t *height, const uint8_t *solid)
 int lbm_set_flags_mesh(lbm_t *h, const int32_t *height, int n_tri, const float *tri, int min_votes)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (n_tri < 0 || (n_tri > 0 && !tri)) return fail(h, LBM_EINVAL, "set_flags_mesh: bad triangle array");
     if (min_votes < 1 || min_votes > 3) return fail(h, LBM_EINVAL, "set_flags_mesh: min_votes must be 1, 2 or 3");
     h->nmodes = 0;
@@ -1065,14 +1167,15 @@ int lbm_set_flags_mesh(lbm_t *h, const int32_t *height, int n_tri, const float *
     release_in(h, &in, 1);
     if (rc) return rc;
     // the heightmap staging of do_set_flags may reuse the scratch area now: the triangles are consumed
-    return h->fp64 ? do_set_flags<double>(h, height, votes, min_votes) : do_set_flags<float>(h, height, votes, min_votes);
+    return DISPATCH(h, do_set_flags, h, height, votes, min_votes);
 }
 
 int lbm_set_flags(lbm_t *h, const int32_t *height)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     h->nmodes = 0; // a new voxelisation resets the state and the boundary velocities
-    return h->fp64 ? do_set_flags<double>(h, height) : do_set_flags<float>(h, height);
+    return DISPATCH(h, do_set_flags, h, height);
 }
 
 int lbm_set_inlet_profile(lbm_t *h, const float *u, const float *v, const float *w) { return set_inlet_profile_any<float>(h, u, v, w); }
@@ -1083,44 +1186,50 @@ int lbm_set_inlet_plane_f64(lbm_t *h, int face, const double *uvw) { return set_
 int lbm_feed_inlet(lbm_t *dst, const lbm_t *src, int src_x_plane)
 {
     if (!dst || !src) return LBM_EINVAL;
+    DevGuard dg_(dst);
     if (!dst->have_flags || !src->have_flags) return fail(dst, LBM_ESTATE, "feed_inlet: flags not set");
     if (dst->nmodes > 0) return fail(dst, LBM_ESTATE, "feed_inlet: the mean boundary state is fixed while inflow fluctuations are on");
-    if (dst->fp64 != src->fp64) return fail(dst, LBM_EINVAL, "feed_inlet: precision mismatch");
+    if (dst->precision != src->precision) return fail(dst, LBM_EINVAL, "feed_inlet: precision mismatch");
     if (dst->nz != src->nz) return fail(dst, LBM_EINVAL, "feed_inlet: nz mismatch");
     if (src_x_plane < 0 || src_x_plane >= src->nx) return fail(dst, LBM_EINVAL, "feed_inlet: plane out of range");
-    return dst->fp64 ? do_feed<double>(dst, src, src_x_plane) : do_feed<float>(dst, src, src_x_plane);
+    return DISPATCH(dst, do_feed, dst, src, src_x_plane);
 }
 
 int lbm_balance_flux(lbm_t *h, double *flux_before, double *flux_after)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!h->have_flags) return fail(h, LBM_ESTATE, "balance_flux: flags not set");
     if (h->nmodes > 0) return fail(h, LBM_ESTATE, "balance_flux: the mean boundary state is fixed while inflow fluctuations are on");
-    return h->fp64 ? do_balance_flux<double>(h, flux_before, flux_after) : do_balance_flux<float>(h, flux_before, flux_after);
+    return DISPATCH(h, do_balance_flux, h, flux_before, flux_after);
 }
 
 int lbm_set_macros(lbm_t *h, const float *rho, const float *ux, const float *uy, const float *uz)
 {
     if (!h) return LBM_EINVAL;
-    return h->fp64 ? do_set_macros<double, float>(h, rho, ux, uy, uz) : do_set_macros<float, float>(h, rho, ux, uy, uz);
+    DevGuard dg_(h);
+    return DISPATCH_T(h, do_set_macros, float, h, rho, ux, uy, uz);
 }
 int lbm_set_macros_f64(lbm_t *h, const double *rho, const double *ux, const double *uy, const double *uz)
 {
     if (!h) return LBM_EINVAL;
-    return h->fp64 ? do_set_macros<double, double>(h, rho, ux, uy, uz) : do_set_macros<float, double>(h, rho, ux, uy, uz);
+    DevGuard dg_(h);
+    return DISPATCH_T(h, do_set_macros, double, h, rho, ux, uy, uz);
 }
 
 int lbm_step(lbm_t *h, int n)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (n < 0) return fail(h, LBM_EINVAL, "step: n < 0");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "step: flags not set");
-    return h->fp64 ? do_step<double>(h, n) : do_step<float>(h, n);
+    return DISPATCH(h, do_step, h, n);
 }
 
 int lbm_mean_config(lbm_t *h, long start_step, int every)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!h->want_mean) return fail(h, LBM_ESTATE, "mean_config: handle created without mean sums");
     if (every < 0 || start_step < 0) return fail(h, LBM_EINVAL, "mean_config: negative argument");
     h->mstart = start_step; h->mevery = every;
@@ -1130,6 +1239,7 @@ int lbm_mean_config(lbm_t *h, long start_step, int every)
 int lbm_mean_reset(lbm_t *h)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!h->want_mean) return fail(h, LBM_ESTATE, "mean_reset: handle created without mean sums");
     CUDA_TRY(h, cudaMemsetAsync(h->mean(), 0, (size_t)3 * h->L.stride * (h->fp64 ? 8 : 4), h->stream));
     h->mcount = 0;
@@ -1139,28 +1249,33 @@ int lbm_mean_reset(lbm_t *h)
 int lbm_get_macros(lbm_t *h, float *rho, float *ux, float *uy, float *uz)
 {
     if (!h) return LBM_EINVAL;
-    return h->fp64 ? do_get_macros<double, float>(h, rho, ux, uy, uz) : do_get_macros<float, float>(h, rho, ux, uy, uz);
+    DevGuard dg_(h);
+    return DISPATCH_T(h, do_get_macros, float, h, rho, ux, uy, uz);
 }
 int lbm_get_macros_f64(lbm_t *h, double *rho, double *ux, double *uy, double *uz)
 {
     if (!h) return LBM_EINVAL;
-    return h->fp64 ? do_get_macros<double, double>(h, rho, ux, uy, uz) : do_get_macros<float, double>(h, rho, ux, uy, uz);
+    DevGuard dg_(h);
+    return DISPATCH_T(h, do_get_macros, double, h, rho, ux, uy, uz);
 }
 
 int lbm_get_mean(lbm_t *h, float *ux, float *uy, float *uz, long *n_samples)
 {
     if (!h) return LBM_EINVAL;
-    return h->fp64 ? do_get_mean<double, float>(h, ux, uy, uz, n_samples) : do_get_mean<float, float>(h, ux, uy, uz, n_samples);
+    DevGuard dg_(h);
+    return DISPATCH_T(h, do_get_mean, float, h, ux, uy, uz, n_samples);
 }
 int lbm_get_mean_f64(lbm_t *h, double *ux, double *uy, double *uz, long *n_samples)
 {
     if (!h) return LBM_EINVAL;
-    return h->fp64 ? do_get_mean<double, double>(h, ux, uy, uz, n_samples) : do_get_mean<float, double>(h, ux, uy, uz, n_samples);
+    DevGuard dg_(h);
+    return DISPATCH_T(h, do_get_mean, double, h, ux, uy, uz, n_samples);
 }
 
 int lbm_get_flags(lbm_t *h, uint8_t *flags)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!flags) return fail(h, LBM_EINVAL, "get_flags: NULL");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "get_flags: flags not set");
     OutBuf o;
@@ -1177,27 +1292,30 @@ int lbm_get_flags(lbm_t *h, uint8_t *flags)
 int lbm_get_links(lbm_t *h, uint32_t *links)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!links) return fail(h, LBM_EINVAL, "get_links: NULL");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "get_links: flags not set");
-    return h->fp64 ? do_get_links<double>(h, links) : do_get_links<float>(h, links);
+    return DISPATCH(h, do_get_links, h, links);
 }
 
 int lbm_get_state(lbm_t *h, double *f)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!f) return fail(h, LBM_EINVAL, "get_state: NULL");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "get_state: flags not set");
-    return h->fp64 ? do_get_state<double>(h, f) : do_get_state<float>(h, f);
+    return DISPATCH(h, do_get_state, h, f);
 }
 
 int lbm_set_state(lbm_t *h, const double *f)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (!f) return fail(h, LBM_EINVAL, "set_state: NULL");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_state: flags not set");
-    int rc = h->fp64 ? do_set_state<double>(h, f) : do_set_state<float>(h, f);
+    int rc = DISPATCH(h, do_set_state, h, f);
     // the state brought its own boundary cells; the next launch must still find u_b(step + 1) in the side array
-    if (!rc && h->nmodes > 0) rc = h->fp64 ? turb_publish<double>(h, false) : turb_publish<float>(h, false);
+    if (!rc && h->nmodes > 0) rc = DISPATCH(h, turb_publish, h, false);
     return rc;
 }
 
@@ -1205,14 +1323,16 @@ long lbm_get_step(const lbm_t *h) { return h ? h->step : -1; }
 int lbm_set_step(lbm_t *h, long step)
 {
     if (!h || step < 0) return LBM_EINVAL;
+    DevGuard dg_(h);
     h->step = step;
-    if (h->nmodes > 0 && h->have_flags) return h->fp64 ? turb_publish<double>(h, false) : turb_publish<float>(h, false);
+    if (h->nmodes > 0 && h->have_flags) return DISPATCH(h, turb_publish, h, false);
     return LBM_OK;
 }
 
 int lbm_sync(lbm_t *h)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     return LBM_OK;
 }
@@ -1233,6 +1353,7 @@ int lbm_lattice(int *c, int *opposite)
 int lbm_set_variant(lbm_t *h, int variant)
 {
     if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
     if (variant < 0 || variant >= N_VARIANTS) return fail(h, LBM_EINVAL, "set_variant: unknown variant");
     h->variant = variant;
     return LBM_OK;

@@ -5,6 +5,9 @@
 // at padded x = 8, x pitch rounded up to 32 cells (every row is 128-byte aligned).  g_i = f_i - w_i ("shifted": the rest
 // state is exactly 0, stored numbers are O(Ma), FP32 rounding stays two orders below the 1e-5 parity bar).
 // Two buffers A/B, pull scheme: every FLUID cell reads A[i][p - off_i] for ALL i with no case distinction.
+// Storage type S of the populations: the arithmetic type `real` (float / double), or __half with FP32 arithmetic
+// (lbm_create_ex precision 2; binary16 of the shifted population, rounded to nearest even at every store).
+// Rows start on a 32-byte sector: interior x = 0 sits at padded x = P.xoff (8 cells; 16 for __half).
 //
 // What makes that possible is a write-side boundary rule ("mailboxes").  A population j that leaves cell x
 // towards a cell that cannot be pulled from is stored, by x itself, where the pull of the next step will look:
@@ -17,6 +20,7 @@
 #include <cstdint>
 #include <type_traits>
 #include <cuda_runtime.h>
+#include <cuda_fp16.h>
 
 namespace lbmk {
 
@@ -59,7 +63,8 @@ __host__ __device__ __forceinline__ void static_for(F &&f)
 template <typename real>
 struct Params {
     int nx, ny, nz;   // interior cells
-    int px, py, pxy;  // padded x pitch (multiple of 32, >= nx + XOFF + 1), padded rows per plane (ny + 2), px * py
+    int px, py, pxy;  // padded x pitch (multiple of 32, >= nx + xoff + 1), padded rows per plane (ny + 2), px * py
+    int xoff, sec;    // padded x of interior x = 0 (one 32-byte sector of storage elements), cells per 32-byte sector (8; 16 for __half)
     int Np;           // padded cells = pxy * (nz + 2)
     int N;            // interior cells
     int nxy;          // nx * ny
@@ -82,14 +87,16 @@ struct Params {
     real gbeta, theta_ref, omega_t;
 };
 
-// Interior x = 0 sits at padded x = XOFF = 8: every interior row starts on a 32-byte sector boundary (and ends on one
-// when nx % 8 == 0), so full-row stores never leave partially written sectors, which would cost a DRAM fill read each.
-constexpr int XOFF = 8;
+// Interior x = 0 sits at padded x = P.xoff (8 cells of 4 or 8 bytes, 16 cells of 2): every interior row starts on a
+// 32-byte sector boundary (and ends on one when nx % P.sec == 0), so full-row stores never leave partially written
+// sectors, which would cost a DRAM fill read each.
+template <typename S>
+constexpr int xoff_for() { return sizeof(S) == 2 ? 16 : 8; }
 // padded linear index of interior cell (x,y,z); also valid for halo coordinates -1 and n
 template <typename real>
 __host__ __device__ __forceinline__ int pidx(const Params<real> &P, int x, int y, int z)
 {
-    return ((z + 1) * P.py + (y + 1)) * P.px + (x + XOFF);
+    return ((z + 1) * P.py + (y + 1)) * P.px + (x + P.xoff);
 }
 // offset (in cells) of the pull source of direction i relative to the cell: source = p - poff
 template <int I, typename real>
@@ -276,11 +283,25 @@ __device__ __forceinline__ Macro<real> local_macros(const real (&g)[Q], int cls,
     return Macro<real>{rho, mx * inv, my * inv, mz * inv};
 }
 
-template <typename real>
-__device__ __forceinline__ void load_cell(real (&g)[Q], const real *__restrict__ A, long long stride, int p)
+// one stored population <-> the arithmetic type (S = real: a plain access; S = __half: widen / round to nearest even)
+template <typename real, typename S>
+__device__ __forceinline__ real ld_s(const S *p)
+{
+    if constexpr (std::is_same<S, __half>::value) return real(__half2float(*p));
+    else return real(*p);
+}
+template <typename real, typename S>
+__device__ __forceinline__ void st_s(S *p, real v)
+{
+    if constexpr (std::is_same<S, __half>::value) *p = __float2half_rn(float(v));
+    else *p = S(v);
+}
+
+template <typename real, typename S>
+__device__ __forceinline__ void load_cell(real (&g)[Q], const S *__restrict__ A, long long stride, int p)
 {
 #pragma unroll
-    for (int i = 0; i < Q; ++i) g[i] = A[(long long)i * stride + p];
+    for (int i = 0; i < Q; ++i) g[i] = ld_s<real>(A + ((long long)i * stride + p));
 }
 
 // ---- the write-side boundary rule ------------------------------------------------------------------------------------
@@ -353,14 +374,14 @@ __device__ __forceinline__ void ghost_stores(const Params<real> &P, int x, int y
 }
 
 // All stores of one cell's post-collision state into buffer B: own 19 slots, wall mailboxes, ghost slots.
-template <typename real>
-__device__ __forceinline__ void store_cell(real *__restrict__ B, const Params<real> &P, int p, int x, int y, int z, uint8_t fl,
+template <typename real, typename S>
+__device__ __forceinline__ void store_cell(S *__restrict__ B, const Params<real> &P, int p, int x, int y, int z, uint8_t fl,
                                            uint32_t lk, const real (&g)[Q])
 {
 #pragma unroll
-    for (int i = 0; i < Q; ++i) B[(long long)i * P.stride + p] = g[i];
+    for (int i = 0; i < Q; ++i) st_s(B + ((long long)i * P.stride + p), g[i]);
     if (fl & (SLOW_BIT | EDGE_BIT)) {
-        auto st = [&](int i, int pt, auto jc) { B[(long long)i * P.stride + pt] = g[decltype(jc)::value]; };
+        auto st = [&](int i, int pt, auto jc) { st_s(B + ((long long)i * P.stride + pt), g[decltype(jc)::value]); };
         if (fl & SLOW_BIT) wall_stores(P, p, lk, st);
         if (fl & EDGE_BIT) ghost_stores(P, x, y, z, lk, st);
     }

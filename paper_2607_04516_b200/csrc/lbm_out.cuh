@@ -13,8 +13,8 @@ __device__ __forceinline__ real stored_theta_shift(const real *__restrict__ H, l
 }
 
 // local macros of the stored state (DESIGN.md §3 step 7)
-template <typename real, typename out_t>
-__global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
+template <typename real, typename S, typename out_t>
+__global__ void macros_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
                               out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz, Params<real> P,
                               const real *__restrict__ H = nullptr)
 {
@@ -35,27 +35,6 @@ __global__ void macros_kernel(const real *__restrict__ A, const uint8_t *__restr
     if (ux) ux[c] = out_t(m.ux);
     if (uy) uy[c] = out_t(m.uy);
     if (uz) uz[c] = out_t(m.uz);
-}
-
-// standalone sample (a sample due at a step the fused kernel did not produce, e.g. step 0); DESIGN.md §3 step 8
-template <typename real>
-__global__ void mean_sample_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, real *__restrict__ msum, Params<real> P,
-                                   const real *__restrict__ H = nullptr)
-{
-    const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= P.N) return;
-    int x, y, z;
-    cell_xyz(P, c, x, y, z);
-    const int p = pidx(P, x, y, z);
-    const int cls = flags[p] & CLASS_MASK;
-    if (cls == SOLID) return;
-    real g[Q];
-    load_cell(g, A, P.stride, p);
-    if (H) P.Fz += P.gbeta * stored_theta_shift(H, P.stride, p);
-    const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
-    msum[p] += m.ux;
-    msum[P.stride + p] += m.uy;
-    msum[2 * P.stride + p] += m.uz;
 }
 
 template <typename real, typename out_t>

@@ -18,7 +18,7 @@ __global__ void voxelise_kernel(const int32_t *__restrict__ height, const uint8_
 {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= P.Np) return;
-    int x = p % P.px - XOFF, y = (p / P.px) % P.py - 1, z = p / P.pxy - 1;
+    int x = p % P.px - P.xoff, y = (p / P.px) % P.py - 1, z = p / P.pxy - 1;
     if (x < -1 || x > P.nx) { flags[p] = SOLID; return; }
     const int n[3] = {P.nx, P.ny, P.nz};
     int c[3] = {x, y, z};
@@ -80,9 +80,9 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restric
     } else if (cls == SOLID) {
         // slot i of this cell must be zero-filled every step iff some cell of its 32-byte sector is written in
         // population i (a live cell, or a solid cell whose slot i is a neighbour's mailbox) and this one is not
-        const int s0 = p & ~7; // the 8 cells of the sector (FP32; a superset of the FP64 sector)
+        const int s0 = p & ~(P.sec - 1); // the cells of the 32-byte sector (8 for FP32; also used for FP64: a superset; 16 for __half)
         uint32_t written = 0, own = 0;
-        for (int q = s0; q < s0 + 8; ++q) {
+        for (int q = s0; q < s0 + P.sec; ++q) {
             const int cq = flags[q] & CLASS_MASK;
             if (cq == FLUID || cq == EQ_OUTFLOW || cq == EQ_FIXED) written |= 0x7FFFFu;
             else if (cq == SOLID) {
@@ -113,8 +113,8 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restric
 
 // store one cell's state into BOTH buffers (set-up paths: the two buffers start identical), and publish its velocity
 // to the outflow cells it feeds (both halves of the double-buffered side array)
-template <typename real>
-__device__ __forceinline__ void store_cell_both(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const Params<real> &P,
+template <typename real, typename S>
+__device__ __forceinline__ void store_cell_both(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const Params<real> &P,
                                                 int p, int x, int y, int z, uint8_t fl, uint32_t lk, const real (&g)[Q])
 {
     store_cell(A, P, p, x, y, z, fl, lk, g);
@@ -146,8 +146,8 @@ __device__ __forceinline__ void publish_fixed(real *__restrict__ fu, const Param
 
 // ---- a3: inlet write -------------------------------------------------------------------------------------------------
 // mode 0: profile prof[nz] per component by level; mode 1: plane uvw[3][n2][n1] of one face
-template <typename real, typename in_t>
-__global__ void inlet_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+template <typename real, typename S, typename in_t>
+__global__ void inlet_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                              const in_t *__restrict__ pu, const in_t *__restrict__ pv, const in_t *__restrict__ pw,
                              int mode, int face, Params<real> P)
 {
@@ -193,8 +193,8 @@ template <typename real>
 struct Turb { const real *fum; const double *modes; int n; double t; };
 
 // one slot: boundary velocity of time t -> dst0 / dst1 (the halves to publish to; dst1 may be null)
-template <typename real, bool CELLS>
-__device__ __forceinline__ void fluct_slot(int s, real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, real *__restrict__ dst0,
+template <typename real, bool CELLS, typename S = real>
+__device__ __forceinline__ void fluct_slot(int s, S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, real *__restrict__ dst0,
                                            real *__restrict__ dst1, const uint8_t *__restrict__ flags, const Turb<real> &tb, const Params<real> &P)
 {
     int k = 5;
@@ -242,20 +242,20 @@ __device__ __forceinline__ void fluct_slot(int s, real *__restrict__ A, real *__
 
 // stand-alone form (set-up, switch-off, re-initialisation): both halves; CELLS = also the cells' populations in both buffers.
 // During a run the step kernel itself carries the slots (lbm_step.cuh, TURB blocks): no extra launch.
-template <typename real, bool CELLS>
-__global__ void fluct_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+template <typename real, typename S, bool CELLS>
+__global__ void fluct_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                              const Turb<real> tb, Params<real> P)
 {
     const int s = blockIdx.x * blockDim.x + threadIdx.x;
     if (s >= P.F) return;
-    fluct_slot<real, CELLS>(s, A, B, fu, fu, fu + 3 * (size_t)P.F, flags, tb, P);
+    fluct_slot<real, CELLS, S>(s, A, B, fu, fu, fu + 3 * (size_t)P.F, flags, tb, P);
 }
 
 // Re-publish the velocities the outflow cells will read next step from the CURRENT state (both halves of the side
 // array).  Needed when something that enters the local macro inversion changes between steps (lbm_set_damping): the
 // rule is u_loc(G_k, c - n) evaluated with the parameters in force when the step runs (DESIGN.md §3 step 6).
-template <typename real>
-__global__ void refeed_kernel(const real *__restrict__ A, real *__restrict__ fu, const uint8_t *__restrict__ flags, Params<real> P)
+template <typename real, typename S>
+__global__ void refeed_kernel(const S *__restrict__ A, real *__restrict__ fu, const uint8_t *__restrict__ flags, Params<real> P)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -274,10 +274,10 @@ __global__ void refeed_kernel(const real *__restrict__ A, real *__restrict__ fu,
 }
 
 // ---- a8: precursor plane -> main inlet (config 5) -----------------------------------------------------------------------
-template <typename real>
-__global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, real *__restrict__ dfu, const uint8_t *__restrict__ dflags,
+template <typename real, typename S>
+__global__ void feed_kernel(S *__restrict__ dA, S *__restrict__ dB, real *__restrict__ dfu, const uint8_t *__restrict__ dflags,
                             Params<real> D,
-                            const real *__restrict__ sA, const uint8_t *__restrict__ sflags, Params<real> S, int sx)
+                            const S *__restrict__ sA, const uint8_t *__restrict__ sflags, Params<real> Ps, int sx)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= D.ny * D.nz) return;
@@ -285,10 +285,10 @@ __global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, real *
     const int dp = pidx(D, 0, y, z);
     const uint8_t fl = dflags[dp];
     if ((fl & CLASS_MASK) != EQ_FIXED) return;
-    const int sp = pidx(S, sx, y % S.ny, z);
+    const int sp = pidx(Ps, sx, y % Ps.ny, z);
     real g[Q];
-    load_cell(g, sA, S.stride, sp);
-    const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, S, damp_at(S, sx, y % S.ny, z));
+    load_cell(g, sA, Ps.stride, sp);
+    const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, Ps, damp_at(Ps, sx, y % Ps.ny, z));
     equilibrium(g, real(0), m.ux, m.uy, m.uz);
     store_cell_both(dA, dB, dfu, D, dp, 0, y, z, fl, 0u, g);
     publish_fixed(dfu, D, 0, y, z, m.ux, m.uy, m.uz);
@@ -296,8 +296,8 @@ __global__ void feed_kernel(real *__restrict__ dA, real *__restrict__ dB, real *
 
 // ---- a4: init ------------------------------------------------------------------------------------------------------------
 // G0 = f_eq(rho0, u0) in FLUID and EQ_OUTFLOW cells (EQ_FIXED keep their boundary state; SOLID cells hold mailboxes)
-template <typename real, typename in_t>
-__global__ void init_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+template <typename real, typename S, typename in_t>
+__global__ void init_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                             const uint32_t *__restrict__ links, const in_t *__restrict__ rho, const in_t *__restrict__ ux,
                             const in_t *__restrict__ uy, const in_t *__restrict__ uz, Params<real> P)
 {
@@ -318,8 +318,8 @@ __global__ void init_kernel(real *__restrict__ A, real *__restrict__ B, real *__
 
 // ---- checkpoint ------------------------------------------------------------------------------------------------------------
 // f [19][nz][ny][nx] double, NOT shifted.  SOLID cells export the rest state w_i (their slots are mailboxes).
-template <typename real>
-__global__ void state_out_kernel(const real *__restrict__ A, const uint8_t *__restrict__ flags, double *__restrict__ f, Params<real> P)
+template <typename real, typename S>
+__global__ void state_out_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, double *__restrict__ f, Params<real> P)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -328,11 +328,11 @@ __global__ void state_out_kernel(const real *__restrict__ A, const uint8_t *__re
     const int p = pidx(P, x, y, z);
     const bool solid = (flags[p] & CLASS_MASK) == SOLID;
 #pragma unroll
-    for (int i = 0; i < Q; ++i) f[(long long)i * P.N + c] = (solid ? 0.0 : double(A[(long long)i * P.stride + p])) + weight_f64(i);
+    for (int i = 0; i < Q; ++i) f[(long long)i * P.N + c] = (solid ? 0.0 : double(ld_s<real>(A + ((long long)i * P.stride + p)))) + weight_f64(i);
 }
 
-template <typename real>
-__global__ void state_in_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+template <typename real, typename S>
+__global__ void state_in_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                                 const uint32_t *__restrict__ links, const double *__restrict__ f, Params<real> P)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -393,8 +393,8 @@ __global__ void flux_sum_kernel(const real *__restrict__ fu, const uint8_t *__re
     if ((threadIdx.x & 31) == 0 && cnt != 0.0) { atomicAdd(&acc[0], un); atomicAdd(&acc[1], cnt); }
 }
 
-template <typename real>
-__global__ void flux_apply_kernel(real *__restrict__ A, real *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+template <typename real, typename S>
+__global__ void flux_apply_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                                   const double *__restrict__ acc, Params<real> P)
 {
     const int sl = blockIdx.x * blockDim.x + threadIdx.x;

@@ -33,6 +33,12 @@ __device__ __forceinline__ double ld_pinned(const double *p)
     asm volatile("ld.volatile.global.f64 %0, [%1];" : "=d"(v) : "l"(p));
     return v;
 }
+__device__ __forceinline__ float ld_pinned(const __half *p)
+{
+    unsigned short v;
+    asm volatile("ld.volatile.global.u16 %0, [%1];" : "=h"(v) : "l"(p));
+    return __half2float(__ushort_as_half(v));
+}
 __device__ __forceinline__ uint8_t ld_pinned(const uint8_t *p)
 {
     uint32_t v;
@@ -42,15 +48,15 @@ __device__ __forceinline__ uint8_t ld_pinned(const uint8_t *p)
 
 // Per-launch address table: src[i] = A + i stride - off_i (so the pull of direction i is src[i][p]), dst[i] = B + i stride.
 // One 64-bit multiply-add per access instead of rebuilding i * stride - off_i in every thread.
-template <typename real>
+template <typename S>
 struct StepPtrs {
-    const real *src[Q];
-    real *dst[Q];
+    const S *src[Q];
+    S *dst[Q];
 };
-template <typename real>
-inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> &P)
+template <typename S, typename real>
+inline StepPtrs<S> make_step_ptrs(const S *A, S *B, const Params<real> &P)
 {
-    StepPtrs<real> t;
+    StepPtrs<S> t;
     for (int i = 0; i < Q; ++i) {
         const long long off = dir_cx(i) + (long long)dir_cy(i) * P.px + (long long)dir_cz(i) * P.pxy;
         t.src[i] = A + ((long long)i * P.stride - off);
@@ -61,10 +67,10 @@ inline StepPtrs<real> make_step_ptrs(const real *A, real *B, const Params<real> 
 
 // The step of one thread (one cell, or one face slot in a TURB block row).  A plain device function so that it can be
 // called once per launch (step_kernel) or in a loop with grid-wide barriers (step_loop_kernel, lattices that fit L2).
-template <typename real, bool MEAN, bool SPEC, int BLOCK, bool DAMP, bool TURB>
-__device__ __forceinline__ void step_body(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags,
+template <typename real, typename S, bool MEAN, bool SPEC, int BLOCK, bool DAMP, bool TURB>
+__device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict__ B, const uint8_t *__restrict__ flags,
                                           const uint32_t *__restrict__ links, real *__restrict__ msum, const real *__restrict__ fur,
-                                          real *__restrict__ fuw, const Params<real> &P, const StepPtrs<real> &T, const Turb<real> &tb,
+                                          real *__restrict__ fuw, const Params<real> &P, const StepPtrs<S> &T, const Turb<real> &tb,
                                           const int turb_planes)
 {
     int zb = blockIdx.y;
@@ -74,7 +80,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
         // next launch read it from there.  They are dispatched first and run beside the memory-bound lattice blocks.
         if (zb < turb_planes) {
             const int s = (zb * (int)gridDim.x + (int)blockIdx.x) * BLOCK + (int)threadIdx.x;
-            if (s < P.F) fluct_slot<real, false>(s, nullptr, nullptr, nullptr, fuw, nullptr, flags, tb, P);
+            if (s < P.F) fluct_slot<real, false, S>(s, nullptr, nullptr, nullptr, fuw, nullptr, flags, tb, P);
             return;
         }
         zb -= turb_planes;
@@ -94,7 +100,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     if constexpr (SPEC) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            g[i] = ld_pinned(T.src[i] + p);
+            g[i] = real(ld_pinned(T.src[i] + p));
         });
         // a cell on an EQ face fetches its face velocity now, from geometry alone (EQ_FIXED wins, as in the voxeliser);
         // if the flag then says SOLID the three values are simply not used
@@ -126,7 +132,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
             else m = collide(g, P);
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
-                T.dst[i][p] = g[i];
+                st_s(T.dst[i] + p, g[i]);
             });
             if constexpr (MEAN) {
                 msum[p] = ms0 + m.ux;
@@ -152,7 +158,7 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
         if constexpr (!SPEC) {
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
-                g[i] = T.src[i][p];
+                g[i] = ld_s<real>(T.src[i] + p);
             });
         }
         if constexpr (DAMP) m = collide<real, true>(g, P, SPEC ? dmp : damp_at(P, x, y, z));
@@ -174,12 +180,12 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     if (__any_sync(__activemask(), merged_solid)) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            if ((wm >> i) & 1u) T.dst[i][p] = g[i];
+            if ((wm >> i) & 1u) st_s(T.dst[i] + p, g[i]);
         });
     } else {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            T.dst[i][p] = g[i];
+            st_s(T.dst[i] + p, g[i]);
         });
     }
     if (merged_solid) return;
@@ -187,11 +193,11 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
         // wall links (lbm_core.cuh wall_stores, with the launch's address table): slot (i, p - off_i) <- g[opp(i)]
         static_for<1, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            if ((lk >> i) & 1u) T.dst[i][p - poff<i>(P)] = g[dir_opp(i)];
+            if ((lk >> i) & 1u) st_s(T.dst[i] + (p - poff<i>(P)), g[dir_opp(i)]);
         });
     }
     if (fl & EDGE_BIT)
-        ghost_stores(P, x, y, z, lk, [&](int i, int pt, auto jc) { B[(long long)i * P.stride + pt] = g[decltype(jc)::value]; });
+        ghost_stores(P, x, y, z, lk, [&](int i, int pt, auto jc) { st_s(B + ((long long)i * P.stride + pt), g[decltype(jc)::value]); });
     if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) { fuw[comp * P.F + sl] = v; });
     if constexpr (MEAN) {
         if constexpr (SPEC) {
@@ -206,13 +212,13 @@ __device__ __forceinline__ void step_body(const real *__restrict__ A, real *__re
     }
 }
 
-template <typename real, bool MEAN, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
+template <typename real, typename S, bool MEAN, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
-step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-            real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<real> T,
+step_kernel(const S *__restrict__ A, S *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+            real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<S> T,
             const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
 {
-    step_body<real, MEAN, SPEC, BLOCK, DAMP, TURB>(A, B, flags, links, msum, fur, fuw, P, T, tb, turb_planes);
+    step_body<real, S, MEAN, SPEC, BLOCK, DAMP, TURB>(A, B, flags, links, msum, fur, fuw, P, T, tb, turb_planes);
 }
 
 // Several steps in ONE cooperative launch, a grid-wide barrier between them: for lattices whose whole grid is resident
@@ -221,18 +227,18 @@ step_kernel(const real *__restrict__ A, real *__restrict__ B, const uint8_t *__r
 // Every pull, the flag byte and the face velocities are read with ld.volatile / from read-only data, the barrier orders
 // the stores of one step before the loads of the next.  No time mean, no inflow fluctuations on this path (the host
 // falls back to single launches for those steps).
-template <typename real, int BLOCK, int MINB, bool DAMP>
+template <typename real, typename S, int BLOCK, int MINB, bool DAMP>
 __global__ void __launch_bounds__(BLOCK, MINB)
-step_loop_kernel(real *__restrict__ A, real *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-                 real *__restrict__ fu0, real *__restrict__ fu1, const Params<real> P, const StepPtrs<real> T0, const StepPtrs<real> T1,
+step_loop_kernel(S *__restrict__ A, S *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+                 real *__restrict__ fu0, real *__restrict__ fu1, const Params<real> P, const StepPtrs<S> T0, const StepPtrs<S> T1,
                  const int pairs)
 {
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const Turb<real> tb{};
     for (int s = 0; s < pairs; ++s) {
-        step_body<real, false, true, BLOCK, DAMP, false>(A, B, flags, links, nullptr, fu0, fu1, P, T0, tb, 0);
+        step_body<real, S, false, true, BLOCK, DAMP, false>(A, B, flags, links, nullptr, fu0, fu1, P, T0, tb, 0);
         grid.sync();
-        step_body<real, false, true, BLOCK, DAMP, false>(B, A, flags, links, nullptr, fu1, fu0, P, T1, tb, 0);
+        step_body<real, S, false, true, BLOCK, DAMP, false>(B, A, flags, links, nullptr, fu1, fu0, P, T1, tb, 0);
         grid.sync();
     }
 }

@@ -46,6 +46,19 @@ struct VecIO<float, 2> {
     static __device__ __forceinline__ void st(float *p, const float (&v)[2]) { *reinterpret_cast<float2 *>(p) = make_float2(v[0], v[1]); }
 };
 template <>
+struct VecIO<float, 8> { // the mean sums of the 8-cell kernel: two 128-bit accesses
+    static __device__ __forceinline__ void ld(const float *p, float (&v)[8])
+    {
+        asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[0]), "=f"(v[1]), "=f"(v[2]), "=f"(v[3]) : "l"(p));
+        asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v[4]), "=f"(v[5]), "=f"(v[6]), "=f"(v[7]) : "l"(p + 4));
+    }
+    static __device__ __forceinline__ void st(float *p, const float (&v)[8])
+    {
+        reinterpret_cast<float4 *>(p)[0] = make_float4(v[0], v[1], v[2], v[3]);
+        reinterpret_cast<float4 *>(p)[1] = make_float4(v[4], v[5], v[6], v[7]);
+    }
+};
+template <>
 struct VecIO<__half, 4> {
     static __device__ __forceinline__ void ld(const __half *p, float (&v)[4])
     {

@@ -169,6 +169,43 @@ __global__ void thermal_init_kernel(real *__restrict__ HA, real *__restrict__ HB
     store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
 }
 
+// ---- checkpoint of the thermal lattice (lbm_get_thermal_state / lbm_set_thermal_state) -----------------------------------
+// h [7][nz][ny][nx] double, NOT shifted; non-FLUID cells export the rest state wT_i theta_ref and ignore their input.
+__host__ __device__ inline double weight_t_f64(int i) { return i == 0 ? 0.25 : 0.125; }
+
+template <typename real>
+__global__ void thermal_state_out_kernel(const real *__restrict__ H, const uint8_t *__restrict__ flags, double *__restrict__ h, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const bool live = (flags[p] & CLASS_MASK) == FLUID;
+#pragma unroll
+    for (int i = 0; i < QT; ++i)
+        h[(long long)i * P.N + c] = (live ? double(H[(long long)i * P.stride + p]) : 0.0) + weight_t_f64(i) * double(P.theta_ref);
+}
+
+template <typename real>
+__global__ void thermal_state_in_kernel(real *__restrict__ HA, real *__restrict__ HB, const uint8_t *__restrict__ flags,
+                                        const uint32_t *__restrict__ links, const double *__restrict__ h, Params<real> P)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= P.N) return;
+    int x, y, z;
+    cell_xyz(P, c, x, y, z);
+    const int p = pidx(P, x, y, z);
+    const uint8_t fl = flags[p];
+    if ((fl & CLASS_MASK) != FLUID) return;
+    real t[QT];
+#pragma unroll
+    for (int i = 0; i < QT; ++i) t[i] = real(h[(long long)i * P.N + c] - weight_t_f64(i) * double(P.theta_ref));
+    const uint32_t lk = links[p];
+    store_cell_thermal(HA, P, p, x, y, z, fl, lk, t);
+    store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
+}
+
 // theta of the stored state (lbm_get_theta); SOLID cells report theta_ref
 template <typename real, typename out_t>
 __global__ void theta_out_kernel(const real *__restrict__ H, const uint8_t *__restrict__ flags, out_t *__restrict__ theta, Params<real> P)

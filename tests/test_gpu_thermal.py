@@ -238,3 +238,36 @@ def test_density_current_fronts_gpu_at_25m_against_the_papers_printed_values(B):
     for T, ref, plat in _paper_fronts():
         assert abs(got[T] / ref - 1.0) < 0.08 and abs(got[T] / plat - 1.0) < 0.08, (T, got[T], ref, plat)
     print("density current 25 m fronts (km):", got)
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_thermal_checkpoint_restarts_exactly(B, fp64):
+    """lbm_get_state + lbm_get_thermal_state + the step counter are a complete checkpoint of a thermal run: a fresh handle
+    loaded with them continues bit for bit like the uninterrupted one (mailboxes and ghost slots of both lattices are
+    rebuilt by the set calls)."""
+    nx, ny, nz = 36, 10, 14
+    rng = np.random.default_rng(8)
+    hm = np.zeros((ny, nx), np.int32); hm[3:6, 8:14] = 5
+    theta = 1.0 + 0.2 * rng.standard_normal((nz, ny, nx))
+    args = (nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), (P, P, FS, W, W, FS))
+
+    def fresh():
+        s = B.Lbm(*args, fp64=fp64)
+        s.set_flags(hm)
+        s.set_macros()
+        s.set_thermal(0.01, 2e-3, 1.0)
+        return s
+    a = fresh()
+    a.set_theta(theta, f64=True)
+    a.step(40)
+    f, hpop, k = a.get_state(out="host"), a.get_thermal_state(), a.get_step()
+    assert hpop.shape == (7, nz, ny, nx)
+    th = a.get_theta(out="host", f64=True)
+    np.testing.assert_allclose(hpop.sum(axis=0)[hm[None] <= np.arange(nz)[:, None, None]], th[hm[None] <= np.arange(nz)[:, None, None]], rtol=0, atol=1e-6 if not fp64 else 1e-13)
+    b = fresh()
+    b.set_state(f); b.set_thermal_state(hpop); b.set_step(k)
+    a.step(25); b.step(25)
+    np.testing.assert_array_equal(a.get_state(out="host"), b.get_state(out="host"))
+    np.testing.assert_array_equal(a.get_thermal_state(), b.get_thermal_state())
+    assert a.get_step() == b.get_step() == 65
+    a.close(); b.close()
