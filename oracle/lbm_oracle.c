@@ -123,6 +123,8 @@ typedef struct oracle {
     int thermal;
     double alpha, gbeta, theta_ref; /* diffusivity, g*beta (buoyancy per unit theta, along +z), reference theta */
     double *H, *Hn;                 /* [cell][7] post-collision thermal populations, directions 0..6 of CI */
+    int thd[6];                     /* WALL faces held at a fixed temperature (Dirichlet; reading 26): 1 = on */
+    double thw[6];                  /* ... their temperatures theta_w */
     /* 16-bit population storage: 0 = populations kept in FP64 (default),
      * 1 = every population is rounded to IEEE binary16 at the moment it is written into the state */
     int store16;
@@ -766,6 +768,37 @@ int oracle_balance_flux(oracle_t *o, double *flux_before, double *flux_after)
     return 0;
 }
 
+/* Fixed-temperature walls of the thermal lattice (DESIGN.md §4 reading 26).  The paper's thermal workload is a closed
+ * adiabatic box and its Table 1 only names the lattice; a wall held at a temperature is the
+ * textbook halfway anti-bounce-back rule for an advection-diffusion lattice: a thermal population that leaves a cell
+ * towards a WALL face k held at theta_w returns as  h_ibar <- -h_i + 2 wT_i theta_w  (wall at rest), which puts
+ * theta = theta_w half a cell outside the last node, where halfway bounce-back puts the no-slip wall.  Only domain faces
+ * of type WALL can be held; buildings and all other faces stay adiabatic (plain bounce-back / specular reflection).
+ * Which face does the pull of direction i (1..6, an axis direction) of cell (x,y,z) cross?  -1 if none that is held. */
+static int fixed_temperature_face(const oracle_t *o, int x, int y, int z, int i)
+{
+    if (i < 1 || i > 6) return -1;
+    int p[3] = {x - CI[i][0], y - CI[i][1], z - CI[i][2]};
+    int n[3] = {o->nx, o->ny, o->nz};
+    for (int a = 0; a < 3; ++a) {
+        int k = -1;
+        if (p[a] < 0) k = 2 * a;
+        else if (p[a] >= n[a]) k = 2 * a + 1;
+        if (k >= 0 && o->face[k] == F_WALL && o->thd[k]) return k;
+    }
+    return -1;
+}
+
+/* on[6] (x-,x+,y-,y+,z-,z+): 1 = hold that face at theta_w[k].  The face must be a WALL face (-1 otherwise). */
+int oracle_set_thermal_walls(oracle_t *o, const int *on, const double *theta_w)
+{
+    if (!o || !on || !theta_w || !o->thermal) return -3;
+    for (int k = 0; k < 6; ++k)
+        if (on[k] && o->face[k] != F_WALL) return -1;
+    for (int k = 0; k < 6; ++k) { o->thd[k] = on[k] ? 1 : 0; o->thw[k] = theta_w[k]; }
+    return 0;
+}
+
 int oracle_step(oracle_t *o, int nsteps)
 {
     if (!o->have_flags) return -3;
@@ -811,6 +844,10 @@ int oracle_step(oracle_t *o, int nsteps)
                                     r = 1;
                                 }
                                 h[i] = r ? o->H[cell * QT + opposite(i)] : o->H[s * QT + j];
+                                /* a WALL face held at theta_w (reading 26): anti-bounce-back, the population comes
+                                 * back with the opposite sign plus twice the wall's equilibrium share */
+                                int kf = r ? fixed_temperature_face(o, x, y, z, i) : -1;
+                                if (kf >= 0) h[i] = -o->H[cell * QT + opposite(i)] + 2.0 * weight_t(i) * o->thw[kf];
                                 theta += h[i];
                             }
                             double Fb[3] = {o->F[0], o->F[1], o->F[2] + o->gbeta * (theta - o->theta_ref)};

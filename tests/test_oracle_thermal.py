@@ -186,3 +186,96 @@ def test_density_current_front_positions_against_the_papers_printed_values():
     th = o.get_theta()
     assert -15.0 < th.min() < -8.0 and th.max() < 1.0   # the pool stays cold; BGK overshoot ahead of the front stays < 1 K
     o.close()
+
+
+# ---- fixed-temperature walls (DESIGN.md §4 reading 26) and the coupled loop: Rayleigh-Benard onset ----------------------
+
+def test_conduction_between_two_held_walls_is_the_linear_profile():
+    """No flow (g beta = 0), WALL z faces held at 1 (below) and 0.25 (above), periodic x, y: the steady state of the
+    diffusion equation is theta(zeta) = theta_b + (theta_t - theta_b) zeta / H, zeta = z + 1/2, H = nz (walls half a cell
+    outside the last nodes, where halfway bounce-back puts the no-slip wall).  Anti-bounce-back reproduces a linear
+    profile exactly; a wrong sign, a missing factor 2 or a wall one half cell off fails at the 1e-2 level."""
+    nx, ny, nz, alpha = 4, 3, 10, 0.12
+    o = O.Oracle(nx, ny, nz, 0.05, 0.0, 0.0, (0, 0, 0), (0, 0, 0, 0, 1, 1))
+    o.set_flags(None)
+    o.set_thermal(alpha, 0.0, 0.0)
+    o.set_thermal_walls([0, 0, 0, 0, 1, 1], [9, 9, 9, 9, 1.0, 0.25])
+    o.set_macros()
+    o.set_theta(np.full((nz, ny, nx), 0.6))
+    o.step(6000)                                   # H^2 / alpha = 830 steps per diffusion time
+    th = o.get_theta()
+    zeta = np.arange(nz) + 0.5
+    exact = 1.0 + (0.25 - 1.0) * zeta / nz
+    assert np.abs(th - exact[:, None, None]).max() < 1e-10
+    # an adiabatic (not held) wall keeps the heat in: hold only the bottom -> uniform theta_b
+    o.set_thermal_walls([0, 0, 0, 0, 1, 0], [0, 0, 0, 0, 1.0, 0.0])
+    o.step(12000)
+    assert np.abs(o.get_theta() - 1.0).max() < 1e-9
+    # only WALL faces can be held
+    with pytest.raises(RuntimeError):
+        o.set_thermal_walls([1, 0, 0, 0, 0, 0], [0.0] * 6)
+    o.close()
+
+
+def test_heat_flux_through_held_walls_is_fouriers_law():
+    """Transient check of the coupling constant: with the linear profile established the heat entering through the hot wall
+    per step and unit area is alpha (theta_b - theta_t) / H; switch the top wall to adiabatic and the box's heat content
+    must start to rise at exactly that rate (first step)."""
+    nx, ny, nz, alpha = 3, 3, 12, 0.08
+    o = O.Oracle(nx, ny, nz, 0.05, 0.0, 0.0, (0, 0, 0), (0, 0, 0, 0, 1, 1))
+    o.set_flags(None)
+    o.set_thermal(alpha, 0.0, 0.0)
+    o.set_thermal_walls([0, 0, 0, 0, 1, 1], [0, 0, 0, 0, 2.0, 0.5])
+    o.set_macros()
+    o.set_theta(np.full((nz, ny, nx), 1.0))
+    o.step(8000)
+    q0 = o.get_theta().sum()
+    o.set_thermal_walls([0, 0, 0, 0, 1, 0], [0, 0, 0, 0, 2.0, 0.0])
+    o.step(1)
+    q1 = o.get_theta().sum()
+    assert (q1 - q0) / (nx * ny) == pytest.approx(alpha * (2.0 - 0.5) / nz, rel=1e-9)
+    o.close()
+
+
+def _rb_growth_rate(Ra, H, nu=0.05, alpha=0.05):
+    """Growth rate per step of the critical roll mode between no-slip plates held at 1 (below) and 0 (above)."""
+    nx = 2 * H                                        # one roll pair: k H = pi (critical k_c H = 3.117: Ra_c(k) is flat there)
+    gb = Ra * nu * alpha / H ** 3                     # Ra = g beta dT H^3 / (nu alpha), dT = 1
+    o = O.Oracle(nx, 1, H, nu, 0.0, 0.0, (0, 0, 0), (0, 0, 0, 0, 1, 1))
+    o.set_flags(None)
+    o.set_thermal(alpha, gb, 0.5)
+    o.set_thermal_walls([0, 0, 0, 0, 1, 1], [0, 0, 0, 0, 1.0, 0.0])
+    zeta = (np.arange(H) + 0.5) / H
+    x = np.arange(nx) + 0.5
+    k = 2 * np.pi / nx
+    mode = np.sin(np.pi * zeta)[:, None] * np.cos(k * x)[None, :]
+    o.set_macros()
+    o.set_theta(((1.0 - zeta)[:, None] + 1e-7 * mode)[:, None, :])
+    o.step(int(0.5 * H * H / alpha))                  # let the seeded shape relax onto the eigenmode
+    t, a = [], []
+    for _ in range(12):
+        t.append(o.get_step()); a.append(abs((o.get_macros()[3][:, 0, :] * mode).sum()))
+        o.step(int(H * H / alpha / 6))
+    o.close()
+    slope, _ = np.polyfit(np.array(t, float), np.log(np.array(a)), 1)
+    resid = np.log(np.array(a)) - np.polyval([slope, _], np.array(t, float))
+    assert np.abs(resid).max() < 0.02                 # a clean exponential: one mode
+    return slope
+
+
+def test_rayleigh_benard_onset_between_no_slip_plates():
+    """The coupled loop buoyancy -> velocity -> advection of theta -> buoyancy, pinned by linear stability theory: between
+    no-slip isothermal plates the conduction state loses stability at Ra_c = 1707.76 (k_c H = 3.117; textbook value,
+    Chandrasekhar 1961 §II).  The roll mode of wavelength 2H decays at 0.9 Ra_c and grows at 1.1 Ra_c; the zero of the
+    growth rate (linear in Ra near onset) lies within 2 % of 1707.76 at H = 24 and the error falls like 1/H^2 from H = 16
+    (measured: +2.1 % at 16, +1.0 % at 24).  A wrong g beta, a wrong sign of the buoyancy or of the advection term, a
+    wrong thermal diffusivity or viscosity (Ra contains both) moves the zero by far more."""
+    Rac = 1707.76
+    est = {}
+    for H in (16, 24):
+        lo, hi = _rb_growth_rate(0.9 * Rac, H), _rb_growth_rate(1.1 * Rac, H)
+        assert lo < 0 < hi
+        est[H] = 0.9 * Rac + (0.0 - lo) * 0.2 * Rac / (hi - lo)
+    print("Rayleigh-Benard onset: Ra_c estimate", {h: round(v, 1) for h, v in est.items()})
+    assert abs(est[24] / Rac - 1) < 0.02
+    assert abs(est[24] - Rac) < 0.6 * abs(est[16] - Rac)        # second-order convergence (ratio (16/24)^2 = 0.44)
