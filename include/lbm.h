@@ -191,6 +191,14 @@ int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const dou
 /* theta = sum_i h_i of the current state, [nz][ny][nx], host or device; SOLID cells report theta_ref.  Synchronises. */
 int lbm_get_theta(lbm_t *h, float *theta);
 int lbm_get_theta_f64(lbm_t *h, double *theta);
+/* Fixed-temperature walls (DESIGN.md §4 reading 26): on[k] != 0 holds domain face k (order x-,x+,y-,y+,z-,z+), which must be
+ * a WALL face (else LBM_EINVAL), at temperature theta_w[k] by halfway anti-bounce-back — a thermal population leaving
+ * towards it returns as -h_i + 2 wT_i theta_w, theta = theta_w half a cell outside the last node; all other walls and the
+ * buildings stay adiabatic.  Host arrays.  The change applies to the populations stored from the next step on (the
+ * mailboxes written by the last step / by lbm_set_theta keep the rule in force when they were written: call it before
+ * lbm_set_theta for an exact start).  Needs lbm_set_thermal (else LBM_ESTATE).  With it the thermal lattice covers heated
+ * / cooled ground and lids — e.g. Rayleigh-Benard convection, the closed-form pin of the coupled loop. */
+int lbm_set_thermal_walls(lbm_t *h, const int on[6], const double theta_w[6]);
 /* Checkpoint of the thermal lattice: the 7 thermal populations h_i (NOT shifted), double, [7][nz][ny][nx], directions
  * 0..6 of the flow lattice; host or device.  Together with lbm_get_state / lbm_set_state and lbm_set_step a thermal run
  * restarts exactly.  Non-FLUID cells export the rest state wT_i theta_ref and ignore their input.  Needs

@@ -29,7 +29,7 @@ SYMBOLS = [
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
     "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
     "lbm_set_thermal", "lbm_set_theta", "lbm_set_theta_f64", "lbm_get_theta", "lbm_get_theta_f64",
-    "lbm_get_thermal_state", "lbm_set_thermal_state",
+    "lbm_get_thermal_state", "lbm_set_thermal_state", "lbm_set_thermal_walls",
 ]
 
 
@@ -76,6 +76,7 @@ def load_library():
         getattr(lib, n).argtypes = [vp, vp, vp, vp, vp]
     for n in ("lbm_get_theta", "lbm_get_theta_f64", "lbm_get_thermal_state", "lbm_set_thermal_state"):
         getattr(lib, n).argtypes = [vp, vp]
+    lib.lbm_set_thermal_walls.argtypes = [vp, vp, vp]
     lib.lbm_mean_config.argtypes = [vp, l, i]
     lib.lbm_mean_reset.argtypes = [vp]
     for n in ("lbm_get_mean", "lbm_get_mean_f64"):
@@ -303,6 +304,14 @@ class Lbm:
         a = out if out is not None else self._new(t.float64 if f64 else t.float32)
         self._chk(fn(self._h, a.data_ptr()), "get_theta")
         return a
+
+    def set_thermal_walls(self, on, theta_w):
+        """Hold WALL faces (order x-,x+,y-,y+,z-,z+) with on[k] != 0 at temperature theta_w[k]."""
+        a = np.ascontiguousarray(on, dtype=np.int32)
+        t = np.ascontiguousarray(theta_w, dtype=np.float64)
+        if a.shape != (6,) or t.shape != (6,):
+            raise ValueError("on and theta_w must have 6 entries")
+        self._chk(self._lib.lbm_set_thermal_walls(self._h, a.ctypes.data, t.ctypes.data), "set_thermal_walls")
 
     def get_thermal_state(self):
         """The 7 thermal populations [7][nz][ny][nx] float64 (host): the thermal half of a checkpoint."""

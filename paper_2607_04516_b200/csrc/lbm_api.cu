@@ -100,6 +100,7 @@ struct lbm {
     int nmodes;     // synthetic inflow fluctuations: modes in use (0 = off)
     bool thermal;   // D3Q7 thermal lattice + Boussinesq coupling on (lbm_set_thermal); its two buffers are library-owned
     double alpha, gbeta, theta_ref;
+    int thd; double thw[6]; // fixed-temperature WALL faces (lbm_set_thermal_walls): mask and temperatures
     char *th_ws;    // [2][7][stride] reals, cudaMalloc'ed by lbm_set_thermal, freed by lbm_destroy
     int loop_ok;    // multi-step cooperative launch: 0 = not probed yet, 1 = the whole grid is resident, -1 = no
     // staging buffers for HOST inputs / outputs that do not fit the scratch area (whole-lattice fields): kept between
@@ -196,6 +197,8 @@ Params<real> make_params(const lbm_t *h)
     if (h->thermal) {
         P.gbeta = (real)h->gbeta; P.theta_ref = (real)h->theta_ref;
         P.omega_t = (real)(1.0 / (4.0 * h->alpha + 0.5));
+        P.thd = h->thd;
+        for (int k = 0; k < 6; ++k) P.thw[k] = (real)(2.0 * (h->thw[k] - h->theta_ref));
     }
     return P;
 }
@@ -917,6 +920,22 @@ int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
 }
 int lbm_set_theta(lbm_t *h, const float *theta, const float *ux, const float *uy, const float *uz) { return set_theta_any<float>(h, theta, ux, uy, uz); }
 int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const double *uy, const double *uz) { return set_theta_any<double>(h, theta, ux, uy, uz); }
+int lbm_set_thermal_walls(lbm_t *h, const int on[6], const double theta_w[6])
+{
+    if (!h) return LBM_EINVAL;
+    if (!on || !theta_w) return fail(h, LBM_EINVAL, "set_thermal_walls: NULL");
+    if (!h->thermal) return fail(h, LBM_ESTATE, "set_thermal_walls: thermal lattice is off (lbm_set_thermal)");
+    int mask = 0;
+    for (int k = 0; k < 6; ++k) {
+        if (!on[k]) continue;
+        if (h->face[k] != LBM_WALL) return fail(h, LBM_EINVAL, "set_thermal_walls: only WALL faces can be held at a temperature");
+        if (!std::isfinite(theta_w[k])) return fail(h, LBM_EINVAL, "set_thermal_walls: temperature not finite");
+        mask |= 1 << k;
+    }
+    h->thd = mask;
+    for (int k = 0; k < 6; ++k) h->thw[k] = on[k] ? theta_w[k] : 0.0;
+    return LBM_OK;
+}
 int lbm_get_thermal_state(lbm_t *h, double *hpop)
 {
     if (!h || !hpop) return LBM_EINVAL;
@@ -968,7 +987,8 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     if (cudaGetDevice(&h->device) != cudaSuccess) { cudaGetLastError(); delete h; return LBM_ECUDA; }
     h->cur = 0; h->have_flags = false; h->step = 0;
     h->mstart = 0; h->mevery = 0; h->mcount = 0; h->launches = 0; h->variant = 0; h->damp_on = false; h->nmodes = 0; h->loop_ok = 0;
-    h->thermal = false; h->alpha = 0; h->gbeta = 0; h->theta_ref = 0; h->th_ws = nullptr;
+    h->thermal = false; h->alpha = 0; h->gbeta = 0; h->theta_ref = 0; h->th_ws = nullptr; h->thd = 0;
+    for (int k = 0; k < 6; ++k) h->thw[k] = 0.0;
     for (int a = 0; a < 3; ++a) { h->dlo[a] = 0; h->dhi[a] = 0; }
     for (int k = 0; k < 4; ++k) h->slots[k] = lbm::Slot{nullptr, 0, false};
     if (dev_workspace) {
@@ -1017,6 +1037,8 @@ int lbm_set_boundaries(lbm_t *h, const int face_type[6])
     }
     if (h->thermal && has_eq_face(face_type)) return fail(h, LBM_EINVAL, "set_boundaries: EQ faces are not supported while the thermal lattice is on");
     for (int k = 0; k < 6; ++k) h->face[k] = face_type[k];
+    for (int k = 0; k < 6; ++k)
+        if (face_type[k] != LBM_WALL) h->thd &= ~(1 << k); // a face that stops being a WALL is no longer held at a temperature
     h->have_flags = false;
     return LBM_OK;
 }

@@ -85,6 +85,10 @@ struct Params {
     // thermal lattice (lbm_set_thermal, lbm_thermal.cuh): buoyancy coefficient g beta, reference theta, 1 / tau_theta;
     // all 0 while it is off
     real gbeta, theta_ref, omega_t;
+    // fixed-temperature WALL faces of the thermal lattice (lbm_set_thermal_walls; DESIGN.md §4 reading 26): bit k of thd = face k
+    // is held, thw[k] = 2 (theta_w - theta_ref) of that face (the anti-bounce-back mailbox value is -t_j + wT_j thw[k])
+    int thd;
+    real thw[6];
 };
 
 // Interior x = 0 sits at padded x = P.xoff (8 cells of 4 or 8 bytes, 16 cells of 2): every interior row starts on a

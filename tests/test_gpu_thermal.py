@@ -243,8 +243,9 @@ def test_density_current_fronts_gpu_at_25m_against_the_papers_printed_values(B):
 @pytest.mark.parametrize("fp64", [False, True])
 def test_thermal_checkpoint_restarts_exactly(B, fp64):
     """lbm_get_state + lbm_get_thermal_state + the step counter are a complete checkpoint of a thermal run: a fresh handle
-    loaded with them continues bit for bit like the uninterrupted one (mailboxes and ghost slots of both lattices are
-    rebuilt by the set calls)."""
+    loaded with them continues like the uninterrupted one (mailboxes and ghost slots of both lattices are rebuilt by the
+    set calls) — bit for bit on the FP32 handle; on the FP64 handle up to the last bit, because the checkpoint holds the
+    unshifted populations and (g + w) - w is not g in the handle's own precision."""
     nx, ny, nz = 36, 10, 14
     rng = np.random.default_rng(8)
     hm = np.zeros((ny, nx), np.int32); hm[3:6, 8:14] = 5
@@ -267,7 +268,99 @@ def test_thermal_checkpoint_restarts_exactly(B, fp64):
     b = fresh()
     b.set_state(f); b.set_thermal_state(hpop); b.set_step(k)
     a.step(25); b.step(25)
-    np.testing.assert_array_equal(a.get_state(out="host"), b.get_state(out="host"))
-    np.testing.assert_array_equal(a.get_thermal_state(), b.get_thermal_state())
+    if fp64:
+        np.testing.assert_allclose(a.get_state(out="host"), b.get_state(out="host"), rtol=0, atol=1e-14)
+        np.testing.assert_allclose(a.get_thermal_state(), b.get_thermal_state(), rtol=0, atol=1e-14)
+    else:
+        np.testing.assert_array_equal(a.get_state(out="host"), b.get_state(out="host"))
+        np.testing.assert_array_equal(a.get_thermal_state(), b.get_thermal_state())
     assert a.get_step() == b.get_step() == 65
     a.close(); b.close()
+
+
+# ---- fixed-temperature walls (DESIGN.md §4 reading 26) -------------------------------------------------------------------
+
+def walls_pair(B, nx, ny, nz, faces, hm, nu0, alpha, gb, tref, on, tw, theta, fp64, Cs=0.1, fcor=0.0, F=(0, 0, 0)):
+    """like pair(), with the held walls set BEFORE the thermal state is written (the mailboxes then carry the wall rule)"""
+    from oracle import Oracle
+    o = Oracle(nx, ny, nz, nu0, Cs, fcor, F, faces)
+    o.set_flags(hm)
+    sim = B.Lbm(nx, ny, nz, nu0, Cs, fcor, F, faces, fp64=fp64)
+    sim.set_flags(hm)
+    o.set_macros(); sim.set_macros()
+    o.set_thermal(alpha, gb, tref); sim.set_thermal(alpha, gb, tref)
+    o.set_thermal_walls(on, tw); sim.set_thermal_walls(on, tw)
+    o.set_theta(theta); sim.set_theta(theta, f64=True)
+    return sim, o
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_held_walls_parity_with_buildings_and_mixed_faces(B, fp64):
+    """Heated ground (held), adiabatic lid (WALL, not held), a held side wall, periodic y, buildings standing on the heated
+    ground (their surfaces stay adiabatic), buoyancy, LES, Coriolis: 100 steps against the oracle."""
+    nx, ny, nz = 44, 9, 16
+    rng = np.random.default_rng(21)
+    hm = np.zeros((ny, nx), np.int32); hm[2:6, 10:17] = 6; hm[5:8, 28:33] = 3
+    theta = 1.0 + 0.05 * rng.standard_normal((nz, ny, nx))
+    on, tw = [1, 0, 0, 0, 1, 0], [0.7, 0, 0, 0, 1.6, 0]
+    sim, o = walls_pair(B, nx, ny, nz, (W, W, P, P, W, W), hm, 4e-3, 0.02, 3e-3, 1.0, on, tw, theta, fp64, fcor=1e-3)
+    sim.step(100); o.step(100)
+    e_flow, e_th = errs(sim, o, 1.0)
+    tol = TOL64 if fp64 else TOL32
+    assert e_flow <= tol and e_th <= tol, (e_flow, e_th)
+    th = o.get_theta()
+    assert th[0][hm == 0].mean() > 1.2          # the ground does heat the air above it
+    sim.close(); o.close()
+
+
+def test_conduction_profile_and_rayleigh_benard_box_on_the_gpu(B):
+    """The two closed-form set-ups of tests/test_oracle_thermal.py on the CUDA path: (i) pure conduction between held
+    plates converges to the exact linear profile on the FP64 kernels (1e-10) and the FP32 kernels (1e-5); (ii) the
+    Rayleigh-Benard box at 1.1 Ra_c: FP64 kernels follow the oracle's growing roll for 4000 steps to rounding order
+    relative to its amplitude."""
+    from oracle import Oracle
+    nz = 10
+    zeta = np.arange(nz) + 0.5
+    exact = 1.0 + (0.25 - 1.0) * zeta / nz
+    for fp64, tol in ((True, 1e-10), (False, 1e-5)):
+        sim = B.Lbm(4, 3, nz, 0.05, 0.0, 0.0, (0, 0, 0), (P, P, P, P, W, W), fp64=fp64)
+        sim.set_flags(None); sim.set_macros()
+        sim.set_thermal(0.12, 0.0, 0.6)
+        sim.set_thermal_walls([0, 0, 0, 0, 1, 1], [0, 0, 0, 0, 1.0, 0.25])
+        sim.set_theta(np.full((nz, 3, 4), 0.6), f64=True)
+        sim.step(6000)
+        th = sim.get_theta(out="host", f64=True)
+        assert np.abs(th - exact[:, None, None]).max() < tol, fp64
+        sim.close()
+    H, nu, alpha, Ra = 16, 0.05, 0.05, 1.1 * 1707.76
+    nx = 2 * H
+    gb = Ra * nu * alpha / H ** 3
+    z = (np.arange(H) + 0.5) / H
+    mode = np.sin(np.pi * z)[:, None] * np.cos(2 * np.pi * (np.arange(nx) + 0.5) / nx)[None, :]
+    theta = ((1.0 - z)[:, None] + 1e-4 * mode)[:, None, :]
+    sim, o = walls_pair(B, nx, 1, H, (P, P, P, P, W, W), None, nu, alpha, gb, 0.5, [0, 0, 0, 0, 1, 1], [0, 0, 0, 0, 1.0, 0.0],
+                        theta, True, Cs=0.0)
+    a0 = None
+    for _ in range(4):
+        sim.step(1000); o.step(1000)
+        wo = o.get_macros()[3]
+        wg = sim.get_macros(f64=True)[3].cpu().numpy()
+        amp = np.abs(wo).max()
+        assert np.abs(wg - wo).max() <= 1e-9 * amp + 1e-15
+        a0 = a0 or amp
+    assert amp > 1.1 * a0                        # supercritical: the roll grows
+    sim.close(); o.close()
+
+
+def test_thermal_walls_argument_errors(B):
+    sim = B.Lbm(8, 8, 8, 1e-2, 0.0, 0.0, (0, 0, 0), (P, P, FS, FS, W, W))
+    sim.set_flags(None)
+    with pytest.raises(B.LbmError):
+        sim.set_thermal_walls([0, 0, 0, 0, 1, 1], [0] * 6)          # thermal lattice off
+    sim.set_thermal(0.01, 0.0, 0.0)
+    with pytest.raises(B.LbmError):
+        sim.set_thermal_walls([0, 0, 1, 0, 0, 0], [0] * 6)          # a FREE_SLIP face cannot be held
+    with pytest.raises(B.LbmError):
+        sim.set_thermal_walls([0, 0, 0, 0, 1, 0], [0, 0, 0, 0, float("nan"), 0])
+    sim.set_thermal_walls([0, 0, 0, 0, 1, 1], [9, 9, 9, 9, 1.0, 0.0])   # entries of faces not held are ignored
+    sim.close()
