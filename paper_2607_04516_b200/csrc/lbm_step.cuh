@@ -124,16 +124,25 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
         fl = flags[p];
     }
     if constexpr (SPEC) {
-        // Fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, no feed, nothing to complete)
-        // — the bulk of the lattice.  Straight-line collide + 19 stores, none of the per-feature tests below.
-        if (__all_sync(__activemask(), fl == 0)) {
+        // Fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, nothing to complete) — the
+        // bulk of the lattice — or an EQ cell / a feeding cell without wall link or ghost slot (the inlet and outflow cells
+        // at the two ends of every row).  Straight-line collide (or equilibrium re-expansion) + 19 stores, none of the
+        // per-feature tests below.
+        const bool plain = (fl & (SLOW_BIT | EDGE_BIT | SURF_BIT)) == 0 && (fl & CLASS_MASK) != SOLID && (fl & CLASS_MASK) != GHOST;
+        if (__all_sync(__activemask(), plain)) {
             Macro<real> m;
-            if constexpr (DAMP) m = collide<real, true>(g, P, dmp);
-            else m = collide(g, P);
+            if ((fl & CLASS_MASK) == FLUID) {
+                if constexpr (DAMP) m = collide<real, true>(g, P, dmp);
+                else m = collide(g, P);
+            } else {
+                m = Macro<real>{real(1), fu0, fu1, fu2};
+                equilibrium(g, real(0), fu0, fu1, fu2);
+            }
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 st_s(T.dst[i] + p, g[i]);
             });
+            if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) { fuw[comp * P.F + sl] = v; });
             if constexpr (MEAN) {
                 msum[p] = ms0 + m.ux;
                 msum[P.stride + p] = ms1 + m.uy;
