@@ -465,7 +465,7 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     if (!rc) {
         const int B = 256;
         init_kernel<real, S, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+            (S *)h->bufA(), (S *)nullptr, (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
         rc = check_launch(h, "init_kernel");
     }
@@ -613,7 +613,7 @@ int try_step_loop(lbm_t *h, const Params<real> &P, int want)
         if (h->variant != 0 || h->nmodes > 0 || h->thermal || want < 4 || h->loop_ok < 0) return 0;
         constexpr int BLOCK = 128;
         const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
-        const void *fn = h->damp_on ? (const void *)step_loop_kernel<float, S, BLOCK, 10, true> : (const void *)step_loop_kernel<float, S, BLOCK, 10, false>;
+        const void *fn = h->damp_on ? (const void *)step_loop_kernel<float, S, BLOCK, 8, true> : (const void *)step_loop_kernel<float, S, BLOCK, 8, false>;
         if (h->loop_ok == 0) { // once per handle: can the whole grid be resident?
             int dev = 0, sms = 0, coop = 0, per_sm = 0;
             cudaGetDevice(&dev);
@@ -745,7 +745,7 @@ int do_set_state(lbm_t *h, const double *f)
     int rc = stage_in(h, f, (size_t)Q * P.N * sizeof(double), h->L.scratch_bytes, &in);
     if (rc) return rc;
     const int B = 256;
-    state_in_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), h->links(),
+    state_in_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((S *)h->bufA(), (S *)nullptr, (real *)h->fu(), h->flags(), h->links(),
                                                                     (const double *)in.dev, P);
     rc = check_launch(h, "state_in_kernel");
     release_in(h, &in, 1);

@@ -140,29 +140,6 @@ __device__ __forceinline__ Damp<real> damp_at(const Params<real> &P, int x, int 
     return Damp<real>{sg, t[z], t[P.nz + z], t[2 * P.nz + z]};
 }
 
-// 1 / x and sqrt(x) of the collision.  FP64: IEEE.  FP32: the hardware approximation (MUFU), the reciprocal refined by one
-// Newton step — both within ~1 ulp for the operands that occur (rho, tau in [0.5, 2]; Q, tau0^2 + ... >= 0; sqrt.approx
-// returns 0 for 0), without the denormal / special-case slow paths of the IEEE sequences, which cost ~30 instructions
-// and 8 branch-structure instructions per cell for cases that cannot occur (two orders below the 1e-5 bar).
-template <typename real>
-__device__ __forceinline__ real rcp_c(real x) { return real(1) / x; }
-template <>
-__device__ __forceinline__ float rcp_c<float>(float x)
-{
-    float r;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return fmaf(r, fmaf(-x, r, 1.0f), r);
-}
-template <typename real>
-__device__ __forceinline__ real sqrt_c(real x) { return sqrt(x); }
-template <>
-__device__ __forceinline__ float sqrt_c<float>(float x)
-{
-    float r;
-    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
-    return r;
-}
-
 // ---- collision (DESIGN.md §3 steps 4b-4e) on shifted populations ---------------------------------------------------
 // In: pulled g[19].  Out: post-collision g[19]; returns the (rho,u) the collision used.
 template <typename real, bool DAMP = false>
@@ -181,7 +158,7 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
     const real Mzz = (s[3] + s[5]) + (s[6] + s[8]) + s[9];
     const real Mxy = s[4] - s[7], Mxz = s[5] - s[8], Myz = s[6] - s[9];
     const real rho = real(1) + drho;
-    const real inv = rcp_c(rho);
+    const real inv = real(1) / rho;
     // 4c: implicit half-force velocity.  a(u) = F - f x u, so rho u = m + rho a(u)/2 reads u + h x u = b with h = f/2,
     // b = m/rho + F/2, whose solution is u = (b - h x b + h (h.b)) / (1 + |h|^2)
     const real bx = mx * inv + real(0.5) * P.Fx, by = my * inv + real(0.5) * P.Fy, bz = mz * inv + real(0.5) * P.Fz;
@@ -202,15 +179,6 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
         Fdx = rho * (P.Fx - (P.fy * uz - P.fz * uy) + dm.sg * (dm.utx - ux));
         Fdy = rho * (P.Fy - (P.fz * ux - P.fx * uz) + dm.sg * (dm.uty - uy));
         Fdz = rho * (P.Fz - (P.fx * uy - P.fy * ux) + dm.sg * (dm.utz - uz));
-    } else if (P.fx == real(0) && P.fy == real(0)) {
-        // rotation about z only (lbm_create's scalar f_cor, every BASELINE.json config): the same solve with h = (0, 0, hz)
-        // written out — u_z = b_z exactly; a launch-uniform branch
-        ux = (bx + P.hz * by) * P.inv1ph2;
-        uy = (by - P.hz * bx) * P.inv1ph2;
-        uz = bz;
-        Fdx = rho * (P.Fx + P.fz * uy);
-        Fdy = rho * (P.Fy - P.fz * ux);
-        Fdz = rho * P.Fz;
     } else {
         const real hb = P.hx * bx + P.hy * by + P.hz * bz;
         ux = (bx - (P.hy * bz - P.hz * by) + P.hx * hb) * P.inv1ph2;
@@ -226,9 +194,9 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
     const real Pyy = Myy - third * drho - rho * uy * uy;
     const real Pzz = Mzz - third * drho - rho * uz * uz;
     const real Pxy = Mxy - rho * ux * uy, Pxz = Mxz - rho * ux * uz, Pyz = Myz - rho * uy * uz;
-    const real Qn = sqrt_c(Pxx * Pxx + Pyy * Pyy + Pzz * Pzz + real(2) * (Pxy * Pxy + Pxz * Pxz + Pyz * Pyz));
-    const real tau = real(0.5) * (P.tau0 + sqrt_c(P.tau0 * P.tau0 + P.Kles * Qn * inv));
-    const real omega = rcp_c(tau);
+    const real Qn = sqrt(Pxx * Pxx + Pyy * Pyy + Pzz * Pzz + real(2) * (Pxy * Pxy + Pxz * Pxz + Pyz * Pyz));
+    const real tau = real(0.5) * (P.tau0 + sqrt(P.tau0 * P.tau0 + P.Kles * Qn * inv));
+    const real omega = real(1) / tau;
     const real phi = real(1) - real(0.5) * omega;
     // 4e: BGK + Guo source.  With base = omega A0 - 3 phi uF, P1 = omega rho u, P2 = phi Fd and, per weight group,
     //   E0 = w base,  v = w (4.5 P1 + 9 P2),  o = 3 w (P1 + P2):

@@ -111,14 +111,17 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restric
     flags[p] = (uint8_t)(cls | extra);
 }
 
-// store one cell's state into BOTH buffers (set-up paths: the two buffers start identical), and publish its velocity
-// to the outflow cells it feeds (both halves of the double-buffered side array)
+// store one cell's state into BOTH buffers (boundary cells rewritten while a run is under way: whichever buffer is current
+// must hold them) or, with B == nullptr, into A only (whole-lattice writes, after which A is the current buffer: the first
+// step rewrites every slot of B that is ever read — own slots, mailboxes, ghost slots, EQ cells, sector completions — so
+// filling B too would be 76 B per cell of wasted writes), and publish its velocity to the outflow cells it feeds (both
+// halves of the double-buffered side array)
 template <typename real, typename S>
 __device__ __forceinline__ void store_cell_both(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const Params<real> &P,
                                                 int p, int x, int y, int z, uint8_t fl, uint32_t lk, const real (&g)[Q])
 {
     store_cell(A, P, p, x, y, z, fl, lk, g);
-    store_cell(B, P, p, x, y, z, fl, lk, g);
+    if (B) store_cell(B, P, p, x, y, z, fl, lk, g); // B == nullptr: whole-lattice writes (init, checkpoint) fill the current buffer only
     const int cls = fl & CLASS_MASK;
     if ((fl & FEED_BIT) || cls == EQ_FIXED) {
         const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));

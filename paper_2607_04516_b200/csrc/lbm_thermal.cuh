@@ -50,12 +50,15 @@ __device__ __forceinline__ void store_cell_thermal(real *__restrict__ HB, const 
         // pull direction i = 1..6 crosses face k = i - 1 when the cell lies on it (1: x-, 2: x+, 3: y-, 4: y+, 5: z-, 6: z+).
         // A WALL face held at theta_w returns the population anti-bounced: -t_j + 2 wT_j (theta_w - theta_ref), wT_j = 1/8
         // (DESIGN.md §4 reading 26); every other wall link (buildings, adiabatic walls) bounces it back unchanged.
-        const int at[6] = {x == 0, x == P.nx - 1, y == 0, y == P.ny - 1, z == 0, z == P.nz - 1};
         static_for<1, QT>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             if ((lk >> i) & 1u) {
-                const bool held = ((P.thd >> (i - 1)) & 1) && at[i - 1];
-                HB[(long long)i * P.stride + (p - poff<i>(P))] = held ? real(0.125) * P.thw[i - 1] - t[dir_opp(i)] : t[dir_opp(i)];
+                real v = t[dir_opp(i)];
+                if (P.thd) { // rare: only handles with held walls pay for the test
+                    const bool at = i == 1 ? x == 0 : i == 2 ? x == P.nx - 1 : i == 3 ? y == 0 : i == 4 ? y == P.ny - 1 : i == 5 ? z == 0 : z == P.nz - 1;
+                    if (at && ((P.thd >> (i - 1)) & 1)) v = real(0.125) * P.thw[i - 1] - v;
+                }
+                HB[(long long)i * P.stride + (p - poff<i>(P))] = v;
             }
         });
     }
