@@ -366,7 +366,8 @@ def run_ours(args):
         BYTES_PER_CELL = {"thermal": 209, "c3-fp16": 77}.get(args.workload, globals()["BYTES_PER_CELL"])
         achieved = BYTES_PER_CELL * cells / per_launch_s / 1e9
         traffic, traffic_src = (load_traffic("step") if args.workload == "c3" else
-                                load_traffic("thermal") if args.workload == "thermal" else (None, None))
+                                load_traffic("thermal") if args.workload == "thermal" else
+                                load_traffic("s16") if args.workload == "c3-fp16" else (None, None))
         if traffic_src:
             traffic_src += " (committed ncu --set full capture; a constant, not measured in this run)"
         if sustained is not None:

@@ -164,7 +164,8 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
  * other EQ_FIXED cell keeps the mean.  The mean is the boundary state in force when the call is made: while
  * fluctuations are on, lbm_set_inlet_profile / _plane, lbm_feed_inlet and lbm_balance_flux return LBM_ESTATE.
  * n_modes = 0 switches them off and restores the mean (modes may be NULL).  lbm_set_flags switches them off too.
- * Cost per step: one extra small launch over the face slots (n_modes cosines per active cell), no lattice traffic.
+ * Cost per step: no extra launch — the face slots ride in extra leading block rows of the step launch itself (n_modes
+ * cosines per active cell), no lattice traffic.
  * LBM_EINVAL: n_modes < 0 or > LBM_MAX_INFLOW_MODES, k_e <= 0, u_rms < 0, k_eta < 0, dkappa < 0, non-finite or device
  * table.  Needs flags (else LBM_ESTATE).  Synchronises. */
 #define LBM_MAX_INFLOW_MODES 1024

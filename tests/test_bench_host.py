@@ -82,3 +82,5 @@ def test_traffic_figure_comes_from_the_committed_profile():
     assert (t is None) == (src is None) and (src is None or os.path.exists(os.path.join(ROOT, src)))
     th, _ = bench.load_traffic("thermal")  # fused flow + thermal kernel: (19 + 7) x 4 B x 2 + 1 flag byte = 209 B/cell
     assert th is None or 0.9 * 209 * 16e6 < th < 1.3 * 209 * 16e6
+    s16, _ = bench.load_traffic("s16")      # 16-bit population storage: 19 x 2 B x 2 + 1 flag byte = 77 B/cell
+    assert s16 is None or 0.9 * 77 * 16e6 < s16 < 1.3 * 77 * 16e6
