@@ -535,6 +535,9 @@ constexpr int N_VARIANTS = 4;
 #ifndef DAMP_MINB
 #define DAMP_MINB 9
 #endif
+#ifndef THERMAL_MINB
+#define THERMAL_MINB 9
+#endif
 #ifndef VEC4_MINB
 #define VEC4_MINB 4
 #endif
@@ -548,11 +551,13 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         const real *A = (const real *)h->state();
         real *B = (real *)h->other();
         dim3 grid(blocks_for((long long)P.nxy, 128), (unsigned)P.nz);
-        // 19 + 7 populations: 72 registers hold them without spills = 7 CTAs per SM (measured 24 900 MLUPS; 6 CTAs / 80
-        // registers 24 000, 5 CTAs 22 600, 8 CTAs / 64 registers with 16 B of spills 24 900)
-        constexpr int BLOCK = 128, MINB = std::is_same<real, float>::value ? 7 : 2;
-        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
-        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(A, B, (const real *)h->th_state(), (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P);
+        // 19 + 7 populations.  With the buoyancy passed into collide() as a value (P stays in the constant bank) and the address
+        // table, 56 registers (9 CTAs per SM, 16 B of spills) measure best: 26 030 MLUPS against 25 860 at 8 CTAs (64 registers, no
+        // spills), 24 450 at 10 CTAs (48 registers, 108 B of spills) and round 1's 24 600 at 7 CTAs (72 registers)
+        constexpr int BLOCK = 128, MINB = std::is_same<real, float>::value ? THERMAL_MINB : 2;
+        const ThermalPtrs<real> T = make_thermal_ptrs<real>(A, B, (const real *)h->th_state(), (real *)h->th_other(), P);
+        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T);
+        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T);
         return check_launch(h, "thermal_step_kernel");
     }
     const bool turb = h->nmodes > 0 && P.F > 0;

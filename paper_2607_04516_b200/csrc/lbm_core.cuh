@@ -142,9 +142,12 @@ __device__ __forceinline__ Damp<real> damp_at(const Params<real> &P, int x, int 
 
 // ---- collision (DESIGN.md §3 steps 4b-4e) on shifted populations ---------------------------------------------------
 // In: pulled g[19].  Out: post-collision g[19]; returns the (rho,u) the collision used.
-template <typename real, bool DAMP = false>
-__device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> &P, const Damp<real> dm = Damp<real>{})
+// BUOY: fb = an extra acceleration along z of this cell (the Boussinesq buoyancy g beta (theta - theta_ref) of the thermal
+// lattice, lbm_thermal.cuh), added to P.Fz — passed as a value so that P stays the kernel parameter (constant bank).
+template <typename real, bool DAMP = false, bool BUOY = false>
+__device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> &P, const Damp<real> dm = Damp<real>{}, const real fb = real(0))
 {
+    const real PFz = BUOY ? P.Fz + fb : P.Fz;
     real s[10], d[10];
 #pragma unroll
     for (int k = 1; k <= 9; ++k) { s[k] = g[2 * k - 1] + g[2 * k]; d[k] = g[2 * k - 1] - g[2 * k]; }
@@ -161,7 +164,7 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
     const real inv = real(1) / rho;
     // 4c: implicit half-force velocity.  a(u) = F - f x u, so rho u = m + rho a(u)/2 reads u + h x u = b with h = f/2,
     // b = m/rho + F/2, whose solution is u = (b - h x b + h (h.b)) / (1 + |h|^2)
-    const real bx = mx * inv + real(0.5) * P.Fx, by = my * inv + real(0.5) * P.Fy, bz = mz * inv + real(0.5) * P.Fz;
+    const real bx = mx * inv + real(0.5) * P.Fx, by = my * inv + real(0.5) * P.Fy, bz = mz * inv + real(0.5) * PFz;
     real ux, uy, uz, Fdx, Fdy, Fdz;
     bool damped = false;
     if constexpr (DAMP) damped = dm.sg > real(0);
@@ -178,7 +181,7 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
         uz = (A2 * cz - A * (P.hx * cy - P.hy * cx) + P.hz * hb) * den;
         Fdx = rho * (P.Fx - (P.fy * uz - P.fz * uy) + dm.sg * (dm.utx - ux));
         Fdy = rho * (P.Fy - (P.fz * ux - P.fx * uz) + dm.sg * (dm.uty - uy));
-        Fdz = rho * (P.Fz - (P.fx * uy - P.fy * ux) + dm.sg * (dm.utz - uz));
+        Fdz = rho * (PFz - (P.fx * uy - P.fy * ux) + dm.sg * (dm.utz - uz));
     } else {
         const real hb = P.hx * bx + P.hy * by + P.hz * bz;
         ux = (bx - (P.hy * bz - P.hz * by) + P.hx * hb) * P.inv1ph2;
@@ -186,7 +189,7 @@ __device__ __forceinline__ Macro<real> collide(real (&g)[Q], const Params<real> 
         uz = (bz - (P.hx * by - P.hy * bx) + P.hz * hb) * P.inv1ph2;
         Fdx = rho * (P.Fx - (P.fy * uz - P.fz * uy));
         Fdy = rho * (P.Fy - (P.fz * ux - P.fx * uz));
-        Fdz = rho * (P.Fz - (P.fx * uy - P.fy * ux));
+        Fdz = rho * (PFz - (P.fx * uy - P.fy * ux));
     }
     // 4d: Pi = sum c c (f - feq) = M - (drho/3) I - rho u u   (second moment of the shifted equilibrium is exact)
     const real third = real(1) / real(3);

@@ -89,7 +89,10 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
     if (c2 >= (unsigned)P.nxy) return;
     const int y = P.nx_magic ? (int)__umulhi(c2, P.nx_magic) : (int)(c2 / (unsigned)P.nx);
     const int x = (int)c2 - y * P.nx;
-    const int z = zb;
+    // Block rows are dispatched in order; the planes whose cells all take the slow path (the top plane under a FREE_SLIP /
+    // PERIODIC lid: a ghost store sequence per cell) must not be the tail of the launch, where nothing is left to overlap
+    // them with: the last plane goes first, everything else one later.
+    const int z = zb == 0 ? P.nz - 1 : zb - 1;
     const int p = pidx(P, x, y, z);
 
     real g[Q];

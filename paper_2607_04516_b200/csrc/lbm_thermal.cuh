@@ -69,43 +69,59 @@ __device__ __forceinline__ void store_cell_thermal(real *__restrict__ HB, const 
         });
 }
 
-// Params with the buoyancy of a cell added to the body force (the arithmetic of collide / local_macros is untouched)
+// Per-launch address table of the 26 streams, as StepPtrs for the plain kernel: src = buffer + i stride - off_i (the pull of
+// direction i is src[i][p]), dst = buffer + i stride.  One 64-bit add per access instead of a 64-bit multiply-add chain.
 template <typename real>
-__device__ __forceinline__ Params<real> with_buoyancy(const Params<real> &P, real dth)
+struct ThermalPtrs {
+    const real *gsrc[Q];
+    real *gdst[Q];
+    const real *tsrc[QT];
+    real *tdst[QT];
+};
+template <typename real>
+inline ThermalPtrs<real> make_thermal_ptrs(const real *A, real *B, const real *HA, real *HB, const Params<real> &P)
 {
-    Params<real> Pl = P;
-    Pl.Fz = P.Fz + P.gbeta * dth;
-    return Pl;
+    ThermalPtrs<real> t;
+    for (int i = 0; i < Q; ++i) {
+        const long long off = dir_cx(i) + (long long)dir_cy(i) * P.px + (long long)dir_cz(i) * P.pxy;
+        t.gsrc[i] = A + ((long long)i * P.stride - off);
+        t.gdst[i] = B + (long long)i * P.stride;
+        if (i < QT) {
+            t.tsrc[i] = HA + ((long long)i * P.stride - off);
+            t.tdst[i] = HB + (long long)i * P.stride;
+        }
+    }
+    return t;
 }
 
 template <typename real, bool MEAN, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
-thermal_step_kernel(const real *__restrict__ A, real *__restrict__ B, const real *__restrict__ HA, real *__restrict__ HB,
-                    const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links, real *__restrict__ msum, const Params<real> P)
+thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+                    real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T)
 {
     const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x;
     if (c2 >= (unsigned)P.nxy) return;
     const int y = P.nx_magic ? (int)__umulhi(c2, P.nx_magic) : (int)(c2 / (unsigned)P.nx);
     const int x = (int)c2 - y * P.nx;
-    const int z = blockIdx.y;
+    const int z = blockIdx.y == 0 ? P.nz - 1 : (int)blockIdx.y - 1; // the all-slow top plane first, not as the tail (lbm_step.cuh)
     const int p = pidx(P, x, y, z);
     // as in step_kernel's SPEC instantiations: all 26 pulls are issued before the flag byte has arrived (no dependent
     // round trip; a SOLID cell then costs its reads), pinned by volatile asm so that the flag test cannot move above them
     real g[Q], t[QT];
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        g[i] = ld_pinned(A + ((long long)i * P.stride + (p - poff<i>(P))));
+        g[i] = ld_pinned(T.gsrc[i] + p);
     });
     static_for<0, QT>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        t[i] = ld_pinned(HA + ((long long)i * P.stride + (p - poff<i>(P))));
+        t[i] = ld_pinned(T.tsrc[i] + p);
     });
     const uint8_t fl = ld_pinned(flags + p);
     // the collision pair of one FLUID cell: buoyancy from the pulled theta into the flow collision, thermal BGK towards
     // h_eq(theta, u) of that collision's velocity
     auto collide_both = [&]() {
         const real dth = theta_shift(t);
-        const Macro<real> m = collide(g, with_buoyancy(P, dth));
+        const Macro<real> m = collide<real, false, true>(g, P, Damp<real>{}, P.gbeta * dth);
         real e[QT];
         thermal_equilibrium(e, dth, P.theta_ref, m.ux, m.uy, m.uz);
 #pragma unroll
@@ -117,11 +133,11 @@ thermal_step_kernel(const real *__restrict__ A, real *__restrict__ B, const real
         const Macro<real> m = collide_both();
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            B[(long long)i * P.stride + p] = g[i];
+            T.gdst[i][p] = g[i];
         });
         static_for<0, QT>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            HB[(long long)i * P.stride + p] = t[i];
+            T.tdst[i][p] = t[i];
         });
         if constexpr (MEAN) {
             msum[p] += m.ux;
