@@ -213,7 +213,8 @@ int lbm_set_thermal_state(lbm_t *h, const double *hpop);
 int lbm_feed_inlet(lbm_t *dst, const lbm_t *src, int src_x_plane);
 
 /* Initial state G0 = f_eq(rho, u) (DESIGN.md §3 step 3).  NULL rho = 1; NULL component = 0.  SOLID cells get
- * rho = 1, u = 0; EQ_FIXED cells keep their boundary state.  Resets the step counter.  Needs flags. */
+ * rho = 1, u = 0; EQ_FIXED cells keep their boundary state.  Resets the step counter; the mean sums and their sample count
+ * are left alone (lbm_mean_reset clears them; a new lbm_set_flags* does too).  Needs flags. */
 int lbm_set_macros(lbm_t *h, const float *rho, const float *ux, const float *uy, const float *uz);
 int lbm_set_macros_f64(lbm_t *h, const double *rho, const double *ux, const double *uy, const double *uz);
 

@@ -367,7 +367,7 @@ int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, con
     if (!rc) rc = stage_in(h, w, bytes, 2 * align_up(bytes, ALIGN), &in[2]); else in[2] = InBuf{nullptr, nullptr, false, -1};
     if (!rc) {
         const int B = 256;
-        const long long threads = mode == 0 ? (long long)P.N : (long long)count;
+        const long long threads = mode == 0 ? (long long)std::max(P.F, 1) : (long long)count;
         inlet_kernel<real, S, in_t><<<blocks_for(threads, B), B, 0, h->stream>>>(
             (S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, mode, face, P);

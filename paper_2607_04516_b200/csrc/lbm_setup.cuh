@@ -148,7 +148,12 @@ __device__ __forceinline__ void publish_fixed(real *__restrict__ fu, const Param
 }
 
 // ---- a3: inlet write -------------------------------------------------------------------------------------------------
-// mode 0: profile prof[nz] per component by level; mode 1: plane uvw[3][n2][n1] of one face
+template <typename real>
+__device__ __forceinline__ bool fixed_slot_cell(const Params<real> &P, const uint8_t *__restrict__ flags, int sl, int &k, int &x, int &y,
+                                                int &z);
+
+// mode 0: profile prof[nz] per component by level, one thread per face-velocity slot (= per face-plane cell of every EQ
+// face; a cell is handled by the slot of its owner face); mode 1: plane uvw[3][n2][n1] of one face, one thread per plane cell
 template <typename real, typename S, typename in_t>
 __global__ void inlet_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                              const in_t *__restrict__ pu, const in_t *__restrict__ pv, const in_t *__restrict__ pw,
@@ -158,8 +163,8 @@ __global__ void inlet_kernel(S *__restrict__ A, S *__restrict__ B, real *__restr
     int x, y, z;
     long long src;
     if (mode == 0) {
-        if (t >= P.N) return;
-        cell_xyz(P, t, x, y, z);
+        int k;
+        if (t >= P.F || !fixed_slot_cell(P, flags, t, k, x, y, z)) return;
         src = z;
     } else {
         const int axis = face >> 1;
