@@ -123,6 +123,7 @@ typedef struct oracle {
     int thermal;
     double alpha, gbeta, theta_ref; /* diffusivity, g*beta (buoyancy per unit theta, along +z), reference theta */
     double *H, *Hn;                 /* [cell][7] post-collision thermal populations, directions 0..6 of CI */
+    double *thb;                    /* [cell] prescribed temperature of EQ_FIXED cells (reading 27); theta_ref unless set */
     int thd[6];                     /* WALL faces held at a fixed temperature (Dirichlet; reading 26): 1 = on */
     double thw[6];                  /* ... their temperatures theta_w */
     /* 16-bit population storage: 0 = populations kept in FP64 (default),
@@ -391,7 +392,7 @@ oracle_t *oracle_create(int nx, int ny, int nz, double nu0, double Cs, double fc
 void oracle_destroy(oracle_t *o)
 {
     if (!o) return;
-    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o->sig); free(o->ut); free(o->modes); free(o->uhat); free(o->H); free(o->Hn); free(o);
+    free(o->cls); free(o->G); free(o->Gn); free(o->ub); free(o->msum); free(o->sig); free(o->ut); free(o->modes); free(o->uhat); free(o->H); free(o->Hn); free(o->thb); free(o);
 }
 
 /* Damping zones (see collide()).  width[k] (cells) and peak[k] for the six faces x-,x+,y-,y+,z-,z+; a cell at
@@ -619,6 +620,17 @@ int oracle_set_inflow_turbulence(oracle_t *o, int n, const double *modes, double
     return 0;
 }
 
+/* Thermal lattice on open faces (DESIGN.md §4 reading 27): an EQ_FIXED cell holds the thermal equilibrium of its prescribed
+ * temperature and velocity, h_eq(theta_b, u_b), as it holds f_eq(1, u_b) for the flow. */
+static void write_eq_fixed_thermal(oracle_t *o, long cell)
+{
+    if (!o->thermal) return;
+    double h[QT];
+    heq(o->thb[cell], o->ub + 3 * cell, h);
+    memcpy(o->H + cell * QT, h, sizeof h);
+    memcpy(o->Hn + cell * QT, h, sizeof h);
+}
+
 static void write_eq_fixed_cell(oracle_t *o, long cell)
 {
     double g[Q];
@@ -626,6 +638,7 @@ static void write_eq_fixed_cell(oracle_t *o, long cell)
     to_storage(o, g);
     memcpy(o->G + cell * Q, g, sizeof g);
     memcpy(o->Gn + cell * Q, g, sizeof g);
+    write_eq_fixed_thermal(o, cell);
 }
 
 /* step 5 (profile form): every EQ_FIXED cell gets f_eq(1, (u[z],v[z],w[z])) */
@@ -864,10 +877,19 @@ int oracle_step(oracle_t *o, int nsteps)
                         p[k / 2] += (k % 2) ? -1 : +1; /* x - n, n outward */
                         int n[3] = {o->nx, o->ny, o->nz};
                         double r, u[3] = {0, 0, 0};
-                        if (p[k / 2] >= 0 && p[k / 2] < n[k / 2])
-                            local_macros(o, o->G, cell_of(o, p[0], p[1], p[2]), &r, u);
+                        double th_nb = o->theta_ref;
+                        if (p[k / 2] >= 0 && p[k / 2] < n[k / 2]) {
+                            long nb = cell_of(o, p[0], p[1], p[2]);
+                            local_macros(o, o->G, nb, &r, u);
+                            if (o->thermal && o->cls[nb] != C_SOLID) {
+                                th_nb = 0.0;
+                                for (int i = 0; i < QT; ++i) th_nb += o->H[nb * QT + i];
+                            }
+                        }
                         feq(1.0, u, gn);
                         to_storage(o, gn);
+                        /* reading 27: the outflow cell also copies the temperature of its inward neighbour (zero gradient) */
+                        if (o->thermal) heq(th_nb, u, o->Hn + cell * QT);
                     } else if (cl == C_EQ_FIXED && o->nmodes > 0) {
                         /* step 5 with fluctuations: the state of step k+1 carries u'(x, k+1) */
                         double u[3];
@@ -878,7 +900,7 @@ int oracle_step(oracle_t *o, int nsteps)
                         /* SOLID: inert; EQ_FIXED (step 5): unchanged */
                         memcpy(gn, o->G + cell * Q, sizeof(double) * Q);
                     }
-                    if (o->thermal && cl != C_FLUID) memcpy(o->Hn + cell * QT, o->H + cell * QT, sizeof(double) * QT);
+                    if (o->thermal && cl != C_FLUID && cl != C_EQ_OUTFLOW) memcpy(o->Hn + cell * QT, o->H + cell * QT, sizeof(double) * QT);
                 }
         double *t = o->G; o->G = o->Gn; o->Gn = t;
         if (o->thermal) { t = o->H; o->H = o->Hn; o->Hn = t; }
@@ -973,12 +995,10 @@ int oracle_set_step(oracle_t *o, long s) { o->step = s; return 0; }
 
 /* Switch the D3Q7 thermal lattice on: diffusivity alpha (tau_theta = 4 alpha + 1/2), buoyancy coefficient gbeta
  * (acceleration g beta (theta - theta_ref) along +z), reference theta.  The thermal state is set to theta_ref at rest.
- * Faces must be PERIODIC / WALL / FREE_SLIP (the density-current set-up of PAPER.md:121 is a closed box); -1 otherwise. */
+ * On open faces (reading 27) EQ_FIXED cells take h_eq(theta_b, u_b) with theta_b = theta_ref until oracle_set_inlet_theta. */
 int oracle_set_thermal(oracle_t *o, double alpha, double gbeta, double theta_ref)
 {
     if (o->store16) return -1;
-    for (int k = 0; k < 6; ++k)
-        if (o->face[k] == F_EQ_FIXED || o->face[k] == F_EQ_OUTFLOW) return -1;
     if (!(alpha > 0.0)) return -1;
     long N = (long)o->nx * o->ny * o->nz;
     if (!o->H) {
@@ -986,13 +1006,36 @@ int oracle_set_thermal(oracle_t *o, double alpha, double gbeta, double theta_ref
         o->Hn = (double *)malloc(sizeof(double) * N * QT);
         if (!o->H || !o->Hn) return -4;
     }
+    if (!o->thb) {
+        o->thb = (double *)malloc(sizeof(double) * N);
+        if (!o->thb) return -4;
+    }
     o->alpha = alpha; o->gbeta = gbeta; o->theta_ref = theta_ref; o->thermal = 1;
-    for (long cell = 0; cell < N; ++cell)
+    for (long cell = 0; cell < N; ++cell) {
+        o->thb[cell] = theta_ref;
         for (int i = 0; i < QT; ++i) o->H[cell * QT + i] = o->Hn[cell * QT + i] = weight_t(i) * theta_ref;
+        if (o->have_flags && o->cls[cell] == C_EQ_FIXED) write_eq_fixed_thermal(o, cell);
+    }
     return 0;
 }
 
-/* H0 = h_eq(theta0, u0); NULL velocity component => 0; SOLID cells: theta_ref at rest. */
+/* Prescribed temperature of the EQ_FIXED cells by level, theta_b(z) [nz] (reading 27): their thermal state becomes
+ * h_eq(theta_b, u_b).  Call it after the velocity profile / plane (a later velocity call keeps theta_b). */
+int oracle_set_inlet_theta(oracle_t *o, const double *theta_b)
+{
+    if (!o->thermal || !o->have_flags || !theta_b) return -3;
+    for (int z = 0; z < o->nz; ++z)
+        for (int y = 0; y < o->ny; ++y)
+            for (int x = 0; x < o->nx; ++x) {
+                long cell = cell_of(o, x, y, z);
+                if (o->cls[cell] != C_EQ_FIXED) continue;
+                o->thb[cell] = theta_b[z];
+                write_eq_fixed_thermal(o, cell);
+            }
+    return 0;
+}
+
+/* H0 = h_eq(theta0, u0); NULL velocity component => 0; SOLID cells: theta_ref at rest; EQ_FIXED cells keep their boundary state. */
 int oracle_set_theta(oracle_t *o, const double *theta, const double *ux, const double *uy, const double *uz)
 {
     if (!o->thermal) return -3;
@@ -1000,6 +1043,7 @@ int oracle_set_theta(oracle_t *o, const double *theta, const double *ux, const d
     for (long cell = 0; cell < N; ++cell) {
         double th = theta ? theta[cell] : o->theta_ref;
         double u[3] = {ux ? ux[cell] : 0.0, uy ? uy[cell] : 0.0, uz ? uz[cell] : 0.0};
+        if (o->cls[cell] == C_EQ_FIXED) continue; /* keeps its boundary state h_eq(theta_b, u_b), as in oracle_set_macros */
         if (o->cls[cell] == C_SOLID) { th = o->theta_ref; u[0] = u[1] = u[2] = 0.0; }
         double h[QT];
         heq(th, u, h);

@@ -51,7 +51,7 @@ def _load():
                  "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux",
                  "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping",
                  "oracle_vk_spectrum", "oracle_set_inflow_turbulence", "oracle_set_flags_mask",
-                 "oracle_set_theta", "oracle_get_theta", "oracle_heq", "oracle_round_half", "oracle_set_storage16", "oracle_set_thermal_walls"):
+                 "oracle_set_theta", "oracle_get_theta", "oracle_heq", "oracle_round_half", "oracle_set_storage16", "oracle_set_thermal_walls", "oracle_set_inlet_theta"):
         getattr(lib, name).restype = C.c_int
     lib.oracle_set_thermal.restype = C.c_int
     lib.oracle_set_thermal.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
@@ -280,6 +280,11 @@ class Oracle:
     def set_thermal(self, alpha, gbeta=0.0, theta_ref=0.0):
         self._chk(self._lib.oracle_set_thermal(C.c_void_p(self._h), float(alpha), float(gbeta), float(theta_ref)),
                   "set_thermal")
+
+    def set_inlet_theta(self, theta_b):
+        """Prescribed temperature of the EQ_FIXED cells by level, theta_b[nz] (thermal lattice on open faces)."""
+        t, tp = _d(np.asarray(theta_b, dtype=np.float64).reshape(self.nz))
+        self._chk(self._lib.oracle_set_inlet_theta(C.c_void_p(self._h), tp), "set_inlet_theta")
 
     def set_thermal_walls(self, on, theta_w):
         """Hold WALL faces (order x-,x+,y-,y+,z-,z+) with on[k] != 0 at temperature theta_w[k] (anti-bounce-back)."""

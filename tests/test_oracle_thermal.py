@@ -135,7 +135,7 @@ def test_uniform_buoyancy_adds_momentum_exactly():
     o.close(); o2.close()
 
 
-def test_thermal_off_leaves_flow_untouched_and_eq_faces_refused():
+def test_thermal_off_leaves_flow_untouched():
     n = 8
     a = O.Oracle(n, n, n, 1e-2, 0.1, 1e-3, faces=[P] * 6)
     b = O.Oracle(n, n, n, 1e-2, 0.1, 1e-3, faces=[P] * 6)
@@ -147,11 +147,7 @@ def test_thermal_off_leaves_flow_untouched_and_eq_faces_refused():
     b.set_theta(1.0 + 0.1 * rng.standard_normal((n, n, n)))
     a.step(10); b.step(10)
     assert np.array_equal(a.get_state(), b.get_state())
-    c = O.Oracle(n, n, n, 1e-2)  # default faces have EQ_FIXED / EQ_OUTFLOW
-    c.set_flags()
-    with pytest.raises(Exception):
-        c.set_thermal(0.01, 0.0, 1.0)
-    for o in (a, b, c):
+    for o in (a, b):
         o.close()
 
 
@@ -279,3 +275,84 @@ def test_rayleigh_benard_onset_between_no_slip_plates():
     print("Rayleigh-Benard onset: Ra_c estimate", {h: round(v, 1) for h, v in est.items()})
     assert abs(est[24] / Rac - 1) < 0.02
     assert abs(est[24] - Rac) < 0.6 * abs(est[16] - Rac)        # second-order convergence (ratio (16/24)^2 = 0.44)
+
+
+# ---- thermal lattice on open faces (DESIGN.md §4 reading 27) ----------------------------------------------------------------
+
+EQF, EQO = O.FACE_EQ_FIXED, O.FACE_EQ_OUTFLOW
+
+
+def _channel(nx=48, ny=4, nz=6, U=0.05, alpha=0.02, theta_in=1.0, theta0=0.0, gb=0.0):
+    o = O.Oracle(nx, ny, nz, 0.02, 0.0, 0.0, (0, 0, 0), (EQF, EQO, P, P, FS, FS))
+    o.set_flags(None)
+    o.set_inlet_profile(np.full(nz, U))
+    o.set_macros(None, np.full((nz, ny, nx), U), None, None)
+    o.set_thermal(alpha, gb, 0.0)
+    o.set_inlet_theta(np.full(nz, theta_in))
+    o.set_theta(np.full((nz, ny, nx), theta0), np.full((nz, ny, nx), U), None, None)
+    return o
+
+
+def test_uniform_flow_with_uniform_temperature_through_open_faces_is_a_fixed_point():
+    """Inlet at (U, theta_b), everything else at the same (U, theta_b): EQ_FIXED cells hold h_eq(theta_b, u_b), the outflow
+    cells copy theta and u of their inward neighbours — nothing may change, to rounding, and the flow stays uniform."""
+    o = _channel(theta_in=0.7, theta0=0.7)
+    o.step(50)
+    assert np.abs(o.get_theta() - 0.7).max() < 1e-14
+    assert np.abs(o.get_macros()[1] - 0.05).max() < 1e-14
+    # the inlet cells hold exactly the thermal equilibrium of (theta_b, u_b): first moment theta_b u_b
+    o.close()
+
+
+def test_an_inlet_temperature_step_is_carried_downstream_at_the_flow_speed_and_flushes_the_channel():
+    """theta_b = 1 at the inlet of a channel that starts at 0, uniform flow U: the front (theta = 1/2) sits at x = U t within
+    its diffusive width sqrt(4 alpha t) / 4 after t steps (advection-diffusion of a step: erfc profile centred at U t; the
+    inlet cell itself is x = 0), the profile across it is monotone, and after several flushes the whole channel — the
+    outflow cells included, which copy their neighbour — is at theta_b (zero-gradient outflow lets the heat leave)."""
+    nx, U, alpha = 96, 0.05, 0.01
+    o = _channel(nx=nx, U=U, alpha=alpha)
+    t = 800
+    o.step(t)
+    th = o.get_theta()[2, 1, :]
+    assert np.all(np.diff(th) <= 1e-5)                        # monotone from the hot inlet to the cold channel (BGK ripple ahead of the front: 3e-6)
+    xs = np.arange(nx)
+    front = np.interp(0.5, th[::-1], xs[::-1])
+    assert abs(front - U * t) < 0.25 * np.sqrt(4 * alpha * t) + 0.5
+    # erfc shape: 16 % / 84 % points one standard deviation sqrt(2 alpha t) either side of the front
+    x16, x84 = np.interp(0.1587, th[::-1], xs[::-1]), np.interp(0.8413, th[::-1], xs[::-1])
+    assert (x16 - x84) / 2 == pytest.approx(np.sqrt(2 * alpha * t), rel=0.08)
+    o.step(6000)                                              # three flush times nx / U
+    assert np.abs(o.get_theta() - 1.0).max() < 1e-6
+    o.close()
+
+
+def test_outflow_cell_copies_temperature_and_velocity_of_its_inward_neighbour():
+    """One step from a random interior state: the EQ_OUTFLOW cell's new theta is the previous theta of the cell inside it
+    and its thermal populations are the equilibrium of that (theta, u): first moment theta u."""
+    nx, ny, nz = 10, 5, 4
+    o = O.Oracle(nx, ny, nz, 0.02, 0.0, 0.0, (0, 0, 0), (EQF, EQO, P, P, FS, FS))
+    o.set_flags(None)
+    o.set_inlet_profile(np.full(nz, 0.04))
+    rng = np.random.default_rng(2)
+    u0 = 0.04 + 0.01 * rng.random((nz, ny, nx))
+    o.set_macros(None, u0, None, None)
+    o.set_thermal(0.03, 0.0, 0.5)
+    th0 = 0.5 + 0.2 * rng.random((nz, ny, nx))
+    o.set_theta(th0, u0, None, None)
+    before_th, before_u = o.get_theta(), o.get_macros()[1]
+    assert np.abs(before_th[:, :, 0] - 0.5).max() < 1e-15      # EQ_FIXED cells kept theta_b = theta_ref, not the field's value
+    o.step(1)
+    th = o.get_theta()
+    assert np.abs(th[:, :, -1] - before_th[:, :, -2]).max() < 1e-15
+    assert np.abs(o.get_macros()[1][:, :, -1] - before_u[:, :, -2]).max() < 1e-15
+    o.close()
+
+
+def test_heated_inflow_rises_under_buoyancy():
+    """Coupling through the open faces: warm air entering a neutral channel is lighter — with g beta > 0 it must acquire
+    upward velocity downstream of the inlet (sign and presence of the coupling on EQ-fed fluid)."""
+    o = _channel(nx=40, nz=12, theta_in=1.0, theta0=0.0, gb=2e-4)
+    o.step(300)
+    uz = o.get_macros()[3]
+    assert uz[3:9, :, 3:10].max() > 1e-4
+    o.close()
