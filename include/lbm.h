@@ -180,13 +180,22 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
  * acceleration F + g_beta (theta - theta_ref) e_z (+z = up), and the thermal populations relax towards h_eq(theta, u)
  * with the velocity of that collision.  lbm_get_macros then reports the velocity corrected by the same buoyancy.
  * lbm_set_thermal switches it on with theta = theta_ref at rest; it allocates 2 x 7 population arrays of the handle's
- * precision (library-owned, freed by lbm_destroy).  All six faces must be PERIODIC / WALL / FREE_SLIP, and damping zones
- * and inflow fluctuations must be off (LBM_EINVAL otherwise, also from the calls that would switch those on later).
- * alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
+ * precision (library-owned, freed by lbm_destroy).  Open faces (DESIGN.md §4 reading 27): an EQ_FIXED cell holds
+ * h_eq(theta_b, u_b) beside f_eq(1, u_b), with theta_b = theta_ref until lbm_set_inlet_theta prescribes it; an EQ_OUTFLOW
+ * cell holds the equilibria of the theta and u its inward neighbour had at the previous step (zero gradient).  Damping zones,
+ * inflow fluctuations and 16-bit storage must be off (LBM_EINVAL otherwise, also from the calls that would switch those on
+ * later).  alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
 int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref);
+/* Prescribed temperature of the EQ_FIXED cells by level (reading 27): theta_b[nz], host or device; the cells' thermal state
+ * becomes h_eq(theta_b(z), u_b) at once and is re-expanded from it every step.  A later lbm_set_inlet_profile / _plane,
+ * lbm_feed_inlet or lbm_balance_flux keeps theta_b and refreshes the cells for the new u_b.  Needs lbm_set_thermal and flags
+ * (else LBM_ESTATE); a new lbm_set_flags* resets theta_b to theta_ref. */
+int lbm_set_inlet_theta(lbm_t *h, const float *theta_b);
+int lbm_set_inlet_theta_f64(lbm_t *h, const double *theta_b);
 /* Initial thermal state H0 = h_eq(theta, u): theta, ux, uy, uz each [nz][ny][nx], host or device; NULL theta =
- * theta_ref, NULL component = 0; SOLID cells are skipped.  Needs lbm_set_thermal and flags (else LBM_ESTATE); a new
- * lbm_set_flags* leaves the thermal state stale until this is called again. */
+ * theta_ref, NULL component = 0; SOLID cells are skipped, EQ_FIXED cells keep their boundary state.  Call it AFTER
+ * lbm_set_macros (what the cells next to an outflow face hand to it is derived from both states).  Needs lbm_set_thermal
+ * and flags (else LBM_ESTATE); a new lbm_set_flags* leaves the thermal state stale until this is called again. */
 int lbm_set_theta(lbm_t *h, const float *theta, const float *ux, const float *uy, const float *uz);
 int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const double *uy, const double *uz);
 /* theta = sum_i h_i of the current state, [nz][ny][nx], host or device; SOLID cells report theta_ref.  Synchronises. */

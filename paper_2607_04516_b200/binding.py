@@ -29,7 +29,7 @@ SYMBOLS = [
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
     "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
     "lbm_set_thermal", "lbm_set_theta", "lbm_set_theta_f64", "lbm_get_theta", "lbm_get_theta_f64",
-    "lbm_get_thermal_state", "lbm_set_thermal_state", "lbm_set_thermal_walls",
+    "lbm_get_thermal_state", "lbm_set_thermal_state", "lbm_set_thermal_walls", "lbm_set_inlet_theta", "lbm_set_inlet_theta_f64",
 ]
 
 
@@ -74,7 +74,8 @@ def load_library():
     lib.lbm_set_thermal.argtypes = [vp, C.c_double, C.c_double, C.c_double]
     for n in ("lbm_set_theta", "lbm_set_theta_f64"):
         getattr(lib, n).argtypes = [vp, vp, vp, vp, vp]
-    for n in ("lbm_get_theta", "lbm_get_theta_f64", "lbm_get_thermal_state", "lbm_set_thermal_state"):
+    for n in ("lbm_get_theta", "lbm_get_theta_f64", "lbm_get_thermal_state", "lbm_set_thermal_state", "lbm_set_inlet_theta",
+              "lbm_set_inlet_theta_f64"):
         getattr(lib, n).argtypes = [vp, vp]
     lib.lbm_set_thermal_walls.argtypes = [vp, vp, vp]
     lib.lbm_mean_config.argtypes = [vp, l, i]
@@ -304,6 +305,14 @@ class Lbm:
         a = out if out is not None else self._new(t.float64 if f64 else t.float32)
         self._chk(fn(self._h, a.data_ptr()), "get_theta")
         return a
+
+    def set_inlet_theta(self, theta_b, f64=False):
+        """Prescribed temperature of the EQ_FIXED cells by level, theta_b[nz] (thermal lattice on open faces)."""
+        k, p = _ptr(theta_b, np.float64 if f64 else np.float32)
+        if tuple(k.shape) != (self.nz,):
+            raise ValueError("theta_b must have nz entries")
+        fn = self._lib.lbm_set_inlet_theta_f64 if f64 else self._lib.lbm_set_inlet_theta
+        self._chk(fn(self._h, p), "set_inlet_theta")
 
     def set_thermal_walls(self, on, theta_w):
         """Hold WALL faces (order x-,x+,y-,y+,z-,z+) with on[k] != 0 at temperature theta_w[k]."""

@@ -101,7 +101,7 @@ struct lbm {
     bool thermal;   // D3Q7 thermal lattice + Boussinesq coupling on (lbm_set_thermal); its two buffers are library-owned
     double alpha, gbeta, theta_ref;
     int thd; double thw[6]; // fixed-temperature WALL faces (lbm_set_thermal_walls): mask and temperatures
-    char *th_ws;    // [2][7][stride] reals, cudaMalloc'ed by lbm_set_thermal, freed by lbm_destroy
+    char *th_ws;    // [2][7][stride] reals + ft[2][F], cudaMalloc'ed by lbm_set_thermal, freed by lbm_destroy
     int loop_ok;    // multi-step cooperative launch: 0 = not probed yet, 1 = the whole grid is resident, -1 = no
     // staging buffers for HOST inputs / outputs that do not fit the scratch area (whole-lattice fields): kept between
     // calls, grown on demand, freed by lbm_destroy — a cudaMalloc + cudaFree pair per field per call costs milliseconds
@@ -122,6 +122,9 @@ struct lbm {
     void *scratch() const { return ws + L.off_scratch; }
     size_t pop_bytes() const { return (size_t)Q * (size_t)L.stride * (fp64 ? 8 : (s16 ? 2 : 4)); } // one population buffer
     size_t th_half() const { return (size_t)QT * (size_t)L.stride * (fp64 ? 8 : 4); }
+    // thermal companion of the face-velocity side array: ft[2 halves][F] reals behind the two thermal buffers (F <= fu_bytes / 6 reals)
+    size_t ft_bytes() const { return L.fu_bytes / 3; }
+    char *ft() const { return th_ws + 2 * th_half(); }
     void *th_state() const { return thermal ? th_ws + (cur ? th_half() : 0) : nullptr; }
     void *th_other() const { return thermal ? th_ws + (cur ? 0 : th_half()) : nullptr; }
     long long N() const { return (long long)nx * ny * nz; }
@@ -349,9 +352,16 @@ int do_set_flags(lbm_t *h, const int32_t *height, const uint8_t *dev_mask = null
     CUDA_TRY(h, cudaMemsetAsync(h->bufB(), 0, h->pop_bytes(), h->stream));
     if (h->want_mean) CUDA_TRY(h, cudaMemsetAsync(h->mean(), 0, (size_t)3 * h->L.stride * rs, h->stream));
     CUDA_TRY(h, cudaMemsetAsync(h->fu(), 0, h->L.fu_bytes, h->stream));
+    if (h->thermal) CUDA_TRY(h, cudaMemsetAsync(h->ft(), 0, h->ft_bytes(), h->stream)); // theta_b back to theta_ref; the thermal state is stale until lbm_set_theta
     h->cur = 0; h->step = 0; h->mcount = 0; h->have_flags = true;
     return LBM_OK;
 }
+
+template <typename real, typename in_t>
+int do_inlet_theta(lbm_t *h, const in_t *theta_b);
+// the boundary velocity changed while the thermal lattice is on: the EQ_FIXED cells' thermal state h_eq(theta_b, u_b) follows
+template <typename real>
+int thermal_refresh(lbm_t *h) { return h->thermal ? do_inlet_theta<real, float>(h, nullptr) : LBM_OK; }
 
 template <typename real, typename S, typename in_t>
 int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, const in_t *w, size_t count)
@@ -372,6 +382,7 @@ int do_set_inlet(lbm_t *h, int mode, int face, const in_t *u, const in_t *v, con
             (S *)h->bufA(), (S *)h->bufB(), (real *)h->fu(), h->flags(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
             (const in_t *)in[2].dev, mode, face, P);
         rc = check_launch(h, "inlet_kernel");
+        if (!rc) rc = thermal_refresh<real>(h);
     }
     release_in(h, in, 3);
     return rc;
@@ -556,8 +567,12 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         // spills), 24 450 at 10 CTAs (48 registers, 108 B of spills) and round 1's 24 600 at 7 CTAs (72 registers)
         constexpr int BLOCK = 128, MINB = std::is_same<real, float>::value ? THERMAL_MINB : 2;
         const ThermalPtrs<real> T = make_thermal_ptrs<real>(A, B, (const real *)h->th_state(), (real *)h->th_other(), P);
-        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T);
-        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T);
+        // the side arrays' halves follow the population buffers (as in launch_step_as)
+        real *fu = (real *)h->fu(), *ft = (real *)h->ft();
+        const OpenFaces<real> O{fu + (size_t)(h->cur ? 3 : 0) * P.F, fu + (size_t)(h->cur ? 0 : 3) * P.F, ft + (size_t)(h->cur ? 1 : 0) * P.F,
+                                ft + (size_t)(h->cur ? 0 : 1) * P.F};
+        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T, O);
+        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T, O);
         return check_launch(h, "thermal_step_kernel");
     }
     const bool turb = h->nmodes > 0 && P.F > 0;
@@ -778,6 +793,7 @@ int do_balance_flux(lbm_t *h, double *before, double *after)
         rc = check_launch(h, "flux_sum_kernel");
         if (rc) return rc;
     }
+    { int rc = thermal_refresh<real>(h); if (rc) return rc; }
     CUDA_TRY(h, cudaMemcpyAsync(host, acc, sizeof host, cudaMemcpyDeviceToHost, h->stream));
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     if (before) *before = host[0];
@@ -811,7 +827,8 @@ int do_feed(lbm_t *dst, const lbm_t *src, int sx)
     }
     feed_kernel<real, S><<<blocks_for((long long)D.ny * D.nz, B), B, 0, dst->stream>>>(
         (S *)dst->bufA(), (S *)dst->bufB(), (real *)dst->fu(), dst->flags(), D, (const S *)src->state(), src->flags(), Ps, sx);
-    return check_launch(dst, "feed_kernel");
+    int rc = check_launch(dst, "feed_kernel");
+    return rc ? rc : thermal_refresh<real>(dst);
 }
 
 } // namespace
@@ -832,7 +849,7 @@ int do_set_theta(lbm_t *h, const in_t *theta, const in_t *ux, const in_t *uy, co
         real *H0 = (real *)h->th_ws, *H1 = (real *)(h->th_ws + h->th_half());
         thermal_init_kernel<real, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
             H0, H1, h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev, (const in_t *)in[2].dev,
-            (const in_t *)in[3].dev, P);
+            (const in_t *)in[3].dev, P, (const real *)h->state(), (real *)h->fu(), (real *)h->ft());
         rc = check_launch(h, "thermal_init_kernel");
     }
     release_in(h, in, 4);
@@ -893,10 +910,41 @@ int do_thermal_state(lbm_t *h, double *out, const double *in)
     int rc = stage_in(h, in, bytes, h->L.scratch_bytes, &ib);
     if (rc) return rc;
     real *H0 = (real *)h->th_ws, *H1 = (real *)(h->th_ws + h->th_half());
-    thermal_state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(H0, H1, h->flags(), h->links(), (const double *)ib.dev, P);
+    thermal_state_in_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(H0, H1, h->flags(), h->links(), (const double *)ib.dev, P,
+                                                                           (const real *)h->state(), (real *)h->fu(), (real *)h->ft());
     rc = check_launch(h, "thermal_state_in_kernel");
     release_in(h, &ib, 1);
     return rc;
+}
+
+namespace {
+// theta_b[nz] -> the EQ_FIXED slots and cells (thermal_inlet_kernel); theta_b == nullptr refreshes the cells from the slots
+template <typename real, typename in_t>
+int do_inlet_theta(lbm_t *h, const in_t *theta_b)
+{
+    const Params<real> P = make_params<real>(h);
+    if (P.F == 0) return LBM_OK;
+    InBuf in;
+    int rc = stage_in(h, theta_b, (size_t)h->nz * sizeof(in_t), 0, &in);
+    if (rc) return rc;
+    const int B = 128;
+    real *H0 = (real *)h->th_ws, *H1 = (real *)(h->th_ws + h->th_half());
+    thermal_inlet_kernel<real, in_t><<<blocks_for(P.F, B), B, 0, h->stream>>>(H0, H1, h->flags(), (const in_t *)in.dev, (const real *)h->fu(),
+                                                                              (real *)h->ft(), P);
+    rc = check_launch(h, "thermal_inlet_kernel");
+    release_in(h, &in, 1);
+    return rc;
+}
+} // namespace
+template <typename in_t>
+int set_inlet_theta_any(lbm_t *h, const in_t *theta_b)
+{
+    if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!theta_b) return fail(h, LBM_EINVAL, "set_inlet_theta: NULL");
+    if (!h->thermal) return fail(h, LBM_ESTATE, "set_inlet_theta: thermal lattice is off (lbm_set_thermal)");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inlet_theta: flags not set");
+    return h->fp64 ? do_inlet_theta<double, in_t>(h, theta_b) : do_inlet_theta<float, in_t>(h, theta_b);
 }
 
 bool has_eq_face(const int face[6])
@@ -915,14 +963,18 @@ int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
     if (!(alpha > 0.0) || !std::isfinite(alpha) || !std::isfinite(g_beta) || !std::isfinite(theta_ref))
         return fail(h, LBM_EINVAL, "set_thermal: alpha must be > 0 and all arguments finite");
     if (h->s16) return fail(h, LBM_EINVAL, "set_thermal: not combinable with 16-bit population storage");
-    if (has_eq_face(h->face)) return fail(h, LBM_EINVAL, "set_thermal: EQ_FIXED / EQ_OUTFLOW faces are not supported with the thermal lattice");
     if (h->damp_on || h->nmodes > 0) return fail(h, LBM_EINVAL, "set_thermal: not combinable with damping zones / inflow fluctuations");
-    if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half()));
-    CUDA_TRY(h, cudaMemsetAsync(h->th_ws, 0, 2 * h->th_half(), h->stream)); // theta_ref at rest (shifted storage)
+    if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half() + h->ft_bytes()));
+    CUDA_TRY(h, cudaMemsetAsync(h->th_ws, 0, 2 * h->th_half() + h->ft_bytes(), h->stream)); // theta_ref at rest (shifted storage), theta_b = theta_ref
     h->alpha = alpha; h->gbeta = g_beta; h->theta_ref = theta_ref; h->thermal = true;
+    int rc = LBM_OK;
+    // open faces (reading 27): the EQ_FIXED cells hold h_eq(theta_ref, u_b) until lbm_set_inlet_theta says otherwise
+    if (h->have_flags && has_eq_face(h->face)) rc = h->fp64 ? do_inlet_theta<double, float>(h, nullptr) : do_inlet_theta<float, float>(h, nullptr);
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
-    return LBM_OK;
+    return rc;
 }
+int lbm_set_inlet_theta(lbm_t *h, const float *theta_b) { return set_inlet_theta_any<float>(h, theta_b); }
+int lbm_set_inlet_theta_f64(lbm_t *h, const double *theta_b) { return set_inlet_theta_any<double>(h, theta_b); }
 int lbm_set_theta(lbm_t *h, const float *theta, const float *ux, const float *uy, const float *uz) { return set_theta_any<float>(h, theta, ux, uy, uz); }
 int lbm_set_theta_f64(lbm_t *h, const double *theta, const double *ux, const double *uy, const double *uz) { return set_theta_any<double>(h, theta, ux, uy, uz); }
 int lbm_set_thermal_walls(lbm_t *h, const int on[6], const double theta_w[6])
@@ -1040,7 +1092,6 @@ int lbm_set_boundaries(lbm_t *h, const int face_type[6])
         if (lo < 0 || lo > 4 || hi < 0 || hi > 4) return fail(h, LBM_EINVAL, "set_boundaries: unknown face type");
         if ((lo == LBM_PERIODIC) != (hi == LBM_PERIODIC)) return fail(h, LBM_EINVAL, "set_boundaries: PERIODIC must be set on both faces of an axis");
     }
-    if (h->thermal && has_eq_face(face_type)) return fail(h, LBM_EINVAL, "set_boundaries: EQ faces are not supported while the thermal lattice is on");
     for (int k = 0; k < 6; ++k) h->face[k] = face_type[k];
     for (int k = 0; k < 6; ++k)
         if (face_type[k] != LBM_WALL) h->thd &= ~(1 << k); // a face that stops being a WALL is no longer held at a temperature

@@ -94,10 +94,18 @@ inline ThermalPtrs<real> make_thermal_ptrs(const real *A, real *B, const real *H
     return t;
 }
 
+// Open faces (DESIGN.md §4 reading 27).  The face-velocity side array of the flow lattice (lbm_core.cuh: fu[2 halves][3][F]) has a
+// thermal companion ft[2 halves][F] holding theta - theta_ref per face slot: an EQ_FIXED cell re-expands f_eq(1, u_b) and
+// h_eq(theta_b, u_b) from its slot every step, an EQ_OUTFLOW cell f_eq(1, u) and h_eq(theta, u) of what its inward neighbour
+// published while writing the previous state (u as in the plain kernel, theta = the neighbour's pulled theta, which its thermal
+// collision conserves).  r = the half written together with the state being read, w = the half this launch writes.
+template <typename real>
+struct OpenFaces { const real *fur; real *fuw; const real *ftr; real *ftw; };
+
 template <typename real, bool MEAN, int BLOCK, int MINB>
 __global__ void __launch_bounds__(BLOCK, MINB)
 thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-                    real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T)
+                    real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O)
 {
     const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x;
     if (c2 >= (unsigned)P.nxy) return;
@@ -162,8 +170,22 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
         }
         return;
     }
-    if (cls != FLUID) return; // no EQ cells while the thermal lattice is on (lbm_set_thermal refuses EQ faces)
-    const Macro<real> m = collide_both();
+    Macro<real> m;
+    if (cls == FLUID) {
+        const real dth = theta_shift(t); // the pulled theta: what a feeding cell publishes (its collision conserves it)
+        m = collide_both();
+        if (fl & FEED_BIT)
+            outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) {
+                O.fuw[comp * P.F + sl] = v;
+                if (comp == 0) O.ftw[sl] = dth;
+            });
+    } else { // EQ_FIXED / EQ_OUTFLOW: both equilibria of the slot's (theta, u), re-stored every step like the plain kernel's EQ cells
+        const int sl = eq_slot(P, cls, x, y, z);
+        const real u0 = O.fur[sl], u1 = O.fur[P.F + sl], u2 = O.fur[2 * P.F + sl], dth = O.ftr[sl];
+        m = Macro<real>{real(1), u0, u1, u2};
+        equilibrium(g, real(0), u0, u1, u2);
+        thermal_equilibrium(t, dth, P.theta_ref, u0, u1, u2);
+    }
     store_cell(B, P, p, x, y, z, fl, lk, g);
     store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
     if constexpr (MEAN) {
@@ -173,11 +195,31 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
     }
 }
 
-// H0 = h_eq(theta0, u0) into both buffers (lbm_set_theta); NULL theta = theta_ref, NULL component = 0
+// Publish what a feeding cell (one layer inside an EQ_OUTFLOW face) hands to the outflow cells for the next step, from the
+// CURRENT states A (flow) and its thermal shift dth: the local velocity with the cell's buoyancy in the force, and theta; both
+// halves of both side arrays (set-up paths).
+template <typename real>
+__device__ __forceinline__ void thermal_feed_both(const real *__restrict__ A, real *__restrict__ fu, real *__restrict__ ft, Params<real> P,
+                                                  int p, int x, int y, int z, int cls, real dth)
+{
+    real g[Q];
+    load_cell(g, A, P.stride, p);
+    P.Fz += P.gbeta * dth;
+    const Macro<real> m = local_macros(g, cls, P);
+    outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) {
+        fu[comp * P.F + sl] = v;
+        fu[(3 + comp) * P.F + sl] = v;
+        if (comp == 0) { ft[sl] = dth; ft[P.F + sl] = dth; }
+    });
+}
+
+// H0 = h_eq(theta0, u0) into both buffers (lbm_set_theta); NULL theta = theta_ref, NULL component = 0.  FLUID and EQ_OUTFLOW
+// cells; EQ_FIXED cells keep their boundary state h_eq(theta_b, u_b) (as lbm_set_macros keeps f_eq(1, u_b)).
 template <typename real, typename in_t>
 __global__ void thermal_init_kernel(real *__restrict__ HA, real *__restrict__ HB, const uint8_t *__restrict__ flags,
                                     const uint32_t *__restrict__ links, const in_t *__restrict__ theta, const in_t *__restrict__ ux,
-                                    const in_t *__restrict__ uy, const in_t *__restrict__ uz, Params<real> P)
+                                    const in_t *__restrict__ uy, const in_t *__restrict__ uz, Params<real> P,
+                                    const real *__restrict__ A, real *__restrict__ fu, real *__restrict__ ft)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -185,7 +227,8 @@ __global__ void thermal_init_kernel(real *__restrict__ HA, real *__restrict__ HB
     cell_xyz(P, c, x, y, z);
     const int p = pidx(P, x, y, z);
     const uint8_t fl = flags[p];
-    if ((fl & CLASS_MASK) != FLUID) return;
+    const int cls = fl & CLASS_MASK;
+    if (cls != FLUID && cls != EQ_OUTFLOW) return;
     // theta - theta_ref formed in the input's precision (FP64 input on an FP32 handle keeps the small perturbation)
     const real dth = theta ? real(theta[c] - in_t(P.theta_ref)) : real(0);
     real t[QT];
@@ -193,10 +236,31 @@ __global__ void thermal_init_kernel(real *__restrict__ HA, real *__restrict__ HB
     const uint32_t lk = links[p];
     store_cell_thermal(HA, P, p, x, y, z, fl, lk, t);
     store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
+    if ((fl & FEED_BIT) && P.F > 0) thermal_feed_both(A, fu, ft, P, p, x, y, z, cls, dth);
+}
+
+// Prescribed temperature of the EQ_FIXED cells (lbm_set_inlet_theta; reading 27): one thread per face slot; theta_b[nz] by level,
+// or NULL = keep the slot's value (refresh after the boundary velocity changed, or after lbm_set_thermal).  Writes the slot
+// (both halves) and the cell's thermal state h_eq(theta_b, u_b) in both buffers, u_b from the flow's side array.
+template <typename real, typename in_t>
+__global__ void thermal_inlet_kernel(real *__restrict__ HA, real *__restrict__ HB, const uint8_t *__restrict__ flags,
+                                     const in_t *__restrict__ theta_b, const real *__restrict__ fu, real *__restrict__ ft, Params<real> P)
+{
+    const int sl = blockIdx.x * blockDim.x + threadIdx.x;
+    int k, x, y, z;
+    if (sl >= P.F || !fixed_slot_cell(P, flags, sl, k, x, y, z)) return;
+    const real dth = theta_b ? real(theta_b[z] - in_t(P.theta_ref)) : ft[sl];
+    ft[sl] = dth; ft[P.F + sl] = dth;
+    real t[QT];
+    thermal_equilibrium(t, dth, P.theta_ref, fu[sl], fu[P.F + sl], fu[2 * P.F + sl]);
+    const int p = pidx(P, x, y, z);
+    store_cell_thermal(HA, P, p, x, y, z, flags[p], 0u, t);
+    store_cell_thermal(HB, P, p, x, y, z, flags[p], 0u, t);
 }
 
 // ---- checkpoint of the thermal lattice (lbm_get_thermal_state / lbm_set_thermal_state) -----------------------------------
-// h [7][nz][ny][nx] double, NOT shifted; non-FLUID cells export the rest state wT_i theta_ref and ignore their input.
+// h [7][nz][ny][nx] double, NOT shifted; SOLID cells export the rest state wT_i theta_ref and ignore their input; EQ_FIXED
+// cells export their boundary state and keep it on input (it belongs to the prescribed theta_b, u_b).
 __host__ __device__ inline double weight_t_f64(int i) { return i == 0 ? 0.25 : 0.125; }
 
 template <typename real>
@@ -207,7 +271,7 @@ __global__ void thermal_state_out_kernel(const real *__restrict__ H, const uint8
     int x, y, z;
     cell_xyz(P, c, x, y, z);
     const int p = pidx(P, x, y, z);
-    const bool live = (flags[p] & CLASS_MASK) == FLUID;
+    const bool live = (flags[p] & CLASS_MASK) != SOLID;
 #pragma unroll
     for (int i = 0; i < QT; ++i)
         h[(long long)i * P.N + c] = (live ? double(H[(long long)i * P.stride + p]) : 0.0) + weight_t_f64(i) * double(P.theta_ref);
@@ -215,7 +279,8 @@ __global__ void thermal_state_out_kernel(const real *__restrict__ H, const uint8
 
 template <typename real>
 __global__ void thermal_state_in_kernel(real *__restrict__ HA, real *__restrict__ HB, const uint8_t *__restrict__ flags,
-                                        const uint32_t *__restrict__ links, const double *__restrict__ h, Params<real> P)
+                                        const uint32_t *__restrict__ links, const double *__restrict__ h, Params<real> P,
+                                        const real *__restrict__ A, real *__restrict__ fu, real *__restrict__ ft)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -223,13 +288,15 @@ __global__ void thermal_state_in_kernel(real *__restrict__ HA, real *__restrict_
     cell_xyz(P, c, x, y, z);
     const int p = pidx(P, x, y, z);
     const uint8_t fl = flags[p];
-    if ((fl & CLASS_MASK) != FLUID) return;
+    const int cls = fl & CLASS_MASK;
+    if (cls != FLUID && cls != EQ_OUTFLOW) return;
     real t[QT];
 #pragma unroll
     for (int i = 0; i < QT; ++i) t[i] = real(h[(long long)i * P.N + c] - weight_t_f64(i) * double(P.theta_ref));
     const uint32_t lk = links[p];
     store_cell_thermal(HA, P, p, x, y, z, fl, lk, t);
     store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
+    if ((fl & FEED_BIT) && P.F > 0) thermal_feed_both(A, fu, ft, P, p, x, y, z, cls, theta_shift(t));
 }
 
 // theta of the stored state (lbm_get_theta); SOLID cells report theta_ref
@@ -244,7 +311,7 @@ __global__ void theta_out_kernel(const real *__restrict__ H, const uint8_t *__re
     real t[QT];
 #pragma unroll
     for (int i = 0; i < QT; ++i) t[i] = H[(long long)i * P.stride + p];
-    const bool live = (flags[p] & CLASS_MASK) == FLUID;
+    const bool live = (flags[p] & CLASS_MASK) != SOLID;
     theta[c] = out_t(P.theta_ref) + (live ? out_t(theta_shift(t)) : out_t(0));
 }
 

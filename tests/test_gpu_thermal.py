@@ -132,15 +132,13 @@ def test_thermal_error_behaviour(B):
     with pytest.raises(B.LbmError):
         sim.get_theta()
     with pytest.raises(B.LbmError):
-        sim.set_thermal(0.01, 0.0, 1.0)
+        sim.set_inlet_theta(np.ones(8, np.float32))     # thermal lattice off
     sim.set_boundaries([P] * 6)
     with pytest.raises(B.LbmError):
         sim.set_thermal(0.0, 0.0, 1.0)  # alpha must be > 0
     sim.set_thermal(0.01, 1e-3, 1.0)
     with pytest.raises(B.LbmError):
         sim.set_theta()  # flags were invalidated by set_boundaries
-    with pytest.raises(B.LbmError):
-        sim.set_boundaries([3, 4, 0, 0, 1, 2])
     with pytest.raises(B.LbmError):
         sim.set_damping([0, 0, 0, 0, 0, 4], [0, 0, 0, 0, 0, 0.1])
     sim.set_flags(np.zeros((8, 8), np.int32))
@@ -364,3 +362,82 @@ def test_thermal_walls_argument_errors(B):
         sim.set_thermal_walls([0, 0, 0, 0, 1, 0], [0, 0, 0, 0, float("nan"), 0])
     sim.set_thermal_walls([0, 0, 0, 0, 1, 1], [9, 9, 9, 9, 1.0, 0.0])   # entries of faces not held are ignored
     sim.close()
+
+
+# ---- thermal lattice on open faces (DESIGN.md §4 reading 27) ---------------------------------------------------------------
+
+EQF, EQO = 3, 4
+
+
+def open_pair(B, nx, ny, nz, faces, hm, fp64, gb=3e-4, alpha=0.02, tref=1.0, seed=0, want_mean=False):
+    from oracle import Oracle
+    rng = np.random.default_rng(seed)
+    prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+    thb = tref + 0.4 * np.exp(-np.arange(nz) / 4.0)            # warm air near the ground at the inlet
+    u0 = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+    th0 = tref + 0.05 * rng.standard_normal((nz, ny, nx))
+    args = (nx, ny, nz, 3e-3, 0.1, 1e-3, (1e-6, 0, 0), faces)
+    o = Oracle(*args)
+    sim = B.Lbm(*args, fp64=fp64, want_mean=want_mean)
+    for obj, kw in ((o, {}), (sim, {"f64": True})):
+        obj.set_flags(hm)
+        obj.set_inlet_profile(prof, 0.1 * prof, None, **kw)
+        obj.set_macros(None, u0, None, None, **kw)
+        obj.set_thermal(alpha, gb, tref)
+        obj.set_inlet_theta(thb, **kw)
+        obj.set_theta(th0, u0, None, None, **kw)
+    return sim, o, prof, thb
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+@pytest.mark.parametrize("faces", [(EQF, EQO, P, P, W, FS), (EQF, EQO, FS, FS, W, FS), (EQF, EQO, EQF, EQF, W, FS), (EQO, EQF, W, FS, P, P)])
+def test_open_faces_parity(B, faces, fp64):
+    """Inlet with a prescribed theta_b(z) and u_b(z), outflow copying theta and u, buildings, buoyancy, LES, Coriolis, a body
+    force: rho, u, theta against the oracle after 100 steps; the state right after set-up too (boundary cells included)."""
+    nx, ny, nz = 52, 14, 12
+    hm = np.zeros((ny, nx), np.int32); hm[3:8, 14:20] = 5; hm[8:12, 30:36] = 3
+    sim, o, prof, thb = open_pair(B, nx, ny, nz, faces, hm, fp64, seed=FACES.index(FACES[0]) + len(faces))
+    tol = TOL64 if fp64 else TOL32
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= tol and e_th <= tol, ("set-up", faces, e_flow, e_th)
+    sim.step(100); o.step(100)
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= tol and e_th <= tol, (faces, e_flow, e_th)
+    th = o.get_theta()
+    assert np.abs(th - 1.0).max() > 0.05                         # the warm inflow is really there
+    sim.close(); o.close()
+
+
+def test_open_faces_boundary_updates_mean_and_checkpoint(B):
+    """A new velocity profile keeps theta_b and refreshes the inlet cells; the fused time mean runs on EQ cells too; state +
+    thermal state + step restart a run with open faces exactly (FP32)."""
+    nx, ny, nz = 40, 8, 10
+    hm = np.zeros((ny, nx), np.int32); hm[2:5, 12:17] = 4
+    faces = (EQF, EQO, P, P, W, FS)
+    sim, o, prof, thb = open_pair(B, nx, ny, nz, faces, hm, False, seed=5, want_mean=True)
+    sim.step(20); o.step(20)
+    for obj, kw in ((o, {}), (sim, {"f64": True})):
+        obj.set_inlet_profile(1.2 * prof, None, None, **kw)
+        obj.mean_config(25, 5)
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= TOL32 and e_th <= TOL32
+    sim.step(40); o.step(40)
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= TOL32 and e_th <= TOL32, (e_flow, e_th)
+    gm = sim.get_mean(f64=True); om = o.get_mean()
+    assert gm[3] == om[3] == 8
+    assert max(float(np.abs(a.cpu().numpy() - b).max()) for a, b in zip(gm[:3], om[:3])) <= TOL32
+    # checkpoint
+    f, hpop, k = sim.get_state(out="host"), sim.get_thermal_state(), sim.get_step()
+    b = B.Lbm(nx, ny, nz, 3e-3, 0.1, 1e-3, (1e-6, 0, 0), faces)
+    b.set_flags(hm)
+    b.set_inlet_profile(1.2 * prof, None, None, f64=True)
+    b.set_macros()
+    b.set_thermal(0.02, 3e-4, 1.0)
+    b.set_inlet_theta(thb, f64=True)
+    b.set_state(f); b.set_inlet_profile(1.2 * prof, None, None, f64=True); b.set_thermal_state(hpop); b.set_step(k)
+    sim.step(15); b.step(15)
+    ga = [a.cpu().numpy() for a in sim.get_macros()] + [sim.get_theta(out="host")]
+    gb_ = [a.cpu().numpy() for a in b.get_macros()] + [b.get_theta(out="host")]
+    assert max(float(np.abs(x - y).max()) for x, y in zip(ga, gb_)) <= 2e-6
+    sim.close(); o.close(); b.close()
