@@ -503,8 +503,19 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
     real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
     // sampling steps hold three more values per thread (the prefetched sums): one CTA per SM less, 56 registers, no spills
     constexpr int MINB_S = (SPEC && MINB == 10) ? 9 : MINB;
-    if (sample) step_kernel<real, S, true, SPEC, BLOCK, MINB_S, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
-    else step_kernel<real, S, false, SPEC, BLOCK, MINB, DAMP, TURB><<<grid, BLOCK, 0, h->stream>>>(A, B, h->flags(), h->links(), ms, fur, fuw, P, T, tb, turb_planes);
+    // Programmatic dependent launch (lbm_step.cuh): back-to-back steps overlap the next launch's set-up and index arithmetic with
+    // the drain of the running one; the kernel touches no memory before griddepcontrol.wait.  Measured: config 2 (65 us per
+    // step) +2.6 %, config 3 +0.5 %, config 1 with one launch per step +7 %.
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = grid; cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    const uint8_t *fl = h->flags();
+    const uint32_t *lk = h->links();
+    if (sample) cudaLaunchKernelEx(&cfg, step_kernel<real, S, true, SPEC, BLOCK, MINB_S, DAMP, TURB>, A, B, fl, lk, ms, fur, fuw, P, T, tb, turb_planes);
+    else cudaLaunchKernelEx(&cfg, step_kernel<real, S, false, SPEC, BLOCK, MINB, DAMP, TURB>, A, B, fl, lk, ms, fur, fuw, P, T, tb, turb_planes);
     return check_launch(h, "step_kernel");
 }
 
@@ -571,8 +582,17 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         real *fu = (real *)h->fu(), *ft = (real *)h->ft();
         const OpenFaces<real> O{fu + (size_t)(h->cur ? 3 : 0) * P.F, fu + (size_t)(h->cur ? 0 : 3) * P.F, ft + (size_t)(h->cur ? 1 : 0) * P.F,
                                 ft + (size_t)(h->cur ? 0 : 1) * P.F};
-        if (sample) thermal_step_kernel<real, true, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T, O);
-        else thermal_step_kernel<real, false, BLOCK, MINB><<<grid, BLOCK, 0, h->stream>>>(B, (real *)h->th_other(), h->flags(), h->links(), (real *)h->mean(), P, T, O);
+        cudaLaunchConfig_t cfg{}; // programmatic dependent launch, as for the plain step (launch_step_as)
+        cfg.gridDim = grid; cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = h->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        real *HB = (real *)h->th_other(), *msum = (real *)h->mean();
+        const uint8_t *fl = h->flags();
+        const uint32_t *lk = h->links();
+        if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB>, B, HB, fl, lk, msum, P, T, O);
+        else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB>, B, HB, fl, lk, msum, P, T, O);
         return check_launch(h, "thermal_step_kernel");
     }
     const bool turb = h->nmodes > 0 && P.F > 0;

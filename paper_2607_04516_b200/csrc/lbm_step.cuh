@@ -79,6 +79,8 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
         // boundary velocity of the step AFTER this one (tb.t) into the half this launch writes — the EQ_FIXED cells of the
         // next launch read it from there.  They are dispatched first and run beside the memory-bound lattice blocks.
         if (zb < turb_planes) {
+            asm volatile("griddepcontrol.launch_dependents;");
+            asm volatile("griddepcontrol.wait;" ::: "memory"); // the half written here is the one the previous launch reads
             const int s = (zb * (int)gridDim.x + (int)blockIdx.x) * BLOCK + (int)threadIdx.x;
             if (s < P.F) fluct_slot<real, false, S>(s, nullptr, nullptr, nullptr, fuw, nullptr, flags, tb, P);
             return;
@@ -94,6 +96,12 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
     // them with: the last plane goes first, everything else one later.
     const int z = zb == 0 ? P.nz - 1 : zb - 1;
     const int p = pidx(P, x, y, z);
+    // Programmatic dependent launch: the next step's launch may be set up while this one drains (launch_dependents, issued at
+    // once: the dependent grid is admitted only when every CTA of this one has started), and this grid's threads do their
+    // index arithmetic before the previous step has finished — but touch no memory until it has (wait).  Both are no-ops for
+    // a launch without the attribute.
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
 
     real g[Q];
     uint8_t fl;

@@ -113,6 +113,8 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
     const int x = (int)c2 - y * P.nx;
     const int z = blockIdx.y == 0 ? P.nz - 1 : (int)blockIdx.y - 1; // the all-slow top plane first, not as the tail (lbm_step.cuh)
     const int p = pidx(P, x, y, z);
+    asm volatile("griddepcontrol.launch_dependents;");   // programmatic dependent launch, as in step_body (lbm_step.cuh)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     // as in step_kernel's SPEC instantiations: all 26 pulls are issued before the flag byte has arrived (no dependent
     // round trip; a SOLID cell then costs its reads), pinned by volatile asm so that the flag test cannot move above them
     real g[Q], t[QT];
