@@ -135,7 +135,7 @@ def load_traffic(kernel="step"):
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap,timestamp")
 
     def __init__(self, index=0):
         self.index = index
@@ -145,11 +145,30 @@ class ClockSampler:
     def start(self):
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "20"], stdout=self.f, stderr=subprocess.DEVNULL)
         except Exception:
             self.p = None
 
-    def stop(self):
+    def wait_first_sample(self, timeout=2.0):
+        """nvidia-smi needs ~0.1-0.3 s to print its first line: a short timed region must not start before it samples."""
+        if self.p is None:
+            return
+        t0 = time.perf_counter()
+        while time.perf_counter() - t0 < timeout:
+            try:
+                if os.path.getsize(self.f.name) > 0:
+                    return
+            except OSError:
+                return
+            time.sleep(0.01)
+
+    def mark(self):
+        """host wall-clock time, to cut the samples down to a window (nvidia-smi stamps each line with the same clock)"""
+        return time.time()
+
+    def stop(self, t_from=None, t_to=None):
+        """Median SM clock and throttle reasons of the samples stamped within [t_from, t_to] (+- one sampling period); if the
+        window is shorter than the sampling period and holds none, the sample nearest to it."""
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
         if self.p is None:
             return out
@@ -162,6 +181,21 @@ class ClockSampler:
         self.f.flush()
         rows = [r.strip().split(",") for r in open(self.f.name) if r.strip()]
         os.unlink(self.f.name)
+        if t_from is not None and t_to is not None:
+            import datetime
+            stamped = []
+            for r in rows:
+                try:
+                    ts = datetime.datetime.strptime(r[7].strip(), "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                except Exception:
+                    continue
+                stamped.append((ts, r))
+            inside = [r for ts, r in stamped if t_from - 0.02 <= ts <= t_to + 0.02]
+            if not inside and stamped:
+                mid = 0.5 * (t_from + t_to)
+                inside = [min(stamped, key=lambda q: abs(q[0] - mid))[1]]
+            if stamped:
+                rows = inside
         sm, reasons, mx = [], set(), None
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for r in rows:
@@ -288,11 +322,13 @@ def run_ours(args):
     if args.variant:
         for s_ in job_.sims:
             s_.set_variant(args.variant)
-    job_.step(Wm)
-    barrier()
     sampler = ClockSampler(local)
     if rank == 0:
         sampler.start()
+        sampler.wait_first_sample()   # sampling (every 20 ms) runs through warm-up and the timed region
+    t_load0 = sampler.mark()          # the clock record covers warm-up + timed region (the latter alone can be a few ms)
+    job_.step(Wm)
+    barrier()
     l0 = job_.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     reps = max(1, args.repeats)
@@ -306,7 +342,7 @@ def run_ours(args):
         ms = e0.elapsed_time(e1)
         best = ms if best is None else min(best, ms)
     launches = (job_.launch_count() - l0) // reps
-    clocks = sampler.stop() if rank == 0 else None
+    clocks = sampler.stop(t_load0, sampler.mark()) if rank == 0 else None
     # second region: the same step back to back for >= SUSTAINED_SECONDS, where the board sits at its power cap (the K-step
     # region above can be a burst at boost clock when the driver asks for few steps)
     sustained = None
@@ -315,14 +351,16 @@ def run_ours(args):
         s2 = ClockSampler(local)
         if rank == 0:
             s2.start()
+            s2.wait_first_sample()
         barrier()
+        t_s0 = s2.mark()
         e0.record()
         job_.step(ks)
         e1.record()
         barrier()
         ms_s = max_over_ranks(e0.elapsed_time(e1), world, dev)
         sustained = {"value": job_mlups(cells, ks, world, ms_s * 1e-3), "unit": "MLUPS", "steps": ks, "ms_per_step": ms_s / ks,
-                     "clocks": s2.stop() if rank == 0 else None}
+                     "clocks": s2.stop(t_s0, s2.mark()) if rank == 0 else None}
     rho, ux, uy, uz = sim.get_macros()
     finite = bool(torch.isfinite(ux).all().item())
     ms_total = max_over_ranks(best, world, dev)
