@@ -423,10 +423,10 @@ def lattice():
     return c, opp
 
 
-def from_workload(wl, fp64=False, want_mean=True, device="cuda:0", storage16=False) -> Lbm:
+def from_workload(wl, fp64=False, want_mean=True, device="cuda:0", storage16=False, stream=None) -> Lbm:
     """Create a handle for a workloads.Workload and load its flags, inlet profile and initial field."""
     sim = Lbm(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces, fp64=fp64, want_mean=want_mean,
-              device=device, storage16=storage16)
+              device=device, storage16=storage16, stream=stream)
     sim.set_flags(wl.height)
     if wl.inlet_profile is not None:
         sim.set_inlet_profile(*wl.inlet_profile)

@@ -836,18 +836,26 @@ int do_feed(lbm_t *dst, const lbm_t *src, int sx)
 {
     const Params<real> D = make_params<real>(dst), Ps = make_params<real>(src);
     const int B = 128;
-    if (src->stream != dst->stream) {
-        // the plane is read on dst's stream: order it after everything queued on src's stream (the precursor's last step)
-        cudaEvent_t ev;
+    const bool cross = src->stream != dst->stream;
+    cudaEvent_t ev = nullptr;
+    if (cross) {
+        // the plane is read on dst's stream: order it after everything queued on src's stream (the precursor's last step) ...
         CUDA_TRY(dst, cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
         cudaError_t e = cudaEventRecord(ev, src->stream);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(dst->stream, ev, 0);
-        cudaEventDestroy(ev); // released once the recorded work has completed
-        if (e != cudaSuccess) return fail(dst, LBM_ECUDA, std::string("feed_inlet: ") + cudaGetErrorString(e));
+        if (e != cudaSuccess) { cudaEventDestroy(ev); return fail(dst, LBM_ECUDA, std::string("feed_inlet: ") + cudaGetErrorString(e)); }
     }
     feed_kernel<real, S><<<blocks_for((long long)D.ny * D.nz, B), B, 0, dst->stream>>>(
         (S *)dst->bufA(), (S *)dst->bufB(), (real *)dst->fu(), dst->flags(), D, (const S *)src->state(), src->flags(), Ps, sx);
     int rc = check_launch(dst, "feed_kernel");
+    if (cross) {
+        // ... and what src does next after the read: its step after next rewrites the buffer this plane lies in, and src's
+        // stream may run ahead of dst's by any number of steps
+        cudaError_t e = cudaEventRecord(ev, dst->stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(src->stream, ev, 0);
+        cudaEventDestroy(ev); // released once the recorded work has completed
+        if (e != cudaSuccess && !rc) rc = fail(dst, LBM_ECUDA, std::string("feed_inlet: ") + cudaGetErrorString(e));
+    }
     return rc ? rc : thermal_refresh<real>(dst);
 }
 

@@ -216,6 +216,31 @@ def test_config5_chain_precursor_plane_feeds_main_inlet_every_step(B):
     assert e_pre <= TOL32 and e_main <= TOL32
 
 
+def test_config5_chain_on_two_streams_equals_the_chain_on_one(B):
+    """lbm_feed_inlet with the precursor and the main lattice on different streams: the read of the plane waits for the
+    precursor's last step, and the precursor's next steps wait for the read (its stream runs far ahead of the 7x larger
+    main lattice otherwise and rewrites the buffer the plane lies in).  Bit-identical to the single-stream chain."""
+    import torch
+    from paper_2607_04516_b200 import workloads as W
+    pre = W.config5_precursor(nx=32, ny=24, nz=40)
+    main = W.config5_main(nx=224, ny=60, nz=40)
+    xs = 16
+    results = []
+    for two in (False, True):
+        sp = torch.cuda.Stream() if two else None
+        sm = torch.cuda.Stream() if two else None
+        torch.cuda.synchronize()
+        gp, gm = B.from_workload(pre, stream=sp), B.from_workload(main, stream=sm)
+        for _ in range(40):
+            gm.feed_inlet(gp, xs)
+            gp.step(1); gm.step(1)
+        results.append([a.cpu().numpy() for a in gm.get_macros()] + [a.cpu().numpy() for a in gp.get_macros()])
+        torch.cuda.synchronize()
+        gp.close(); gm.close()
+    for a, b in zip(*results):
+        np.testing.assert_array_equal(a, b)
+
+
 def test_inlet_plane_host_and_device_pointers(B):
     import torch
     from oracle import Oracle
