@@ -188,8 +188,17 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
         equilibrium(g, real(0), u0, u1, u2);
         thermal_equilibrium(t, dth, P.theta_ref, u0, u1, u2);
     }
-    store_cell(B, P, p, x, y, z, fl, lk, g);
-    store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
+    // own slots and wall mailboxes of both lattices (store_cell / store_cell_thermal with the EDGE part masked off), then ONE
+    // ghost-store sequence for both: the face logic per direction is shared, which halves that code (the fused body is larger
+    // than the instruction cache)
+    store_cell(B, P, p, x, y, z, (uint8_t)(fl & ~EDGE_BIT), lk, g);
+    store_cell_thermal(HB, P, p, x, y, z, (uint8_t)(fl & ~EDGE_BIT), lk, t);
+    if (fl & EDGE_BIT)
+        ghost_stores(P, x, y, z, lk, [&](int i, int pt, auto jc) {
+            constexpr int j = decltype(jc)::value;
+            B[(long long)i * P.stride + pt] = g[j];
+            if constexpr (j < QT) HB[(long long)i * P.stride + pt] = t[j]; // an axis direction reflects into an axis direction
+        });
     if constexpr (MEAN) {
         msum[p] += m.ux;
         msum[P.stride + p] += m.uy;
