@@ -138,9 +138,19 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
         for (int i = 0; i < QT; ++i) t[i] = t[i] - P.omega_t * (t[i] - e[i]);
         return m;
     };
+    // ONE instance of the collision pair serves both paths (a second inlined copy put the body further beyond the instruction
+    // cache): the link word of a wall-link / surface cell is requested first, so that it travels while the collision runs
+    const int cls = fl & CLASS_MASK;
+    uint32_t lk = 0;
+    if (fl & (SLOW_BIT | SURF_BIT)) lk = links[p];
+    Macro<real> m{real(1), real(0), real(0), real(0)};
+    real dth = real(0); // the pulled theta: what a feeding cell publishes (its collision conserves it)
+    if (cls == FLUID) {
+        dth = theta_shift(t);
+        m = collide_both();
+    }
     // fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, nothing to complete)
     if (__all_sync(__activemask(), fl == 0)) {
-        const Macro<real> m = collide_both();
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             T.gdst[i][p] = g[i];
@@ -156,9 +166,6 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
         }
         return;
     }
-    const int cls = fl & CLASS_MASK;
-    uint32_t lk = 0;
-    if (fl & (SLOW_BIT | SURF_BIT)) lk = links[p];
     if (cls == SOLID) {
         // surface solid: completes the 32-byte sectors its live neighbours write, with zeros, in both lattices
         if (fl & SURF_BIT) {
@@ -172,10 +179,7 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
         }
         return;
     }
-    Macro<real> m;
     if (cls == FLUID) {
-        const real dth = theta_shift(t); // the pulled theta: what a feeding cell publishes (its collision conserves it)
-        m = collide_both();
         if (fl & FEED_BIT)
             outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) {
                 O.fuw[comp * P.F + sl] = v;
@@ -183,10 +187,10 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
             });
     } else { // EQ_FIXED / EQ_OUTFLOW: both equilibria of the slot's (theta, u), re-stored every step like the plain kernel's EQ cells
         const int sl = eq_slot(P, cls, x, y, z);
-        const real u0 = O.fur[sl], u1 = O.fur[P.F + sl], u2 = O.fur[2 * P.F + sl], dth = O.ftr[sl];
+        const real u0 = O.fur[sl], u1 = O.fur[P.F + sl], u2 = O.fur[2 * P.F + sl], db = O.ftr[sl];
         m = Macro<real>{real(1), u0, u1, u2};
         equilibrium(g, real(0), u0, u1, u2);
-        thermal_equilibrium(t, dth, P.theta_ref, u0, u1, u2);
+        thermal_equilibrium(t, db, P.theta_ref, u0, u1, u2);
     }
     // own slots and wall mailboxes of both lattices (store_cell / store_cell_thermal with the EDGE part masked off), then ONE
     // ghost-store sequence for both: the face logic per direction is shared, which halves that code (the fused body is larger
