@@ -134,20 +134,46 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
     } else {
         fl = flags[p];
     }
-    const int cls = fl & CLASS_MASK;
-    // Fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, nothing to complete) — the bulk of
-    // the lattice — or an EQ cell / a feeding cell without wall link or ghost slot (the inlet and outflow cells at the two
-    // ends of every row): collide (or re-expand the equilibrium), 19 stores, none of the per-feature tests further down.
-    bool fast = false;
-    if constexpr (SPEC) fast = __all_sync(__activemask(), (fl & (SLOW_BIT | EDGE_BIT | SURF_BIT)) == 0 && cls != SOLID && cls != GHOST);
-    // link word: wall links of a FLUID cell / zero-fill mask of a surface SOLID cell; one predicated load for both, issued
-    // as soon as the flag is there and consumed only after the collision (fast warps have neither)
-    uint32_t lk = 0;
-    if (!fast) {
-        if (fl & (SLOW_BIT | SURF_BIT)) lk = links[p];
+    if constexpr (SPEC) {
+        // Fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, nothing to complete) — the
+        // bulk of the lattice — or an EQ cell / a feeding cell without wall link or ghost slot (the inlet and outflow cells
+        // at the two ends of every row).  Straight-line collide (or equilibrium re-expansion) + 19 stores, none of the
+        // per-feature tests below.
+        const bool plain = (fl & (SLOW_BIT | EDGE_BIT | SURF_BIT)) == 0 && (fl & CLASS_MASK) != SOLID && (fl & CLASS_MASK) != GHOST;
+        if (__all_sync(__activemask(), plain)) {
+            Macro<real> m;
+            if ((fl & CLASS_MASK) == FLUID) {
+                if constexpr (DAMP) m = collide<real, true>(g, P, dmp);
+                else m = collide(g, P);
+            } else {
+                m = Macro<real>{real(1), fu0, fu1, fu2};
+                equilibrium(g, real(0), fu0, fu1, fu2);
+            }
+            static_for<0, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                st_s(T.dst[i] + p, g[i]);
+            });
+            if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) { fuw[comp * P.F + sl] = v; });
+            if constexpr (MEAN) {
+                msum[p] = ms0 + m.ux;
+                msum[P.stride + p] = ms1 + m.uy;
+                msum[2 * P.stride + p] = ms2 + m.uz;
+            }
+            return;
+        }
     }
-    // ONE instance of the collision (and of the equilibrium re-expansion) serves both paths
+    const int cls = fl & CLASS_MASK;
+    // link word: wall links of a FLUID cell / zero-fill mask of a surface SOLID cell; one predicated load for both,
+    // issued as soon as the flag is there and consumed only after the collision
+    uint32_t lk = 0;
+    if (fl & (SLOW_BIT | SURF_BIT)) lk = links[p];
+    if (cls == SOLID && !(fl & SURF_BIT)) return;
     Macro<real> m{real(1), real(0), real(0), real(0)};
+    const bool merged_solid = cls == SOLID; // a surface solid: it only completes sectors, with zeros
+    if (merged_solid) {
+#pragma unroll
+        for (int i = 0; i < Q; ++i) g[i] = real(0);
+    }
     if (cls == FLUID) {
         if constexpr (!SPEC) {
             static_for<0, Q>([&](auto ic) {
@@ -157,32 +183,13 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
         }
         if constexpr (DAMP) m = collide<real, true>(g, P, SPEC ? dmp : damp_at(P, x, y, z));
         else m = collide(g, P);
-    } else if (cls == EQ_FIXED || cls == EQ_OUTFLOW) { // a3 / a6: f_eq(1, u) of the cell's face velocity (lbm_core.cuh)
+    } else if (cls != SOLID) { // EQ_FIXED (a3) / EQ_OUTFLOW (a6): f_eq(1, u) of the cell's face velocity (lbm_core.cuh)
         if constexpr (!SPEC) {
             const int sl = eq_slot(P, cls, x, y, z);
             fu0 = fur[sl]; fu1 = fur[P.F + sl]; fu2 = fur[2 * P.F + sl];
         }
         m = Macro<real>{real(1), fu0, fu1, fu2};
-        equilibrium(g, real(0), fu0, fu1, fu2);
-    }
-    if (fast) {
-        static_for<0, Q>([&](auto ic) {
-            constexpr int i = decltype(ic)::value;
-            st_s(T.dst[i] + p, g[i]);
-        });
-        if (fl & FEED_BIT) outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) { fuw[comp * P.F + sl] = v; });
-        if constexpr (MEAN) {
-            msum[p] = ms0 + m.ux;
-            msum[P.stride + p] = ms1 + m.uy;
-            msum[2 * P.stride + p] = ms2 + m.uz;
-        }
-        return;
-    }
-    if (cls == SOLID && !(fl & SURF_BIT)) return;
-    const bool merged_solid = cls == SOLID; // a surface solid: it only completes sectors, with zeros
-    if (merged_solid) {
-#pragma unroll
-        for (int i = 0; i < Q; ++i) g[i] = real(0);
+        equilibrium(g, real(0), m.ux, m.uy, m.uz);
     }
     // ONE store sequence for the whole warp.  A surface solid takes part in it with zeros, predicated by its completion
     // mask: a solid cell whose 32-byte sector is written by others (live cells, neighbours' mailboxes) completes it, so
