@@ -175,6 +175,7 @@ Params<real> make_params(const lbm_t *h)
     P.nx = h->nx; P.ny = h->ny; P.nz = h->nz;
     P.px = h->L.px; P.py = h->L.py; P.pxy = h->L.px * h->L.py;
     P.xoff = h->s16 ? 16 : 8; P.sec = h->s16 ? 16 : 8;
+    P.perx = h->face[0] == LBM_PERIODIC ? 1 : 0; // set_boundaries guarantees both x faces then
     P.Np = (int)h->L.Np;
     P.N = (int)h->N();
     P.nxy = h->nx * h->ny;
@@ -486,9 +487,13 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     return rc;
 }
 
-template <typename real, typename S, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
+template <typename real, typename S, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false, bool PERX = false>
 int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 {
+    if constexpr (!PERX) {
+        // the read-side wrap instantiation carries two more cell indices: one CTA per SM less instead of spills
+        if (P.perx) return launch_step_as<real, S, SPEC, BLOCK, (SPEC && MINB == 10) ? 9 : MINB, DAMP, TURB, true>(h, P, sample);
+    }
     const S *A = (const S *)h->state();
     S *B = (S *)h->other();
     real *ms = (real *)h->mean();
@@ -514,8 +519,8 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
     cfg.attrs = at; cfg.numAttrs = 1;
     const uint8_t *fl = h->flags();
     const uint32_t *lk = h->links();
-    if (sample) cudaLaunchKernelEx(&cfg, step_kernel<real, S, true, SPEC, BLOCK, MINB_S, DAMP, TURB>, A, B, fl, lk, ms, fur, fuw, P, T, tb, turb_planes);
-    else cudaLaunchKernelEx(&cfg, step_kernel<real, S, false, SPEC, BLOCK, MINB, DAMP, TURB>, A, B, fl, lk, ms, fur, fuw, P, T, tb, turb_planes);
+    if (sample) cudaLaunchKernelEx(&cfg, step_kernel<real, S, true, SPEC, BLOCK, MINB_S, DAMP, TURB, PERX>, A, B, fl, lk, ms, fur, fuw, P, T, tb, turb_planes);
+    else cudaLaunchKernelEx(&cfg, step_kernel<real, S, false, SPEC, BLOCK, MINB, DAMP, TURB, PERX>, A, B, fl, lk, ms, fur, fuw, P, T, tb, turb_planes);
     return check_launch(h, "step_kernel");
 }
 
@@ -523,7 +528,7 @@ int launch_step_as(lbm_t *h, const Params<real> &P, bool sample)
 template <int V>
 bool vec_geom(const Params<float> &P, VecGeom *G)
 {
-    if (P.nx % V != 0) return false;
+    if (P.nx % V != 0 || P.perx) return false; // periodic x: the read-side wrap lives in the one-cell kernel only
     G->qpr = (unsigned)(P.nx / V);
     G->nq = (unsigned)((long long)P.nxy / V);
     G->qmagic = 0;
@@ -591,8 +596,13 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         real *HB = (real *)h->th_other(), *msum = (real *)h->mean();
         const uint8_t *fl = h->flags();
         const uint32_t *lk = h->links();
-        if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB>, B, HB, fl, lk, msum, P, T, O);
-        else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB>, B, HB, fl, lk, msum, P, T, O);
+        if (P.perx) {
+            if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O);
+            else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O);
+        } else {
+            if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB, false>, B, HB, fl, lk, msum, P, T, O);
+            else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB, false>, B, HB, fl, lk, msum, P, T, O);
+        }
         return check_launch(h, "thermal_step_kernel");
     }
     const bool turb = h->nmodes > 0 && P.F > 0;
@@ -653,7 +663,8 @@ int try_step_loop(lbm_t *h, const Params<real> &P, int want)
         if (h->variant != 0 || h->nmodes > 0 || h->thermal || want < 4 || h->loop_ok < 0) return 0;
         constexpr int BLOCK = 128;
         const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
-        const void *fn = h->damp_on ? (const void *)step_loop_kernel<float, S, BLOCK, 8, true> : (const void *)step_loop_kernel<float, S, BLOCK, 8, false>;
+        const void *fn = P.perx ? (h->damp_on ? (const void *)step_loop_kernel<float, S, BLOCK, 8, true, true> : (const void *)step_loop_kernel<float, S, BLOCK, 8, false, true>)
+                                : (h->damp_on ? (const void *)step_loop_kernel<float, S, BLOCK, 8, true, false> : (const void *)step_loop_kernel<float, S, BLOCK, 8, false, false>);
         if (h->loop_ok == 0) { // once per handle: can the whole grid be resident?
             int dev = 0, sms = 0, coop = 0, per_sm = 0;
             cudaGetDevice(&dev);

@@ -64,6 +64,7 @@ template <typename real>
 struct Params {
     int nx, ny, nz;   // interior cells
     int px, py, pxy;  // padded x pitch (multiple of 32, >= nx + xoff + 1), padded rows per plane (ny + 2), px * py
+    int perx;         // both x faces PERIODIC: the pull across them wraps on the READ side (xwrap below), no x ghost slots
     int xoff, sec;    // padded x of interior x = 0 (one 32-byte sector of storage elements), cells per 32-byte sector (8; 16 for __half)
     int Np;           // padded cells = pxy * (nz + 2)
     int N;            // interior cells
@@ -107,6 +108,20 @@ template <int I, typename real>
 __host__ __device__ __forceinline__ int poff(const Params<real> &P)
 {
     return dir_cx(I) + dir_cy(I) * P.px + dir_cz(I) * P.pxy;
+}
+
+// PERIODIC x faces.  A ghost slot in the x halo would be a single element in an otherwise untouched 32-byte sector (a DRAM
+// read-modify-write per row and direction: 2.4 - 6 % of the step), so the wrap across the x faces is done by
+// the READER instead: the pull of a direction with c_x = +1 by a cell at x = 0 comes from x = nx - 1 of the same source row
+// (index + nx), with c_x = -1 at x = nx - 1 from x = 0 (index - nx).  Everything addressed relative to a pull source moves
+// with it: the bounce-back mailbox of such a link lies in the wrapped cell, and a population that leaves through a periodic
+// x face AND a y / z face goes to the y / z halo slot of its own x column.  xwrap = cells to add to p - off_i.
+template <int I, typename real>
+__host__ __device__ __forceinline__ int xwrap(const Params<real> &P, int x)
+{
+    if constexpr (dir_cx(I) == 1) return (P.perx && x == 0) ? P.nx : 0;
+    else if constexpr (dir_cx(I) == -1) return (P.perx && x == P.nx - 1) ? -P.nx : 0;
+    else return 0;
 }
 
 // c . a for a lattice vector known at compile time: only the non-zero components are touched (no 0 * x terms,
@@ -315,11 +330,11 @@ __device__ __forceinline__ void load_cell(real (&g)[Q], const S *__restrict__ A,
 // st(i, pt, jc): "slot (direction i, padded cell pt) <- g[jc]" with jc an integral_constant (register indexing).
 // Wall links: bit i of lk set <=> the pull source of direction i is SOLID <=> population opp(i) leaves towards it.
 template <typename real, class St>
-__device__ __forceinline__ void wall_stores(const Params<real> &P, int p, uint32_t lk, St &&st)
+__device__ __forceinline__ void wall_stores(const Params<real> &P, int p, int x, uint32_t lk, St &&st)
 {
     static_for<1, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        if ((lk >> i) & 1u) st(i, p - poff<i>(P), std::integral_constant<int, dir_opp(i)>{});
+        if ((lk >> i) & 1u) st(i, p - poff<i>(P) + xwrap<i>(P, x), std::integral_constant<int, dir_opp(i)>{});
     });
 }
 
@@ -336,11 +351,11 @@ __device__ __forceinline__ void ghost_stores(const Params<real> &P, int x, int y
         if constexpr (cx != 0) {
             const bool lo = x + cx < 0, hi = x + cx >= P.nx;
             if (lo | hi) {
-                out = true;
                 const int ft = lo ? P.face[0] : P.face[1];
-                if (ft == PERIODIC) hx = x - cx * P.nx;
-                else if (ft == FREE_SLIP) { hx = x + cx; fx = true; }
-                else ok = false;
+                if (ft == PERIODIC) { /* read-side wrap (xwrap): the slot stays in the cell's own x column and exists only if a
+                                         y / z face is crossed as well */ }
+                else if (ft == FREE_SLIP) { out = true; hx = x + cx; fx = true; }
+                else { out = true; ok = false; }
             }
         }
         if constexpr (cy != 0) {
@@ -389,7 +404,7 @@ __device__ __forceinline__ void store_cell(S *__restrict__ B, const Params<real>
     for (int i = 0; i < Q; ++i) st_s(B + ((long long)i * P.stride + p), g[i]);
     if (fl & (SLOW_BIT | EDGE_BIT)) {
         auto st = [&](int i, int pt, auto jc) { st_s(B + ((long long)i * P.stride + pt), g[decltype(jc)::value]); };
-        if (fl & SLOW_BIT) wall_stores(P, p, lk, st);
+        if (fl & SLOW_BIT) wall_stores(P, p, x, lk, st);
         if (fl & EDGE_BIT) ghost_stores(P, x, y, z, lk, st);
     }
 }

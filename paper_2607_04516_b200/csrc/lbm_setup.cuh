@@ -84,12 +84,19 @@ __global__ void classify_kernel(uint8_t *__restrict__ flags, uint32_t *__restric
         uint32_t written = 0, own = 0;
         for (int q = s0; q < s0 + P.sec; ++q) {
             const int cq = flags[q] & CLASS_MASK;
+            const int xq = q % P.px - P.xoff; // the sector lies in the cell's own row; at a row end it reaches into the x halo
+            if (P.perx && (xq < 0 || xq >= P.nx)) continue; // PERIODIC x: nothing is ever stored in the x halo (xwrap)
             if (cq == FLUID || cq == EQ_OUTFLOW || cq == EQ_FIXED) written |= 0x7FFFFu;
             else if (cq == SOLID) {
                 uint32_t mb = 0;
                 static_for<1, Q>([&](auto ic) {
                     constexpr int i = decltype(ic)::value;
-                    const int t = q + poff<i>(P);
+                    // the cell whose mailbox slot (i, q) is: the one that pulls direction i from q, across a periodic x face too
+                    int t = q + poff<i>(P);
+                    if (P.perx) {
+                        if (dir_cx(i) == 1 && xq == P.nx - 1) t -= P.nx;
+                        if (dir_cx(i) == -1 && xq == 0) t += P.nx;
+                    }
                     if (t >= 0 && t < P.Np) mb |= (((flags[t] & CLASS_MASK) == FLUID) ? 1u : 0u) << i;
                 });
                 written |= mb;

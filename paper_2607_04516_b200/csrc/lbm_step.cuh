@@ -67,7 +67,7 @@ inline StepPtrs<S> make_step_ptrs(const S *A, S *B, const Params<real> &P)
 
 // The step of one thread (one cell, or one face slot in a TURB block row).  A plain device function so that it can be
 // called once per launch (step_kernel) or in a loop with grid-wide barriers (step_loop_kernel, lattices that fit L2).
-template <typename real, typename S, bool MEAN, bool SPEC, int BLOCK, bool DAMP, bool TURB>
+template <typename real, typename S, bool MEAN, bool SPEC, int BLOCK, bool DAMP, bool TURB, bool PERX>
 __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict__ B, const uint8_t *__restrict__ flags,
                                           const uint32_t *__restrict__ links, real *__restrict__ msum, const real *__restrict__ fur,
                                           real *__restrict__ fuw, const Params<real> &P, const StepPtrs<S> &T, const Turb<real> &tb,
@@ -102,6 +102,19 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
     // a launch without the attribute.
     asm volatile("griddepcontrol.launch_dependents;");
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    // PERX (both x faces PERIODIC): the pulls with c_x = +1 / -1 of the first / last cell of a row wrap to the other end of
+    // their source row (lbm_core.cuh xwrap); an instantiation of its own, so that the other lattices carry no second index
+    int pL = p, pR = p;
+    if constexpr (PERX) {
+        if (x == 0) pL = p + P.nx;
+        if (x == P.nx - 1) pR = p - P.nx;
+    }
+    auto psrc = [&](auto ic) { // cell index of the pull source slot of direction i, before the table's - off_i
+        constexpr int i = decltype(ic)::value;
+        if constexpr (PERX && dir_cx(i) == 1) return pL;
+        else if constexpr (PERX && dir_cx(i) == -1) return pR;
+        else return p;
+    };
 
     real g[Q];
     uint8_t fl;
@@ -111,7 +124,7 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
     if constexpr (SPEC) {
         static_for<0, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            g[i] = real(ld_pinned(T.src[i] + p));
+            g[i] = real(ld_pinned(T.src[i] + psrc(ic)));
         });
         // a cell on an EQ face fetches its face velocity now, from geometry alone (EQ_FIXED wins, as in the voxeliser);
         // if the flag then says SOLID the three values are simply not used
@@ -178,7 +191,7 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
         if constexpr (!SPEC) {
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
-                g[i] = ld_s<real>(T.src[i] + p);
+                g[i] = ld_s<real>(T.src[i] + psrc(ic));
             });
         }
         if constexpr (DAMP) m = collide<real, true>(g, P, SPEC ? dmp : damp_at(P, x, y, z));
@@ -213,7 +226,7 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
         // wall links (lbm_core.cuh wall_stores, with the launch's address table): slot (i, p - off_i) <- g[opp(i)]
         static_for<1, Q>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
-            if ((lk >> i) & 1u) st_s(T.dst[i] + (p - poff<i>(P)), g[dir_opp(i)]);
+            if ((lk >> i) & 1u) st_s(T.dst[i] + (psrc(ic) - poff<i>(P)), g[dir_opp(i)]);
         });
     }
     if (fl & EDGE_BIT)
@@ -232,13 +245,13 @@ __device__ __forceinline__ void step_body(const S *__restrict__ A, S *__restrict
     }
 }
 
-template <typename real, typename S, bool MEAN, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false>
+template <typename real, typename S, bool MEAN, bool SPEC, int BLOCK, int MINB, bool DAMP = false, bool TURB = false, bool PERX = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 step_kernel(const S *__restrict__ A, S *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
             real *__restrict__ msum, const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> P, const StepPtrs<S> T,
             const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
 {
-    step_body<real, S, MEAN, SPEC, BLOCK, DAMP, TURB>(A, B, flags, links, msum, fur, fuw, P, T, tb, turb_planes);
+    step_body<real, S, MEAN, SPEC, BLOCK, DAMP, TURB, PERX>(A, B, flags, links, msum, fur, fuw, P, T, tb, turb_planes);
 }
 
 // Several steps in ONE cooperative launch, a grid-wide barrier between them: for lattices whose whole grid is resident
@@ -247,7 +260,7 @@ step_kernel(const S *__restrict__ A, S *__restrict__ B, const uint8_t *__restric
 // Every pull, the flag byte and the face velocities are read with ld.volatile / from read-only data, the barrier orders
 // the stores of one step before the loads of the next.  No time mean, no inflow fluctuations on this path (the host
 // falls back to single launches for those steps).
-template <typename real, typename S, int BLOCK, int MINB, bool DAMP>
+template <typename real, typename S, int BLOCK, int MINB, bool DAMP, bool PERX>
 __global__ void __launch_bounds__(BLOCK, MINB)
 step_loop_kernel(S *__restrict__ A, S *__restrict__ B, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
                  real *__restrict__ fu0, real *__restrict__ fu1, const Params<real> P, const StepPtrs<S> T0, const StepPtrs<S> T1,
@@ -256,9 +269,9 @@ step_loop_kernel(S *__restrict__ A, S *__restrict__ B, const uint8_t *__restrict
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const Turb<real> tb{};
     for (int s = 0; s < pairs; ++s) {
-        step_body<real, S, false, true, BLOCK, DAMP, false>(A, B, flags, links, nullptr, fu0, fu1, P, T0, tb, 0);
+        step_body<real, S, false, true, BLOCK, DAMP, false, PERX>(A, B, flags, links, nullptr, fu0, fu1, P, T0, tb, 0);
         grid.sync();
-        step_body<real, S, false, true, BLOCK, DAMP, false>(B, A, flags, links, nullptr, fu1, fu0, P, T1, tb, 0);
+        step_body<real, S, false, true, BLOCK, DAMP, false, PERX>(B, A, flags, links, nullptr, fu1, fu0, P, T1, tb, 0);
         grid.sync();
     }
 }

@@ -58,7 +58,7 @@ __device__ __forceinline__ void store_cell_thermal(real *__restrict__ HB, const 
                     const bool at = i == 1 ? x == 0 : i == 2 ? x == P.nx - 1 : i == 3 ? y == 0 : i == 4 ? y == P.ny - 1 : i == 5 ? z == 0 : z == P.nz - 1;
                     if (at && ((P.thd >> (i - 1)) & 1)) v = real(0.125) * P.thw[i - 1] - v;
                 }
-                HB[(long long)i * P.stride + (p - poff<i>(P))] = v;
+                HB[(long long)i * P.stride + (p - poff<i>(P) + xwrap<i>(P, x))] = v;
             }
         });
     }
@@ -102,7 +102,7 @@ inline ThermalPtrs<real> make_thermal_ptrs(const real *A, real *B, const real *H
 template <typename real>
 struct OpenFaces { const real *fur; real *fuw; const real *ftr; real *ftw; };
 
-template <typename real, bool MEAN, int BLOCK, int MINB>
+template <typename real, bool MEAN, int BLOCK, int MINB, bool PERX = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
                     real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O)
@@ -115,16 +115,27 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
     const int p = pidx(P, x, y, z);
     asm volatile("griddepcontrol.launch_dependents;");   // programmatic dependent launch, as in step_body (lbm_step.cuh)
     asm volatile("griddepcontrol.wait;" ::: "memory");
+    int pL = p, pR = p; // PERX: read-side wrap of the pulls across periodic x faces (lbm_core.cuh xwrap), as in step_body
+    if constexpr (PERX) {
+        if (x == 0) pL = p + P.nx;
+        if (x == P.nx - 1) pR = p - P.nx;
+    }
+    auto psrc = [&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        if constexpr (PERX && dir_cx(i) == 1) return pL;
+        else if constexpr (PERX && dir_cx(i) == -1) return pR;
+        else return p;
+    };
     // as in step_kernel's SPEC instantiations: all 26 pulls are issued before the flag byte has arrived (no dependent
     // round trip; a SOLID cell then costs its reads), pinned by volatile asm so that the flag test cannot move above them
     real g[Q], t[QT];
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        g[i] = ld_pinned(T.gsrc[i] + p);
+        g[i] = ld_pinned(T.gsrc[i] + psrc(ic));
     });
     static_for<0, QT>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        t[i] = ld_pinned(T.tsrc[i] + p);
+        t[i] = ld_pinned(T.tsrc[i] + psrc(ic));
     });
     const uint8_t fl = ld_pinned(flags + p);
     // the collision pair of one FLUID cell: buoyancy from the pulled theta into the flow collision, thermal BGK towards
