@@ -275,8 +275,9 @@ int lbm_lattice(int *c, int *opposite);
  *   0  default: 4 x-cells per thread with 128-bit loads / stores where nx % 4 == 0, else one cell per thread; lattices
  *      whose whole grid is resident at once run several steps per cooperative launch;
  *   1  one cell per thread, 32-bit accesses, one launch per step;
- *   2  2 x-cells per thread, 64-bit accesses (nx % 2 == 0, else as 1), one launch per step;
- *   3  4 x-cells per thread, 128-bit accesses (nx % 4 == 0, else as 1), one launch per step.
+ *   2  2 x-cells per thread, 64-bit accesses (32-bit with 16-bit storage; nx % 2 == 0, else as 1), one launch per step;
+ *   3  4 x-cells per thread, 128-bit accesses (64-bit with 16-bit storage; nx % 4 == 0, else as 1), one launch per step.
+ * Lattices with PERIODIC x faces always run one cell per thread (the read-side wrap lives there).
  * FP64 handles, damping zones, inflow fluctuations and the thermal lattice have one launch shape each and ignore it.
  * Returns LBM_EINVAL for an unknown variant. */
 int lbm_set_variant(lbm_t *h, int variant);

@@ -556,7 +556,7 @@ int launch_step_vec(lbm_t *h, const Params<float> &P, const VecGeom &G, bool sam
 //   0 = default: one cell per thread; lattices whose whole grid is resident at once run several steps per cooperative
 //       launch (step_loop_kernel)
 //   1 = one cell per thread, one launch per step
-//   2 = 2 cells per thread with 64-bit accesses where nx % 2 == 0 (16-bit storage: 8 cells, 128-bit, nx % 8 == 0), else as 1
+//   2 = 2 cells per thread with 64-bit accesses (16-bit storage: 32-bit) where nx % 2 == 0, else as 1
 //   3 = 4 cells per thread with 128-bit accesses (16-bit storage: 64-bit) where nx % 4 == 0, else as 1
 constexpr int N_VARIANTS = 4;
 #ifndef DAMP_MINB
@@ -623,7 +623,7 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         if constexpr (std::is_same<S, float>::value) {
             if (h->variant == 2 && vec_geom<2>(P, &G)) return launch_step_vec<S, 2, VEC2_MINB, 5>(h, P, G, sample);
         } else {
-            if (h->variant == 2 && vec_geom<8>(P, &G)) return launch_step_vec<S, 8, 2, 2>(h, P, G, sample);
+            if (h->variant == 2 && vec_geom<2>(P, &G)) return launch_step_vec<S, 2, VEC2_MINB, 5>(h, P, G, sample);
         }
         return launch_step_as<real, S, true, 128, 10>(h, P, sample);
     } else return launch_step_as<real, S, false, 256, 2>(h, P, sample);

@@ -59,6 +59,21 @@ struct VecIO<float, 8> { // the mean sums of the 8-cell kernel: two 128-bit acce
     }
 };
 template <>
+struct VecIO<__half, 2> {
+    static __device__ __forceinline__ void ld(const __half *p, float (&v)[2])
+    {
+        uint32_t a;
+        asm volatile("ld.global.b32 %0, [%1];" : "=r"(a) : "l"(p));
+        const float2 f = __half22float2(*reinterpret_cast<const __half2 *>(&a));
+        v[0] = f.x; v[1] = f.y;
+    }
+    static __device__ __forceinline__ void st(__half *p, const float (&v)[2])
+    {
+        const __half2 h = __floats2half2_rn(v[0], v[1]);
+        *reinterpret_cast<uint32_t *>(p) = *reinterpret_cast<const uint32_t *>(&h);
+    }
+};
+template <>
 struct VecIO<__half, 4> {
     static __device__ __forceinline__ void ld(const __half *p, float (&v)[4])
     {
