@@ -118,6 +118,23 @@ int lbm_set_flags_mask(lbm_t *h, const int32_t *height, const uint8_t *solid);
  * LBM_EINVAL: min_votes out of range, NULL tri, a vertex not finite or out of range.  Synchronises. */
 int lbm_set_flags_mesh(lbm_t *h, const int32_t *height, int n_tri, const float *tri, int min_votes);
 
+/* The same mesh voxeliser (DESIGN.md §4 reading 22; same tie rules, same kernels) WITHOUT a handle and
+ * WITHOUT any allocation: for callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it).  The scratch of the ray-cast passes lives in a file-scope device array inside the library, sized
+ * for boxes of at most LBM_STATIC_VOXEL_MAX_CELLS cells (2^21 = 128^3; 4 MiB held by every GPU that loads the library until
+ * the process exits); nx ny nz beyond that returns LBM_EINVAL with a message naming the limit — use lbm_set_flags_mesh there.
+ * dev_tri: float [n_tri][3][3], DEVICE memory; dev_solid: uint8 [nz][ny][nx], DEVICE memory, 1 = SOLID (at least min_votes
+ * of the three passes odd), 0 otherwise — both the caller's (host pointers are refused: staging them would allocate).
+ * cuda_stream: a cudaStream_t passed as void* (NULL = default stream).  Runs on the CURRENT device; calls no cudaMalloc,
+ * cudaFree or allocating library routine.  Synchronises the stream (the out-of-range-vertex flag is read back).
+ * Every call shares the one scratch array, which keeps the last call's contents (the call clears what must start at zero):
+ * calls that OVERLAP on the GPU — other streams, other host threads — race; serialise them.
+ * err: optional host buffer of err_len bytes for the message (no handle to keep it).  LBM_EINVAL: size beyond the limit, bad
+ * sizes / min_votes / NULL or host pointers, a vertex not finite or out of range.  LBM_ECUDA: a CUDA call failed. */
+#define LBM_STATIC_VOXEL_MAX_CELLS 2097152
+int lbm_voxelise_mesh_static(int nx, int ny, int nz, int n_tri, const float *dev_tri, int min_votes, uint8_t *dev_solid,
+                             void *cuda_stream, char *err, size_t err_len);
+
 /* Boundary wind profile ("macroscopic boundary states"): every EQ_FIXED cell at level z is set
  * to f_eq(1, (u[z], v[z], w[z])).  Each array [nz]; v, w may be NULL (= 0).  Needs flags. */
 int lbm_set_inlet_profile(lbm_t *h, const float *u, const float *v, const float *w);

@@ -30,6 +30,7 @@ SYMBOLS = [
     "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
     "lbm_set_thermal", "lbm_set_theta", "lbm_set_theta_f64", "lbm_get_theta", "lbm_get_theta_f64",
     "lbm_get_thermal_state", "lbm_set_thermal_state", "lbm_set_thermal_walls", "lbm_set_inlet_theta", "lbm_set_inlet_theta_f64",
+    "lbm_voxelise_mesh_static",
 ]
 
 
@@ -96,6 +97,7 @@ def load_library():
     lib.lbm_launch_count.restype = l
     lib.lbm_lattice.argtypes = [vp, vp]
     lib.lbm_set_variant.argtypes = [vp, i]
+    lib.lbm_voxelise_mesh_static.argtypes = [i, i, i, i, vp, i, vp, vp, C.c_char_p, C.c_size_t]
     _lib = lib
     return lib
 
@@ -119,6 +121,29 @@ def _ptr(a, dtype):
 
 
 PREC_F32, PREC_F64, PREC_F32_S16 = 0, 1, 2   # include/lbm.h LBM_PREC_*
+STATIC_VOXEL_MAX_CELLS = 2097152              # include/lbm.h LBM_STATIC_VOXEL_MAX_CELLS
+
+
+def voxelise_mesh_static(tri, nx, ny, nz, min_votes=2, out=None, stream=None):
+    """lbm_voxelise_mesh_static: the mesh voxeliser without a handle and without any allocation inside the library (its
+    scratch is a static device array; boxes of at most STATIC_VOXEL_MAX_CELLS cells; overlapping calls race).
+    tri: DEVICE float32 tensor [n][3][3]; out: DEVICE uint8 tensor [nz][ny][nx] (allocated here, by torch, if None).
+    Runs on the device of `tri`.  Returns out (1 = SOLID)."""
+    import torch
+    lib = load_library()
+    if not (isinstance(tri, torch.Tensor) and tri.is_cuda and tri.dtype == torch.float32 and tri.is_contiguous()):
+        raise ValueError("tri must be a contiguous float32 CUDA tensor [n][3][3] (host arrays are refused: no staging, no allocation)")
+    n_tri = int(tri.numel() // 9)
+    with torch.cuda.device(tri.device):
+        if out is None:
+            out = torch.empty((int(nz), int(ny), int(nx)), dtype=torch.uint8, device=tri.device)
+        st = stream if stream is not None else torch.cuda.current_stream(tri.device)
+        err = C.create_string_buffer(256)
+        rc = lib.lbm_voxelise_mesh_static(int(nx), int(ny), int(nz), n_tri, tri.data_ptr() if n_tri else None, int(min_votes),
+                                          out.data_ptr(), st.cuda_stream, err, 256)
+    if rc != 0:
+        raise LbmError(f"lbm_voxelise_mesh_static failed: {_ERR.get(rc, rc)}: {err.value.decode()}")
+    return out
 
 
 class Lbm:

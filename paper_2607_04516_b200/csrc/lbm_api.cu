@@ -1477,3 +1477,120 @@ int lbm_set_variant(lbm_t *h, int variant)
 }
 
 } // extern "C"
+
+// ---- mesh voxeliser without a handle and without any allocation ---------------------------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it).
+// The scratch of the ray-cast passes (one vote byte and one toggle byte per cell, one error word) lives in a file-scope
+// device array of LBM_STATIC_VOXEL_MAX_CELLS cells: every GPU that loads this library holds its 4 MiB until exit.
+// Every call shares the array and it keeps the last call's contents: the call clears what must start at zero, and two
+// calls that overlap on the GPU (different streams, different host threads) RACE — serialise them.
+namespace {
+
+constexpr size_t SV_MAX_CELLS = LBM_STATIC_VOXEL_MAX_CELLS;
+constexpr size_t SV_VOTES_OFF = 0;                               // votes   [SV_MAX_CELLS] bytes
+constexpr size_t SV_TOG_OFF = SV_MAX_CELLS;                      // toggles [SV_MAX_CELLS + 256] bytes (words, padded)
+constexpr size_t SV_ERR_OFF = 2 * SV_MAX_CELLS + 256;            // one int
+constexpr size_t SV_BYTES = 2 * SV_MAX_CELLS + 512;
+static_assert(SV_MAX_CELLS % 256 == 0, "offsets must stay 256-byte aligned");
+
+static __device__ __align__(256) unsigned char g_static_voxel_scratch[SV_BYTES];
+
+// In host code the array's name is a host-side stand-in, NOT a device address: the address a kernel may use comes from
+// cudaGetSymbolAddress, asked once per device with that device current, and cached here.
+constexpr int SV_MAX_DEVICES = 64;
+unsigned char *g_sv_addr[SV_MAX_DEVICES] = {};
+
+int static_voxel_scratch(unsigned char **out, char *err, size_t err_len)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess && (dev < 0 || dev >= SV_MAX_DEVICES)) {
+        if (err && err_len) snprintf(err, err_len, "voxelise_mesh_static: device index %d beyond %d", dev, SV_MAX_DEVICES - 1);
+        return LBM_EINVAL;
+    }
+    if (e == cudaSuccess && !g_sv_addr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_static_voxel_scratch);
+        if (e == cudaSuccess) g_sv_addr[dev] = (unsigned char *)p;
+    }
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        if (err && err_len) snprintf(err, err_len, "voxelise_mesh_static: cudaGetSymbolAddress: %s", cudaGetErrorString(e));
+        return LBM_ECUDA;
+    }
+    *out = g_sv_addr[dev];
+    return LBM_OK;
+}
+
+// solid[c] = votes[c] >= min_votes
+__global__ void static_voxel_out_kernel(const uint8_t *__restrict__ votes, uint8_t *__restrict__ solid, long long N, int min_votes)
+{
+    const long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (c < N) solid[c] = votes[c] >= min_votes ? 1 : 0;
+}
+
+} // namespace
+
+extern "C" int lbm_voxelise_mesh_static(int nx, int ny, int nz, int n_tri, const float *dev_tri, int min_votes, uint8_t *dev_solid,
+                                        void *cuda_stream, char *err, size_t err_len)
+{
+    auto bad = [&](int code, const char *msg) {
+        if (err && err_len) snprintf(err, err_len, "voxelise_mesh_static: %s", msg);
+        return code;
+    };
+    if (err && err_len) err[0] = 0;
+    if (nx < 1 || ny < 1 || nz < 1) return bad(LBM_EINVAL, "nx, ny, nz must be >= 1");
+    const unsigned long long N = (unsigned long long)nx * (unsigned long long)ny * (unsigned long long)nz;
+    if (N > SV_MAX_CELLS) {
+        if (err && err_len)
+            snprintf(err, err_len, "voxelise_mesh_static: %llu cells exceed the static scratch of %llu cells (LBM_STATIC_VOXEL_MAX_CELLS); "
+                                   "use lbm_set_flags_mesh for larger boxes", N, (unsigned long long)SV_MAX_CELLS);
+        return LBM_EINVAL;
+    }
+    if (n_tri < 0 || (n_tri > 0 && !dev_tri)) return bad(LBM_EINVAL, "bad triangle array");
+    if (min_votes < 1 || min_votes > 3) return bad(LBM_EINVAL, "min_votes must be 1, 2 or 3");
+    if (!dev_solid) return bad(LBM_EINVAL, "dev_solid is NULL");
+    if (!is_device_ptr(dev_solid) || (n_tri > 0 && !is_device_ptr(dev_tri))) return bad(LBM_EINVAL, "tri and solid must be DEVICE pointers (nothing is staged: no allocation)");
+    unsigned char *base = nullptr;
+    int rc = static_voxel_scratch(&base, err, err_len);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    uint8_t *votes = base + SV_VOTES_OFF, *toggles = base + SV_TOG_OFF;
+    int *errw = (int *)(base + SV_ERR_OFF);
+    const size_t tog_bytes = align_up((size_t)N, 4) + 4;
+    cudaError_t e = cudaMemsetAsync(votes, 0, (size_t)N, st);               // the array keeps the last call's contents
+    if (e == cudaSuccess) e = cudaMemsetAsync(errw, 0, sizeof(int), st);
+    const int B = 128;
+    const unsigned tg = blocks_for((long long)n_tri * 32, B);
+    const int n[3] = {nx, ny, nz};
+    for (int d = 0; d < 3 && n_tri > 0 && e == cudaSuccess; ++d) {
+        e = cudaMemsetAsync(toggles, 0, tog_bytes, st);
+        if (e != cudaSuccess) break;
+        const unsigned sg = blocks_for((long long)n[(d + 1) % 3] * n[(d + 2) % 3], B);
+        if (d == 0) {
+            mesh_toggle_kernel<0><<<tg, B, 0, st>>>(dev_tri, n_tri, (uint32_t *)toggles, nx, ny, nz, errw);
+            mesh_scan_kernel<0><<<sg, B, 0, st>>>(toggles, votes, nx, ny, nz);
+        } else if (d == 1) {
+            mesh_toggle_kernel<1><<<tg, B, 0, st>>>(dev_tri, n_tri, (uint32_t *)toggles, nx, ny, nz, errw);
+            mesh_scan_kernel<1><<<sg, B, 0, st>>>(toggles, votes, nx, ny, nz);
+        } else {
+            mesh_toggle_kernel<2><<<tg, B, 0, st>>>(dev_tri, n_tri, (uint32_t *)toggles, nx, ny, nz, errw);
+            mesh_scan_kernel<2><<<sg, B, 0, st>>>(toggles, votes, nx, ny, nz);
+        }
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) {
+        static_voxel_out_kernel<<<blocks_for((long long)N, 256), 256, 0, st>>>(votes, dev_solid, (long long)N, min_votes);
+        e = cudaGetLastError();
+    }
+    int badv = 0;
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&badv, errw, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        if (err && err_len) snprintf(err, err_len, "voxelise_mesh_static: %s", cudaGetErrorString(e));
+        return LBM_ECUDA;
+    }
+    if (badv) return bad(LBM_EINVAL, "a vertex is not finite or outside [-1024, 2048) cells");
+    return LBM_OK;
+}
