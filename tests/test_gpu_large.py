@@ -118,15 +118,21 @@ def test_tall_box_through_the_free_slip_top_of_config4(B):
     assert e <= TOL32, e
 
 
-@pytest.mark.parametrize("cfg,steps,start", [("config3", 3000, 1000), ("config4", 1500, 500)])
+@pytest.mark.parametrize("cfg,steps,start", [("config3", 20000, 10000), ("config4", 1500, 500)])
 def test_fp32_mean_profiles_agree_with_fp64_within_2_percent(B, cfg, steps, start):
+    """horizontally averaged, time-averaged u(z), v(z) of the FP32 run against the FP64 run of the same
+    kernels, max_z |d u| / max(u64, 0.25 u_ref) <= 2 %.  Config 3 runs the protocol at full length (20 000 steps, mean over
+    steps 10 000 .. 20 000 every 10: ~10 s FP32 + ~20 s FP64 on a B200) and includes the 16-bit storage mode (DESIGN.md §13:
+    its mean wind must be as close to FP64 as FP32's is).  Config 4 as BASELINE.json words it diverges near step 9 000 in FP64
+    as in FP32 (reflecting Dirichlet faces), so it is compared over its first 1 500 steps."""
     import torch
     from paper_2607_04516_b200 import workloads as W
     wl = getattr(W, cfg)()
     prof = {}
     flags = None
-    for fp64 in (False, True):
-        sim = B.from_workload(wl, fp64=fp64, want_mean=True)
+    modes = [("fp32", {}), ("fp64", {"fp64": True})] + ([("s16", {"storage16": True})] if cfg == "config3" else [])
+    for name, kw in modes:
+        sim = B.from_workload(wl, want_mean=True, **kw)
         sim.mean_config(start, 10)
         sim.step(steps)
         mx, my, mz, n = sim.get_mean(f64=True)
@@ -135,16 +141,20 @@ def test_fp32_mean_profiles_agree_with_fp64_within_2_percent(B, cfg, steps, star
             flags = sim.get_flags()
         fl = torch.from_numpy(flags != 1).to(mx.device)
         cnt = fl.sum(dim=(1, 2)).clamp(min=1)
-        prof[fp64] = [((m * fl).sum(dim=(1, 2)) / cnt).cpu().numpy() for m in (mx, my)]
+        prof[name] = [((m * fl).sum(dim=(1, 2)) / cnt).cpu().numpy() for m in (mx, my)]
         sim.close()
         del sim, mx, my, mz
         torch.cuda.empty_cache()
     u_ref = 0.08
-    for c in range(2):
-        p32, p64 = prof[False][c], prof[True][c]
-        assert np.isfinite(p32).all() and np.isfinite(p64).all()
-        rel = np.abs(p32 - p64) / np.maximum(np.abs(p64), 0.25 * u_ref)
-        assert rel.max() <= 0.02, (cfg, c, float(rel.max()))
+    for name in prof:
+        if name == "fp64":
+            continue
+        for c in range(2):
+            p, p64 = prof[name][c], prof["fp64"][c]
+            assert np.isfinite(p).all() and np.isfinite(p64).all()
+            rel = np.abs(p - p64) / np.maximum(np.abs(p64), 0.25 * u_ref)
+            print(f"{cfg} {name} component {c}: max relative deviation of the mean profile from FP64 {rel.max():.4f}")
+            assert rel.max() <= 0.02, (cfg, name, c, float(rel.max()))
 
 
 def test_config3_city_as_a_triangle_mesh_full_size(B):
