@@ -343,7 +343,11 @@ int do_set_flags(lbm_t *h, const int32_t *height, const uint8_t *dev_mask = null
     }
     if (!rc) {
         // in place: class bits are never changed by classify, only the SLOW / EDGE bits are added
-        classify_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->flags(), h->links(), P);
+        const dim3 cg((unsigned)(P.px / CT_X), blocks_for(P.ny, CT_Y), blocks_for(P.nz, CT_Z));
+        if (cg.y <= 65535u && cg.z <= 65535u) // tiled through shared memory; very flat / long boxes beyond the grid limits: one thread per cell
+            classify_tiled_kernel<real><<<cg, dim3(CT_X, CT_Y, CT_Z), 0, h->stream>>>(h->flags(), h->links(), P);
+        else
+            classify_kernel<real><<<blocks_for(P.N, B), B, 0, h->stream>>>(h->flags(), h->links(), P);
         rc = check_launch(h, "classify_kernel");
     }
     release_in(h, &in, 1);
