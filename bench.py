@@ -35,6 +35,9 @@ def metric_for(workload):
         return METRIC
     if workload == "c3-fp16":
         return "MLUPS (D3Q19, FP32 arithmetic, 16-bit population storage), fused stream-collide, 400x400x100 urban config, 1 B200"
+    if workload.endswith("-inplace"):
+        return (f"MLUPS (D3Q19 {'FP32 arithmetic, 16-bit storage' if 'fp16' in workload else 'FP32'}), fused stream-collide with in-place "
+                f"streaming (one population buffer), workload {workload} (a separate line, not the headline), 1 B200")
     return f"MLUPS (D3Q19 FP32), fused stream-collide, workload {workload} (per-config table line, not the headline), 1 B200"
 
 # --workload: the headline is c3 (BASELINE.json: the config the metric is quoted on); the others are the parity configs,
@@ -48,6 +51,11 @@ WORKLOADS = {
     "c3-fp16": "C3 urban 400x400x100 with 16-bit population storage (LBM_PREC_F32_S16, DESIGN.md §13): FP32 arithmetic, binary16 "
                "storage of the shifted populations, 77 B/cell — a separate line, NOT the FP32 headline",
     "c5": "C5 chain: periodic precursor 256x256x200 feeding the x- inlet of the 1200x1200x200 urban domain every step (BASELINE.json configs[4])",
+    # in-place streaming (LBM_STREAM_INPLACE): the same step on ONE population buffer, half the memory, same 153 B/cell
+    "c3-inplace": "C3 urban 400x400x100 with in-place streaming (one population buffer; DESIGN.md §14) — a separate line, NOT the headline",
+    "c4-inplace": "C4 refined urban 800x800x200 with in-place streaming (one population buffer; DESIGN.md §14)",
+    "c5-inplace": "C5 chain with in-place streaming on both lattices (one population buffer each; DESIGN.md §14)",
+    "c3-fp16-inplace": "C3 urban 400x400x100, 16-bit population storage AND in-place streaming: 77 B/cell, a quarter of the FP32 two-buffer memory",
 }
 
 
@@ -56,19 +64,23 @@ class Job:
 
     def __init__(self, name, binding, W, device):
         self.name, self.binding, self.device = name, binding, device
-        if name == "c5":
+        inplace = name.endswith("-inplace")
+        base = name[:-len("-inplace")] if inplace else name
+        if base == "c5":
             self.wls = [W.config5_precursor(), W.config5_main()]
         else:
             self.wls = [{"c1": W.config1, "c2": lambda: W.config2(Cs=0.1), "c3": W.config3, "c4": W.config4,
-                         "thermal": W.thermal_city, "c3-fp16": W.config3}[name]()]
+                         "thermal": W.thermal_city, "c3-fp16": W.config3}[base]()]
         self.cells = sum(w.cells for w in self.wls)
-        self.sims = [binding.from_workload(w, want_mean=False, device=device, storage16=(name == "c3-fp16")) for w in self.wls]
+        self.sims = [binding.from_workload(w, want_mean=False, device=device, storage16=(base == "c3-fp16"), inplace=inplace)
+                     for w in self.wls]
+        self.workspace_bytes = sum(s.workspace_bytes for s in self.sims)
 
     def step(self, n):
         if len(self.sims) == 1:
             self.sims[0].step(n)
             return
-        pre, main = self.sims
+        pre, main = self.sims  # config-5 chain
         xs = self.wls[0].extra["sample_plane_x"]
         for _ in range(n):
             main.feed_inlet(pre, xs)
@@ -401,11 +413,12 @@ def run_ours(args):
         per_launch_s = ms_total * 1e-3 / K
         # thermal workload: (19 + 7) x 4 B loads + (19 + 7) x 4 B stores + 1 flag byte (lbm_thermal.cuh)
         # 16-bit storage: 19 x 2 B loads + 19 x 2 B stores + 1 flag byte
-        BYTES_PER_CELL = {"thermal": 209, "c3-fp16": 77}.get(args.workload, globals()["BYTES_PER_CELL"])
+        BYTES_PER_CELL = {"thermal": 209, "c3-fp16": 77, "c3-fp16-inplace": 77}.get(args.workload, globals()["BYTES_PER_CELL"])
         achieved = BYTES_PER_CELL * cells / per_launch_s / 1e9
         traffic, traffic_src = (load_traffic("step") if args.workload == "c3" else
                                 load_traffic("thermal") if args.workload == "thermal" else
-                                load_traffic("s16") if args.workload == "c3-fp16" else (None, None))
+                                load_traffic("s16") if args.workload == "c3-fp16" else
+                                load_traffic("inplace") if args.workload == "c3-inplace" else (None, None))
         if traffic_src:
             traffic_src += " (committed ncu --set full capture; a constant, not measured in this run)"
         if sustained is not None:
@@ -414,13 +427,13 @@ def run_ours(args):
         line = {
             "metric": metric_for(args.workload), "value": mlups, "unit": "MLUPS", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32 arithmetic, f16 storage" if args.workload == "c3-fp16" else "f32", "data": "synthetic",
+            "dtype": "f32 arithmetic, f16 storage" if "fp16" in args.workload else "f32", "data": "synthetic",
             "config": {"workload": WORKLOADS[args.workload],
                        "cells": cells, "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": (f"no flush needed: each step streams {BYTES_PER_CELL * cells / 1e9:.1f} GB (>> 126 MB L2)"
                               if BYTES_PER_CELL * cells > 4 * 126e6 else
                               f"NOT flushed: the {2 * 76 * cells / 1e6:.0f} MB of this parity config stay L2-resident; not a bench line"),
-                       "best_of": reps, "variant": int(args.variant),
+                       "best_of": reps, "variant": int(args.variant), "workspace_bytes": int(job_.workspace_bytes),
                        "state_finite": finite},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,

@@ -62,9 +62,20 @@ enum { LBM_FLUID = 0, LBM_SOLID = 1, LBM_CELL_EQ_FIXED = 2, LBM_CELL_EQ_OUTFLOW 
  *                     with the thermal lattice (lbm_set_thermal returns LBM_EINVAL). */
 enum { LBM_PREC_F32 = 0, LBM_PREC_F64 = 1, LBM_PREC_F32_S16 = 2 };
 
-/* Bytes of device workspace a handle of this size needs (two population buffers of 19 stored values per cell,
- * one flag byte and one link word per cell, optional 3 reals per cell of time-mean sums, small profile/plane scratch).
- * precision: LBM_PREC_*; anything else returns LBM_EINVAL. */
+/* Streaming scheme, OR-ed into the `precision` argument of lbm_workspace_bytes / lbm_create_ex ("in-place
+ * streaming").  Default (bit clear): two population buffers, A -> B pull.  LBM_STREAM_INPLACE: ONE population
+ * buffer — every step reads and overwrites the same 19 addresses per cell, the two slots of a lattice link swapping roles from
+ * step to step — so a lattice takes about half the memory (config 5's 2.9e8 cells: 24 GB instead of 46 GB; 1.2e9 FP32 cells fit
+ * one B200), for the same 153 B per cell and step and the same arithmetic: every call works the same and returns the same
+ * values (lbm_get_state / lbm_set_state exchange the same post-collision populations).  Combinable with all three precisions,
+ * every face type, damping zones, flux correction, the time mean and lbm_feed_inlet (either side); NOT with the thermal lattice
+ * and the synthetic inflow fluctuations (lbm_set_thermal / lbm_set_inflow_turbulence return LBM_EINVAL), and lbm_set_variant has
+ * no effect (one launch shape: one cell per thread, one launch per step). */
+#define LBM_STREAM_INPLACE 16
+
+/* Bytes of device workspace a handle of this size needs (two population buffers of 19 stored values per cell — one with
+ * LBM_STREAM_INPLACE —, one flag byte and one link word per cell, optional 3 reals per cell of time-mean sums, small
+ * profile/plane scratch).  precision: LBM_PREC_* [| LBM_STREAM_INPLACE]; anything else returns LBM_EINVAL. */
 int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int precision, size_t *out);
 
 /* Create an FP32 handle that allocates its own workspace (cudaMalloc) and uses the default stream.
@@ -75,7 +86,8 @@ int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int precision, si
 int lbm_create(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3], lbm_t **out);
 
 /* Same, with a caller-owned DEVICE workspace of at least lbm_workspace_bytes() bytes (256-byte aligned;
- * NULL = allocate), a cudaStream_t passed as void* (NULL = default stream), and the precision (LBM_PREC_*).
+ * NULL = allocate), a cudaStream_t passed as void* (NULL = default stream), and the precision (LBM_PREC_*, optionally
+ * | LBM_STREAM_INPLACE).
  * want_mean = 0 omits the time-mean sums (lbm_mean_config then returns LBM_ESTATE). */
 int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, const double F[3],
                   void *dev_workspace, size_t workspace_bytes, void *cuda_stream, int precision, int want_mean,

@@ -121,6 +121,7 @@ def _ptr(a, dtype):
 
 
 PREC_F32, PREC_F64, PREC_F32_S16 = 0, 1, 2   # include/lbm.h LBM_PREC_*
+STREAM_INPLACE = 16                           # include/lbm.h LBM_STREAM_INPLACE (OR-ed into the precision argument)
 STATIC_VOXEL_MAX_CELLS = 2097152              # include/lbm.h LBM_STATIC_VOXEL_MAX_CELLS
 
 
@@ -150,7 +151,7 @@ class Lbm:
     """One lattice on one GPU.  Same call names as include/lbm.h without the ``lbm_`` prefix."""
 
     def __init__(self, nx, ny, nz, nu0, Cs=0.0, f_cor=0.0, F=(0.0, 0.0, 0.0), faces=None, fp64=False,
-                 want_mean=True, device="cuda:0", stream=None, storage16=False):
+                 want_mean=True, device="cuda:0", stream=None, storage16=False, inplace=False):
         import torch
         if not torch.cuda.is_available():
             raise LbmError("no CUDA device: the LBM path has no CPU fallback")
@@ -164,6 +165,9 @@ class Lbm:
         if fp64 and storage16:
             raise ValueError("fp64 and storage16 exclude each other")
         precision = PREC_F64 if fp64 else (PREC_F32_S16 if storage16 else PREC_F32)     # include/lbm.h LBM_PREC_*
+        self.inplace = bool(inplace)
+        if inplace:
+            precision |= STREAM_INPLACE                                                  # include/lbm.h LBM_STREAM_INPLACE
         F = np.atleast_1d(np.asarray(F, dtype=np.float64))
         if F.size == 1:
             F = np.array([F[0], 0.0, 0.0])
@@ -448,10 +452,10 @@ def lattice():
     return c, opp
 
 
-def from_workload(wl, fp64=False, want_mean=True, device="cuda:0", storage16=False, stream=None) -> Lbm:
+def from_workload(wl, fp64=False, want_mean=True, device="cuda:0", storage16=False, stream=None, inplace=False) -> Lbm:
     """Create a handle for a workloads.Workload and load its flags, inlet profile and initial field."""
     sim = Lbm(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces, fp64=fp64, want_mean=want_mean,
-              device=device, storage16=storage16, stream=stream)
+              device=device, storage16=storage16, stream=stream, inplace=inplace)
     sim.set_flags(wl.height)
     if wl.inlet_profile is not None:
         sim.set_inlet_profile(*wl.inlet_profile)

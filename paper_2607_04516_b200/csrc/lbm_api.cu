@@ -4,6 +4,7 @@
 #include "lbm_setup.cuh"
 #include "lbm_step.cuh"
 #include "lbm_step_vec.cuh"
+#include "lbm_inplace.cuh"
 #include "lbm_thermal.cuh"
 #include "lbm_out.cuh"
 #include "lbm_mesh.cuh"
@@ -38,7 +39,7 @@ inline size_t real_bytes(int precision) { return precision == LBM_PREC_F64 ? 8 :
 inline size_t store_bytes(int precision) { return precision == LBM_PREC_F64 ? 8 : (precision == LBM_PREC_F32_S16 ? 2 : 4); }
 inline int xoff_of(int precision) { return precision == LBM_PREC_F32_S16 ? 16 : 8; }
 
-Layout make_layout(int nx, int ny, int nz, int want_mean, int precision)
+Layout make_layout(int nx, int ny, int nz, int want_mean, int precision, int inplace = 0)
 {
     Layout L{};
     const size_t rs = real_bytes(precision), ss = store_bytes(precision);
@@ -49,6 +50,7 @@ Layout make_layout(int nx, int ny, int nz, int want_mean, int precision)
     size_t o = 0;
     L.off_A = o; o += align_up((size_t)Q * L.stride * ss, ALIGN);
     L.off_B = o; o += align_up((size_t)Q * L.stride * ss, ALIGN);
+    if (inplace) { o = L.off_B; L.off_B = L.off_A; } // in-place streaming (lbm_inplace.cuh): one buffer serves as both
     L.off_flags = o; o += align_up((size_t)L.Np, ALIGN);
     L.off_links = o; o += align_up((size_t)L.Np * sizeof(uint32_t), ALIGN);
     // outflow-velocity side buffer (a6): 2 halves x 3 components x one slot per face-plane cell of all six faces (upper bound)
@@ -83,7 +85,8 @@ struct lbm {
     double nu0, Cs, fv[3], F[3]; // fv = Coriolis vector f = 2 Omega; lbm_create's scalar f_cor is fv[2]
     int face[6];
     int fp64, s16, want_mean; // fp64: FP64 arithmetic and storage; s16: FP32 arithmetic, binary16 population storage
-    int precision;            // LBM_PREC_*
+    int precision;            // LBM_PREC_* (without the streaming bit)
+    int inplace;              // LBM_STREAM_INPLACE: one population buffer, cur = parity of the next step (lbm_inplace.cuh)
     int device;               // the CUDA device the handle was created on; every ABI call runs there (DevGuard)
     Layout L;
     char *ws;       // device workspace
@@ -204,6 +207,7 @@ Params<real> make_params(const lbm_t *h)
         P.thd = h->thd;
         for (int k = 0; k < 6; ++k) P.thw[k] = (real)(2.0 * (h->thw[k] - h->theta_ref));
     }
+    P.ipq = h->inplace ? h->cur : -1;
     return P;
 }
 
@@ -354,7 +358,7 @@ int do_set_flags(lbm_t *h, const int32_t *height, const uint8_t *dev_mask = null
     if (rc) return rc;
     const size_t rs = sizeof(real);
     CUDA_TRY(h, cudaMemsetAsync(h->bufA(), 0, h->pop_bytes(), h->stream));
-    CUDA_TRY(h, cudaMemsetAsync(h->bufB(), 0, h->pop_bytes(), h->stream));
+    if (!h->inplace) CUDA_TRY(h, cudaMemsetAsync(h->bufB(), 0, h->pop_bytes(), h->stream));
     if (h->want_mean) CUDA_TRY(h, cudaMemsetAsync(h->mean(), 0, (size_t)3 * h->L.stride * rs, h->stream));
     CUDA_TRY(h, cudaMemsetAsync(h->fu(), 0, h->L.fu_bytes, h->stream));
     if (h->thermal) CUDA_TRY(h, cudaMemsetAsync(h->ft(), 0, h->ft_bytes(), h->stream)); // theta_b back to theta_ref; the thermal state is stale until lbm_set_theta
@@ -486,7 +490,7 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
         rc = check_launch(h, "init_kernel");
     }
     release_in(h, in, 4);
-    if (!rc) { h->step = 0; h->cur = 0; }
+    if (!rc) { h->step = 0; if (!h->inplace) h->cur = 0; } // in-place streaming: written in the layout of the current parity
     if (!rc && h->nmodes > 0) rc = turb_publish<real, S>(h, true); // the step counter restarts: the inflow cells carry u'(x, 0)
     return rc;
 }
@@ -575,9 +579,45 @@ constexpr int N_VARIANTS = 4;
 #ifndef VEC2_MINB
 #define VEC2_MINB 6
 #endif
+// in-place streaming (lbm_inplace.cuh): one launch shape, one cell per thread; cur = parity of this step
+template <typename real, typename S, int MINB, bool DAMP, bool PERX>
+int launch_ip_step_as(lbm_t *h, const Params<real> &P, bool sample)
+{
+    constexpr int BLOCK = 128;
+    dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
+    const IpPtrs<S> T = make_ip_ptrs<S>((S *)h->bufA(), h->cur, P);
+    const real *fur = (const real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
+    real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
+    real *ms = (real *)h->mean();
+    cudaLaunchConfig_t cfg{}; // programmatic dependent launch, as for the two-buffer step (launch_step_as)
+    cfg.gridDim = grid; cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = h->stream;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    const uint8_t *fl = h->flags();
+    const uint32_t *lk = h->links();
+    constexpr int MINB_S = MINB == 10 ? 9 : MINB; // sampling steps hold three more values per thread
+    if (sample) cudaLaunchKernelEx(&cfg, ip_step_kernel<real, S, true, BLOCK, MINB_S, DAMP, PERX>, fl, lk, ms, fur, fuw, P, T);
+    else cudaLaunchKernelEx(&cfg, ip_step_kernel<real, S, false, BLOCK, MINB, DAMP, PERX>, fl, lk, ms, fur, fuw, P, T);
+    return check_launch(h, "ip_step_kernel");
+}
+#ifndef IP_MINB
+#define IP_MINB 10
+#endif
+template <typename real, typename S>
+int launch_ip_step(lbm_t *h, const Params<real> &P, bool sample)
+{
+    constexpr int M = std::is_same<real, float>::value ? IP_MINB : 4;
+    constexpr int M9 = std::is_same<real, float>::value ? (IP_MINB == 10 ? 9 : IP_MINB) : 4;
+    if (h->damp_on) return P.perx ? launch_ip_step_as<real, S, M9, true, true>(h, P, sample) : launch_ip_step_as<real, S, M9, true, false>(h, P, sample);
+    return P.perx ? launch_ip_step_as<real, S, M9, false, true>(h, P, sample) : launch_ip_step_as<real, S, M, false, false>(h, P, sample);
+}
+
 template <typename real, typename S>
 int launch_step(lbm_t *h, const Params<real> &P, bool sample)
 {
+    if (h->inplace) return launch_ip_step<real, S>(h, P, sample);
     if (h->thermal) { // fused flow + thermal step (lbm_thermal.cuh); S = real there (lbm_set_thermal refuses 16-bit storage)
         const real *A = (const real *)h->state();
         real *B = (real *)h->other();
@@ -664,7 +704,7 @@ int try_step_loop(lbm_t *h, const Params<real> &P, int want)
 {
     if constexpr (!std::is_same<real, float>::value) return 0;
     else {
-        if (h->variant != 0 || h->nmodes > 0 || h->thermal || want < 4 || h->loop_ok < 0) return 0;
+        if (h->variant != 0 || h->nmodes > 0 || h->thermal || h->inplace || want < 4 || h->loop_ok < 0) return 0;
         constexpr int BLOCK = 128;
         const dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
         const void *fn = P.perx ? (h->damp_on ? (const void *)step_loop_kernel<float, S, BLOCK, 8, true, true> : (const void *)step_loop_kernel<float, S, BLOCK, 8, false, true>)
@@ -735,7 +775,7 @@ int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
         const int B = 256;
         macros_kernel<real, S, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
             (const S *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
-            (const real *)h->th_state());
+            (const real *)h->th_state(), h->links());
         rc = check_launch(h, "macros_kernel");
     }
     int rc2 = finish_out(h, o, staged);
@@ -786,7 +826,7 @@ int do_get_state(lbm_t *h, double *f)
     int rc = stage_out(h, f, (size_t)Q * P.N * sizeof(double), &o);
     if (rc) return rc;
     const int B = 256;
-    state_out_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), h->flags(), (double *)o.dev, P);
+    state_out_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), h->flags(), h->links(), (double *)o.dev, P);
     rc = check_launch(h, "state_out_kernel");
     int rc2 = finish_out(h, &o, 1);
     return rc ? rc : rc2;
@@ -804,7 +844,7 @@ int do_set_state(lbm_t *h, const double *f)
                                                                     (const double *)in.dev, P);
     rc = check_launch(h, "state_in_kernel");
     release_in(h, &in, 1);
-    if (!rc) h->cur = 0;
+    if (!rc && !h->inplace) h->cur = 0;
     return rc;
 }
 
@@ -842,7 +882,7 @@ int do_refeed(lbm_t *h)
     const Params<real> P = make_params<real>(h);
     if (P.F == 0) return LBM_OK;
     const int B = 256;
-    refeed_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), (real *)h->fu(), h->flags(), P);
+    refeed_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), (real *)h->fu(), h->flags(), h->links(), P);
     return check_launch(h, "refeed_kernel");
 }
 
@@ -861,7 +901,7 @@ int do_feed(lbm_t *dst, const lbm_t *src, int sx)
         if (e != cudaSuccess) { cudaEventDestroy(ev); return fail(dst, LBM_ECUDA, std::string("feed_inlet: ") + cudaGetErrorString(e)); }
     }
     feed_kernel<real, S><<<blocks_for((long long)D.ny * D.nz, B), B, 0, dst->stream>>>(
-        (S *)dst->bufA(), (S *)dst->bufB(), (real *)dst->fu(), dst->flags(), D, (const S *)src->state(), src->flags(), Ps, sx);
+        (S *)dst->bufA(), (S *)dst->bufB(), (real *)dst->fu(), dst->flags(), D, (const S *)src->state(), src->flags(), src->links(), Ps, sx);
     int rc = check_launch(dst, "feed_kernel");
     if (cross) {
         // ... and what src does next after the read: its step after next rewrites the buffer this plane lies in, and src's
@@ -1006,6 +1046,7 @@ int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
     if (!(alpha > 0.0) || !std::isfinite(alpha) || !std::isfinite(g_beta) || !std::isfinite(theta_ref))
         return fail(h, LBM_EINVAL, "set_thermal: alpha must be > 0 and all arguments finite");
     if (h->s16) return fail(h, LBM_EINVAL, "set_thermal: not combinable with 16-bit population storage");
+    if (h->inplace) return fail(h, LBM_EINVAL, "set_thermal: not combinable with in-place streaming");
     if (h->damp_on || h->nmodes > 0) return fail(h, LBM_EINVAL, "set_thermal: not combinable with damping zones / inflow fluctuations");
     if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half() + h->ft_bytes()));
     CUDA_TRY(h, cudaMemsetAsync(h->th_ws, 0, 2 * h->th_half() + h->ft_bytes(), h->stream)); // theta_ref at rest (shifted storage), theta_b = theta_ref
@@ -1058,8 +1099,10 @@ int lbm_get_theta_f64(lbm_t *h, double *theta) { return get_theta_any<double>(h,
 int lbm_workspace_bytes(int nx, int ny, int nz, int want_mean, int precision, size_t *out)
 {
     if (!out || !size_ok(nx, ny, nz)) return LBM_EINVAL;
+    const int inplace = (precision >= 0 && (precision & LBM_STREAM_INPLACE)) ? 1 : 0;
+    if (precision >= 0) precision &= ~LBM_STREAM_INPLACE;
     if (precision != LBM_PREC_F32 && precision != LBM_PREC_F64 && precision != LBM_PREC_F32_S16) return LBM_EINVAL;
-    *out = make_layout(nx, ny, nz, want_mean, precision).total;
+    *out = make_layout(nx, ny, nz, want_mean, precision, inplace).total;
     return LBM_OK;
 }
 
@@ -1069,6 +1112,8 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     if (!out) return LBM_EINVAL;
     *out = nullptr;
     if (!size_ok(nx, ny, nz)) return LBM_EINVAL;
+    const int inplace = (precision >= 0 && (precision & LBM_STREAM_INPLACE)) ? 1 : 0;
+    if (precision >= 0) precision &= ~LBM_STREAM_INPLACE;
     if (precision != LBM_PREC_F32 && precision != LBM_PREC_F64 && precision != LBM_PREC_F32_S16) return LBM_EINVAL;
     if (!(nu0 > 0.0) || Cs < 0.0 || !std::isfinite(nu0) || !std::isfinite(Cs) || !std::isfinite(f_cor)) return LBM_EINVAL;
     int ndev = 0;
@@ -1082,7 +1127,8 @@ int lbm_create_ex(int nx, int ny, int nz, double nu0, double Cs, double f_cor, c
     for (int k = 0; k < 6; ++k) h->face[k] = def[k];
     h->precision = precision; h->fp64 = precision == LBM_PREC_F64; h->s16 = precision == LBM_PREC_F32_S16;
     h->want_mean = want_mean ? 1 : 0;
-    h->L = make_layout(nx, ny, nz, h->want_mean, precision);
+    h->inplace = inplace;
+    h->L = make_layout(nx, ny, nz, h->want_mean, precision, inplace);
     h->stream = (cudaStream_t)cuda_stream;
     if (cudaGetDevice(&h->device) != cudaSuccess) { cudaGetLastError(); delete h; return LBM_ECUDA; }
     h->cur = 0; h->have_flags = false; h->step = 0;
@@ -1220,6 +1266,7 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
     DevGuard dg_(h);
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inflow_turbulence: flags not set");
     if (n_modes < 0 || n_modes > MAX_MODES) return fail(h, LBM_EINVAL, "set_inflow_turbulence: n_modes out of range");
+    if (h->inplace && n_modes > 0) return fail(h, LBM_EINVAL, "set_inflow_turbulence: not combinable with in-place streaming");
     auto rewrite = [&]() { return DISPATCH(h, turb_publish, h, true); };
     if (n_modes == 0) {
         if (h->nmodes == 0) return LBM_OK;

@@ -90,6 +90,9 @@ struct Params {
     // is held, thw[k] = 2 (theta_w - theta_ref) of that face (the anti-bounce-back mailbox value is -t_j + wT_j thw[k])
     int thd;
     real thw[6];
+    // in-place streaming (lbm_create_ex precision | LBM_STREAM_INPLACE): -1 = two buffers (A/B pull, everything
+    // above), else the handle has ONE population buffer and ipq = parity of the step that reads the current state next
+    int ipq;
 };
 
 // Interior x = 0 sits at padded x = P.xoff (8 cells of 4 or 8 bytes, 16 cells of 2): every interior row starts on a
@@ -407,6 +410,83 @@ __device__ __forceinline__ void store_cell(S *__restrict__ B, const Params<real>
         if (fl & SLOW_BIT) wall_stores(P, p, x, lk, st);
         if (fl & EDGE_BIT) ghost_stores(P, x, y, z, lk, st);
     }
+}
+
+// ---- in-place streaming: one population buffer --------------------------------------------------------------
+// Every link between a cell y and its neighbour y - c_k (pair k = 1..9) owns the two slots 2k-1 and 2k of cell y.  In a state of
+// parity q a cell x' finds its incoming population of direction i
+//     i odd  (= +c_k):  in slot ip_slot(q, i) of x' itself          (the neighbour x' - c_k pushed it there),
+//     i even (= -c_k):  in slot ip_slot(q, i) of x' + c_k            (the neighbour x' + c_k kept it at home),
+// with ip_slot(0, i) = i and ip_slot(1, i) = opp(i).  A step of parity q reads these 19 addresses and writes its outgoing
+// population j to the address it read opp(j) from — which is exactly where x' = x + c_j looks for direction j in parity q ^ 1.
+// Nobody else touches those two addresses during the step, so one buffer is enough.  The write-side boundary rule carries
+// over unchanged: a population that cannot go to x + c_j (wall link, ghost slot) is put where its receiving cell x' will look
+// for its receiving direction i next step; that slot belongs to a link whose other end is SOLID / GHOST (a cell that never
+// runs), so nobody reads it during this step either.  The slot of the link that the dead end would have used stays unused, and
+// a live cell may store its outgoing population towards a dead cell there unconditionally (never read).
+__host__ __device__ constexpr int ip_slot(int q, int i) { return q ? dir_opp(i) : i; }
+
+// element index (slot * stride + cell) at which cell p (interior x coordinate x) reads its incoming direction I in parity q
+template <int I, typename real>
+__device__ __forceinline__ long long ip_read_at(const Params<real> &P, int q, int p, int x)
+{
+    if constexpr (I == 0 || (I & 1)) return (long long)ip_slot(q, I) * P.stride + p;
+    else return (long long)ip_slot(q, I) * P.stride + (p - poff<I>(P) + xwrap<I>(P, x));
+}
+// cell offset of direction i, i known only at run time (ghost slots: the reflected direction)
+template <typename real>
+__device__ __forceinline__ int poff_rt(const Params<real> &P, int i)
+{
+    return dir_cx(i) + dir_cy(i) * P.px + dir_cz(i) * P.pxy;
+}
+// Visit the addresses that hold the post-collision state of cell p = (x,y,z) in a state of parity q: f(jc, e) is called with
+// direction j (integral_constant) and element index e, first with the plain destination of every direction, then once more
+// for every redirected direction (wall links, ghost slots) — a later call overrides an earlier one.  A store visitor writes
+// g[j] to every address it is shown (the plain destination of a redirected direction is an unused slot); a load visitor
+// reads g[j] from the last one.
+template <typename real, class F>
+__device__ __forceinline__ void ip_visit(const Params<real> &P, int q, int p, int x, int y, int z, uint8_t fl, uint32_t lk, F &&f)
+{
+    f(std::integral_constant<int, 0>{}, (long long)p);
+    static_for<1, Q>([&](auto jc) {
+        constexpr int j = decltype(jc)::value;
+        // arrives at x + c_j with direction j: odd j is kept by the receiving cell itself, even j stays at home (= x)
+        if constexpr (j & 1) {
+            const int wrap = (dir_cx(j) == 1 && P.perx && x == P.nx - 1) ? -P.nx : 0;
+            f(jc, (long long)ip_slot(q, j) * P.stride + (p + poff<j>(P) + wrap));
+        } else f(jc, (long long)ip_slot(q, j) * P.stride + p);
+    });
+    if (fl & SLOW_BIT) {
+        // wall link i: population opp(i) comes back to this cell as direction i
+        static_for<1, Q>([&](auto ic) {
+            constexpr int i = decltype(ic)::value;
+            if ((lk >> i) & 1u) f(std::integral_constant<int, dir_opp(i)>{}, ip_read_at<i>(P, q, p, x));
+        });
+    }
+    if (fl & EDGE_BIT) {
+        // ghost slot (i, pt) of the two-buffer scheme = "the cell pt + c_i receives direction i"
+        ghost_stores(P, x, y, z, lk, [&](int i, int pt, auto jc) {
+            int cell = pt;
+            if (i & 1) cell = pt + poff_rt(P, i) + ((dir_cx(i) == 1 && P.perx && x == P.nx - 1) ? -P.nx : 0);
+            f(jc, (long long)ip_slot(q, i) * P.stride + cell);
+        });
+    }
+}
+
+// the stored (post-collision) state of a cell, whichever streaming scheme the handle uses; A = the current buffer
+template <typename real, typename S>
+__device__ __forceinline__ void load_cell_any(real (&g)[Q], const S *__restrict__ A, const Params<real> &P, int p, int x, int y, int z,
+                                              uint8_t fl, uint32_t lk)
+{
+    if (P.ipq < 0) { load_cell(g, A, P.stride, p); return; }
+    ip_visit(P, P.ipq, p, x, y, z, fl, lk, [&](auto jc, long long e) { g[decltype(jc)::value] = ld_s<real>(A + e); });
+}
+template <typename real, typename S>
+__device__ __forceinline__ void store_cell_any(S *__restrict__ A, const Params<real> &P, int p, int x, int y, int z, uint8_t fl,
+                                               uint32_t lk, const real (&g)[Q])
+{
+    if (P.ipq < 0) { store_cell(A, P, p, x, y, z, fl, lk, g); return; }
+    ip_visit(P, P.ipq, p, x, y, z, fl, lk, [&](auto jc, long long e) { st_s(A + e, g[decltype(jc)::value]); });
 }
 
 // ---- a3 / a6: EQ face cells -------------------------------------------------------------------------------------------

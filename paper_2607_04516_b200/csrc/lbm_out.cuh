@@ -16,18 +16,20 @@ __device__ __forceinline__ real stored_theta_shift(const real *__restrict__ H, l
 template <typename real, typename S, typename out_t>
 __global__ void macros_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
                               out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz, Params<real> P,
-                              const real *__restrict__ H = nullptr)
+                              const real *__restrict__ H = nullptr, const uint32_t *__restrict__ links = nullptr)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
     int x, y, z;
     cell_xyz(P, c, x, y, z);
     const int p = pidx(P, x, y, z);
-    const int cls = flags[p] & CLASS_MASK;
+    const uint8_t fl = flags[p];
+    const int cls = fl & CLASS_MASK;
     real g[Q];
     Macro<real> m{real(1), real(0), real(0), real(0)};
     if (cls != SOLID) {
-        load_cell(g, A, P.stride, p);
+        if (P.ipq < 0) load_cell(g, A, P.stride, p);
+        else load_cell_any(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? links[p] : 0u); // in-place streaming: the state lies at its destinations
         if (H) P.Fz += P.gbeta * stored_theta_shift(H, P.stride, p); // Boussinesq: the buoyancy the cell's collision used
         m = local_macros(g, cls, P, damp_at(P, x, y, z));
     }

@@ -230,8 +230,8 @@ template <typename real, typename S>
 __device__ __forceinline__ void store_cell_both(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const Params<real> &P,
                                                 int p, int x, int y, int z, uint8_t fl, uint32_t lk, const real (&g)[Q])
 {
-    store_cell(A, P, p, x, y, z, fl, lk, g);
-    if (B) store_cell(B, P, p, x, y, z, fl, lk, g); // B == nullptr: whole-lattice writes (init, checkpoint) fill the current buffer only
+    store_cell_any(A, P, p, x, y, z, fl, lk, g);
+    if (B && P.ipq < 0) store_cell(B, P, p, x, y, z, fl, lk, g); // B == nullptr: whole-lattice writes (init, checkpoint) fill the current buffer only; in-place streaming: there is one buffer
     const int cls = fl & CLASS_MASK;
     if ((fl & FEED_BIT) || cls == EQ_FIXED) {
         const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
@@ -373,7 +373,8 @@ __global__ void fluct_kernel(S *__restrict__ A, S *__restrict__ B, real *__restr
 // array).  Needed when something that enters the local macro inversion changes between steps (lbm_set_damping): the
 // rule is u_loc(G_k, c - n) evaluated with the parameters in force when the step runs (DESIGN.md §3 step 6).
 template <typename real, typename S>
-__global__ void refeed_kernel(const S *__restrict__ A, real *__restrict__ fu, const uint8_t *__restrict__ flags, Params<real> P)
+__global__ void refeed_kernel(const S *__restrict__ A, real *__restrict__ fu, const uint8_t *__restrict__ flags,
+                              const uint32_t *__restrict__ links, Params<real> P)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -383,7 +384,7 @@ __global__ void refeed_kernel(const S *__restrict__ A, real *__restrict__ fu, co
     const uint8_t fl = flags[p];
     if (!(fl & FEED_BIT)) return;
     real g[Q];
-    load_cell(g, A, P.stride, p);
+    load_cell_any(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? links[p] : 0u);
     const Macro<real> m = local_macros(g, fl & CLASS_MASK, P, damp_at(P, x, y, z));
     outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int s, int comp, real v) {
         fu[comp * P.F + s] = v;
@@ -395,7 +396,8 @@ __global__ void refeed_kernel(const S *__restrict__ A, real *__restrict__ fu, co
 template <typename real, typename S>
 __global__ void feed_kernel(S *__restrict__ dA, S *__restrict__ dB, real *__restrict__ dfu, const uint8_t *__restrict__ dflags,
                             Params<real> D,
-                            const S *__restrict__ sA, const uint8_t *__restrict__ sflags, Params<real> Ps, int sx)
+                            const S *__restrict__ sA, const uint8_t *__restrict__ sflags, const uint32_t *__restrict__ slinks,
+                            Params<real> Ps, int sx)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= D.ny * D.nz) return;
@@ -405,8 +407,9 @@ __global__ void feed_kernel(S *__restrict__ dA, S *__restrict__ dB, real *__rest
     if ((fl & CLASS_MASK) != EQ_FIXED) return;
     const int sp = pidx(Ps, sx, y % Ps.ny, z);
     real g[Q];
-    load_cell(g, sA, Ps.stride, sp);
-    const Macro<real> m = local_macros(g, sflags[sp] & CLASS_MASK, Ps, damp_at(Ps, sx, y % Ps.ny, z));
+    const uint8_t sfl = sflags[sp];
+    load_cell_any(g, sA, Ps, sp, sx, y % Ps.ny, z, sfl, (sfl & SLOW_BIT) ? slinks[sp] : 0u);
+    const Macro<real> m = local_macros(g, sfl & CLASS_MASK, Ps, damp_at(Ps, sx, y % Ps.ny, z));
     equilibrium(g, real(0), m.ux, m.uy, m.uz);
     store_cell_both(dA, dB, dfu, D, dp, 0, y, z, fl, 0u, g);
     publish_fixed(dfu, D, 0, y, z, m.ux, m.uy, m.uz);
@@ -437,16 +440,20 @@ __global__ void init_kernel(S *__restrict__ A, S *__restrict__ B, real *__restri
 // ---- checkpoint ------------------------------------------------------------------------------------------------------------
 // f [19][nz][ny][nx] double, NOT shifted.  SOLID cells export the rest state w_i (their slots are mailboxes).
 template <typename real, typename S>
-__global__ void state_out_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, double *__restrict__ f, Params<real> P)
+__global__ void state_out_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+                                 double *__restrict__ f, Params<real> P)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
     int x, y, z;
     cell_xyz(P, c, x, y, z);
     const int p = pidx(P, x, y, z);
-    const bool solid = (flags[p] & CLASS_MASK) == SOLID;
+    const uint8_t fl = flags[p];
+    const bool solid = (fl & CLASS_MASK) == SOLID;
+    real g[Q];
+    if (!solid) load_cell_any(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? links[p] : 0u);
 #pragma unroll
-    for (int i = 0; i < Q; ++i) f[(long long)i * P.N + c] = (solid ? 0.0 : double(ld_s<real>(A + ((long long)i * P.stride + p)))) + weight_f64(i);
+    for (int i = 0; i < Q; ++i) f[(long long)i * P.N + c] = (solid ? 0.0 : double(g[i])) + weight_f64(i);
 }
 
 template <typename real, typename S>

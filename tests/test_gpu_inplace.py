@@ -1,0 +1,304 @@
+"""In-place streaming (LBM_STREAM_INPLACE): one population buffer instead of two.
+
+It is a storage scheme, not a different method: the oracle is the same FP64 oracle, the bars are the same (flags and links
+bit-exact, max-abs(rho, u) <= 1e-5 after 100 steps in FP32, ~1e-12 in FP64), and the exported post-collision state must be
+the one the two-buffer path exports.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL32 = 1e-5    # north_star
+TOL64 = 2e-12   # rounding order only
+TOL16 = 2e-4    # 16-bit storage
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2607_04516_b200 import binding, build
+    build.build()
+    return binding
+
+
+def make_oracle(wl, storage16=False):
+    from oracle import Oracle
+    o = Oracle(wl.nx, wl.ny, wl.nz, wl.nu0, wl.Cs, wl.f_cor, wl.F, wl.faces)
+    if storage16:
+        o.set_storage16(True)
+    o.set_flags(wl.height)
+    if wl.inlet_profile is not None:
+        o.set_inlet_profile(*wl.inlet_profile)
+    if wl.init is not None:
+        o.set_macros(*wl.init)
+    else:
+        o.set_macros()
+    return o
+
+
+def max_err(sim, o, f64=False):
+    g = [a.cpu().numpy() for a in sim.get_macros(f64=f64)]
+    r = o.get_macros()
+    assert all(np.isfinite(a).all() for a in g)
+    return max(float(np.abs(a.astype(np.float64) - b).max()) for a, b in zip(g, r))
+
+
+FACE_SETS = [
+    (0, 0, 0, 0, 0, 0), (3, 4, 0, 0, 1, 2), (3, 4, 2, 2, 1, 2), (3, 4, 3, 3, 1, 2), (0, 0, 0, 0, 1, 2),
+    (1, 1, 1, 1, 1, 1), (2, 2, 2, 2, 2, 2), (2, 1, 0, 0, 2, 1), (4, 3, 1, 2, 0, 0), (3, 4, 2, 4, 1, 2),
+    (0, 0, 2, 2, 2, 2), (2, 2, 0, 0, 0, 0),
+]
+
+
+def _case(shape, seed):
+    nx, ny, nz = shape
+    rng = np.random.default_rng(seed)
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    for _ in range(6):
+        x0, y0 = int(rng.integers(0, max(nx - 6, 1))), int(rng.integers(0, max(ny - 3, 1)))
+        hm[y0:y0 + 3, x0:x0 + 4] = int(rng.integers(1, nz + 1))
+    prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+    ux0 = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+    uy0 = 0.01 * np.sin(2 * np.pi * (np.arange(nx)[None, None, :] + 0.5) / nx) * np.ones((nz, ny, 1))
+    return hm, prof, ux0, uy0
+
+
+@pytest.mark.parametrize("faces", FACE_SETS)
+@pytest.mark.parametrize("shape", [(37, 11, 9), (64, 12, 10), (8, 3, 3), (5, 1, 4), (1, 6, 5)])
+def test_every_face_rule_matches_the_oracle_in_fp64_and_fp32(B, faces, shape):
+    """Ragged boxes with buildings (also up to the lid), every face type on every axis, edges where two face rules meet,
+    rows shorter than a warp, boxes one cell thick; Coriolis, LES and a body force on; the time mean; an odd and an even
+    number of steps (both parities of the slot roles are read back)."""
+    from oracle import Oracle
+    nx, ny, nz = shape
+    hm, prof, ux0, uy0 = _case(shape, nx * 1000 + ny)
+    args = (nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 2e-7, 0), faces)
+    o = Oracle(*args)
+    o.set_flags(hm)
+    o.set_inlet_profile(prof, 0.1 * prof, None)
+    o.set_macros(None, ux0, uy0, None)
+    o.mean_config(10, 5)
+    sims = []
+    for fp64 in (True, False):
+        sim = B.Lbm(*args, fp64=fp64, inplace=True)
+        sim.set_flags(hm)
+        np.testing.assert_array_equal(sim.get_flags(), o.get_flags())
+        np.testing.assert_array_equal(sim.get_links(), o.get_links())
+        if fp64:
+            sim.set_inlet_profile(prof, 0.1 * prof, None, f64=True)
+            sim.set_macros(None, ux0, uy0, None, f64=True)
+        else:
+            sim.set_inlet_profile(prof.astype(np.float32), (0.1 * prof).astype(np.float32), None)
+            sim.set_macros(None, ux0.astype(np.float32), uy0.astype(np.float32), None)
+        sim.mean_config(10, 5)
+        sims.append(sim)
+    assert max_err(sims[0], o, f64=True) <= TOL64   # step 0: the initial state read back through the in-place layout
+    for upto in (1, 40, 41):
+        o.step(upto - o.get_step())
+        for sim, fp64 in zip(sims, (True, False)):
+            sim.step(upto - sim.get_step())
+            e = max_err(sim, o, f64=fp64)
+            assert e <= (TOL64 if fp64 else TOL32), (faces, shape, upto, fp64, e)
+    *om, on = o.get_mean()
+    for sim, fp64 in zip(sims, (True, False)):
+        *gm, n = sim.get_mean(f64=fp64) if fp64 else sim.get_mean()
+        assert n == on == 7
+        em = max(float(np.abs(a.cpu().numpy().astype(np.float64) - b).max()) for a, b in zip(gm, om))
+        assert em <= (TOL64 if fp64 else TOL32), (faces, shape, fp64, em)
+        sim.close()
+
+
+@pytest.mark.parametrize("fp64", [True, False])
+def test_exported_state_equals_the_two_buffer_path_and_round_trips(B, fp64):
+    """lbm_get_state returns the post-collision populations G_k(x, i) whatever the streaming scheme: population by
+    population equal to the two-buffer handle's (same collision code; FP64 to rounding order, FP32 to a few ulp of the
+    stored values), at an odd and at an even step; lbm_set_state is its inverse bit for bit, into either parity."""
+    shape = (37, 11, 9)
+    nx, ny, nz = shape
+    hm, prof, ux0, uy0 = _case(shape, 5)
+    for faces in [(3, 4, 0, 0, 1, 2), (0, 0, 2, 2, 1, 2), (2, 2, 0, 0, 0, 0)]:
+        args = (nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), faces)
+        pair = []
+        for inplace in (False, True):
+            sim = B.Lbm(*args, fp64=fp64, inplace=inplace)
+            sim.set_flags(hm)
+            sim.set_inlet_profile(prof, 0.1 * prof, None, f64=True)
+            sim.set_macros(None, ux0, uy0, None, f64=True)
+            pair.append(sim)
+        for upto in (0, 7, 20):
+            for sim in pair:
+                sim.step(upto - sim.get_step())
+            a, b = (sim.get_state(out="host") for sim in pair)
+            fluid = np.broadcast_to(pair[0].get_flags()[None] != 1, a.shape)
+            assert float(np.abs(a - b)[fluid].max()) <= (1e-14 if fp64 else 2e-7), (faces, upto)
+        st = pair[1].get_state(out="host")
+        for presteps in (0, 1):     # the receiving handle stands at parity 0 / 1
+            sim2 = B.Lbm(*args, fp64=fp64, inplace=True)
+            sim2.set_flags(hm)
+            sim2.set_inlet_profile(prof, 0.1 * prof, None, f64=True)
+            sim2.set_macros(f64=True)
+            sim2.step(presteps)
+            sim2.set_state(st)
+            sim2.set_step(20)
+            assert np.array_equal(sim2.get_state(out="host"), st)
+            sim2.step(13); pair[1].step(13)
+            # not bit for bit: lbm_set_state re-derives the inlet cells' boundary velocity from the populations it is given
+            # (moments of an equilibrium carry rounding noise), the running handle still holds the prescribed one
+            d = float(np.abs(sim2.get_state(out="host") - pair[1].get_state(out="host")).max())
+            assert d <= (1e-13 if fp64 else 1e-6), (faces, presteps, d)
+            pair[1].set_state(st); pair[1].set_step(20)
+            sim2.close()
+        for sim in pair:
+            sim.close()
+
+
+def test_config1_100_and_200_steps_all_three_precisions(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config1()
+    o, o16 = make_oracle(wl), make_oracle(wl, storage16=True)
+    s32 = B.from_workload(wl, inplace=True)
+    s64 = B.from_workload(wl, fp64=True, inplace=True)
+    s16 = B.from_workload(wl, storage16=True, inplace=True)
+    for upto in (100, 200):
+        for h in (o, o16, s32, s64, s16):
+            h.step(upto - h.get_step())
+        e32, e64, e16 = max_err(s32, o), max_err(s64, o, f64=True), max_err(s16, o16)
+        print(f"C1 in place, step {upto}: fp32 {e32:.3e} fp64 {e64:.3e} 16-bit storage {e16:.3e}")
+        assert e32 <= TOL32 and e64 <= TOL64
+        if upto == 100:     # the 16-bit mode's bar is stated for 100 steps; the two-buffer path measures the same
+            assert e16 <= TOL16
+
+
+def test_config2_periodic_box_wraps_both_sides_of_the_same_address(B):
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config2(Cs=0.1, n=48)
+    o = make_oracle(wl)
+    s32, s64 = B.from_workload(wl, inplace=True), B.from_workload(wl, fp64=True, inplace=True)
+    for h in (o, s32, s64):
+        h.step(101)
+    e32, e64 = max_err(s32, o), max_err(s64, o, f64=True)
+    print(f"C2 48^3 in place, step 101: fp32 {e32:.3e} fp64 {e64:.3e}")
+    assert e32 <= TOL32 and e64 <= TOL64
+    # mass is conserved to rounding on one buffer too
+    rho = s64.get_macros(f64=True)[0].cpu().numpy()
+    assert abs(rho.sum() - make_oracle(wl).get_macros()[0].sum()) <= 1e-9
+
+
+def test_config3_and_config4_crops_with_time_mean(B):
+    from paper_2607_04516_b200 import workloads as W
+    for wl in (W.config3(nx=150, ny=77, nz=50), W.config4(nx=120, ny=90, nz=60)):
+        o = make_oracle(wl)
+        sim = B.from_workload(wl, inplace=True)
+        o.mean_config(50, 10); sim.mean_config(50, 10)
+        o.step(100); sim.step(100)
+        e = max_err(sim, o)
+        *gm, n = sim.get_mean()
+        *om, on = o.get_mean()
+        em = max(float(np.abs(a.cpu().numpy() - b).max()) for a, b in zip(gm, om))
+        print(f"{wl.nx}x{wl.ny}x{wl.nz} in place, step 100: {e:.3e}, mean {em:.3e}")
+        assert n == on == 6 and e <= TOL32 and em <= TOL32
+
+
+def test_config3_full_100_steps_and_half_the_memory(B):
+    """The bench workload in the launch configuration bench.py --workload c3-inplace times, every cell against the oracle."""
+    from paper_2607_04516_b200 import workloads as W
+    wl = W.config3()
+    o = make_oracle(wl)
+    sim = B.from_workload(wl, want_mean=False, inplace=True)
+    two = B.Lbm(wl.nx, wl.ny, wl.nz, wl.nu0, want_mean=False)
+    pops = 19 * 4 * (wl.nx * wl.ny * wl.nz)
+    assert two.workspace_bytes - sim.workspace_bytes >= pops           # a whole population buffer less
+    assert sim.workspace_bytes <= 0.56 * two.workspace_bytes
+    two.close()
+    o.step(100)
+    sim.step(100)
+    e = max_err(sim, o)
+    print(f"C3 400x400x100 in place, step 100: max|gpu32 - oracle| = {e:.3e}; workspace {sim.workspace_bytes / 2**30:.2f} GiB")
+    assert e <= TOL32
+
+
+@pytest.mark.parametrize("main_inplace,pre_inplace", [(True, False), (True, True), (False, True)])
+def test_config5_chain_with_either_side_in_place(B, main_inplace, pre_inplace):
+    from paper_2607_04516_b200 import workloads as W
+    pre = W.config5_precursor(nx=32, ny=24, nz=40)
+    main = W.config5_main(nx=96, ny=60, nz=40)
+    xs = 16
+    op, om = make_oracle(pre), make_oracle(main)
+    gp, gm = B.from_workload(pre, inplace=pre_inplace), B.from_workload(main, inplace=main_inplace)
+    reps = -(-main.ny // pre.ny)
+    for _ in range(31):
+        _, ux, uy, uz = op.get_macros()
+        plane = np.stack([np.tile(q[:, :, xs], (1, reps))[:, :main.ny] for q in (ux, uy, uz)])
+        om.set_inlet_plane(0, plane)
+        gm.feed_inlet(gp, xs)
+        op.step(1); om.step(1)
+        gp.step(1); gm.step(1)
+    e_pre, e_main = max_err(gp, op), max_err(gm, om)
+    print(f"C5 chain step 31 (main in place {main_inplace}, precursor in place {pre_inplace}): {e_pre:.3e} / {e_main:.3e}")
+    assert e_pre <= TOL32 and e_main <= TOL32
+
+
+@pytest.mark.parametrize("fp64", [True, False])
+def test_flux_correction_and_damping_zones_in_place(B, fp64):
+    """The paper's open-boundary set-up: equilibrium faces all round, flux-balanced, top sponge and lateral
+    buffers; the boundary cells are rewritten between steps at both parities."""
+    from oracle import Oracle
+    nx, ny, nz = 40, 26, 16
+    hm, prof, ux0, uy0 = _case((nx, ny, nz), 11)
+    faces = (3, 4, 3, 3, 1, 3)
+    args = (nx, ny, nz, 1e-3, 0.1, 1e-4, (0, 0, 0), faces)
+    width, peak = [0, 6, 5, 5, 0, 6], [0.0, 0.05, 0.03, 0.03, 0.0, 0.1]
+    target = np.stack([prof, 0.1 * prof, np.zeros(nz)])
+    o = Oracle(*args)
+    sim = B.Lbm(*args, fp64=fp64, inplace=True)
+    for h in (o, sim):
+        h.set_flags(hm)
+    o.set_inlet_profile(prof, 0.1 * prof, 0.002 * np.ones(nz))
+    o.set_macros(None, ux0, uy0, None)
+    if fp64:
+        sim.set_inlet_profile(prof, 0.1 * prof, 0.002 * np.ones(nz), f64=True)
+        sim.set_macros(None, ux0, uy0, None, f64=True)
+    else:
+        sim.set_inlet_profile(prof.astype(np.float32), (0.1 * prof).astype(np.float32), np.full(nz, 0.002, dtype=np.float32))
+        sim.set_macros(None, ux0.astype(np.float32), uy0.astype(np.float32), None)
+    tol = TOL64 if fp64 else TOL32
+    o.step(3); sim.step(3)                 # parity 1
+    fo, fg = o.balance_flux(), sim.balance_flux()
+    assert fg[0] == pytest.approx(fo[0], rel=1e-12 if fp64 else 1e-5, abs=1e-9 if fp64 else 1e-6)
+    assert abs(fo[1]) < 1e-12 and abs(fg[1]) < (1e-12 if fp64 else 2e-5)
+    o.set_damping(width, peak, target); sim.set_damping(width, peak, target)
+    o.step(50); sim.step(50)
+    assert max_err(sim, o, f64=fp64) <= tol
+    o.set_damping([0] * 6, [0.0] * 6, None); sim.set_damping([0] * 6, [0.0] * 6, None)
+    o.step(20); sim.step(20)
+    assert max_err(sim, o, f64=fp64) <= tol
+
+
+def test_rest_state_is_exact_and_refused_combinations_say_so(B):
+    hm = np.zeros((12, 16), dtype=np.int32)
+    hm[3:6, 4:8] = 5
+    _, w, _ = __import__("oracle").lattice()
+    for faces in [(3, 4, 0, 0, 1, 2), (2, 2, 1, 1, 0, 0), (0,) * 6]:
+        sim = B.Lbm(16, 12, 8, 1e-3, 0.1, 0.0, (0, 0, 0), faces, inplace=True)
+        sim.set_flags(hm)
+        sim.set_inlet_profile(np.zeros(8, dtype=np.float32))
+        sim.set_macros()
+        sim.step(51)
+        st = sim.get_state(out="host")
+        assert np.array_equal(st, np.broadcast_to(w[:, None, None, None], st.shape))
+        sim.close()
+    sim = B.Lbm(16, 12, 8, 1e-3, 0.1, 0.0, (0, 0, 0), (3, 4, 0, 0, 1, 2), inplace=True)
+    sim.set_flags(hm)
+    with pytest.raises(B.LbmError, match="in-place"):
+        sim.set_thermal(0.01, 1e-4, 0.0)
+    from paper_2607_04516_b200 import workloads as W
+    with pytest.raises(B.LbmError, match="in-place"):
+        sim.set_inflow_turbulence(W.inflow_modes(4, 1, 0.1, 1.0, (0.05, 0, 0)), 0.01, 0.3, 0.0)
+    sim.set_variant(3)          # accepted, no effect: one launch shape
+    sim.set_inlet_profile(np.full(8, 0.03, dtype=np.float32))
+    sim.set_macros()
+    sim.step(4)
+    assert np.isfinite(sim.get_macros()[1].cpu().numpy()).all()
