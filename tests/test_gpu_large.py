@@ -85,12 +85,14 @@ def boxes_for(wl):
     ]
 
 
-@pytest.mark.parametrize("cfg", ["config3", "config4", "config5_main"])
-def test_full_size_lattice_matches_the_oracle_on_sampled_boxes(B, cfg):
+@pytest.mark.parametrize("cfg,inplace", [("config3", False), ("config4", False), ("config5_main", False), ("config5_main", True)])
+def test_full_size_lattice_matches_the_oracle_on_sampled_boxes(B, cfg, inplace):
+    """inplace: the same lattice on one population buffer (LBM_STREAM_INPLACE) — lbm_get_state gathers the
+    populations from their destinations."""
     import torch
     from paper_2607_04516_b200 import workloads as W
     wl = getattr(W, cfg)()
-    sim = B.from_workload(wl, want_mean=False)
+    sim = B.from_workload(wl, want_mean=False, inplace=inplace)
     K, T = 40, 10
     worst = 0.0
     for i, box in enumerate(boxes_for(wl)):
@@ -102,7 +104,79 @@ def test_full_size_lattice_matches_the_oracle_on_sampled_boxes(B, cfg):
     sim.close()
     del sim
     torch.cuda.empty_cache()
-    print(f"{cfg}: worst sampled-box error {worst:.3e}")
+    print(f"{cfg}{' in place' if inplace else ''}: worst sampled-box error {worst:.3e}")
+
+
+def test_a_lattice_too_large_for_two_buffers_runs_in_place(B):
+    """2000 x 2000 x 300 = 1.2e9 FP32 cells — the paper's 5 m, 10 km x 10 km x 1.5 km box (PAPER.md:181-185 scales) — needs
+    191 GB with two population buffers, more than one B200 has, and 99 GB in place.  lbm_get_state of such a
+    lattice would itself be 182 GB, so the sampled boxes are compared from the INITIAL condition: the oracle advances a box
+    plus a halo of T + 1 cells from the same f_eq(1, u0) for T steps; information travels one cell per step, so the box
+    interior is exact whatever happens on the artificial faces.  Bar 1e-5 (north_star)."""
+    import torch
+    from oracle import Oracle
+    from paper_2607_04516_b200 import workloads as W
+    nx, ny, nz = 2000, 2000, 300
+    c3 = W.config3()
+    height = np.ascontiguousarray(np.tile(c3.height, (5, 5)))
+    prof = W.log_law_profile(nz, 0.08, 20.0, 0.2)
+    faces = c3.faces
+    free, total = torch.cuda.mem_get_info()
+    import ctypes as C
+    lib = B.load_library()
+    nb2, nb1 = C.c_size_t(), C.c_size_t()
+    assert lib.lbm_workspace_bytes(nx, ny, nz, 0, B.PREC_F32, C.byref(nb2)) == 0
+    assert lib.lbm_workspace_bytes(nx, ny, nz, 0, B.PREC_F32 | B.STREAM_INPLACE, C.byref(nb1)) == 0
+    print(f"two buffers {nb2.value / 1e9:.1f} GB, in place {nb1.value / 1e9:.1f} GB, device {total / 1e9:.1f} GB")
+    assert nb2.value > total, "the point of this test is a lattice that cannot be double-buffered on this device"
+    if nb1.value + 6e9 > free:
+        pytest.skip("not enough free device memory for the in-place lattice")
+    sim = B.Lbm(nx, ny, nz, c3.nu0, c3.Cs, c3.f_cor, c3.F, faces, want_mean=False, inplace=True)
+    sim.set_flags(height)
+    sim.set_inlet_profile(prof.astype(np.float32))
+    ux0 = torch.from_numpy(prof.astype(np.float32)).cuda()[:, None, None].expand(nz, ny, nx).contiguous()
+    sim.set_macros(None, ux0, None, None)
+    del ux0
+    torch.cuda.empty_cache()
+    T, s = 10, 32
+    H = T + 1
+    sim.step(T)
+    g = sim.get_macros()
+    worst = 0.0
+    n = (nx, ny, nz)
+    boxes = [(nx // 2, nx // 2 + s, ny // 2, ny // 2 + s, 0, s), (nx - s, nx, ny // 3, ny // 3 + s, 0, s), (0, s, 0, s, 0, s),
+             (1200, 1200 + s, ny - s, ny, 0, 24), (700, 716, 1500, 1516, 0, nz)]
+    for box in boxes:
+        lo = [max(box[2 * a] - H, 0) for a in range(3)]
+        hi = [min(box[2 * a + 1] + H, n[a]) for a in range(3)]
+        fb = []
+        for a in range(3):
+            for side in (0, 1):
+                real = (lo[a] == 0) if side == 0 else (hi[a] == n[a])
+                fb.append(faces[2 * a + side] if real else WALL)
+        o = Oracle(hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], c3.nu0, c3.Cs, c3.f_cor, c3.F, tuple(fb))
+        o.set_flags(np.ascontiguousarray(height[lo[1]:hi[1], lo[0]:hi[0]]))
+        o.set_inlet_profile(prof[lo[2]:hi[2]])
+        o.set_macros(None, np.broadcast_to(prof[lo[2]:hi[2], None, None], (hi[2] - lo[2], hi[1] - lo[1], hi[0] - lo[0])).copy(), None, None)
+        o.step(T)
+        r = o.get_macros()
+        sl = tuple(slice(box[2 * a] - lo[a], box[2 * a + 1] - lo[a]) for a in (2, 1, 0))
+        gl = (slice(box[4], box[5]), slice(box[2], box[3]), slice(box[0], box[1]))
+        for ga, ra in zip(g, r):
+            d = np.abs(ga[gl].cpu().numpy().astype(np.float64) - ra[sl])
+            assert np.isfinite(d).all()
+            worst = max(worst, float(d.max()))
+        o.close()
+        assert worst <= TOL32, (box, worst)
+    # a timing of the same lattice, for the record (not a bench line): 50 more steps
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(); sim.step(50); e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 50
+    assert bool(torch.isfinite(sim.get_macros()[1]).all())
+    print(f"2000x2000x300 in place: worst sampled-box error {worst:.3e}; {ms:.1f} ms per step = {nx * ny * nz / ms / 1e3:.0f} MLUPS")
+    sim.close()
+    del sim, g
+    torch.cuda.empty_cache()
 
 
 def test_tall_box_through_the_free_slip_top_of_config4(B):
