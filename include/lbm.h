@@ -68,9 +68,9 @@ enum { LBM_PREC_F32 = 0, LBM_PREC_F64 = 1, LBM_PREC_F32_S16 = 2 };
  * step to step — so a lattice takes about half the memory (config 5's 2.9e8 cells: 24 GB instead of 46 GB; 1.2e9 FP32 cells fit
  * one B200), for the same 153 B per cell and step and the same arithmetic: every call works the same and returns the same
  * values (lbm_get_state / lbm_set_state exchange the same post-collision populations).  Combinable with all three precisions,
- * every face type, damping zones, flux correction, the time mean and lbm_feed_inlet (either side); NOT with the thermal lattice
- * and the synthetic inflow fluctuations (lbm_set_thermal / lbm_set_inflow_turbulence return LBM_EINVAL), and lbm_set_variant has
- * no effect (one launch shape: one cell per thread, one launch per step). */
+ * every face type, damping zones, flux correction, synthetic inflow fluctuations, the time mean and lbm_feed_inlet (either side);
+ * NOT with the thermal lattice (lbm_set_thermal returns LBM_EINVAL), and lbm_set_variant has no effect (one launch shape: one cell
+ * per thread, one launch per step). */
 #define LBM_STREAM_INPLACE 16
 
 /* Bytes of device workspace a handle of this size needs (two population buffers of 19 stored values per cell — one with

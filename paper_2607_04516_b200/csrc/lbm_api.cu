@@ -4,7 +4,7 @@
 #include "lbm_setup.cuh"
 #include "lbm_step.cuh"
 #include "lbm_step_vec.cuh"
-#include "lbm_inplace.cuh"
+#include "lbm_inplace_launch.h"
 #include "lbm_thermal.cuh"
 #include "lbm_out.cuh"
 #include "lbm_mesh.cuh"
@@ -579,39 +579,24 @@ constexpr int N_VARIANTS = 4;
 #ifndef VEC2_MINB
 #define VEC2_MINB 6
 #endif
-// in-place streaming (lbm_inplace.cuh): one launch shape, one cell per thread; cur = parity of this step
-template <typename real, typename S, int MINB, bool DAMP, bool PERX>
-int launch_ip_step_as(lbm_t *h, const Params<real> &P, bool sample)
-{
-    constexpr int BLOCK = 128;
-    dim3 grid(blocks_for((long long)P.nxy, BLOCK), (unsigned)P.nz);
-    const IpPtrs<S> T = make_ip_ptrs<S>((S *)h->bufA(), h->cur, P);
-    const real *fur = (const real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
-    real *fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
-    real *ms = (real *)h->mean();
-    cudaLaunchConfig_t cfg{}; // programmatic dependent launch, as for the two-buffer step (launch_step_as)
-    cfg.gridDim = grid; cfg.blockDim = dim3(BLOCK); cfg.dynamicSmemBytes = 0; cfg.stream = h->stream;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    const uint8_t *fl = h->flags();
-    const uint32_t *lk = h->links();
-    constexpr int MINB_S = MINB == 10 ? 9 : MINB; // sampling steps hold three more values per thread
-    if (sample) cudaLaunchKernelEx(&cfg, ip_step_kernel<real, S, true, BLOCK, MINB_S, DAMP, PERX>, fl, lk, ms, fur, fuw, P, T);
-    else cudaLaunchKernelEx(&cfg, ip_step_kernel<real, S, false, BLOCK, MINB, DAMP, PERX>, fl, lk, ms, fur, fuw, P, T);
-    return check_launch(h, "ip_step_kernel");
-}
-#ifndef IP_MINB
-#define IP_MINB 10
-#endif
+// in-place streaming (lbm_inplace.cuh; kernels and launch in lbm_inplace_launch.cu): one launch shape, one cell per thread;
+// cur = parity of this step
 template <typename real, typename S>
 int launch_ip_step(lbm_t *h, const Params<real> &P, bool sample)
 {
-    constexpr int M = std::is_same<real, float>::value ? IP_MINB : 4;
-    constexpr int M9 = std::is_same<real, float>::value ? (IP_MINB == 10 ? 9 : IP_MINB) : 4;
-    if (h->damp_on) return P.perx ? launch_ip_step_as<real, S, M9, true, true>(h, P, sample) : launch_ip_step_as<real, S, M9, true, false>(h, P, sample);
-    return P.perx ? launch_ip_step_as<real, S, M9, false, true>(h, P, sample) : launch_ip_step_as<real, S, M, false, false>(h, P, sample);
+    IpLaunch L{};
+    L.prec = h->fp64 ? 1 : (h->s16 ? 2 : 0);
+    L.sample = sample; L.damp = h->damp_on; L.turb = h->nmodes > 0 && P.F > 0;
+    L.parity = h->cur;
+    L.G = h->bufA(); L.flags = h->flags(); L.links = h->links(); L.msum = h->mean();
+    // the side buffer's halves follow the parity as they follow the buffers of the two-buffer scheme
+    L.fur = (const real *)h->fu() + (size_t)(h->cur ? 3 : 0) * P.F;
+    L.fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
+    L.params = &P;
+    L.fum = h->fum(); L.modes = h->modes(); L.nmodes = h->nmodes; L.t = (double)(h->step + 2);
+    L.stream = h->stream;
+    ip_launch(L);
+    return check_launch(h, "ip_step_kernel");
 }
 
 template <typename real, typename S>
@@ -1266,7 +1251,6 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
     DevGuard dg_(h);
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inflow_turbulence: flags not set");
     if (n_modes < 0 || n_modes > MAX_MODES) return fail(h, LBM_EINVAL, "set_inflow_turbulence: n_modes out of range");
-    if (h->inplace && n_modes > 0) return fail(h, LBM_EINVAL, "set_inflow_turbulence: not combinable with in-place streaming");
     auto rewrite = [&]() { return DISPATCH(h, turb_publish, h, true); };
     if (n_modes == 0) {
         if (h->nmodes == 0) return LBM_OK;

@@ -46,11 +46,49 @@ inline IpPtrs<S> make_ip_ptrs(S *G, int q, const Params<real> &P)
     return t;
 }
 
-template <typename real, typename S, bool MEAN, int BLOCK, bool DAMP, bool PERX>
-__device__ __forceinline__ void ip_step_body(const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links, real *__restrict__ msum,
-                                             const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> &P, const IpPtrs<S> &T)
+#ifndef IP_LD
+#define IP_LD 0
+#endif
+// the 19 loads of the in-place step: pinned ahead of the flag test like the two-buffer kernel's (ld_pinned)
+template <typename T>
+__device__ __forceinline__ auto ip_ld(const T *p)
 {
-    const int zb = blockIdx.y;
+#if IP_LD == 1
+    if constexpr (std::is_same<T, float>::value) {
+        float v;
+        asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p));
+        return v;
+    } else return ld_pinned(p);
+#elif IP_LD == 2
+    if constexpr (std::is_same<T, float>::value) {
+        float v;
+        asm volatile("ld.relaxed.gpu.global.f32 %0, [%1];" : "=f"(v) : "l"(p));
+        return v;
+    } else return ld_pinned(p);
+#else
+    return ld_pinned(p);
+#endif
+}
+
+// TURB: the launch carries the synthetic inflow fluctuations in extra leading block rows, exactly as the two-buffer kernel does
+// (lbm_step.cuh): one thread per face slot publishes the boundary velocity of the step after this one into the half of the side
+// array this launch writes.
+template <typename real, typename S, bool MEAN, int BLOCK, bool DAMP, bool PERX, bool TURB>
+__device__ __forceinline__ void ip_step_body(const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links, real *__restrict__ msum,
+                                             const real *__restrict__ fur, real *__restrict__ fuw, const Params<real> &P, const IpPtrs<S> &T,
+                                             const Turb<real> &tb, const int turb_planes)
+{
+    int zb = blockIdx.y;
+    if constexpr (TURB) {
+        if (zb < turb_planes) {
+            asm volatile("griddepcontrol.launch_dependents;");
+            asm volatile("griddepcontrol.wait;" ::: "memory"); // the half written here is the one the previous launch reads
+            const int s = (zb * (int)gridDim.x + (int)blockIdx.x) * BLOCK + (int)threadIdx.x;
+            if (s < P.F) fluct_slot<real, false, S>(s, nullptr, nullptr, nullptr, fuw, nullptr, flags, tb, P);
+            return;
+        }
+        zb -= turb_planes;
+    }
     const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x; // cell of the z plane, linear over interior (y, x)
     if (c2 >= (unsigned)P.nxy) return;
     const int y = P.nx_magic ? (int)__umulhi(c2, P.nx_magic) : (int)(c2 / (unsigned)P.nx);
@@ -75,7 +113,7 @@ __device__ __forceinline__ void ip_step_body(const uint8_t *__restrict__ flags, 
     Damp<real> dmp{real(0), real(0), real(0), real(0)};
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        g[i] = real(ld_pinned(T.rd[i] + at(ic)));
+        g[i] = real(ip_ld(T.rd[i] + at(ic)));
     });
     const bool onface = ((unsigned)(x - 1) >= (unsigned)(P.nx - 2)) | ((unsigned)(y - 1) >= (unsigned)(P.ny - 2)) |
                         ((unsigned)(z - 1) >= (unsigned)(P.nz - 2));
@@ -146,12 +184,12 @@ __device__ __forceinline__ void ip_step_body(const uint8_t *__restrict__ flags, 
     finish(m);
 }
 
-template <typename real, typename S, bool MEAN, int BLOCK, int MINB, bool DAMP = false, bool PERX = false>
+template <typename real, typename S, bool MEAN, int BLOCK, int MINB, bool DAMP = false, bool PERX = false, bool TURB = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 ip_step_kernel(const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links, real *__restrict__ msum, const real *__restrict__ fur,
-               real *__restrict__ fuw, const Params<real> P, const IpPtrs<S> T)
+               real *__restrict__ fuw, const Params<real> P, const IpPtrs<S> T, const Turb<real> tb, const int turb_planes)
 {
-    ip_step_body<real, S, MEAN, BLOCK, DAMP, PERX>(flags, links, msum, fur, fuw, P, T);
+    ip_step_body<real, S, MEAN, BLOCK, DAMP, PERX, TURB>(flags, links, msum, fur, fuw, P, T, tb, turb_planes);
 }
 
 } // namespace lbmk

@@ -277,6 +277,56 @@ def test_flux_correction_and_damping_zones_in_place(B, fp64):
     assert max_err(sim, o, f64=fp64) <= tol
 
 
+@pytest.mark.parametrize("fp64", [False, True])
+def test_open_boundary_stack_with_inflow_fluctuations_in_place(B, fp64):
+    """Everything PAPER.md:175 / Table 1 PAPER.md:86 lists for the open faces at once, on one buffer: equilibrium velocity
+    faces, global flux correction, sponge + buffer nudging, synthetic fluctuations on the active inflow cells (extra block
+    rows of the in-place launch), the time mean; then another mode table from the developed state (odd parity), then off."""
+    from oracle import Oracle
+    from paper_2607_04516_b200 import workloads as W
+    nx, ny, nz = 44, 38, 20
+    hm = np.zeros((ny, nx), dtype=np.int32)
+    hm[14:20, 16:22] = 9
+    hm[24:27, 28:33] = 5
+    prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+    args = (nx, ny, nz, 2e-3, 0.1, 2e-4, (0.0, 0.0, 0.0), (3, 4, 3, 3, 1, 3))
+    target = np.stack([prof, 0.3 * prof, np.zeros(nz)])
+    modes = W.inflow_modes(48, 41, 2 * np.pi / 30, np.pi, convect=(0.05, 0.015, 0.0))
+    ux0 = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+    o = Oracle(*args)
+    sim = B.Lbm(*args, fp64=fp64, inplace=True)
+    for obj, kw in ((o, {}), (sim, {"f64": True})):
+        obj.set_flags(hm)
+        obj.set_inlet_profile(prof, 0.3 * prof, None, **kw)
+        obj.set_macros(None, ux0, 0.3 * ux0, None, **kw)
+        b, a = obj.balance_flux()
+        assert abs(a) < (1e-9 if (obj is o or fp64) else 2e-4)
+        obj.set_damping((5, 8, 5, 5, 0, 6), (0.05, 0.15, 0.05, 0.05, 0.0, 0.2), target)
+        obj.set_inflow_turbulence(modes, 0.003, 2 * np.pi / 12, 2.5)
+        obj.mean_config(20, 5)
+    tol = TOL64 if fp64 else TOL32
+    assert max_err(sim, o, f64=fp64) <= tol            # the inflow cells at t = 0
+    o.step(101); sim.step(101)
+    e = max_err(sim, o, f64=fp64)
+    assert e <= tol, (fp64, e)
+    gm, om = sim.get_mean(f64=fp64), o.get_mean()
+    assert gm[3] == om[3] == 17
+    em = max(float(np.abs(a.cpu().numpy().astype(np.float64) - b).max()) for a, b in zip(gm[:3], om[:3]))
+    assert em <= tol, (fp64, em)
+    ref = Oracle(*args)     # the same run without fluctuations: they matter
+    ref.set_flags(hm); ref.set_inlet_profile(prof, 0.3 * prof, None); ref.set_macros(None, ux0, 0.3 * ux0, None)
+    ref.balance_flux(); ref.set_damping((5, 8, 5, 5, 0, 6), (0.05, 0.15, 0.05, 0.05, 0.0, 0.2), target); ref.step(101)
+    assert max(np.abs(a - b).max() for a, b in zip(o.get_macros(), ref.get_macros())) > 1e-3
+    modes2 = W.inflow_modes(17, 5, 0.2, 2.0, convect=(0.04, 0.0, 0.0))
+    o.set_inflow_turbulence(modes2, 0.002, 0.3); sim.set_inflow_turbulence(modes2, 0.002, 0.3)
+    o.step(30); sim.step(30)
+    assert max_err(sim, o, f64=fp64) <= tol
+    o.set_inflow_turbulence(None); sim.set_inflow_turbulence(None)
+    o.step(20); sim.step(20)
+    assert max_err(sim, o, f64=fp64) <= tol
+    sim.close()
+
+
 def test_rest_state_is_exact_and_refused_combinations_say_so(B):
     hm = np.zeros((12, 16), dtype=np.int32)
     hm[3:6, 4:8] = 5
@@ -294,9 +344,6 @@ def test_rest_state_is_exact_and_refused_combinations_say_so(B):
     sim.set_flags(hm)
     with pytest.raises(B.LbmError, match="in-place"):
         sim.set_thermal(0.01, 1e-4, 0.0)
-    from paper_2607_04516_b200 import workloads as W
-    with pytest.raises(B.LbmError, match="in-place"):
-        sim.set_inflow_turbulence(W.inflow_modes(4, 1, 0.1, 1.0, (0.05, 0, 0)), 0.01, 0.3, 0.0)
     sim.set_variant(3)          # accepted, no effect: one launch shape
     sim.set_inlet_profile(np.full(8, 0.03, dtype=np.float32))
     sim.set_macros()
