@@ -46,30 +46,6 @@ inline IpPtrs<S> make_ip_ptrs(S *G, int q, const Params<real> &P)
     return t;
 }
 
-#ifndef IP_LD
-#define IP_LD 0
-#endif
-// the 19 loads of the in-place step: pinned ahead of the flag test like the two-buffer kernel's (ld_pinned)
-template <typename T>
-__device__ __forceinline__ auto ip_ld(const T *p)
-{
-#if IP_LD == 1
-    if constexpr (std::is_same<T, float>::value) {
-        float v;
-        asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p));
-        return v;
-    } else return ld_pinned(p);
-#elif IP_LD == 2
-    if constexpr (std::is_same<T, float>::value) {
-        float v;
-        asm volatile("ld.relaxed.gpu.global.f32 %0, [%1];" : "=f"(v) : "l"(p));
-        return v;
-    } else return ld_pinned(p);
-#else
-    return ld_pinned(p);
-#endif
-}
-
 // TURB: the launch carries the synthetic inflow fluctuations in extra leading block rows, exactly as the two-buffer kernel does
 // (lbm_step.cuh): one thread per face slot publishes the boundary velocity of the step after this one into the half of the side
 // array this launch writes.
@@ -113,7 +89,7 @@ __device__ __forceinline__ void ip_step_body(const uint8_t *__restrict__ flags, 
     Damp<real> dmp{real(0), real(0), real(0), real(0)};
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        g[i] = real(ip_ld(T.rd[i] + at(ic)));
+        g[i] = real(ld_pinned(T.rd[i] + at(ic)));
     });
     const bool onface = ((unsigned)(x - 1) >= (unsigned)(P.nx - 2)) | ((unsigned)(y - 1) >= (unsigned)(P.ny - 2)) |
                         ((unsigned)(z - 1) >= (unsigned)(P.nz - 2));
