@@ -288,6 +288,15 @@ int lbm_get_links(lbm_t *h, uint32_t *links);
 int lbm_get_state(lbm_t *h, double *f);
 int lbm_set_state(lbm_t *h, const double *f);
 
+/* The same checkpoint for the box lo[a] <= c_a < hi[a] (axes x, y, z; 0 <= lo < hi <= n, else LBM_EINVAL):
+ * f [19][hi[2]-lo[2]][hi[1]-lo[1]][hi[0]-lo[0]] doubles, host or device.  For lattices whose whole state (152 B per cell in
+ * this format) does not fit beside the lattice itself — 2.9e8 cells and more, or anything on LBM_STREAM_INPLACE scale — a run is
+ * checkpointed and restored slab by slab, and a sampled sub-box can be handed to a reference solver.  lbm_set_state_box writes the
+ * cells of the box into the CURRENT state (wall-link and ghost copies of their populations included) and leaves every other cell,
+ * the step counter and the mean sums alone; boxes that together cover the lattice restore exactly what lbm_set_state restores. */
+int lbm_get_state_box(lbm_t *h, const int lo[3], const int hi[3], double *f);
+int lbm_set_state_box(lbm_t *h, const int lo[3], const int hi[3], const double *f);
+
 long lbm_get_step(const lbm_t *h);
 int lbm_set_step(lbm_t *h, long step);
 int lbm_sync(lbm_t *h);

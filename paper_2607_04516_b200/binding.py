@@ -25,7 +25,7 @@ SYMBOLS = [
     "lbm_set_inlet_profile", "lbm_set_inlet_profile_f64", "lbm_set_inlet_plane", "lbm_set_inlet_plane_f64",
     "lbm_feed_inlet", "lbm_set_macros", "lbm_set_macros_f64", "lbm_step", "lbm_mean_config", "lbm_mean_reset",
     "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
-    "lbm_get_state", "lbm_set_state", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
+    "lbm_get_state", "lbm_set_state", "lbm_get_state_box", "lbm_set_state_box", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
     "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
     "lbm_set_thermal", "lbm_set_theta", "lbm_set_theta_f64", "lbm_get_theta", "lbm_get_theta_f64",
@@ -87,6 +87,8 @@ def load_library():
     lib.lbm_get_links.argtypes = [vp, vp]
     lib.lbm_get_state.argtypes = [vp, vp]
     lib.lbm_set_state.argtypes = [vp, vp]
+    lib.lbm_get_state_box.argtypes = [vp, vp, vp, vp]
+    lib.lbm_set_state_box.argtypes = [vp, vp, vp, vp]
     lib.lbm_get_step.argtypes = [vp]
     lib.lbm_get_step.restype = l
     lib.lbm_set_step.argtypes = [vp, l]
@@ -421,6 +423,32 @@ class Lbm:
         if tuple(k.shape) != (19,) + self.shape:
             raise ValueError("state must be [19][nz][ny][nx]")
         self._chk(self._lib.lbm_set_state(self._h, p), "set_state")
+
+    def _box(self, lo, hi):
+        lo = np.ascontiguousarray(lo, dtype=np.int32)
+        hi = np.ascontiguousarray(hi, dtype=np.int32)
+        if lo.shape != (3,) or hi.shape != (3,):
+            raise ValueError("lo and hi must be (x, y, z)")
+        return lo, hi
+
+    def get_state_box(self, lo, hi, out=None):
+        """populations of the box lo <= (x, y, z) < hi: [19][hi_z-lo_z][hi_y-lo_y][hi_x-lo_x] float64"""
+        lo, hi = self._box(lo, hi)
+        shape = (19, max(int(hi[2] - lo[2]), 0), max(int(hi[1] - lo[1]), 0), max(int(hi[0] - lo[0]), 0))
+        if out == "host":
+            a = np.empty(shape, dtype=np.float64)
+            self._chk(self._lib.lbm_get_state_box(self._h, lo.ctypes.data, hi.ctypes.data, a.ctypes.data), "get_state_box")
+            return a
+        a = self._new(self._torch.float64, shape)
+        self._chk(self._lib.lbm_get_state_box(self._h, lo.ctypes.data, hi.ctypes.data, a.data_ptr()), "get_state_box")
+        return a
+
+    def set_state_box(self, lo, hi, f):
+        lo, hi = self._box(lo, hi)
+        k, p = _ptr(f, np.float64)
+        if tuple(k.shape) != (19, int(hi[2] - lo[2]), int(hi[1] - lo[1]), int(hi[0] - lo[0])):
+            raise ValueError("state must be [19][hi_z-lo_z][hi_y-lo_y][hi_x-lo_x]")
+        self._chk(self._lib.lbm_set_state_box(self._h, lo.ctypes.data, hi.ctypes.data, p), "set_state_box")
 
     def get_step(self):
         return int(self._lib.lbm_get_step(self._h))

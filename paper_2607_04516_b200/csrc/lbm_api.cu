@@ -803,33 +803,48 @@ int do_get_links(lbm_t *h, uint32_t *links)
     return rc ? rc : rc2;
 }
 
+// box == nullptr: the whole lattice
+inline Box whole_or(const lbm_t *h, const Box *box)
+{
+    if (box) return *box;
+    Box b{};
+    b.bn[0] = h->nx; b.bn[1] = h->ny; b.bn[2] = h->nz;
+    return b;
+}
 template <typename real, typename S>
-int do_get_state(lbm_t *h, double *f)
+int do_get_state(lbm_t *h, double *f, const Box *box)
 {
     const Params<real> P = make_params<real>(h);
+    const Box bx = whole_or(h, box);
+    const long long NB = (long long)bx.bn[0] * bx.bn[1] * bx.bn[2];
     OutBuf o;
-    int rc = stage_out(h, f, (size_t)Q * P.N * sizeof(double), &o);
+    int rc = stage_out(h, f, (size_t)Q * NB * sizeof(double), &o);
     if (rc) return rc;
     const int B = 256;
-    state_out_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), h->flags(), h->links(), (double *)o.dev, P);
+    state_out_kernel<real, S><<<blocks_for(NB, B), B, 0, h->stream>>>((const S *)h->state(), h->flags(), h->links(), (double *)o.dev, P, bx);
     rc = check_launch(h, "state_out_kernel");
     int rc2 = finish_out(h, &o, 1);
     return rc ? rc : rc2;
 }
 
+// the whole lattice goes into buffer A, which becomes the current one (the first step rewrites every slot of B that is ever
+// read); a box goes into the CURRENT buffer, whichever it is, and leaves the rest of the state alone
 template <typename real, typename S>
-int do_set_state(lbm_t *h, const double *f)
+int do_set_state(lbm_t *h, const double *f, const Box *box)
 {
     const Params<real> P = make_params<real>(h);
+    const Box bx = whole_or(h, box);
+    const long long NB = (long long)bx.bn[0] * bx.bn[1] * bx.bn[2];
     InBuf in;
-    int rc = stage_in(h, f, (size_t)Q * P.N * sizeof(double), h->L.scratch_bytes, &in);
+    int rc = stage_in(h, f, (size_t)Q * NB * sizeof(double), h->L.scratch_bytes, &in);
     if (rc) return rc;
     const int B = 256;
-    state_in_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((S *)h->bufA(), (S *)nullptr, (real *)h->fu(), h->flags(), h->links(),
-                                                                    (const double *)in.dev, P);
+    S *dst = (S *)(box ? h->state() : h->bufA());
+    state_in_kernel<real, S><<<blocks_for(NB, B), B, 0, h->stream>>>(dst, (S *)nullptr, (real *)h->fu(), h->flags(), h->links(),
+                                                                   (const double *)in.dev, P, bx);
     rc = check_launch(h, "state_in_kernel");
     release_in(h, &in, 1);
-    if (!rc && !h->inplace) h->cur = 0;
+    if (!rc && !h->inplace && !box) h->cur = 0;
     return rc;
 }
 
@@ -1456,7 +1471,7 @@ int lbm_get_state(lbm_t *h, double *f)
     DevGuard dg_(h);
     if (!f) return fail(h, LBM_EINVAL, "get_state: NULL");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "get_state: flags not set");
-    return DISPATCH(h, do_get_state, h, f);
+    return DISPATCH(h, do_get_state, h, f, nullptr);
 }
 
 int lbm_set_state(lbm_t *h, const double *f)
@@ -1465,8 +1480,45 @@ int lbm_set_state(lbm_t *h, const double *f)
     DevGuard dg_(h);
     if (!f) return fail(h, LBM_EINVAL, "set_state: NULL");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_state: flags not set");
-    int rc = DISPATCH(h, do_set_state, h, f);
+    int rc = DISPATCH(h, do_set_state, h, f, nullptr);
     // the state brought its own boundary cells; the next launch must still find u_b(step + 1) in the side array
+    if (!rc && h->nmodes > 0) rc = DISPATCH(h, turb_publish, h, false);
+    return rc;
+}
+
+static int check_box(lbm_t *h, const int lo[3], const int hi[3], Box *bx, const char *what)
+{
+    if (!lo || !hi) return fail(h, LBM_EINVAL, std::string(what) + ": NULL");
+    const int n[3] = {h->nx, h->ny, h->nz};
+    for (int a = 0; a < 3; ++a) {
+        if (lo[a] < 0 || hi[a] > n[a] || lo[a] >= hi[a]) return fail(h, LBM_EINVAL, std::string(what) + ": need 0 <= lo < hi <= n on every axis");
+        bx->lo[a] = lo[a]; bx->bn[a] = hi[a] - lo[a];
+    }
+    return LBM_OK;
+}
+
+int lbm_get_state_box(lbm_t *h, const int lo[3], const int hi[3], double *f)
+{
+    if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!f) return fail(h, LBM_EINVAL, "get_state_box: NULL");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_state_box: flags not set");
+    Box bx{};
+    int rc = check_box(h, lo, hi, &bx, "get_state_box");
+    if (rc) return rc;
+    return DISPATCH(h, do_get_state, h, f, &bx);
+}
+
+int lbm_set_state_box(lbm_t *h, const int lo[3], const int hi[3], const double *f)
+{
+    if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!f) return fail(h, LBM_EINVAL, "set_state_box: NULL");
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "set_state_box: flags not set");
+    Box bx{};
+    int rc = check_box(h, lo, hi, &bx, "set_state_box");
+    if (rc) return rc;
+    rc = DISPATCH(h, do_set_state, h, f, &bx);
     if (!rc && h->nmodes > 0) rc = DISPATCH(h, turb_publish, h, false);
     return rc;
 }

@@ -438,38 +438,49 @@ __global__ void init_kernel(S *__restrict__ A, S *__restrict__ B, real *__restri
 }
 
 // ---- checkpoint ------------------------------------------------------------------------------------------------------------
-// f [19][nz][ny][nx] double, NOT shifted.  SOLID cells export the rest state w_i (their slots are mailboxes).
+// f [19][bz][by][bx] double, NOT shifted, of the box lo <= (x,y,z) < lo + bn (the whole lattice: lo = 0, bn = n).  SOLID cells
+// export the rest state w_i (their slots are mailboxes).
+struct Box { int lo[3], bn[3]; };
+__device__ __forceinline__ bool box_cell(const Box &bx, int c, int &x, int &y, int &z)
+{
+    if (c >= bx.bn[0] * bx.bn[1] * bx.bn[2]) return false;
+    x = bx.lo[0] + c % bx.bn[0];
+    const int r = c / bx.bn[0];
+    y = bx.lo[1] + r % bx.bn[1];
+    z = bx.lo[2] + r / bx.bn[1];
+    return true;
+}
 template <typename real, typename S>
 __global__ void state_out_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-                                 double *__restrict__ f, Params<real> P)
+                                 double *__restrict__ f, Params<real> P, const Box bx)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= P.N) return;
     int x, y, z;
-    cell_xyz(P, c, x, y, z);
+    if (!box_cell(bx, c, x, y, z)) return;
+    const long long NB = (long long)bx.bn[0] * bx.bn[1] * bx.bn[2];
     const int p = pidx(P, x, y, z);
     const uint8_t fl = flags[p];
     const bool solid = (fl & CLASS_MASK) == SOLID;
     real g[Q];
     if (!solid) load_cell_any(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? links[p] : 0u);
 #pragma unroll
-    for (int i = 0; i < Q; ++i) f[(long long)i * P.N + c] = (solid ? 0.0 : double(g[i])) + weight_f64(i);
+    for (int i = 0; i < Q; ++i) f[(long long)i * NB + c] = (solid ? 0.0 : double(g[i])) + weight_f64(i);
 }
 
 template <typename real, typename S>
 __global__ void state_in_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
-                                const uint32_t *__restrict__ links, const double *__restrict__ f, Params<real> P)
+                                const uint32_t *__restrict__ links, const double *__restrict__ f, Params<real> P, const Box bx)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= P.N) return;
     int x, y, z;
-    cell_xyz(P, c, x, y, z);
+    if (!box_cell(bx, c, x, y, z)) return;
+    const long long NB = (long long)bx.bn[0] * bx.bn[1] * bx.bn[2];
     const int p = pidx(P, x, y, z);
     const uint8_t fl = flags[p];
     if ((fl & CLASS_MASK) == SOLID) return;
     real g[Q];
 #pragma unroll
-    for (int i = 0; i < Q; ++i) g[i] = real(f[(long long)i * P.N + c] - weight_f64(i));
+    for (int i = 0; i < Q; ++i) g[i] = real(f[(long long)i * NB + c] - weight_f64(i));
     store_cell_both(A, B, fu, P, p, x, y, z, fl, links[p], g);
 }
 

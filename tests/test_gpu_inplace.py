@@ -327,6 +327,55 @@ def test_open_boundary_stack_with_inflow_fluctuations_in_place(B, fp64):
     sim.close()
 
 
+@pytest.mark.parametrize("inplace", [False, True])
+@pytest.mark.parametrize("fp64", [False, True])
+def test_state_box_is_a_slice_of_the_state_and_restores_slab_by_slab(B, fp64, inplace):
+    """lbm_get_state_box / lbm_set_state_box (include/lbm.h): the checkpoint of a sub-box, for lattices whose whole state does
+    not fit beside the lattice.  Both streaming schemes, at an odd step (buffer B / parity 1 current)."""
+    shape = (37, 11, 9)
+    nx, ny, nz = shape
+    hm, prof, ux0, uy0 = _case(shape, 5)
+    for faces in [(3, 4, 0, 0, 1, 2), (0, 0, 2, 2, 1, 2)]:
+        args = (nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), faces)
+
+        def fresh(presteps):
+            sim = B.Lbm(*args, fp64=fp64, inplace=inplace)
+            sim.set_flags(hm)
+            sim.set_inlet_profile(prof, 0.1 * prof, None, f64=True)
+            sim.set_macros(None, ux0, uy0, None, f64=True)
+            sim.step(presteps)
+            return sim
+        src = fresh(15)
+        full = src.get_state(out="host")
+        for lo, hi in [((0, 0, 0), (nx, ny, nz)), ((5, 2, 1), (20, 9, 4)), ((nx - 3, 0, 0), (nx, ny, nz)), ((0, 3, nz - 1), (1, 4, nz))]:
+            box = src.get_state_box(lo, hi, out="host")
+            assert np.array_equal(box, full[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]]), (lo, hi)
+            dev = src.get_state_box(lo, hi).cpu().numpy()      # device destination
+            assert np.array_equal(dev, box)
+        ref = fresh(4)
+        ref.set_state(full)
+        ref.set_step(15)
+        for presteps in (4, 7):     # the receiving handle's current buffer / parity is A / 0 and B / 1
+            dst = fresh(presteps)
+            for z0, z1 in [(0, 2), (2, 3), (3, nz)]:            # three slabs that cover the lattice
+                dst.set_state_box((0, 0, z0), (nx, ny, z1), np.ascontiguousarray(full[:, z0:z1]))
+            dst.set_step(15)
+            assert np.array_equal(dst.get_state(out="host"), full)
+            dst.step(12)
+            if presteps == 4:
+                ref.step(12)
+            d = float(np.abs(dst.get_state(out="host") - ref.get_state(out="host")).max())
+            assert d <= (1e-13 if fp64 else 1e-6), (faces, presteps, d)   # restored slab by slab = restored in one call
+            dst.close()
+        with pytest.raises(B.LbmError):
+            src.get_state_box((0, 0, 0), (nx + 1, ny, nz))
+        with pytest.raises(B.LbmError):
+            src.get_state_box((3, 0, 0), (3, ny, nz))
+        with pytest.raises(B.LbmError):
+            src.set_state_box((-1, 0, 0), (2, 2, 2), np.zeros((19, 2, 2, 3)))
+        src.close(); ref.close()
+
+
 def test_rest_state_is_exact_and_refused_combinations_say_so(B):
     hm = np.zeros((12, 16), dtype=np.int32)
     hm[3:6, 4:8] = 5

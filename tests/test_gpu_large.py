@@ -168,6 +168,36 @@ def test_a_lattice_too_large_for_two_buffers_runs_in_place(B):
             worst = max(worst, float(d.max()))
         o.close()
         assert worst <= TOL32, (box, worst)
+    del g
+    # ... and from a DEVELOPED state: lbm_get_state_box of the box + halo at step K -> the oracle continues T steps
+    K = sim.get_step() + 10
+    sim.step(K - sim.get_step())
+    subs = []
+    for box in boxes[:3]:
+        lo = [max(box[2 * a] - H, 0) for a in range(3)]
+        hi = [min(box[2 * a + 1] + H, n[a]) for a in range(3)]
+        subs.append((box, lo, hi, sim.get_state_box(lo, hi).cpu().numpy()))
+    sim.step(T)
+    g = sim.get_macros()
+    for box, lo, hi, sub in subs:
+        fb = []
+        for a in range(3):
+            for side in (0, 1):
+                real = (lo[a] == 0) if side == 0 else (hi[a] == n[a])
+                fb.append(faces[2 * a + side] if real else WALL)
+        o = Oracle(hi[0] - lo[0], hi[1] - lo[1], hi[2] - lo[2], c3.nu0, c3.Cs, c3.f_cor, c3.F, tuple(fb))
+        o.set_flags(np.ascontiguousarray(height[lo[1]:hi[1], lo[0]:hi[0]]))
+        o.set_state(sub)
+        o.step(T)
+        r = o.get_macros()
+        sl = tuple(slice(box[2 * a] - lo[a], box[2 * a + 1] - lo[a]) for a in (2, 1, 0))
+        gl = (slice(box[4], box[5]), slice(box[2], box[3]), slice(box[0], box[1]))
+        for ga, ra in zip(g, r):
+            d = np.abs(ga[gl].cpu().numpy().astype(np.float64) - ra[sl])
+            assert np.isfinite(d).all()
+            worst = max(worst, float(d.max()))
+        o.close()
+        assert worst <= TOL32, (box, worst)
     # a timing of the same lattice, for the record (not a bench line): 50 more steps
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(); sim.step(50); e1.record(); torch.cuda.synchronize()
