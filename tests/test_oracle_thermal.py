@@ -356,3 +356,50 @@ def test_heated_inflow_rises_under_buoyancy():
     uz = o.get_macros()[3]
     assert uz[3:9, :, 3:10].max() > 1e-4
     o.close()
+
+
+def test_buoyancy_against_a_uniform_damping_zone_settles_at_a_over_sigma():
+    """The thermal lattice together with the damping zones of PAPER.md:175 (DESIGN.md §4 readings 20 and 23): the relaxation
+    acceleration sigma (u_t - u) and the buoyancy g beta (theta - theta_ref) e_z enter the SAME implicit half-force solve, so
+    a uniformly warm, uniformly damped periodic box obeys dw/dt = a - sigma (w - w_t) by the trapezoidal rule exactly: the
+    collision velocity settles at w* = w_t + a / sigma and its defect shrinks by q = (1 - sigma/2)/(1 + sigma/2) per step —
+    a closed form that a dropped term, a double-counted half step or a sign error in either force breaks.  Two-layer slab,
+    periodic in x, y and z, width-1 zones on z- and z+ (the same sigma in every cell); theta stays uniform (fixed point)."""
+    nx, ny, nz = 5, 4, 2
+    sigma, gbeta, dth, wt = 0.25, 2e-4, 1.5, 0.01
+    a = gbeta * dth
+    o = O.Oracle(nx, ny, nz, 5e-3, 0.1, 0.0, faces=[P] * 6)
+    o.set_flags(None)
+    ut = np.zeros((3, nz)); ut[2] = wt
+    o.set_damping((0, 0, 0, 0, 1, 1), (0, 0, 0, 0, sigma, sigma), ut)
+    assert np.all(o.get_damping() == sigma)
+    o.set_thermal(0.02, gbeta, 300.0)
+    w0 = 0.03
+    o.set_macros(None, None, None, np.full((nz, ny, nx), w0))
+    o.set_theta(np.full((nz, ny, nx), 300.0 + dth))
+    q = (1 - sigma / 2) / (1 + sigma / 2)
+    wstar = wt + a / sigma
+    # the stored (post-collision) momentum m* and the collision velocity w_k: w_k = w* + (w_1 - w*) q^(k-1), and the local
+    # macros of the state after k steps return w_k (DESIGN.md §3 step 7)
+    c, _, _ = O.lattice()
+    f0 = o.get_state()
+    m0 = float((c[:, 2, None, None, None] * f0).sum(axis=0).mean())        # = rho w0 (the initial state is f_eq(1, w0))
+    # first collision: (1 + sigma/2) w_1 = m0 + a/2 + (sigma/2) w_t
+    w1 = (m0 + a / 2 + sigma / 2 * wt) / (1 + sigma / 2)
+    for k in range(1, 41):
+        o.step(1)
+        rho, ux, uy, uz = o.get_macros()
+        wk = wstar + (w1 - wstar) * q ** (k - 1)
+        assert np.abs(uz - wk).max() < 2e-15, (k, float(np.abs(uz - wk).max()))
+        assert np.abs(ux).max() < 1e-16 and np.abs(uy).max() < 1e-16 and np.abs(rho - 1).max() < 1e-13
+        assert np.abs(o.get_theta() - (300.0 + dth)).max() < 1e-12
+    assert abs(wk - wstar) < abs(w1 - wstar) * 1e-4        # it has settled at a / sigma above the target
+    # without the zone the same box accelerates without bound (k a per step): the zone is what balances the buoyancy
+    o2 = O.Oracle(nx, ny, nz, 5e-3, 0.1, 0.0, faces=[P] * 6)
+    o2.set_flags(None)
+    o2.set_thermal(0.02, gbeta, 300.0)
+    o2.set_macros(None, None, None, np.full((nz, ny, nx), w0))
+    o2.set_theta(np.full((nz, ny, nx), 300.0 + dth))
+    o2.step(40)
+    assert abs(float(o2.get_macros()[3].mean()) - (w0 + 39.5 * a)) < 1e-14
+    o.close(); o2.close()
