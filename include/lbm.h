@@ -211,9 +211,10 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
  * lbm_set_thermal switches it on with theta = theta_ref at rest; it allocates 2 x 7 population arrays of the handle's
  * precision (library-owned, freed by lbm_destroy).  Open faces (DESIGN.md §4 reading 27): an EQ_FIXED cell holds
  * h_eq(theta_b, u_b) beside f_eq(1, u_b), with theta_b = theta_ref until lbm_set_inlet_theta prescribes it; an EQ_OUTFLOW
- * cell holds the equilibria of the theta and u its inward neighbour had at the previous step (zero gradient).  Damping zones,
- * inflow fluctuations and 16-bit storage must be off (LBM_EINVAL otherwise, also from the calls that would switch those on
- * later).  alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
+ * cell holds the equilibria of the theta and u its inward neighbour had at the previous step (zero gradient).  Damping zones
+ * (lbm_set_damping) combine with it: the relaxation acceleration and the buoyancy enter the same implicit half-force solve.
+ * Inflow fluctuations, 16-bit storage and in-place streaming must be off (LBM_EINVAL otherwise, also from the calls that would
+ * switch those on later).  alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
 int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref);
 /* Prescribed temperature of the EQ_FIXED cells by level (reading 27): theta_b[nz], host or device; the cells' thermal state
  * becomes h_eq(theta_b(z), u_b) at once and is re-expanded from it every step.  A later lbm_set_inlet_profile / _plane,

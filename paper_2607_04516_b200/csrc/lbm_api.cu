@@ -625,7 +625,16 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         real *HB = (real *)h->th_other(), *msum = (real *)h->mean();
         const uint8_t *fl = h->flags();
         const uint32_t *lk = h->links();
-        if (P.perx) {
+        if (h->damp_on) { // damping zones together with the thermal lattice: their own instantiation (one CTA per SM less)
+            constexpr int MD = std::is_same<real, float>::value ? (MINB > 8 ? 8 : MINB) : MINB;
+            if (P.perx) {
+                if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MD, true, true>, B, HB, fl, lk, msum, P, T, O);
+                else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MD, true, true>, B, HB, fl, lk, msum, P, T, O);
+            } else {
+                if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MD, false, true>, B, HB, fl, lk, msum, P, T, O);
+                else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MD, false, true>, B, HB, fl, lk, msum, P, T, O);
+            }
+        } else if (P.perx) {
             if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O);
             else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O);
         } else {
@@ -882,7 +891,8 @@ int do_refeed(lbm_t *h)
     const Params<real> P = make_params<real>(h);
     if (P.F == 0) return LBM_OK;
     const int B = 256;
-    refeed_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), (real *)h->fu(), h->flags(), h->links(), P);
+    refeed_kernel<real, S><<<blocks_for(P.N, B), B, 0, h->stream>>>((const S *)h->state(), (real *)h->fu(), h->flags(), h->links(), P,
+                                                                  (const real *)h->th_state());
     return check_launch(h, "refeed_kernel");
 }
 
@@ -1047,7 +1057,7 @@ int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
         return fail(h, LBM_EINVAL, "set_thermal: alpha must be > 0 and all arguments finite");
     if (h->s16) return fail(h, LBM_EINVAL, "set_thermal: not combinable with 16-bit population storage");
     if (h->inplace) return fail(h, LBM_EINVAL, "set_thermal: not combinable with in-place streaming");
-    if (h->damp_on || h->nmodes > 0) return fail(h, LBM_EINVAL, "set_thermal: not combinable with damping zones / inflow fluctuations");
+    if (h->nmodes > 0) return fail(h, LBM_EINVAL, "set_thermal: not combinable with inflow fluctuations");
     if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half() + h->ft_bytes()));
     CUDA_TRY(h, cudaMemsetAsync(h->th_ws, 0, 2 * h->th_half() + h->ft_bytes(), h->stream)); // theta_ref at rest (shifted storage), theta_b = theta_ref
     h->alpha = alpha; h->gbeta = g_beta; h->theta_ref = theta_ref; h->thermal = true;
@@ -1204,7 +1214,6 @@ int lbm_set_damping(lbm_t *h, const int width[6], const double peak[6], const do
     if (!h) return LBM_EINVAL;
     DevGuard dg_(h);
     if (!width || !peak) return fail(h, LBM_EINVAL, "set_damping: NULL");
-    if (h->thermal) return fail(h, LBM_EINVAL, "set_damping: not combinable with the thermal lattice");
     bool any = false;
     for (int k = 0; k < 6; ++k) {
         if (width[k] < 0 || !(peak[k] >= 0.0) || peak[k] > 1.0) return fail(h, LBM_EINVAL, "set_damping: need width >= 0 and 0 <= peak <= 1");
@@ -1266,6 +1275,7 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
     DevGuard dg_(h);
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inflow_turbulence: flags not set");
     if (n_modes < 0 || n_modes > MAX_MODES) return fail(h, LBM_EINVAL, "set_inflow_turbulence: n_modes out of range");
+    if (h->thermal && n_modes > 0) return fail(h, LBM_EINVAL, "set_inflow_turbulence: not combinable with the thermal lattice");
     auto rewrite = [&]() { return DISPATCH(h, turb_publish, h, true); };
     if (n_modes == 0) {
         if (h->nmodes == 0) return LBM_OK;

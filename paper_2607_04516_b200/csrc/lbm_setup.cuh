@@ -374,7 +374,7 @@ __global__ void fluct_kernel(S *__restrict__ A, S *__restrict__ B, real *__restr
 // rule is u_loc(G_k, c - n) evaluated with the parameters in force when the step runs (DESIGN.md §3 step 6).
 template <typename real, typename S>
 __global__ void refeed_kernel(const S *__restrict__ A, real *__restrict__ fu, const uint8_t *__restrict__ flags,
-                              const uint32_t *__restrict__ links, Params<real> P)
+                              const uint32_t *__restrict__ links, Params<real> P, const real *__restrict__ H = nullptr)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= P.N) return;
@@ -385,6 +385,9 @@ __global__ void refeed_kernel(const S *__restrict__ A, real *__restrict__ fu, co
     if (!(fl & FEED_BIT)) return;
     real g[Q];
     load_cell_any(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? links[p] : 0u);
+    if (H) // thermal lattice on (H = its current state, 7 shifted populations): the cell's buoyancy belongs to its force (lbm_thermal.cuh)
+        P.Fz += P.gbeta * (H[p] + ((H[P.stride + p] + H[2 * P.stride + p]) + (H[3 * P.stride + p] + H[4 * P.stride + p]) +
+                                   (H[5 * P.stride + p] + H[6 * P.stride + p])));
     const Macro<real> m = local_macros(g, fl & CLASS_MASK, P, damp_at(P, x, y, z));
     outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int s, int comp, real v) {
         fu[comp * P.F + s] = v;

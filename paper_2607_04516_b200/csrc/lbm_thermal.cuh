@@ -102,7 +102,10 @@ inline ThermalPtrs<real> make_thermal_ptrs(const real *A, real *B, const real *H
 template <typename real>
 struct OpenFaces { const real *fur; real *fuw; const real *ftr; real *ftw; };
 
-template <typename real, bool MEAN, int BLOCK, int MINB, bool PERX = false>
+// DAMP: the damping-zone instantiation (lbm_set_damping together with the thermal lattice): the relaxation acceleration
+// sigma (u_t - u) and the buoyancy enter the same implicit half-force solve (collide<real, true, true>); launched only while
+// zones are configured, so the plain thermal kernel carries none of it.
+template <typename real, bool MEAN, int BLOCK, int MINB, bool PERX = false, bool DAMP = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
                     real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O)
@@ -142,7 +145,9 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
     // h_eq(theta, u) of that collision's velocity
     auto collide_both = [&]() {
         const real dth = theta_shift(t);
-        const Macro<real> m = collide<real, false, true>(g, P, Damp<real>{}, P.gbeta * dth);
+        Macro<real> m;
+        if constexpr (DAMP) m = collide<real, true, true>(g, P, damp_at(P, x, y, z), P.gbeta * dth); // table look-ups: L1 / L2 resident
+        else m = collide<real, false, true>(g, P, Damp<real>{}, P.gbeta * dth);
         real e[QT];
         thermal_equilibrium(e, dth, P.theta_ref, m.ux, m.uy, m.uz);
 #pragma unroll
@@ -231,7 +236,7 @@ __device__ __forceinline__ void thermal_feed_both(const real *__restrict__ A, re
     real g[Q];
     load_cell(g, A, P.stride, p);
     P.Fz += P.gbeta * dth;
-    const Macro<real> m = local_macros(g, cls, P);
+    const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
     outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) {
         fu[comp * P.F + sl] = v;
         fu[(3 + comp) * P.F + sl] = v;

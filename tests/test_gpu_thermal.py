@@ -139,9 +139,10 @@ def test_thermal_error_behaviour(B):
     sim.set_thermal(0.01, 1e-3, 1.0)
     with pytest.raises(B.LbmError):
         sim.set_theta()  # flags were invalidated by set_boundaries
-    with pytest.raises(B.LbmError):
-        sim.set_damping([0, 0, 0, 0, 0, 4], [0, 0, 0, 0, 0, 0.1])
     sim.set_flags(np.zeros((8, 8), np.int32))
+    from paper_2607_04516_b200 import workloads as Wl
+    with pytest.raises(B.LbmError, match="thermal"):      # inflow fluctuations stay refused together with the thermal lattice
+        sim.set_inflow_turbulence(Wl.inflow_modes(4, 1, 0.1, 1.0, (0.05, 0, 0)), 0.01, 0.3, 0.0)
     sim.set_macros(); sim.set_theta()
     sim.step(3)
     assert float(np.abs(sim.get_theta().cpu().numpy() - 1.0).max()) == 0.0  # isothermal rest state is exact
@@ -441,3 +442,66 @@ def test_open_faces_boundary_updates_mean_and_checkpoint(B):
     gb_ = [a.cpu().numpy() for a in b.get_macros()] + [b.get_theta(out="host")]
     assert max(float(np.abs(x - y).max()) for x, y in zip(ga, gb_)) <= 2e-6
     sim.close(); o.close(); b.close()
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+@pytest.mark.parametrize("faces", [(EQF, EQO, EQF, EQF, W, EQF), (EQF, EQO, P, P, W, FS), (P, P, P, P, W, FS)])
+def test_damping_zones_together_with_the_thermal_lattice(B, faces, fp64):
+    """The paper's open-boundary damping (top sponge + lateral buffer nudging) on a thermal run: the relaxation
+    acceleration and the buoyancy share one implicit half-force solve (oracle pin: test_oracle_thermal.py
+    ::test_buoyancy_against_a_uniform_damping_zone_settles_at_a_over_sigma).  Buildings, warm inflow, LES, Coriolis; zones set
+    before the run, changed from a developed state (the outflow velocities are re-published with buoyancy AND damping in the
+    local macros), switched off; the time mean; rho, u, theta against the oracle."""
+    nx, ny, nz = 52, 14, 12
+    hm = np.zeros((ny, nx), np.int32); hm[3:8, 14:20] = 5; hm[8:12, 30:36] = 3
+    sim, o, prof, thb = open_pair(B, nx, ny, nz, faces, hm, fp64, seed=3, want_mean=True)
+    target = np.stack([prof, 0.1 * prof, np.zeros(nz)])
+    tol = TOL64 if fp64 else TOL32
+    for obj in (o, sim):
+        obj.set_damping((4, 8, 3, 3, 0, 5), (0.05, 0.2, 0.05, 0.05, 0.0, 0.3), target)
+        obj.mean_config(10, 5)
+    sim.step(61); o.step(61)
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= tol and e_th <= tol, ("zones", faces, fp64, e_flow, e_th)
+    gm = sim.get_mean(f64=True); om = o.get_mean()
+    assert gm[3] == om[3] == 11
+    assert max(float(np.abs(a.cpu().numpy() - b).max()) for a, b in zip(gm[:3], om[:3])) <= tol
+    for obj in (o, sim):
+        obj.set_damping((0, 12, 0, 0, 0, 3), (0.0, 0.4, 0.0, 0.0, 0.0, 0.1), target)
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= tol and e_th <= tol
+    sim.step(30); o.step(30)
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= tol and e_th <= tol, ("changed", faces, fp64, e_flow, e_th)
+    for obj in (o, sim):
+        obj.set_damping([0] * 6, [0.0] * 6, None)
+    sim.step(20); o.step(20)
+    e_flow, e_th = errs(sim, o, 1.0)
+    assert e_flow <= tol and e_th <= tol, ("off", faces, fp64, e_flow, e_th)
+    # the zones matter: the same run without them differs
+    sim2, o2, _, _ = open_pair(B, nx, ny, nz, faces, hm, fp64, seed=3)
+    o2.step(111)
+    assert max(float(np.abs(a - b).max()) for a, b in zip(o.get_macros(), o2.get_macros())) > 1e-4
+    sim.close(); o.close(); sim2.close(); o2.close()
+
+
+def test_uniformly_warm_damped_box_settles_at_a_over_sigma_on_the_gpu(B):
+    """The closed form that pins the oracle (w* = w_t + g beta dtheta / sigma, defect x (1 - sigma/2)/(1 + sigma/2) per step), on
+    the FP32 path itself."""
+    nx, ny, nz = 40, 6, 2
+    sigma, gbeta, dth, wt, w0 = 0.25, 2e-4, 1.5, 0.01, 0.03
+    sim = B.Lbm(nx, ny, nz, 5e-3, 0.1, 0.0, (0, 0, 0), [P] * 6)
+    sim.set_flags(None)
+    ut = np.zeros((3, nz)); ut[2] = wt
+    sim.set_damping((0, 0, 0, 0, 1, 1), (0, 0, 0, 0, sigma, sigma), ut)
+    sim.set_thermal(0.02, gbeta, 300.0)
+    sim.set_macros(None, None, None, np.full((nz, ny, nx), w0, dtype=np.float32))
+    sim.set_theta(np.full((nz, ny, nx), 300.0 + dth), f64=True)
+    a, q = gbeta * dth, (1 - sigma / 2) / (1 + sigma / 2)
+    wstar = wt + a / sigma
+    w1 = (w0 + a / 2 + sigma / 2 * wt) / (1 + sigma / 2)
+    for k in (1, 2, 10, 40):
+        sim.step(k - sim.get_step())
+        uz = sim.get_macros()[3].cpu().numpy()
+        assert np.abs(uz - (wstar + (w1 - wstar) * q ** (k - 1))).max() < 2e-7, k
+    sim.close()
