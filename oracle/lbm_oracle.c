@@ -593,6 +593,12 @@ static void write_fixed_cells_at(oracle_t *o, double t)
                 to_storage(o, g);
                 memcpy(o->G + cell * Q, g, sizeof g);
                 memcpy(o->Gn + cell * Q, g, sizeof g);
+                if (o->thermal) { /* reading 28: the thermal state of the cell is the equilibrium of the SAME velocity */
+                    double h[QT];
+                    heq(o->thb[cell], u, h);
+                    memcpy(o->H + cell * QT, h, sizeof h);
+                    memcpy(o->Hn + cell * QT, h, sizeof h);
+                }
             }
 }
 
@@ -896,11 +902,15 @@ int oracle_step(oracle_t *o, int nsteps)
                         boundary_velocity(o, x, y, z, (double)(o->step + 1), u);
                         feq(1.0, u, gn);
                         to_storage(o, gn);
+                        /* reading 28: with the thermal lattice on, the cell holds h_eq(theta_b, u_b + u') beside
+                         * f_eq(1, u_b + u') — one boundary velocity for both lattices, as reading 27 has it for the mean */
+                        if (o->thermal) heq(o->thb[cell], u, o->Hn + cell * QT);
                     } else {
                         /* SOLID: inert; EQ_FIXED (step 5): unchanged */
                         memcpy(gn, o->G + cell * Q, sizeof(double) * Q);
                     }
-                    if (o->thermal && cl != C_FLUID && cl != C_EQ_OUTFLOW) memcpy(o->Hn + cell * QT, o->H + cell * QT, sizeof(double) * QT);
+                    if (o->thermal && cl != C_FLUID && cl != C_EQ_OUTFLOW && !(cl == C_EQ_FIXED && o->nmodes > 0))
+                        memcpy(o->Hn + cell * QT, o->H + cell * QT, sizeof(double) * QT);
                 }
         double *t = o->G; o->G = o->Gn; o->Gn = t;
         if (o->thermal) { t = o->H; o->H = o->Hn; o->Hn = t; }

@@ -403,3 +403,51 @@ def test_buoyancy_against_a_uniform_damping_zone_settles_at_a_over_sigma():
     o2.step(40)
     assert abs(float(o2.get_macros()[3].mean()) - (w0 + 39.5 * a)) < 1e-14
     o.close(); o2.close()
+
+
+def test_thermal_state_of_a_fluctuating_inlet_cell_follows_the_same_velocity():
+    """Reading 28: with synthetic inflow fluctuations on an active inflow cell holds
+    h_eq(theta_b, u_b + u') beside f_eq(1, u_b + u') — ONE boundary velocity for both lattices.  Observable through the heat the
+    inlet cell hands to its fluid neighbour: one mode kappa = (0, pi/4, 0) with sigma = e_x gives u'_x(y, t) = 2 uhat cos(pi y/4
+    - omega t), and the cell at x = 1 pulls h_1 = (theta_b / 8)(1 + 4 (U + u'_x)) from the inlet, so after ONE step its
+    temperature exceeds that of the same run without fluctuations by exactly (theta_b / 2) u'_x(y, 0) — zero if the thermal
+    state had stayed at the mean velocity, doubled by a double-counted term, sign-flipped by a wrong direction."""
+    nx, ny, nz, U = 8, 16, 6, 0.05
+    theta_ref, theta_b = 1.0, 1.3
+    u_rms, k_e, dk, kap, om = 0.01, 0.5, 0.125, np.pi / 4, np.pi / 4
+    uhat = np.sqrt(O.vk_spectrum([kap], u_rms, k_e)[0] * dk)
+
+    def make(turb):
+        o = O.Oracle(nx, ny, nz, 1e-2, 0.0, 0.0, faces=[3, 4, P, P, P, P])      # EQ_FIXED inlet on x-, EQ_OUTFLOW on x+
+        o.set_flags(None)
+        o.set_inlet_profile(np.full(nz, U))
+        o.set_macros(None, np.full((nz, ny, nx), U), None, None)
+        o.set_thermal(0.05, 0.0, theta_ref)
+        o.set_inlet_theta(np.full(nz, theta_b))
+        o.set_theta(np.full((nz, ny, nx), theta_ref), np.full((nz, ny, nx), U), None, None)
+        if turb:
+            o.set_inflow_turbulence([[0, kap, 0, 1, 0, 0, 0.0, om, dk]], u_rms, k_e)
+        return o
+    a, b = make(True), make(False)
+    y = np.arange(ny)
+    up0 = 2 * uhat * np.cos(kap * y)
+    assert np.abs(a.get_macros()[1][2, :, 0] - (U + up0)).max() < 1e-16          # the flow side (pinned in test_oracle_inflow.py)
+    assert np.abs(a.get_theta()[:, :, 0] - theta_b).max() < 1e-15                # the inlet cell's temperature is theta_b either way
+    a.step(1); b.step(1)
+    d = a.get_theta()[2, :, 1] - b.get_theta()[2, :, 1]
+    assert np.abs(d - 0.5 * theta_b * up0).max() < 1e-15, float(np.abs(d - 0.5 * theta_b * up0).max())
+    assert np.abs(d).max() > 1e-4                                                 # and it is not a statement about zero
+    assert np.abs(a.get_theta()[:, :, 2:] - b.get_theta()[:, :, 2:]).max() < 1e-15   # nothing further in has heard of it yet
+    # the cell written BY THE STEP carries u'(x, 1): second step, same law with the crest moved by one cell (omega = kappa)
+    ta, tb = a.get_theta().copy(), b.get_theta().copy()
+    ua = a.get_macros()[1][2, :, 0]
+    assert np.abs(ua - (U + 2 * uhat * np.cos(kap * y - om))).max() < 1e-15
+    # switched off: the inlet cell returns to the mean in both lattices — from then on the two runs receive the same heat
+    a.set_inflow_turbulence(None)
+    ha, hb = a.get_theta()[:, :, 0], b.get_theta()[:, :, 0]
+    assert np.abs(ha - hb).max() < 1e-15
+    a.step(1); b.step(1)
+    # one step later the extra heat handed over at x = 1 is what the mean hands over: the difference of the two runs at x = 1
+    # only relaxes by diffusion / advection of what is already there (no new source): its y-mean stays zero
+    assert abs(float((a.get_theta()[2, :, 1] - b.get_theta()[2, :, 1]).mean())) < 1e-15
+    a.close(); b.close()
