@@ -213,8 +213,9 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
  * h_eq(theta_b, u_b) beside f_eq(1, u_b), with theta_b = theta_ref until lbm_set_inlet_theta prescribes it; an EQ_OUTFLOW
  * cell holds the equilibria of the theta and u its inward neighbour had at the previous step (zero gradient).  Damping zones
  * (lbm_set_damping) combine with it: the relaxation acceleration and the buoyancy enter the same implicit half-force solve.
- * Inflow fluctuations, 16-bit storage and in-place streaming must be off (LBM_EINVAL otherwise, also from the calls that would
- * switch those on later).  alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
+ * So do the synthetic inflow fluctuations (lbm_set_inflow_turbulence): an active inflow cell holds h_eq(theta_b, u_b + u') beside
+ * f_eq(1, u_b + u'), one boundary velocity for both lattices (DESIGN.md §4 reading 28); theta_b itself does not fluctuate.
+ * 16-bit storage and in-place streaming must be off (LBM_EINVAL).  alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
 int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref);
 /* Prescribed temperature of the EQ_FIXED cells by level (reading 27): theta_b[nz], host or device; the cells' thermal state
  * becomes h_eq(theta_b(z), u_b) at once and is re-expanded from it every step.  A later lbm_set_inlet_profile / _plane,

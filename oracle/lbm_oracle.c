@@ -1026,6 +1026,8 @@ int oracle_set_thermal(oracle_t *o, double alpha, double gbeta, double theta_ref
         for (int i = 0; i < QT; ++i) o->H[cell * QT + i] = o->Hn[cell * QT + i] = weight_t(i) * theta_ref;
         if (o->have_flags && o->cls[cell] == C_EQ_FIXED) write_eq_fixed_thermal(o, cell);
     }
+    /* reading 28: inflow cells that carry fluctuations hold the thermal equilibrium of the velocity they have now */
+    if (o->have_flags && o->nmodes > 0) write_fixed_cells_at(o, (double)o->step);
     return 0;
 }
 
@@ -1042,6 +1044,7 @@ int oracle_set_inlet_theta(oracle_t *o, const double *theta_b)
                 o->thb[cell] = theta_b[z];
                 write_eq_fixed_thermal(o, cell);
             }
+    if (o->nmodes > 0) write_fixed_cells_at(o, (double)o->step); /* reading 28: ... of the velocity the cells have now */
     return 0;
 }
 

@@ -625,21 +625,26 @@ int launch_step(lbm_t *h, const Params<real> &P, bool sample)
         real *HB = (real *)h->th_other(), *msum = (real *)h->mean();
         const uint8_t *fl = h->flags();
         const uint32_t *lk = h->links();
-        if (h->damp_on) { // damping zones together with the thermal lattice: their own instantiation (one CTA per SM less)
+        const bool turb = h->nmodes > 0 && P.F > 0;
+        if (h->damp_on || turb) { // damping zones / inflow fluctuations together with the thermal lattice: their own instantiation (one CTA per SM less)
             constexpr int MD = std::is_same<real, float>::value ? (MINB > 8 ? 8 : MINB) : MINB;
+            // leading block rows that carry the face slots; they publish the boundary velocity of step (this one) + 1 (launch_step_as)
+            const int turb_planes = turb ? (int)((blocks_for(P.F, BLOCK) + grid.x - 1) / grid.x) : 0;
+            cfg.gridDim.y += turb_planes;
+            const Turb<real> tb{(const real *)h->fum(), h->modes(), h->nmodes, (double)(h->step + 2)};
             if (P.perx) {
-                if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MD, true, true>, B, HB, fl, lk, msum, P, T, O);
-                else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MD, true, true>, B, HB, fl, lk, msum, P, T, O);
+                if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MD, true, true>, B, HB, fl, lk, msum, P, T, O, tb, turb_planes);
+                else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MD, true, true>, B, HB, fl, lk, msum, P, T, O, tb, turb_planes);
             } else {
-                if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MD, false, true>, B, HB, fl, lk, msum, P, T, O);
-                else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MD, false, true>, B, HB, fl, lk, msum, P, T, O);
+                if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MD, false, true>, B, HB, fl, lk, msum, P, T, O, tb, turb_planes);
+                else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MD, false, true>, B, HB, fl, lk, msum, P, T, O, tb, turb_planes);
             }
         } else if (P.perx) {
-            if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O);
-            else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O);
+            if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O, Turb<real>{}, 0);
+            else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB, true>, B, HB, fl, lk, msum, P, T, O, Turb<real>{}, 0);
         } else {
-            if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB, false>, B, HB, fl, lk, msum, P, T, O);
-            else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB, false>, B, HB, fl, lk, msum, P, T, O);
+            if (sample) cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, true, BLOCK, MINB, false>, B, HB, fl, lk, msum, P, T, O, Turb<real>{}, 0);
+            else cudaLaunchKernelEx(&cfg, thermal_step_kernel<real, false, BLOCK, MINB, false>, B, HB, fl, lk, msum, P, T, O, Turb<real>{}, 0);
         }
         return check_launch(h, "thermal_step_kernel");
     }
@@ -687,6 +692,9 @@ template <typename real, typename S>
 int turb_publish(lbm_t *h, bool cells)
 {
     int rc = cells ? do_fluct<real, S>(h, (double)h->step, true) : LBM_OK;
+    // the cells now hold f_eq(1, u_b(step)) and the side array that velocity: their thermal state follows it (reading 28) ...
+    if (!rc && cells) rc = thermal_refresh<real>(h);
+    // ... before the side array moves on to u_b(step + 1), which the next launch re-expands
     if (!rc) rc = do_fluct<real, S>(h, (double)(h->step + 1), false);
     return rc;
 }
@@ -1037,7 +1045,10 @@ int set_inlet_theta_any(lbm_t *h, const in_t *theta_b)
     if (!theta_b) return fail(h, LBM_EINVAL, "set_inlet_theta: NULL");
     if (!h->thermal) return fail(h, LBM_ESTATE, "set_inlet_theta: thermal lattice is off (lbm_set_thermal)");
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inlet_theta: flags not set");
-    return h->fp64 ? do_inlet_theta<double, in_t>(h, theta_b) : do_inlet_theta<float, in_t>(h, theta_b);
+    int rc = h->fp64 ? do_inlet_theta<double, in_t>(h, theta_b) : do_inlet_theta<float, in_t>(h, theta_b);
+    // inflow fluctuations on: the side array holds u_b(step + 1); the cells belong to u_b(step) (reading 28)
+    if (!rc && h->nmodes > 0) rc = DISPATCH(h, turb_publish, h, true);
+    return rc;
 }
 
 bool has_eq_face(const int face[6])
@@ -1057,13 +1068,14 @@ int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
         return fail(h, LBM_EINVAL, "set_thermal: alpha must be > 0 and all arguments finite");
     if (h->s16) return fail(h, LBM_EINVAL, "set_thermal: not combinable with 16-bit population storage");
     if (h->inplace) return fail(h, LBM_EINVAL, "set_thermal: not combinable with in-place streaming");
-    if (h->nmodes > 0) return fail(h, LBM_EINVAL, "set_thermal: not combinable with inflow fluctuations");
     if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half() + h->ft_bytes()));
     CUDA_TRY(h, cudaMemsetAsync(h->th_ws, 0, 2 * h->th_half() + h->ft_bytes(), h->stream)); // theta_ref at rest (shifted storage), theta_b = theta_ref
     h->alpha = alpha; h->gbeta = g_beta; h->theta_ref = theta_ref; h->thermal = true;
     int rc = LBM_OK;
     // open faces (reading 27): the EQ_FIXED cells hold h_eq(theta_ref, u_b) until lbm_set_inlet_theta says otherwise
     if (h->have_flags && has_eq_face(h->face)) rc = h->fp64 ? do_inlet_theta<double, float>(h, nullptr) : do_inlet_theta<float, float>(h, nullptr);
+    // inflow fluctuations on: the cells hold u_b(step), the side array u_b(step + 1) — rewrite both lattices' cells for the velocity they have now (reading 28)
+    if (!rc && h->have_flags && h->nmodes > 0) rc = DISPATCH(h, turb_publish, h, true);
     CUDA_TRY(h, cudaStreamSynchronize(h->stream));
     return rc;
 }
@@ -1275,7 +1287,6 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
     DevGuard dg_(h);
     if (!h->have_flags) return fail(h, LBM_ESTATE, "set_inflow_turbulence: flags not set");
     if (n_modes < 0 || n_modes > MAX_MODES) return fail(h, LBM_EINVAL, "set_inflow_turbulence: n_modes out of range");
-    if (h->thermal && n_modes > 0) return fail(h, LBM_EINVAL, "set_inflow_turbulence: not combinable with the thermal lattice");
     auto rewrite = [&]() { return DISPATCH(h, turb_publish, h, true); };
     if (n_modes == 0) {
         if (h->nmodes == 0) return LBM_OK;

@@ -102,19 +102,36 @@ inline ThermalPtrs<real> make_thermal_ptrs(const real *A, real *B, const real *H
 template <typename real>
 struct OpenFaces { const real *fur; real *fuw; const real *ftr; real *ftw; };
 
-// DAMP: the damping-zone instantiation (lbm_set_damping together with the thermal lattice): the relaxation acceleration
-// sigma (u_t - u) and the buoyancy enter the same implicit half-force solve (collide<real, true, true>); launched only while
-// zones are configured, so the plain thermal kernel carries none of it.
+// DAMP: the open-boundary-stack instantiation, launched only while damping zones or inflow fluctuations are configured together
+// with the thermal lattice, so the plain thermal kernel carries none of it:
+//  * damping zones (lbm_set_damping): the relaxation acceleration sigma (u_t - u) and the buoyancy enter the same implicit
+//    half-force solve (collide<real, true, true>; outside the zones sigma = 0 takes the undamped branch);
+//  * synthetic inflow fluctuations (lbm_set_inflow_turbulence): the first turb_planes block rows carry the face slots, exactly as
+//    in step_body (lbm_step.cuh) — the boundary velocity of the step after this one goes into the half of the side array this
+//    launch writes; an EQ_FIXED cell re-expands BOTH equilibria from its slot's velocity every step, so its thermal state
+//    follows u_b + u' with no further code (DESIGN.md §4 reading 28).  turb_planes = 0 while there are no modes.
 template <typename real, bool MEAN, int BLOCK, int MINB, bool PERX = false, bool DAMP = false>
 __global__ void __launch_bounds__(BLOCK, MINB)
 thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-                    real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O)
+                    real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O,
+                    const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
 {
+    int zb = blockIdx.y;
+    if constexpr (DAMP) {
+        if (zb < turb_planes) {
+            asm volatile("griddepcontrol.launch_dependents;");
+            asm volatile("griddepcontrol.wait;" ::: "memory"); // the half written here is the one the previous launch reads
+            const int s = (zb * (int)gridDim.x + (int)blockIdx.x) * BLOCK + (int)threadIdx.x;
+            if (s < P.F) fluct_slot<real, false, real>(s, nullptr, nullptr, nullptr, O.fuw, nullptr, flags, tb, P);
+            return;
+        }
+        zb -= turb_planes;
+    }
     const unsigned c2 = blockIdx.x * BLOCK + threadIdx.x;
     if (c2 >= (unsigned)P.nxy) return;
     const int y = P.nx_magic ? (int)__umulhi(c2, P.nx_magic) : (int)(c2 / (unsigned)P.nx);
     const int x = (int)c2 - y * P.nx;
-    const int z = blockIdx.y == 0 ? P.nz - 1 : (int)blockIdx.y - 1; // the all-slow top plane first, not as the tail (lbm_step.cuh)
+    const int z = zb == 0 ? P.nz - 1 : zb - 1; // the all-slow top plane first, not as the tail (lbm_step.cuh)
     const int p = pidx(P, x, y, z);
     asm volatile("griddepcontrol.launch_dependents;");   // programmatic dependent launch, as in step_body (lbm_step.cuh)
     asm volatile("griddepcontrol.wait;" ::: "memory");

@@ -140,9 +140,7 @@ def test_thermal_error_behaviour(B):
     with pytest.raises(B.LbmError):
         sim.set_theta()  # flags were invalidated by set_boundaries
     sim.set_flags(np.zeros((8, 8), np.int32))
-    from paper_2607_04516_b200 import workloads as Wl
-    with pytest.raises(B.LbmError, match="thermal"):      # inflow fluctuations stay refused together with the thermal lattice
-        sim.set_inflow_turbulence(Wl.inflow_modes(4, 1, 0.1, 1.0, (0.05, 0, 0)), 0.01, 0.3, 0.0)
+
     sim.set_macros(); sim.set_theta()
     sim.step(3)
     assert float(np.abs(sim.get_theta().cpu().numpy() - 1.0).max()) == 0.0  # isothermal rest state is exact
@@ -505,3 +503,63 @@ def test_uniformly_warm_damped_box_settles_at_a_over_sigma_on_the_gpu(B):
         uz = sim.get_macros()[3].cpu().numpy()
         assert np.abs(uz - (wstar + (w1 - wstar) * q ** (k - 1))).max() < 2e-7, k
     sim.close()
+
+
+@pytest.mark.parametrize("fp64", [False, True])
+def test_whole_open_boundary_stack_on_a_thermal_run(B, fp64):
+    """Everything PAPER.md:175 / Table 1 lists, at once: equilibrium velocity faces with a warm inflow, the
+    global flux correction, sponge + buffer nudging, synthetic fluctuations on the active inflow cells — whose thermal state
+    follows the same velocity (reading 28) — buoyancy, LES, Coriolis, the time mean.  Fluctuations switched on before the
+    thermal lattice and after it, theta_b changed while they run, a second mode table from a developed state, off again."""
+    from paper_2607_04516_b200 import workloads as Wl
+    nx, ny, nz = 48, 20, 12
+    hm = np.zeros((ny, nx), np.int32); hm[5:10, 14:20] = 5; hm[11:15, 30:36] = 3
+    faces = (EQF, EQO, EQF, EQF, W, EQF)
+    modes = Wl.inflow_modes(32, 41, 2 * np.pi / 30, np.pi, convect=(0.05, 0.01, 0.0))
+    tol = TOL64 if fp64 else TOL32
+    for order in ("turbulence first", "thermal first"):
+        from oracle import Oracle
+        prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
+        thb = 1.0 + 0.4 * np.exp(-np.arange(nz) / 4.0)
+        u0 = np.broadcast_to(prof[:, None, None], (nz, ny, nx)).copy()
+        th0 = 1.0 + 0.05 * np.random.default_rng(8).standard_normal((nz, ny, nx))
+        target = np.stack([prof, 0.1 * prof, np.zeros(nz)])
+        args = (nx, ny, nz, 3e-3, 0.1, 1e-3, (0.0, 0, 0), faces)
+        o = Oracle(*args)
+        sim = B.Lbm(*args, fp64=fp64, want_mean=True)
+        for obj, kw in ((o, {}), (sim, {"f64": True})):
+            obj.set_flags(hm)
+            obj.set_inlet_profile(prof, 0.1 * prof, None, **kw)
+            obj.set_macros(None, u0, None, None, **kw)
+            obj.balance_flux()
+            obj.set_damping((4, 8, 3, 3, 0, 5), (0.05, 0.2, 0.05, 0.05, 0.0, 0.3), target)
+            if order == "turbulence first":
+                obj.set_inflow_turbulence(modes, 0.004, 2 * np.pi / 12, 2.5)
+            obj.set_thermal(0.02, 3e-4, 1.0)
+            obj.set_inlet_theta(thb, **kw)
+            obj.set_theta(th0, u0, None, None, **kw)
+            if order == "thermal first":
+                obj.set_inflow_turbulence(modes, 0.004, 2 * np.pi / 12, 2.5)
+            obj.mean_config(10, 5)
+        e_flow, e_th = errs(sim, o, 1.0)
+        assert e_flow <= tol and e_th <= tol, ("set-up", order, e_flow, e_th)
+        sim.step(61); o.step(61)
+        e_flow, e_th = errs(sim, o, 1.0)
+        assert e_flow <= tol and e_th <= tol, (order, fp64, e_flow, e_th)
+        gm = sim.get_mean(f64=True); om = o.get_mean()
+        assert gm[3] == om[3] == 11
+        assert max(float(np.abs(a.cpu().numpy() - b).max()) for a, b in zip(gm[:3], om[:3])) <= tol
+        for obj, kw in ((o, {}), (sim, {"f64": True})):
+            obj.set_inlet_theta(thb + 0.1, **kw)            # while the fluctuations run
+            obj.set_inflow_turbulence(Wl.inflow_modes(9, 5, 0.2, 2.0, convect=(0.04, 0.0, 0.0)), 0.002, 0.3)
+        e_flow, e_th = errs(sim, o, 1.0)
+        assert e_flow <= tol and e_th <= tol
+        sim.step(30); o.step(30)
+        e_flow, e_th = errs(sim, o, 1.0)
+        assert e_flow <= tol and e_th <= tol, ("second table", order, fp64, e_flow, e_th)
+        for obj in (o, sim):
+            obj.set_inflow_turbulence(None)
+        sim.step(20); o.step(20)
+        e_flow, e_th = errs(sim, o, 1.0)
+        assert e_flow <= tol and e_th <= tol, ("off", order, fp64, e_flow, e_th)
+        sim.close(); o.close()
