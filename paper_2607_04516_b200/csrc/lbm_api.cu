@@ -484,9 +484,14 @@ int do_set_macros(lbm_t *h, const in_t *rho, const in_t *ux, const in_t *uy, con
     for (int k = 0; k < 4 && !rc; ++k) rc = stage_in(h, src[k], bytes, h->L.scratch_bytes, &in[k]); // never fits: temp
     if (!rc) {
         const int B = 256;
-        init_kernel<real, S, in_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (S *)h->bufA(), (S *)nullptr, (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
-            (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
+        if (h->inplace)
+            init_kernel<real, S, in_t, 1><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+                (S *)h->bufA(), (S *)nullptr, (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+                (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
+        else
+            init_kernel<real, S, in_t, 0><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+                (S *)h->bufA(), (S *)nullptr, (real *)h->fu(), h->flags(), h->links(), (const in_t *)in[0].dev, (const in_t *)in[1].dev,
+                (const in_t *)in[2].dev, (const in_t *)in[3].dev, P);
         rc = check_launch(h, "init_kernel");
     }
     release_in(h, in, 4);
@@ -775,9 +780,14 @@ int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
     for (; staged < 4 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)P.N * sizeof(out_t), &o[staged]);
     if (!rc) {
         const int B = 256;
-        macros_kernel<real, S, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (const S *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
-            (const real *)h->th_state(), h->links());
+        if (h->inplace)
+            macros_kernel<real, S, out_t, 1><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+                (const S *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
+                (const real *)h->th_state(), h->links());
+        else
+            macros_kernel<real, S, out_t, 0><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+                (const S *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
+                (const real *)h->th_state(), h->links());
         rc = check_launch(h, "macros_kernel");
     }
     int rc2 = finish_out(h, o, staged);

@@ -473,20 +473,29 @@ __device__ __forceinline__ void ip_visit(const Params<real> &P, int q, int p, in
     }
 }
 
-// the stored (post-collision) state of a cell, whichever streaming scheme the handle uses; A = the current buffer
-template <typename real, typename S>
+// the stored (post-collision) state of a cell, whichever streaming scheme the handle uses; A = the current buffer.
+// IPM: -1 = decided at run time (P.ipq; the small set-up kernels), 0 = two buffers, 1 = in place — the whole-lattice kernels
+// (init, macros) are instantiated per scheme, so that the two-buffer instantiation carries none of the in-place code (with the
+// run-time branch macros_kernel took 448 us instead of 243 us on config 3: registers)
+template <typename real, typename S, int IPM = -1>
 __device__ __forceinline__ void load_cell_any(real (&g)[Q], const S *__restrict__ A, const Params<real> &P, int p, int x, int y, int z,
                                               uint8_t fl, uint32_t lk)
 {
-    if (P.ipq < 0) { load_cell(g, A, P.stride, p); return; }
-    ip_visit(P, P.ipq, p, x, y, z, fl, lk, [&](auto jc, long long e) { g[decltype(jc)::value] = ld_s<real>(A + e); });
+    if constexpr (IPM == 0) load_cell(g, A, P.stride, p);
+    else {
+        if (IPM < 0 && P.ipq < 0) { load_cell(g, A, P.stride, p); return; }
+        ip_visit(P, P.ipq, p, x, y, z, fl, lk, [&](auto jc, long long e) { g[decltype(jc)::value] = ld_s<real>(A + e); });
+    }
 }
-template <typename real, typename S>
+template <typename real, typename S, int IPM = -1>
 __device__ __forceinline__ void store_cell_any(S *__restrict__ A, const Params<real> &P, int p, int x, int y, int z, uint8_t fl,
                                                uint32_t lk, const real (&g)[Q])
 {
-    if (P.ipq < 0) { store_cell(A, P, p, x, y, z, fl, lk, g); return; }
-    ip_visit(P, P.ipq, p, x, y, z, fl, lk, [&](auto jc, long long e) { st_s(A + e, g[decltype(jc)::value]); });
+    if constexpr (IPM == 0) store_cell(A, P, p, x, y, z, fl, lk, g);
+    else {
+        if (IPM < 0 && P.ipq < 0) { store_cell(A, P, p, x, y, z, fl, lk, g); return; }
+        ip_visit(P, P.ipq, p, x, y, z, fl, lk, [&](auto jc, long long e) { st_s(A + e, g[decltype(jc)::value]); });
+    }
 }
 
 // ---- a3 / a6: EQ face cells -------------------------------------------------------------------------------------------

@@ -13,7 +13,7 @@ __device__ __forceinline__ real stored_theta_shift(const real *__restrict__ H, l
 }
 
 // local macros of the stored state (DESIGN.md §3 step 7)
-template <typename real, typename S, typename out_t>
+template <typename real, typename S, typename out_t, int IPM = 0>
 __global__ void macros_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
                               out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz, Params<real> P,
                               const real *__restrict__ H = nullptr, const uint32_t *__restrict__ links = nullptr)
@@ -28,8 +28,8 @@ __global__ void macros_kernel(const S *__restrict__ A, const uint8_t *__restrict
     real g[Q];
     Macro<real> m{real(1), real(0), real(0), real(0)};
     if (cls != SOLID) {
-        if (P.ipq < 0) load_cell(g, A, P.stride, p);
-        else load_cell_any(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? links[p] : 0u); // in-place streaming: the state lies at its destinations
+        if constexpr (IPM == 0) load_cell(g, A, P.stride, p);
+        else load_cell_any<real, S, 1>(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? links[p] : 0u); // in-place streaming: the state lies at its destinations
         if (H) P.Fz += P.gbeta * stored_theta_shift(H, P.stride, p); // Boussinesq: the buoyancy the cell's collision used
         m = local_macros(g, cls, P, damp_at(P, x, y, z));
     }

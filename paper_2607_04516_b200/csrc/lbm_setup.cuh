@@ -226,12 +226,12 @@ classify_tiled_kernel(uint8_t *__restrict__ flags, uint32_t *__restrict__ links,
 // step rewrites every slot of B that is ever read — own slots, mailboxes, ghost slots, EQ cells, sector completions — so
 // filling B too would be 76 B per cell of wasted writes), and publish its velocity to the outflow cells it feeds (both
 // halves of the double-buffered side array)
-template <typename real, typename S>
+template <typename real, typename S, int IPM = -1>
 __device__ __forceinline__ void store_cell_both(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const Params<real> &P,
                                                 int p, int x, int y, int z, uint8_t fl, uint32_t lk, const real (&g)[Q])
 {
-    store_cell_any(A, P, p, x, y, z, fl, lk, g);
-    if (B && P.ipq < 0) store_cell(B, P, p, x, y, z, fl, lk, g); // B == nullptr: whole-lattice writes (init, checkpoint) fill the current buffer only; in-place streaming: there is one buffer
+    store_cell_any<real, S, IPM>(A, P, p, x, y, z, fl, lk, g);
+    if (IPM != 1 && B && P.ipq < 0) store_cell(B, P, p, x, y, z, fl, lk, g); // B == nullptr: whole-lattice writes (init, checkpoint) fill the current buffer only; in-place streaming: there is one buffer
     const int cls = fl & CLASS_MASK;
     if ((fl & FEED_BIT) || cls == EQ_FIXED) {
         const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
@@ -420,7 +420,7 @@ __global__ void feed_kernel(S *__restrict__ dA, S *__restrict__ dB, real *__rest
 
 // ---- a4: init ------------------------------------------------------------------------------------------------------------
 // G0 = f_eq(rho0, u0) in FLUID and EQ_OUTFLOW cells (EQ_FIXED keep their boundary state; SOLID cells hold mailboxes)
-template <typename real, typename S, typename in_t>
+template <typename real, typename S, typename in_t, int IPM>
 __global__ void init_kernel(S *__restrict__ A, S *__restrict__ B, real *__restrict__ fu, const uint8_t *__restrict__ flags,
                             const uint32_t *__restrict__ links, const in_t *__restrict__ rho, const in_t *__restrict__ ux,
                             const in_t *__restrict__ uy, const in_t *__restrict__ uz, Params<real> P)
@@ -437,7 +437,7 @@ __global__ void init_kernel(S *__restrict__ A, S *__restrict__ B, real *__restri
     const real u = ux ? real(ux[c]) : real(0), v = uy ? real(uy[c]) : real(0), w = uz ? real(uz[c]) : real(0);
     real g[Q];
     equilibrium(g, drho, u, v, w);
-    store_cell_both(A, B, fu, P, p, x, y, z, fl, links[p], g);
+    store_cell_both<real, S, IPM>(A, B, fu, P, p, x, y, z, fl, links[p], g);
 }
 
 // ---- checkpoint ------------------------------------------------------------------------------------------------------------
