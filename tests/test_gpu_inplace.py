@@ -108,6 +108,10 @@ def test_every_face_rule_matches_the_oracle_in_fp64_and_fp32(B, faces, shape):
         assert n == on == 7
         em = max(float(np.abs(a.cpu().numpy().astype(np.float64) - b).max()) for a, b in zip(gm, om))
         assert em <= (TOL64 if fp64 else TOL32), (faces, shape, fp64, em)
+        # the population buffer is followed by the flag bytes and the link words in the workspace: no store of the in-place
+        # kernel (also not the unconditional ones towards dead cells in the halo) has reached them
+        np.testing.assert_array_equal(sim.get_flags(), o.get_flags())
+        np.testing.assert_array_equal(sim.get_links(), o.get_links())
         sim.close()
 
 
