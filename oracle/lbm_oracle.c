@@ -1079,4 +1079,16 @@ int oracle_get_theta(const oracle_t *o, double *theta)
     return 0;
 }
 
+/* the 7 thermal populations h_i of the stored state, [7][nz][ny][nx] (directions 0..6 of the flow lattice); SOLID cells report
+ * the rest state wT_i theta_ref — the format of the library's lbm_get_thermal_state */
+int oracle_get_thermal_state(const oracle_t *o, double *h)
+{
+    if (!o->thermal) return -3;
+    long N = (long)o->nx * o->ny * o->nz;
+    for (long cell = 0; cell < N; ++cell)
+        for (int i = 0; i < QT; ++i)
+            h[(long)i * N + cell] = o->cls[cell] == C_SOLID ? weight_t(i) * o->theta_ref : o->H[cell * QT + i];
+    return 0;
+}
+
 int oracle_heq(double theta, const double *u, double *out) { heq(theta, u, out); return 0; }

@@ -51,7 +51,7 @@ def _load():
                  "oracle_collide_cell_vec", "oracle_set_coriolis", "oracle_balance_flux",
                  "oracle_collide_cell_damped", "oracle_set_damping", "oracle_get_damping",
                  "oracle_vk_spectrum", "oracle_set_inflow_turbulence", "oracle_set_flags_mask",
-                 "oracle_set_theta", "oracle_get_theta", "oracle_heq", "oracle_round_half", "oracle_set_storage16", "oracle_set_thermal_walls", "oracle_set_inlet_theta"):
+                 "oracle_set_theta", "oracle_get_theta", "oracle_get_thermal_state", "oracle_heq", "oracle_round_half", "oracle_set_storage16", "oracle_set_thermal_walls", "oracle_set_inlet_theta"):
         getattr(lib, name).restype = C.c_int
     lib.oracle_set_thermal.restype = C.c_int
     lib.oracle_set_thermal.argtypes = [C.c_void_p, C.c_double, C.c_double, C.c_double]
@@ -301,6 +301,12 @@ class Oracle:
     def get_theta(self):
         out = np.zeros(self.shape)
         self._chk(self._lib.oracle_get_theta(C.c_void_p(self._h), out.ctypes.data_as(C.c_void_p)), "get_theta")
+        return out
+
+    def get_thermal_state(self):
+        """the 7 thermal populations of the stored state, [7][nz][ny][nx]"""
+        out = np.zeros((7,) + self.shape)
+        self._chk(self._lib.oracle_get_thermal_state(C.c_void_p(self._h), out.ctypes.data_as(C.c_void_p)), "get_thermal_state")
         return out
 
     def step(self, n=1):

@@ -45,6 +45,9 @@ def errs(sim, o, tref):
     th = sim.get_theta(f64=True).cpu().numpy()
     assert np.isfinite(th).all()
     e_th = float(np.abs(th - o.get_theta()).max())
+    # and the seven thermal populations themselves (lbm_get_thermal_state against the oracle's), boundary cells included: their
+    # first moment is the heat flux, which theta alone does not see
+    e_th = max(e_th, float(np.abs(sim.get_thermal_state() - o.get_thermal_state()).max()))
     return e_flow, e_th
 
 

@@ -438,16 +438,25 @@ def test_thermal_state_of_a_fluctuating_inlet_cell_follows_the_same_velocity():
     assert np.abs(d - 0.5 * theta_b * up0).max() < 1e-15, float(np.abs(d - 0.5 * theta_b * up0).max())
     assert np.abs(d).max() > 1e-4                                                 # and it is not a statement about zero
     assert np.abs(a.get_theta()[:, :, 2:] - b.get_theta()[:, :, 2:]).max() < 1e-15   # nothing further in has heard of it yet
-    # the cell written BY THE STEP carries u'(x, 1): second step, same law with the crest moved by one cell (omega = kappa)
-    ta, tb = a.get_theta().copy(), b.get_theta().copy()
-    ua = a.get_macros()[1][2, :, 0]
-    assert np.abs(ua - (U + 2 * uhat * np.cos(kap * y - om))).max() < 1e-15
-    # switched off: the inlet cell returns to the mean in both lattices — from then on the two runs receive the same heat
+    # the cell written BY THE STEP carries u'(x, k): its thermal populations are h_eq(theta_b, U + u'(y, k)) — zeroth moment
+    # theta_b, first moment theta_b (U + u'(y, k)) e_x (crest moving by one cell per step, omega = kappa) — and the flow side agrees
+    c7 = O.lattice()[0][:7].astype(float)
+    for k in (1, 2, 5):
+        a.step(k - a.get_step()); b.step(k - b.get_step())
+        upk = 2 * uhat * np.cos(kap * y - om * k)
+        h = a.get_thermal_state()[:, 2, :, 0]                                     # [7][ny] at the inlet column
+        assert np.abs(h.sum(axis=0) - theta_b).max() < 1e-15
+        flux = np.einsum("ia,iy->ay", c7, h)
+        assert np.abs(flux[0] - theta_b * (U + upk)).max() < 1e-16, k
+        assert np.abs(flux[1:]).max() < 1e-17
+        assert np.abs(a.get_macros()[1][2, :, 0] - (U + upk)).max() < 1e-15
+        hb = b.get_thermal_state()[:, 2, :, 0]                                     # without fluctuations: the mean
+        assert np.abs(np.einsum("ia,iy->ay", c7, hb)[0] - theta_b * U).max() < 1e-16
+    # switched off: the inlet cell returns to the mean in both lattices, at once and for the steps that follow
     a.set_inflow_turbulence(None)
-    ha, hb = a.get_theta()[:, :, 0], b.get_theta()[:, :, 0]
-    assert np.abs(ha - hb).max() < 1e-15
-    a.step(1); b.step(1)
-    # one step later the extra heat handed over at x = 1 is what the mean hands over: the difference of the two runs at x = 1
-    # only relaxes by diffusion / advection of what is already there (no new source): its y-mean stays zero
-    assert abs(float((a.get_theta()[2, :, 1] - b.get_theta()[2, :, 1]).mean())) < 1e-15
+    for _ in range(2):
+        ha, hb = a.get_thermal_state()[:, :, :, 0], b.get_thermal_state()[:, :, :, 0]
+        assert np.abs(ha - hb).max() < 1e-16
+        assert np.abs(a.get_macros()[1][:, :, 0] - U).max() < 1e-16
+        a.step(1); b.step(1)
     a.close(); b.close()
