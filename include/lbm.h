@@ -273,9 +273,19 @@ int lbm_mean_reset(lbm_t *h);
 int lbm_get_macros(lbm_t *h, float *rho, float *ux, float *uy, float *uz);
 int lbm_get_macros_f64(lbm_t *h, double *rho, double *ux, double *uy, double *uz);
 
+/* The same fields for the box lo[a] <= c_a < hi[a] only (axes x, y, z; 0 <= lo < hi <= n, else LBM_EINVAL): outputs are the
+ * box's own C-order arrays [hi[2]-lo[2]][hi[1]-lo[1]][hi[0]-lo[0]], host or device, any may be NULL.  What the paper's
+ * application reads back is of this kind — a horizontal plane at pedestrian height ("wind speeds ... at a pedestrian
+ * height of 2 m"), a vertical profile above a station (PAPER.md:137-148 lidar comparison) — and on a 1.2e9-cell lattice the four
+ * whole fields would be 19 GB. */
+int lbm_get_macros_box(lbm_t *h, const int lo[3], const int hi[3], float *rho, float *ux, float *uy, float *uz);
+int lbm_get_macros_box_f64(lbm_t *h, const int lo[3], const int hi[3], double *rho, double *ux, double *uy, double *uz);
+
 /* mean = sum / n_samples (0 where n_samples == 0 and in SOLID cells); n_samples is a host pointer, may be NULL */
 int lbm_get_mean(lbm_t *h, float *ux, float *uy, float *uz, long *n_samples);
 int lbm_get_mean_f64(lbm_t *h, double *ux, double *uy, double *uz, long *n_samples);
+/* the time mean of a box (as lbm_get_macros_box) */
+int lbm_get_mean_box(lbm_t *h, const int lo[3], const int hi[3], float *ux, float *uy, float *uz, long *n_samples);
 
 /* Parity exports.  flags: uint8 [nz][ny][nx] cell classes.  links: uint32 [nz][ny][nx], bit i (1..18) set
  * iff pulling direction i into that FLUID cell takes the bounce-back branch; 0 for non-FLUID cells. */

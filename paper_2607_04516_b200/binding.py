@@ -25,7 +25,7 @@ SYMBOLS = [
     "lbm_set_inlet_profile", "lbm_set_inlet_profile_f64", "lbm_set_inlet_plane", "lbm_set_inlet_plane_f64",
     "lbm_feed_inlet", "lbm_set_macros", "lbm_set_macros_f64", "lbm_step", "lbm_mean_config", "lbm_mean_reset",
     "lbm_get_macros", "lbm_get_macros_f64", "lbm_get_mean", "lbm_get_mean_f64", "lbm_get_flags", "lbm_get_links",
-    "lbm_get_state", "lbm_set_state", "lbm_get_state_box", "lbm_set_state_box", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
+    "lbm_get_state", "lbm_set_state", "lbm_get_state_box", "lbm_set_state_box", "lbm_get_macros_box", "lbm_get_macros_box_f64", "lbm_get_mean_box", "lbm_get_step", "lbm_set_step", "lbm_sync", "lbm_last_error",
     "lbm_launch_count", "lbm_lattice", "lbm_set_variant", "lbm_set_coriolis", "lbm_balance_flux",
     "lbm_set_damping", "lbm_set_inflow_turbulence", "lbm_set_flags_mask", "lbm_set_flags_mesh",
     "lbm_set_thermal", "lbm_set_theta", "lbm_set_theta_f64", "lbm_get_theta", "lbm_get_theta_f64",
@@ -89,6 +89,9 @@ def load_library():
     lib.lbm_set_state.argtypes = [vp, vp]
     lib.lbm_get_state_box.argtypes = [vp, vp, vp, vp]
     lib.lbm_set_state_box.argtypes = [vp, vp, vp, vp]
+    lib.lbm_get_macros_box.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.lbm_get_macros_box_f64.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.lbm_get_mean_box.argtypes = [vp, vp, vp, vp, vp, vp, C.POINTER(C.c_long)]
     lib.lbm_get_step.argtypes = [vp]
     lib.lbm_get_step.restype = l
     lib.lbm_set_step.argtypes = [vp, l]
@@ -442,6 +445,24 @@ class Lbm:
         a = self._new(self._torch.float64, shape)
         self._chk(self._lib.lbm_get_state_box(self._h, lo.ctypes.data, hi.ctypes.data, a.data_ptr()), "get_state_box")
         return a
+
+    def get_macros_box(self, lo, hi, f64=False):
+        """rho, ux, uy, uz of the box lo <= (x, y, z) < hi: device tensors [hi_z-lo_z][hi_y-lo_y][hi_x-lo_x]"""
+        lo, hi = self._box(lo, hi)
+        t = self._torch
+        shape = (max(int(hi[2] - lo[2]), 1), max(int(hi[1] - lo[1]), 1), max(int(hi[0] - lo[0]), 1))
+        arrs = [self._new(t.float64 if f64 else t.float32, shape) for _ in range(4)]
+        fn = self._lib.lbm_get_macros_box_f64 if f64 else self._lib.lbm_get_macros_box
+        self._chk(fn(self._h, lo.ctypes.data, hi.ctypes.data, *[a.data_ptr() for a in arrs]), "get_macros_box")
+        return tuple(arrs)
+
+    def get_mean_box(self, lo, hi):
+        lo, hi = self._box(lo, hi)
+        shape = (max(int(hi[2] - lo[2]), 1), max(int(hi[1] - lo[1]), 1), max(int(hi[0] - lo[0]), 1))
+        arrs = [self._new(self._torch.float32, shape) for _ in range(3)]
+        n = C.c_long()
+        self._chk(self._lib.lbm_get_mean_box(self._h, lo.ctypes.data, hi.ctypes.data, *[a.data_ptr() for a in arrs], C.byref(n)), "get_mean_box")
+        return arrs[0], arrs[1], arrs[2], n.value
 
     def set_state_box(self, lo, hi, f):
         lo, hi = self._box(lo, hi)

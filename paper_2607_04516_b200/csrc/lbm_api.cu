@@ -768,26 +768,37 @@ int do_step(lbm_t *h, int n)
     return LBM_OK;
 }
 
+// box == nullptr: the whole lattice
+inline Box whole_or(const lbm_t *h, const Box *box)
+{
+    if (box) return *box;
+    Box b{};
+    b.bn[0] = h->nx; b.bn[1] = h->ny; b.bn[2] = h->nz;
+    return b;
+}
+
 template <typename real, typename S, typename out_t>
-int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
+int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz, const Box *box = nullptr)
 {
     if (!h->have_flags) return fail(h, LBM_ESTATE, "get_macros: flags not set");
     const Params<real> P = make_params<real>(h);
+    const Box bx = whole_or(h, box);
+    const long long NB = (long long)bx.bn[0] * bx.bn[1] * bx.bn[2];
     OutBuf o[4];
     out_t *dst[4] = {rho, ux, uy, uz};
     int rc = LBM_OK;
     int staged = 0;
-    for (; staged < 4 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)P.N * sizeof(out_t), &o[staged]);
+    for (; staged < 4 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)NB * sizeof(out_t), &o[staged]);
     if (!rc) {
         const int B = 256;
         if (h->inplace)
-            macros_kernel<real, S, out_t, 1><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            macros_kernel<real, S, out_t, 1><<<blocks_for(NB, B), B, 0, h->stream>>>(
                 (const S *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
-                (const real *)h->th_state(), h->links());
+                (const real *)h->th_state(), h->links(), bx);
         else
-            macros_kernel<real, S, out_t, 0><<<blocks_for(P.N, B), B, 0, h->stream>>>(
+            macros_kernel<real, S, out_t, 0><<<blocks_for(NB, B), B, 0, h->stream>>>(
                 (const S *)h->state(), h->flags(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, (out_t *)o[3].dev, P,
-                (const real *)h->th_state(), h->links());
+                (const real *)h->th_state(), h->links(), bx);
         rc = check_launch(h, "macros_kernel");
     }
     int rc2 = finish_out(h, o, staged);
@@ -795,21 +806,23 @@ int do_get_macros(lbm_t *h, out_t *rho, out_t *ux, out_t *uy, out_t *uz)
 }
 
 template <typename real, typename S, typename out_t>
-int do_get_mean(lbm_t *h, out_t *ux, out_t *uy, out_t *uz, long *n_samples)
+int do_get_mean(lbm_t *h, out_t *ux, out_t *uy, out_t *uz, long *n_samples, const Box *box = nullptr)
 {
     if (!h->want_mean) return fail(h, LBM_ESTATE, "get_mean: handle created without mean sums");
     const Params<real> P = make_params<real>(h);
+    const Box bx = whole_or(h, box);
+    const long long NB = (long long)bx.bn[0] * bx.bn[1] * bx.bn[2];
     if (n_samples) *n_samples = h->mcount;
     OutBuf o[3];
     out_t *dst[3] = {ux, uy, uz};
     int rc = LBM_OK;
     int staged = 0;
-    for (; staged < 3 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)P.N * sizeof(out_t), &o[staged]);
+    for (; staged < 3 && !rc; ++staged) rc = stage_out(h, dst[staged], (size_t)NB * sizeof(out_t), &o[staged]);
     if (!rc) {
         const int B = 256;
         const double inv = h->mcount > 0 ? 1.0 / (double)h->mcount : 0.0;
-        mean_out_kernel<real, out_t><<<blocks_for(P.N, B), B, 0, h->stream>>>(
-            (const real *)h->mean(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, inv, P);
+        mean_out_kernel<real, out_t><<<blocks_for(NB, B), B, 0, h->stream>>>(
+            (const real *)h->mean(), (out_t *)o[0].dev, (out_t *)o[1].dev, (out_t *)o[2].dev, inv, P, bx);
         rc = check_launch(h, "mean_out_kernel");
     }
     int rc2 = finish_out(h, o, staged);
@@ -830,14 +843,6 @@ int do_get_links(lbm_t *h, uint32_t *links)
     return rc ? rc : rc2;
 }
 
-// box == nullptr: the whole lattice
-inline Box whole_or(const lbm_t *h, const Box *box)
-{
-    if (box) return *box;
-    Box b{};
-    b.bn[0] = h->nx; b.bn[1] = h->ny; b.bn[2] = h->nz;
-    return b;
-}
 template <typename real, typename S>
 int do_get_state(lbm_t *h, double *f, const Box *box)
 {
@@ -1552,6 +1557,37 @@ int lbm_set_state_box(lbm_t *h, const int lo[3], const int hi[3], const double *
     rc = DISPATCH(h, do_set_state, h, f, &bx);
     if (!rc && h->nmodes > 0) rc = DISPATCH(h, turb_publish, h, false);
     return rc;
+}
+
+int lbm_get_macros_box(lbm_t *h, const int lo[3], const int hi[3], float *rho, float *ux, float *uy, float *uz)
+{
+    if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_macros_box: flags not set");
+    Box bx{};
+    int rc = check_box(h, lo, hi, &bx, "get_macros_box");
+    if (rc) return rc;
+    return DISPATCH_T(h, do_get_macros, float, h, rho, ux, uy, uz, &bx);
+}
+int lbm_get_macros_box_f64(lbm_t *h, const int lo[3], const int hi[3], double *rho, double *ux, double *uy, double *uz)
+{
+    if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_macros_box: flags not set");
+    Box bx{};
+    int rc = check_box(h, lo, hi, &bx, "get_macros_box");
+    if (rc) return rc;
+    return DISPATCH_T(h, do_get_macros, double, h, rho, ux, uy, uz, &bx);
+}
+int lbm_get_mean_box(lbm_t *h, const int lo[3], const int hi[3], float *ux, float *uy, float *uz, long *n_samples)
+{
+    if (!h) return LBM_EINVAL;
+    DevGuard dg_(h);
+    if (!h->have_flags) return fail(h, LBM_ESTATE, "get_mean_box: flags not set");
+    Box bx{};
+    int rc = check_box(h, lo, hi, &bx, "get_mean_box");
+    if (rc) return rc;
+    return DISPATCH_T(h, do_get_mean, float, h, ux, uy, uz, n_samples, &bx);
 }
 
 long lbm_get_step(const lbm_t *h) { return h ? h->step : -1; }

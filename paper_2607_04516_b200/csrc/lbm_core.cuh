@@ -581,6 +581,18 @@ __device__ __forceinline__ void cell_xyz(const Params<real> &P, int c, int &x, i
     z = r / P.ny;
 }
 
+// a sub-box lo <= (x,y,z) < lo + bn of the lattice (the whole lattice: lo = 0, bn = n); cell c of the box, C order [bz][by][bx]
+struct Box { int lo[3], bn[3]; };
+__device__ __forceinline__ bool box_cell(const Box &bx, int c, int &x, int &y, int &z)
+{
+    if (c >= bx.bn[0] * bx.bn[1] * bx.bn[2]) return false;
+    x = bx.lo[0] + c % bx.bn[0];
+    const int r = c / bx.bn[0];
+    y = bx.lo[1] + r % bx.bn[1];
+    z = bx.lo[2] + r / bx.bn[1];
+    return true;
+}
+
 __host__ __device__ inline double weight_f64(int i) { return i == 0 ? 1.0 / 3.0 : (i <= 6 ? 1.0 / 18.0 : 1.0 / 36.0); }
 
 } // namespace lbmk

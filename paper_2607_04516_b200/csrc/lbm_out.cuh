@@ -16,12 +16,11 @@ __device__ __forceinline__ real stored_theta_shift(const real *__restrict__ H, l
 template <typename real, typename S, typename out_t, int IPM = 0>
 __global__ void macros_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, out_t *__restrict__ rho,
                               out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz, Params<real> P,
-                              const real *__restrict__ H = nullptr, const uint32_t *__restrict__ links = nullptr)
+                              const real *__restrict__ H, const uint32_t *__restrict__ links, const Box bx)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= P.N) return;
     int x, y, z;
-    cell_xyz(P, c, x, y, z);
+    if (!box_cell(bx, c, x, y, z)) return; // outputs are the box's own C-order arrays (the whole lattice: the box is the lattice)
     const int p = pidx(P, x, y, z);
     const uint8_t fl = flags[p];
     const int cls = fl & CLASS_MASK;
@@ -41,12 +40,11 @@ __global__ void macros_kernel(const S *__restrict__ A, const uint8_t *__restrict
 
 template <typename real, typename out_t>
 __global__ void mean_out_kernel(const real *__restrict__ msum, out_t *__restrict__ ux, out_t *__restrict__ uy, out_t *__restrict__ uz,
-                                double inv_count, Params<real> P)
+                                double inv_count, Params<real> P, const Box bx)
 {
     const int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= P.N) return;
     int x, y, z;
-    cell_xyz(P, c, x, y, z);
+    if (!box_cell(bx, c, x, y, z)) return;
     const int p = pidx(P, x, y, z);
     if (ux) ux[c] = out_t(double(msum[p]) * inv_count);
     if (uy) uy[c] = out_t(double(msum[P.stride + p]) * inv_count);

@@ -443,16 +443,6 @@ __global__ void init_kernel(S *__restrict__ A, S *__restrict__ B, real *__restri
 // ---- checkpoint ------------------------------------------------------------------------------------------------------------
 // f [19][bz][by][bx] double, NOT shifted, of the box lo <= (x,y,z) < lo + bn (the whole lattice: lo = 0, bn = n).  SOLID cells
 // export the rest state w_i (their slots are mailboxes).
-struct Box { int lo[3], bn[3]; };
-__device__ __forceinline__ bool box_cell(const Box &bx, int c, int &x, int &y, int &z)
-{
-    if (c >= bx.bn[0] * bx.bn[1] * bx.bn[2]) return false;
-    x = bx.lo[0] + c % bx.bn[0];
-    const int r = c / bx.bn[0];
-    y = bx.lo[1] + r % bx.bn[1];
-    z = bx.lo[2] + r / bx.bn[1];
-    return true;
-}
 template <typename real, typename S>
 __global__ void state_out_kernel(const S *__restrict__ A, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
                                  double *__restrict__ f, Params<real> P, const Box bx)

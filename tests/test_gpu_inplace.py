@@ -343,7 +343,7 @@ def test_state_box_is_a_slice_of_the_state_and_restores_slab_by_slab(B, fp64, in
         args = (nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), faces)
 
         def fresh(presteps):
-            sim = B.Lbm(*args, fp64=fp64, inplace=inplace)
+            sim = B.Lbm(*args, fp64=fp64, inplace=inplace, want_mean=True)
             sim.set_flags(hm)
             sim.set_inlet_profile(prof, 0.1 * prof, None, f64=True)
             sim.set_macros(None, ux0, uy0, None, f64=True)
@@ -356,6 +356,26 @@ def test_state_box_is_a_slice_of_the_state_and_restores_slab_by_slab(B, fp64, in
             assert np.array_equal(box, full[:, lo[2]:hi[2], lo[1]:hi[1], lo[0]:hi[0]]), (lo, hi)
             dev = src.get_state_box(lo, hi).cpu().numpy()      # device destination
             assert np.array_equal(dev, box)
+        # lbm_get_macros_box / lbm_get_mean_box: a pedestrian-height plane, a vertical profile, a box — slices of the whole fields
+        src.mean_config(16, 2)
+        src.step(6); src.set_step(15)      # back on step 15 for what follows; six more steps of the same state, three sampled
+        full = src.get_state(out="host")
+        whole = [a.cpu().numpy() for a in src.get_macros(f64=True)]
+        whole32 = [a.cpu().numpy() for a in src.get_macros()]
+        *mean, nm = src.get_mean()
+        assert nm == 3
+        for lo, hi in [((0, 0, 1), (nx, ny, 2)), ((7, 4, 0), (8, 5, nz)), ((5, 2, 1), (20, 9, 4))]:
+            sl = (slice(lo[2], hi[2]), slice(lo[1], hi[1]), slice(lo[0], hi[0]))
+            for a, w in zip(src.get_macros_box(lo, hi, f64=True), whole):
+                assert np.array_equal(a.cpu().numpy(), w[sl])
+            for a, w in zip(src.get_macros_box(lo, hi), whole32):
+                assert np.array_equal(a.cpu().numpy(), w[sl])
+            *mb, nb = src.get_mean_box(lo, hi)
+            assert nb == 3
+            for a, w in zip(mb, mean):
+                assert np.array_equal(a.cpu().numpy(), w.cpu().numpy()[sl])
+        with pytest.raises(B.LbmError):
+            src.get_macros_box((0, 0, 0), (nx, ny, nz + 1))
         ref = fresh(4)
         ref.set_state(full)
         ref.set_step(15)
