@@ -889,10 +889,12 @@ def test_mesh_on_terrain_heightmap_and_user_mask(B):
     sim.close()
 
 
+@pytest.mark.parametrize("inplace", [False, True])
 @pytest.mark.parametrize("fp64", [False, True])
-def test_flow_around_mesh_voxelised_overhangs_matches_the_oracle(B, fp64):
+def test_flow_around_mesh_voxelised_overhangs_matches_the_oracle(B, fp64, inplace):
     """Solids that no heightmap can express (a slab on two legs, a floating sphere): the step kernel works from the flags
-    alone — bounce-back from below and above, sector completion inside hollow rows; 100 steps against the oracle."""
+    alone — bounce-back from below and above, sector completion inside hollow rows; 100 steps against the oracle.
+    inplace: the same on one population buffer (wall links in all 18 directions through the link slots)."""
     from oracle import Oracle, mesh_voxel
     from paper_2607_04516_b200 import workloads as W
     nx, ny, nz = 56, 36, 24
@@ -903,7 +905,7 @@ def test_flow_around_mesh_voxelised_overhangs_matches_the_oracle(B, fp64):
     args = (nx, ny, nz, 2e-3, 0.1, 1e-4, (0, 0, 0), (3, 4, 2, 2, 1, 2))
     o = Oracle(*args)
     o.set_flags_mask(hm, mesh_voxel.voxelise(tri, nx, ny, nz))
-    sim = B.Lbm(*args, fp64=fp64)
+    sim = B.Lbm(*args, fp64=fp64, inplace=inplace)
     sim.set_flags_mesh(tri, hm)
     check_flags_links(sim, o)
     fl = o.get_flags()
@@ -912,10 +914,10 @@ def test_flow_around_mesh_voxelised_overhangs_matches_the_oracle(B, fp64):
     for obj, kw in ((o, {}), (sim, {"f64": True})):
         obj.set_inlet_profile(prof, None, None, **kw)
         obj.set_macros(None, ux0, None, None, **kw)
-    o.step(100)
-    sim.step(100)
+    o.step(101)
+    sim.step(101)
     e = max_err(sim, o, f64=fp64)
-    assert e <= (TOL64 if fp64 else TOL32), (fp64, e)
+    assert e <= (TOL64 if fp64 else TOL32), (fp64, inplace, e)
     sim.close()
 
 
