@@ -125,8 +125,13 @@ def test_a_lattice_too_large_for_two_buffers_runs_in_place(B):
     import ctypes as C
     lib = B.load_library()
     nb2, nb1 = C.c_size_t(), C.c_size_t()
-    assert lib.lbm_workspace_bytes(nx, ny, nz, 0, B.PREC_F32, C.byref(nb2)) == 0
-    assert lib.lbm_workspace_bytes(nx, ny, nz, 0, B.PREC_F32 | B.STREAM_INPLACE, C.byref(nb1)) == 0
+    while True:     # (a board that reports more memory than this pool's 191.5 GB gets a taller box: the point is "cannot be double-buffered")
+        assert lib.lbm_workspace_bytes(nx, ny, nz, 0, B.PREC_F32, C.byref(nb2)) == 0
+        assert lib.lbm_workspace_bytes(nx, ny, nz, 0, B.PREC_F32 | B.STREAM_INPLACE, C.byref(nb1)) == 0
+        if nb2.value > total or nz >= 480:
+            break
+        nz += 10
+    prof = W.log_law_profile(nz, 0.08, 20.0, 0.2)
     print(f"two buffers {nb2.value / 1e9:.1f} GB, in place {nb1.value / 1e9:.1f} GB, device {total / 1e9:.1f} GB")
     assert nb2.value > total, "the point of this test is a lattice that cannot be double-buffered on this device"
     if nb1.value + 6e9 > free:
@@ -203,7 +208,7 @@ def test_a_lattice_too_large_for_two_buffers_runs_in_place(B):
     e0.record(); sim.step(50); e1.record(); torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / 50
     assert bool(torch.isfinite(sim.get_macros()[1]).all())
-    print(f"2000x2000x300 in place: worst sampled-box error {worst:.3e}; {ms:.1f} ms per step = {nx * ny * nz / ms / 1e3:.0f} MLUPS")
+    print(f"2000x2000x{nz} in place: worst sampled-box error {worst:.3e}; {ms:.1f} ms per step = {nx * ny * nz / ms / 1e3:.0f} MLUPS")
     sim.close()
     del sim, g
     torch.cuda.empty_cache()
