@@ -68,9 +68,9 @@ enum { LBM_PREC_F32 = 0, LBM_PREC_F64 = 1, LBM_PREC_F32_S16 = 2 };
  * step to step — so a lattice takes about half the memory (config 5's 2.9e8 cells: 24 GB instead of 46 GB; 1.2e9 FP32 cells fit
  * one B200), for the same 153 B per cell and step and the same arithmetic: every call works the same and returns the same
  * values (lbm_get_state / lbm_set_state exchange the same post-collision populations).  Combinable with all three precisions,
- * every face type, damping zones, flux correction, synthetic inflow fluctuations, the time mean and lbm_feed_inlet (either side);
- * NOT with the thermal lattice (lbm_set_thermal returns LBM_EINVAL), and lbm_set_variant has no effect (one launch shape: one cell
- * per thread, one launch per step). */
+ * every face type, damping zones, flux correction, synthetic inflow fluctuations, the time mean, lbm_feed_inlet (either side) and
+ * the thermal lattice (whose seven populations per cell stay double-buffered: 19 + 14 instead of 38 + 14 stored values per cell);
+ * lbm_set_variant has no effect (one launch shape: one cell per thread, one launch per step). */
 #define LBM_STREAM_INPLACE 16
 
 /* Bytes of device workspace a handle of this size needs (two population buffers of 19 stored values per cell — one with
@@ -215,7 +215,7 @@ int lbm_set_inflow_turbulence(lbm_t *h, int n_modes, const double *modes, double
  * (lbm_set_damping) combine with it: the relaxation acceleration and the buoyancy enter the same implicit half-force solve.
  * So do the synthetic inflow fluctuations (lbm_set_inflow_turbulence): an active inflow cell holds h_eq(theta_b, u_b + u') beside
  * f_eq(1, u_b + u'), one boundary velocity for both lattices (DESIGN.md §4 reading 28); theta_b itself does not fluctuate.
- * 16-bit storage and in-place streaming must be off (LBM_EINVAL).  alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
+ * 16-bit storage must be off (LBM_EINVAL); with LBM_STREAM_INPLACE the flow lattice streams in place and the thermal one stays double-buffered.  alpha > 0 (lattice units); LBM_ENOMEM / LBM_ECUDA if the allocation fails.  Synchronises. */
 int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref);
 /* Prescribed temperature of the EQ_FIXED cells by level (reading 27): theta_b[nz], host or device; the cells' thermal state
  * becomes h_eq(theta_b(z), u_b) at once and is re-expanded from it every step.  A later lbm_set_inlet_profile / _plane,

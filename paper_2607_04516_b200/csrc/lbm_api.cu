@@ -599,9 +599,14 @@ int launch_ip_step(lbm_t *h, const Params<real> &P, bool sample)
     L.fuw = (real *)h->fu() + (size_t)(h->cur ? 0 : 3) * P.F;
     L.params = &P;
     L.fum = h->fum(); L.modes = h->modes(); L.nmodes = h->nmodes; L.t = (double)(h->step + 2);
+    if (h->thermal) { // the thermal populations stay double-buffered; their halves follow the parity as the side arrays do
+        real *ft = (real *)h->ft();
+        L.HA = h->th_state(); L.HB = h->th_other();
+        L.ftr = ft + (size_t)(h->cur ? 1 : 0) * P.F; L.ftw = ft + (size_t)(h->cur ? 0 : 1) * P.F;
+    }
     L.stream = h->stream;
     ip_launch(L);
-    return check_launch(h, "ip_step_kernel");
+    return check_launch(h, h->thermal ? "ip_thermal_step_kernel" : "ip_step_kernel");
 }
 
 template <typename real, typename S>
@@ -1082,7 +1087,6 @@ int lbm_set_thermal(lbm_t *h, double alpha, double g_beta, double theta_ref)
     if (!(alpha > 0.0) || !std::isfinite(alpha) || !std::isfinite(g_beta) || !std::isfinite(theta_ref))
         return fail(h, LBM_EINVAL, "set_thermal: alpha must be > 0 and all arguments finite");
     if (h->s16) return fail(h, LBM_EINVAL, "set_thermal: not combinable with 16-bit population storage");
-    if (h->inplace) return fail(h, LBM_EINVAL, "set_thermal: not combinable with in-place streaming");
     if (!h->th_ws) CUDA_TRY(h, cudaMalloc((void **)&h->th_ws, 2 * h->th_half() + h->ft_bytes()));
     CUDA_TRY(h, cudaMemsetAsync(h->th_ws, 0, 2 * h->th_half() + h->ft_bytes(), h->stream)); // theta_ref at rest (shifted storage), theta_b = theta_ref
     h->alpha = alpha; h->gbeta = g_beta; h->theta_ref = theta_ref; h->thermal = true;

@@ -21,6 +21,12 @@ struct IpLaunch {
     const double *modes;
     int nmodes;
     double t;
+    // thermal lattice on (lbm_set_thermal): its two buffers stay double (HA = the one that goes with the current state, HB = the
+    // one this step writes) and the thermal companion of the side array (halves to read / to write); null while it is off
+    const void *HA;
+    void *HB;
+    const void *ftr;
+    void *ftw;
     cudaStream_t stream;
 };
 

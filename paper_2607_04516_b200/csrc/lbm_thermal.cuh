@@ -14,6 +14,7 @@
 #pragma once
 #include "lbm_core.cuh"
 #include "lbm_step.cuh"
+#include "lbm_inplace.cuh"
 
 namespace lbmk {
 
@@ -110,11 +111,14 @@ struct OpenFaces { const real *fur; real *fuw; const real *ftr; real *ftw; };
 //    in step_body (lbm_step.cuh) — the boundary velocity of the step after this one goes into the half of the side array this
 //    launch writes; an EQ_FIXED cell re-expands BOTH equilibria from its slot's velocity every step, so its thermal state
 //    follows u_b + u' with no further code (DESIGN.md §4 reading 28).  turb_planes = 0 while there are no modes.
-template <typename real, bool MEAN, int BLOCK, int MINB, bool PERX = false, bool DAMP = false>
-__global__ void __launch_bounds__(BLOCK, MINB)
-thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
-                    real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O,
-                    const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
+// IP: the FLOW lattice streams in place (one buffer; lbm_inplace.cuh: loads through I.rd, every outgoing population over the
+// address its opposite was read from, wall links through I.nx, ghost slots by slot and cell); the seven thermal populations
+// stay double-buffered (they are 7 of 26 values per cell), so everything thermal below is the same in both schemes.
+template <typename real, bool MEAN, int BLOCK, bool PERX, bool DAMP, bool IP>
+__device__ __forceinline__ void thermal_step_body(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags,
+                                                  const uint32_t *__restrict__ links, real *__restrict__ msum, const Params<real> &P,
+                                                  const ThermalPtrs<real> &T, const OpenFaces<real> &O, const Turb<real> &tb,
+                                                  const int turb_planes, const IpPtrs<real> &I)
 {
     int zb = blockIdx.y;
     if constexpr (DAMP) {
@@ -146,12 +150,25 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
         else if constexpr (PERX && dir_cx(i) == -1) return pR;
         else return p;
     };
+    real g[Q], t[QT];
+    auto ipat = [&](auto ic) { // IP: the cell index that goes with I.rd[i] / I.nx[i] (lbm_inplace.cuh)
+        constexpr int i = decltype(ic)::value;
+        if constexpr (PERX && i > 0 && (i & 1) == 0 && dir_cx(i) == -1) return pR;
+        else return p;
+    };
+    // IP: the outgoing flow population j overwrites the address the incoming opp(j) was read from
+    auto ip_store_all = [&]() {
+        static_for<0, Q>([&](auto jc) {
+            constexpr int j = decltype(jc)::value;
+            I.rd[dir_opp(j)][ipat(std::integral_constant<int, dir_opp(j)>{})] = g[j];
+        });
+    };
     // as in step_kernel's SPEC instantiations: all 26 pulls are issued before the flag byte has arrived (no dependent
     // round trip; a SOLID cell then costs its reads), pinned by volatile asm so that the flag test cannot move above them
-    real g[Q], t[QT];
     static_for<0, Q>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
-        g[i] = ld_pinned(T.gsrc[i] + psrc(ic));
+        if constexpr (IP) g[i] = ld_pinned(I.rd[i] + ipat(ic));
+        else g[i] = ld_pinned(T.gsrc[i] + psrc(ic));
     });
     static_for<0, QT>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
@@ -184,10 +201,12 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
     }
     // fast path, warp-uniform: every lane a plain FLUID cell (no wall link, no ghost slot, nothing to complete)
     if (__all_sync(__activemask(), fl == 0)) {
-        static_for<0, Q>([&](auto ic) {
-            constexpr int i = decltype(ic)::value;
-            T.gdst[i][p] = g[i];
-        });
+        if constexpr (IP) ip_store_all();
+        else
+            static_for<0, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                T.gdst[i][p] = g[i];
+            });
         static_for<0, QT>([&](auto ic) {
             constexpr int i = decltype(ic)::value;
             T.tdst[i][p] = t[i];
@@ -205,7 +224,7 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
             static_for<0, Q>([&](auto ic) {
                 constexpr int i = decltype(ic)::value;
                 if ((lk >> i) & 1u) {
-                    B[(long long)i * P.stride + p] = real(0);
+                    if constexpr (!IP) B[(long long)i * P.stride + p] = real(0); // (in place: the flow sectors were read whole)
                     if constexpr (i < QT) HB[(long long)i * P.stride + p] = real(0);
                 }
             });
@@ -228,12 +247,23 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
     // own slots and wall mailboxes of both lattices (store_cell / store_cell_thermal with the EDGE part masked off), then ONE
     // ghost-store sequence for both: the face logic per direction is shared, which halves that code (the fused body is larger
     // than the instruction cache)
-    store_cell(B, P, p, x, y, z, (uint8_t)(fl & ~EDGE_BIT), lk, g);
+    if constexpr (IP) {
+        ip_store_all(); // towards a dead cell this fills the link's unused slot
+        if (fl & SLOW_BIT)
+            static_for<1, Q>([&](auto ic) {
+                constexpr int i = decltype(ic)::value;
+                if ((lk >> i) & 1u) I.nx[i][ipat(ic)] = g[dir_opp(i)];
+            });
+    } else store_cell(B, P, p, x, y, z, (uint8_t)(fl & ~EDGE_BIT), lk, g);
     store_cell_thermal(HB, P, p, x, y, z, (uint8_t)(fl & ~EDGE_BIT), lk, t);
     if (fl & EDGE_BIT)
         ghost_stores(P, x, y, z, lk, [&](int i, int pt, auto jc) {
             constexpr int j = decltype(jc)::value;
-            B[(long long)i * P.stride + pt] = g[j];
+            if constexpr (IP) { // ghost slot (i, pt) = "cell pt + c_i receives direction i" (lbm_core.cuh ip_visit)
+                int cell = pt;
+                if (i & 1) cell = pt + poff_rt(P, i) + ((dir_cx(i) == 1 && P.perx && x == P.nx - 1) ? -P.nx : 0);
+                I.G[(long long)ip_slot(I.qn, i) * P.stride + cell] = g[j];
+            } else B[(long long)i * P.stride + pt] = g[j];
             if constexpr (j < QT) HB[(long long)i * P.stride + pt] = t[j]; // an axis direction reflects into an axis direction
         });
     if constexpr (MEAN) {
@@ -243,15 +273,35 @@ thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *
     }
 }
 
+template <typename real, bool MEAN, int BLOCK, int MINB, bool PERX = false, bool DAMP = false>
+__global__ void __launch_bounds__(BLOCK, MINB)
+thermal_step_kernel(real *__restrict__ B, real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links,
+                    real *__restrict__ msum, const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O,
+                    const Turb<real> tb = Turb<real>{}, const int turb_planes = 0)
+{
+    IpPtrs<real> none; // not touched by the two-buffer instantiation
+    thermal_step_body<real, MEAN, BLOCK, PERX, DAMP, false>(B, HB, flags, links, msum, P, T, O, tb, turb_planes, none);
+}
+
+// the same step with the flow lattice on ONE buffer (lbm_create_ex precision | LBM_STREAM_INPLACE)
+template <typename real, bool MEAN, int BLOCK, int MINB, bool PERX, bool DAMP>
+__global__ void __launch_bounds__(BLOCK, MINB)
+ip_thermal_step_kernel(real *__restrict__ HB, const uint8_t *__restrict__ flags, const uint32_t *__restrict__ links, real *__restrict__ msum,
+                       const Params<real> P, const ThermalPtrs<real> T, const OpenFaces<real> O, const Turb<real> tb, const int turb_planes,
+                       const IpPtrs<real> I)
+{
+    thermal_step_body<real, MEAN, BLOCK, PERX, DAMP, true>(nullptr, HB, flags, links, msum, P, T, O, tb, turb_planes, I);
+}
+
 // Publish what a feeding cell (one layer inside an EQ_OUTFLOW face) hands to the outflow cells for the next step, from the
 // CURRENT states A (flow) and its thermal shift dth: the local velocity with the cell's buoyancy in the force, and theta; both
 // halves of both side arrays (set-up paths).
 template <typename real>
 __device__ __forceinline__ void thermal_feed_both(const real *__restrict__ A, real *__restrict__ fu, real *__restrict__ ft, Params<real> P,
-                                                  int p, int x, int y, int z, int cls, real dth)
+                                                  int p, int x, int y, int z, int cls, real dth, uint8_t fl, uint32_t lk)
 {
     real g[Q];
-    load_cell(g, A, P.stride, p);
+    load_cell_any(g, A, P, p, x, y, z, fl, (fl & SLOW_BIT) ? lk : 0u); // the flow state, whichever streaming scheme holds it
     P.Fz += P.gbeta * dth;
     const Macro<real> m = local_macros(g, cls, P, damp_at(P, x, y, z));
     outflow_feed(P, x, y, z, m.ux, m.uy, m.uz, [&](int sl, int comp, real v) {
@@ -284,7 +334,7 @@ __global__ void thermal_init_kernel(real *__restrict__ HA, real *__restrict__ HB
     const uint32_t lk = links[p];
     store_cell_thermal(HA, P, p, x, y, z, fl, lk, t);
     store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
-    if ((fl & FEED_BIT) && P.F > 0) thermal_feed_both(A, fu, ft, P, p, x, y, z, cls, dth);
+    if ((fl & FEED_BIT) && P.F > 0) thermal_feed_both(A, fu, ft, P, p, x, y, z, cls, dth, fl, lk);
 }
 
 // Prescribed temperature of the EQ_FIXED cells (lbm_set_inlet_theta; reading 27): one thread per face slot; theta_b[nz] by level,
@@ -344,7 +394,7 @@ __global__ void thermal_state_in_kernel(real *__restrict__ HA, real *__restrict_
     const uint32_t lk = links[p];
     store_cell_thermal(HA, P, p, x, y, z, fl, lk, t);
     store_cell_thermal(HB, P, p, x, y, z, fl, lk, t);
-    if ((fl & FEED_BIT) && P.F > 0) thermal_feed_both(A, fu, ft, P, p, x, y, z, cls, theta_shift(t));
+    if ((fl & FEED_BIT) && P.F > 0) thermal_feed_both(A, fu, ft, P, p, x, y, z, cls, theta_shift(t), fl, lk);
 }
 
 // theta of the stored state (lbm_get_theta); SOLID cells report theta_ref

@@ -21,11 +21,11 @@ def B():
     return binding
 
 
-def pair(B, nx, ny, nz, faces, hm, nu0, Cs, fcor, F, alpha, gb, tref, theta, u0=None, fp64=False, want_mean=False):
+def pair(B, nx, ny, nz, faces, hm, nu0, Cs, fcor, F, alpha, gb, tref, theta, u0=None, fp64=False, want_mean=False, inplace=False):
     from oracle import Oracle
     o = Oracle(nx, ny, nz, nu0, Cs, fcor, F, faces)
     o.set_flags(hm)
-    sim = B.Lbm(nx, ny, nz, nu0, Cs, fcor, F, faces, fp64=fp64, want_mean=want_mean)
+    sim = B.Lbm(nx, ny, nz, nu0, Cs, fcor, F, faces, fp64=fp64, want_mean=want_mean, inplace=inplace)
     sim.set_flags(hm)
     np.testing.assert_array_equal(sim.get_flags(), o.get_flags())
     u0 = u0 or (None, None, None)
@@ -54,9 +54,10 @@ def errs(sim, o, tref):
 FACES = [(P, P, P, P, P, P), (W, FS, P, P, W, FS), (FS, FS, FS, FS, FS, FS), (W, W, W, W, W, W), (FS, W, P, P, FS, W)]
 
 
+@pytest.mark.parametrize("inplace", [False, True])    # the flow lattice on one buffer; the thermal one stays double
 @pytest.mark.parametrize("fp64", [False, True])
 @pytest.mark.parametrize("faces", FACES)
-def test_thermal_parity_ragged_boxes_with_solids(B, faces, fp64):
+def test_thermal_parity_ragged_boxes_with_solids(B, faces, fp64, inplace):
     rng = np.random.default_rng(11 + FACES.index(faces))
     for nx, ny, nz in [(33, 7, 9), (70, 5, 12)]:
         hm = np.zeros((ny, nx), np.int32)
@@ -64,8 +65,8 @@ def test_thermal_parity_ragged_boxes_with_solids(B, faces, fp64):
         hm[ny - 2, nx - 9:nx - 3] = 2
         theta = 1.0 + 0.3 * rng.standard_normal((nz, ny, nx))
         u0 = tuple(0.02 * rng.standard_normal((nz, ny, nx)) for _ in range(3))
-        sim, o = pair(B, nx, ny, nz, faces, hm, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), 0.01, 2e-3, 1.0, theta, u0, fp64=fp64)
-        sim.step(100); o.step(100)
+        sim, o = pair(B, nx, ny, nz, faces, hm, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), 0.01, 2e-3, 1.0, theta, u0, fp64=fp64, inplace=inplace)
+        sim.step(101); o.step(101)
         e_flow, e_th = errs(sim, o, 1.0)
         tol = TOL64 if fp64 else TOL32
         assert e_flow <= tol and e_th <= tol, (faces, (nx, ny, nz), e_flow, e_th)
@@ -371,7 +372,7 @@ def test_thermal_walls_argument_errors(B):
 EQF, EQO = 3, 4
 
 
-def open_pair(B, nx, ny, nz, faces, hm, fp64, gb=3e-4, alpha=0.02, tref=1.0, seed=0, want_mean=False):
+def open_pair(B, nx, ny, nz, faces, hm, fp64, gb=3e-4, alpha=0.02, tref=1.0, seed=0, want_mean=False, inplace=False):
     from oracle import Oracle
     rng = np.random.default_rng(seed)
     prof = (0.05 * np.log((np.arange(nz) + 0.5) / 0.1) / np.log(nz / 0.1)).clip(0)
@@ -380,7 +381,7 @@ def open_pair(B, nx, ny, nz, faces, hm, fp64, gb=3e-4, alpha=0.02, tref=1.0, see
     th0 = tref + 0.05 * rng.standard_normal((nz, ny, nx))
     args = (nx, ny, nz, 3e-3, 0.1, 1e-3, (1e-6, 0, 0), faces)
     o = Oracle(*args)
-    sim = B.Lbm(*args, fp64=fp64, want_mean=want_mean)
+    sim = B.Lbm(*args, fp64=fp64, want_mean=want_mean, inplace=inplace)
     for obj, kw in ((o, {}), (sim, {"f64": True})):
         obj.set_flags(hm)
         obj.set_inlet_profile(prof, 0.1 * prof, None, **kw)
@@ -391,14 +392,15 @@ def open_pair(B, nx, ny, nz, faces, hm, fp64, gb=3e-4, alpha=0.02, tref=1.0, see
     return sim, o, prof, thb
 
 
+@pytest.mark.parametrize("inplace", [False, True])
 @pytest.mark.parametrize("fp64", [False, True])
 @pytest.mark.parametrize("faces", [(EQF, EQO, P, P, W, FS), (EQF, EQO, FS, FS, W, FS), (EQF, EQO, EQF, EQF, W, FS), (EQO, EQF, W, FS, P, P)])
-def test_open_faces_parity(B, faces, fp64):
+def test_open_faces_parity(B, faces, fp64, inplace):
     """Inlet with a prescribed theta_b(z) and u_b(z), outflow copying theta and u, buildings, buoyancy, LES, Coriolis, a body
     force: rho, u, theta against the oracle after 100 steps; the state right after set-up too (boundary cells included)."""
     nx, ny, nz = 52, 14, 12
     hm = np.zeros((ny, nx), np.int32); hm[3:8, 14:20] = 5; hm[8:12, 30:36] = 3
-    sim, o, prof, thb = open_pair(B, nx, ny, nz, faces, hm, fp64, seed=FACES.index(FACES[0]) + len(faces))
+    sim, o, prof, thb = open_pair(B, nx, ny, nz, faces, hm, fp64, seed=FACES.index(FACES[0]) + len(faces), inplace=inplace)
     tol = TOL64 if fp64 else TOL32
     e_flow, e_th = errs(sim, o, 1.0)
     assert e_flow <= tol and e_th <= tol, ("set-up", faces, e_flow, e_th)
@@ -445,9 +447,10 @@ def test_open_faces_boundary_updates_mean_and_checkpoint(B):
     sim.close(); o.close(); b.close()
 
 
+@pytest.mark.parametrize("inplace", [False, True])
 @pytest.mark.parametrize("fp64", [False, True])
 @pytest.mark.parametrize("faces", [(EQF, EQO, EQF, EQF, W, EQF), (EQF, EQO, P, P, W, FS), (P, P, P, P, W, FS)])
-def test_damping_zones_together_with_the_thermal_lattice(B, faces, fp64):
+def test_damping_zones_together_with_the_thermal_lattice(B, faces, fp64, inplace):
     """The paper's open-boundary damping (top sponge + lateral buffer nudging) on a thermal run: the relaxation
     acceleration and the buoyancy share one implicit half-force solve (oracle pin: test_oracle_thermal.py
     ::test_buoyancy_against_a_uniform_damping_zone_settles_at_a_over_sigma).  Buildings, warm inflow, LES, Coriolis; zones set
@@ -455,7 +458,7 @@ def test_damping_zones_together_with_the_thermal_lattice(B, faces, fp64):
     local macros), switched off; the time mean; rho, u, theta against the oracle."""
     nx, ny, nz = 52, 14, 12
     hm = np.zeros((ny, nx), np.int32); hm[3:8, 14:20] = 5; hm[8:12, 30:36] = 3
-    sim, o, prof, thb = open_pair(B, nx, ny, nz, faces, hm, fp64, seed=3, want_mean=True)
+    sim, o, prof, thb = open_pair(B, nx, ny, nz, faces, hm, fp64, seed=3, want_mean=True, inplace=inplace)
     target = np.stack([prof, 0.1 * prof, np.zeros(nz)])
     tol = TOL64 if fp64 else TOL32
     for obj in (o, sim):
@@ -508,8 +511,9 @@ def test_uniformly_warm_damped_box_settles_at_a_over_sigma_on_the_gpu(B):
     sim.close()
 
 
+@pytest.mark.parametrize("inplace", [False, True])
 @pytest.mark.parametrize("fp64", [False, True])
-def test_whole_open_boundary_stack_on_a_thermal_run(B, fp64):
+def test_whole_open_boundary_stack_on_a_thermal_run(B, fp64, inplace):
     """Everything PAPER.md:175 / Table 1 lists, at once: equilibrium velocity faces with a warm inflow, the
     global flux correction, sponge + buffer nudging, synthetic fluctuations on the active inflow cells — whose thermal state
     follows the same velocity (reading 28) — buoyancy, LES, Coriolis, the time mean.  Fluctuations switched on before the
@@ -529,7 +533,7 @@ def test_whole_open_boundary_stack_on_a_thermal_run(B, fp64):
         target = np.stack([prof, 0.1 * prof, np.zeros(nz)])
         args = (nx, ny, nz, 3e-3, 0.1, 1e-3, (0.0, 0, 0), faces)
         o = Oracle(*args)
-        sim = B.Lbm(*args, fp64=fp64, want_mean=True)
+        sim = B.Lbm(*args, fp64=fp64, want_mean=True, inplace=inplace)
         for obj, kw in ((o, {}), (sim, {"f64": True})):
             obj.set_flags(hm)
             obj.set_inlet_profile(prof, 0.1 * prof, None, **kw)
