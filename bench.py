@@ -56,6 +56,7 @@ WORKLOADS = {
     "c4-inplace": "C4 refined urban 800x800x200 with in-place streaming (one population buffer; DESIGN.md §14)",
     "c5-inplace": "C5 chain with in-place streaming on both lattices (one population buffer each; DESIGN.md §14)",
     "c3-fp16-inplace": "C3 urban 400x400x100, 16-bit population storage AND in-place streaming: 77 B/cell, a quarter of the FP32 two-buffer memory",
+    "thermal-inplace": "closed 400x400x100 city box with the thermal lattice on, the flow lattice streaming in place (thermal populations double-buffered): 209 B/cell",
 }
 
 
@@ -405,7 +406,7 @@ def run_ours(args):
     d2h = sum(o.numel() * 4 for o in outs)
     e2e = {"value": job_mlups(cells, K, world, e2e_s), "unit": "MLUPS", "h2d_bytes_per_step": h2d / K,
            "d2h_bytes_per_step": d2h / K,
-           "what": f"one job = set_flags + set_inlet_profile + set_macros{' + set_theta' if args.workload == 'thermal' else ''} from pinned host buffers, lbm_step({K}), "
+           "what": f"one job = set_flags + set_inlet_profile + set_macros{' + set_theta' if args.workload.startswith('thermal') else ''} from pinned host buffers, lbm_step({K}), "
                    "lbm_get_macros into pinned host buffers; best of 2 jobs"}
 
     if rank == 0:
@@ -413,7 +414,7 @@ def run_ours(args):
         per_launch_s = ms_total * 1e-3 / K
         # thermal workload: (19 + 7) x 4 B loads + (19 + 7) x 4 B stores + 1 flag byte (lbm_thermal.cuh)
         # 16-bit storage: 19 x 2 B loads + 19 x 2 B stores + 1 flag byte
-        BYTES_PER_CELL = {"thermal": 209, "c3-fp16": 77, "c3-fp16-inplace": 77}.get(args.workload, globals()["BYTES_PER_CELL"])
+        BYTES_PER_CELL = {"thermal": 209, "thermal-inplace": 209, "c3-fp16": 77, "c3-fp16-inplace": 77}.get(args.workload, globals()["BYTES_PER_CELL"])
         achieved = BYTES_PER_CELL * cells / per_launch_s / 1e9
         traffic, traffic_src = (load_traffic("step") if args.workload == "c3" else
                                 load_traffic("thermal") if args.workload == "thermal" else

@@ -298,7 +298,8 @@ def thermal_city(nx: int = 400, ny: int = 400, nz: int = 100, seed: int = 7) -> 
     theta = (300.0 + rng.standard_normal((nz, ny, nx))).astype(np.float32)
     return Workload("thermal_city", nx, ny, nz, c3.nu0, c3.Cs, c3.f_cor, (1e-6, 0.0, 0.0),
                     (FREE_SLIP, FREE_SLIP, FREE_SLIP, FREE_SLIP, WALL, FREE_SLIP), 1000, c3.height,
-                    extra={"thermal": (1e-3, 1e-5, 300.0), "theta": theta})
+                    extra={"thermal": (1e-2, 1e-5, 300.0), "theta": theta})   # alpha 1e-2: tau_theta = 0.54 (at 1e-3 = 0.504 the
+                    # cell-scale temperature noise, fed back through the buoyancy, blows the BGK thermal lattice up after ~500 steps)
 
 
 def density_current_benchmark(dx_m: float = 100.0, u_lat: float = 0.1):
