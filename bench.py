@@ -376,6 +376,8 @@ def run_ours(args):
                      "clocks": s2.stop(t_s0, s2.mark()) if rank == 0 else None}
     rho, ux, uy, uz = sim.get_macros()
     finite = bool(torch.isfinite(ux).all().item())
+    if not finite and rank == 0:   # a timing on a state that has blown up is not a measurement of this workload
+        print("bench.py: WARNING: the state is not finite after the timed regions (config.state_finite = false)", file=sys.stderr)
     ms_total = max_over_ranks(best, world, dev)
     mlups = job_mlups(cells, K, world, ms_total * 1e-3)
 
