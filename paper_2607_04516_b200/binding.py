@@ -156,7 +156,7 @@ class Lbm:
     """One lattice on one GPU.  Same call names as include/lbm.h without the ``lbm_`` prefix."""
 
     def __init__(self, nx, ny, nz, nu0, Cs=0.0, f_cor=0.0, F=(0.0, 0.0, 0.0), faces=None, fp64=False,
-                 want_mean=True, device="cuda:0", stream=None, storage16=False, inplace=False):
+                 want_mean=True, device="cuda:0", stream=None, storage16=False, inplace=False, guard_bytes=0):
         import torch
         if not torch.cuda.is_available():
             raise LbmError("no CUDA device: the LBM path has no CPU fallback")
@@ -180,9 +180,13 @@ class Lbm:
         self._chk0(self._lib.lbm_workspace_bytes(self.nx, self.ny, self.nz, int(want_mean), precision, C.byref(nbytes)),
                    "workspace_bytes")
         with torch.cuda.device(self.device):
-            self._ws = torch.empty(nbytes.value + 256, dtype=torch.uint8, device=self.device)
+            # guard_bytes > 0 (tests): the workspace handed to the library sits between two bands filled with 0xA5, which
+            # guards_intact() inspects — a store of any kernel outside its workspace shows up there
+            self._guard = int(guard_bytes) // 256 * 256
+            self._ws = torch.full((nbytes.value + 512 + 2 * self._guard,), 0xA5, dtype=torch.uint8, device=self.device)
             base = self._ws.data_ptr()
-            aligned = (base + 255) // 256 * 256
+            aligned = (base + 255) // 256 * 256 + self._guard
+            self._ws_off = aligned - base
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
             h = C.c_void_p()
             rc = self._lib.lbm_create_ex(self.nx, self.ny, self.nz, float(nu0), float(Cs), float(f_cor), F.ctypes.data,
@@ -203,6 +207,12 @@ class Lbm:
         if rc != 0:
             msg = self._lib.lbm_last_error(self._h)
             raise LbmError(f"lbm_{what} failed: {_ERR.get(rc, rc)}: {msg.decode() if msg else ''}")
+
+    def guards_intact(self) -> bool:
+        """True if no byte outside the workspace handed to the library (guard bands before and after it) has been written."""
+        lo = self._ws[: self._ws_off]
+        hi = self._ws[self._ws_off + self.workspace_bytes:]
+        return bool((lo == 0xA5).all().item()) and bool((hi == 0xA5).all().item())
 
     def close(self):
         if getattr(self, "_h", None):

@@ -400,6 +400,36 @@ def test_state_box_is_a_slice_of_the_state_and_restores_slab_by_slab(B, fp64, in
         src.close(); ref.close()
 
 
+@pytest.mark.parametrize("inplace", [False, True])
+def test_no_kernel_writes_outside_its_workspace(B, inplace):
+    """Guard bands of 1 MiB filled with 0xA5 on both sides of the workspace (binding guard_bytes): after set-up, steps with every
+    face rule, sampling, state round trips and the box calls — boxes one cell thick and rows shorter than a sector included — no
+    byte of them has changed.  (compute-sanitizer is not available on this pool; the population buffer of a handle is the first
+    thing in its workspace, the scratch area the last.)"""
+    for faces in FACE_SETS:
+        for shape in [(37, 11, 9), (5, 1, 4), (1, 6, 5), (8, 3, 3)]:
+            nx, ny, nz = shape
+            hm, prof, ux0, uy0 = _case(shape, 3)
+            for kw in ({}, {"fp64": True}, {"storage16": True}):
+                sim = B.Lbm(nx, ny, nz, 2e-3, 0.1, 1e-3, (1e-6, 0, 0), faces, inplace=inplace, guard_bytes=1 << 20, **kw)
+                sim.set_flags(hm)
+                sim.set_inlet_profile(prof, 0.1 * prof, None, f64=True)
+                sim.set_macros(None, ux0, uy0, None, f64=True)
+                sim.mean_config(2, 3)
+                sim.step(7)
+                st = sim.get_state(out="host")
+                sim.set_state(st)
+                sim.set_state_box((0, 0, 0), (nx, ny, 1), np.ascontiguousarray(st[:, :1]))
+                sim.get_macros_box((0, 0, nz - 1), (nx, ny, nz))
+                sim.step(6)
+                sim.sync()
+                assert sim.guards_intact(), (faces, shape, kw)
+                if faces == FACE_SETS[0] and shape == (8, 3, 3) and not kw:    # the check itself sees a stray byte
+                    sim._ws[sim._ws_off + sim.workspace_bytes + 3] = 0
+                    assert not sim.guards_intact()
+                sim.close()
+
+
 def test_rest_state_is_exact_and_refused_combinations_say_so(B):
     hm = np.zeros((12, 16), dtype=np.int32)
     hm[3:6, 4:8] = 5
